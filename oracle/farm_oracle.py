@@ -1,0 +1,151 @@
+"""ctypes wrapper of the CPU oracle (oracle/farm_oracle.cpp).  TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+Argument marshalling only; every rule lives in the C++ file.
+"""
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import build as _build  # noqa: E402  (oracle/build.py)
+
+sys.path.pop(0)
+
+OBJECT_DTYPE = np.dtype(
+    [("id", "<i4"), ("n_voxels", "<u4"), ("n_obs", "<u4"), ("aabb_min", "<f4", 3), ("aabb_max", "<f4", 3),
+     ("best_frame", "<i4"), ("best_det", "<i4"), ("best_pixels", "<u4"), ("best_cam_pos", "<f4", 3),
+     ("n_points", "<u8")], align=True)
+STATS_DTYPE = np.dtype(
+    [("valid_points", "<u8"), ("dropped_points", "<u8"), ("ignored_pixels", "<u8"), ("unique_voxels", "<u8"),
+     ("matches", "<u4"), ("spawns", "<u4"), ("skipped", "<u4"), ("n_det", "<u4")], align=True)
+assert OBJECT_DTYPE.itemsize == 72
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.oracle_create.restype = C.c_void_p
+        _lib.oracle_create.argtypes = [C.c_float, C.c_int, C.c_float, C.c_float, C.c_float, C.c_int, C.c_int,
+                                       C.c_int, C.c_float, C.c_float]
+        _lib.oracle_clone.restype = C.c_void_p
+        _lib.oracle_clone.argtypes = [C.c_void_p]
+        _lib.oracle_n_voxels.restype = C.c_longlong
+        _lib.oracle_round_to_storage.restype = C.c_float
+        _lib.oracle_round_to_storage.argtypes = [C.c_float, C.c_int]
+        _lib.oracle_cosine.restype = C.c_float
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class OracleMap:
+    def __init__(self, voxel_size, D, w_geo, w_sem, tau, dtype, H, W, z_min=0.0, z_max=float("inf")):
+        self.D, self.dtype, self.H, self.W = D, dtype, H, W
+        self.h = C.c_void_p(lib().oracle_create(voxel_size, D, w_geo, w_sem, tau, dtype, H, W, z_min, z_max))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().oracle_destroy(self.h)
+            self.h = None
+
+    def clone(self):
+        c = OracleMap.__new__(OracleMap)
+        c.D, c.dtype, c.H, c.W = self.D, self.dtype, self.H, self.W
+        c.h = C.c_void_p(lib().oracle_clone(self.h))
+        return c
+
+    def backproject(self, depth, mask, K, T, n_det):
+        depth = np.ascontiguousarray(depth, np.float32)
+        mask = np.ascontiguousarray(mask, np.uint16)
+        K = np.ascontiguousarray(K, np.float32)
+        T = np.ascontiguousarray(T, np.float32)
+        xyz = np.empty((self.H, self.W, 3), np.float32)
+        keys = np.empty((self.H, self.W), np.uint64)
+        lib().oracle_backproject(self.h, _p(depth), _p(mask), _p(K), _p(T), C.c_int(n_det), _p(xyz), _p(keys))
+        return xyz, keys
+
+    def integrate_batch(self, depth, mask, K, T, desc, n_det):
+        n_det = np.ascontiguousarray(n_det, np.int32).reshape(-1)
+        F = n_det.shape[0]
+        depth = np.ascontiguousarray(depth, np.float32).reshape(F, self.H, self.W)
+        mask = np.ascontiguousarray(mask, np.uint16).reshape(F, self.H, self.W)
+        K = np.ascontiguousarray(K, np.float32).reshape(F, 3, 3)
+        T = np.ascontiguousarray(T, np.float32).reshape(F, 4, 4)
+        desc = np.ascontiguousarray(desc)
+        assert desc.dtype.itemsize == (4 if self.dtype == 0 else 2)
+        assert desc.size == int(n_det.sum()) * self.D
+        return lib().oracle_integrate_batch(self.h, C.c_int(F), _p(depth), _p(mask), _p(K), _p(T), _p(desc),
+                                            _p(n_det))
+
+    def integrate(self, depth, mask, K, T, desc, n_det):
+        return self.integrate_batch(depth, mask, K, T, desc, [n_det])
+
+    def last_assoc(self):
+        M = lib().oracle_last_M(self.h)
+        assoc = np.empty(M, np.int32)
+        is_new = np.empty(M, np.uint8)
+        best = np.empty(M, np.float32)
+        second = np.empty(M, np.float32)
+        st = np.zeros(1, STATS_DTYPE)
+        lib().oracle_last_assoc(self.h, _p(assoc), _p(is_new), _p(best), _p(second), _p(st))
+        return assoc, is_new, best, second, st[0]
+
+    def last_voxels(self):
+        M = lib().oracle_last_M(self.h)
+        off = np.empty(M + 1, np.int64)
+        lib().oracle_last_voxels(self.h, _p(off), None, None, None)
+        keys = np.empty(int(off[M]), np.uint64)
+        n_px = np.empty(M, np.uint32)
+        box = np.empty((M, 6), np.float32)
+        lib().oracle_last_voxels(self.h, _p(off), _p(keys), _p(n_px), _p(box))
+        return off, keys, n_px, box
+
+    def last_overlaps(self):
+        M = lib().oracle_last_M(self.h)
+        off = np.empty(M + 1, np.int64)
+        lib().oracle_last_overlaps(self.h, _p(off), None, None)
+        obj = np.empty(int(off[M]), np.int32)
+        cnt = np.empty(int(off[M]), np.uint32)
+        lib().oracle_last_overlaps(self.h, _p(off), _p(obj), _p(cnt))
+        return off, obj, cnt
+
+    def read(self, voxels=True):
+        N = lib().oracle_n_objects(self.h)
+        nv = lib().oracle_n_voxels(self.h)
+        objs = np.zeros(N, OBJECT_DTYPE)
+        desc = np.empty((N, self.D), np.float32)
+        keys = np.empty(nv if voxels else 0, np.uint64)
+        owners = np.empty(nv if voxels else 0, np.uint32)
+        lib().oracle_read(self.h, _p(objs), _p(desc), _p(keys) if voxels else None, _p(owners) if voxels else None)
+        return objs, desc, keys, owners
+
+    def import_(self, objs, desc, keys, owners):
+        objs = np.ascontiguousarray(objs, OBJECT_DTYPE)
+        desc = np.ascontiguousarray(desc, np.float32)
+        keys = np.ascontiguousarray(keys, np.uint64)
+        owners = np.ascontiguousarray(owners, np.uint32)
+        return lib().oracle_import(self.h, _p(objs), C.c_int(len(objs)), _p(desc), _p(keys), _p(owners),
+                                   C.c_longlong(len(keys)))
+
+
+def round_to_storage(x, dtype):
+    x = np.asarray(x, np.float32)
+    out = np.empty_like(x)
+    flat_in, flat_out = x.reshape(-1), out.reshape(-1)
+    for i in range(flat_in.size):
+        flat_out[i] = lib().oracle_round_to_storage(float(flat_in[i]), dtype)
+    return out
+
+
+def cosine(a, b):
+    a = np.ascontiguousarray(a, np.float32)
+    b = np.ascontiguousarray(b, np.float32)
+    return float(lib().oracle_cosine(_p(a), _p(b), C.c_int(a.size)))
