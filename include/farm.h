@@ -1,0 +1,168 @@
+/* farm.h -- C ABI of the B200-native FARM mapping hot path (libfarm_map.so).
+ *
+ * The library implements the data-parallel part of FARM's per-batch synchronous memory update
+ *     M_t = f(M_{t-1}, o_t)                    ("Online construction", steps 1-5)
+ * in the voxel-overlap formulation fixed by BASELINE.json `north_star`:
+ *   (1) back-project masked RGB-D detections to world points        ("masked depth points")
+ *   (2) quantise the points to voxel keys, one key set V_d per detection
+ *   (3) count voxel overlap |V_d ∩ V_o| of every detection with every map object
+ *   (4) cosine similarity of detection descriptors against all map descriptors
+ *                                                   ("a single batched detection-by-entity similarity matrix")
+ *   (5) score = w_geo*|V_d∩V_o|/min(|V_d|,|V_o|) + w_sem*cos, argmax, `> tau` else new object
+ *                                                   (BASELINE.json rule), then merge voxels,
+ *       AABBs, count-weighted descriptors and view evidence into the map.
+ * The exact rules (R1..R26) are listed in DESIGN.md section 3.  Every step runs in hand-written sm_100a
+ * CUDA kernels; there is no CPU fallback -- without a CUDA device every call below except the option
+ * setters fails with FARM_ERR_CUDA.
+ *
+ * Conventions
+ *   - "DEVICE pointer": caller-owned CUDA device memory, must stay valid until the map's stream has
+ *     executed the call.  "HOST pointer": ordinary host memory, consumed/filled before the call returns.
+ *   - integrate calls are asynchronous on the map's stream and never synchronise the device.  Only
+ *     host-visible arguments are validated at call time.  Data-dependent failures (hash table full,
+ *     object capacity, per-call scratch overflow) set a sticky device error word that the next
+ *     farm_map_sync / farm_map_read / farm_map_last_assoc returns as FARM_ERR_CAPACITY; after that the
+ *     map content is unspecified.
+ *   - one host thread per map handle.
+ *   - K: row-major 3x3, fx=K[0], fy=K[4], cx=K[2], cy=K[5], skew ignored.  T_world_cam: row-major 4x4,
+ *     camera (x right, y down, z forward; depth = camera z, not ray length) -> world; top 3x4 is read.
+ *   - instance_mask: 0 = background, k in 1..n_det = detection k-1 of that frame (descriptor row k-1),
+ *     k > n_det = ignored (counted in stats).
+ *   - voxel key: ix = floor(X * (1/voxel_size)) etc. in fp32, each in [-2^20, 2^20);
+ *     key = (ix+2^20)<<42 | (iy+2^20)<<21 | (iz+2^20);  0xFFFFFFFFFFFFFFFF = no key.
+ */
+#ifndef FARM_H_
+#define FARM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FARM_OK 0
+#define FARM_ERR_INVALID_ARG (-1)
+#define FARM_ERR_CUDA (-2)
+#define FARM_ERR_CAPACITY (-3)
+#define FARM_ERR_STATE (-4)
+#define FARM_ERR_RANGE (-5)
+
+#define FARM_KEY_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+/* descriptor storage dtypes (one per map; detection rows and the map's similarity operands use it) */
+#define FARM_DTYPE_F32 0
+#define FARM_DTYPE_F16 1
+#define FARM_DTYPE_BF16 2
+
+/* integer options (farm_map_set_option_i); legal only before the first integrate / import / debug call */
+#define FARM_OPT_DESC_DTYPE 1        /* FARM_DTYPE_*, default F32                                              */
+#define FARM_OPT_MAX_OBJECTS 2       /* object capacity, default 65536                                         */
+#define FARM_OPT_MAX_VOXELS 3        /* owned-voxel capacity; table = next pow2 >= 2x, default 1<<22           */
+#define FARM_OPT_IMG_W 4             /* image width  (required)                                                */
+#define FARM_OPT_IMG_H 5             /* image height (required)                                                */
+#define FARM_OPT_MAX_DET_PER_CALL 6  /* sum of n_det over the frames of one call, default 4096, max 2^21-1      */
+#define FARM_OPT_STREAM 7            /* cudaStream_t as integer, default 0 (legacy default stream)             */
+#define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
+#define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
+#define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
+/* float options (farm_map_set_option_f) */
+#define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
+#define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
+
+typedef struct farm_map farm_map; /* opaque; the library owns all map memory */
+
+/* One map object as exported / imported.  (PAPER.md:63 entity attributes reduced to BASELINE.json's fields.) */
+typedef struct {
+  int32_t id;               /* dense 0..N-1, creation order                                                  */
+  uint32_t n_voxels;        /* |V_o|, number of owned voxel keys                                             */
+  uint32_t n_obs;           /* detections merged so far                                                      */
+  float aabb_min[3];        /* AABB over all merged world points (fp32, exact min/max)                       */
+  float aabb_max[3];
+  int32_t best_frame;       /* best view: frame sequence number (0-based over all integrated frames)         */
+  int32_t best_det;         /*            detection index inside that frame                                  */
+  uint32_t best_pixels;     /*            its valid masked pixel count (the view quality measure)            */
+  float best_cam_pos[3];    /*            camera position (translation of T_world_cam)                       */
+  uint64_t n_points;        /* total valid masked pixels merged                                              */
+} farm_object;
+
+typedef struct {
+  uint64_t valid_points;    /* valid masked pixels of the call (R4 and key in range)                         */
+  uint64_t dropped_points;  /* valid pixels whose voxel index left [-2^20, 2^20)                             */
+  uint64_t ignored_pixels;  /* pixels with label > n_det                                                     */
+  uint64_t unique_voxels;   /* sum over detections of |V_d|                                                  */
+  uint32_t matches, spawns, skipped, n_det;
+} farm_frame_stats;
+
+typedef struct {
+  uint64_t frames, calls, valid_points, unique_voxels, matches, spawns;
+} farm_totals; /* cumulative since create / import */
+
+/* Create an empty map.  BASELINE.json: farm_map_create(voxel_size, D, w_geo, w_sem, tau).
+ * voxel_size > 0 metres; 1 <= D <= 8192; w_geo >= 0, w_sem >= 0.  *out receives the handle.
+ * Device memory is allocated at the first integrate / import, when the options are frozen. */
+int farm_map_create(float voxel_size, int D, float w_geo, float w_sem, float tau, farm_map **out);
+int farm_map_destroy(farm_map *m);
+
+int farm_map_set_option_i(farm_map *m, int key, long long value);
+int farm_map_set_option_f(farm_map *m, int key, float value);
+
+/* One frame.  BASELINE.json: farm_map_integrate(depth, instance_mask, K, T_world_cam, det_descriptors, n_det).
+ * depth [H,W] fp32 metres, instance_mask [H,W] u16, K [9], T_world_cam [16], det_descriptors [n_det, D] in
+ * the map's storage dtype: all DEVICE pointers (det_descriptors may be NULL iff n_det == 0).
+ * Equivalent to farm_map_integrate_batch with one frame. */
+int farm_map_integrate(farm_map *m, const float *depth, const uint16_t *instance_mask, const float *K,
+                       const float *T_world_cam, const void *det_descriptors, int n_det);
+
+/* F frames scored against ONE snapshot of the map (the paper's "RGB-D batch").
+ * depth [F,H,W], mask [F,H,W], K [F,9], T [F,16], desc [sum n_det, D]: DEVICE pointers.  n_det: HOST array [F].
+ * Global detection index j = position in the concatenation of the frames' detection lists. */
+int farm_map_integrate_batch(farm_map *m, int n_frames, const float *depth, const uint16_t *instance_mask,
+                             const float *K, const float *T_world_cam, const void *det_descriptors,
+                             const int *n_det);
+
+/* Results of the LAST integrate call, HOST buffers of M = sum n_det entries (any may be NULL).
+ * obj_id: object the detection was merged into (-1 = skipped, R8); is_new: 1 if that object was spawned by it;
+ * best_score: R18.  Synchronises the stream; returns the sticky device error if set. */
+int farm_map_last_assoc(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score, farm_frame_stats *stats);
+
+/* Export (HOST buffers).  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
+ * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary
+ * order (may be NULL).  Synchronises; returns the sticky device error if set. */
+int farm_map_read(farm_map *m, farm_object *objects, int *n_objects, float *descriptors, uint64_t *voxel_keys,
+                  uint32_t *voxel_owner, long long *n_voxels);
+
+/* Bulk load into an EMPTY map (checkpoint resume; pre-populated maps).  HOST pointers.  Objects are
+ * installed verbatim (ids must be 0..n-1 in order), descriptors are renormalised and shadowed (R26), every
+ * voxel key must be unique and its owner < n_objects, else FARM_ERR_INVALID_ARG. */
+int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, const float *descriptors,
+                    const uint64_t *voxel_keys, const uint32_t *voxel_owner, long long n_voxels);
+
+/* Stream sync + sticky device error.  totals may be NULL. */
+int farm_map_sync(farm_map *m, farm_totals *totals);
+
+/* Number of kernels this library has launched for the map so far (host counter). */
+long long farm_map_kernel_launches(const farm_map *m);
+
+/* Thread-local description of the last error returned on this thread. */
+const char *farm_last_error(void);
+
+/* ---- parity / debug entry points (not on the production path) ---- */
+/* Dense per-pixel world point (NaN where invalid) and voxel key (FARM_KEY_EMPTY where invalid or out of
+ * range) of one frame.  All DEVICE pointers; xyz [H,W,3], keys [H,W].  n_det bounds the valid labels. */
+int farm_debug_backproject(farm_map *m, const float *depth, const uint16_t *instance_mask, const float *K,
+                           const float *T_world_cam, int n_det, float *xyz, uint64_t *keys);
+/* For the LAST integrate call, HOST buffers; pass keys == NULL first to obtain offsets[M] = total.
+ * offsets [M+1]; keys: the distinct voxel keys of each detection (arbitrary order inside a detection);
+ * n_px [M]; box [M,6] = min xyz, max xyz of the detection's world points. */
+int farm_debug_last_voxels(farm_map *m, long long *offsets, uint64_t *keys, uint32_t *n_px, float *box);
+/* Sparse overlap histogram of the LAST call: offsets [M+1]; obj_id/count: (object, |V_d ∩ V_o|) with
+ * count > 0, arbitrary order inside a detection.  Pass obj_id == NULL first to size. */
+int farm_debug_last_overlaps(farm_map *m, long long *offsets, int32_t *obj_id, uint32_t *count);
+/* Dense pass of the LAST call: per detection the maximum clamped cosine over all objects at entry and
+ * its argmax (lowest id on ties; -1 when the map was empty).  HOST buffers [M]. */
+int farm_debug_last_dense(farm_map *m, float *max_cos, int32_t *argmax);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FARM_H_ */

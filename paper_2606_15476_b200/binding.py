@@ -1,0 +1,217 @@
+"""Thin ctypes binding of libfarm_map.so (include/farm.h).  Argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; this module owns no arithmetic and has
+no CPU fallback: if the library is missing, or no CUDA device is present, calls fail loudly.
+PyTorch appears only as the owner of device memory and streams (tensors in, `.data_ptr()` out).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libfarm_map.so")
+
+FARM_OK, ERR_INVALID_ARG, ERR_CUDA, ERR_CAPACITY, ERR_STATE, ERR_RANGE = 0, -1, -2, -3, -4, -5
+DTYPE_F32, DTYPE_F16, DTYPE_BF16 = 0, 1, 2
+OPT_DESC_DTYPE, OPT_MAX_OBJECTS, OPT_MAX_VOXELS, OPT_IMG_W, OPT_IMG_H = 1, 2, 3, 4, 5
+OPT_MAX_DET_PER_CALL, OPT_STREAM, OPT_MAX_PAIRS_PER_CALL, OPT_MAX_FRAMES_PER_CALL, OPT_SIM_PATH = 6, 7, 8, 9, 10
+OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
+KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
+
+OBJECT_DTYPE = np.dtype(
+    [("id", "<i4"), ("n_voxels", "<u4"), ("n_obs", "<u4"), ("aabb_min", "<f4", 3), ("aabb_max", "<f4", 3),
+     ("best_frame", "<i4"), ("best_det", "<i4"), ("best_pixels", "<u4"), ("best_cam_pos", "<f4", 3),
+     ("n_points", "<u8")], align=True)
+STATS_DTYPE = np.dtype(
+    [("valid_points", "<u8"), ("dropped_points", "<u8"), ("ignored_pixels", "<u8"), ("unique_voxels", "<u8"),
+     ("matches", "<u4"), ("spawns", "<u4"), ("skipped", "<u4"), ("n_det", "<u4")], align=True)
+TOTALS_DTYPE = np.dtype([("frames", "<u8"), ("calls", "<u8"), ("valid_points", "<u8"), ("unique_voxels", "<u8"),
+                         ("matches", "<u8"), ("spawns", "<u8")])
+
+EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm_map_set_option_f",
+           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_last_assoc", "farm_map_read",
+           "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
+           "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
+
+
+class FarmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"farm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libfarm_map.so.  Raises if it has not been built (python -m paper_2606_15476_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} missing: build it with `python -m paper_2606_15476_b200.build` "
+                                    "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        vp, ci, cf, ll = C.c_void_p, C.c_int, C.c_float, C.c_longlong
+        lib.farm_map_create.argtypes = [cf, ci, cf, cf, cf, C.POINTER(vp)]
+        lib.farm_map_destroy.argtypes = [vp]
+        lib.farm_map_set_option_i.argtypes = [vp, ci, ll]
+        lib.farm_map_set_option_f.argtypes = [vp, ci, cf]
+        lib.farm_map_integrate.argtypes = [vp, vp, vp, vp, vp, vp, ci]
+        lib.farm_map_integrate_batch.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp]
+        lib.farm_map_last_assoc.argtypes = [vp, vp, vp, vp, vp]
+        lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
+        lib.farm_map_sync.argtypes = [vp, vp]
+        lib.farm_map_kernel_launches.argtypes = [vp]
+        lib.farm_map_kernel_launches.restype = ll
+        lib.farm_last_error.restype = C.c_char_p
+        lib.farm_debug_backproject.argtypes = [vp, vp, vp, vp, vp, ci, vp, vp]
+        lib.farm_debug_last_voxels.argtypes = [vp, vp, vp, vp, vp]
+        lib.farm_debug_last_overlaps.argtypes = [vp, vp, vp, vp]
+        lib.farm_debug_last_dense.argtypes = [vp, vp, vp]
+        _lib = lib
+    return _lib
+
+
+def _check(rc):
+    if rc != FARM_OK:
+        raise FarmError(rc, load_library().farm_last_error().decode())
+
+
+def _hp(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _dp(t):
+    """device pointer of a CUDA torch tensor (or a raw int)"""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    return C.c_void_p(t.data_ptr())
+
+
+class FarmMap:
+    """farm_map_* with the same names and argument order as the C ABI."""
+
+    def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
+                 max_voxels=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
+                 stream=None, z_min=None, z_max=None, sim_path=None):
+        lib = load_library()
+        self.D, self.dtype, self.H, self.W = D, dtype, H, W
+        self._h = C.c_void_p()
+        _check(lib.farm_map_create(voxel_size, D, w_geo, w_sem, tau, C.byref(self._h)))
+        self.set_option_i(OPT_IMG_H, H)
+        self.set_option_i(OPT_IMG_W, W)
+        self.set_option_i(OPT_DESC_DTYPE, dtype)
+        for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels),
+                       (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
+                       (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path)):
+            if v is not None:
+                self.set_option_i(key, int(v))
+        if z_min is not None:
+            self.set_option_f(OPTF_Z_MIN, z_min)
+        if z_max is not None:
+            self.set_option_f(OPTF_Z_MAX, z_max)
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load_library().farm_map_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = destroy
+
+    def set_option_i(self, key, value):
+        _check(load_library().farm_map_set_option_i(self._h, key, int(value)))
+
+    def set_option_f(self, key, value):
+        _check(load_library().farm_map_set_option_f(self._h, key, float(value)))
+
+    # ---- the hot path (device tensors)
+    def integrate(self, depth, instance_mask, K, T_world_cam, det_descriptors, n_det):
+        _check(load_library().farm_map_integrate(self._h, _dp(depth), _dp(instance_mask), _dp(K), _dp(T_world_cam),
+                                                 _dp(det_descriptors), int(n_det)))
+        self._last_M = int(n_det)
+
+    def integrate_batch(self, n_frames, depth, instance_mask, K, T_world_cam, det_descriptors, n_det):
+        n_det = np.ascontiguousarray(n_det, np.int32)
+        assert n_det.size == n_frames
+        _check(load_library().farm_map_integrate_batch(self._h, int(n_frames), _dp(depth), _dp(instance_mask), _dp(K),
+                                                       _dp(T_world_cam), _dp(det_descriptors), _hp(n_det)))
+        self._last_M = int(n_det.sum())
+
+    # ---- results (host arrays)
+    def last_assoc(self, M=None):
+        M = self._last_M if M is None else M
+        obj = np.empty(M, np.int32)
+        is_new = np.empty(M, np.uint8)
+        best = np.empty(M, np.float32)
+        st = np.zeros(1, STATS_DTYPE)
+        _check(load_library().farm_map_last_assoc(self._h, _hp(obj), _hp(is_new), _hp(best), _hp(st)))
+        return obj, is_new, best, st[0]
+
+    def read(self, voxels=True, descriptors=True):
+        lib = load_library()
+        n = C.c_int(0)
+        nv = C.c_longlong(0)
+        _check(lib.farm_map_read(self._h, None, C.byref(n), None, None, None, C.byref(nv) if voxels else None))
+        objs = np.zeros(n.value, OBJECT_DTYPE)
+        desc = np.empty((n.value, self.D), np.float32) if descriptors else None
+        keys = np.empty(nv.value, np.uint64) if voxels else None
+        owners = np.empty(nv.value, np.uint32) if voxels else None
+        _check(lib.farm_map_read(self._h, _hp(objs), C.byref(n), _hp(desc), _hp(keys), _hp(owners),
+                                 C.byref(nv) if voxels else None))
+        return objs, desc, keys, owners
+
+    def import_(self, objects, descriptors, voxel_keys, voxel_owner):
+        objects = np.ascontiguousarray(objects, OBJECT_DTYPE)
+        descriptors = np.ascontiguousarray(descriptors, np.float32)
+        voxel_keys = np.ascontiguousarray(voxel_keys, np.uint64)
+        voxel_owner = np.ascontiguousarray(voxel_owner, np.uint32)
+        _check(load_library().farm_map_import(self._h, _hp(objects), len(objects), _hp(descriptors), _hp(voxel_keys),
+                                              _hp(voxel_owner), len(voxel_keys)))
+
+    def sync(self):
+        t = np.zeros(1, TOTALS_DTYPE)
+        _check(load_library().farm_map_sync(self._h, _hp(t)))
+        return t[0]
+
+    def kernel_launches(self):
+        return int(load_library().farm_map_kernel_launches(self._h))
+
+    # ---- parity / debug
+    def debug_backproject(self, depth, instance_mask, K, T_world_cam, n_det, xyz, keys):
+        _check(load_library().farm_debug_backproject(self._h, _dp(depth), _dp(instance_mask), _dp(K), _dp(T_world_cam),
+                                                     int(n_det), _dp(xyz), _dp(keys)))
+
+    def debug_last_voxels(self):
+        lib = load_library()
+        M = self._last_M
+        off = np.zeros(M + 1, np.int64)
+        _check(lib.farm_debug_last_voxels(self._h, _hp(off), None, None, None))
+        keys = np.empty(int(off[M]), np.uint64)
+        n_px = np.empty(M, np.uint32)
+        box = np.empty((M, 6), np.float32)
+        _check(lib.farm_debug_last_voxels(self._h, _hp(off), _hp(keys), _hp(n_px), _hp(box)))
+        return off, keys, n_px, box
+
+    def debug_last_overlaps(self):
+        lib = load_library()
+        M = self._last_M
+        off = np.zeros(M + 1, np.int64)
+        _check(lib.farm_debug_last_overlaps(self._h, _hp(off), None, None))
+        obj = np.empty(int(off[M]), np.int32)
+        cnt = np.empty(int(off[M]), np.uint32)
+        _check(lib.farm_debug_last_overlaps(self._h, _hp(off), _hp(obj), _hp(cnt)))
+        return off, obj, cnt
+
+    def debug_last_dense(self):
+        M = self._last_M
+        mc = np.empty(M, np.float32)
+        am = np.empty(M, np.int32)
+        _check(load_library().farm_debug_last_dense(self._h, _hp(mc), _hp(am)))
+        return mc, am

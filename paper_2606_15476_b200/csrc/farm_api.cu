@@ -1,0 +1,705 @@
+// farm_api.cu -- the C ABI of include/farm.h: handle, options, allocation, the per-call launch sequence,
+// export / import and the debug reads.  Host logic only; every step of the path runs in the kernels of
+// farm_lift.cu, farm_sim_fma.cu, farm_sim_tc.cu and farm_assoc.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <vector>
+
+#include "farm_internal.cuh"
+
+namespace farm {
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state);
+void *tc_state_create(const DevMap &m);
+void tc_state_destroy(void *);
+bool tc_supported(const DevMap &m);
+}  // namespace farm
+
+using namespace farm;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+#define CU(expr)                                                                                      \
+  do {                                                                                                \
+    cudaError_t e_ = (expr);                                                                          \
+    if (e_ != cudaSuccess) return fail(FARM_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+struct farm_map {
+  float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
+  int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
+  long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16;
+  int sim_path = 0;
+  cudaStream_t stream = 0;
+  bool finalised = false;
+  DevMap dm{};
+  std::vector<void *> allocs;
+  long long launches = 0;
+  unsigned long long frame_seq = 0;
+  uint32_t epoch = 0;
+  uint32_t n_upper = 0;  // host upper bound of N (no device sync on the integrate path)
+  int last_M = 0;
+  bool has_last = false;
+  void *tc = nullptr;
+  size_t elem() const { return dtype == FARM_DTYPE_F32 ? 4 : 2; }
+};
+
+namespace {
+
+__global__ void init_objects_kernel(DevMap m) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m.max_objects) return;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    m.aabb[i * 6 + k] = 0x7FFFFFFF;  // +NaN-side maximum of the ordered image: any finite value is smaller
+    m.aabb[i * 6 + 3 + k] = (int)0x80000000;
+  }
+  m.leader[i] = 0xFFFFFFFFu;
+}
+
+__global__ void export_objects_kernel(DevMap m, farm_object *out, uint32_t n) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  farm_object o;
+  o.id = (int32_t)i;
+  o.n_voxels = m.n_voxels[i];
+  o.n_obs = m.n_obs[i];
+  for (int k = 0; k < 3; ++k) {
+    o.aabb_min[k] = ord2f(m.aabb[i * 6 + k]);
+    o.aabb_max[k] = ord2f(m.aabb[i * 6 + 3 + k]);
+    o.best_cam_pos[k] = m.best_cam[i * 3 + k];
+  }
+  const unsigned long long bv = m.best_view[i];
+  if (bv) {
+    o.best_pixels = (uint32_t)(bv >> 40);
+    o.best_frame = (int32_t)(~(bv >> 16) & 0xFFFFFFull);
+    o.best_det = (int32_t)(~bv & 0xFFFFull);
+  } else {
+    o.best_pixels = 0, o.best_frame = -1, o.best_det = -1;
+  }
+  o.n_points = m.n_points[i];
+  out[i] = o;
+}
+
+__global__ void import_objects_kernel(DevMap m, const farm_object *in, uint32_t n) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const farm_object o = in[i];
+  m.n_voxels[i] = o.n_voxels;
+  m.n_obs[i] = o.n_obs;
+  m.n_points[i] = o.n_points;
+  for (int k = 0; k < 3; ++k) {
+    m.aabb[i * 6 + k] = f2ord(o.aabb_min[k]);
+    m.aabb[i * 6 + 3 + k] = f2ord(o.aabb_max[k]);
+    m.best_cam[i * 3 + k] = o.best_cam_pos[k];
+  }
+  m.best_view[i] = o.best_frame < 0 ? 0ull
+                                    : ((unsigned long long)(o.best_pixels & 0xFFFFFFu) << 40) |
+                                          ((~(unsigned long long)o.best_frame & 0xFFFFFFull) << 16) |
+                                          (~(unsigned long long)o.best_det & 0xFFFFull);
+}
+
+// R26: renormalise imported fp32 rows (fp32 arithmetic), write master, shadow and inverse shadow norm
+template <typename T>
+__global__ void __launch_bounds__(256) renorm_rows_kernel(DevMap m, uint32_t n) {
+  __shared__ float red[8];
+  __shared__ float bc;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (uint32_t r = blockIdx.x; r < n; r += gridDim.x) {
+    float *row = m.desc_master + (size_t)r * m.D;
+    T *sh = (T *)m.desc_shadow + (size_t)r * m.D;
+    float ss = 0.f;
+    for (int i = tid; i < m.D; i += 256) ss = fmaf(row[i], row[i], ss);
+    for (int s = 16; s; s >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, s);
+    if (lane == 0) red[warp] = ss;
+    __syncthreads();
+    if (tid == 0) {
+      float t = 0.f;
+      for (int w = 0; w < 8; ++w) t += red[w];
+      bc = t;
+    }
+    __syncthreads();
+    const float inv = bc > 0.f ? 1.0f / sqrtf(bc) : 0.f;
+    float s2 = 0.f;
+    for (int i = tid; i < m.D; i += 256) {
+      const float v = row[i] * inv;
+      row[i] = v;
+      const T q = from_f32<T>(v);
+      sh[i] = q;
+      const float qv = to_f32<T>(q);
+      s2 = fmaf(qv, qv, s2);
+    }
+    for (int s = 16; s; s >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, s);
+    __syncthreads();
+    if (lane == 0) red[warp] = s2;
+    __syncthreads();
+    if (tid == 0) {
+      float t = 0.f;
+      for (int w = 0; w < 8; ++w) t += red[w];
+      m.inv_norm[r] = t > 0.f ? 1.0f / sqrtf(t) : 0.f;
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void import_voxels_kernel(DevMap m, const unsigned long long *keys, const uint32_t *owners, long long n,
+                                     uint32_t n_objects) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const unsigned long long key = keys[i];
+    const uint32_t owner = owners[i];
+    if (owner >= n_objects || key == KEY_EMPTY) {
+      atomicOr(m.err, ERR_IMPORT_DUPLICATE);
+      continue;
+    }
+    unsigned long long h = mix64(key) & m.table_mask;
+    bool done = false;
+    for (unsigned long long probe = 0; probe <= m.table_mask && probe < (1ull << 20); ++probe) {
+      unsigned long long k = m.table[h].key;
+      if (k == KEY_EMPTY) {
+        k = atomicCAS(&m.table[h].key, KEY_EMPTY, key);
+        if (k == KEY_EMPTY) {
+          m.table[h].owner = owner;
+          done = true;
+          break;
+        }
+      }
+      if (k == key) {
+        atomicOr(m.err, ERR_IMPORT_DUPLICATE);
+        done = true;
+        break;
+      }
+      h = (h + 1) & m.table_mask;
+    }
+    if (!done) atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
+  }
+}
+
+__global__ void count_voxels_kernel(DevMap m, unsigned long long *count) {
+  unsigned long long c = 0;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
+       i += (unsigned long long)gridDim.x * blockDim.x)
+    c += m.table[i].key != KEY_EMPTY;
+  for (int s = 16; s; s >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, s);
+  if ((threadIdx.x & 31) == 0 && c) atomicAdd(count, c);
+}
+
+__global__ void export_voxels_kernel(DevMap m, unsigned long long *keys, uint32_t *owners, unsigned long long *cursor,
+                                     unsigned long long cap) {
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    const VoxelSlot sl = m.table[i];
+    if (sl.key != KEY_EMPTY) {
+      const unsigned long long p = atomicAdd(cursor, 1ull);
+      if (p < cap) {
+        keys[p] = sl.key;
+        owners[p] = sl.owner;
+      }
+    }
+  }
+}
+
+__global__ void gather_pairs_kernel(DevMap m, uint32_t n, uint32_t *js, unsigned long long *keys) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const unsigned long long p = m.pair_list[i];
+  js[i] = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
+  keys[i] = m.table[(uint32_t)p].key;
+}
+
+long long next_pow2(long long x) {
+  long long p = 1;
+  while (p < x) p <<= 1;
+  return p;
+}
+
+template <typename T>
+int dev_alloc(farm_map *m, T **p, size_t count, int fill_byte) {
+  void *q = nullptr;
+  const size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+  CU(cudaMalloc(&q, bytes));
+  m->allocs.push_back(q);
+  CU(cudaMemsetAsync(q, fill_byte, bytes, m->stream));
+  *p = (T *)q;
+  return FARM_OK;
+}
+
+int finalise(farm_map *m) {
+  if (m->finalised) return FARM_OK;
+  if (m->H <= 0 || m->W <= 0) return fail(FARM_ERR_STATE, "FARM_OPT_IMG_W / FARM_OPT_IMG_H must be set before the first call");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(FARM_ERR_CUDA, "no CUDA device: the FARM mapping path has no CPU fallback");
+  if (m->max_pairs <= 0) m->max_pairs = std::min<long long>((long long)m->H * m->W * std::min<long long>(m->max_frames, 4), 1ll << 23);
+  DevMap &d = m->dm;
+  d.inv_vs = 1.0f / m->voxel_size;  // R6: fp32 reciprocal, computed once
+  d.w_geo = m->w_geo, d.w_sem = m->w_sem, d.tau = m->tau, d.z_min = m->z_min, d.z_max = m->z_max;
+  d.D = m->D, d.dtype = m->dtype, d.H = m->H, d.W = m->W;
+  d.max_objects = (uint32_t)m->max_objects;
+  const size_t NO = (size_t)m->max_objects, D = (size_t)m->D;
+  int rc;
+#define A(ptr, count, fill)                                        \
+  if ((rc = dev_alloc(m, &(ptr), (count), (fill))) != FARM_OK) return rc
+  A(d.n_objects, 1, 0);
+  A(d.desc_master, NO * D, 0);
+  {
+    uint8_t *p;
+    A(p, NO * D * m->elem(), 0);
+    d.desc_shadow = p;
+  }
+  A(d.inv_norm, NO, 0);
+  A(d.n_voxels, NO, 0);
+  A(d.n_obs, NO, 0);
+  A(d.n_points, NO, 0);
+  A(d.aabb, NO * 6, 0);
+  A(d.best_view, NO, 0);
+  A(d.best_cam, NO * 3, 0);
+  A(d.leader, NO, 0xFF);
+  const long long tcap = next_pow2(std::max<long long>(2 * m->max_voxels, 1024));
+  A(d.table, (size_t)tcap, 0xFF);  // key = EMPTY, owner = PENDING, claim = NONE
+  d.table_mask = (unsigned long long)tcap - 1;
+  const long long pcap = next_pow2(2 * m->max_pairs);
+  A(d.pair_set, (size_t)pcap, 0);
+  d.pair_mask = (uint32_t)(pcap - 1);
+  A(d.pair_list, (size_t)m->max_pairs, 0);
+  d.pair_cap = (uint32_t)m->max_pairs;
+  const long long ccap = std::min<long long>(std::max<long long>(m->max_pairs / 4, 16384), 1ll << 22);
+  const long long ocap = next_pow2(2 * ccap);
+  A(d.ov_keys, (size_t)ocap, 0);
+  A(d.ov_cnt, (size_t)ocap, 0);
+  d.ov_mask = (uint32_t)(ocap - 1);
+  A(d.cand_slot, (size_t)ccap, 0);
+  A(d.cand_j, (size_t)ccap, 0);
+  A(d.cand_o, (size_t)ccap, 0);
+  A(d.cand_c, (size_t)ccap, 0);
+  d.cand_cap = (uint32_t)ccap;
+  A(d.counters, 4, 0);
+  const size_t MD = (size_t)m->max_det;
+  d.max_det = (uint32_t)MD;
+  A(d.det_nv, MD, 0);
+  A(d.det_npx, MD, 0);
+  A(d.det_box, MD * 6, 0);
+  A(d.det_inv_norm, MD, 0);
+  A(d.best_cand, MD, 0);
+  A(d.best_dense, MD, 0);
+  A(d.assoc, MD, 0);
+  A(d.is_new, MD, 0);
+  A(d.best_score, MD, 0);
+  A(d.stats, 1, 0);
+  A(d.totals, 1, 0);
+  A(d.err, 1, 0);
+#undef A
+  init_objects_kernel<<<(unsigned)((NO + 255) / 256), 256, 0, m->stream>>>(d);
+  m->launches++;
+  CU(cudaGetLastError());
+  if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
+  if (m->sim_path == 2 && !m->tc) return fail(FARM_ERR_INVALID_ARG, "tensor-core similarity path not available for this dtype / D");
+  m->finalised = true;
+  return FARM_OK;
+}
+
+int device_error(farm_map *m) {
+  uint32_t e = 0;
+  CU(cudaMemcpyAsync(&e, m->dm.err, 4, cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  if (e == 0) return FARM_OK;
+  char buf[160];
+  snprintf(buf, sizeof buf, "sticky device error 0x%x:%s%s%s%s%s", e, (e & ERR_VOXEL_TABLE_FULL) ? " voxel table full" : "",
+           (e & ERR_PAIR_TABLE_FULL) ? " per-call pair scratch full" : "",
+           (e & ERR_OVERLAP_TABLE_FULL) ? " per-call overlap scratch full" : "",
+           (e & ERR_OBJECT_CAPACITY) ? " object capacity" : "", (e & ERR_IMPORT_DUPLICATE) ? " import: duplicate key or bad owner" : "");
+  return fail((e & ERR_IMPORT_DUPLICATE) ? FARM_ERR_INVALID_ARG : FARM_ERR_CAPACITY, buf);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *farm_last_error(void) { return g_err.c_str(); }
+
+int farm_map_create(float voxel_size, int D, float w_geo, float w_sem, float tau, farm_map **out) {
+  if (!out) return fail(FARM_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (!(voxel_size > 0.f) || !std::isfinite(voxel_size)) return fail(FARM_ERR_INVALID_ARG, "voxel_size must be > 0");
+  if (D < 1 || D > 8192) return fail(FARM_ERR_INVALID_ARG, "D must be in 1..8192");
+  if (!(w_geo >= 0.f) || !(w_sem >= 0.f) || !std::isfinite(w_geo) || !std::isfinite(w_sem) || std::isnan(tau))
+    return fail(FARM_ERR_INVALID_ARG, "w_geo and w_sem must be finite and >= 0");
+  farm_map *m = new farm_map();
+  m->voxel_size = voxel_size, m->D = D, m->w_geo = w_geo, m->w_sem = w_sem, m->tau = tau;
+  *out = m;
+  return FARM_OK;
+}
+
+int farm_map_destroy(farm_map *m) {
+  if (!m) return FARM_OK;
+  if (m->finalised || !m->allocs.empty()) cudaStreamSynchronize(m->stream);
+  if (m->tc) tc_state_destroy(m->tc);
+  for (void *p : m->allocs) cudaFree(p);
+  delete m;
+  return FARM_OK;
+}
+
+int farm_map_set_option_i(farm_map *m, int key, long long v) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (m->finalised) return fail(FARM_ERR_STATE, "options are frozen after the first integrate / import");
+  switch (key) {
+    case FARM_OPT_DESC_DTYPE:
+      if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad dtype");
+      m->dtype = (int)v;
+      break;
+    case FARM_OPT_MAX_OBJECTS:
+      if (v < 1 || v > (1ll << 31) - 2) return fail(FARM_ERR_INVALID_ARG, "bad MAX_OBJECTS");
+      m->max_objects = v;
+      break;
+    case FARM_OPT_MAX_VOXELS:
+      if (v < 1 || v > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_VOXELS");
+      m->max_voxels = v;
+      break;
+    case FARM_OPT_IMG_W:
+      if (v < 1 || v > 65536) return fail(FARM_ERR_INVALID_ARG, "bad IMG_W");
+      m->W = (int)v;
+      break;
+    case FARM_OPT_IMG_H:
+      if (v < 1 || v > 65536) return fail(FARM_ERR_INVALID_ARG, "bad IMG_H");
+      m->H = (int)v;
+      break;
+    case FARM_OPT_MAX_DET_PER_CALL:
+      if (v < 1 || v >= (1ll << DET_BITS)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_DET_PER_CALL");
+      m->max_det = v;
+      break;
+    case FARM_OPT_STREAM:
+      m->stream = (cudaStream_t)(uintptr_t)v;
+      break;
+    case FARM_OPT_MAX_PAIRS_PER_CALL:
+      if (v < 1024 || v > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_PAIRS_PER_CALL");
+      m->max_pairs = v;
+      break;
+    case FARM_OPT_MAX_FRAMES_PER_CALL:
+      if (v < 1 || v > MAX_FRAMES) return fail(FARM_ERR_INVALID_ARG, "bad MAX_FRAMES_PER_CALL");
+      m->max_frames = v;
+      break;
+    case FARM_OPT_SIM_PATH:
+      if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad SIM_PATH");
+      m->sim_path = (int)v;
+      break;
+    default:
+      return fail(FARM_ERR_INVALID_ARG, "unknown integer option");
+  }
+  return FARM_OK;
+}
+
+int farm_map_set_option_f(farm_map *m, int key, float v) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (m->finalised) return fail(FARM_ERR_STATE, "options are frozen after the first integrate / import");
+  if (std::isnan(v)) return fail(FARM_ERR_INVALID_ARG, "NaN option");
+  if (key == FARM_OPTF_Z_MIN)
+    m->z_min = v;
+  else if (key == FARM_OPTF_Z_MAX)
+    m->z_max = v;
+  else
+    return fail(FARM_ERR_INVALID_ARG, "unknown float option");
+  return FARM_OK;
+}
+
+int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint16_t *mask, const float *K,
+                             const float *T, const void *desc, const int *n_det) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (F < 1 || F > m->max_frames) return fail(FARM_ERR_INVALID_ARG, "n_frames out of range (FARM_OPT_MAX_FRAMES_PER_CALL)");
+  if (!depth || !mask || !K || !T || !n_det) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  CallArgs a{};
+  a.F = F;
+  long long M = 0;
+  for (int f = 0; f < F; ++f) {
+    if (n_det[f] < 0 || n_det[f] > 65535) return fail(FARM_ERR_INVALID_ARG, "n_det must be in 0..65535");
+    a.base[f] = (int)M;
+    M += n_det[f];
+  }
+  a.base[F] = (int)M;
+  if (M > m->max_det) return fail(FARM_ERR_INVALID_ARG, "too many detections in one call (FARM_OPT_MAX_DET_PER_CALL)");
+  if (M > 0 && !desc) return fail(FARM_ERR_INVALID_ARG, "det_descriptors is NULL");
+  int rc = finalise(m);
+  if (rc != FARM_OK) return rc;
+  if (m->epoch == EPOCH_MAX) {  // the epoch tag wrapped: clear the per-call scratch tables once
+    CU(cudaMemsetAsync(m->dm.pair_set, 0, ((size_t)m->dm.pair_mask + 1) * 8, m->stream));
+    CU(cudaMemsetAsync(m->dm.ov_keys, 0, ((size_t)m->dm.ov_mask + 1) * 8, m->stream));
+    m->epoch = 0;
+  }
+  a.M = (int)M;
+  a.epoch = ++m->epoch;
+  a.depth = depth, a.mask = mask, a.K = K, a.T = T, a.desc = desc;
+  const DevMap &d = m->dm;
+  m->launches += launch_prep(d, a, m->stream);
+  m->launches += launch_lift(d, a, m->stream);
+  if (m->tc)
+    m->launches += launch_similarity_tc(d, a, m->n_upper, m->stream, m->tc);
+  else
+    m->launches += launch_similarity_fma(d, a, m->n_upper, m->stream);
+  m->launches += launch_assoc_merge_seq(d, a, m->frame_seq, m->stream);
+  CU(cudaGetLastError());
+  m->frame_seq += F;
+  m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
+  m->last_M = (int)M;
+  m->has_last = true;
+  return FARM_OK;
+}
+
+int farm_map_integrate(farm_map *m, const float *depth, const uint16_t *mask, const float *K, const float *T,
+                       const void *desc, int n_det) {
+  return farm_map_integrate_batch(m, 1, depth, mask, K, T, desc, &n_det);
+}
+
+int farm_map_sync(farm_map *m, farm_totals *totals) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->finalised) {
+    if (totals) memset(totals, 0, sizeof *totals);
+    return FARM_OK;
+  }
+  if (totals) CU(cudaMemcpyAsync(totals, m->dm.totals, sizeof(Totals), cudaMemcpyDeviceToHost, m->stream));
+  uint32_t n = 0;
+  CU(cudaMemcpyAsync(&n, m->dm.n_objects, 4, cudaMemcpyDeviceToHost, m->stream));
+  int rc = device_error(m);
+  m->n_upper = n;  // tighten the host bound
+  return rc;
+}
+
+long long farm_map_kernel_launches(const farm_map *m) { return m ? m->launches : 0; }
+
+int farm_map_last_assoc(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score, farm_frame_stats *stats) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  const size_t M = (size_t)m->last_M;
+  if (obj_id && M) CU(cudaMemcpyAsync(obj_id, m->dm.assoc, M * 4, cudaMemcpyDeviceToHost, m->stream));
+  if (is_new && M) CU(cudaMemcpyAsync(is_new, m->dm.is_new, M, cudaMemcpyDeviceToHost, m->stream));
+  if (best_score && M) CU(cudaMemcpyAsync(best_score, m->dm.best_score, M * 4, cudaMemcpyDeviceToHost, m->stream));
+  static_assert(sizeof(farm_frame_stats) == sizeof(CallStats), "stats layout");
+  if (stats) CU(cudaMemcpyAsync(stats, m->dm.stats, sizeof(CallStats), cudaMemcpyDeviceToHost, m->stream));
+  return device_error(m);
+}
+
+int farm_map_read(farm_map *m, farm_object *objects, int *n_objects, float *descriptors, uint64_t *voxel_keys,
+                  uint32_t *voxel_owner, long long *n_voxels) {
+  if (!m || !n_objects) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->finalised) {
+    *n_objects = 0;
+    if (n_voxels) *n_voxels = 0;
+    return FARM_OK;
+  }
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  m->n_upper = N;
+  *n_objects = (int)N;
+  unsigned long long nv = 0;
+  if (n_voxels || voxel_keys || voxel_owner) {
+    unsigned long long *cnt;
+    CU(cudaMalloc(&cnt, 8));
+    CU(cudaMemsetAsync(cnt, 0, 8, m->stream));
+    count_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm, cnt);
+    m->launches++;
+    CU(cudaMemcpyAsync(&nv, cnt, 8, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+    if (n_voxels) *n_voxels = (long long)nv;
+    if ((voxel_keys || voxel_owner) && nv) {
+      unsigned long long *dk;
+      uint32_t *dvo;
+      CU(cudaMalloc(&dk, nv * 8));
+      CU(cudaMalloc(&dvo, nv * 4));
+      CU(cudaMemsetAsync(cnt, 0, 8, m->stream));
+      export_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm, dk, dvo, cnt, nv);
+      m->launches++;
+      if (voxel_keys) CU(cudaMemcpyAsync(voxel_keys, dk, nv * 8, cudaMemcpyDeviceToHost, m->stream));
+      if (voxel_owner) CU(cudaMemcpyAsync(voxel_owner, dvo, nv * 4, cudaMemcpyDeviceToHost, m->stream));
+      CU(cudaStreamSynchronize(m->stream));
+      cudaFree(dk);
+      cudaFree(dvo);
+    }
+    cudaFree(cnt);
+  }
+  if (objects && N) {
+    farm_object *dobj;
+    CU(cudaMalloc(&dobj, (size_t)N * sizeof(farm_object)));
+    export_objects_kernel<<<(N + 255) / 256, 256, 0, m->stream>>>(m->dm, dobj, N);
+    m->launches++;
+    CU(cudaMemcpyAsync(objects, dobj, (size_t)N * sizeof(farm_object), cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+    cudaFree(dobj);
+  }
+  if (descriptors && N) {
+    CU(cudaMemcpyAsync(descriptors, m->dm.desc_master, (size_t)N * m->D * 4, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+  }
+  return FARM_OK;
+}
+
+int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, const float *descriptors,
+                    const uint64_t *voxel_keys, const uint32_t *voxel_owner, long long n_voxels) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (n_objects < 0 || n_voxels < 0 || (n_objects && (!objects || !descriptors)) || (n_voxels && (!voxel_keys || !voxel_owner)))
+    return fail(FARM_ERR_INVALID_ARG, "bad import arguments");
+  if (m->has_last || m->n_upper) return fail(FARM_ERR_STATE, "import needs an empty map");
+  if (n_objects > m->max_objects) return fail(FARM_ERR_CAPACITY, "more objects than FARM_OPT_MAX_OBJECTS");
+  if (n_voxels > m->max_voxels) return fail(FARM_ERR_CAPACITY, "more voxels than FARM_OPT_MAX_VOXELS");
+  for (int i = 0; i < n_objects; ++i)
+    if (objects[i].id != i) return fail(FARM_ERR_INVALID_ARG, "object ids must be 0..n-1 in order");
+  int rc = finalise(m);
+  if (rc != FARM_OK) return rc;
+  const DevMap &d = m->dm;
+  if (n_objects) {
+    farm_object *dobj;
+    CU(cudaMalloc(&dobj, (size_t)n_objects * sizeof(farm_object)));
+    CU(cudaMemcpyAsync(dobj, objects, (size_t)n_objects * sizeof(farm_object), cudaMemcpyHostToDevice, m->stream));
+    import_objects_kernel<<<(n_objects + 255) / 256, 256, 0, m->stream>>>(d, dobj, (uint32_t)n_objects);
+    CU(cudaMemcpyAsync(d.desc_master, descriptors, (size_t)n_objects * m->D * 4, cudaMemcpyHostToDevice, m->stream));
+    const int grid = std::min(n_objects, 148 * 8);
+    if (m->dtype == FARM_DTYPE_F32)
+      renorm_rows_kernel<float><<<grid, 256, 0, m->stream>>>(d, (uint32_t)n_objects);
+    else if (m->dtype == FARM_DTYPE_F16)
+      renorm_rows_kernel<__half><<<grid, 256, 0, m->stream>>>(d, (uint32_t)n_objects);
+    else
+      renorm_rows_kernel<__nv_bfloat16><<<grid, 256, 0, m->stream>>>(d, (uint32_t)n_objects);
+    m->launches += 2;
+    uint32_t n = (uint32_t)n_objects;
+    CU(cudaMemcpyAsync(d.n_objects, &n, 4, cudaMemcpyHostToDevice, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+    cudaFree(dobj);
+  }
+  // voxels in chunks so that the staging buffers stay small
+  const long long chunk = 1ll << 24;
+  if (n_voxels) {
+    unsigned long long *dk;
+    uint32_t *dow;
+    CU(cudaMalloc(&dk, (size_t)std::min(chunk, n_voxels) * 8));
+    CU(cudaMalloc(&dow, (size_t)std::min(chunk, n_voxels) * 4));
+    for (long long off = 0; off < n_voxels; off += chunk) {
+      const long long n = std::min(chunk, n_voxels - off);
+      CU(cudaMemcpyAsync(dk, voxel_keys + off, (size_t)n * 8, cudaMemcpyHostToDevice, m->stream));
+      CU(cudaMemcpyAsync(dow, voxel_owner + off, (size_t)n * 4, cudaMemcpyHostToDevice, m->stream));
+      import_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(d, dk, dow, n, (uint32_t)n_objects);
+      m->launches++;
+      CU(cudaStreamSynchronize(m->stream));
+    }
+    cudaFree(dk);
+    cudaFree(dow);
+  }
+  CU(cudaGetLastError());
+  m->n_upper = (uint32_t)n_objects;
+  return device_error(m);
+}
+
+int farm_debug_backproject(farm_map *m, const float *depth, const uint16_t *mask, const float *K, const float *T,
+                           int n_det, float *xyz, uint64_t *keys) {
+  if (!m || !depth || !mask || !K || !T || !xyz || !keys) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  int rc = finalise(m);
+  if (rc != FARM_OK) return rc;
+  m->launches += launch_debug_backproject(m->dm, depth, mask, K, T, n_det, xyz, (unsigned long long *)keys, m->stream);
+  CU(cudaGetLastError());
+  return FARM_OK;
+}
+
+int farm_debug_last_voxels(farm_map *m, long long *offsets, uint64_t *keys, uint32_t *n_px, float *box) {
+  if (!m || !offsets) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  const int M = m->last_M;
+  uint32_t n = 0;
+  CU(cudaMemcpy(&n, m->dm.counters, 4, cudaMemcpyDeviceToHost));
+  std::vector<uint32_t> js(n);
+  std::vector<unsigned long long> ks(n);
+  if (n) {
+    uint32_t *dj;
+    unsigned long long *dk;
+    CU(cudaMalloc(&dj, (size_t)n * 4));
+    CU(cudaMalloc(&dk, (size_t)n * 8));
+    gather_pairs_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->dm, n, dj, dk);
+    m->launches++;
+    CU(cudaMemcpyAsync(js.data(), dj, (size_t)n * 4, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaMemcpyAsync(ks.data(), dk, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+    cudaFree(dj);
+    cudaFree(dk);
+  }
+  std::vector<long long> cnt(M + 1, 0);
+  for (uint32_t i = 0; i < n; ++i)
+    if ((int)js[i] < M) cnt[js[i] + 1]++;
+  for (int j = 0; j < M; ++j) cnt[j + 1] += cnt[j];
+  for (int j = 0; j <= M; ++j) offsets[j] = cnt[j];
+  if (keys) {
+    std::vector<long long> cur(cnt.begin(), cnt.end() - 1);
+    for (uint32_t i = 0; i < n; ++i)
+      if ((int)js[i] < M) keys[cur[js[i]]++] = ks[i];
+  }
+  if (n_px && M) CU(cudaMemcpy(n_px, m->dm.det_npx, (size_t)M * 4, cudaMemcpyDeviceToHost));
+  if (box && M) {
+    std::vector<int> ob((size_t)M * 6);
+    CU(cudaMemcpy(ob.data(), m->dm.det_box, (size_t)M * 24, cudaMemcpyDeviceToHost));
+    for (size_t i = 0; i < ob.size(); ++i) {
+      const int v = ob[i] ^ ((ob[i] >> 31) & 0x7FFFFFFF);
+      memcpy(&box[i], &v, 4);
+    }
+  }
+  return FARM_OK;
+}
+
+int farm_debug_last_overlaps(farm_map *m, long long *offsets, int32_t *obj_id, uint32_t *count) {
+  if (!m || !offsets) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  const int M = m->last_M;
+  uint32_t n = 0;
+  CU(cudaMemcpy(&n, m->dm.counters + 1, 4, cudaMemcpyDeviceToHost));
+  std::vector<uint32_t> js(n), cs(n);
+  std::vector<int32_t> os(n);
+  if (n) {
+    CU(cudaMemcpy(js.data(), m->dm.cand_j, (size_t)n * 4, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(os.data(), m->dm.cand_o, (size_t)n * 4, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(cs.data(), m->dm.cand_c, (size_t)n * 4, cudaMemcpyDeviceToHost));
+  }
+  std::vector<long long> cnt(M + 1, 0);
+  for (uint32_t i = 0; i < n; ++i)
+    if ((int)js[i] < M) cnt[js[i] + 1]++;
+  for (int j = 0; j < M; ++j) cnt[j + 1] += cnt[j];
+  for (int j = 0; j <= M; ++j) offsets[j] = cnt[j];
+  if (obj_id || count) {
+    std::vector<long long> cur(cnt.begin(), cnt.end() - 1);
+    for (uint32_t i = 0; i < n; ++i)
+      if ((int)js[i] < M) {
+        const long long p = cur[js[i]]++;
+        if (obj_id) obj_id[p] = os[i];
+        if (count) count[p] = cs[i];
+      }
+  }
+  return FARM_OK;
+}
+
+int farm_debug_last_dense(farm_map *m, float *max_cos, int32_t *argmax) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  const int M = m->last_M;
+  std::vector<unsigned long long> bd(M);
+  if (M) CU(cudaMemcpy(bd.data(), m->dm.best_dense, (size_t)M * 8, cudaMemcpyDeviceToHost));
+  for (int j = 0; j < M; ++j) {
+    if (bd[j]) {
+      const uint32_t u = (uint32_t)(bd[j] >> 32) ^ 0x80000000u;
+      const int i = (int)u;
+      const int f = i ^ ((i >> 31) & 0x7FFFFFFF);
+      if (max_cos) memcpy(&max_cos[j], &f, 4);
+      if (argmax) argmax[j] = (int32_t)(0xFFFFFFFFu - (uint32_t)bd[j]);
+    } else {
+      if (max_cos) max_cos[j] = 0.f;
+      if (argmax) argmax[j] = -1;
+    }
+  }
+  return FARM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,324 @@
+// farm_assoc.cu -- step 5: candidate scoring, association (argmax / threshold / spawn) and merge.
+//   R10, R17-R20 (score, strict threshold, ids in detection index order; BASELINE.json rule)
+//   R12 (voxel commit, lowest detection index wins), R21 (count-weighted descriptor mean),
+//   R22 (AABB), R23 (view evidence).
+#include "farm_internal.cuh"
+
+namespace farm {
+namespace {
+
+constexpr uint32_t NONE32 = 0xFFFFFFFFu;
+
+// ---- candidate scoring: one warp per non-zero overlap entry (d, o, c)
+template <typename T>
+__global__ void __launch_bounds__(128) cand_score_kernel(DevMap m, CallArgs a) {
+  const uint32_t n_cand = min(m.counters[1], m.cand_cap);
+  const int lane = threadIdx.x & 31;
+  const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+  const int D = m.D;
+  for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < n_cand; c += warps) {
+    const uint32_t slot = m.cand_slot[c];
+    const unsigned long long kv = m.ov_keys[slot];
+    const uint32_t j = (uint32_t)(kv >> 32) & ((1u << DET_BITS) - 1);
+    const uint32_t o = (uint32_t)kv;
+    const uint32_t cnt = m.ov_cnt[slot];
+    __syncwarp();
+    if (lane == 0) {
+      m.ov_cnt[slot] = 0;  // invariant: counts are zero between calls (the tables are epoch tagged)
+      m.cand_j[c] = j;
+      m.cand_o[c] = (int32_t)o;
+      m.cand_c[c] = cnt;
+    }
+    const T *x = (const T *)a.desc + (size_t)j * D;
+    const T *y = (const T *)m.desc_shadow + (size_t)o * D;
+    float dot = 0.f;
+    if (sizeof(T) == 2 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {
+      for (int i = lane * 8; i < D; i += 256) {
+        const uint4 xv = *reinterpret_cast<const uint4 *>(x + i);
+        const uint4 yv = *reinterpret_cast<const uint4 *>(y + i);
+        const T *xe = reinterpret_cast<const T *>(&xv);
+        const T *ye = reinterpret_cast<const T *>(&yv);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) dot = fmaf(to_f32<T>(xe[q]), to_f32<T>(ye[q]), dot);
+      }
+    } else {
+      for (int i = lane; i < D; i += 32) dot = fmaf(to_f32<T>(x[i]), to_f32<T>(y[i]), dot);
+    }
+#pragma unroll
+    for (int s = 16; s; s >>= 1) dot += __shfl_xor_sync(0xFFFFFFFFu, dot, s);
+    if (lane == 0) {
+      float cs = dot * m.det_inv_norm[j] * m.inv_norm[o];
+      cs = fminf(1.f, fmaxf(-1.f, cs));                                  // R15
+      const uint32_t mn = min(m.det_nv[j], m.n_voxels[o]);
+      const float g = mn ? __fdiv_rn((float)cnt, (float)mn) : 0.f;       // R10
+      const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));  // R17
+      atomicMax(&m.best_cand[j], pack_score(score, o));
+    }
+  }
+}
+
+// ---- association: one CTA; decisions, new ids by an exclusive scan in detection index order (R18, R20)
+__global__ void __launch_bounds__(1024) associate_kernel(DevMap m, CallArgs a) {
+  __shared__ uint32_t warp_sum[32];
+  __shared__ uint32_t s_running, s_matches, s_skipped;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t N = *m.n_objects;
+  if (tid == 0) s_running = 0, s_matches = 0, s_skipped = 0;
+  __syncthreads();
+  for (int base = 0; base < a.M; base += 1024) {
+    const int j = base + tid;
+    uint32_t spawn = 0, matched = 0, skipped = 0;
+    int32_t target = -1;
+    float score = 0.f;
+    if (j < a.M) {
+      if (m.det_npx[j] == 0) {
+        skipped = 1;  // R8
+      } else {
+        unsigned long long best = m.best_cand[j];
+        const unsigned long long bd = m.best_dense[j];
+        if (bd) {
+          // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
+          const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd)));
+          const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd) : 0u);
+          best = pd > best ? pd : best;
+        }
+        if (best) {
+          score = unpack_score(best);
+          if (score > m.tau) {  // strict (R18)
+            matched = 1;
+            target = (int32_t)unpack_id(best);
+          }
+        }
+        spawn = matched ? 0u : 1u;
+      }
+    }
+    // block exclusive scan of the spawn flags
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, spawn);
+    if (lane == 0) warp_sum[warp] = __popc(b);
+    __syncthreads();
+    uint32_t before = 0, total = 0;
+    for (int w = 0; w < 32; ++w) {
+      const uint32_t c = warp_sum[w];
+      before += w < warp ? c : 0;
+      total += c;
+    }
+    const uint32_t running = s_running;
+    if (spawn) {
+      const uint32_t id = N + running + before + __popc(b & ((1u << lane) - 1));
+      if (id < m.max_objects) {
+        target = (int32_t)id;
+      } else {
+        atomicOr(m.err, ERR_OBJECT_CAPACITY);
+        spawn = 0, skipped = 1;
+      }
+    }
+    if (j < a.M) {
+      m.assoc[j] = target;
+      m.is_new[j] = (uint8_t)spawn;
+      m.best_score[j] = score;
+      if (target >= 0) atomicMin(&m.leader[target], (uint32_t)j);
+    }
+    const unsigned bm = __ballot_sync(0xFFFFFFFFu, matched), bs = __ballot_sync(0xFFFFFFFFu, skipped);
+    if (lane == 0) {
+      if (bm) atomicAdd(&s_matches, (uint32_t)__popc(bm));
+      if (bs) atomicAdd(&s_skipped, (uint32_t)__popc(bs));
+    }
+    __syncthreads();
+    if (tid == 0) s_running = running + total;
+    __syncthreads();
+  }
+  if (tid == 0) {
+    uint32_t spawns = s_running;
+    if (N + spawns > m.max_objects) spawns = m.max_objects - N;
+    *m.n_objects = N + spawns;
+    m.stats->matches = s_matches;
+    m.stats->spawns = spawns;
+    m.stats->skipped = s_skipped;
+    m.stats->unique_voxels = m.counters[0];
+    m.totals->frames += a.F;
+    m.totals->calls += 1;
+    m.totals->valid_points += m.stats->valid_points;
+    m.totals->unique_voxels += m.counters[0];
+    m.totals->matches += s_matches;
+    m.totals->spawns += spawns;
+  }
+}
+
+// ---- voxel commit (R12 pass 2): the claim winner of every key inserted by this call sets the owner
+__global__ void __launch_bounds__(256) commit_voxels_kernel(DevMap m) {
+  const uint32_t n = min(m.counters[0], m.pair_cap);
+  const int lane = threadIdx.x & 31;
+  for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const uint32_t i = i0 + lane;
+    int32_t t = -1;
+    if (i < n) {
+      const unsigned long long p = m.pair_list[i];
+      if (p >> 63) {
+        const uint32_t j = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
+        const uint32_t slot = (uint32_t)p;
+        if (m.table[slot].claim == j) {
+          t = m.assoc[j];
+          if (t >= 0) m.table[slot].owner = (uint32_t)t;
+        }
+      }
+    }
+    const unsigned act = __ballot_sync(0xFFFFFFFFu, t >= 0);
+    if (t >= 0) {
+      const unsigned same = __match_any_sync(act, t);
+      if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], (uint32_t)__popc(same));
+    }
+  }
+}
+
+// ---- object merge: the lowest-index detection of every target object folds the whole group (R21-R23).
+// One CTA per detection; non-leaders exit at once.  No atomics, deterministic summation order.
+template <typename T>
+__global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0) {
+  extern __shared__ float acc[];  // [D]
+  __shared__ uint32_t list[256];
+  __shared__ uint32_t warp_cnt[8];
+  __shared__ float red[8];
+  __shared__ float s_bcast;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int D = m.D;
+  for (int j = blockIdx.x; j < a.M; j += gridDim.x) {
+    const int32_t t = m.assoc[j];
+    if (t < 0 || m.leader[t] != (uint32_t)j) continue;  // uniform per CTA
+    for (int i = tid; i < D; i += 256) acc[i] = 0.f;
+    // scalar aggregates live in thread 0
+    uint32_t k_members = 0;
+    unsigned long long pts = 0, best = 0;
+    int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+    int best_frame = -1;
+    __syncthreads();
+    for (int base = j & ~255; base < a.M; base += 256) {  // members have index >= j
+      const int jj = base + tid;
+      const bool flag = jj < a.M && jj >= j && m.assoc[jj] == t;
+      const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
+      if (lane == 0) warp_cnt[warp] = __popc(b);
+      __syncthreads();
+      uint32_t before = 0, total = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) {
+        before += w < warp ? warp_cnt[w] : 0;
+        total += warp_cnt[w];
+      }
+      if (flag) list[before + __popc(b & ((1u << lane) - 1))] = (uint32_t)jj;
+      __syncthreads();
+      for (uint32_t q = 0; q < total; ++q) {
+        const uint32_t jm = list[q];
+        const float inv = m.det_inv_norm[jm];  // zero-norm rows contribute nothing (R21)
+        const T *row = (const T *)a.desc + (size_t)jm * D;
+        for (int i = tid; i < D; i += 256) acc[i] = fmaf(to_f32<T>(row[i]), inv, acc[i]);
+        if (tid == 0) {
+          k_members++;
+          const uint32_t npx = m.det_npx[jm];
+          pts += npx;
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            bmn[c] = min(bmn[c], m.det_box[jm * 6 + c]);
+            bmx[c] = max(bmx[c], m.det_box[jm * 6 + 3 + c]);
+          }
+          int f = 0;
+          while (f + 1 < a.F && (int)jm >= a.base[f + 1]) ++f;
+          const unsigned long long seq = frame_seq0 + f;
+          const uint32_t det = jm - a.base[f];
+          // R23: most pixels wins, ties -> smallest (frame_seq, det)
+          const unsigned long long pv = ((unsigned long long)(npx & 0xFFFFFFu) << 40) |
+                                        ((~seq & 0xFFFFFFull) << 16) | (unsigned long long)(~det & 0xFFFFu);
+          if (pv > best) best = pv, best_frame = f;
+        }
+      }
+      __syncthreads();
+    }
+    // f_o <- normalise(n_obs * f_o + sum)   (R21)
+    const uint32_t n_old = m.n_obs[t];
+    float *master = m.desc_master + (size_t)t * D;
+    T *shadow = (T *)m.desc_shadow + (size_t)t * D;
+    float ss = 0.f;
+    for (int i = tid; i < D; i += 256) {
+      const float v = fmaf((float)n_old, master[i], acc[i]);
+      acc[i] = v;
+      ss = fmaf(v, v, ss);
+    }
+#pragma unroll
+    for (int s = 16; s; s >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, s);
+    if (lane == 0) red[warp] = ss;
+    __syncthreads();
+    if (tid == 0) {
+      float tot = 0.f;
+      for (int w = 0; w < 8; ++w) tot += red[w];
+      s_bcast = tot;
+    }
+    __syncthreads();
+    const float tot = s_bcast;
+    if (tot > 0.f) {  // a zero sum keeps the old value
+      const float inv = 1.0f / sqrtf(tot);
+      float s2 = 0.f;
+      for (int i = tid; i < D; i += 256) {
+        const float v = acc[i] * inv;
+        master[i] = v;
+        const T sh = from_f32<T>(v);  // round-to-nearest-even shadow (R1, R14)
+        shadow[i] = sh;
+        const float sv = to_f32<T>(sh);
+        s2 = fmaf(sv, sv, s2);
+      }
+#pragma unroll
+      for (int s = 16; s; s >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, s);
+      __syncthreads();
+      if (lane == 0) red[warp] = s2;
+      __syncthreads();
+      if (tid == 0) {
+        float t2 = 0.f;
+        for (int w = 0; w < 8; ++w) t2 += red[w];
+        m.inv_norm[t] = t2 > 0.f ? 1.0f / sqrtf(t2) : 0.f;
+      }
+    }
+    if (tid == 0) {
+      m.n_obs[t] = n_old + k_members;
+      m.n_points[t] += pts;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {  // R22
+        m.aabb[t * 6 + c] = min(m.aabb[t * 6 + c], bmn[c]);
+        m.aabb[t * 6 + 3 + c] = max(m.aabb[t * 6 + 3 + c], bmx[c]);
+      }
+      if (best > m.best_view[t]) {
+        m.best_view[t] = best;
+        const float *Tf = a.T + 16 * best_frame;
+        m.best_cam[t * 3 + 0] = Tf[3];
+        m.best_cam[t * 3 + 1] = Tf[7];
+        m.best_cam[t * 3 + 2] = Tf[11];
+      }
+      m.leader[t] = NONE32;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace
+
+template <typename T>
+static int launch_assoc_merge_t(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
+  int launches = 0;
+  if (a.M > 0) {
+    cand_score_kernel<T><<<296, 128, 0, s>>>(m, a);
+    ++launches;
+  }
+  associate_kernel<<<1, 1024, 0, s>>>(m, a);
+  ++launches;
+  if (a.M > 0) {
+    commit_voxels_kernel<<<296, 256, 0, s>>>(m);
+    const int grid = a.M < 148 * 8 ? a.M : 148 * 8;
+    merge_objects_kernel<T><<<grid, 256, (size_t)m.D * sizeof(float), s>>>(m, a, frame_seq0);
+    launches += 2;
+  }
+  return launches;
+}
+
+int launch_assoc_merge_seq(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
+  if (m.dtype == FARM_DTYPE_F32) return launch_assoc_merge_t<float>(m, a, frame_seq0, s);
+  if (m.dtype == FARM_DTYPE_F16) return launch_assoc_merge_t<__half>(m, a, frame_seq0, s);
+  return launch_assoc_merge_t<__nv_bfloat16>(m, a, frame_seq0, s);
+}
+
+}  // namespace farm

@@ -1,0 +1,158 @@
+// farm_internal.cuh -- device-side data layout and small helpers shared by the library's own kernels.
+// (Product code.  Shares nothing with oracle/.)
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/farm.h"
+
+namespace farm {
+
+constexpr uint64_t KEY_EMPTY = 0xFFFFFFFFFFFFFFFFull;
+constexpr uint32_t OWNER_PENDING = 0xFFFFFFFFu;  // slot inserted but not yet committed to an object
+constexpr uint32_t CLAIM_NONE = 0xFFFFFFFFu;
+constexpr int KEY_BIAS = 1 << 20;
+constexpr int MAX_FRAMES = 64;
+constexpr int EPOCH_BITS = 11;                    // per-call scratch tables are epoch tagged, never cleared
+constexpr int DET_BITS = 21;
+constexpr uint32_t EPOCH_MAX = (1u << EPOCH_BITS) - 1;
+
+// sticky device error bits
+constexpr uint32_t ERR_VOXEL_TABLE_FULL = 1u;
+constexpr uint32_t ERR_PAIR_TABLE_FULL = 2u;
+constexpr uint32_t ERR_OVERLAP_TABLE_FULL = 4u;
+constexpr uint32_t ERR_OBJECT_CAPACITY = 8u;
+constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
+
+// Global voxel -> object hash slot (R11: one owner per key).  16 bytes, one 32-byte sector per probe.
+struct __align__(16) VoxelSlot {
+  unsigned long long key;  // KEY_EMPTY when free
+  uint32_t owner;          // OWNER_PENDING until the inserting call commits
+  uint32_t claim;          // lowest detection index j of the inserting call that contains the key (R12)
+};
+
+struct CallStats {  // device mirror of farm_frame_stats
+  unsigned long long valid_points, dropped_points, ignored_pixels, unique_voxels;
+  uint32_t matches, spawns, skipped, n_det;
+};
+struct Totals {
+  unsigned long long frames, calls, valid_points, unique_voxels, matches, spawns;
+};
+
+// Everything a kernel needs, passed by value.
+struct DevMap {
+  // parameters
+  float inv_vs, w_geo, w_sem, tau, z_min, z_max;
+  int D, dtype, H, W;
+  // objects (SoA).  HBM layout: descriptors are [max_objects, D] row-major, D contiguous.
+  uint32_t max_objects;
+  uint32_t *n_objects;               // device scalar N
+  float *desc_master;                // fp32 masters (R21)
+  void *desc_shadow;                 // storage-dtype shadows: similarity operand B (R14)
+  float *inv_norm;                   // 1/|shadow_o| (0 for a zero row)
+  uint32_t *n_voxels, *n_obs;
+  unsigned long long *n_points;
+  int *aabb;                         // [max_objects,6] order-preserving int image of fp32 min xyz, max xyz
+  unsigned long long *best_view;     // packed (n_px, ~frame_seq, ~det) for max()
+  float *best_cam;                   // [max_objects,3]
+  uint32_t *leader;                  // scratch: lowest j of the call that targets the object
+  // voxel hash
+  VoxelSlot *table;
+  unsigned long long table_mask;     // capacity-1
+  // per-call scratch
+  unsigned long long *pair_set;      // epoch-tagged set of (j, slot)
+  uint32_t pair_mask;
+  unsigned long long *pair_list;     // unique (pending<<63 | j<<32 | slot)
+  uint32_t pair_cap;
+  unsigned long long *ov_keys;       // epoch-tagged map (j, owner) -> count
+  uint32_t *ov_cnt;
+  uint32_t ov_mask;
+  uint32_t *cand_slot;               // list of overlap-map slots created this call
+  uint32_t cand_cap;
+  uint32_t *cand_j;                  // compact copy for the debug read
+  int32_t *cand_o;
+  uint32_t *cand_c;
+  uint32_t *counters;                // [0]=pair_count [1]=cand_count
+  // per detection [max_det]
+  uint32_t max_det;
+  uint32_t *det_nv, *det_npx;
+  int *det_box;                      // [max_det,6] ordered ints
+  float *det_inv_norm;
+  unsigned long long *best_cand, *best_dense;
+  int32_t *assoc;
+  uint8_t *is_new;
+  float *best_score;
+  CallStats *stats;
+  Totals *totals;
+  uint32_t *err;
+};
+
+struct CallArgs {
+  int F, M;
+  uint32_t epoch;
+  const float *depth;
+  const uint16_t *mask;
+  const float *K;
+  const float *T;
+  const void *desc;
+  int base[MAX_FRAMES + 1];  // global detection index of each frame's first detection
+};
+
+// ---- order-preserving float <-> int (for atomicMin/Max on fp32 values; exact)
+__device__ __forceinline__ int f2ord(float f) {
+  int i = __float_as_int(f);
+  return i ^ ((i >> 31) & 0x7FFFFFFF);
+}
+__device__ __forceinline__ float ord2f(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7FFFFFFF)); }
+__host__ __device__ __forceinline__ int f2ord_host(float f) {
+  int i;
+  memcpy(&i, &f, 4);
+  return i ^ ((i >> 31) & 0x7FFFFFFF);
+}
+
+// (score, lowest id wins) packed for atomicMax
+__device__ __forceinline__ unsigned long long pack_score(float s, uint32_t id) {
+  uint32_t u = (uint32_t)f2ord(s) ^ 0x80000000u;  // order-preserving unsigned
+  return ((unsigned long long)u << 32) | (unsigned long long)(0xFFFFFFFFu - id);
+}
+__device__ __forceinline__ float unpack_score(unsigned long long p) { return ord2f((int)((uint32_t)(p >> 32) ^ 0x80000000u)); }
+__device__ __forceinline__ uint32_t unpack_id(unsigned long long p) { return 0xFFFFFFFFu - (uint32_t)p; }
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
+  x ^= x >> 33;
+  x *= 0xff51afd7ed558ccdull;
+  x ^= x >> 33;
+  x *= 0xc4ceb9fe1a85ec53ull;
+  x ^= x >> 33;
+  return x;
+}
+
+template <typename T>
+__device__ __forceinline__ float to_f32(T v);
+template <>
+__device__ __forceinline__ float to_f32<float>(float v) { return v; }
+template <>
+__device__ __forceinline__ float to_f32<__half>(__half v) { return __half2float(v); }
+template <>
+__device__ __forceinline__ float to_f32<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+template <typename T>
+__device__ __forceinline__ T from_f32(float v);
+template <>
+__device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <>
+__device__ __forceinline__ __half from_f32<__half>(float v) { return __float2half_rn(v); }
+template <>
+__device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+
+// host-side launchers (one per translation unit); each returns the number of kernels it launched
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,
+                             const float *T, int n_det, float *xyz, unsigned long long *keys, cudaStream_t s);
+int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
+int launch_assoc_merge_seq(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
+
+}  // namespace farm

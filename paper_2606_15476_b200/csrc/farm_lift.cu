@@ -1,0 +1,484 @@
+// farm_lift.cu -- steps 1-3 of the hot path in one pass over the images:
+//   back-project masked pixels (R5), quantise to voxel keys (R6), per-detection dedupe (R7),
+//   probe / insert the global voxel->object hash (R11, R12 pass 1) and build the sparse overlap
+//   histogram (R9).  BASELINE.json north_star steps (1)-(3); PAPER.md:65, 347 ("masked depth points").
+//
+// HBM-bound by design: the only mandatory traffic is 6 B/pixel of depth+mask (128-bit loads) plus one
+// 32-byte sector per distinct (detection, voxel) pair that survives the shared-memory tile dedupe.
+#include "farm_internal.cuh"
+
+namespace farm {
+
+namespace {
+
+constexpr int TILE_W = 128;
+constexpr int TILE_H = 8;
+constexpr int LIFT_THREADS = 128;
+constexpr int TILE_PX = TILE_W * TILE_H;
+constexpr int TILE_HASH = 2048;  // smem dedupe set, load <= 0.5
+constexpr int MAX_LABELS = 32;   // per-tile detection accumulators
+constexpr uint32_t NONE32 = 0xFFFFFFFFu;
+
+struct Camera {
+  float inv_fx, inv_fy, cx, cy;
+  float r[9], t[3];
+};
+
+__device__ __forceinline__ Camera load_camera(const float *__restrict__ K, const float *__restrict__ T) {
+  Camera c;
+  c.inv_fx = __fdiv_rn(1.0f, __ldg(K + 0));  // R5: IEEE fp32 reciprocal, once per frame
+  c.inv_fy = __fdiv_rn(1.0f, __ldg(K + 4));
+  c.cx = __ldg(K + 2);
+  c.cy = __ldg(K + 5);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    c.r[3 * i + 0] = __ldg(T + 4 * i + 0);
+    c.r[3 * i + 1] = __ldg(T + 4 * i + 1);
+    c.r[3 * i + 2] = __ldg(T + 4 * i + 2);
+    c.t[i] = __ldg(T + 4 * i + 3);
+  }
+  return c;
+}
+
+// R5: every multiply and add individually rounded (the _rn intrinsics are never contracted into FMA).
+__device__ __forceinline__ void backproject(const Camera &c, int u, int v, float z, float p[3]) {
+  const float xn = __fmul_rn(__fsub_rn((float)u, c.cx), c.inv_fx);
+  const float yn = __fmul_rn(__fsub_rn((float)v, c.cy), c.inv_fy);
+  const float xc = __fmul_rn(xn, z), yc = __fmul_rn(yn, z);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+    p[i] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.r[3 * i], xc), __fmul_rn(c.r[3 * i + 1], yc)),
+                               __fmul_rn(c.r[3 * i + 2], z)),
+                     c.t[i]);
+}
+
+// R6
+__device__ __forceinline__ bool voxel_key(const float p[3], float inv_vs, unsigned long long *key) {
+  const float qx = floorf(__fmul_rn(p[0], inv_vs));
+  const float qy = floorf(__fmul_rn(p[1], inv_vs));
+  const float qz = floorf(__fmul_rn(p[2], inv_vs));
+  const float lo = (float)-KEY_BIAS, hi = (float)KEY_BIAS;
+  if (!(qx >= lo && qx < hi && qy >= lo && qy < hi && qz >= lo && qz < hi)) return false;
+  *key = ((unsigned long long)((int)qx + KEY_BIAS) << 42) | ((unsigned long long)((int)qy + KEY_BIAS) << 21) |
+         (unsigned long long)((int)qz + KEY_BIAS);
+  return true;
+}
+
+__device__ __forceinline__ bool depth_valid(float z, float z_min, float z_max) {
+  return (fabsf(z) <= 3.402823466e+38f) && z > z_min && z <= z_max;  // finite, in (z_min, z_max]  (R4)
+}
+
+// ---------------------------------------------------------------------------------------------------
+// prep: reset per-call state and compute detection row norms (operand A of step 4).  One warp per row.
+template <typename T>
+__global__ void prep_kernel(DevMap m, CallArgs a) {
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    m.counters[0] = 0;
+    m.counters[1] = 0;
+    CallStats z = {};
+    z.n_det = (uint32_t)a.M;
+    *m.stats = z;
+  }
+  if (warp >= a.M) return;
+  const T *row = (const T *)a.desc + (size_t)warp * m.D;
+  float s = 0.f;
+  for (int i = lane; i < m.D; i += 32) {
+    const float x = to_f32<T>(row[i]);
+    s = fmaf(x, x, s);
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+  if (lane == 0) {
+    m.det_inv_norm[warp] = s > 0.f ? 1.0f / sqrtf(s) : 0.f;
+    m.det_nv[warp] = 0;
+    m.det_npx[warp] = 0;
+    m.best_cand[warp] = 0ull;
+    m.best_dense[warp] = 0ull;
+    m.assoc[warp] = -1;
+    m.is_new[warp] = 0;
+    m.best_score[warp] = 0.f;
+  }
+  if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// global structures
+
+// find-or-insert `key` in the voxel table; returns slot index or NONE32 when the table is full.
+__device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsigned long long key) {
+  unsigned long long h = mix64(key) & m.table_mask;
+  for (unsigned long long probe = 0; probe <= m.table_mask; ++probe) {
+    unsigned long long k = __ldcg(&m.table[h].key);
+    if (k == KEY_EMPTY) {
+      k = atomicCAS(&m.table[h].key, KEY_EMPTY, key);
+      if (k == KEY_EMPTY) return (uint32_t)h;  // inserted: owner == OWNER_PENDING, claim == CLAIM_NONE already
+    }
+    if (k == key) return (uint32_t)h;
+    h = (h + 1) & m.table_mask;
+    if (probe > 4096) break;
+  }
+  atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
+  return NONE32;
+}
+
+// epoch-tagged set/map insert: entries whose epoch field differs from `epoch` count as free.
+// returns 1 = newly inserted, 0 = already present, -1 = table full.
+__device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t mask, unsigned long long v,
+                                            uint32_t epoch, uint32_t *slot) {
+  uint32_t h = (uint32_t)mix64(v) & mask;
+  for (uint32_t probe = 0; probe <= mask; ++probe) {
+    unsigned long long cur = __ldcg(&tab[h]);
+    for (;;) {
+      if (cur == v) {
+        *slot = h;
+        return 0;
+      }
+      if ((uint32_t)(cur >> (64 - EPOCH_BITS)) == epoch) break;  // live entry of another pair
+      const unsigned long long old = atomicCAS(&tab[h], cur, v);
+      if (old == cur) {
+        *slot = h;
+        return 1;
+      }
+      cur = old;
+    }
+    h = (h + 1) & mask;
+    if (probe > 8192) break;
+  }
+  return -1;
+}
+
+struct TileSmem {
+  unsigned long long hkey[TILE_HASH];
+  unsigned long long qkey[TILE_PX];
+  uint32_t hlab[TILE_HASH];
+  uint32_t qj[TILE_PX];
+  uint32_t lab_j[MAX_LABELS];
+  uint32_t lab_cnt[MAX_LABELS];
+  int lab_box[MAX_LABELS][6];
+  uint32_t q_count;
+  uint32_t n_valid, n_dropped, n_ignored;
+};
+
+// accumulate one thread's run (j, cnt, box) into the tile's per-detection accumulators
+__device__ __forceinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32_t j, uint32_t cnt, const int mn[3],
+                                               const int mx[3]) {
+  uint32_t h = j % MAX_LABELS;
+  for (int probe = 0; probe < MAX_LABELS; ++probe) {
+    uint32_t l = *(volatile uint32_t *)&s.lab_j[h];
+    if (l == NONE32) {
+      l = atomicCAS(&s.lab_j[h], NONE32, j);
+      if (l == NONE32) l = j;
+    }
+    if (l == j) {
+      atomicAdd(&s.lab_cnt[h], cnt);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        atomicMin(&s.lab_box[h][k], mn[k]);
+        atomicMax(&s.lab_box[h][3 + k], mx[k]);
+      }
+      return;
+    }
+    h = (h + 1) % MAX_LABELS;
+  }
+  // more than MAX_LABELS detections inside one tile: go to global memory directly
+  atomicAdd(&m.det_npx[j], cnt);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    atomicMin(&m.det_box[j * 6 + k], mn[k]);
+    atomicMax(&m.det_box[j * 6 + 3 + k], mx[k]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// The lift kernel.  One 128x8 pixel tile per CTA; each thread owns 8 consecutive pixels of one row
+// (2 x 128-bit depth loads + 1 x 128-bit mask load).
+template <bool VEC>
+__global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+  __shared__ TileSmem s;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int tile = blockIdx.x;
+  const int f = tile / (tiles_x * tiles_y);
+  const int trem = tile - f * tiles_x * tiles_y;
+  const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
+  const int v = ty * TILE_H + (tid >> 4);
+  const int u0 = tx * TILE_W + (tid & 15) * 8;
+
+  // ---- issue the loads first (all independent), then initialise shared memory while they fly
+  float z[8];
+  uint16_t lab[8];
+  const size_t frame_off = (size_t)f * m.H * m.W;
+  const bool row_ok = v < m.H;
+  if (VEC && row_ok && u0 + 7 < m.W) {
+    const size_t off = frame_off + (size_t)v * m.W + u0;
+    const float4 d0 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off));
+    const float4 d1 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off + 4));
+    const uint4 mk = __ldcs(reinterpret_cast<const uint4 *>(a.mask + off));
+    z[0] = d0.x, z[1] = d0.y, z[2] = d0.z, z[3] = d0.w, z[4] = d1.x, z[5] = d1.y, z[6] = d1.z, z[7] = d1.w;
+    lab[0] = mk.x & 0xFFFF, lab[1] = mk.x >> 16, lab[2] = mk.y & 0xFFFF, lab[3] = mk.y >> 16;
+    lab[4] = mk.z & 0xFFFF, lab[5] = mk.z >> 16, lab[6] = mk.w & 0xFFFF, lab[7] = mk.w >> 16;
+  } else {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool ok = row_ok && u0 + i < m.W;
+      const size_t off = frame_off + (size_t)v * m.W + u0 + i;
+      lab[i] = ok ? __ldcs(a.mask + off) : (uint16_t)0;
+      z[i] = ok ? __ldcs(a.depth + off) : 0.f;
+    }
+  }
+  for (int i = tid; i < TILE_HASH; i += LIFT_THREADS) {
+    s.hkey[i] = KEY_EMPTY;
+    s.hlab[i] = NONE32;
+  }
+  if (tid < MAX_LABELS) {
+    s.lab_j[tid] = NONE32;
+    s.lab_cnt[tid] = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      s.lab_box[tid][k] = 0x7FFFFFFF;
+      s.lab_box[tid][3 + k] = (int)0x80000000;
+    }
+  }
+  if (tid == 0) s.q_count = 0, s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
+  const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
+  const int det_base = a.base[f];
+  const int n_det_f = a.base[f + 1] - det_base;
+  __syncthreads();
+
+  // ---- per pixel: validity (R3, R4), back-projection (R5), key (R6), tile-level dedupe
+  uint32_t cur_j = NONE32, cur_cnt = 0;
+  int mn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+  unsigned long long prev_key = KEY_EMPTY;
+  uint32_t prev_j = NONE32;
+  uint32_t n_valid = 0, n_dropped = 0, n_ignored = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    bool fresh = false;
+    unsigned long long key = KEY_EMPTY;
+    uint32_t j = NONE32;
+    const uint32_t l = lab[i];
+    if (l != 0) {
+      if ((int)l > n_det_f) {
+        n_ignored++;
+      } else if (depth_valid(z[i], m.z_min, m.z_max)) {
+        float p[3];
+        backproject(cam, u0 + i, v, z[i], p);
+        if (voxel_key(p, m.inv_vs, &key)) {
+          n_valid++;
+          j = (uint32_t)(det_base + (int)l - 1);
+          if (j != cur_j) {
+            if (cur_j != NONE32) tile_label_add(s, m, cur_j, cur_cnt, mn, mx);
+            cur_j = j, cur_cnt = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) mn[k] = 0x7FFFFFFF, mx[k] = (int)0x80000000;
+          }
+          cur_cnt++;
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            const int o = f2ord(p[k]);
+            mn[k] = min(mn[k], o), mx[k] = max(mx[k], o);
+          }
+          if (!(key == prev_key && j == prev_j)) {  // thread-local dedupe of consecutive pixels
+            prev_key = key, prev_j = j;
+            // shared-memory set keyed (key, j): a filter only, the global pair set is exact
+            uint32_t h = ((uint32_t)(key ^ (key >> 21) ^ (key >> 42)) * 0x9E3779B1u + j * 0x85EBCA6Bu) >> 21;
+            fresh = true;
+            for (int probe = 0; probe < 32; ++probe) {
+              unsigned long long k2 = *(volatile unsigned long long *)&s.hkey[h];
+              if (k2 == KEY_EMPTY) {
+                k2 = atomicCAS(&s.hkey[h], KEY_EMPTY, key);
+                if (k2 == KEY_EMPTY) {
+                  *(volatile uint32_t *)&s.hlab[h] = j;
+                  break;
+                }
+              }
+              if (k2 == key && *(volatile uint32_t *)&s.hlab[h] == j) {
+                fresh = false;
+                break;
+              }
+              h = (h + 1) & (TILE_HASH - 1);
+            }
+          }
+        } else {
+          n_dropped++;
+        }
+      }
+    }
+    // warp-ballot compaction of the surviving (detection, key) pairs into the tile queue
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, fresh);
+    if (b) {
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (fresh) {
+        const uint32_t pos = base + __popc(b & ((1u << lane) - 1));
+        s.qkey[pos] = key;
+        s.qj[pos] = j;
+      }
+    }
+  }
+  // per-detection pixel count and point AABB (R7): warp-uniform fast path through REDUX, else per thread
+  {
+    const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_j != NONE32);
+    if (has) {
+      const uint32_t lead_j = __shfl_sync(0xFFFFFFFFu, cur_j, __ffs(has) - 1);
+      const bool uniform = __all_sync(0xFFFFFFFFu, cur_j == NONE32 || cur_j == lead_j);
+      if (uniform) {
+        const uint32_t cnt = __reduce_add_sync(0xFFFFFFFFu, cur_cnt);
+        int rmn[3], rmx[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          rmn[k] = __reduce_min_sync(0xFFFFFFFFu, mn[k]);
+          rmx[k] = __reduce_max_sync(0xFFFFFFFFu, mx[k]);
+        }
+        if (lane == 0) tile_label_add(s, m, lead_j, cnt, rmn, rmx);
+      } else if (cur_j != NONE32) {
+        tile_label_add(s, m, cur_j, cur_cnt, mn, mx);
+      }
+    }
+    n_valid = __reduce_add_sync(0xFFFFFFFFu, n_valid);
+    n_dropped = __reduce_add_sync(0xFFFFFFFFu, n_dropped);
+    n_ignored = __reduce_add_sync(0xFFFFFFFFu, n_ignored);
+    if (lane == 0) {
+      if (n_valid) atomicAdd(&s.n_valid, n_valid);
+      if (n_dropped) atomicAdd(&s.n_dropped, n_dropped);
+      if (n_ignored) atomicAdd(&s.n_ignored, n_ignored);
+    }
+  }
+  __syncthreads();
+
+  // ---- survivors: global voxel table (find or insert), exact per-call pair set, |V_d|, overlap histogram
+  const uint32_t nq = s.q_count;
+  for (uint32_t i0 = (tid & ~31u); i0 < nq; i0 += LIFT_THREADS) {
+    const uint32_t i = i0 + lane;
+    bool is_new = false, owned = false;
+    uint32_t j = 0, slot = NONE32, owner = OWNER_PENDING;
+    if (i < nq) {
+      const unsigned long long key = s.qkey[i];
+      j = s.qj[i];
+      slot = voxel_find_or_insert(m, key);
+      if (slot != NONE32) {
+        const unsigned long long pv =
+            ((unsigned long long)a.epoch << (64 - EPOCH_BITS)) | ((unsigned long long)j << 32) | slot;
+        uint32_t ps;
+        const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
+        if (r < 0) atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+        is_new = r == 1;
+        if (is_new) {
+          owner = __ldcg(&m.table[slot].owner);
+          owned = owner != OWNER_PENDING;  // owned at entry (R9); pending = inserted by this call (R12)
+        }
+      }
+    }
+    const unsigned act = __ballot_sync(0xFFFFFFFFu, is_new);
+    if (act) {
+      // append to the pair list (one atomic per warp)
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(&m.counters[0], (uint32_t)__popc(act));
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (is_new) {
+        const uint32_t pos = base + __popc(act & ((1u << lane) - 1));
+        if (pos < m.pair_cap)
+          m.pair_list[pos] = ((unsigned long long)(owned ? 0 : 1) << 63) | ((unsigned long long)j << 32) | slot;
+        else
+          atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+        // |V_d| += 1, aggregated over the lanes of the same detection
+        const unsigned same = __match_any_sync(act, j);
+        if (lane == __ffs(same) - 1) atomicAdd(&m.det_nv[j], (uint32_t)__popc(same));
+        if (!owned) atomicMin(&m.table[slot].claim, j);  // R12: lowest detection index wins
+      }
+      // overlap histogram c[j][owner] += 1, aggregated over lanes with the same (j, owner)
+      const unsigned oact = __ballot_sync(act, owned);
+      if (owned) {
+        const unsigned long long jo = ((unsigned long long)j << 32) | owner;
+        const unsigned same = __match_any_sync(oact, jo);
+        if (lane == __ffs(same) - 1) {
+          const unsigned long long ov = ((unsigned long long)a.epoch << (64 - EPOCH_BITS)) | jo;
+          uint32_t os;
+          const int r = epoch_insert(m.ov_keys, m.ov_mask, ov, a.epoch, &os);
+          if (r < 0) {
+            atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+          } else {
+            if (r == 1) {
+              const uint32_t c = atomicAdd(&m.counters[1], 1u);
+              if (c < m.cand_cap)
+                m.cand_slot[c] = os;
+              else
+                atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+            }
+            atomicAdd(&m.ov_cnt[os], (uint32_t)__popc(same));
+          }
+        }
+      }
+    }
+  }
+
+  // ---- flush the tile's per-detection accumulators and counters
+  if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
+    const uint32_t j = s.lab_j[tid];
+    atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
+      atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
+    }
+  }
+  if (tid == 0) {
+    if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
+    if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
+    if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
+  }
+}
+
+__global__ void debug_backproject_kernel(DevMap m, const float *__restrict__ depth, const uint16_t *__restrict__ mask,
+                                         const float *__restrict__ K, const float *__restrict__ T, int n_det,
+                                         float *__restrict__ xyz, unsigned long long *__restrict__ keys) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m.H * m.W) return;
+  const Camera cam = load_camera(K, T);
+  const int v = i / m.W, u = i - v * m.W;
+  float p[3] = {__int_as_float(0x7FC00000), __int_as_float(0x7FC00000), __int_as_float(0x7FC00000)};
+  unsigned long long key = KEY_EMPTY;
+  const uint32_t l = mask[i];
+  const float z = depth[i];
+  if (l != 0 && (int)l <= n_det && depth_valid(z, m.z_min, m.z_max)) {
+    backproject(cam, u, v, z, p);
+    if (!voxel_key(p, m.inv_vs, &key)) key = KEY_EMPTY;
+  }
+  xyz[3 * (size_t)i] = p[0], xyz[3 * (size_t)i + 1] = p[1], xyz[3 * (size_t)i + 2] = p[2];
+  keys[i] = key;
+}
+
+}  // namespace
+
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  const int blocks = a.M > 0 ? (a.M + 3) / 4 : 1;
+  if (m.dtype == FARM_DTYPE_F32)
+    prep_kernel<float><<<blocks, 128, 0, s>>>(m, a);
+  else if (m.dtype == FARM_DTYPE_F16)
+    prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a);
+  else
+    prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a);
+  return 1;
+}
+
+int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
+  const int grid = tiles_x * tiles_y * a.F;
+  const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
+  if (vec)
+    lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  else
+    lift_voxelise_kernel<false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  return 1;
+}
+
+int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K, const float *T,
+                             int n_det, float *xyz, unsigned long long *keys, cudaStream_t s) {
+  const int n = m.H * m.W;
+  debug_backproject_kernel<<<(n + 255) / 256, 256, 0, s>>>(m, depth, mask, K, T, n_det, xyz, keys);
+  return 1;
+}
+
+}  // namespace farm

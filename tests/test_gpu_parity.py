@@ -1,0 +1,202 @@
+"""`-m gpu`: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs."""
+import numpy as np
+import pytest
+import torch
+
+from helpers import (KEY_EMPTY, hand_frame, integrate_frames, margin_filter, pack_key, pow2_K, unit_rows)
+from paper_2606_15476_b200 import FarmMap, scenes as S
+from parity import TOL, compare_call, compare_maps, gpu_integrate, make_pair, upload
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_sequence(oracle, cfg, frames_per_call, n_calls, start=0, filter_margins=True, **kw):
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg, **kw)
+    k = start
+    for _ in range(n_calls):
+        frames = [sc.frame(k + i) for i in range(frames_per_call)]
+        k += frames_per_call
+        if filter_margins:
+            frames = margin_filter(o.clone, frames, cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+    compare_maps(g, o)
+    return o, g
+
+
+def test_debug_backproject_bit_exact(oracle):
+    """R5/R6: per-pixel world points and keys; fp32 op order identical, no FMA contraction."""
+    cfg = S.get_config(1)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    for k in (30, 200):
+        fr = sc.frame(k)
+        d = upload([fr], cfg.dtype)
+        xyz = torch.empty((cfg.H, cfg.W, 3), dtype=torch.float32, device="cuda")
+        keys = torch.empty((cfg.H, cfg.W), dtype=torch.int64, device="cuda")
+        g.debug_backproject(d["depth"], d["mask"], d["K"], d["T"], fr.n_det, xyz, keys)
+        torch.cuda.synchronize()
+        xo, ko = o.backproject(fr.depth, fr.mask, fr.K, fr.T, fr.n_det)
+        xg = xyz.cpu().numpy()
+        kg = keys.cpu().numpy().view(np.uint64)
+        assert np.array_equal(kg, ko)
+        assert np.array_equal(np.isnan(xg), np.isnan(xo))
+        assert np.array_equal(xg[~np.isnan(xg)], xo[~np.isnan(xo)])       # bit-exact, stronger than 1e-4
+        assert (ko != KEY_EMPTY).sum() > 10000
+
+
+def test_config0_full_sequence(oracle):
+    """BASELINE.json configs[0]: all 20 frames, every intermediate and the final map."""
+    cfg = S.get_config(0)
+    o, g = _run_sequence(oracle, cfg, 1, cfg.n_frames)
+    objs, _, _, _ = g.read()
+    assert 5 <= len(objs) <= 40
+
+
+def test_config1_prefix_f16(oracle):
+    """configs[1] (room, D=512 fp16, misses and false positives): a prefix spanning many tiles."""
+    cfg = S.get_config(1)
+    _run_sequence(oracle, cfg, 1, 10, start=25)
+
+
+def test_config2_prefix_bf16(oracle):
+    """configs[2] (house, D=1024 bf16, 0.9-cosine distractor clusters)."""
+    cfg = S.get_config(2)
+    _run_sequence(oracle, cfg, 1, 6, start=0)
+
+
+def test_batched_frames_one_snapshot(oracle):
+    """F > 1: frames of one call share the entry snapshot (R2); ragged F."""
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    k = 0
+    for F in (3, 1, 5, 4):
+        frames = margin_filter(o.clone, [sc.frame(k + i) for i in range(F)], cfg.tau)
+        k += F
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+    compare_maps(g, o)
+
+
+def test_hand_cases(oracle):
+    """The oracle's hand pins run through the CUDA path: strict threshold, R12 lowest index, R8, R3, R23."""
+    H, W = 96, 128
+    I4 = np.eye(4, dtype=np.float32)
+    e = np.eye(4, dtype=np.float32)
+
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.25, 4, 0.5, 0.5, 0.5, 0
+
+    def frame(px, desc, T=I4):
+        depth, mask = hand_frame(H, W, px)
+        return S.Frame(depth, mask, pow2_K(), T, np.ascontiguousarray(desc, np.float32), len(desc), np.zeros(len(desc), np.int64))
+
+    o, g = make_pair(oracle, Cfg, H=H, W=W)
+    seq = [
+        frame([(64, 40, 2.0, 2), (66, 41, 2.0, 1), (96, 48, 2.0, 1)], e[:2]),           # R2/R12/R13/R20
+        frame([(64, 40, 2.0, 2), (66, 41, 2.0, 1), (96, 48, 2.0, 1)], e[:2]),
+        frame([(64, 48, 2.0, 1), (70, 48, 2.0, 3)], e[:3]),                              # R8: label 2 empty
+        frame([(10, 10, 0.0, 1), (12, 10, np.nan, 1), (13, 10, np.inf, 1), (17, 10, 1.0, 3), (18, 10, 1.0, 2)], e[:2]),
+        frame([], e[:0]),                                                                # no detections at all
+        frame([(64, 48, 2.0, 1), (80, 48, 2.0, 1), (96, 48, 2.0, 1), (112, 48, 2.0, 1)], e[:1]),
+    ]
+    for fr in seq:
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+    compare_maps(g, o)
+
+
+def test_score_hand_case_via_import(oracle):
+    """P6 through import + integrate: 0.875 match, and 0.5 is NOT > 0.5."""
+    H, W = 96, 128
+    I4 = np.eye(4, dtype=np.float32)
+    e1 = np.array([[1, 0, 0, 0]], np.float32)
+    depth, mask = hand_frame(H, W, [(64, 48, 2.0, 1), (80, 48, 2.0, 1), (96, 48, 2.0, 1), (112, 48, 2.0, 1)])
+    fr = S.Frame(depth, mask, pow2_K(), I4, e1, 1, np.zeros(1, np.int64))
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    for own, expect, new in (([(0, 0, 8), (1, 0, 8), (2, 0, 8)] + [(50 + i, 0, 0) for i in range(5)], 0.875, 0),
+                             ([(50 + i, 0, 0) for i in range(8)], 0.5, 1)):
+        keys = np.array([pack_key(*k) for k in own], np.uint64)
+        obj = np.zeros(1, OBJECT_DTYPE)
+        obj["n_voxels"], obj["n_obs"], obj["best_frame"], obj["best_det"] = 8, 1, -1, -1
+        g = FarmMap(0.25, 4, 0.5, 0.5, 0.5, H=H, W=W)
+        g.import_(obj, e1, keys, np.zeros(8, np.uint32))
+        gpu_integrate(g, [fr], 0)
+        a, n, b, st = g.last_assoc()
+        assert b[0] == np.float32(expect) and n[0] == new and a[0] == (1 if new else 0)
+
+
+def test_import_round_trip_and_continue(oracle):
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    for k in range(6):
+        fr = sc.frame(k)
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], cfg.dtype)
+    objs, desc, keys, owners = g.read()
+    g2 = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype)
+    g2.import_(objs, desc, keys, owners)
+    compare_maps(g2, o)
+    frames = margin_filter(o.clone, [sc.frame(6)], cfg.tau)
+    integrate_frames(o, frames)
+    gpu_integrate(g2, frames, cfg.dtype)
+    compare_call(g2, o, check_sets=True)
+    compare_maps(g2, o)
+    # duplicate key is rejected
+    g3 = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype)
+    from paper_2606_15476_b200 import FarmError
+    with pytest.raises(FarmError):
+        g3.import_(objs, desc, np.concatenate([keys, keys[:1]]), np.concatenate([owners, owners[:1]]))
+
+
+def test_determinism_two_runs_byte_equal(oracle):
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    outs = []
+    for _ in range(2):
+        g = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype)
+        for k in range(10):
+            gpu_integrate(g, [sc.frame(k)], cfg.dtype)
+        objs, desc, keys, owners = g.read()
+        order = np.argsort(keys)
+        outs.append((objs.tobytes(), desc.tobytes(), keys[order].tobytes(), owners[order].tobytes()))
+    assert outs[0] == outs[1]
+
+
+def test_odd_width_scalar_path(oracle):
+    """W not a multiple of 8 takes the scalar-load variant of the lift kernel; ragged tiles on both axes."""
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.05, 8, 0.5, 0.5, 0.5, 0
+    H, W = 37, 203
+    g0 = np.random.default_rng(3)
+    o, g = make_pair(oracle, Cfg, H=H, W=W)
+    K = np.array([[150, 0, 100], [0, 150, 18], [0, 0, 1]], np.float32)
+    for it in range(3):
+        depth = (1.5 + 0.5 * g0.random((H, W))).astype(np.float32)
+        mask = np.zeros((H, W), np.uint16)
+        mask[5:30, 10:90] = 1
+        mask[8:36, 100:203] = 2
+        mask[0:4, :] = 3
+        T = S.pose_from_yaw(np.array([0.1 * it, 0.0, 1.0]), 0.3)
+        fr = S.Frame(depth, mask, K, T, unit_rows(3, 8, 5), 3, np.zeros(3, np.int64))
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+    compare_maps(g, o)
+
+
+def test_capacity_error_is_sticky(oracle):
+    from paper_2606_15476_b200 import FarmError
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    g = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype, max_objects=2)
+    gpu_integrate(g, [sc.frame(0)], cfg.dtype)
+    with pytest.raises(FarmError) as ei:
+        g.last_assoc()
+    assert ei.value.code == -3
