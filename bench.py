@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- mapping throughput of the FARM hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+Workload (N=1 and every rank of N>1): BASELINE.json configs[4], the batched throughput stress -- a map
+pre-populated with 50,000 objects (random connected voxel blobs, mean ~2,000 voxels at 2.5 cm, D=1024 bf16
+descriptors), then batches of 16 frames at 640x480 with 100 detections each, half of which overlap existing
+objects.  One "step" = one farm_map_integrate_batch call = one pass of the whole hot path (all of steps
+1-5) over one 16-frame batch.  configs[4] is the largest single-GPU configuration and the one the
+north-star target is stated on; the other configs are parity-test cases (--config 0..3 times them too).
+
+Multi-GPU: replicas only.  Under torchrun every rank owns an independent map and
+stream of batches; there is no data-path collective; `value` is total frames over max-over-ranks time.
+
+Prints ONE JSON line (rank 0).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FRAMES_PER_BATCH = 16
+DET_PER_FRAME = 100
+
+
+def parse():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=32)
+    p.add_argument("--warmup", type=int, default=4)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--config", type=int, default=4)
+    p.add_argument("--n-objects", type=int, default=50000, help="pre-populated objects (config 4); the benchmark value is only valid at 50000")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--breakdown", action="store_true", help="bracket every kernel with CUDA events (perturbs `value`)")
+    return p.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return {"hbm_gbs": d["hbm_gbs"], "tf_burst": d["bf16_tflops"], "tf_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "tf_burst": 1590.0, "tf_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.stop_flag, self.max_mhz = [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def sample(self):
+        if not self.nv:
+            return
+        nv = self.nv
+        try:
+            self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                     0x80: "hw_power_brake_slowdown"}
+            for bit, name in names.items():
+                if r & bit:
+                    self.reasons.add(name)
+        except Exception:
+            pass
+
+    def run(self):
+        while not self.stop_flag:
+            self.sample()
+            time.sleep(0.002)
+
+    def result(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def pack_key(ijk):
+    """voxel key layout of include/farm.h (interface format, used to hand the generated map to farm_map_import)"""
+    b = 1 << 20
+    q = ijk.astype(np.int64) + b
+    return ((q[:, 0] << 42) | (q[:, 1] << 21) | q[:, 2]).astype(np.uint64)
+
+
+def build_stress(args, seed_offset=0):
+    from paper_2606_15476_b200 import scenes as S
+    n_batches = args.steps + args.warmup
+    sc = S.StressScene(n_batches=n_batches, frames_per_batch=FRAMES_PER_BATCH, n_objects=args.n_objects,
+                       seed=S.get_config(4).seed + seed_offset)
+    ijk, owner, n_vox, desc = sc.build_map()
+    return sc, pack_key(ijk), owner, n_vox, desc
+
+
+def object_records(dtype, n_vox):
+    objs = np.zeros(len(n_vox), dtype)
+    objs["id"] = np.arange(len(n_vox))
+    objs["n_voxels"] = n_vox
+    objs["n_obs"] = 1
+    objs["best_frame"] = -1
+    objs["best_det"] = -1
+    return objs
+
+
+def batch_host_arrays(frames):
+    depth = np.stack([f.depth for f in frames])
+    mask = np.stack([f.mask for f in frames])
+    K = np.stack([f.K for f in frames]).astype(np.float32)
+    T = np.stack([f.T for f in frames]).astype(np.float32)
+    desc = np.concatenate([f.desc for f in frames], axis=0)
+    n_det = np.array([f.n_det for f in frames], np.int32)
+    return depth, mask, K, T, desc, n_det
+
+
+# ------------------------------------------------------------------------------------------------ ours
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_15476_b200 import FarmMap, binding, build as farm_build, scenes as S
+
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if not os.path.exists(binding.LIB_PATH):
+        farm_build.build()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product has no CPU fallback"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = S.get_config(4)
+    K_steps, W_steps = args.steps, args.warmup
+    sc, keys, owner, n_vox, desc = build_stress(args, seed_offset=rank)
+    objs = object_records(binding.OBJECT_DTYPE, n_vox)
+    N0 = len(objs)
+    max_objects = N0 + (K_steps + W_steps + 1) * FRAMES_PER_BATCH * DET_PER_FRAME
+    max_voxels = int(len(keys) * 1.05) + (K_steps + W_steps + 1) * 600000
+
+    stream = torch.cuda.Stream(device=dev)
+
+    def new_map(timing):
+        m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
+                    max_objects=max_objects, max_voxels=max_voxels, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
+                    max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
+                    timing=timing)
+        m.import_(objs, desc, keys, owner)
+        return m
+
+    host_batches = [batch_host_arrays(sc.batch(b)) for b in range(K_steps + W_steps)]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    # ---------------- device-resident run (value)
+    m = new_map(2 if args.breakdown else 1)
+    dev_batches = []
+    with torch.cuda.stream(stream):
+        for (depth, mask, Kc, T, dsc, n_det) in host_batches:
+            dev_batches.append((torch.from_numpy(depth).to(dev), torch.from_numpy(mask.view(np.int16)).to(dev),
+                                torch.from_numpy(Kc).to(dev), torch.from_numpy(T).to(dev),
+                                torch.from_numpy(dsc.view(np.int16)).to(dev), n_det))
+    stream.synchronize()
+    for b in range(W_steps):
+        d = dev_batches[b]
+        m.integrate_batch(FRAMES_PER_BATCH, d[0], d[1], d[2], d[3], d[4], d[5])
+    tot0 = m.sync()
+    n_before = len(m.read(voxels=False, descriptors=False)[0])
+    m.stage_times(reset=True)
+    launches0 = m.kernel_launches()
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    e0.record(stream)
+    for b in range(W_steps, W_steps + K_steps):
+        d = dev_batches[b]
+        m.integrate_batch(FRAMES_PER_BATCH, d[0], d[1], d[2], d[3], d[4], d[5])
+    e1.record(stream)
+    sampler.sample()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    launches = m.kernel_launches() - launches0
+    tot1 = m.sync()
+    stage_ms, stage_launches = m.stage_times(reset=True)
+    n_after = len(m.read(voxels=False, descriptors=False)[0])
+    frames = int(tot1["frames"] - tot0["frames"])
+    points = int(tot1["valid_points"] - tot0["valid_points"])
+    uniq = int(tot1["unique_voxels"] - tot0["unique_voxels"])
+    total_frames = sum_over_ranks(frames)
+    total_points = sum_over_ranks(points)
+    value = total_frames / (ms * 1e-3)
+    del m, dev_batches
+    torch.cuda.empty_cache()
+
+    # ---------------- end-to-end run through the host-buffer entry point (e2e)
+    e2e = None
+    if not args.no_e2e:
+        m2 = new_map(0)
+        pinned = []
+        for (depth, mask, Kc, T, dsc, n_det) in host_batches:
+            pinned.append((torch.from_numpy(depth).pin_memory(), torch.from_numpy(mask.view(np.int16)).pin_memory(),
+                           torch.from_numpy(Kc).pin_memory(), torch.from_numpy(T).pin_memory(),
+                           torch.from_numpy(dsc.view(np.int16)).pin_memory(), n_det))
+        for b in range(W_steps):
+            d = pinned[b]
+            m2.integrate_batch_host(FRAMES_PER_BATCH, d[0], d[1], d[2], d[3], d[4], d[5])
+            m2.last_assoc()
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for b in range(W_steps, W_steps + K_steps):
+            d = pinned[b]
+            m2.integrate_batch_host(FRAMES_PER_BATCH, d[0], d[1], d[2], d[3], d[4], d[5])
+            m2.last_assoc()                                   # D2H of the step's result (assoc, is_new, score, stats)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        barrier()
+        ms2 = max_over_ranks(max(e0.elapsed_time(e1), wall_ms))
+        d = pinned[0]
+        h2d = sum(int(x.numel() * x.element_size()) for x in d[:5])
+        d2h = FRAMES_PER_BATCH * DET_PER_FRAME * (4 + 1 + 4) + 48 + 4
+        e2e = {"value": world * K_steps * FRAMES_PER_BATCH / (ms2 * 1e-3), "unit": "frames/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": ms2 / K_steps}
+        del m2, pinned
+        torch.cuda.empty_cache()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---------------- roofline of the dominant kernel (similarity: dense contraction -> tensor bound)
+    pk = peaks()
+    M = FRAMES_PER_BATCH * DET_PER_FRAME
+    n_mean = n_before + (K_steps - 1) / (2.0 * K_steps) * (n_after - n_before)
+    sim_flops = 2.0 * M * n_mean * cfg.D
+    sim_ms = float(stage_ms[binding.STAGE_NAMES.index("similarity")]) / max(K_steps, 1)
+    lift_ms = float(stage_ms[binding.STAGE_NAMES.index("lift")]) / max(K_steps, 1)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tinfo = json.load(open(tpath)) if os.path.exists(tpath) else {}
+    sim_tf = sim_flops / (sim_ms * 1e-3) / 1e12 if sim_ms > 0 else None
+    roofline = {"kernel": "similarity (step 4)", "bound": "tensor", "achieved": sim_tf, "peak": pk["tf_sustained"],
+                "unit": "TFLOP/s", "frac": (sim_tf / pk["tf_sustained"]) if sim_tf else None,
+                "traffic": tinfo.get("similarity_dram_bytes_per_launch", traffic), "peak_source": pk["source"] + ", sustained bf16",
+                "ms_per_launch": sim_ms, "flops_per_launch": sim_flops}
+    # memory-bound group: the lift kernel (steps 1-3).  Algorithmic bytes: 6 B/pixel images + 8 B pair list write
+    # + 16 B probe per distinct (detection, voxel) pair + 16 B insert per new voxel
+    px_bytes = FRAMES_PER_BATCH * cfg.H * cfg.W * 6
+    pairs = uniq / max(K_steps, 1)
+    lift_bytes = px_bytes + pairs * (8 + 16)
+    lift_gbs = lift_bytes / (lift_ms * 1e-3) / 1e9 if lift_ms > 0 else None
+    roofline_hbm = {"kernel": "lift_voxelise (steps 1-3)", "bound": "hbm", "achieved": lift_gbs, "peak": pk["hbm_gbs"],
+                    "unit": "GB/s", "frac": (lift_gbs / pk["hbm_gbs"]) if lift_gbs else None,
+                    "traffic": tinfo.get("lift_dram_bytes_per_launch"), "ms_per_launch": lift_ms, "bytes_per_launch": lift_bytes}
+    step_bytes = px_bytes + M * cfg.D * 2 + n_mean * cfg.D * 2 + pairs * (8 + 16 + 16) + M * cfg.D * (4 + 4 + 2)
+    out = {
+        "metric": "mapping_frames_per_sec", "value": value, "unit": "frames/s", "n_gpus": world, "steps": K_steps,
+        "warmup": W_steps, "ms_per_step": ms / K_steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "configs[4] batched throughput stress", "frames_per_step": FRAMES_PER_BATCH,
+                   "image": f"{cfg.W}x{cfg.H}", "detections_per_frame": DET_PER_FRAME, "D": cfg.D, "voxel_m": cfg.voxel,
+                   "map_objects_at_start": n_before, "map_objects_at_end": n_after, "map_voxels_at_import": int(len(keys)),
+                   "parallelism": "replicas" if world > 1 else "single",
+                   "l2": "inputs larger than L2: every step reads a fresh 29.5 MB batch (all batches staged, >1 GB) and probes a multi-GB voxel table"},
+        "masked_points_per_sec": total_points / (ms * 1e-3),
+        "masked_points_per_step": points / max(K_steps, 1),
+        "unique_voxels_per_step": pairs,
+        "gpu_launches": int(launches),
+        "clocks": sampler.result(),
+        "e2e": e2e,
+        "roofline": roofline,
+        "roofline_hbm": roofline_hbm,
+        "step_algorithmic_bytes": step_bytes,
+        "step_hbm_frac_literal": step_bytes / (ms / K_steps * 1e-3) / 1e9 / pk["hbm_gbs"],
+        "stage_ms_per_step": {n: float(stage_ms[i]) / max(K_steps, 1) for i, n in enumerate(binding.STAGE_NAMES)},
+        "stage_launches": {n: int(stage_launches[i]) for i, n in enumerate(binding.STAGE_NAMES)},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(sc, keys, owner, n_vox, desc, n_steps=1)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------- oracle (reference arm)
+SAMPLE_DET = 25          # detections of one frame per reference step
+SAMPLE_OBJECTS_WITH_VOXELS = 2000
+
+
+def _oracle_sample_map(sc, keys, owner, n_vox, desc):
+    """The oracle as it stands, fed a bounded sample of the workload: ALL object descriptors (the dense
+    similarity cost per frame is the real one) but voxels only for the first SAMPLE_OBJECTS_WITH_VOXELS objects
+    (building a std::map of 1e8 keys takes minutes and is not what is being timed)."""
+    from oracle import farm_oracle as O
+    cfg = sc.cfg
+    m = O.OracleMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, cfg.dtype, cfg.H, cfg.W)
+    sel = owner < SAMPLE_OBJECTS_WITH_VOXELS
+    objs = object_records(O.OBJECT_DTYPE, np.where(np.arange(len(n_vox)) < SAMPLE_OBJECTS_WITH_VOXELS, n_vox, 0))
+    rc = m.import_(objs, desc, keys[sel], owner[sel])
+    assert rc == 0
+    return m
+
+
+def _sample_frame(fr, n_keep):
+    from paper_2606_15476_b200 import scenes as S
+    return S.drop_detections(fr, list(range(n_keep, fr.n_det)))
+
+
+def cpu_baseline(sc, keys, owner, n_vox, desc, n_steps):
+    m = _oracle_sample_map(sc, keys, owner, n_vox, desc)
+    frames = [_sample_frame(sc.batch(0)[i], SAMPLE_DET) for i in range(n_steps * 4)]
+    t0 = time.perf_counter()
+    for fr in frames:
+        m.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
+    dt = time.perf_counter() - t0
+    frame_equiv = len(frames) * SAMPLE_DET / DET_PER_FRAME
+    return {"value": frame_equiv / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
+            "sample": f"{len(frames)} frames of batch 0 cut to their first {SAMPLE_DET} of {DET_PER_FRAME} detections "
+                      f"({frame_equiv:g} frame-equivalents), against all {len(n_vox)} object descriptors and the voxels of the "
+                      f"first {SAMPLE_OBJECTS_WITH_VOXELS} objects; {dt:.1f} s on 1 of {os.cpu_count()} host cores"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    from oracle import build as oracle_build
+    oracle_build.build()
+    small = argparse.Namespace(**vars(args))
+    small.steps, small.warmup = 1, 0          # one batch of frames is enough to draw the samples from
+    sc, keys, owner, n_vox, desc = build_stress(small)
+    m = _oracle_sample_map(sc, keys, owner, n_vox, desc)
+    frames = sc.batch(0)
+    K_steps, W_steps = args.steps, args.warmup
+    seq = [_sample_frame(frames[i % len(frames)], SAMPLE_DET) for i in range(K_steps + W_steps)]
+    for fr in seq[:W_steps]:
+        m.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
+    t0 = time.perf_counter()
+    for fr in seq[W_steps:]:
+        m.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
+    dt = time.perf_counter() - t0
+    frame_equiv = K_steps * SAMPLE_DET / DET_PER_FRAME
+    value = frame_equiv / dt
+    cfg = sc.cfg
+    sample = (f"each step = one frame cut to its first {SAMPLE_DET} of {DET_PER_FRAME} detections ({SAMPLE_DET / DET_PER_FRAME:g} "
+              f"frame-equivalents) against all {len(n_vox)} object descriptors and the voxels of the first "
+              f"{SAMPLE_OBJECTS_WITH_VOXELS} objects")
+    print(json.dumps({
+        "impl": "reference", "metric": "mapping_frames_per_sec", "value": value, "unit": "frames/s", "n_gpus": args.gpus,
+        "steps": K_steps, "warmup": W_steps, "ms_per_step": dt * 1e3 / K_steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[4] batched throughput stress", "frames_per_step": FRAMES_PER_BATCH,
+                   "image": f"{cfg.W}x{cfg.H}", "detections_per_frame": DET_PER_FRAME, "D": cfg.D, "voxel_m": cfg.voxel},
+        "cpu_baseline": {"value": value, "unit": "frames/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

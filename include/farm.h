@@ -65,6 +65,7 @@ extern "C" {
 #define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
 #define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
 #define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
+#define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the lift and similarity kernels; 2 every kernel */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -120,6 +121,13 @@ int farm_map_integrate_batch(farm_map *m, int n_frames, const float *depth, cons
                              const float *K, const float *T_world_cam, const void *det_descriptors,
                              const int *n_det);
 
+/* Same call with HOST buffers (pinned memory recommended): the library copies the batch into its own
+ * device staging buffers with cudaMemcpyAsync on the map's stream, then runs the identical kernels.
+ * The host buffers may be reused once the stream has passed the copies (farm_map_sync / last_assoc). */
+int farm_map_integrate_batch_host(farm_map *m, int n_frames, const float *depth, const uint16_t *instance_mask,
+                                  const float *K, const float *T_world_cam, const void *det_descriptors,
+                                  const int *n_det);
+
 /* Results of the LAST integrate call, HOST buffers of M = sum n_det entries (any may be NULL).
  * obj_id: object the detection was merged into (-1 = skipped, R8); is_new: 1 if that object was spawned by it;
  * best_score: R18.  Synchronises the stream; returns the sticky device error if set. */
@@ -139,6 +147,19 @@ int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, cons
 
 /* Stream sync + sticky device error.  totals may be NULL. */
 int farm_map_sync(farm_map *m, farm_totals *totals);
+
+/* Per-stage device time accumulated since the last reset (needs FARM_OPT_TIMING >= 1; stages that are not
+ * bracketed report 0) and kernel launches per stage.  ms / launches: HOST arrays [FARM_N_STAGES], may be
+ * NULL.  Synchronises the stream. */
+#define FARM_N_STAGES 7
+#define FARM_STAGE_PREP 0        /* reset of per-call state + detection row norms            */
+#define FARM_STAGE_LIFT 1        /* steps 1-3: back-project, voxelise, dedupe, probe, overlap */
+#define FARM_STAGE_SIMILARITY 2  /* step 4: dense cosine with fused row max / argmax          */
+#define FARM_STAGE_CAND_SCORE 3  /* step 5a: scores of the sparse overlap candidates          */
+#define FARM_STAGE_ASSOCIATE 4   /* step 5a: argmax, threshold, new ids                       */
+#define FARM_STAGE_COMMIT 5      /* step 5b: voxel ownership commit                           */
+#define FARM_STAGE_MERGE 6       /* step 5b: descriptors, AABB, view evidence                 */
+int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset);
 
 /* Number of kernels this library has launched for the map so far (host counter). */
 long long farm_map_kernel_launches(const farm_map *m);

@@ -18,6 +18,9 @@ FARM_OK, ERR_INVALID_ARG, ERR_CUDA, ERR_CAPACITY, ERR_STATE, ERR_RANGE = 0, -1, 
 DTYPE_F32, DTYPE_F16, DTYPE_BF16 = 0, 1, 2
 OPT_DESC_DTYPE, OPT_MAX_OBJECTS, OPT_MAX_VOXELS, OPT_IMG_W, OPT_IMG_H = 1, 2, 3, 4, 5
 OPT_MAX_DET_PER_CALL, OPT_STREAM, OPT_MAX_PAIRS_PER_CALL, OPT_MAX_FRAMES_PER_CALL, OPT_SIM_PATH = 6, 7, 8, 9, 10
+OPT_TIMING = 11
+N_STAGES = 7
+STAGE_NAMES = ["prep", "lift", "similarity", "cand_score", "associate", "commit", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
 KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
 
@@ -32,7 +35,7 @@ TOTALS_DTYPE = np.dtype([("frames", "<u8"), ("calls", "<u8"), ("valid_points", "
                          ("matches", "<u8"), ("spawns", "<u8")])
 
 EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm_map_set_option_f",
-           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_last_assoc", "farm_map_read",
+           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
@@ -61,6 +64,8 @@ def load_library():
         lib.farm_map_set_option_f.argtypes = [vp, ci, cf]
         lib.farm_map_integrate.argtypes = [vp, vp, vp, vp, vp, vp, ci]
         lib.farm_map_integrate_batch.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp]
+        lib.farm_map_integrate_batch_host.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp]
+        lib.farm_map_stage_times.argtypes = [vp, vp, vp, ci]
         lib.farm_map_last_assoc.argtypes = [vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
@@ -100,7 +105,7 @@ class FarmMap:
 
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
                  max_voxels=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
-                 stream=None, z_min=None, z_max=None, sim_path=None):
+                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._h = C.c_void_p()
@@ -110,7 +115,8 @@ class FarmMap:
         self.set_option_i(OPT_DESC_DTYPE, dtype)
         for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels),
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
-                       (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path)):
+                       (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
+                       (OPT_TIMING, timing)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:
@@ -143,6 +149,24 @@ class FarmMap:
         _check(load_library().farm_map_integrate_batch(self._h, int(n_frames), _dp(depth), _dp(instance_mask), _dp(K),
                                                        _dp(T_world_cam), _dp(det_descriptors), _hp(n_det)))
         self._last_M = int(n_det.sum())
+
+    def integrate_batch_host(self, n_frames, depth, instance_mask, K, T_world_cam, det_descriptors, n_det):
+        """Host (numpy or pinned torch CPU) buffers; the library stages them itself."""
+        n_det = np.ascontiguousarray(n_det, np.int32)
+
+        def hp(x):
+            if x is None:
+                return None
+            return C.c_void_p(x.data_ptr()) if hasattr(x, "data_ptr") else _hp(x)
+        _check(load_library().farm_map_integrate_batch_host(self._h, int(n_frames), hp(depth), hp(instance_mask), hp(K),
+                                                            hp(T_world_cam), hp(det_descriptors), _hp(n_det)))
+        self._last_M = int(n_det.sum())
+
+    def stage_times(self, reset=False):
+        ms = np.zeros(N_STAGES, np.float32)
+        ln = np.zeros(N_STAGES, np.int64)
+        _check(load_library().farm_map_stage_times(self._h, _hp(ms), _hp(ln), int(bool(reset))))
+        return ms, ln
 
     # ---- results (host arrays)
     def last_assoc(self, M=None):

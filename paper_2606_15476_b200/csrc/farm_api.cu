@@ -47,6 +47,16 @@ struct farm_map {
   int last_M = 0;
   bool has_last = false;
   void *tc = nullptr;
+  // optional per-stage timing (FARM_OPT_TIMING)
+  int timing = 0;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pending[FARM_N_STAGES];
+  std::vector<cudaEvent_t> ev_free;
+  double stage_ms[FARM_N_STAGES] = {};
+  long long stage_launches[FARM_N_STAGES] = {};
+  // staging buffers of farm_map_integrate_batch_host
+  float *h_depth = nullptr, *h_K = nullptr, *h_T = nullptr;
+  uint16_t *h_mask = nullptr;
+  void *h_desc = nullptr;
   size_t elem() const { return dtype == FARM_DTYPE_F32 ? 4 : 2; }
 };
 
@@ -303,6 +313,17 @@ int finalise(farm_map *m) {
   return FARM_OK;
 }
 
+cudaEvent_t get_event(farm_map *m) {
+  if (!m->ev_free.empty()) {
+    cudaEvent_t e = m->ev_free.back();
+    m->ev_free.pop_back();
+    return e;
+  }
+  cudaEvent_t e;
+  cudaEventCreate(&e);
+  return e;
+}
+
 int device_error(farm_map *m) {
   uint32_t e = 0;
   CU(cudaMemcpyAsync(&e, m->dm.err, 4, cudaMemcpyDeviceToHost, m->stream));
@@ -340,6 +361,9 @@ int farm_map_destroy(farm_map *m) {
   if (m->finalised || !m->allocs.empty()) cudaStreamSynchronize(m->stream);
   if (m->tc) tc_state_destroy(m->tc);
   for (void *p : m->allocs) cudaFree(p);
+  for (auto &v : m->ev_pending)
+    for (auto &p : v) cudaEventDestroy(p.first), cudaEventDestroy(p.second);
+  for (cudaEvent_t e : m->ev_free) cudaEventDestroy(e);
   delete m;
   return FARM_OK;
 }
@@ -387,6 +411,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad SIM_PATH");
       m->sim_path = (int)v;
       break;
+    case FARM_OPT_TIMING:
+      if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
+      m->timing = (int)v;
+      break;
     default:
       return fail(FARM_ERR_INVALID_ARG, "unknown integer option");
   }
@@ -433,13 +461,31 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   a.epoch = ++m->epoch;
   a.depth = depth, a.mask = mask, a.K = K, a.T = T, a.desc = desc;
   const DevMap &d = m->dm;
-  m->launches += launch_prep(d, a, m->stream);
-  m->launches += launch_lift(d, a, m->stream);
-  if (m->tc)
-    m->launches += launch_similarity_tc(d, a, m->n_upper, m->stream, m->tc);
-  else
-    m->launches += launch_similarity_fma(d, a, m->n_upper, m->stream);
-  m->launches += launch_assoc_merge_seq(d, a, m->frame_seq, m->stream);
+  cudaStream_t st = m->stream;
+  auto stage = [&](int id, auto &&fn) {
+    const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_SIMILARITY));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (timed) {
+      e0 = get_event(m), e1 = get_event(m);
+      cudaEventRecord(e0, st);
+    }
+    const int n = fn();
+    m->launches += n;
+    m->stage_launches[id] += n;
+    if (timed) {
+      cudaEventRecord(e1, st);
+      m->ev_pending[id].push_back({e0, e1});
+    }
+  };
+  stage(FARM_STAGE_PREP, [&] { return launch_prep(d, a, st); });
+  stage(FARM_STAGE_LIFT, [&] { return launch_lift(d, a, st); });
+  stage(FARM_STAGE_SIMILARITY, [&] {
+    return m->tc ? launch_similarity_tc(d, a, m->n_upper, st, m->tc) : launch_similarity_fma(d, a, m->n_upper, st);
+  });
+  stage(FARM_STAGE_CAND_SCORE, [&] { return launch_cand_score(d, a, st); });
+  stage(FARM_STAGE_ASSOCIATE, [&] { return launch_associate(d, a, st); });
+  stage(FARM_STAGE_COMMIT, [&] { return launch_commit(d, a, st); });
+  stage(FARM_STAGE_MERGE, [&] { return launch_merge(d, a, m->frame_seq, st); });
   CU(cudaGetLastError());
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
@@ -590,6 +636,55 @@ int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, cons
   CU(cudaGetLastError());
   m->n_upper = (uint32_t)n_objects;
   return device_error(m);
+}
+
+int farm_map_integrate_batch_host(farm_map *m, int F, const float *depth, const uint16_t *mask, const float *K,
+                                  const float *T, const void *desc, const int *n_det) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (F < 1 || F > m->max_frames) return fail(FARM_ERR_INVALID_ARG, "n_frames out of range (FARM_OPT_MAX_FRAMES_PER_CALL)");
+  if (!depth || !mask || !K || !T || !n_det) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  long long M = 0;
+  for (int f = 0; f < F; ++f) {
+    if (n_det[f] < 0 || n_det[f] > 65535) return fail(FARM_ERR_INVALID_ARG, "n_det must be in 0..65535");
+    M += n_det[f];
+  }
+  if (M > m->max_det) return fail(FARM_ERR_INVALID_ARG, "too many detections in one call (FARM_OPT_MAX_DET_PER_CALL)");
+  if (M > 0 && !desc) return fail(FARM_ERR_INVALID_ARG, "det_descriptors is NULL");
+  int rc = finalise(m);
+  if (rc != FARM_OK) return rc;
+  const size_t px = (size_t)m->H * m->W;
+  if (!m->h_depth) {  // device staging, sized for the largest call
+    void *p;
+    CU(cudaMalloc(&p, px * m->max_frames * 4)); m->allocs.push_back(p); m->h_depth = (float *)p;
+    CU(cudaMalloc(&p, px * m->max_frames * 2)); m->allocs.push_back(p); m->h_mask = (uint16_t *)p;
+    CU(cudaMalloc(&p, (size_t)m->max_frames * 9 * 4)); m->allocs.push_back(p); m->h_K = (float *)p;
+    CU(cudaMalloc(&p, (size_t)m->max_frames * 16 * 4)); m->allocs.push_back(p); m->h_T = (float *)p;
+    CU(cudaMalloc(&p, (size_t)m->max_det * m->D * m->elem())); m->allocs.push_back(p); m->h_desc = p;
+  }
+  CU(cudaMemcpyAsync(m->h_depth, depth, px * F * 4, cudaMemcpyHostToDevice, m->stream));
+  CU(cudaMemcpyAsync(m->h_mask, mask, px * F * 2, cudaMemcpyHostToDevice, m->stream));
+  CU(cudaMemcpyAsync(m->h_K, K, (size_t)F * 36, cudaMemcpyHostToDevice, m->stream));
+  CU(cudaMemcpyAsync(m->h_T, T, (size_t)F * 64, cudaMemcpyHostToDevice, m->stream));
+  if (M) CU(cudaMemcpyAsync(m->h_desc, desc, (size_t)M * m->D * m->elem(), cudaMemcpyHostToDevice, m->stream));
+  return farm_map_integrate_batch(m, F, m->h_depth, m->h_mask, m->h_K, m->h_T, M ? m->h_desc : nullptr, n_det);
+}
+
+int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (m->finalised) CU(cudaStreamSynchronize(m->stream));
+  for (int s = 0; s < FARM_N_STAGES; ++s) {
+    for (auto &p : m->ev_pending[s]) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, p.first, p.second) == cudaSuccess) m->stage_ms[s] += t;
+      m->ev_free.push_back(p.first);
+      m->ev_free.push_back(p.second);
+    }
+    m->ev_pending[s].clear();
+    if (ms) ms[s] = (float)m->stage_ms[s];
+    if (launches) launches[s] = m->stage_launches[s];
+    if (reset) m->stage_ms[s] = 0.0, m->stage_launches[s] = 0;
+  }
+  return FARM_OK;
 }
 
 int farm_debug_backproject(farm_map *m, const float *depth, const uint16_t *mask, const float *K, const float *T,

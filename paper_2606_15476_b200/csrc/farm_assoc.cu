@@ -297,28 +297,30 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
 
 }  // namespace
 
-template <typename T>
-static int launch_assoc_merge_t(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
-  int launches = 0;
-  if (a.M > 0) {
-    cand_score_kernel<T><<<296, 128, 0, s>>>(m, a);
-    ++launches;
-  }
-  associate_kernel<<<1, 1024, 0, s>>>(m, a);
-  ++launches;
-  if (a.M > 0) {
-    commit_voxels_kernel<<<296, 256, 0, s>>>(m);
-    const int grid = a.M < 148 * 8 ? a.M : 148 * 8;
-    merge_objects_kernel<T><<<grid, 256, (size_t)m.D * sizeof(float), s>>>(m, a, frame_seq0);
-    launches += 2;
-  }
-  return launches;
-}
+#define FARM_DISPATCH(call)                                   \
+  if (m.dtype == FARM_DTYPE_F32) { using T = float; call; }   \
+  else if (m.dtype == FARM_DTYPE_F16) { using T = __half; call; } \
+  else { using T = __nv_bfloat16; call; }
 
-int launch_assoc_merge_seq(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
-  if (m.dtype == FARM_DTYPE_F32) return launch_assoc_merge_t<float>(m, a, frame_seq0, s);
-  if (m.dtype == FARM_DTYPE_F16) return launch_assoc_merge_t<__half>(m, a, frame_seq0, s);
-  return launch_assoc_merge_t<__nv_bfloat16>(m, a, frame_seq0, s);
+int launch_cand_score(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  if (a.M == 0) return 0;
+  FARM_DISPATCH((cand_score_kernel<T><<<296, 128, 0, s>>>(m, a)));
+  return 1;
+}
+int launch_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  associate_kernel<<<1, 1024, 0, s>>>(m, a);
+  return 1;
+}
+int launch_commit(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  if (a.M == 0) return 0;
+  commit_voxels_kernel<<<296, 256, 0, s>>>(m);
+  return 1;
+}
+int launch_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
+  if (a.M == 0) return 0;
+  const int grid = a.M < 148 * 8 ? a.M : 148 * 8;
+  FARM_DISPATCH((merge_objects_kernel<T><<<grid, 256, (size_t)m.D * sizeof(float), s>>>(m, a, frame_seq0)));
+  return 1;
 }
 
 }  // namespace farm

@@ -153,6 +153,9 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,
                              const float *T, int n_det, float *xyz, unsigned long long *keys, cudaStream_t s);
 int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
-int launch_assoc_merge_seq(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
+int launch_cand_score(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_commit(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
 
 }  // namespace farm

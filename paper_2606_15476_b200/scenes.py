@@ -454,3 +454,163 @@ class BoxScene:
     def frames(self, k0: int = 0, k1: Optional[int] = None) -> List[Frame]:
         k1 = self.n_frames if k1 is None else k1
         return [self.frame(k) for k in range(k0, k1)]
+
+
+# --------------------------------------------------------------------------------------- config 4: stress
+class StressScene:
+    """Config 4 (batched throughput stress): a pre-populated map of `n_objects` voxel blobs plus batches of
+    `frames_per_batch` frames with 100 detections each on a 10x10 grid of 64x48 tiles; 50 % of the detections
+    look at an existing object.
+
+    Geometry only: the blob of a looked-at object is the set of voxels its depth patch passes through
+    (every pixel ray at its depth), extruded along the same pixel rays to the requested size.  The voxel
+    index of a scene point is floor(point / voxel) in float64 -- the scene's own bookkeeping of where its
+    surfaces are, independent of the method's fp32 arithmetic (the two agree except for points within an
+    ulp of a voxel face, which merely become new voxels of the matched object).
+    All cameras look along world +x; frames are placed on a y-z lattice wide enough that their frusta and
+    blobs never meet.  Filler objects are random stacks of overlapping rectangles (6-connected) far away.
+    """
+
+    GRID = 10
+    TILE_W, TILE_H = 64, 48
+
+    def __init__(self, n_batches: int, frames_per_batch: int = 16, n_objects: int = 50000,
+                 mean_blob: int = 2000, seed: Optional[int] = None, cfg: Optional[SceneConfig] = None):
+        self.cfg = cfg or get_config(4)
+        self.n_batches, self.F = n_batches, frames_per_batch
+        self.seed = self.cfg.seed if seed is None else seed
+        self.n_objects, self.mean_blob = n_objects, mean_blob
+        self.n_frames = n_batches * frames_per_batch
+        self._frames: List[Frame] = []
+        self._blob_ijk: List[np.ndarray] = []      # per target object: int32 [n,3]
+        self._blob_desc: List[np.ndarray] = []
+        side = int(np.ceil(np.sqrt(self.n_frames)))
+        self._lattice = side
+        for g in range(self.n_frames):
+            self._make_frame(g)
+
+    # ---- frames
+    MASK_W, MASK_H = 48, 36      # labelled region, centred in each 64x48 tile (56 % of the image is masked)
+
+    def _make_frame(self, g: int):
+        cfg = self.cfg
+        rng = rng_for(self.seed, 100 + g)
+        H, W, fx, cx, cy, vs = cfg.H, cfg.W, cfg.fx, cfg.cx, cfg.cy, cfg.voxel
+        pos = np.array([0.0, 10.0 * (g % self._lattice), 8.0 * (g // self._lattice) + 2.0])
+        T = pose_from_yaw(pos, 0.0)                       # right=(0,-1,0) down=(0,0,-1) fwd=(1,0,0)
+        depth = np.full((H, W), 4.5, dtype=np.float64)    # far wall behind everything, unlabelled
+        mask = np.zeros((H, W), dtype=np.uint16)
+        n_det = self.GRID * self.GRID
+        z0_frame = rng.uniform(0.9, 3.2)
+        uu, vv = np.meshgrid(np.arange(self.TILE_W), np.arange(self.TILE_H))
+        base = rng.standard_normal((n_det, cfg.D))
+        base /= np.linalg.norm(base, axis=1, keepdims=True)
+        is_target = np.zeros(n_det, dtype=bool)
+        is_target[rng.permutation(n_det)[: n_det // 2]] = True
+        mu0, mv0 = (self.TILE_W - self.MASK_W) // 2, (self.TILE_H - self.MASK_H) // 2
+        for d in range(n_det):
+            ty, tx = divmod(d, self.GRID)
+            u0, v0 = tx * self.TILE_W, ty * self.TILE_H
+            z0 = z0_frame * rng.uniform(0.9, 1.1)
+            a, b = rng.uniform(-0.0015, 0.0015, size=2) * z0
+            c, ph = rng.uniform(0.0, 0.02) * z0, rng.uniform(0, 2 * np.pi)
+            z = z0 + a * (uu - 32) + b * (vv - 24) + c * np.sin(uu / 9.0 + ph) * np.cos(vv / 7.0)
+            z = z + 0.002 * z * z * rng.standard_normal(z.shape)          # sensor noise sigma = 0.002 z^2
+            depth[v0:v0 + self.TILE_H, u0:u0 + self.TILE_W] = np.clip(z, 0.5, 4.0)
+            mask[v0 + mv0:v0 + mv0 + self.MASK_H, u0 + mu0:u0 + mu0 + self.MASK_W] = d + 1
+        depth32 = depth.astype(np.float32)
+
+        def pack(P):  # scene bookkeeping: voxel cell of a float64 point, three 21-bit fields in one int64
+            q = np.floor(P / vs).astype(np.int64) + (1 << 20)
+            return (q[..., 0] << 42) | (q[..., 1] << 21) | q[..., 2]
+
+        # blobs of the looked-at objects, from the depth actually stored in the frame
+        keys_l, owner_l = [], []
+        targets = np.nonzero(is_target)[0]
+        for slot, d in enumerate(targets):
+            ty, tx = divmod(int(d), self.GRID)
+            u = np.arange(tx * self.TILE_W + mu0, tx * self.TILE_W + mu0 + self.MASK_W)
+            v = np.arange(ty * self.TILE_H + mv0, ty * self.TILE_H + mv0 + self.MASK_H)
+            U, V = np.meshgrid(u, v)
+            zz = depth32[V, U].astype(np.float64)
+            xn, yn = (U - cx) / fx, (V - cy) / fx
+            surf = np.unique(pack(np.stack([pos[0] + zz, pos[1] - xn * zz, pos[2] - yn * zz], -1)).ravel())
+            target_size = rng.uniform(0.5, 1.5) * self.mean_blob
+            # extrude along the pixel rays; layer k lies 0.8*k voxels behind the surface and is wider by (z_k/z)^2
+            zm = float(zz.mean())
+            k = np.arange(1, int(2.0 / (0.8 * vs)) + 1)
+            grow = np.cumsum(0.8 * len(surf) * ((zm + k * 0.8 * vs) / zm) ** 2 / 3.0)
+            L = int(np.searchsorted(grow, max(target_size - len(surf), 0.0))) + 1
+            stride = int(max(1, np.floor(0.5 * vs * fx / zz.max())))
+            zs = zz[::stride, ::stride][None] + (k[:L, None, None] * (0.8 * vs))
+            xs, ys = xn[::stride, ::stride][None], yn[::stride, ::stride][None]
+            deep = np.unique(pack(np.stack([pos[0] + zs, pos[1] - xs * zs, pos[2] - ys * zs], -1)).ravel())
+            kk = np.union1d(surf, deep)
+            keys_l.append(kk)
+            owner_l.append(np.full(len(kk), slot, dtype=np.int64))
+        # exclusive ownership inside the frame: the lowest slot keeps a voxel two blobs share
+        if keys_l:
+            allk, allo = np.concatenate(keys_l), np.concatenate(owner_l)
+            order = np.lexsort((allo, allk))
+            allk, allo = allk[order], allo[order]
+            first = np.ones(len(allk), dtype=bool)
+            first[1:] = allk[1:] != allk[:-1]
+            allk, allo = allk[first], allo[first]
+            m21 = (1 << 21) - 1
+            ijk = np.stack([(allk >> 42) & m21, (allk >> 21) & m21, allk & m21], 1) - (1 << 20)
+            for slot, d in enumerate(targets):
+                self._blob_ijk.append(ijk[allo == slot].astype(np.int32))
+                self._blob_desc.append(base[d])
+        descs = self._view_desc(rng, base)
+        frame = Frame(depth32, mask, intrinsics(cfg), T, to_storage(descs.astype(np.float32), cfg.dtype), n_det,
+                      np.where(is_target, 1, -1).astype(np.int64))
+        self._frames.append(frame)
+
+    @staticmethod
+    def _view_desc(rng, base):
+        D = base.shape[-1]
+        v = base + (0.1 / np.sqrt(D)) * rng.standard_normal(base.shape)
+        return v / np.linalg.norm(v, axis=-1, keepdims=True)
+
+    def batch(self, b: int) -> List[Frame]:
+        return self._frames[b * self.F:(b + 1) * self.F]
+
+    # ---- the pre-populated map
+    def build_map(self):
+        """Returns (ijk int32 [nv,3], owner uint32 [nv], n_voxels uint32 [N], desc float32 [N,D], aabb [N,6])."""
+        cfg = self.cfg
+        rng = rng_for(self.seed, 7)
+        n_t = len(self._blob_ijk)
+        n_fill = max(self.n_objects - n_t, 0)
+        N = n_t + n_fill
+        # filler objects: L layers, each an axis-aligned rectangle overlapping the previous one
+        L = 12
+        side = max(int(round(np.sqrt(self.mean_blob / L))), 2)
+        w = rng.integers(max(side - 3, 1), side + 4, size=(n_fill, L))
+        h = rng.integers(max(side - 3, 1), side + 4, size=(n_fill, L))
+        x0 = 20 + np.cumsum(rng.integers(-2, 3, size=(n_fill, L)), axis=1)
+        y0 = 20 + np.cumsum(rng.integers(-2, 3, size=(n_fill, L)), axis=1)
+        cells = int(np.ceil(np.sqrt(max(n_fill, 1))))
+        cell_i = np.arange(n_fill) % cells
+        cell_j = np.arange(n_fill) // cells
+        area = (w * h).reshape(-1)
+        tot = int(area.sum())
+        rect = np.repeat(np.arange(n_fill * L), area)                       # rectangle id per voxel
+        within = np.arange(tot) - np.repeat(np.cumsum(area) - area, area)   # index inside the rectangle
+        wf = w.reshape(-1)[rect]
+        dx, dy = within % wf, within // wf
+        obj = rect // L
+        lay = rect % L
+        fill_ijk = np.stack([-4000 + x0.reshape(-1)[rect] + dx - 64 * cell_i[obj],
+                             y0.reshape(-1)[rect] + dy + 64 * cell_j[obj],
+                             lay + 40], axis=1).astype(np.int32)
+        fill_owner = (n_t + obj).astype(np.uint32)
+        t_owner = np.concatenate([np.full(len(b), i, dtype=np.uint32) for i, b in enumerate(self._blob_ijk)]) \
+            if n_t else np.zeros(0, np.uint32)
+        ijk = np.concatenate(self._blob_ijk + [fill_ijk]) if n_t else fill_ijk
+        owner = np.concatenate([t_owner, fill_owner])
+        n_vox = np.bincount(owner, minlength=N).astype(np.uint32)
+        fd = rng.standard_normal((n_fill, cfg.D)).astype(np.float32)
+        fd /= np.linalg.norm(fd, axis=1, keepdims=True)
+        desc = np.concatenate([np.array(self._blob_desc, dtype=np.float32).reshape(n_t, cfg.D), fd])
+        return ijk, owner, n_vox, desc

@@ -200,3 +200,46 @@ def test_capacity_error_is_sticky(oracle):
     with pytest.raises(FarmError) as ei:
         g.last_assoc()
     assert ei.value.code == -3
+
+
+def _stress_pair(oracle, sc, **kw):
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    cfg = sc.cfg
+    ijk, owner, n_vox, desc = sc.build_map()
+    keys = pack_key(ijk[:, 0], ijk[:, 1], ijk[:, 2])
+    objs = np.zeros(len(n_vox), OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(len(n_vox)), n_vox, 1, -1, -1
+    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, **kw)
+    assert o.import_(objs, desc, keys, owner) == 0
+    g.import_(objs, desc, keys, owner)
+    return o, g
+
+
+def test_config4_mini_stress_batches(oracle):
+    """configs[4] structure at reduced size: imported blob map, batches of 4 frames x 100 detections, half of
+    them overlapping existing objects; whole pipeline and final map against the oracle."""
+    sc = S.StressScene(n_batches=2, frames_per_batch=4, n_objects=700)
+    o, g = _stress_pair(oracle, sc)
+    compare_maps(g, o)
+    for b in range(2):
+        frames = margin_filter(o.clone, sc.batch(b), sc.cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, sc.cfg.dtype)
+        compare_call(g, o)
+        a, n, _, st = g.last_assoc()
+        assert 0.4 < st["matches"] / st["n_det"] < 0.6
+    compare_maps(g, o)
+
+
+def test_host_buffer_entry_point_matches_device_path(oracle):
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    from helpers import stack_frames
+    for k in range(5):
+        fr = sc.frame(k)
+        integrate_frames(o, [fr])
+        depth, mask, K, T, desc, n_det = stack_frames([fr])
+        g.integrate_batch_host(1, depth, mask, K, T, np.ascontiguousarray(desc), n_det)
+        compare_call(g, o)
+    compare_maps(g, o)
