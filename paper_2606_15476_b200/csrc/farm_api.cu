@@ -167,7 +167,7 @@ __global__ void import_voxels_kernel(DevMap m, const unsigned long long *keys, c
       atomicOr(m.err, ERR_IMPORT_DUPLICATE);
       continue;
     }
-    unsigned long long h = mix64(key) & m.table_mask;
+    unsigned long long h = voxel_hash(key) & m.table_mask;
     bool done = false;
     for (unsigned long long probe = 0; probe <= m.table_mask && probe < (1ull << 20); ++probe) {
       unsigned long long k = m.table[h].key;
@@ -462,6 +462,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   a.depth = depth, a.mask = mask, a.K = K, a.T = T, a.desc = desc;
   const DevMap &d = m->dm;
   cudaStream_t st = m->stream;
+  bool launch_failed = false;
   auto stage = [&](int id, auto &&fn) {
     const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_SIMILARITY));
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -469,7 +470,8 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
       e0 = get_event(m), e1 = get_event(m);
       cudaEventRecord(e0, st);
     }
-    const int n = fn();
+    int n = fn();
+    if (n < 0) launch_failed = true, n = 0;
     m->launches += n;
     m->stage_launches[id] += n;
     if (timed) {
@@ -487,6 +489,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   stage(FARM_STAGE_COMMIT, [&] { return launch_commit(d, a, st); });
   stage(FARM_STAGE_MERGE, [&] { return launch_merge(d, a, m->frame_seq, st); });
   CU(cudaGetLastError());
+  if (launch_failed) return fail(FARM_ERR_CUDA, "similarity: cuTensorMapEncodeTiled failed (descriptor pointer must be 16-byte aligned)");
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
   m->last_M = (int)M;

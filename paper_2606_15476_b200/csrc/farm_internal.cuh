@@ -129,6 +129,18 @@ __device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
   return x;
 }
 
+// cheap 2-word hash (multiply-xorshift); used for the voxel table, the per-call scratch tables and the tile set
+__device__ __forceinline__ uint32_t hash32(uint32_t a, uint32_t b) {
+  uint32_t h = (a * 0x9E3779B1u) ^ (b * 0x85EBCA77u);
+  h ^= h >> 15;
+  h *= 0x2C1B3C6Du;
+  h ^= h >> 12;
+  h *= 0x297A2D39u;
+  h ^= h >> 15;
+  return h;
+}
+__device__ __forceinline__ uint32_t voxel_hash(unsigned long long key) { return hash32((uint32_t)key, (uint32_t)(key >> 32)); }
+
 template <typename T>
 __device__ __forceinline__ float to_f32(T v);
 template <>

@@ -15,7 +15,7 @@ constexpr int TILE_W = 128;
 constexpr int TILE_H = 8;
 constexpr int LIFT_THREADS = 128;
 constexpr int TILE_PX = TILE_W * TILE_H;
-constexpr int TILE_HASH = 2048;  // smem dedupe set, load <= 0.5
+constexpr int TILE_HASH = 1024;  // smem dedupe set (a filter: overflow passes through to the exact global set)
 constexpr int MAX_LABELS = 32;   // per-tile detection accumulators
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
@@ -52,15 +52,17 @@ __device__ __forceinline__ void backproject(const Camera &c, int u, int v, float
                      c.t[i]);
 }
 
-// R6
+// R6: index = floor(fp32(X * inv_vs)) per axis, valid iff in [-2^20, 2^20).  cvt.rmi (round towards -inf,
+// saturating) is floor-then-convert in one instruction; the float pre-test rejects NaN and anything the
+// saturation would alias.
 __device__ __forceinline__ bool voxel_key(const float p[3], float inv_vs, unsigned long long *key) {
-  const float qx = floorf(__fmul_rn(p[0], inv_vs));
-  const float qy = floorf(__fmul_rn(p[1], inv_vs));
-  const float qz = floorf(__fmul_rn(p[2], inv_vs));
-  const float lo = (float)-KEY_BIAS, hi = (float)KEY_BIAS;
-  if (!(qx >= lo && qx < hi && qy >= lo && qy < hi && qz >= lo && qz < hi)) return false;
-  *key = ((unsigned long long)((int)qx + KEY_BIAS) << 42) | ((unsigned long long)((int)qy + KEY_BIAS) << 21) |
-         (unsigned long long)((int)qz + KEY_BIAS);
+  const float fx = __fmul_rn(p[0], inv_vs), fy = __fmul_rn(p[1], inv_vs), fz = __fmul_rn(p[2], inv_vs);
+  const bool finite = fabsf(fx) < 2.0e6f && fabsf(fy) < 2.0e6f && fabsf(fz) < 2.0e6f;
+  const uint32_t ix = (uint32_t)(__float2int_rd(fx) + KEY_BIAS), iy = (uint32_t)(__float2int_rd(fy) + KEY_BIAS),
+                 iz = (uint32_t)(__float2int_rd(fz) + KEY_BIAS);
+  if (!finite || ((ix | iy | iz) >> 21) != 0) return false;
+  const uint32_t lo = iz | (iy << 21), hi = (iy >> 11) | (ix << 10);
+  *key = ((unsigned long long)hi << 32) | lo;
   return true;
 }
 
@@ -108,7 +110,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
 
 // find-or-insert `key` in the voxel table; returns slot index or NONE32 when the table is full.
 __device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsigned long long key) {
-  unsigned long long h = mix64(key) & m.table_mask;
+  unsigned long long h = voxel_hash(key) & m.table_mask;
   for (unsigned long long probe = 0; probe <= m.table_mask; ++probe) {
     unsigned long long k = __ldcg(&m.table[h].key);
     if (k == KEY_EMPTY) {
@@ -127,7 +129,7 @@ __device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsign
 // returns 1 = newly inserted, 0 = already present, -1 = table full.
 __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t mask, unsigned long long v,
                                             uint32_t epoch, uint32_t *slot) {
-  uint32_t h = (uint32_t)mix64(v) & mask;
+  uint32_t h = hash32((uint32_t)v, (uint32_t)(v >> 32) * 0x632BE5ABu) & mask;
   for (uint32_t probe = 0; probe <= mask; ++probe) {
     unsigned long long cur = __ldcg(&tab[h]);
     for (;;) {
@@ -161,9 +163,9 @@ struct TileSmem {
   uint32_t n_valid, n_dropped, n_ignored;
 };
 
-// accumulate one thread's run (j, cnt, box) into the tile's per-detection accumulators
-__device__ __forceinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32_t j, uint32_t cnt, const int mn[3],
-                                               const int mx[3]) {
+// accumulate a run (j, cnt, box as ordered ints) into the tile's per-detection accumulators
+__device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32_t j, uint32_t cnt, int mn0, int mn1,
+                                            int mn2, int mx0, int mx1, int mx2) {
   uint32_t h = j % MAX_LABELS;
   for (int probe = 0; probe < MAX_LABELS; ++probe) {
     uint32_t l = *(volatile uint32_t *)&s.lab_j[h];
@@ -173,22 +175,35 @@ __device__ __forceinline__ void tile_label_add(TileSmem &s, const DevMap &m, uin
     }
     if (l == j) {
       atomicAdd(&s.lab_cnt[h], cnt);
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        atomicMin(&s.lab_box[h][k], mn[k]);
-        atomicMax(&s.lab_box[h][3 + k], mx[k]);
-      }
+      atomicMin(&s.lab_box[h][0], mn0), atomicMin(&s.lab_box[h][1], mn1), atomicMin(&s.lab_box[h][2], mn2);
+      atomicMax(&s.lab_box[h][3], mx0), atomicMax(&s.lab_box[h][4], mx1), atomicMax(&s.lab_box[h][5], mx2);
       return;
     }
     h = (h + 1) % MAX_LABELS;
   }
   // more than MAX_LABELS detections inside one tile: go to global memory directly
   atomicAdd(&m.det_npx[j], cnt);
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    atomicMin(&m.det_box[j * 6 + k], mn[k]);
-    atomicMax(&m.det_box[j * 6 + 3 + k], mx[k]);
+  atomicMin(&m.det_box[j * 6 + 0], mn0), atomicMin(&m.det_box[j * 6 + 1], mn1), atomicMin(&m.det_box[j * 6 + 2], mn2);
+  atomicMax(&m.det_box[j * 6 + 3], mx0), atomicMax(&m.det_box[j * 6 + 4], mx1), atomicMax(&m.det_box[j * 6 + 5], mx2);
+}
+
+// shared-memory set keyed (key, j): a filter only, the global pair set is exact.  Returns true when the
+// pair has not been seen in this tile (or the probe budget ran out).
+__device__ __noinline__ bool tile_set_insert(TileSmem &s, unsigned long long key, uint32_t j) {
+  uint32_t h = hash32((uint32_t)key, (uint32_t)(key >> 32) + j * 0x632BE5ABu) & (TILE_HASH - 1);
+  for (int probe = 0; probe < 16; ++probe) {
+    unsigned long long k2 = *(volatile unsigned long long *)&s.hkey[h];
+    if (k2 == KEY_EMPTY) {
+      k2 = atomicCAS(&s.hkey[h], KEY_EMPTY, key);
+      if (k2 == KEY_EMPTY) {
+        *(volatile uint32_t *)&s.hlab[h] = j;
+        return true;
+      }
+    }
+    if (k2 == key && *(volatile uint32_t *)&s.hlab[h] == j) return false;
+    h = (h + 1) & (TILE_HASH - 1);
   }
+  return true;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -207,7 +222,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
 
   // ---- issue the loads first (all independent), then initialise shared memory while they fly
   float z[8];
-  uint16_t lab[8];
+  uint32_t lab[8];
   const size_t frame_off = (size_t)f * m.H * m.W;
   const bool row_ok = v < m.H;
   if (VEC && row_ok && u0 + 7 < m.W) {
@@ -223,7 +238,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
     for (int i = 0; i < 8; ++i) {
       const bool ok = row_ok && u0 + i < m.W;
       const size_t off = frame_off + (size_t)v * m.W + u0 + i;
-      lab[i] = ok ? __ldcs(a.mask + off) : (uint16_t)0;
+      lab[i] = ok ? (uint32_t)__ldcs(a.mask + off) : 0u;
       z[i] = ok ? __ldcs(a.depth + off) : 0.f;
     }
   }
@@ -243,62 +258,49 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
   if (tid == 0) s.q_count = 0, s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
   const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
   const int det_base = a.base[f];
-  const int n_det_f = a.base[f + 1] - det_base;
+  const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
+  // R5 terms that are shared by the thread's 8 pixels (same row)
+  const float yn = __fmul_rn(__fsub_rn((float)v, cam.cy), cam.inv_fy);
   __syncthreads();
 
   // ---- per pixel: validity (R3, R4), back-projection (R5), key (R6), tile-level dedupe
-  uint32_t cur_j = NONE32, cur_cnt = 0;
-  int mn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+  const float INF = __int_as_float(0x7F800000);
+  uint32_t cur_l = 0, cur_cnt = 0;  // current run of equal labels (label 0 = none)
+  float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
   unsigned long long prev_key = KEY_EMPTY;
-  uint32_t prev_j = NONE32;
+  uint32_t prev_l = 0;
   uint32_t n_valid = 0, n_dropped = 0, n_ignored = 0;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     bool fresh = false;
     unsigned long long key = KEY_EMPTY;
-    uint32_t j = NONE32;
     const uint32_t l = lab[i];
     if (l != 0) {
-      if ((int)l > n_det_f) {
+      if (l > n_det_f) {
         n_ignored++;
       } else if (depth_valid(z[i], m.z_min, m.z_max)) {
         float p[3];
-        backproject(cam, u0 + i, v, z[i], p);
+        const float xn = __fmul_rn(__fsub_rn((float)(u0 + i), cam.cx), cam.inv_fx);
+        const float xc = __fmul_rn(xn, z[i]), yc = __fmul_rn(yn, z[i]);
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+          p[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(cam.r[3 * k], xc), __fmul_rn(cam.r[3 * k + 1], yc)),
+                                     __fmul_rn(cam.r[3 * k + 2], z[i])),
+                           cam.t[k]);
         if (voxel_key(p, m.inv_vs, &key)) {
           n_valid++;
-          j = (uint32_t)(det_base + (int)l - 1);
-          if (j != cur_j) {
-            if (cur_j != NONE32) tile_label_add(s, m, cur_j, cur_cnt, mn, mx);
-            cur_j = j, cur_cnt = 0;
-#pragma unroll
-            for (int k = 0; k < 3; ++k) mn[k] = 0x7FFFFFFF, mx[k] = (int)0x80000000;
+          if (l != cur_l) {
+            if (cur_l) tile_label_add(s, m, (uint32_t)det_base + cur_l - 1, cur_cnt, f2ord(mn0), f2ord(mn1), f2ord(mn2),
+                                      f2ord(mx0), f2ord(mx1), f2ord(mx2));
+            cur_l = l, cur_cnt = 0;
+            mn0 = mn1 = mn2 = INF, mx0 = mx1 = mx2 = -INF;
           }
           cur_cnt++;
-#pragma unroll
-          for (int k = 0; k < 3; ++k) {
-            const int o = f2ord(p[k]);
-            mn[k] = min(mn[k], o), mx[k] = max(mx[k], o);
-          }
-          if (!(key == prev_key && j == prev_j)) {  // thread-local dedupe of consecutive pixels
-            prev_key = key, prev_j = j;
-            // shared-memory set keyed (key, j): a filter only, the global pair set is exact
-            uint32_t h = ((uint32_t)(key ^ (key >> 21) ^ (key >> 42)) * 0x9E3779B1u + j * 0x85EBCA6Bu) >> 21;
-            fresh = true;
-            for (int probe = 0; probe < 32; ++probe) {
-              unsigned long long k2 = *(volatile unsigned long long *)&s.hkey[h];
-              if (k2 == KEY_EMPTY) {
-                k2 = atomicCAS(&s.hkey[h], KEY_EMPTY, key);
-                if (k2 == KEY_EMPTY) {
-                  *(volatile uint32_t *)&s.hlab[h] = j;
-                  break;
-                }
-              }
-              if (k2 == key && *(volatile uint32_t *)&s.hlab[h] == j) {
-                fresh = false;
-                break;
-              }
-              h = (h + 1) & (TILE_HASH - 1);
-            }
+          mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
+          mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
+          if (!(key == prev_key && l == prev_l)) {  // thread-local dedupe of consecutive pixels
+            prev_key = key, prev_l = l;
+            fresh = tile_set_insert(s, key, (uint32_t)det_base + l - 1);
           }
         } else {
           n_dropped++;
@@ -314,27 +316,25 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
       if (fresh) {
         const uint32_t pos = base + __popc(b & ((1u << lane) - 1));
         s.qkey[pos] = key;
-        s.qj[pos] = j;
+        s.qj[pos] = (uint32_t)det_base + l - 1;
       }
     }
   }
   // per-detection pixel count and point AABB (R7): warp-uniform fast path through REDUX, else per thread
   {
-    const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_j != NONE32);
+    const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_l != 0);
     if (has) {
-      const uint32_t lead_j = __shfl_sync(0xFFFFFFFFu, cur_j, __ffs(has) - 1);
-      const bool uniform = __all_sync(0xFFFFFFFFu, cur_j == NONE32 || cur_j == lead_j);
+      const uint32_t lead_l = __shfl_sync(0xFFFFFFFFu, cur_l, __ffs(has) - 1);
+      const bool uniform = __all_sync(0xFFFFFFFFu, cur_l == 0 || cur_l == lead_l);
+      const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
       if (uniform) {
         const uint32_t cnt = __reduce_add_sync(0xFFFFFFFFu, cur_cnt);
-        int rmn[3], rmx[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-          rmn[k] = __reduce_min_sync(0xFFFFFFFFu, mn[k]);
-          rmx[k] = __reduce_max_sync(0xFFFFFFFFu, mx[k]);
-        }
-        if (lane == 0) tile_label_add(s, m, lead_j, cnt, rmn, rmx);
-      } else if (cur_j != NONE32) {
-        tile_label_add(s, m, cur_j, cur_cnt, mn, mx);
+        const int r0 = __reduce_min_sync(0xFFFFFFFFu, o0), r1 = __reduce_min_sync(0xFFFFFFFFu, o1),
+                  r2 = __reduce_min_sync(0xFFFFFFFFu, o2), r3 = __reduce_max_sync(0xFFFFFFFFu, o3),
+                  r4 = __reduce_max_sync(0xFFFFFFFFu, o4), r5 = __reduce_max_sync(0xFFFFFFFFu, o5);
+        if (lane == 0) tile_label_add(s, m, (uint32_t)det_base + lead_l - 1, cnt, r0, r1, r2, r3, r4, r5);
+      } else if (cur_l != 0) {
+        tile_label_add(s, m, (uint32_t)det_base + cur_l - 1, cur_cnt, o0, o1, o2, o3, o4, o5);
       }
     }
     n_valid = __reduce_add_sync(0xFFFFFFFFu, n_valid);
@@ -377,6 +377,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
       uint32_t base = 0;
       if (lane == 0) base = atomicAdd(&m.counters[0], (uint32_t)__popc(act));
       base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      const unsigned oact = __ballot_sync(0xFFFFFFFFu, owned);
       if (is_new) {
         const uint32_t pos = base + __popc(act & ((1u << lane) - 1));
         if (pos < m.pair_cap)
@@ -389,7 +390,6 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
         if (!owned) atomicMin(&m.table[slot].claim, j);  // R12: lowest detection index wins
       }
       // overlap histogram c[j][owner] += 1, aggregated over lanes with the same (j, owner)
-      const unsigned oact = __ballot_sync(act, owned);
       if (owned) {
         const unsigned long long jo = ((unsigned long long)j << 32) | owner;
         const unsigned same = __match_any_sync(oact, jo);

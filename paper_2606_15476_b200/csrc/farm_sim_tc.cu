@@ -1,8 +1,321 @@
-// farm_sim_tc.cu -- step 4 on the 5th-generation tensor cores (placeholder until the tcgen05 kernel lands).
+// farm_sim_tc.cu -- step 4 on the 5th-generation tensor cores (sm_100a: tcgen05.mma + TMEM + TMA).
+//
+//   cos(a_d, b_o) for every detection d and every object o of the entry snapshot (R14-R16; PAPER.md:350
+//   "a single batched detection-by-entity similarity matrix").  A = detection rows [M, D], B = the map's
+//   storage-dtype shadows [N, D], both K-major (D contiguous), bf16 or fp16 in, fp32 accumulate in TMEM.
+//   The M x N result is never written: the epilogue scales every accumulator column by 1/|b_o|, keeps the
+//   row maximum and its lowest-id argmax, and publishes clamp(max/|a_d|) with one atomicMax per row and
+//   tile (R15, R18 tie rule, R19).
+//
+// Shape of the kernel (persistent, one CTA per SM, 256 threads):
+//   warp 0      TMA producer: A tile 128 x 64 and B tile 256 x 64 per stage, SWIZZLE_128B, 4-stage mbarrier ring
+//   warp 1      MMA issuer: one elected thread, tcgen05.mma.cta_group::1.kind::f16, UMMA 128 x 256 x 16
+//   warp 2      TMEM allocator (512 columns = two 128 x 256 fp32 accumulators, double buffered)
+//   warps 4-7   epilogue: tcgen05.ld 32 lanes x 32 columns at a time, one detection row per thread
+// Detections sit on the UMMA M axis (TMEM lanes) so that the per-detection max over objects is a scan
+// along TMEM columns inside one thread -- no cross-thread reduction.
+// N is read from device memory (no host sync); tiles are enumerated m-fastest so that concurrently
+// running CTAs share the B tile in L2.
+#include <cuda.h>
+
 #include "farm_internal.cuh"
+
 namespace farm {
-bool tc_supported(const DevMap &) { return false; }
-void *tc_state_create(const DevMap &) { return nullptr; }
-void tc_state_destroy(void *) {}
-int launch_similarity_tc(const DevMap &, const CallArgs &, uint32_t, cudaStream_t, void *) { return 0; }
+namespace {
+
+constexpr int BLOCK_M = 128;  // detections per tile (UMMA M)
+constexpr int BLOCK_N = 256;  // objects per tile (UMMA N)
+constexpr int BLOCK_K = 64;   // 64 x 16-bit = one 128-byte swizzle row
+constexpr int UMMA_K = 16;
+constexpr int STAGES = 4;
+constexpr int TC_THREADS = 256;
+constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2;  // 16 KB
+constexpr uint32_t B_BYTES = BLOCK_N * BLOCK_K * 2;  // 32 KB
+constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr uint32_t TMEM_COLS = 512;
+constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + STAGES * STAGE_BYTES + 2 * BLOCK_N * 4 + 256;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+      "l"(map), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tcgen05_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tcgen05_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// shared-memory matrix descriptor: K-major operand, SWIZZLE_128B, rows of 128 bytes, 8-row groups 1024 B apart
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);  // start address, 16-byte units
+  d |= (uint64_t)1 << 16;                   // leading byte offset (unused for swizzled K-major), 16-byte units
+  d |= (uint64_t)(1024 >> 4) << 32;         // stride byte offset between 8-row core groups
+  d |= (uint64_t)1 << 46;                   // descriptor version (sm_100)
+  d |= (uint64_t)2 << 61;                   // SWIZZLE_128B
+  return d;
+}
+
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
+                     int M, uint32_t idesc) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // SWIZZLE_128B needs 1024-byte alignment
+  float *ib_s = (float *)(smem + STAGES * STAGE_BYTES);                         // [2][BLOCK_N] inverse norms of B
+  uint64_t *bars = (uint64_t *)(ib_s + 2 * BLOCK_N);
+  uint64_t *full_bar = bars, *empty_bar = bars + STAGES, *tfull_bar = bars + 2 * STAGES, *tempty_bar = bars + 2 * STAGES + 2;
+  uint32_t *tmem_slot = (uint32_t *)(bars + 2 * STAGES + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int N = (int)*m.n_objects;
+  const int tiles_m = (M + BLOCK_M - 1) / BLOCK_M, tiles_n = (N + BLOCK_N - 1) / BLOCK_N;
+  const int n_tiles = tiles_m * tiles_n;
+  const int k_blocks = (m.D + BLOCK_K - 1) / BLOCK_K;
+
+  if (warp == 0 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&map_a) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&map_b) : "memory");
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < STAGES; ++i) {
+      mbar_init(smem_u32(&full_bar[i]), 1);
+      mbar_init(smem_u32(&empty_bar[i]), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&tfull_bar[i]), 1);
+      mbar_init(smem_u32(&tempty_bar[i]), 4);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(TMEM_COLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      uint32_t stage = 0, phase = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int tm = tile % tiles_m, tn = tile / tiles_m;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
+          const uint32_t fb = smem_u32(&full_bar[stage]);
+          mbar_expect_tx(fb, STAGE_BYTES);
+          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES);
+          tma_load_2d(sa, &map_a, fb, kb * BLOCK_K, tm * BLOCK_M);
+          tma_load_2d(sa + A_BYTES, &map_b, fb, kb * BLOCK_K, tn * BLOCK_N);
+          if (++stage == STAGES) stage = 0, phase ^= 1;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      uint32_t stage = 0, phase = 0, as = 0, aphase = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);  // epilogue has drained this accumulator
+        tcgen05_fence_after();
+        const uint32_t tmem_d = tmem_base + as * BLOCK_N;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          mbar_wait(smem_u32(&full_bar[stage]), phase);
+          tcgen05_fence_after();
+          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES);
+          const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sa + A_BYTES);
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+            // advance 32 bytes (16 elements) along K inside the 128-byte swizzle row: +2 in 16-byte units
+            umma_f16(tmem_d, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+          }
+          umma_commit(smem_u32(&empty_bar[stage]));  // frees the smem stage when these MMAs retire
+          if (++stage == STAGES) stage = 0, phase ^= 1;
+        }
+        umma_commit(smem_u32(&tfull_bar[as]));  // accumulator complete
+        if (++as == 2) as = 0, aphase ^= 1;
+      }
+    }
+  } else if (warp >= 4) {
+    // ===== epilogue: one detection row per thread =====
+    const int q = warp & 3;            // TMEM lane quadrant this warp may access
+    const int row_in_tile = q * 32 + lane;
+    const int et = threadIdx.x - 128;  // 0..127
+    uint32_t as = 0, aphase = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int tm = tile % tiles_m, tn = tile / tiles_m;
+      const int n0 = tn * BLOCK_N;
+      const int ncols = min(BLOCK_N, N - n0);
+      float *ib = ib_s + as * BLOCK_N;
+      ib[et] = et < ncols ? m.inv_norm[n0 + et] : 0.f;
+      ib[et + 128] = et + 128 < ncols ? m.inv_norm[n0 + et + 128] : 0.f;
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+      tcgen05_fence_after();
+      float best = -3.0e38f;
+      int best_c = 0;
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
+#pragma unroll 1
+      for (int c0 = 0; c0 < BLOCK_N; c0 += 32) {
+        if (c0 >= ncols) break;
+        uint32_t r[32];
+        tmem_ld32(taddr + c0, r);
+        tmem_ld_wait();
+        if (c0 + 32 <= ncols) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float v = __uint_as_float(r[i]) * ib[c0 + i];
+            if (v > best) best = v, best_c = c0 + i;
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float v = __uint_as_float(r[i]) * ib[c0 + i];
+            if (c0 + i < ncols && v > best) best = v, best_c = c0 + i;
+          }
+        }
+      }
+      tcgen05_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+      const int row = tm * BLOCK_M + row_in_tile;
+      if (row < M) {
+        const float ia = m.det_inv_norm[row];
+        float cs = best * ia;
+        cs = fminf(1.f, fmaxf(-1.f, cs));                    // R15 clamp
+        if (ia == 0.f) cs = 0.f, best_c = 0;                 // zero-norm detection: cos = 0 for every object
+        atomicMax(&m.best_dense[row], pack_score(cs, (uint32_t)(n0 + best_c)));
+      }
+      if (++as == 2) as = 0, aphase ^= 1;
+    }
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS));
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TcState {
+  EncodeTiledFn encode = nullptr;
+  CUtensorMap map_b;
+  CUtensorMapDataType dt;
+  uint32_t idesc;
+  int num_sms = 148;
+  bool ok = false;
+};
+
+bool encode_2d(TcState *st, CUtensorMap *map, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  const cuuint64_t gdim[2] = {cols, rows};
+  const cuuint64_t gstride[1] = {cols * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)BLOCK_K, box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  return st->encode(map, st->dt, 2, const_cast<void *>(base), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+bool tc_supported(const DevMap &m) { return m.dtype != FARM_DTYPE_F32 && m.D % 8 == 0 && m.D >= 8; }
+
+void *tc_state_create(const DevMap &m) {
+  TcState *st = new TcState();
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    delete st;
+    return nullptr;
+  }
+  st->encode = (EncodeTiledFn)fn;
+  st->dt = m.dtype == FARM_DTYPE_F16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+  const uint32_t fmt = m.dtype == FARM_DTYPE_F16 ? 0u : 1u;
+  // instruction descriptor, kind::f16: D = fp32, A/B = fmt, both K-major, N = 256, M = 128
+  st->idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(BLOCK_M >> 4) << 24);
+  if (!encode_2d(st, &st->map_b, m.desc_shadow, m.max_objects, (uint64_t)m.D, BLOCK_N)) {
+    delete st;
+    return nullptr;
+  }
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&st->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaFuncSetAttribute(similarity_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
+    delete st;
+    return nullptr;
+  }
+  st->ok = true;
+  return st;
+}
+
+void tc_state_destroy(void *p) { delete (TcState *)p; }
+
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state) {
+  TcState *st = (TcState *)state;
+  if (a.M == 0 || n_upper == 0) return 0;
+  CUtensorMap map_a;
+  if (!encode_2d(st, &map_a, a.desc, (uint64_t)a.M, (uint64_t)m.D, BLOCK_M)) return -1;  // loud: the caller fails the call
+  const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
+  const int grid = (int)(tiles < st->num_sms ? tiles : st->num_sms);
+  similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc);
+  return 1;
+}
+
 }  // namespace farm
