@@ -41,6 +41,7 @@ def parse():
     p.add_argument("--n-objects", type=int, default=50000, help="pre-populated objects (config 4); the benchmark value is only valid at 50000")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--overlap", type=int, default=1, help="0 = run similarity on the main stream (no lift || similarity overlap)")
     p.add_argument("--breakdown", action="store_true", help="bracket every kernel with CUDA events (perturbs `value`)")
     return p.parse_args()
 
@@ -162,7 +163,7 @@ def run_ours(args):
         m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
                     max_objects=max_objects, max_voxels=max_voxels, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
                     max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
-                    timing=timing)
+                    timing=timing, overlap=args.overlap)
         m.import_(objs, desc, keys, owner)
         return m
 

@@ -60,12 +60,13 @@ extern "C" {
 #define FARM_OPT_MAX_VOXELS 3        /* owned-voxel capacity; table = next pow2 >= 2x, default 1<<22           */
 #define FARM_OPT_IMG_W 4             /* image width  (required)                                                */
 #define FARM_OPT_IMG_H 5             /* image height (required)                                                */
-#define FARM_OPT_MAX_DET_PER_CALL 6  /* sum of n_det over the frames of one call, default 4096, max 2^21-1      */
+#define FARM_OPT_MAX_DET_PER_CALL 6  /* sum of n_det over the frames of one call, default 4096, max 65535        */
 #define FARM_OPT_STREAM 7            /* cudaStream_t as integer, default 0 (legacy default stream)             */
 #define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
 #define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
 #define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
 #define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the lift and similarity kernels; 2 every kernel */
+#define FARM_OPT_OVERLAP 12          /* 1 (default): similarity runs on an internal side stream concurrently with lift */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -155,10 +156,10 @@ int farm_map_sync(farm_map *m, farm_totals *totals);
 #define FARM_STAGE_PREP 0        /* reset of per-call state + detection row norms            */
 #define FARM_STAGE_LIFT 1        /* steps 1-3: back-project, voxelise, dedupe, probe, overlap */
 #define FARM_STAGE_SIMILARITY 2  /* step 4: dense cosine with fused row max / argmax          */
-#define FARM_STAGE_CAND_SCORE 3  /* step 5a: scores of the sparse overlap candidates          */
-#define FARM_STAGE_ASSOCIATE 4   /* step 5a: argmax, threshold, new ids                       */
-#define FARM_STAGE_COMMIT 5      /* step 5b: voxel ownership commit                           */
-#define FARM_STAGE_MERGE 6       /* step 5b: descriptors, AABB, view evidence                 */
+#define FARM_STAGE_CAND_SCORE 3  /* (unused: fused into ASSOCIATE)                            */
+#define FARM_STAGE_ASSOCIATE 4   /* step 5a: candidate scores, argmax, threshold, new ids     */
+#define FARM_STAGE_COMMIT 5      /* (unused: fused into MERGE)                                */
+#define FARM_STAGE_MERGE 6       /* step 5b: voxel commit, descriptors, AABB, view evidence   */
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset);
 
 /* Number of kernels this library has launched for the map so far (host counter). */

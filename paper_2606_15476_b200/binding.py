@@ -19,6 +19,7 @@ DTYPE_F32, DTYPE_F16, DTYPE_BF16 = 0, 1, 2
 OPT_DESC_DTYPE, OPT_MAX_OBJECTS, OPT_MAX_VOXELS, OPT_IMG_W, OPT_IMG_H = 1, 2, 3, 4, 5
 OPT_MAX_DET_PER_CALL, OPT_STREAM, OPT_MAX_PAIRS_PER_CALL, OPT_MAX_FRAMES_PER_CALL, OPT_SIM_PATH = 6, 7, 8, 9, 10
 OPT_TIMING = 11
+OPT_OVERLAP = 12
 N_STAGES = 7
 STAGE_NAMES = ["prep", "lift", "similarity", "cand_score", "associate", "commit", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
@@ -105,7 +106,7 @@ class FarmMap:
 
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
                  max_voxels=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
-                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None):
+                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._h = C.c_void_p()
@@ -116,7 +117,7 @@ class FarmMap:
         for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels),
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
-                       (OPT_TIMING, timing)):
+                       (OPT_TIMING, timing), (OPT_OVERLAP, overlap)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:

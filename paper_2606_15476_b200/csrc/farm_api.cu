@@ -47,6 +47,9 @@ struct farm_map {
   int last_M = 0;
   bool has_last = false;
   void *tc = nullptr;
+  cudaStream_t side = nullptr;             // similarity runs here, concurrently with lift + probe
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  int overlap = 1;
   // optional per-stage timing (FARM_OPT_TIMING)
   int timing = 0;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pending[FARM_N_STAGES];
@@ -190,6 +193,12 @@ __global__ void import_voxels_kernel(DevMap m, const unsigned long long *keys, c
   }
 }
 
+__global__ void clear_visit_kernel(DevMap m) {
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
+       i += (unsigned long long)gridDim.x * blockDim.x)
+    m.table[i].visit = 0xFFFFFFFFu;
+}
+
 __global__ void count_voxels_kernel(DevMap m, unsigned long long *count) {
   unsigned long long c = 0;
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
@@ -270,8 +279,9 @@ int finalise(farm_map *m) {
   A(d.best_view, NO, 0);
   A(d.best_cam, NO * 3, 0);
   A(d.leader, NO, 0xFF);
+  A(d.grp_cnt, NO, 0);
   const long long tcap = next_pow2(std::max<long long>(2 * m->max_voxels, 1024));
-  A(d.table, (size_t)tcap, 0xFF);  // key = EMPTY, owner = PENDING, claim = NONE
+  A(d.table, (size_t)tcap, 0xFF);  // key = EMPTY, owner = OWNER_INIT, visit = dead epoch 0xFFFF
   d.table_mask = (unsigned long long)tcap - 1;
   const long long pcap = next_pow2(2 * m->max_pairs);
   A(d.pair_set, (size_t)pcap, 0);
@@ -288,6 +298,10 @@ int finalise(farm_map *m) {
   A(d.cand_o, (size_t)ccap, 0);
   A(d.cand_c, (size_t)ccap, 0);
   d.cand_cap = (uint32_t)ccap;
+  const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30);
+  A(d.surv_key, (size_t)scap, 0);
+  A(d.surv_j, (size_t)scap, 0);
+  d.surv_cap = (uint32_t)scap;
   A(d.counters, 4, 0);
   const size_t MD = (size_t)m->max_det;
   d.max_det = (uint32_t)MD;
@@ -308,6 +322,13 @@ int finalise(farm_map *m) {
   m->launches++;
   CU(cudaGetLastError());
   if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
+  if (m->overlap) {
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    CU(cudaStreamCreateWithPriority(&m->side, cudaStreamNonBlocking, prio_hi));  // similarity CTAs are placed first
+    CU(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+  }
   if (m->sim_path == 2 && !m->tc) return fail(FARM_ERR_INVALID_ARG, "tensor-core similarity path not available for this dtype / D");
   m->finalised = true;
   return FARM_OK;
@@ -359,6 +380,9 @@ int farm_map_create(float voxel_size, int D, float w_geo, float w_sem, float tau
 int farm_map_destroy(farm_map *m) {
   if (!m) return FARM_OK;
   if (m->finalised || !m->allocs.empty()) cudaStreamSynchronize(m->stream);
+  if (m->side) cudaStreamSynchronize(m->side), cudaStreamDestroy(m->side);
+  if (m->ev_fork) cudaEventDestroy(m->ev_fork);
+  if (m->ev_join) cudaEventDestroy(m->ev_join);
   if (m->tc) tc_state_destroy(m->tc);
   for (void *p : m->allocs) cudaFree(p);
   for (auto &v : m->ev_pending)
@@ -393,7 +417,7 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       m->H = (int)v;
       break;
     case FARM_OPT_MAX_DET_PER_CALL:
-      if (v < 1 || v >= (1ll << DET_BITS)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_DET_PER_CALL");
+      if (v < 1 || v >= (1ll << DET_BITS)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_DET_PER_CALL (1..65535)");
       m->max_det = v;
       break;
     case FARM_OPT_STREAM:
@@ -410,6 +434,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
     case FARM_OPT_SIM_PATH:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad SIM_PATH");
       m->sim_path = (int)v;
+      break;
+    case FARM_OPT_OVERLAP:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad OVERLAP");
+      m->overlap = (int)v;
       break;
     case FARM_OPT_TIMING:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
@@ -452,9 +480,11 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (M > 0 && !desc) return fail(FARM_ERR_INVALID_ARG, "det_descriptors is NULL");
   int rc = finalise(m);
   if (rc != FARM_OK) return rc;
-  if (m->epoch == EPOCH_MAX) {  // the epoch tag wrapped: clear the per-call scratch tables once
+  if (m->epoch == EPOCH_MAX - 1) {  // the 16-bit epoch tag wraps: clear every epoch-tagged word once per 65534 calls
     CU(cudaMemsetAsync(m->dm.pair_set, 0, ((size_t)m->dm.pair_mask + 1) * 8, m->stream));
     CU(cudaMemsetAsync(m->dm.ov_keys, 0, ((size_t)m->dm.ov_mask + 1) * 8, m->stream));
+    clear_visit_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm);
+    m->launches++;
     m->epoch = 0;
   }
   a.M = (int)M;
@@ -463,7 +493,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   const DevMap &d = m->dm;
   cudaStream_t st = m->stream;
   bool launch_failed = false;
-  auto stage = [&](int id, auto &&fn) {
+  auto stage = [&](int id, cudaStream_t st, auto &&fn) {
     const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_SIMILARITY));
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (timed) {
@@ -479,15 +509,23 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
       m->ev_pending[id].push_back({e0, e1});
     }
   };
-  stage(FARM_STAGE_PREP, [&] { return launch_prep(d, a, st); });
-  stage(FARM_STAGE_LIFT, [&] { return launch_lift(d, a, st); });
-  stage(FARM_STAGE_SIMILARITY, [&] {
-    return m->tc ? launch_similarity_tc(d, a, m->n_upper, st, m->tc) : launch_similarity_fma(d, a, m->n_upper, st);
+  // DAG of one call:  prep -> { similarity (side stream) || lift + probe } -> cand_score+associate -> commit+merge
+  const bool fork = m->overlap && m->side && a.M > 0 && m->n_upper > 0;
+  cudaStream_t sim_stream = fork ? m->side : st;
+  stage(FARM_STAGE_PREP, st, [&] { return launch_prep(d, a, st); });
+  if (fork) {
+    cudaEventRecord(m->ev_fork, st);
+    cudaStreamWaitEvent(m->side, m->ev_fork, 0);
+  }
+  // similarity is enqueued first so that its one-CTA-per-SM grid is resident before the lift tiles fill the SMs
+  stage(FARM_STAGE_SIMILARITY, sim_stream, [&] {
+    return m->tc ? launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc) : launch_similarity_fma(d, a, m->n_upper, sim_stream);
   });
-  stage(FARM_STAGE_CAND_SCORE, [&] { return launch_cand_score(d, a, st); });
-  stage(FARM_STAGE_ASSOCIATE, [&] { return launch_associate(d, a, st); });
-  stage(FARM_STAGE_COMMIT, [&] { return launch_commit(d, a, st); });
-  stage(FARM_STAGE_MERGE, [&] { return launch_merge(d, a, m->frame_seq, st); });
+  if (fork) cudaEventRecord(m->ev_join, m->side);
+  stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
+  if (fork) cudaStreamWaitEvent(st, m->ev_join, 0);
+  stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
+  stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
   CU(cudaGetLastError());
   if (launch_failed) return fail(FARM_ERR_CUDA, "similarity: cuTensorMapEncodeTiled failed (descriptor pointer must be 16-byte aligned)");
   m->frame_seq += F;

@@ -9,73 +9,87 @@ namespace {
 
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
-// ---- candidate scoring: one warp per non-zero overlap entry (d, o, c)
+// ---- candidate scoring + association, one launch.
+// Phase 1 (all CTAs): one warp per non-zero overlap entry (d, o, c): cos(a_d, shadow_o) by a gather dot, g (R10),
+//   score (R17), atomicMax into best_cand[d].
+// Phase 2 (the last CTA to finish, found by a ticket): decisions for all detections (R18), new ids by an
+//   exclusive scan in detection index order (R20), per-target leader / group size for the merge.
 template <typename T>
-__global__ void __launch_bounds__(128) cand_score_kernel(DevMap m, CallArgs a) {
-  const uint32_t n_cand = min(m.counters[1], m.cand_cap);
-  const int lane = threadIdx.x & 31;
-  const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
-  const int D = m.D;
-  for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < n_cand; c += warps) {
-    const uint32_t slot = m.cand_slot[c];
-    const unsigned long long kv = m.ov_keys[slot];
-    const uint32_t j = (uint32_t)(kv >> 32) & ((1u << DET_BITS) - 1);
-    const uint32_t o = (uint32_t)kv;
-    const uint32_t cnt = m.ov_cnt[slot];
-    __syncwarp();
-    if (lane == 0) {
-      m.ov_cnt[slot] = 0;  // invariant: counts are zero between calls (the tables are epoch tagged)
-      m.cand_j[c] = j;
-      m.cand_o[c] = (int32_t)o;
-      m.cand_c[c] = cnt;
-    }
-    const T *x = (const T *)a.desc + (size_t)j * D;
-    const T *y = (const T *)m.desc_shadow + (size_t)o * D;
-    float dot = 0.f;
-    if (sizeof(T) == 2 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {
-      for (int i = lane * 8; i < D; i += 256) {
-        const uint4 xv = *reinterpret_cast<const uint4 *>(x + i);
-        const uint4 yv = *reinterpret_cast<const uint4 *>(y + i);
-        const T *xe = reinterpret_cast<const T *>(&xv);
-        const T *ye = reinterpret_cast<const T *>(&yv);
-#pragma unroll
-        for (int q = 0; q < 8; ++q) dot = fmaf(to_f32<T>(xe[q]), to_f32<T>(ye[q]), dot);
-      }
-    } else {
-      for (int i = lane; i < D; i += 32) dot = fmaf(to_f32<T>(x[i]), to_f32<T>(y[i]), dot);
-    }
-#pragma unroll
-    for (int s = 16; s; s >>= 1) dot += __shfl_xor_sync(0xFFFFFFFFu, dot, s);
-    if (lane == 0) {
-      float cs = dot * m.det_inv_norm[j] * m.inv_norm[o];
-      cs = fminf(1.f, fmaxf(-1.f, cs));                                  // R15
-      const uint32_t mn = min(m.det_nv[j], m.n_voxels[o]);
-      const float g = mn ? __fdiv_rn((float)cnt, (float)mn) : 0.f;       // R10
-      const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));  // R17
-      atomicMax(&m.best_cand[j], pack_score(score, o));
-    }
-  }
-}
-
-// ---- association: one CTA; decisions, new ids by an exclusive scan in detection index order (R18, R20)
-__global__ void __launch_bounds__(1024) associate_kernel(DevMap m, CallArgs a) {
+__global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs a) {
   __shared__ uint32_t warp_sum[32];
   __shared__ uint32_t s_running, s_matches, s_skipped;
+  __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t N = *m.n_objects;
-  if (tid == 0) s_running = 0, s_matches = 0, s_skipped = 0;
+  {
+    const uint32_t n_cand = min(m.counters[1], m.cand_cap);
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    const int D = m.D;
+    for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < n_cand; c += warps) {
+      const uint32_t slot = m.cand_slot[c];
+      const unsigned long long kv = m.ov_keys[slot];
+      const uint32_t j = (uint32_t)(kv >> 32) & ((1u << DET_BITS) - 1);
+      const uint32_t o = (uint32_t)kv;
+      const uint32_t cnt = m.ov_cnt[slot];
+      __syncwarp();
+      if (lane == 0) {
+        m.ov_cnt[slot] = 0;  // invariant: counts are zero between calls (the tables are epoch tagged)
+        m.cand_j[c] = j;
+        m.cand_o[c] = (int32_t)o;
+        m.cand_c[c] = cnt;
+      }
+      const T *x = (const T *)a.desc + (size_t)j * D;
+      const T *y = (const T *)m.desc_shadow + (size_t)o * D;
+      float dot = 0.f;
+      if (sizeof(T) == 2 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {
+        for (int i = lane * 8; i < D; i += 256) {
+          const uint4 xv = *reinterpret_cast<const uint4 *>(x + i);
+          const uint4 yv = *reinterpret_cast<const uint4 *>(y + i);
+          const T *xe = reinterpret_cast<const T *>(&xv);
+          const T *ye = reinterpret_cast<const T *>(&yv);
+#pragma unroll
+          for (int q = 0; q < 8; ++q) dot = fmaf(to_f32<T>(xe[q]), to_f32<T>(ye[q]), dot);
+        }
+      } else {
+        for (int i = lane; i < D; i += 32) dot = fmaf(to_f32<T>(x[i]), to_f32<T>(y[i]), dot);
+      }
+#pragma unroll
+      for (int sft = 16; sft; sft >>= 1) dot += __shfl_xor_sync(0xFFFFFFFFu, dot, sft);
+      if (lane == 0) {
+        float cs = dot * m.det_inv_norm[j] * m.inv_norm[o];
+        cs = fminf(1.f, fmaxf(-1.f, cs));                                  // R15
+        const uint32_t mn = min(m.det_nv[j], m.n_voxels[o]);
+        const float g = mn ? __fdiv_rn((float)cnt, (float)mn) : 0.f;       // R10
+        const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));  // R17
+        atomicMax(&m.best_cand[j], pack_score(score, o));
+      }
+    }
+  }
+  // ---- ticket: the last CTA to arrive runs the association
   __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    const uint32_t t = atomicAdd(&m.counters[3], 1u);
+    s_last = t == gridDim.x - 1;
+    if (s_last) m.counters[3] = 0;
+    s_running = 0, s_matches = 0, s_skipped = 0;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const uint32_t N = __ldcg(m.n_objects);
+  unsigned long long valid_points = 0;
+  if (tid == 0) valid_points = __ldcg(&m.stats->valid_points);
   for (int base = 0; base < a.M; base += 1024) {
     const int j = base + tid;
     uint32_t spawn = 0, matched = 0, skipped = 0;
     int32_t target = -1;
     float score = 0.f;
     if (j < a.M) {
-      if (m.det_npx[j] == 0) {
+      if (__ldcg(&m.det_npx[j]) == 0) {
         skipped = 1;  // R8
       } else {
-        unsigned long long best = m.best_cand[j];
-        const unsigned long long bd = m.best_dense[j];
+        unsigned long long best = __ldcg(&m.best_cand[j]);
+        const unsigned long long bd = __ldcg(&m.best_dense[j]);
         if (bd) {
           // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
           const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd)));
@@ -116,7 +130,10 @@ __global__ void __launch_bounds__(1024) associate_kernel(DevMap m, CallArgs a) {
       m.assoc[j] = target;
       m.is_new[j] = (uint8_t)spawn;
       m.best_score[j] = score;
-      if (target >= 0) atomicMin(&m.leader[target], (uint32_t)j);
+      if (target >= 0) {
+        atomicMin(&m.leader[target], (uint32_t)j);
+        atomicAdd(&m.grp_cnt[target], 1u);
+      }
     }
     const unsigned bm = __ballot_sync(0xFFFFFFFFu, matched), bs = __ballot_sync(0xFFFFFFFFu, skipped);
     if (lane == 0) {
@@ -130,70 +147,86 @@ __global__ void __launch_bounds__(1024) associate_kernel(DevMap m, CallArgs a) {
   if (tid == 0) {
     uint32_t spawns = s_running;
     if (N + spawns > m.max_objects) spawns = m.max_objects - N;
+    const uint32_t pairs = __ldcg(&m.counters[0]);
     *m.n_objects = N + spawns;
     m.stats->matches = s_matches;
     m.stats->spawns = spawns;
     m.stats->skipped = s_skipped;
-    m.stats->unique_voxels = m.counters[0];
-    m.totals->frames += a.F;
-    m.totals->calls += 1;
-    m.totals->valid_points += m.stats->valid_points;
-    m.totals->unique_voxels += m.counters[0];
-    m.totals->matches += s_matches;
-    m.totals->spawns += spawns;
+    m.stats->unique_voxels = pairs;
+    atomicAdd(&m.totals->frames, (unsigned long long)a.F);
+    atomicAdd(&m.totals->calls, 1ull);
+    atomicAdd(&m.totals->valid_points, valid_points);
+    atomicAdd(&m.totals->unique_voxels, (unsigned long long)pairs);
+    atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
+    atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
   }
 }
 
-// ---- voxel commit (R12 pass 2): the claim winner of every key inserted by this call sets the owner
-__global__ void __launch_bounds__(256) commit_voxels_kernel(DevMap m) {
-  const uint32_t n = min(m.counters[0], m.pair_cap);
-  const int lane = threadIdx.x & 31;
-  for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < n; i0 += gridDim.x * blockDim.x) {
-    const uint32_t i = i0 + lane;
-    int32_t t = -1;
-    if (i < n) {
-      const unsigned long long p = m.pair_list[i];
-      if (p >> 63) {
-        const uint32_t j = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
-        const uint32_t slot = (uint32_t)p;
-        if (m.table[slot].claim == j) {
-          t = m.assoc[j];
-          if (t >= 0) m.table[slot].owner = (uint32_t)t;
-        }
-      }
-    }
-    const unsigned act = __ballot_sync(0xFFFFFFFFu, t >= 0);
-    if (t >= 0) {
-      const unsigned same = __match_any_sync(act, t);
-      if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], (uint32_t)__popc(same));
-    }
-  }
-}
-
-// ---- object merge: the lowest-index detection of every target object folds the whole group (R21-R23).
-// One CTA per detection; non-leaders exit at once.  No atomics, deterministic summation order.
+// ---- voxel commit + object merge, one launch.
+// CTAs [0, commit_blocks): R12 pass 2 -- the claim winner of every key inserted by this call sets the owner.
+// CTAs [commit_blocks, ...): the lowest-index detection of every target object folds the whole group
+//   (R21 count-weighted descriptor mean, R22 AABB, R23 view evidence).  No atomics on the object, deterministic
+//   summation order.  Groups of one (the common case) skip the member scan.
 template <typename T>
-__global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0) {
+__global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0,
+                                                           int commit_blocks) {
   extern __shared__ float acc[];  // [D]
   __shared__ uint32_t list[256];
   __shared__ uint32_t warp_cnt[8];
   __shared__ float red[8];
   __shared__ float s_bcast;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if ((int)blockIdx.x < commit_blocks) {
+    const uint32_t n = min(m.counters[0], m.pair_cap);
+    for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < n; i0 += commit_blocks * blockDim.x) {
+      const uint32_t i = i0 + lane;
+      int32_t t = -1;
+      if (i < n) {
+        const unsigned long long p = m.pair_list[i];
+        if (p >> 63) {
+          const uint32_t j = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
+          const uint32_t slot = (uint32_t)p;
+          if (m.table[slot].owner == (OWNER_PENDING | j)) {  // this detection holds the claim (R12)
+            t = m.assoc[j];
+            if (t >= 0) m.table[slot].owner = (uint32_t)t;
+          }
+        }
+      }
+      const unsigned act = __ballot_sync(0xFFFFFFFFu, t >= 0);
+      if (t >= 0) {
+        const unsigned same = __match_any_sync(act, t);
+        if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], (uint32_t)__popc(same));
+      }
+    }
+    return;
+  }
   const int D = m.D;
-  for (int j = blockIdx.x; j < a.M; j += gridDim.x) {
+  const int merge_blocks = gridDim.x - commit_blocks;
+  for (int j = blockIdx.x - commit_blocks; j < a.M; j += merge_blocks) {
     const int32_t t = m.assoc[j];
     if (t < 0 || m.leader[t] != (uint32_t)j) continue;  // uniform per CTA
+    const uint32_t group = m.grp_cnt[t];
+    // old object state, loaded early by thread 0 so that the latency hides behind the descriptor work
+    uint32_t n_old_t0 = 0;
+    unsigned long long pts_old = 0, best_old = 0;
+    int box_old[6];
+    if (tid == 0) {
+      n_old_t0 = m.n_obs[t];
+      pts_old = m.n_points[t];
+      best_old = m.best_view[t];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
+    }
     for (int i = tid; i < D; i += 256) acc[i] = 0.f;
-    // scalar aggregates live in thread 0
     uint32_t k_members = 0;
     unsigned long long pts = 0, best = 0;
     int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
     int best_frame = -1;
     __syncthreads();
-    for (int base = j & ~255; base < a.M; base += 256) {  // members have index >= j
+    const int scan_end = group > 1 ? a.M : j + 1;  // a group of one is just the leader itself
+    for (int base = j & ~255; base < scan_end; base += 256) {  // members have index >= j
       const int jj = base + tid;
-      const bool flag = jj < a.M && jj >= j && m.assoc[jj] == t;
+      const bool flag = jj < scan_end && jj >= j && m.assoc[jj] == t;
       const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
       if (lane == 0) warp_cnt[warp] = __popc(b);
       __syncthreads();
@@ -237,12 +270,12 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
     T *shadow = (T *)m.desc_shadow + (size_t)t * D;
     float ss = 0.f;
     for (int i = tid; i < D; i += 256) {
-      const float v = fmaf((float)n_old, master[i], acc[i]);
+      const float v = n_old ? fmaf((float)n_old, master[i], acc[i]) : acc[i];
       acc[i] = v;
       ss = fmaf(v, v, ss);
     }
 #pragma unroll
-    for (int s = 16; s; s >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, s);
+    for (int sft = 16; sft; sft >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, sft);
     if (lane == 0) red[warp] = ss;
     __syncthreads();
     if (tid == 0) {
@@ -264,7 +297,7 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
         s2 = fmaf(sv, sv, s2);
       }
 #pragma unroll
-      for (int s = 16; s; s >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, s);
+      for (int sft = 16; sft; sft >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, sft);
       __syncthreads();
       if (lane == 0) red[warp] = s2;
       __syncthreads();
@@ -275,14 +308,14 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
       }
     }
     if (tid == 0) {
-      m.n_obs[t] = n_old + k_members;
-      m.n_points[t] += pts;
+      m.n_obs[t] = n_old_t0 + k_members;
+      m.n_points[t] = pts_old + pts;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {  // R22
-        m.aabb[t * 6 + c] = min(m.aabb[t * 6 + c], bmn[c]);
-        m.aabb[t * 6 + 3 + c] = max(m.aabb[t * 6 + 3 + c], bmx[c]);
+        m.aabb[t * 6 + c] = min(box_old[c], bmn[c]);
+        m.aabb[t * 6 + 3 + c] = max(box_old[3 + c], bmx[c]);
       }
-      if (best > m.best_view[t]) {
+      if (best > best_old) {
         m.best_view[t] = best;
         const float *Tf = a.T + 16 * best_frame;
         m.best_cam[t * 3 + 0] = Tf[3];
@@ -290,6 +323,7 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
         m.best_cam[t * 3 + 2] = Tf[11];
       }
       m.leader[t] = NONE32;
+      m.grp_cnt[t] = 0;
     }
     __syncthreads();
   }
@@ -302,24 +336,17 @@ __global__ void __launch_bounds__(256) merge_objects_kernel(DevMap m, CallArgs a
   else if (m.dtype == FARM_DTYPE_F16) { using T = __half; call; } \
   else { using T = __nv_bfloat16; call; }
 
-int launch_cand_score(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  if (a.M == 0) return 0;
-  FARM_DISPATCH((cand_score_kernel<T><<<296, 128, 0, s>>>(m, a)));
+int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  const int grid = a.M > 0 ? 37 : 1;  // 37 x 32 warps = one warp per candidate for ~1.2k candidates per wave
+  FARM_DISPATCH((cand_associate_kernel<T><<<grid, 1024, 0, s>>>(m, a)));
   return 1;
 }
-int launch_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  associate_kernel<<<1, 1024, 0, s>>>(m, a);
-  return 1;
-}
-int launch_commit(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
-  commit_voxels_kernel<<<296, 256, 0, s>>>(m);
-  return 1;
-}
-int launch_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
-  if (a.M == 0) return 0;
-  const int grid = a.M < 148 * 8 ? a.M : 148 * 8;
-  FARM_DISPATCH((merge_objects_kernel<T><<<grid, 256, (size_t)m.D * sizeof(float), s>>>(m, a, frame_seq0)));
+  const int commit_blocks = 148 * 4;
+  const int merge_blocks = a.M < 148 * 8 ? a.M : 148 * 8;
+  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, 256, (size_t)m.D * sizeof(float), s>>>(
+      m, a, frame_seq0, commit_blocks)));
   return 1;
 }
 

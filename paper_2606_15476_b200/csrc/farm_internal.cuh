@@ -11,12 +11,12 @@
 namespace farm {
 
 constexpr uint64_t KEY_EMPTY = 0xFFFFFFFFFFFFFFFFull;
-constexpr uint32_t OWNER_PENDING = 0xFFFFFFFFu;  // slot inserted but not yet committed to an object
-constexpr uint32_t CLAIM_NONE = 0xFFFFFFFFu;
+constexpr uint32_t OWNER_PENDING = 0x80000000u;  // owner >= this: inserted by the running call, low bits = claim (R12)
+constexpr uint32_t OWNER_INIT = 0xFFFFFFFFu;     // free slot: pending with no claim yet
 constexpr int KEY_BIAS = 1 << 20;
 constexpr int MAX_FRAMES = 64;
-constexpr int EPOCH_BITS = 11;                    // per-call scratch tables are epoch tagged, never cleared
-constexpr int DET_BITS = 21;
+constexpr int EPOCH_BITS = 16;                    // per-call scratch state is epoch tagged, never cleared
+constexpr int DET_BITS = 16;                      // detections per call < 2^16
 constexpr uint32_t EPOCH_MAX = (1u << EPOCH_BITS) - 1;
 
 // sticky device error bits
@@ -29,8 +29,11 @@ constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
 // Global voxel -> object hash slot (R11: one owner per key).  16 bytes, one 32-byte sector per probe.
 struct __align__(16) VoxelSlot {
   unsigned long long key;  // KEY_EMPTY when free
-  uint32_t owner;          // OWNER_PENDING until the inserting call commits
-  uint32_t claim;          // lowest detection index j of the inserting call that contains the key (R12)
+  uint32_t owner;          // object id; while the inserting call runs: OWNER_PENDING | lowest detection index j
+                           // of that call containing the key (R12: that detection's object will own it)
+  uint32_t visit;          // (epoch << 16 | j) of the first detection that touched the key in the current call:
+                           // makes (detection, key) pairs exact without a second random access; other
+                           // detections of the same call fall back to the per-call pair set
 };
 
 struct CallStats {  // device mirror of farm_frame_stats
@@ -58,6 +61,7 @@ struct DevMap {
   unsigned long long *best_view;     // packed (n_px, ~frame_seq, ~det) for max()
   float *best_cam;                   // [max_objects,3]
   uint32_t *leader;                  // scratch: lowest j of the call that targets the object
+  uint32_t *grp_cnt;                 // scratch: number of detections of the call that target the object
   // voxel hash
   VoxelSlot *table;
   unsigned long long table_mask;     // capacity-1
@@ -74,7 +78,10 @@ struct DevMap {
   uint32_t *cand_j;                  // compact copy for the debug read
   int32_t *cand_o;
   uint32_t *cand_c;
-  uint32_t *counters;                // [0]=pair_count [1]=cand_count
+  unsigned long long *surv_key;      // survivor queue of the lift kernel: (key, j) after tile-level dedupe
+  uint32_t *surv_j;
+  uint32_t surv_cap;
+  uint32_t *counters;                // [0]=pair_count [1]=cand_count [2]=survivor_count [3]=block ticket
   // per detection [max_det]
   uint32_t max_det;
   uint32_t *det_nv, *det_npx;
@@ -165,9 +172,7 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,
                              const float *T, int n_det, float *xyz, unsigned long long *keys, cudaStream_t s);
 int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
-int launch_cand_score(const DevMap &m, const CallArgs &a, cudaStream_t s);
-int launch_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
-int launch_commit(const DevMap &m, const CallArgs &a, cudaStream_t s);
-int launch_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
+int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
 
 }  // namespace farm

@@ -15,7 +15,7 @@ constexpr int TILE_W = 128;
 constexpr int TILE_H = 8;
 constexpr int LIFT_THREADS = 128;
 constexpr int TILE_PX = TILE_W * TILE_H;
-constexpr int TILE_HASH = 1024;  // smem dedupe set (a filter: overflow passes through to the exact global set)
+constexpr int TILE_HASH = 1024;  // slots of the direct-mapped tile filter
 constexpr int MAX_LABELS = 32;   // per-tile detection accumulators
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
@@ -79,6 +79,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     m.counters[0] = 0;
     m.counters[1] = 0;
+    m.counters[2] = 0;
     CallStats z = {};
     z.n_det = (uint32_t)a.M;
     *m.stats = z;
@@ -108,18 +109,24 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
 // ---------------------------------------------------------------------------------------------------
 // global structures
 
-// find-or-insert `key` in the voxel table; returns slot index or NONE32 when the table is full.
-__device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsigned long long key) {
+// find-or-insert `key` in the voxel table with one 16-byte probe per slot; returns the slot index (NONE32 when the
+// table is full) and the slot's owner / visit words as loaded (free slots hold OWNER_INIT / a dead epoch).
+__device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsigned long long key, uint32_t *owner,
+                                                         uint32_t *visit) {
   unsigned long long h = voxel_hash(key) & m.table_mask;
-  for (unsigned long long probe = 0; probe <= m.table_mask; ++probe) {
-    unsigned long long k = __ldcg(&m.table[h].key);
+  for (int probe = 0; probe < 8192; ++probe) {
+    const uint4 w = __ldcg(reinterpret_cast<const uint4 *>(&m.table[h]));
+    unsigned long long k = ((unsigned long long)w.y << 32) | w.x;
     if (k == KEY_EMPTY) {
       k = atomicCAS(&m.table[h].key, KEY_EMPTY, key);
-      if (k == KEY_EMPTY) return (uint32_t)h;  // inserted: owner == OWNER_PENDING, claim == CLAIM_NONE already
+      if (k == KEY_EMPTY) k = key;  // inserted: owner == OWNER_INIT already
     }
-    if (k == key) return (uint32_t)h;
+    if (k == key) {
+      *owner = w.z;
+      *visit = w.w;
+      return (uint32_t)h;
+    }
     h = (h + 1) & m.table_mask;
-    if (probe > 4096) break;
   }
   atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
   return NONE32;
@@ -137,7 +144,7 @@ __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t ma
         *slot = h;
         return 0;
       }
-      if ((uint32_t)(cur >> (64 - EPOCH_BITS)) == epoch) break;  // live entry of another pair
+      if ((uint32_t)(cur >> 48) == epoch) break;  // live entry of another pair
       const unsigned long long old = atomicCAS(&tab[h], cur, v);
       if (old == cur) {
         *slot = h;
@@ -152,14 +159,13 @@ __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t ma
 }
 
 struct TileSmem {
-  unsigned long long hkey[TILE_HASH];
+  unsigned long long tag[TILE_HASH];   // direct-mapped filter of (key, label) pairs already queued by this tile
   unsigned long long qkey[TILE_PX];
-  uint32_t hlab[TILE_HASH];
   uint32_t qj[TILE_PX];
   uint32_t lab_j[MAX_LABELS];
   uint32_t lab_cnt[MAX_LABELS];
   int lab_box[MAX_LABELS][6];
-  uint32_t q_count;
+  uint32_t q_count, q_base;
   uint32_t n_valid, n_dropped, n_ignored;
 };
 
@@ -187,28 +193,24 @@ __device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32
   atomicMax(&m.det_box[j * 6 + 3], mx0), atomicMax(&m.det_box[j * 6 + 4], mx1), atomicMax(&m.det_box[j * 6 + 5], mx2);
 }
 
-// shared-memory set keyed (key, j): a filter only, the global pair set is exact.  Returns true when the
-// pair has not been seen in this tile (or the probe budget ran out).
-__device__ __noinline__ bool tile_set_insert(TileSmem &s, unsigned long long key, uint32_t j) {
-  uint32_t h = hash32((uint32_t)key, (uint32_t)(key >> 32) + j * 0x632BE5ABu) & (TILE_HASH - 1);
-  for (int probe = 0; probe < 16; ++probe) {
-    unsigned long long k2 = *(volatile unsigned long long *)&s.hkey[h];
-    if (k2 == KEY_EMPTY) {
-      k2 = atomicCAS(&s.hkey[h], KEY_EMPTY, key);
-      if (k2 == KEY_EMPTY) {
-        *(volatile uint32_t *)&s.hlab[h] = j;
-        return true;
-      }
-    }
-    if (k2 == key && *(volatile uint32_t *)&s.hlab[h] == j) return false;
-    h = (h + 1) & (TILE_HASH - 1);
-  }
+// Tile-level dedupe: a direct-mapped, lock-free filter in shared memory.  The slot index carries the low 10
+// bits of the label and bit 63 of the tag the 11th, so an equal tag in the same slot means the same
+// (key, label) pair exactly (labels >= 2048 bypass the filter).  It may let duplicates through (evictions,
+// races); it never drops a pair.  The exact set is the global pair set of probe_kernel.
+__device__ __forceinline__ bool tile_filter_fresh(TileSmem &s, unsigned long long key, uint32_t l) {
+  if (l >= 2048u) return true;
+  const uint32_t slot = (hash32((uint32_t)key, (uint32_t)(key >> 32)) ^ l) & (TILE_HASH - 1);
+  const unsigned long long tag = key | ((unsigned long long)((l >> 10) & 1u) << 63);
+  if (tag == KEY_EMPTY) return true;  // indistinguishable from an empty slot: never filtered
+  if (*(volatile unsigned long long *)&s.tag[slot] == tag) return false;
+  *(volatile unsigned long long *)&s.tag[slot] = tag;
   return true;
 }
 
 // ---------------------------------------------------------------------------------------------------
-// The lift kernel.  One 128x8 pixel tile per CTA; each thread owns 8 consecutive pixels of one row
-// (2 x 128-bit depth loads + 1 x 128-bit mask load).
+// lift kernel (steps 1-2).  One 128x8 pixel tile per CTA; each thread owns 8 consecutive pixels of one row
+// (2 x 128-bit depth loads + 1 x 128-bit mask load).  Output: per-detection pixel counts and point boxes,
+// and the tile's distinct (detection, voxel key) pairs appended to the call's survivor queue.
 template <bool VEC>
 __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   __shared__ TileSmem s;
@@ -242,10 +244,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
       z[i] = ok ? __ldcs(a.depth + off) : 0.f;
     }
   }
-  for (int i = tid; i < TILE_HASH; i += LIFT_THREADS) {
-    s.hkey[i] = KEY_EMPTY;
-    s.hlab[i] = NONE32;
-  }
+  for (int i = tid; i < TILE_HASH; i += LIFT_THREADS) s.tag[i] = KEY_EMPTY;
   if (tid < MAX_LABELS) {
     s.lab_j[tid] = NONE32;
     s.lab_cnt[tid] = 0;
@@ -259,7 +258,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
   const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
   const int det_base = a.base[f];
   const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
-  // R5 terms that are shared by the thread's 8 pixels (same row)
+  // R5 term shared by the thread's 8 pixels (same row)
   const float yn = __fmul_rn(__fsub_rn((float)v, cam.cy), cam.inv_fy);
   __syncthreads();
 
@@ -300,7 +299,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
           mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
           if (!(key == prev_key && l == prev_l)) {  // thread-local dedupe of consecutive pixels
             prev_key = key, prev_l = l;
-            fresh = tile_set_insert(s, key, (uint32_t)det_base + l - 1);
+            fresh = tile_filter_fresh(s, key, l);
           }
         } else {
           n_dropped++;
@@ -348,27 +347,80 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
   }
   __syncthreads();
 
-  // ---- survivors: global voxel table (find or insert), exact per-call pair set, |V_d|, overlap histogram
+  // ---- append the tile queue to the call's survivor queue (one global atomic per tile, coalesced copy)
   const uint32_t nq = s.q_count;
-  for (uint32_t i0 = (tid & ~31u); i0 < nq; i0 += LIFT_THREADS) {
+  if (tid == 0 && nq) s.q_base = atomicAdd(&m.counters[2], nq);
+  // ---- flush the tile's per-detection accumulators and counters
+  if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
+    const uint32_t j = s.lab_j[tid];
+    atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
+      atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
+    }
+  }
+  if (tid == 0) {
+    if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
+    if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
+    if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
+  }
+  if (nq == 0) return;
+  __syncthreads();
+  const uint32_t qb = s.q_base;
+  for (uint32_t i = tid; i < nq; i += LIFT_THREADS) {
+    const uint32_t pos = qb + i;
+    if (pos < m.surv_cap) {
+      m.surv_key[pos] = s.qkey[i];
+      m.surv_j[pos] = s.qj[i];
+    } else {
+      atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// probe kernel (step 3 and R12 pass 1).  One thread per queued (detection, key) pair: find or insert the
+// key in the global voxel table, make the pair exact through the per-call pair set, then
+//   |V_d| += 1,  append to the pair list,  overlap c[d][owner] += 1 when the key was owned at entry (R9),
+//   claim = min(claim, d) when this call inserted the key (R12).
+// Atomics are aggregated over the lanes of a warp that hit the same address (__match_any_sync).
+__global__ void __launch_bounds__(256) probe_kernel(DevMap m, CallArgs a) {
+  const uint32_t nq = min(m.counters[2], m.surv_cap);
+  const int lane = threadIdx.x & 31;
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < nq; i0 += stride) {
     const uint32_t i = i0 + lane;
     bool is_new = false, owned = false;
     uint32_t j = 0, slot = NONE32, owner = OWNER_PENDING;
     if (i < nq) {
-      const unsigned long long key = s.qkey[i];
-      j = s.qj[i];
-      slot = voxel_find_or_insert(m, key);
+      const unsigned long long key = __ldcs(&m.surv_key[i]);
+      j = __ldcs(&m.surv_j[i]);
+      uint32_t visit = 0;
+      slot = voxel_find_or_insert(m, key, &owner, &visit);
       if (slot != NONE32) {
-        const unsigned long long pv =
-            ((unsigned long long)a.epoch << (64 - EPOCH_BITS)) | ((unsigned long long)j << 32) | slot;
-        uint32_t ps;
-        const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
-        if (r < 0) atomicOr(m.err, ERR_PAIR_TABLE_FULL);
-        is_new = r == 1;
-        if (is_new) {
-          owner = __ldcg(&m.table[slot].owner);
-          owned = owner != OWNER_PENDING;  // owned at entry (R9); pending = inserted by this call (R12)
+        // exactness of the (detection, key) pair: first toucher of the key in this call wins the slot's
+        // visit word; a second detection on the same key (object boundaries) uses the per-call pair set
+        const uint32_t mine = (a.epoch << 16) | j;
+        for (;;) {
+          if (visit == mine) break;                        // this pair was already counted
+          if ((visit >> 16) != a.epoch) {                  // nobody touched the key in this call yet
+            const uint32_t old = atomicCAS(&m.table[slot].visit, visit, mine);
+            if (old == visit) {
+              is_new = true;
+              break;
+            }
+            visit = old;
+            continue;
+          }
+          const unsigned long long pv = ((unsigned long long)mine << 32) | slot;
+          uint32_t ps;
+          const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
+          if (r < 0) atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+          is_new = r == 1;
+          break;
         }
+        owned = is_new && owner < OWNER_PENDING;  // owned at entry (R9); else inserted by this call (R12)
       }
     }
     const unsigned act = __ballot_sync(0xFFFFFFFFu, is_new);
@@ -387,14 +439,14 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
         // |V_d| += 1, aggregated over the lanes of the same detection
         const unsigned same = __match_any_sync(act, j);
         if (lane == __ffs(same) - 1) atomicAdd(&m.det_nv[j], (uint32_t)__popc(same));
-        if (!owned) atomicMin(&m.table[slot].claim, j);  // R12: lowest detection index wins
+        if (!owned) atomicMin(&m.table[slot].owner, OWNER_PENDING | j);  // R12: lowest detection index wins
       }
       // overlap histogram c[j][owner] += 1, aggregated over lanes with the same (j, owner)
       if (owned) {
         const unsigned long long jo = ((unsigned long long)j << 32) | owner;
         const unsigned same = __match_any_sync(oact, jo);
         if (lane == __ffs(same) - 1) {
-          const unsigned long long ov = ((unsigned long long)a.epoch << (64 - EPOCH_BITS)) | jo;
+          const unsigned long long ov = ((unsigned long long)a.epoch << 48) | jo;
           uint32_t os;
           const int r = epoch_insert(m.ov_keys, m.ov_mask, ov, a.epoch, &os);
           if (r < 0) {
@@ -412,22 +464,6 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
         }
       }
     }
-  }
-
-  // ---- flush the tile's per-detection accumulators and counters
-  if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
-    const uint32_t j = s.lab_j[tid];
-    atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
-      atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
-    }
-  }
-  if (tid == 0) {
-    if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
-    if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
-    if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
   }
 }
 
@@ -471,7 +507,8 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
     lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
   else
     lift_voxelise_kernel<false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
-  return 1;
+  probe_kernel<<<148 * 8, 256, 0, s>>>(m, a);
+  return 2;
 }
 
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K, const float *T,
