@@ -15,7 +15,8 @@ constexpr int TILE_W = 128;
 constexpr int TILE_H = 8;
 constexpr int LIFT_THREADS = 128;
 constexpr int TILE_PX = TILE_W * TILE_H;
-constexpr int TILE_HASH = 1024;  // slots of the direct-mapped tile filter
+constexpr int TILE_HASH = 512;   // slots of the direct-mapped tile filter
+constexpr int TILE_Q = 512;      // tile queue entries in shared memory; overflow goes straight to the global queue
 constexpr int MAX_LABELS = 32;   // per-tile detection accumulators
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
@@ -160,8 +161,8 @@ __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t ma
 
 struct TileSmem {
   unsigned long long tag[TILE_HASH];   // direct-mapped filter of (key, label) pairs already queued by this tile
-  unsigned long long qkey[TILE_PX];
-  uint32_t qj[TILE_PX];
+  unsigned long long qkey[TILE_Q];
+  uint32_t qj[TILE_Q];
   uint32_t lab_j[MAX_LABELS];
   uint32_t lab_cnt[MAX_LABELS];
   int lab_box[MAX_LABELS][6];
@@ -314,8 +315,18 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
       base = __shfl_sync(0xFFFFFFFFu, base, 0);
       if (fresh) {
         const uint32_t pos = base + __popc(b & ((1u << lane) - 1));
-        s.qkey[pos] = key;
-        s.qj[pos] = (uint32_t)det_base + l - 1;
+        if (pos < TILE_Q) {
+          s.qkey[pos] = key;
+          s.qj[pos] = (uint32_t)det_base + l - 1;
+        } else {  // rare: more distinct pairs in one tile than the shared queue holds
+          const uint32_t gp = atomicAdd(&m.counters[2], 1u);
+          if (gp < m.surv_cap) {
+            m.surv_key[gp] = key;
+            m.surv_j[gp] = (uint32_t)det_base + l - 1;
+          } else {
+            atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+          }
+        }
       }
     }
   }
@@ -348,7 +359,7 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
   __syncthreads();
 
   // ---- append the tile queue to the call's survivor queue (one global atomic per tile, coalesced copy)
-  const uint32_t nq = s.q_count;
+  const uint32_t nq = min(s.q_count, (uint32_t)TILE_Q);
   if (tid == 0 && nq) s.q_base = atomicAdd(&m.counters[2], nq);
   // ---- flush the tile's per-detection accumulators and counters
   if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {

@@ -243,3 +243,25 @@ def test_host_buffer_entry_point_matches_device_path(oracle):
         g.integrate_batch_host(1, depth, mask, K, T, np.ascontiguousarray(desc), n_det)
         compare_call(g, o)
     compare_maps(g, o)
+
+
+def test_tile_queue_overflow_every_pixel_its_own_voxel(oracle):
+    """Degenerate case: (almost) every pixel of a tile lands in its own voxel, more distinct pairs per tile
+    than the lift kernel's shared-memory queue holds (overflow goes straight to the global queue)."""
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.01, 8, 0.5, 0.5, 0.5, 0
+    H, W = 24, 256
+    g0 = np.random.default_rng(11)
+    o, g = make_pair(oracle, Cfg, H=H, W=W)
+    K = np.array([[100, 0, 128], [0, 100, 12], [0, 0, 1]], np.float32)
+    for it in range(2):
+        depth = (1.0 + 4.0 * g0.random((H, W))).astype(np.float32)
+        mask = np.ones((H, W), np.uint16)
+        mask[:, 128:] = 2
+        fr = S.Frame(depth, mask, K, np.eye(4, dtype=np.float32), unit_rows(2, 8, 5), 2, np.zeros(2, np.int64))
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+        _, _, _, st = g.last_assoc()
+        assert st["unique_voxels"] > 0.9 * H * W
+    compare_maps(g, o)
