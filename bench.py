@@ -133,6 +133,30 @@ def batch_host_arrays(frames):
     return depth, mask, K, T, desc, n_det
 
 
+# ------------------------------------------------------------------------------------------------ replicas
+def rank_seed(base_seed, rank):
+    """Replicas only: every rank owns an independent map fed by its own seeded stream."""
+    return int(base_seed) + int(rank)
+
+
+def reduce_over_ranks(x, op, world, device=None):
+    """max / sum of a host scalar over the ranks (timing and totals only -- there is no data-path collective)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def aggregate_throughput(frames_local, ms_local, world, device=None):
+    """whole-job value: frames of all ranks over the slowest rank's device time"""
+    total = reduce_over_ranks(float(frames_local), "sum", world, device)
+    ms = reduce_over_ranks(float(ms_local), "max", world, device)
+    return total / (ms * 1e-3), total, ms
+
+
 # ------------------------------------------------------------------------------------------------ ours
 def run_ours(args):
     import torch
@@ -151,7 +175,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     cfg = S.get_config(4)
     K_steps, W_steps = args.steps, args.warmup
-    sc, keys, owner, n_vox, desc = build_stress(args, seed_offset=rank)
+    sc, keys, owner, n_vox, desc = build_stress(args, seed_offset=rank_seed(0, rank))
     objs = object_records(binding.OBJECT_DTYPE, n_vox)
     N0 = len(objs)
     max_objects = N0 + (K_steps + W_steps + 1) * FRAMES_PER_BATCH * DET_PER_FRAME
@@ -174,18 +198,10 @@ def run_ours(args):
             dist.barrier()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(x, "max", world, dev)
 
     def sum_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(x, "sum", world, dev)
 
     # ---------------- device-resident run (value)
     m = new_map(2 if args.breakdown else 1)
@@ -217,7 +233,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     sampler.stop_flag = True
     barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1))
+    ms_local = e0.elapsed_time(e1)
     launches = m.kernel_launches() - launches0
     tot1 = m.sync()
     stage_ms, stage_launches = m.stage_times(reset=True)
@@ -225,9 +241,8 @@ def run_ours(args):
     frames = int(tot1["frames"] - tot0["frames"])
     points = int(tot1["valid_points"] - tot0["valid_points"])
     uniq = int(tot1["unique_voxels"] - tot0["unique_voxels"])
-    total_frames = sum_over_ranks(frames)
+    value, total_frames, ms = aggregate_throughput(frames, ms_local, world, dev)
     total_points = sum_over_ranks(points)
-    value = total_frames / (ms * 1e-3)
     del m, dev_batches
     torch.cuda.empty_cache()
 
