@@ -290,7 +290,7 @@ def run_ours(args):
     n_mean = n_before + (K_steps - 1) / (2.0 * K_steps) * (n_after - n_before)
     sim_flops = 2.0 * M * n_mean * cfg.D
     sim_ms = float(stage_ms[binding.STAGE_NAMES.index("similarity")]) / max(K_steps, 1)
-    lift_ms = float(stage_ms[binding.STAGE_NAMES.index("lift")]) / max(K_steps, 1)
+    lift_ms = float(stage_ms[binding.STAGE_NAMES.index("lift")] + stage_ms[binding.STAGE_NAMES.index("probe")]) / max(K_steps, 1)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     tinfo = json.load(open(tpath)) if os.path.exists(tpath) else {}
@@ -305,7 +305,7 @@ def run_ours(args):
     pairs = uniq / max(K_steps, 1)
     lift_bytes = px_bytes + pairs * (8 + 16)
     lift_gbs = lift_bytes / (lift_ms * 1e-3) / 1e9 if lift_ms > 0 else None
-    roofline_hbm = {"kernel": "lift_voxelise (steps 1-3)", "bound": "hbm", "achieved": lift_gbs, "peak": pk["hbm_gbs"],
+    roofline_hbm = {"kernel": "lift_voxelise + probe (steps 1-3)", "bound": "hbm", "achieved": lift_gbs, "peak": pk["hbm_gbs"],
                     "unit": "GB/s", "frac": (lift_gbs / pk["hbm_gbs"]) if lift_gbs else None,
                     "traffic": tinfo.get("lift_dram_bytes_per_launch"), "ms_per_launch": lift_ms, "bytes_per_launch": lift_bytes}
     step_bytes = px_bytes + M * cfg.D * 2 + n_mean * cfg.D * 2 + pairs * (8 + 16 + 16) + M * cfg.D * (4 + 4 + 2)

@@ -65,8 +65,9 @@ extern "C" {
 #define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
 #define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
 #define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
-#define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the lift and similarity kernels; 2 every kernel */
-#define FARM_OPT_OVERLAP 12          /* 1 (default): similarity runs on an internal side stream concurrently with lift */
+#define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around lift, probe and similarity; 2 every kernel      */
+#define FARM_OPT_OVERLAP 12          /* 1 (default): similarity on an internal side stream, concurrent with lift+probe;
+                                        0 one stream; 2 / 3 experimental orders (see farm_api.cu)                      */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -154,11 +155,11 @@ int farm_map_sync(farm_map *m, farm_totals *totals);
  * NULL.  Synchronises the stream. */
 #define FARM_N_STAGES 7
 #define FARM_STAGE_PREP 0        /* reset of per-call state + detection row norms            */
-#define FARM_STAGE_LIFT 1        /* steps 1-3: back-project, voxelise, dedupe, probe, overlap */
+#define FARM_STAGE_LIFT 1        /* steps 1-2: back-project, voxelise, tile-level dedupe       */
 #define FARM_STAGE_SIMILARITY 2  /* step 4: dense cosine with fused row max / argmax          */
-#define FARM_STAGE_CAND_SCORE 3  /* (unused: fused into ASSOCIATE)                            */
+#define FARM_STAGE_PROBE 3       /* step 3: voxel hash probe / insert, exact dedupe, overlap   */
 #define FARM_STAGE_ASSOCIATE 4   /* step 5a: candidate scores, argmax, threshold, new ids     */
-#define FARM_STAGE_COMMIT 5      /* (unused: fused into MERGE)                                */
+#define FARM_STAGE_UNUSED 5
 #define FARM_STAGE_MERGE 6       /* step 5b: voxel commit, descriptors, AABB, view evidence   */
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset);
 

@@ -21,7 +21,7 @@ OPT_MAX_DET_PER_CALL, OPT_STREAM, OPT_MAX_PAIRS_PER_CALL, OPT_MAX_FRAMES_PER_CAL
 OPT_TIMING = 11
 OPT_OVERLAP = 12
 N_STAGES = 7
-STAGE_NAMES = ["prep", "lift", "similarity", "cand_score", "associate", "commit", "merge"]
+STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "unused", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
 KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
 

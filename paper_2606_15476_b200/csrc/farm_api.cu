@@ -436,7 +436,7 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       m->sim_path = (int)v;
       break;
     case FARM_OPT_OVERLAP:
-      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad OVERLAP");
+      if (v < 0 || v > 3) return fail(FARM_ERR_INVALID_ARG, "bad OVERLAP");
       m->overlap = (int)v;
       break;
     case FARM_OPT_TIMING:
@@ -494,7 +494,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   cudaStream_t st = m->stream;
   bool launch_failed = false;
   auto stage = [&](int id, cudaStream_t st, auto &&fn) {
-    const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_SIMILARITY));
+    const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_PROBE || id == FARM_STAGE_SIMILARITY));
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (timed) {
       e0 = get_event(m), e1 = get_event(m);
@@ -510,20 +510,25 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
     }
   };
   // DAG of one call:  prep -> { similarity (side stream) || lift + probe } -> cand_score+associate -> commit+merge
+  // overlap modes: 1 = similarity || (lift, probe);  2 = similarity || lift, probe after the join;
+  //                3 = lift first, then similarity || probe
   const bool fork = m->overlap && m->side && a.M > 0 && m->n_upper > 0;
   cudaStream_t sim_stream = fork ? m->side : st;
   stage(FARM_STAGE_PREP, st, [&] { return launch_prep(d, a, st); });
+  if (fork && m->overlap == 3) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork) {
     cudaEventRecord(m->ev_fork, st);
     cudaStreamWaitEvent(m->side, m->ev_fork, 0);
   }
-  // similarity is enqueued first so that its one-CTA-per-SM grid is resident before the lift tiles fill the SMs
+  // similarity is enqueued first so that its one-CTA-per-SM grid is resident before the other kernels fill the SMs
   stage(FARM_STAGE_SIMILARITY, sim_stream, [&] {
     return m->tc ? launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc) : launch_similarity_fma(d, a, m->n_upper, sim_stream);
   });
   if (fork) cudaEventRecord(m->ev_join, m->side);
-  stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
-  if (fork) cudaStreamWaitEvent(st, m->ev_join, 0);
+  if (!(fork && m->overlap == 3)) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
+  if (fork && m->overlap == 2) cudaStreamWaitEvent(st, m->ev_join, 0);
+  stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st); });
+  if (fork && m->overlap != 2) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
   CU(cudaGetLastError());

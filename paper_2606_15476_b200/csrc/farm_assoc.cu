@@ -167,13 +167,15 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
 // CTAs [commit_blocks, ...): the lowest-index detection of every target object folds the whole group
 //   (R21 count-weighted descriptor mean, R22 AABB, R23 view evidence).  No atomics on the object, deterministic
 //   summation order.  Groups of one (the common case) skip the member scan.
+constexpr int MERGE_THREADS = 128, MERGE_WARPS = MERGE_THREADS / 32;
+
 template <typename T>
-__global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0,
+__global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0,
                                                            int commit_blocks) {
   extern __shared__ float acc[];  // [D]
-  __shared__ uint32_t list[256];
-  __shared__ uint32_t warp_cnt[8];
-  __shared__ float red[8];
+  __shared__ uint32_t list[MERGE_THREADS];
+  __shared__ uint32_t warp_cnt[MERGE_WARPS];
+  __shared__ float red[MERGE_WARPS];
   __shared__ float s_bcast;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if ((int)blockIdx.x < commit_blocks) {
@@ -217,14 +219,14 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
 #pragma unroll
       for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
     }
-    for (int i = tid; i < D; i += 256) acc[i] = 0.f;
+    for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = 0.f;
     uint32_t k_members = 0;
     unsigned long long pts = 0, best = 0;
     int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
     int best_frame = -1;
     __syncthreads();
     const int scan_end = group > 1 ? a.M : j + 1;  // a group of one is just the leader itself
-    for (int base = j & ~255; base < scan_end; base += 256) {  // members have index >= j
+    for (int base = j & ~(MERGE_THREADS - 1); base < scan_end; base += MERGE_THREADS) {  // members have index >= j
       const int jj = base + tid;
       const bool flag = jj < scan_end && jj >= j && m.assoc[jj] == t;
       const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
@@ -232,7 +234,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
       __syncthreads();
       uint32_t before = 0, total = 0;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) {
+      for (int w = 0; w < MERGE_WARPS; ++w) {
         before += w < warp ? warp_cnt[w] : 0;
         total += warp_cnt[w];
       }
@@ -242,7 +244,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
         const uint32_t jm = list[q];
         const float inv = m.det_inv_norm[jm];  // zero-norm rows contribute nothing (R21)
         const T *row = (const T *)a.desc + (size_t)jm * D;
-        for (int i = tid; i < D; i += 256) acc[i] = fmaf(to_f32<T>(row[i]), inv, acc[i]);
+        for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = fmaf(to_f32<T>(row[i]), inv, acc[i]);
         if (tid == 0) {
           k_members++;
           const uint32_t npx = m.det_npx[jm];
@@ -269,7 +271,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
     float *master = m.desc_master + (size_t)t * D;
     T *shadow = (T *)m.desc_shadow + (size_t)t * D;
     float ss = 0.f;
-    for (int i = tid; i < D; i += 256) {
+    for (int i = tid; i < D; i += MERGE_THREADS) {
       const float v = n_old ? fmaf((float)n_old, master[i], acc[i]) : acc[i];
       acc[i] = v;
       ss = fmaf(v, v, ss);
@@ -280,7 +282,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
     __syncthreads();
     if (tid == 0) {
       float tot = 0.f;
-      for (int w = 0; w < 8; ++w) tot += red[w];
+      for (int w = 0; w < MERGE_WARPS; ++w) tot += red[w];
       s_bcast = tot;
     }
     __syncthreads();
@@ -288,7 +290,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
     if (tot > 0.f) {  // a zero sum keeps the old value
       const float inv = 1.0f / sqrtf(tot);
       float s2 = 0.f;
-      for (int i = tid; i < D; i += 256) {
+      for (int i = tid; i < D; i += MERGE_THREADS) {
         const float v = acc[i] * inv;
         master[i] = v;
         const T sh = from_f32<T>(v);  // round-to-nearest-even shadow (R1, R14)
@@ -303,7 +305,7 @@ __global__ void __launch_bounds__(256) commit_merge_kernel(DevMap m, CallArgs a,
       __syncthreads();
       if (tid == 0) {
         float t2 = 0.f;
-        for (int w = 0; w < 8; ++w) t2 += red[w];
+        for (int w = 0; w < MERGE_WARPS; ++w) t2 += red[w];
         m.inv_norm[t] = t2 > 0.f ? 1.0f / sqrtf(t2) : 0.f;
       }
     }
@@ -343,9 +345,9 @@ int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
-  const int commit_blocks = 148 * 4;
-  const int merge_blocks = a.M < 148 * 8 ? a.M : 148 * 8;
-  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, 256, (size_t)m.D * sizeof(float), s>>>(
+  const int commit_blocks = 148 * 8;
+  const int merge_blocks = a.M < 148 * 16 ? a.M : 148 * 16;  // one CTA per detection: a single wave
+  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, MERGE_THREADS, (size_t)m.D * sizeof(float), s>>>(
       m, a, frame_seq0, commit_blocks)));
   return 1;
 }

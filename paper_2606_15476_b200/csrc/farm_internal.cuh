@@ -169,6 +169,7 @@ __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { retu
 // host-side launchers (one per translation unit); each returns the number of kernels it launched
 int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,
                              const float *T, int n_det, float *xyz, unsigned long long *keys, cudaStream_t s);
 int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);

@@ -212,31 +212,30 @@ __device__ __forceinline__ bool tile_filter_fresh(TileSmem &s, unsigned long lon
 // lift kernel (steps 1-2).  One 128x8 pixel tile per CTA; each thread owns 8 consecutive pixels of one row
 // (2 x 128-bit depth loads + 1 x 128-bit mask load).  Output: per-detection pixel counts and point boxes,
 // and the tile's distinct (detection, voxel key) pairs appended to the call's survivor queue.
+// raw registers of one thread's 8 pixels (2 x 128-bit depth + 1 x 128-bit mask)
+struct TileRegs {
+  float4 d0, d1;
+  uint4 mk;
+};
+
 template <bool VEC>
-__global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
-  __shared__ TileSmem s;
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int tile = blockIdx.x;
+__device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a, int tile, int tiles_x, int tiles_y, int tid) {
   const int f = tile / (tiles_x * tiles_y);
   const int trem = tile - f * tiles_x * tiles_y;
   const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
   const int v = ty * TILE_H + (tid >> 4);
   const int u0 = tx * TILE_W + (tid & 15) * 8;
-
-  // ---- issue the loads first (all independent), then initialise shared memory while they fly
-  float z[8];
-  uint32_t lab[8];
   const size_t frame_off = (size_t)f * m.H * m.W;
   const bool row_ok = v < m.H;
+  TileRegs r;
   if (VEC && row_ok && u0 + 7 < m.W) {
     const size_t off = frame_off + (size_t)v * m.W + u0;
-    const float4 d0 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off));
-    const float4 d1 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off + 4));
-    const uint4 mk = __ldcs(reinterpret_cast<const uint4 *>(a.mask + off));
-    z[0] = d0.x, z[1] = d0.y, z[2] = d0.z, z[3] = d0.w, z[4] = d1.x, z[5] = d1.y, z[6] = d1.z, z[7] = d1.w;
-    lab[0] = mk.x & 0xFFFF, lab[1] = mk.x >> 16, lab[2] = mk.y & 0xFFFF, lab[3] = mk.y >> 16;
-    lab[4] = mk.z & 0xFFFF, lab[5] = mk.z >> 16, lab[6] = mk.w & 0xFFFF, lab[7] = mk.w >> 16;
+    r.d0 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off));
+    r.d1 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off + 4));
+    r.mk = __ldcs(reinterpret_cast<const uint4 *>(a.mask + off));
   } else {
+    float z[8];
+    uint32_t lab[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const bool ok = row_ok && u0 + i < m.W;
@@ -244,7 +243,35 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
       lab[i] = ok ? (uint32_t)__ldcs(a.mask + off) : 0u;
       z[i] = ok ? __ldcs(a.depth + off) : 0.f;
     }
+    r.d0 = make_float4(z[0], z[1], z[2], z[3]);
+    r.d1 = make_float4(z[4], z[5], z[6], z[7]);
+    r.mk = make_uint4(lab[0] | (lab[1] << 16), lab[2] | (lab[3] << 16), lab[4] | (lab[5] << 16), lab[6] | (lab[7] << 16));
   }
+  return r;
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+  __shared__ TileSmem s;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int n_tiles = tiles_x * tiles_y * a.F;
+  // Each CTA walks tiles blockIdx.x, +gridDim.x, ...; the loads of the next tile are issued before the current
+  // one is processed (register double buffering), so DRAM latency hides even at two resident CTAs per SM.
+  TileRegs cur = load_tile<VEC>(m, a, blockIdx.x, tiles_x, tiles_y, tid);
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  TileRegs nxt = cur;
+  if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_y, tid);
+  const int f = tile / (tiles_x * tiles_y);
+  const int trem = tile - f * tiles_x * tiles_y;
+  const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
+  const int v = ty * TILE_H + (tid >> 4);
+  const int u0 = tx * TILE_W + (tid & 15) * 8;
+  float z[8];
+  uint32_t lab[8];
+  z[0] = cur.d0.x, z[1] = cur.d0.y, z[2] = cur.d0.z, z[3] = cur.d0.w;
+  z[4] = cur.d1.x, z[5] = cur.d1.y, z[6] = cur.d1.z, z[7] = cur.d1.w;
+  lab[0] = cur.mk.x & 0xFFFF, lab[1] = cur.mk.x >> 16, lab[2] = cur.mk.y & 0xFFFF, lab[3] = cur.mk.y >> 16;
+  lab[4] = cur.mk.z & 0xFFFF, lab[5] = cur.mk.z >> 16, lab[6] = cur.mk.w & 0xFFFF, lab[7] = cur.mk.w >> 16;
   for (int i = tid; i < TILE_HASH; i += LIFT_THREADS) s.tag[i] = KEY_EMPTY;
   if (tid < MAX_LABELS) {
     s.lab_j[tid] = NONE32;
@@ -376,7 +403,6 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
     if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
     if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
   }
-  if (nq == 0) return;
   __syncthreads();
   const uint32_t qb = s.q_base;
   for (uint32_t i = tid; i < nq; i += LIFT_THREADS) {
@@ -387,6 +413,9 @@ __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, C
     } else {
       atomicOr(m.err, ERR_PAIR_TABLE_FULL);
     }
+  }
+  __syncthreads();  // the tile's shared state is re-initialised by the next iteration
+  cur = nxt;
   }
 }
 
@@ -512,14 +541,19 @@ int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
-  const int grid = tiles_x * tiles_y * a.F;
+  const int n_tiles = tiles_x * tiles_y * a.F;
+  const int grid = n_tiles < 148 * 8 ? n_tiles : 148 * 8;
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
   if (vec)
     lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
   else
     lift_voxelise_kernel<false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  return 1;
+}
+
+int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   probe_kernel<<<148 * 8, 256, 0, s>>>(m, a);
-  return 2;
+  return 1;
 }
 
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K, const float *T,
