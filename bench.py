@@ -180,12 +180,14 @@ def run_ours(args):
     N0 = len(objs)
     max_objects = N0 + (K_steps + W_steps + 1) * FRAMES_PER_BATCH * DET_PER_FRAME
     max_voxels = int(len(keys) * 1.05) + (K_steps + W_steps + 1) * 600000
+    # 4x4x4 voxel blocks: this scene holds ~29 voxels per block (blobs are thick); sized for 16, +20k blocks per step
+    max_blocks = len(keys) // 16 + (K_steps + W_steps + 1) * 20000
 
     stream = torch.cuda.Stream(device=dev)
 
     def new_map(timing):
         m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
-                    max_objects=max_objects, max_voxels=max_voxels, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
+                    max_objects=max_objects, max_voxels=max_voxels, max_blocks=max_blocks, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
                     max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
                     timing=timing, overlap=args.overlap)
         m.import_(objs, desc, keys, owner)

@@ -57,7 +57,7 @@ extern "C" {
 /* integer options (farm_map_set_option_i); legal only before the first integrate / import / debug call */
 #define FARM_OPT_DESC_DTYPE 1        /* FARM_DTYPE_*, default F32                                              */
 #define FARM_OPT_MAX_OBJECTS 2       /* object capacity, default 65536                                         */
-#define FARM_OPT_MAX_VOXELS 3        /* owned-voxel capacity; table = next pow2 >= 2x, default 1<<22           */
+#define FARM_OPT_MAX_VOXELS 3        /* owned-voxel capacity, default 1<<22; sizes the block table unless MAX_BLOCKS is set */
 #define FARM_OPT_IMG_W 4             /* image width  (required)                                                */
 #define FARM_OPT_IMG_H 5             /* image height (required)                                                */
 #define FARM_OPT_MAX_DET_PER_CALL 6  /* sum of n_det over the frames of one call, default 4096, max 65535        */
@@ -68,6 +68,8 @@ extern "C" {
 #define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around lift, probe and similarity; 2 every kernel      */
 #define FARM_OPT_OVERLAP 12          /* 1 (default): similarity on an internal side stream, concurrent with lift+probe;
                                         0 one stream; 2 / 3 experimental orders (see farm_api.cu)                      */
+#define FARM_OPT_MAX_BLOCKS 13       /* capacity in 4x4x4 voxel blocks (256 B each); table = next pow2 >= 2x;
+                                        default MAX_VOXELS / 4.  Exceeding it sets the sticky capacity error           */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */

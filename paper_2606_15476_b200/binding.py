@@ -20,6 +20,7 @@ OPT_DESC_DTYPE, OPT_MAX_OBJECTS, OPT_MAX_VOXELS, OPT_IMG_W, OPT_IMG_H = 1, 2, 3,
 OPT_MAX_DET_PER_CALL, OPT_STREAM, OPT_MAX_PAIRS_PER_CALL, OPT_MAX_FRAMES_PER_CALL, OPT_SIM_PATH = 6, 7, 8, 9, 10
 OPT_TIMING = 11
 OPT_OVERLAP = 12
+OPT_MAX_BLOCKS = 13
 N_STAGES = 7
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "unused", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
@@ -105,7 +106,7 @@ class FarmMap:
     """farm_map_* with the same names and argument order as the C ABI."""
 
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
-                 max_voxels=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
+                 max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
                  stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
@@ -114,7 +115,7 @@ class FarmMap:
         self.set_option_i(OPT_IMG_H, H)
         self.set_option_i(OPT_IMG_W, W)
         self.set_option_i(OPT_DESC_DTYPE, dtype)
-        for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels),
+        for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels), (OPT_MAX_BLOCKS, max_blocks),
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
                        (OPT_TIMING, timing), (OPT_OVERLAP, overlap)):

@@ -34,7 +34,7 @@ static int fail(int code, const std::string &msg) {
 struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
-  long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16;
+  long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
   int sim_path = 0;
   cudaStream_t stream = 0;
   bool finalised = false;
@@ -166,69 +166,66 @@ __global__ void import_voxels_kernel(DevMap m, const unsigned long long *keys, c
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const unsigned long long key = keys[i];
     const uint32_t owner = owners[i];
-    if (owner >= n_objects || key == KEY_EMPTY) {
+    if (owner >= n_objects || (key >> 63)) {
       atomicOr(m.err, ERR_IMPORT_DUPLICATE);
       continue;
     }
-    unsigned long long h = voxel_hash(key) & m.table_mask;
-    bool done = false;
-    for (unsigned long long probe = 0; probe <= m.table_mask && probe < (1ull << 20); ++probe) {
-      unsigned long long k = m.table[h].key;
-      if (k == KEY_EMPTY) {
-        k = atomicCAS(&m.table[h].key, KEY_EMPTY, key);
-        if (k == KEY_EMPTY) {
-          m.table[h].owner = owner;
-          done = true;
-          break;
-        }
-      }
-      if (k == key) {
-        atomicOr(m.err, ERR_IMPORT_DUPLICATE);
-        done = true;
-        break;
-      }
-      h = (h + 1) & m.table_mask;
-    }
-    if (!done) atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
+    const uint32_t ix = (uint32_t)(key >> 42) & 0x1FFFFFu, iy = (uint32_t)(key >> 21) & 0x1FFFFFu, iz = (uint32_t)key & 0x1FFFFFu;
+    const uint32_t slot = block_find_or_insert(m, block_key(ix, iy, iz));
+    if (slot == 0xFFFFFFFFu) continue;  // table full: sticky error already set
+    const uint32_t old = atomicCAS(&m.blk_owner[(size_t)slot * BLK_VOXELS + block_bit(ix, iy, iz)], OWNER_INIT, owner);
+    if (old != OWNER_INIT) atomicOr(m.err, ERR_IMPORT_DUPLICATE);
   }
 }
 
-__global__ void clear_visit_kernel(DevMap m) {
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
-       i += (unsigned long long)gridDim.x * blockDim.x)
-    m.table[i].visit = 0xFFFFFFFFu;
-}
-
+// one thread per (block slot, 32-byte owner sector)
 __global__ void count_voxels_kernel(DevMap m, unsigned long long *count) {
   unsigned long long c = 0;
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
-       i += (unsigned long long)gridDim.x * blockDim.x)
-    c += m.table[i].key != KEY_EMPTY;
+  const unsigned long long n = ((unsigned long long)m.table_mask + 1) * 8;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    if (m.blk_key[i >> 3] == BLK_EMPTY) continue;
+    const uint4 *p = reinterpret_cast<const uint4 *>(m.blk_owner + i * 8);
+    const uint4 w0 = p[0], w1 = p[1];
+    c += (w0.x != OWNER_INIT) + (w0.y != OWNER_INIT) + (w0.z != OWNER_INIT) + (w0.w != OWNER_INIT) + (w1.x != OWNER_INIT) +
+         (w1.y != OWNER_INIT) + (w1.z != OWNER_INIT) + (w1.w != OWNER_INIT);
+  }
   for (int s = 16; s; s >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, s);
   if ((threadIdx.x & 31) == 0 && c) atomicAdd(count, c);
 }
 
 __global__ void export_voxels_kernel(DevMap m, unsigned long long *keys, uint32_t *owners, unsigned long long *cursor,
                                      unsigned long long cap) {
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i <= m.table_mask;
+  const unsigned long long n = ((unsigned long long)m.table_mask + 1) * 8;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n;
        i += (unsigned long long)gridDim.x * blockDim.x) {
-    const VoxelSlot sl = m.table[i];
-    if (sl.key != KEY_EMPTY) {
-      const unsigned long long p = atomicAdd(cursor, 1ull);
-      if (p < cap) {
-        keys[p] = sl.key;
-        owners[p] = sl.owner;
+    const unsigned long long bkey = m.blk_key[i >> 3];
+    if (bkey == BLK_EMPTY) continue;
+    const uint4 *p = reinterpret_cast<const uint4 *>(m.blk_owner + i * 8);
+    const uint4 w0 = p[0], w1 = p[1];
+    const uint32_t own[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) cnt += own[b] != OWNER_INIT;
+    if (!cnt) continue;
+    unsigned long long pos = atomicAdd(cursor, (unsigned long long)cnt);
+#pragma unroll
+    for (int b = 0; b < 8; ++b)
+      if (own[b] != OWNER_INIT) {
+        if (pos < cap) {
+          keys[pos] = voxel_key_of(bkey, (uint32_t)(i & 7) * 8 + b);
+          owners[pos] = own[b];
+        }
+        ++pos;
       }
-    }
   }
 }
 
-__global__ void gather_pairs_kernel(DevMap m, uint32_t n, uint32_t *js, unsigned long long *keys) {
+// debug read: block key of every event of the last call
+__global__ void gather_events_kernel(DevMap m, uint32_t n, unsigned long long *bkeys) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const unsigned long long p = m.pair_list[i];
-  js[i] = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
-  keys[i] = m.table[(uint32_t)p].key;
+  bkeys[i] = m.blk_key[m.pl_slot[i]];
 }
 
 long long next_pow2(long long x) {
@@ -254,6 +251,8 @@ int finalise(farm_map *m) {
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
     return fail(FARM_ERR_CUDA, "no CUDA device: the FARM mapping path has no CPU fallback");
+  if (m->max_blocks <= 0) m->max_blocks = std::max<long long>(m->max_voxels / 4, 1024);
+  if (m->max_blocks > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "voxel-block table too large (FARM_OPT_MAX_BLOCKS <= 2^30)");
   if (m->max_pairs <= 0) m->max_pairs = std::min<long long>((long long)m->H * m->W * std::min<long long>(m->max_frames, 4), 1ll << 23);
   DevMap &d = m->dm;
   d.inv_vs = 1.0f / m->voxel_size;  // R6: fp32 reciprocal, computed once
@@ -280,13 +279,18 @@ int finalise(farm_map *m) {
   A(d.best_cam, NO * 3, 0);
   A(d.leader, NO, 0xFF);
   A(d.grp_cnt, NO, 0);
-  const long long tcap = next_pow2(std::max<long long>(2 * m->max_voxels, 1024));
-  A(d.table, (size_t)tcap, 0xFF);  // key = EMPTY, owner = OWNER_INIT, visit = dead epoch 0xFFFF
-  d.table_mask = (unsigned long long)tcap - 1;
+  const long long tcap = next_pow2(std::max<long long>(2 * m->max_blocks, 1024));
+  A(d.blk_key, (size_t)tcap, 0xFF);                 // BLK_EMPTY
+  A(d.blk_owner, (size_t)tcap * BLK_VOXELS, 0xFF);  // OWNER_INIT
+  d.table_mask = (uint32_t)(tcap - 1);
   const long long pcap = next_pow2(2 * m->max_pairs);
   A(d.pair_set, (size_t)pcap, 0);
+  A(d.pair_bits, (size_t)pcap, 0);
   d.pair_mask = (uint32_t)(pcap - 1);
-  A(d.pair_list, (size_t)m->max_pairs, 0);
+  A(d.pl_bits, (size_t)m->max_pairs, 0);
+  A(d.pl_slot, (size_t)m->max_pairs, 0);
+  A(d.pl_j, (size_t)m->max_pairs, 0);
+  A(d.pl_ps, (size_t)m->max_pairs, 0);
   d.pair_cap = (uint32_t)m->max_pairs;
   const long long ccap = std::min<long long>(std::max<long long>(m->max_pairs / 4, 16384), 1ll << 22);
   const long long ocap = next_pow2(2 * ccap);
@@ -300,6 +304,7 @@ int finalise(farm_map *m) {
   d.cand_cap = (uint32_t)ccap;
   const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30);
   A(d.surv_key, (size_t)scap, 0);
+  A(d.surv_bits, (size_t)scap, 0);
   A(d.surv_j, (size_t)scap, 0);
   d.surv_cap = (uint32_t)scap;
   A(d.counters, 4, 0);
@@ -427,6 +432,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 1024 || v > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_PAIRS_PER_CALL");
       m->max_pairs = v;
       break;
+    case FARM_OPT_MAX_BLOCKS:
+      if (v < 1 || v > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "bad MAX_BLOCKS");
+      m->max_blocks = v;
+      break;
     case FARM_OPT_MAX_FRAMES_PER_CALL:
       if (v < 1 || v > MAX_FRAMES) return fail(FARM_ERR_INVALID_ARG, "bad MAX_FRAMES_PER_CALL");
       m->max_frames = v;
@@ -480,11 +489,9 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (M > 0 && !desc) return fail(FARM_ERR_INVALID_ARG, "det_descriptors is NULL");
   int rc = finalise(m);
   if (rc != FARM_OK) return rc;
-  if (m->epoch == EPOCH_MAX - 1) {  // the 16-bit epoch tag wraps: clear every epoch-tagged word once per 65534 calls
+  if (m->epoch == EPOCH_MAX - 1) {  // the 16-bit epoch tag wraps: clear the epoch-tagged tables once per 65534 calls
     CU(cudaMemsetAsync(m->dm.pair_set, 0, ((size_t)m->dm.pair_mask + 1) * 8, m->stream));
     CU(cudaMemsetAsync(m->dm.ov_keys, 0, ((size_t)m->dm.ov_mask + 1) * 8, m->stream));
-    clear_visit_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm);
-    m->launches++;
     m->epoch = 0;
   }
   a.M = (int)M;
@@ -749,32 +756,35 @@ int farm_debug_last_voxels(farm_map *m, long long *offsets, uint64_t *keys, uint
   int rc = device_error(m);
   if (rc != FARM_OK) return rc;
   const int M = m->last_M;
-  uint32_t n = 0;
+  uint32_t n = 0;  // events (detection, block, new voxel bits) of the last call
   CU(cudaMemcpy(&n, m->dm.counters, 4, cudaMemcpyDeviceToHost));
+  n = std::min(n, m->dm.pair_cap);
   std::vector<uint32_t> js(n);
-  std::vector<unsigned long long> ks(n);
+  std::vector<unsigned long long> bks(n), bits(n);
   if (n) {
-    uint32_t *dj;
     unsigned long long *dk;
-    CU(cudaMalloc(&dj, (size_t)n * 4));
     CU(cudaMalloc(&dk, (size_t)n * 8));
-    gather_pairs_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->dm, n, dj, dk);
+    gather_events_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->dm, n, dk);
     m->launches++;
-    CU(cudaMemcpyAsync(js.data(), dj, (size_t)n * 4, cudaMemcpyDeviceToHost, m->stream));
-    CU(cudaMemcpyAsync(ks.data(), dk, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaMemcpyAsync(bks.data(), dk, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaMemcpyAsync(js.data(), m->dm.pl_j, (size_t)n * 4, cudaMemcpyDeviceToHost, m->stream));
+    CU(cudaMemcpyAsync(bits.data(), m->dm.pl_bits, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream));
     CU(cudaStreamSynchronize(m->stream));
-    cudaFree(dj);
     cudaFree(dk);
   }
   std::vector<long long> cnt(M + 1, 0);
-  for (uint32_t i = 0; i < n; ++i)
-    if ((int)js[i] < M) cnt[js[i] + 1]++;
+  for (uint32_t i = 0; i < n; ++i) {
+    js[i] &= 0x7FFFFFFFu;
+    if ((int)js[i] < M) cnt[js[i] + 1] += __builtin_popcountll(bits[i]);
+  }
   for (int j = 0; j < M; ++j) cnt[j + 1] += cnt[j];
   for (int j = 0; j <= M; ++j) offsets[j] = cnt[j];
   if (keys) {
     std::vector<long long> cur(cnt.begin(), cnt.end() - 1);
     for (uint32_t i = 0; i < n; ++i)
-      if ((int)js[i] < M) keys[cur[js[i]]++] = ks[i];
+      if ((int)js[i] < M)
+        for (unsigned long long w = bits[i]; w; w &= w - 1)
+          keys[cur[js[i]]++] = voxel_key_of(bks[i], (uint32_t)__builtin_ctzll(w));
   }
   if (n_px && M) CU(cudaMemcpy(n_px, m->dm.det_npx, (size_t)M * 4, cudaMemcpyDeviceToHost));
   if (box && M) {

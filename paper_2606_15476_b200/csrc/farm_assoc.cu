@@ -18,6 +18,7 @@ template <typename T>
 __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs a) {
   __shared__ uint32_t warp_sum[32];
   __shared__ uint32_t s_running, s_matches, s_skipped;
+  __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   {
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     const uint32_t t = atomicAdd(&m.counters[3], 1u);
     s_last = t == gridDim.x - 1;
     if (s_last) m.counters[3] = 0;
-    s_running = 0, s_matches = 0, s_skipped = 0;
+    s_running = 0, s_matches = 0, s_skipped = 0, s_uvox = 0ull;
   }
   __syncthreads();
   if (!s_last) return;
@@ -84,6 +85,8 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     uint32_t spawn = 0, matched = 0, skipped = 0;
     int32_t target = -1;
     float score = 0.f;
+    const uint32_t nv = __reduce_add_sync(0xFFFFFFFFu, j < a.M ? __ldcg(&m.det_nv[j]) : 0u);
+    if (lane == 0 && nv) atomicAdd(&s_uvox, (unsigned long long)nv);
     if (j < a.M) {
       if (__ldcg(&m.det_npx[j]) == 0) {
         skipped = 1;  // R8
@@ -147,7 +150,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
   if (tid == 0) {
     uint32_t spawns = s_running;
     if (N + spawns > m.max_objects) spawns = m.max_objects - N;
-    const uint32_t pairs = __ldcg(&m.counters[0]);
+    const unsigned long long pairs = s_uvox;
     *m.n_objects = N + spawns;
     m.stats->matches = s_matches;
     m.stats->spawns = spawns;
@@ -156,7 +159,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     atomicAdd(&m.totals->frames, (unsigned long long)a.F);
     atomicAdd(&m.totals->calls, 1ull);
     atomicAdd(&m.totals->valid_points, valid_points);
-    atomicAdd(&m.totals->unique_voxels, (unsigned long long)pairs);
+    atomicAdd(&m.totals->unique_voxels, pairs);
     atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
     atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
   }
@@ -179,25 +182,40 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   __shared__ float s_bcast;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if ((int)blockIdx.x < commit_blocks) {
+    // 8 lanes per event (one 32-byte owner sector each), 4 events per warp and step
     const uint32_t n = min(m.counters[0], m.pair_cap);
-    for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < n; i0 += commit_blocks * blockDim.x) {
-      const uint32_t i = i0 + lane;
+    const int sec = lane & 7;
+    const uint32_t step = (uint32_t)commit_blocks * MERGE_WARPS * 4;
+    for (uint32_t e0 = (blockIdx.x * MERGE_WARPS + warp) * 4; e0 < n; e0 += step) {
+      const uint32_t e = e0 + (lane >> 3);
       int32_t t = -1;
-      if (i < n) {
-        const unsigned long long p = m.pair_list[i];
-        if (p >> 63) {
-          const uint32_t j = (uint32_t)(p >> 32) & ((1u << DET_BITS) - 1);
-          const uint32_t slot = (uint32_t)p;
-          if (m.table[slot].owner == (OWNER_PENDING | j)) {  // this detection holds the claim (R12)
-            t = m.assoc[j];
-            if (t >= 0) m.table[slot].owner = (uint32_t)t;
+      uint32_t cnt = 0;
+      if (e < n) {
+        const uint32_t jp = m.pl_j[e];
+        if (sec == 0) m.pair_bits[m.pl_ps[e]] = 0ull;  // invariant: the pair set's voxel bits are zero between calls
+        const uint32_t byte = (uint32_t)(m.pl_bits[e] >> (8 * sec)) & 0xFFu;
+        if ((jp >> 31) && byte) {  // some voxel of the event was unowned at entry
+          const uint32_t j = jp & 0x7FFFFFFFu;
+          t = m.assoc[j];
+          uint32_t *base = m.blk_owner + (size_t)m.pl_slot[e] * BLK_VOXELS + sec * 8;
+          const uint4 w0 = __ldcg(reinterpret_cast<const uint4 *>(base));
+          const uint4 w1 = __ldcg(reinterpret_cast<const uint4 *>(base) + 1);
+          const uint32_t own[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+          if (t >= 0) {
+#pragma unroll
+            for (int b = 0; b < 8; ++b)
+              if (((byte >> b) & 1u) && own[b] == (OWNER_PENDING | j)) {  // this detection holds the claim (R12)
+                base[b] = (uint32_t)t;
+                cnt++;
+              }
           }
         }
       }
-      const unsigned act = __ballot_sync(0xFFFFFFFFu, t >= 0);
-      if (t >= 0) {
+      const unsigned act = __ballot_sync(0xFFFFFFFFu, cnt != 0);
+      if (cnt) {
         const unsigned same = __match_any_sync(act, t);
-        if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], (uint32_t)__popc(same));
+        const uint32_t tot = __reduce_add_sync(same, cnt);
+        if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], tot);
       }
     }
     return;

@@ -26,15 +26,29 @@ constexpr uint32_t ERR_OVERLAP_TABLE_FULL = 4u;
 constexpr uint32_t ERR_OBJECT_CAPACITY = 8u;
 constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
 
-// Global voxel -> object hash slot (R11: one owner per key).  16 bytes, one 32-byte sector per probe.
-struct __align__(16) VoxelSlot {
-  unsigned long long key;  // KEY_EMPTY when free
-  uint32_t owner;          // object id; while the inserting call runs: OWNER_PENDING | lowest detection index j
-                           // of that call containing the key (R12: that detection's object will own it)
-  uint32_t visit;          // (epoch << 16 | j) of the first detection that touched the key in the current call:
-                           // makes (detection, key) pairs exact without a second random access; other
-                           // detections of the same call fall back to the per-call pair set
-};
+// Global voxel -> object hash (R11: one owner per key), stored as a hash of 4x4x4 VOXEL BLOCKS so that the
+// voxels of one surface patch share DRAM lines:
+//   blk_key[slot]        57-bit block key (bx<<38 | by<<19 | bz, b = biased voxel index >> 2), BLK_EMPTY when free;
+//                        8 bytes per slot: the whole key array of a 1e8-voxel map fits in L2
+//   blk_owner[slot][64]  owner of voxel (lx<<4 | ly<<2 | lz) of the block: object id, OWNER_INIT = unowned;
+//                        while the inserting call runs: OWNER_PENDING | lowest detection index j of that call
+//                        containing the voxel (R12: that detection's object will own it).  256 bytes per block.
+constexpr unsigned long long BLK_EMPTY = 0xFFFFFFFFFFFFFFFFull;
+constexpr int BLK_VOXELS = 64;
+
+__host__ __device__ __forceinline__ unsigned long long block_key(uint32_t ix, uint32_t iy, uint32_t iz) {
+  return ((unsigned long long)(ix >> 2) << 38) | ((unsigned long long)(iy >> 2) << 19) | (unsigned long long)(iz >> 2);
+}
+__host__ __device__ __forceinline__ uint32_t block_bit(uint32_t ix, uint32_t iy, uint32_t iz) {
+  return ((ix & 3u) << 4) | ((iy & 3u) << 2) | (iz & 3u);
+}
+// voxel key (R6 packing) of voxel `bit` of block `bkey`
+__host__ __device__ __forceinline__ unsigned long long voxel_key_of(unsigned long long bkey, uint32_t bit) {
+  const unsigned long long ix = (((bkey >> 38) & 0x7FFFFull) << 2) | ((bit >> 4) & 3u);
+  const unsigned long long iy = (((bkey >> 19) & 0x7FFFFull) << 2) | ((bit >> 2) & 3u);
+  const unsigned long long iz = ((bkey & 0x7FFFFull) << 2) | (bit & 3u);
+  return (ix << 42) | (iy << 21) | iz;
+}
 
 struct CallStats {  // device mirror of farm_frame_stats
   unsigned long long valid_points, dropped_points, ignored_pixels, unique_voxels;
@@ -62,13 +76,16 @@ struct DevMap {
   float *best_cam;                   // [max_objects,3]
   uint32_t *leader;                  // scratch: lowest j of the call that targets the object
   uint32_t *grp_cnt;                 // scratch: number of detections of the call that target the object
-  // voxel hash
-  VoxelSlot *table;
-  unsigned long long table_mask;     // capacity-1
+  // voxel-block hash
+  unsigned long long *blk_key;       // [table_mask+1]
+  uint32_t *blk_owner;               // [table_mask+1][64]
+  uint32_t table_mask;               // capacity-1 (capacity is a power of two <= 2^31)
   // per-call scratch
-  unsigned long long *pair_set;      // epoch-tagged set of (j, slot)
+  unsigned long long *pair_set;      // epoch-tagged map (epoch, j, block slot) -> pair_bits: voxels of the block
+  unsigned long long *pair_bits;     //   already counted for detection j in this call (zero between calls)
   uint32_t pair_mask;
-  unsigned long long *pair_list;     // unique (pending<<63 | j<<32 | slot)
+  unsigned long long *pl_bits;       // event list: the voxels `bits` of block `slot` are new for detection j
+  uint32_t *pl_slot, *pl_j, *pl_ps;  //   pl_j = j | (1u<<31 when some voxel was unowned at entry), pl_ps = pair-set slot
   uint32_t pair_cap;
   unsigned long long *ov_keys;       // epoch-tagged map (j, owner) -> count
   uint32_t *ov_cnt;
@@ -78,10 +95,11 @@ struct DevMap {
   uint32_t *cand_j;                  // compact copy for the debug read
   int32_t *cand_o;
   uint32_t *cand_c;
-  unsigned long long *surv_key;      // survivor queue of the lift kernel: (key, j) after tile-level dedupe
+  unsigned long long *surv_key;      // survivor queue of the lift kernel: (block key, voxel bits, j) after the
+  unsigned long long *surv_bits;     //   tile-level aggregation
   uint32_t *surv_j;
   uint32_t surv_cap;
-  uint32_t *counters;                // [0]=pair_count [1]=cand_count [2]=survivor_count [3]=block ticket
+  uint32_t *counters;                // [0]=event_count [1]=cand_count [2]=survivor_count [3]=block ticket
   // per detection [max_det]
   uint32_t max_det;
   uint32_t *det_nv, *det_npx;
@@ -146,7 +164,24 @@ __device__ __forceinline__ uint32_t hash32(uint32_t a, uint32_t b) {
   h ^= h >> 15;
   return h;
 }
-__device__ __forceinline__ uint32_t voxel_hash(unsigned long long key) { return hash32((uint32_t)key, (uint32_t)(key >> 32)); }
+__device__ __forceinline__ uint32_t block_hash(unsigned long long bkey) { return hash32((uint32_t)bkey, (uint32_t)(bkey >> 32)); }
+
+// find-or-insert a block key; returns the slot (0xFFFFFFFF when the table is full).  The owners of a fresh slot
+// are all OWNER_INIT already (the payload of a free slot is never written).
+__device__ __forceinline__ uint32_t block_find_or_insert(const DevMap &m, unsigned long long bkey) {
+  uint32_t h = block_hash(bkey) & m.table_mask;
+  for (int probe = 0; probe < 8192; ++probe) {
+    unsigned long long k = __ldcg(&m.blk_key[h]);
+    if (k == BLK_EMPTY) {
+      k = atomicCAS(&m.blk_key[h], BLK_EMPTY, bkey);
+      if (k == BLK_EMPTY) k = bkey;
+    }
+    if (k == bkey) return h;
+    h = (h + 1) & m.table_mask;
+  }
+  atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
+  return 0xFFFFFFFFu;
+}
 
 template <typename T>
 __device__ __forceinline__ float to_f32(T v);

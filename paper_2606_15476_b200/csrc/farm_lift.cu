@@ -1,23 +1,24 @@
-// farm_lift.cu -- steps 1-3 of the hot path in one pass over the images:
-//   back-project masked pixels (R5), quantise to voxel keys (R6), per-detection dedupe (R7),
-//   probe / insert the global voxel->object hash (R11, R12 pass 1) and build the sparse overlap
-//   histogram (R9).  BASELINE.json north_star steps (1)-(3); PAPER.md:65, 347 ("masked depth points").
+// farm_lift.cu -- steps 1-3 of the hot path:
+//   lift_voxelise_kernel  back-project masked pixels (R5), quantise to voxel keys (R6), aggregate the keys of
+//                         a pixel tile per (detection, 4x4x4 voxel block) into 64-bit voxel masks (R7)
+//   probe_kernel          find / insert the blocks in the global voxel-block hash (R11, R12 pass 1), make the
+//                         (detection, voxel) pairs exact and build the sparse overlap histogram (R9)
+// BASELINE.json north_star steps (1)-(3); PAPER.md:65, 347 ("masked depth points").
 //
-// HBM-bound by design: the only mandatory traffic is 6 B/pixel of depth+mask (128-bit loads) plus one
-// 32-byte sector per distinct (detection, voxel) pair that survives the shared-memory tile dedupe.
+// The mandatory traffic is 6 B/pixel of depth+mask (128-bit loads) plus, per distinct (detection, block)
+// pair, one 8-byte key probe and the 32-byte owner sectors of the voxels the detection touches.
 #include "farm_internal.cuh"
 
 namespace farm {
 
 namespace {
 
-constexpr int TILE_W = 128;
-constexpr int TILE_H = 8;
+constexpr int TILE_W = 64;        // 8 threads x 8 pixels per row
+constexpr int TILE_H = 16;
 constexpr int LIFT_THREADS = 128;
-constexpr int TILE_PX = TILE_W * TILE_H;
-constexpr int TILE_HASH = 512;   // slots of the direct-mapped tile filter
-constexpr int TILE_Q = 512;      // tile queue entries in shared memory; overflow goes straight to the global queue
-constexpr int MAX_LABELS = 32;   // per-tile detection accumulators
+constexpr int TILE_ENT = 256;     // (detection, block) entries per tile; overflow goes straight to the global queue
+constexpr int MAX_LABELS = 32;    // per-tile detection accumulators (the entry tag holds a 5-bit label slot)
+constexpr int LABEL_SHIFT = 57;   // block keys use bits 0..56
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
 struct Camera {
@@ -56,12 +57,16 @@ __device__ __forceinline__ void backproject(const Camera &c, int u, int v, float
 // R6: index = floor(fp32(X * inv_vs)) per axis, valid iff in [-2^20, 2^20).  cvt.rmi (round towards -inf,
 // saturating) is floor-then-convert in one instruction; the float pre-test rejects NaN and anything the
 // saturation would alias.
-__device__ __forceinline__ bool voxel_key(const float p[3], float inv_vs, unsigned long long *key) {
+__device__ __forceinline__ bool voxel_index(const float p[3], float inv_vs, uint32_t &ix, uint32_t &iy, uint32_t &iz) {
   const float fx = __fmul_rn(p[0], inv_vs), fy = __fmul_rn(p[1], inv_vs), fz = __fmul_rn(p[2], inv_vs);
   const bool finite = fabsf(fx) < 2.0e6f && fabsf(fy) < 2.0e6f && fabsf(fz) < 2.0e6f;
-  const uint32_t ix = (uint32_t)(__float2int_rd(fx) + KEY_BIAS), iy = (uint32_t)(__float2int_rd(fy) + KEY_BIAS),
-                 iz = (uint32_t)(__float2int_rd(fz) + KEY_BIAS);
-  if (!finite || ((ix | iy | iz) >> 21) != 0) return false;
+  ix = (uint32_t)(__float2int_rd(fx) + KEY_BIAS), iy = (uint32_t)(__float2int_rd(fy) + KEY_BIAS),
+  iz = (uint32_t)(__float2int_rd(fz) + KEY_BIAS);
+  return finite && ((ix | iy | iz) >> 21) == 0;
+}
+__device__ __forceinline__ bool voxel_key(const float p[3], float inv_vs, unsigned long long *key) {
+  uint32_t ix, iy, iz;
+  if (!voxel_index(p, inv_vs, ix, iy, iz)) return false;
   const uint32_t lo = iz | (iy << 21), hi = (iy >> 11) | (ix << 10);
   *key = ((unsigned long long)hi << 32) | lo;
   return true;
@@ -107,31 +112,9 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
   if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
 }
 
-// ---------------------------------------------------------------------------------------------------
-// global structures
 
-// find-or-insert `key` in the voxel table with one 16-byte probe per slot; returns the slot index (NONE32 when the
-// table is full) and the slot's owner / visit words as loaded (free slots hold OWNER_INIT / a dead epoch).
-__device__ __forceinline__ uint32_t voxel_find_or_insert(const DevMap &m, unsigned long long key, uint32_t *owner,
-                                                         uint32_t *visit) {
-  unsigned long long h = voxel_hash(key) & m.table_mask;
-  for (int probe = 0; probe < 8192; ++probe) {
-    const uint4 w = __ldcg(reinterpret_cast<const uint4 *>(&m.table[h]));
-    unsigned long long k = ((unsigned long long)w.y << 32) | w.x;
-    if (k == KEY_EMPTY) {
-      k = atomicCAS(&m.table[h].key, KEY_EMPTY, key);
-      if (k == KEY_EMPTY) k = key;  // inserted: owner == OWNER_INIT already
-    }
-    if (k == key) {
-      *owner = w.z;
-      *visit = w.w;
-      return (uint32_t)h;
-    }
-    h = (h + 1) & m.table_mask;
-  }
-  atomicOr(m.err, ERR_VOXEL_TABLE_FULL);
-  return NONE32;
-}
+// ---------------------------------------------------------------------------------------------------
+// per-call scratch helpers
 
 // epoch-tagged set/map insert: entries whose epoch field differs from `epoch` count as free.
 // returns 1 = newly inserted, 0 = already present, -1 = table full.
@@ -159,10 +142,21 @@ __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t ma
   return -1;
 }
 
+// append one (block, detection, voxel bits) record to the call's survivor queue
+__device__ __forceinline__ void survivor_store(const DevMap &m, uint32_t pos, unsigned long long bkey, uint32_t j,
+                                               uint32_t lo, uint32_t hi) {
+  if (pos < m.surv_cap) {
+    m.surv_key[pos] = bkey;
+    m.surv_bits[pos] = ((unsigned long long)hi << 32) | lo;
+    m.surv_j[pos] = j;
+  } else {
+    atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+  }
+}
+
 struct TileSmem {
-  unsigned long long tag[TILE_HASH];   // direct-mapped filter of (key, label) pairs already queued by this tile
-  unsigned long long qkey[TILE_Q];
-  uint32_t qj[TILE_Q];
+  unsigned long long tag[TILE_ENT];  // block key | label slot << 57, BLK_EMPTY when free
+  uint32_t mlo[TILE_ENT], mhi[TILE_ENT];  // voxel bits of the block seen for that detection inside the tile
   uint32_t lab_j[MAX_LABELS];
   uint32_t lab_cnt[MAX_LABELS];
   int lab_box[MAX_LABELS][6];
@@ -170,9 +164,8 @@ struct TileSmem {
   uint32_t n_valid, n_dropped, n_ignored;
 };
 
-// accumulate a run (j, cnt, box as ordered ints) into the tile's per-detection accumulators
-__device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32_t j, uint32_t cnt, int mn0, int mn1,
-                                            int mn2, int mx0, int mx1, int mx2) {
+// slot of detection j in the tile's label table (-1 when more than MAX_LABELS detections meet in one tile)
+__device__ __forceinline__ int tile_label_slot(TileSmem &s, uint32_t j) {
   uint32_t h = j % MAX_LABELS;
   for (int probe = 0; probe < MAX_LABELS; ++probe) {
     uint32_t l = *(volatile uint32_t *)&s.lab_j[h];
@@ -180,38 +173,51 @@ __device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, uint32
       l = atomicCAS(&s.lab_j[h], NONE32, j);
       if (l == NONE32) l = j;
     }
-    if (l == j) {
-      atomicAdd(&s.lab_cnt[h], cnt);
-      atomicMin(&s.lab_box[h][0], mn0), atomicMin(&s.lab_box[h][1], mn1), atomicMin(&s.lab_box[h][2], mn2);
-      atomicMax(&s.lab_box[h][3], mx0), atomicMax(&s.lab_box[h][4], mx1), atomicMax(&s.lab_box[h][5], mx2);
-      return;
-    }
+    if (l == j) return (int)h;
     h = (h + 1) % MAX_LABELS;
   }
-  // more than MAX_LABELS detections inside one tile: go to global memory directly
+  return -1;
+}
+
+// accumulate a run (cnt pixels, box as ordered ints) of detection j into the tile's per-detection accumulators
+__device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, int li, uint32_t j, uint32_t cnt, int mn0,
+                                            int mn1, int mn2, int mx0, int mx1, int mx2) {
+  if (li >= 0) {
+    atomicAdd(&s.lab_cnt[li], cnt);
+    atomicMin(&s.lab_box[li][0], mn0), atomicMin(&s.lab_box[li][1], mn1), atomicMin(&s.lab_box[li][2], mn2);
+    atomicMax(&s.lab_box[li][3], mx0), atomicMax(&s.lab_box[li][4], mx1), atomicMax(&s.lab_box[li][5], mx2);
+    return;
+  }
   atomicAdd(&m.det_npx[j], cnt);
   atomicMin(&m.det_box[j * 6 + 0], mn0), atomicMin(&m.det_box[j * 6 + 1], mn1), atomicMin(&m.det_box[j * 6 + 2], mn2);
   atomicMax(&m.det_box[j * 6 + 3], mx0), atomicMax(&m.det_box[j * 6 + 4], mx1), atomicMax(&m.det_box[j * 6 + 5], mx2);
 }
 
-// Tile-level dedupe: a direct-mapped, lock-free filter in shared memory.  The slot index carries the low 10
-// bits of the label and bit 63 of the tag the 11th, so an equal tag in the same slot means the same
-// (key, label) pair exactly (labels >= 2048 bypass the filter).  It may let duplicates through (evictions,
-// races); it never drops a pair.  The exact set is the global pair set of probe_kernel.
-__device__ __forceinline__ bool tile_filter_fresh(TileSmem &s, unsigned long long key, uint32_t l) {
-  if (l >= 2048u) return true;
-  const uint32_t slot = (hash32((uint32_t)key, (uint32_t)(key >> 32)) ^ l) & (TILE_HASH - 1);
-  const unsigned long long tag = key | ((unsigned long long)((l >> 10) & 1u) << 63);
-  if (tag == KEY_EMPTY) return true;  // indistinguishable from an empty slot: never filtered
-  if (*(volatile unsigned long long *)&s.tag[slot] == tag) return false;
-  *(volatile unsigned long long *)&s.tag[slot] = tag;
-  return true;
+// OR the voxel bits (lo, hi) of block `bkey` into the tile's entry of (label slot li, block).  Exact: the tag
+// holds the whole block key and the label slot.  Without a label slot, or when the tile table is full, the
+// record goes straight to the global queue (the probe kernel's pair set keeps the result exact).
+__device__ __noinline__ void tile_block_add(TileSmem &s, const DevMap &m, int li, uint32_t j, unsigned long long bkey,
+                                            uint32_t lo, uint32_t hi) {
+  if (li >= 0) {
+    const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
+    uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
+    for (int probe = 0; probe < TILE_ENT; ++probe) {
+      unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
+      if (cur == BLK_EMPTY) {
+        cur = atomicCAS(&s.tag[h], BLK_EMPTY, tag);
+        if (cur == BLK_EMPTY) cur = tag;
+      }
+      if (cur == tag) {
+        if (lo) atomicOr(&s.mlo[h], lo);
+        if (hi) atomicOr(&s.mhi[h], hi);
+        return;
+      }
+      h = (h + 1) & (TILE_ENT - 1);
+    }
+  }
+  survivor_store(m, atomicAdd(&m.counters[2], 1u), bkey, j, lo, hi);
 }
 
-// ---------------------------------------------------------------------------------------------------
-// lift kernel (steps 1-2).  One 128x8 pixel tile per CTA; each thread owns 8 consecutive pixels of one row
-// (2 x 128-bit depth loads + 1 x 128-bit mask load).  Output: per-detection pixel counts and point boxes,
-// and the tile's distinct (detection, voxel key) pairs appended to the call's survivor queue.
 // raw registers of one thread's 8 pixels (2 x 128-bit depth + 1 x 128-bit mask)
 struct TileRegs {
   float4 d0, d1;
@@ -223,8 +229,8 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
   const int f = tile / (tiles_x * tiles_y);
   const int trem = tile - f * tiles_x * tiles_y;
   const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
-  const int v = ty * TILE_H + (tid >> 4);
-  const int u0 = tx * TILE_W + (tid & 15) * 8;
+  const int v = ty * TILE_H + (tid >> 3);
+  const int u0 = tx * TILE_W + (tid & 7) * 8;
   const size_t frame_off = (size_t)f * m.H * m.W;
   const bool row_ok = v < m.H;
   TileRegs r;
@@ -250,241 +256,301 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
   return r;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// lift kernel (steps 1-2).  One 64x16 pixel tile per CTA iteration; each thread owns 8 consecutive pixels of
+// one row (2 x 128-bit depth loads + 1 x 128-bit mask load).  A thread folds its pixels into runs of equal
+// (detection, block): the voxel of a pixel is one bit of the block's 64-bit mask, so the per-detection
+// dedupe (R7) is a bitwise OR -- in registers along the run, across the lanes of a warp that end on the same
+// block (match.any + redux.or), and into the tile's shared-memory table (atomicOr).  Output: per-detection
+// pixel counts and point boxes, and one (block, detection, voxel bits) record per tile entry appended to the
+// call's survivor queue.
 template <bool VEC>
 __global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   __shared__ TileSmem s;
   const int tid = threadIdx.x, lane = tid & 31;
   const int n_tiles = tiles_x * tiles_y * a.F;
   // Each CTA walks tiles blockIdx.x, +gridDim.x, ...; the loads of the next tile are issued before the current
-  // one is processed (register double buffering), so DRAM latency hides even at two resident CTAs per SM.
+  // one is processed (register double buffering), so DRAM latency hides behind the arithmetic.
   TileRegs cur = load_tile<VEC>(m, a, blockIdx.x, tiles_x, tiles_y, tid);
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-  TileRegs nxt = cur;
-  if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_y, tid);
-  const int f = tile / (tiles_x * tiles_y);
-  const int trem = tile - f * tiles_x * tiles_y;
-  const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
-  const int v = ty * TILE_H + (tid >> 4);
-  const int u0 = tx * TILE_W + (tid & 15) * 8;
-  float z[8];
-  uint32_t lab[8];
-  z[0] = cur.d0.x, z[1] = cur.d0.y, z[2] = cur.d0.z, z[3] = cur.d0.w;
-  z[4] = cur.d1.x, z[5] = cur.d1.y, z[6] = cur.d1.z, z[7] = cur.d1.w;
-  lab[0] = cur.mk.x & 0xFFFF, lab[1] = cur.mk.x >> 16, lab[2] = cur.mk.y & 0xFFFF, lab[3] = cur.mk.y >> 16;
-  lab[4] = cur.mk.z & 0xFFFF, lab[5] = cur.mk.z >> 16, lab[6] = cur.mk.w & 0xFFFF, lab[7] = cur.mk.w >> 16;
-  for (int i = tid; i < TILE_HASH; i += LIFT_THREADS) s.tag[i] = KEY_EMPTY;
-  if (tid < MAX_LABELS) {
-    s.lab_j[tid] = NONE32;
-    s.lab_cnt[tid] = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      s.lab_box[tid][k] = 0x7FFFFFFF;
-      s.lab_box[tid][3 + k] = (int)0x80000000;
+    TileRegs nxt = cur;
+    if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_y, tid);
+    const int f = tile / (tiles_x * tiles_y);
+    const int trem = tile - f * tiles_x * tiles_y;
+    const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
+    const int v = ty * TILE_H + (tid >> 3);
+    const int u0 = tx * TILE_W + (tid & 7) * 8;
+    float z[8];
+    uint32_t lab[8];
+    z[0] = cur.d0.x, z[1] = cur.d0.y, z[2] = cur.d0.z, z[3] = cur.d0.w;
+    z[4] = cur.d1.x, z[5] = cur.d1.y, z[6] = cur.d1.z, z[7] = cur.d1.w;
+    lab[0] = cur.mk.x & 0xFFFF, lab[1] = cur.mk.x >> 16, lab[2] = cur.mk.y & 0xFFFF, lab[3] = cur.mk.y >> 16;
+    lab[4] = cur.mk.z & 0xFFFF, lab[5] = cur.mk.z >> 16, lab[6] = cur.mk.w & 0xFFFF, lab[7] = cur.mk.w >> 16;
+    for (int i = tid; i < TILE_ENT; i += LIFT_THREADS) {
+      s.tag[i] = BLK_EMPTY;
+      s.mlo[i] = 0;
+      s.mhi[i] = 0;
     }
-  }
-  if (tid == 0) s.q_count = 0, s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
-  const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
-  const int det_base = a.base[f];
-  const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
-  // R5 term shared by the thread's 8 pixels (same row)
-  const float yn = __fmul_rn(__fsub_rn((float)v, cam.cy), cam.inv_fy);
-  __syncthreads();
-
-  // ---- per pixel: validity (R3, R4), back-projection (R5), key (R6), tile-level dedupe
-  const float INF = __int_as_float(0x7F800000);
-  uint32_t cur_l = 0, cur_cnt = 0;  // current run of equal labels (label 0 = none)
-  float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
-  unsigned long long prev_key = KEY_EMPTY;
-  uint32_t prev_l = 0;
-  uint32_t n_valid = 0, n_dropped = 0, n_ignored = 0;
+    if (tid < MAX_LABELS) {
+      s.lab_j[tid] = NONE32;
+      s.lab_cnt[tid] = 0;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    bool fresh = false;
-    unsigned long long key = KEY_EMPTY;
-    const uint32_t l = lab[i];
-    if (l != 0) {
-      if (l > n_det_f) {
-        n_ignored++;
-      } else if (depth_valid(z[i], m.z_min, m.z_max)) {
-        float p[3];
-        const float xn = __fmul_rn(__fsub_rn((float)(u0 + i), cam.cx), cam.inv_fx);
-        const float xc = __fmul_rn(xn, z[i]), yc = __fmul_rn(yn, z[i]);
-#pragma unroll
-        for (int k = 0; k < 3; ++k)
-          p[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(cam.r[3 * k], xc), __fmul_rn(cam.r[3 * k + 1], yc)),
-                                     __fmul_rn(cam.r[3 * k + 2], z[i])),
-                           cam.t[k]);
-        if (voxel_key(p, m.inv_vs, &key)) {
-          n_valid++;
-          if (l != cur_l) {
-            if (cur_l) tile_label_add(s, m, (uint32_t)det_base + cur_l - 1, cur_cnt, f2ord(mn0), f2ord(mn1), f2ord(mn2),
-                                      f2ord(mx0), f2ord(mx1), f2ord(mx2));
-            cur_l = l, cur_cnt = 0;
-            mn0 = mn1 = mn2 = INF, mx0 = mx1 = mx2 = -INF;
-          }
-          cur_cnt++;
-          mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
-          mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
-          if (!(key == prev_key && l == prev_l)) {  // thread-local dedupe of consecutive pixels
-            prev_key = key, prev_l = l;
-            fresh = tile_filter_fresh(s, key, l);
-          }
-        } else {
-          n_dropped++;
-        }
+      for (int k = 0; k < 3; ++k) {
+        s.lab_box[tid][k] = 0x7FFFFFFF;
+        s.lab_box[tid][3 + k] = (int)0x80000000;
       }
     }
-    // warp-ballot compaction of the surviving (detection, key) pairs into the tile queue
-    const unsigned b = __ballot_sync(0xFFFFFFFFu, fresh);
-    if (b) {
-      uint32_t base = 0;
-      if (lane == 0) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      if (fresh) {
-        const uint32_t pos = base + __popc(b & ((1u << lane) - 1));
-        if (pos < TILE_Q) {
-          s.qkey[pos] = key;
-          s.qj[pos] = (uint32_t)det_base + l - 1;
-        } else {  // rare: more distinct pairs in one tile than the shared queue holds
-          const uint32_t gp = atomicAdd(&m.counters[2], 1u);
-          if (gp < m.surv_cap) {
-            m.surv_key[gp] = key;
-            m.surv_j[gp] = (uint32_t)det_base + l - 1;
+    if (tid == 0) s.q_count = 0, s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
+    const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
+    const int det_base = a.base[f];
+    const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
+    // R5 term shared by the thread's 8 pixels (same row)
+    const float yn = __fmul_rn(__fsub_rn((float)v, cam.cy), cam.inv_fy);
+    const float u0f = (float)u0;  // (float)(u0 + i) == u0f + (float)i exactly (integers below 2^24)
+    __syncthreads();
+
+    // ---- per pixel: validity (R3, R4), back-projection (R5), voxel index (R6), run of equal (label, block)
+    const float INF = __int_as_float(0x7F800000);
+    uint32_t cur_l = 0, cur_cnt = 0;  // current run of equal labels (label 0 = none)
+    int cur_li = -1;
+    float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
+    unsigned long long cur_b = BLK_EMPTY;  // current run of equal blocks inside the label run
+    uint32_t blo = 0, bhi = 0;
+    uint32_t n_valid = 0, n_dropped = 0, n_ignored = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const uint32_t l = lab[i];
+      if (l != 0) {
+        if (l > n_det_f) {
+          n_ignored++;
+        } else if (depth_valid(z[i], m.z_min, m.z_max)) {
+          float p[3];
+          const float xn = __fmul_rn(__fsub_rn(__fadd_rn(u0f, (float)i), cam.cx), cam.inv_fx);
+          const float xc = __fmul_rn(xn, z[i]), yc = __fmul_rn(yn, z[i]);
+#pragma unroll
+          for (int k = 0; k < 3; ++k)
+            p[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(cam.r[3 * k], xc), __fmul_rn(cam.r[3 * k + 1], yc)),
+                                       __fmul_rn(cam.r[3 * k + 2], z[i])),
+                             cam.t[k]);
+          uint32_t ix, iy, iz;
+          if (voxel_index(p, m.inv_vs, ix, iy, iz)) {
+            n_valid++;
+            if (l != cur_l) {
+              if (cur_l) {
+                const uint32_t j = (uint32_t)det_base + cur_l - 1;
+                if (cur_b != BLK_EMPTY) tile_block_add(s, m, cur_li, j, cur_b, blo, bhi);
+                tile_label_add(s, m, cur_li, j, cur_cnt, f2ord(mn0), f2ord(mn1), f2ord(mn2), f2ord(mx0), f2ord(mx1),
+                               f2ord(mx2));
+              }
+              cur_l = l, cur_cnt = 0;
+              cur_li = tile_label_slot(s, (uint32_t)det_base + l - 1);
+              mn0 = mn1 = mn2 = INF, mx0 = mx1 = mx2 = -INF;
+              cur_b = BLK_EMPTY, blo = bhi = 0;
+            }
+            cur_cnt++;
+            mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
+            mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
+            const unsigned long long bkey = block_key(ix, iy, iz);
+            const uint32_t bit = block_bit(ix, iy, iz);
+            if (bkey != cur_b) {
+              if (cur_b != BLK_EMPTY) tile_block_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_b, blo, bhi);
+              cur_b = bkey, blo = bhi = 0;
+            }
+            const uint32_t one = 1u << (bit & 31);
+            blo |= (bit & 32) ? 0u : one;
+            bhi |= (bit & 32) ? one : 0u;
           } else {
-            atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+            n_dropped++;
           }
         }
       }
     }
-  }
-  // per-detection pixel count and point AABB (R7): warp-uniform fast path through REDUX, else per thread
-  {
-    const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_l != 0);
-    if (has) {
-      const uint32_t lead_l = __shfl_sync(0xFFFFFFFFu, cur_l, __ffs(has) - 1);
-      const bool uniform = __all_sync(0xFFFFFFFFu, cur_l == 0 || cur_l == lead_l);
-      const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
-      if (uniform) {
-        const uint32_t cnt = __reduce_add_sync(0xFFFFFFFFu, cur_cnt);
-        const int r0 = __reduce_min_sync(0xFFFFFFFFu, o0), r1 = __reduce_min_sync(0xFFFFFFFFu, o1),
-                  r2 = __reduce_min_sync(0xFFFFFFFFu, o2), r3 = __reduce_max_sync(0xFFFFFFFFu, o3),
-                  r4 = __reduce_max_sync(0xFFFFFFFFu, o4), r5 = __reduce_max_sync(0xFFFFFFFFu, o5);
-        if (lane == 0) tile_label_add(s, m, (uint32_t)det_base + lead_l - 1, cnt, r0, r1, r2, r3, r4, r5);
-      } else if (cur_l != 0) {
-        tile_label_add(s, m, (uint32_t)det_base + cur_l - 1, cur_cnt, o0, o1, o2, o3, o4, o5);
+    // ---- the thread's last block run: OR across the lanes of the warp that ended on the same (label, block)
+    {
+      if (cur_b != BLK_EMPTY && cur_li < 0) {  // no label slot: nothing to merge with, straight to the global queue
+        tile_block_add(s, m, -1, (uint32_t)det_base + cur_l - 1, cur_b, blo, bhi);
+        cur_b = BLK_EMPTY;
+      }
+      const bool has = cur_b != BLK_EMPTY;
+      const unsigned act = __ballot_sync(0xFFFFFFFFu, has);
+      if (has) {
+        const unsigned long long tag = cur_b | ((unsigned long long)cur_li << LABEL_SHIFT);
+        const unsigned same = __match_any_sync(act, tag);
+        const uint32_t lo = __reduce_or_sync(same, blo), hi = __reduce_or_sync(same, bhi);
+        if (lane == __ffs(same) - 1) tile_block_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_b, lo, hi);
       }
     }
-    n_valid = __reduce_add_sync(0xFFFFFFFFu, n_valid);
-    n_dropped = __reduce_add_sync(0xFFFFFFFFu, n_dropped);
-    n_ignored = __reduce_add_sync(0xFFFFFFFFu, n_ignored);
-    if (lane == 0) {
-      if (n_valid) atomicAdd(&s.n_valid, n_valid);
-      if (n_dropped) atomicAdd(&s.n_dropped, n_dropped);
-      if (n_ignored) atomicAdd(&s.n_ignored, n_ignored);
+    // ---- per-detection pixel count and point AABB (R7): warp-uniform fast path through REDUX, else per thread
+    {
+      const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_l != 0);
+      if (has) {
+        const int src = __ffs(has) - 1;
+        const uint32_t lead_l = __shfl_sync(0xFFFFFFFFu, cur_l, src);
+        const int lead_li = __shfl_sync(0xFFFFFFFFu, cur_li, src);
+        const bool uniform = __all_sync(0xFFFFFFFFu, cur_l == 0 || cur_l == lead_l);
+        const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
+        if (uniform) {
+          const uint32_t cnt = __reduce_add_sync(0xFFFFFFFFu, cur_cnt);
+          const int r0 = __reduce_min_sync(0xFFFFFFFFu, o0), r1 = __reduce_min_sync(0xFFFFFFFFu, o1),
+                    r2 = __reduce_min_sync(0xFFFFFFFFu, o2), r3 = __reduce_max_sync(0xFFFFFFFFu, o3),
+                    r4 = __reduce_max_sync(0xFFFFFFFFu, o4), r5 = __reduce_max_sync(0xFFFFFFFFu, o5);
+          if (lane == 0) tile_label_add(s, m, lead_li, (uint32_t)det_base + lead_l - 1, cnt, r0, r1, r2, r3, r4, r5);
+        } else if (cur_l != 0) {
+          tile_label_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_cnt, o0, o1, o2, o3, o4, o5);
+        }
+      }
+      n_valid = __reduce_add_sync(0xFFFFFFFFu, n_valid);
+      n_dropped = __reduce_add_sync(0xFFFFFFFFu, n_dropped);
+      n_ignored = __reduce_add_sync(0xFFFFFFFFu, n_ignored);
+      if (lane == 0) {
+        if (n_valid) atomicAdd(&s.n_valid, n_valid);
+        if (n_dropped) atomicAdd(&s.n_dropped, n_dropped);
+        if (n_ignored) atomicAdd(&s.n_ignored, n_ignored);
+      }
     }
-  }
-  __syncthreads();
+    __syncthreads();
 
-  // ---- append the tile queue to the call's survivor queue (one global atomic per tile, coalesced copy)
-  const uint32_t nq = min(s.q_count, (uint32_t)TILE_Q);
-  if (tid == 0 && nq) s.q_base = atomicAdd(&m.counters[2], nq);
-  // ---- flush the tile's per-detection accumulators and counters
-  if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
-    const uint32_t j = s.lab_j[tid];
-    atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
+    // ---- flush: tile entries -> survivor queue (one global atomic per tile), per-detection accumulators, counters
+    uint32_t my_pos[TILE_ENT / LIFT_THREADS];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
-      atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
+    for (int r = 0; r < TILE_ENT / LIFT_THREADS; ++r) {
+      const bool has = s.tag[tid + r * LIFT_THREADS] != BLK_EMPTY;
+      const unsigned b = __ballot_sync(0xFFFFFFFFu, has);
+      uint32_t base = 0;
+      if (lane == 0 && b) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      my_pos[r] = has ? base + __popc(b & ((1u << lane) - 1)) : NONE32;
     }
-  }
-  if (tid == 0) {
-    if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
-    if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
-    if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
-  }
-  __syncthreads();
-  const uint32_t qb = s.q_base;
-  for (uint32_t i = tid; i < nq; i += LIFT_THREADS) {
-    const uint32_t pos = qb + i;
-    if (pos < m.surv_cap) {
-      m.surv_key[pos] = s.qkey[i];
-      m.surv_j[pos] = s.qj[i];
-    } else {
-      atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+    if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
+      const uint32_t j = s.lab_j[tid];
+      atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
+        atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
+      }
     }
-  }
-  __syncthreads();  // the tile's shared state is re-initialised by the next iteration
-  cur = nxt;
+    __syncthreads();
+    if (tid == 0) {
+      if (s.q_count) s.q_base = atomicAdd(&m.counters[2], s.q_count);
+      if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
+      if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
+      if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
+    }
+    __syncthreads();
+    const uint32_t qb = s.q_base;
+#pragma unroll
+    for (int r = 0; r < TILE_ENT / LIFT_THREADS; ++r) {
+      if (my_pos[r] != NONE32) {
+        const int e = tid + r * LIFT_THREADS;
+        const unsigned long long tag = s.tag[e];
+        survivor_store(m, qb + my_pos[r], tag & ((1ull << LABEL_SHIFT) - 1), s.lab_j[(uint32_t)(tag >> LABEL_SHIFT)], s.mlo[e],
+                       s.mhi[e]);
+      }
+    }
+    __syncthreads();  // the tile's shared state is re-initialised by the next iteration
+    cur = nxt;
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// probe kernel (step 3 and R12 pass 1).  One thread per queued (detection, key) pair: find or insert the
-// key in the global voxel table, make the pair exact through the per-call pair set, then
-//   |V_d| += 1,  append to the pair list,  overlap c[d][owner] += 1 when the key was owned at entry (R9),
-//   claim = min(claim, d) when this call inserted the key (R12).
-// Atomics are aggregated over the lanes of a warp that hit the same address (__match_any_sync).
-__global__ void __launch_bounds__(256) probe_kernel(DevMap m, CallArgs a) {
+// probe kernel (step 3 and R12 pass 1).  Each warp takes 32 survivor records.
+// Phase A, one lane per record: find or insert the block in the global hash, then OR the record's voxel bits
+//   into the per-call pair set entry of (detection, block): the bits that were not set before are the
+//   detection's NEW voxels -- exactly one record wins each (detection, voxel) pair, whatever the tiling.
+// Phase B, eight lanes per record (one 32-byte owner sector each): for every new voxel read its owner;
+//   owned at entry -> overlap c[d][owner] += 1 (R9), else claim = min(claim, d) (R12, lowest index wins).
+//   |V_d| += popc(new bits); the (detection, block, new bits) event is appended to the event list for the
+//   commit pass.  Overlap counts are aggregated over the lanes of a warp (match.any + redux.add).
+constexpr int PROBE_THREADS = 256;
+
+__global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs a) {
   const uint32_t nq = min(m.counters[2], m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < nq; i0 += stride) {
     const uint32_t i = i0 + lane;
-    bool is_new = false, owned = false;
-    uint32_t j = 0, slot = NONE32, owner = OWNER_PENDING;
+    // ---- phase A
+    uint32_t j = 0, slot = NONE32, ps = 0;
+    unsigned long long nb = 0;
     if (i < nq) {
-      const unsigned long long key = __ldcs(&m.surv_key[i]);
+      const unsigned long long bkey = __ldcs(&m.surv_key[i]);
+      const unsigned long long bits = __ldcs(&m.surv_bits[i]);
       j = __ldcs(&m.surv_j[i]);
-      uint32_t visit = 0;
-      slot = voxel_find_or_insert(m, key, &owner, &visit);
+      slot = block_find_or_insert(m, bkey);
       if (slot != NONE32) {
-        // exactness of the (detection, key) pair: first toucher of the key in this call wins the slot's
-        // visit word; a second detection on the same key (object boundaries) uses the per-call pair set
-        const uint32_t mine = (a.epoch << 16) | j;
-        for (;;) {
-          if (visit == mine) break;                        // this pair was already counted
-          if ((visit >> 16) != a.epoch) {                  // nobody touched the key in this call yet
-            const uint32_t old = atomicCAS(&m.table[slot].visit, visit, mine);
-            if (old == visit) {
-              is_new = true;
-              break;
-            }
-            visit = old;
-            continue;
-          }
-          const unsigned long long pv = ((unsigned long long)mine << 32) | slot;
-          uint32_t ps;
-          const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
-          if (r < 0) atomicOr(m.err, ERR_PAIR_TABLE_FULL);
-          is_new = r == 1;
-          break;
+        const unsigned long long pv = ((unsigned long long)((a.epoch << 16) | j) << 32) | slot;
+        const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
+        if (r < 0) {
+          atomicOr(m.err, ERR_PAIR_TABLE_FULL);
+        } else {
+          const unsigned long long old = atomicOr(&m.pair_bits[ps], bits);
+          nb = bits & ~old;
         }
-        owned = is_new && owner < OWNER_PENDING;  // owned at entry (R9); else inserted by this call (R12)
       }
     }
-    const unsigned act = __ballot_sync(0xFFFFFFFFu, is_new);
-    if (act) {
-      // append to the pair list (one atomic per warp)
-      uint32_t base = 0;
-      if (lane == 0) base = atomicAdd(&m.counters[0], (uint32_t)__popc(act));
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      const unsigned oact = __ballot_sync(0xFFFFFFFFu, owned);
-      if (is_new) {
-        const uint32_t pos = base + __popc(act & ((1u << lane) - 1));
-        if (pos < m.pair_cap)
-          m.pair_list[pos] = ((unsigned long long)(owned ? 0 : 1) << 63) | ((unsigned long long)j << 32) | slot;
-        else
-          atomicOr(m.err, ERR_PAIR_TABLE_FULL);
-        // |V_d| += 1, aggregated over the lanes of the same detection
-        const unsigned same = __match_any_sync(act, j);
-        if (lane == __ffs(same) - 1) atomicAdd(&m.det_nv[j], (uint32_t)__popc(same));
-        if (!owned) atomicMin(&m.table[slot].owner, OWNER_PENDING | j);  // R12: lowest detection index wins
+    const unsigned act = __ballot_sync(0xFFFFFFFFu, nb != 0);
+    if (!act) continue;
+    // |V_d| += new voxels (aggregated over the lanes of the same detection)
+    if (nb) {
+      const unsigned same = __match_any_sync(act, j);
+      const uint32_t tot = __reduce_add_sync(same, (uint32_t)__popcll(nb));
+      if (lane == __ffs(same) - 1) atomicAdd(&m.det_nv[j], tot);
+    }
+    // event list slots (one atomic per warp)
+    uint32_t ev = 0;
+    if (lane == 0) ev = atomicAdd(&m.counters[0], (uint32_t)__popc(act));
+    ev = __shfl_sync(0xFFFFFFFFu, ev, 0) + __popc(act & ((1u << lane) - 1));
+    // ---- phase B: 4 records per step, 8 lanes (owner sectors) per record
+    const int sec = lane & 7;
+    uint32_t pend_mine = 0;  // lane r: does record r have a voxel that was unowned at entry
+#pragma unroll 1
+    for (int step = 0; step < 8; ++step) {
+      if (((act >> (step * 4)) & 0xFu) == 0) continue;  // warp-uniform
+      const int src = step * 4 + (lane >> 3);
+      const unsigned long long rnb = __shfl_sync(0xFFFFFFFFu, nb, src);
+      const uint32_t rslot = __shfl_sync(0xFFFFFFFFu, slot, src);
+      const uint32_t rj = __shfl_sync(0xFFFFFFFFu, j, src);
+      const uint32_t byte = (uint32_t)(rnb >> (8 * sec)) & 0xFFu;
+      uint32_t own[8];
+      bool unowned = false;
+      uint32_t o1 = NONE32, c1 = 0;  // first owner seen by this lane and how many of its voxels have it
+      if (byte) {
+        uint32_t *base = m.blk_owner + (size_t)rslot * BLK_VOXELS + sec * 8;
+        const uint4 w0 = __ldcg(reinterpret_cast<const uint4 *>(base));
+        const uint4 w1 = __ldcg(reinterpret_cast<const uint4 *>(base) + 1);
+        own[0] = w0.x, own[1] = w0.y, own[2] = w0.z, own[3] = w0.w, own[4] = w1.x, own[5] = w1.y, own[6] = w1.z, own[7] = w1.w;
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+          if (!((byte >> b) & 1u)) continue;
+          const uint32_t o = own[b];
+          if (o >= OWNER_PENDING) {  // unowned at entry (free, or claimed by a detection of this call)
+            unowned = true;
+            atomicMin(base + b, OWNER_PENDING | rj);  // R12: lowest detection index wins
+          } else if (o1 == NONE32 || o == o1) {
+            o1 = o, c1++;
+          } else {  // a second owner inside one sector: rare, counted on its own
+            const unsigned long long ov = ((unsigned long long)a.epoch << 48) | ((unsigned long long)rj << 32) | o;
+            uint32_t os;
+            const int r = epoch_insert(m.ov_keys, m.ov_mask, ov, a.epoch, &os);
+            if (r < 0) {
+              atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+            } else {
+              if (r == 1) {
+                const uint32_t c = atomicAdd(&m.counters[1], 1u);
+                if (c < m.cand_cap) m.cand_slot[c] = os; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+              }
+              atomicAdd(&m.ov_cnt[os], 1u);
+            }
+          }
+        }
       }
-      // overlap histogram c[j][owner] += 1, aggregated over lanes with the same (j, owner)
-      if (owned) {
-        const unsigned long long jo = ((unsigned long long)j << 32) | owner;
+      // overlap histogram c[j][owner] += count, aggregated over the lanes with the same (j, owner)
+      const unsigned oact = __ballot_sync(0xFFFFFFFFu, c1 != 0);
+      if (c1) {
+        const unsigned long long jo = ((unsigned long long)rj << 32) | o1;
         const unsigned same = __match_any_sync(oact, jo);
+        const uint32_t tot = __reduce_add_sync(same, c1);
         if (lane == __ffs(same) - 1) {
           const unsigned long long ov = ((unsigned long long)a.epoch << 48) | jo;
           uint32_t os;
@@ -494,14 +560,23 @@ __global__ void __launch_bounds__(256) probe_kernel(DevMap m, CallArgs a) {
           } else {
             if (r == 1) {
               const uint32_t c = atomicAdd(&m.counters[1], 1u);
-              if (c < m.cand_cap)
-                m.cand_slot[c] = os;
-              else
-                atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+              if (c < m.cand_cap) m.cand_slot[c] = os; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
             }
-            atomicAdd(&m.ov_cnt[os], (uint32_t)__popc(same));
+            atomicAdd(&m.ov_cnt[os], tot);
           }
         }
+      }
+      const unsigned ub = __ballot_sync(0xFFFFFFFFu, unowned);
+      if ((lane >> 2) == step) pend_mine = (ub >> ((lane & 3) * 8)) & 0xFFu;
+    }
+    if (nb) {
+      if (ev < m.pair_cap) {
+        m.pl_bits[ev] = nb;
+        m.pl_slot[ev] = slot;
+        m.pl_j[ev] = j | (pend_mine ? 0x80000000u : 0u);
+        m.pl_ps[ev] = ps;
+      } else {
+        atomicOr(m.err, ERR_PAIR_TABLE_FULL);
       }
     }
   }
@@ -552,7 +627,7 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 }
 
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  probe_kernel<<<148 * 8, 256, 0, s>>>(m, a);
+  probe_kernel<<<148 * 4, PROBE_THREADS, 0, s>>>(m, a);
   return 1;
 }
 
