@@ -302,7 +302,7 @@ int finalise(farm_map *m) {
   A(d.cand_o, (size_t)ccap, 0);
   A(d.cand_c, (size_t)ccap, 0);
   d.cand_cap = (uint32_t)ccap;
-  const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30);
+  const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30) + 148 * 8 * 512;  // + chunk padding of the lift CTAs
   A(d.surv_key, (size_t)scap, 0);
   A(d.surv_bits, (size_t)scap, 0);
   A(d.surv_j, (size_t)scap, 0);
@@ -319,6 +319,7 @@ int finalise(farm_map *m) {
   A(d.assoc, MD, 0);
   A(d.is_new, MD, 0);
   A(d.best_score, MD, 0);
+  A(d.cam, (size_t)MAX_FRAMES * 16, 0);
   A(d.stats, 1, 0);
   A(d.totals, 1, 0);
   A(d.err, 1, 0);

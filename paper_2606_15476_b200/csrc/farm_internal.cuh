@@ -109,6 +109,7 @@ struct DevMap {
   int32_t *assoc;
   uint8_t *is_new;
   float *best_score;
+  float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
   CallStats *stats;
   Totals *totals;
   uint32_t *err;

@@ -90,6 +90,13 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     z.n_det = (uint32_t)a.M;
     *m.stats = z;
   }
+  if (blockIdx.x == 0 && (int)threadIdx.x < a.F) {  // per-frame camera block of the lift kernel (R5 reciprocals)
+    const Camera c = load_camera(a.K + 9 * threadIdx.x, a.T + 16 * threadIdx.x);
+    float *o = m.cam + 16 * threadIdx.x;
+    o[0] = c.inv_fx, o[1] = c.inv_fy, o[2] = c.cx, o[3] = c.cy;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) o[4 + 4 * i] = c.r[3 * i], o[5 + 4 * i] = c.r[3 * i + 1], o[6 + 4 * i] = c.r[3 * i + 2], o[7 + 4 * i] = c.t[i];
+  }
   if (warp >= a.M) return;
   const T *row = (const T *)a.desc + (size_t)warp * m.D;
   float s = 0.f;
@@ -142,7 +149,7 @@ __device__ __forceinline__ int epoch_insert(unsigned long long *tab, uint32_t ma
   return -1;
 }
 
-// append one (block, detection, voxel bits) record to the call's survivor queue
+// write one (block, detection, voxel bits) record of the call's survivor queue
 __device__ __forceinline__ void survivor_store(const DevMap &m, uint32_t pos, unsigned long long bkey, uint32_t j,
                                                uint32_t lo, uint32_t hi) {
   if (pos < m.surv_cap) {
@@ -155,22 +162,21 @@ __device__ __forceinline__ void survivor_store(const DevMap &m, uint32_t pos, un
 }
 
 struct TileSmem {
-  unsigned long long tag[TILE_ENT];  // block key | label slot << 57, BLK_EMPTY when free
+  unsigned long long tag[TILE_ENT];       // block key | label slot << 57, BLK_EMPTY when free
   uint32_t mlo[TILE_ENT], mhi[TILE_ENT];  // voxel bits of the block seen for that detection inside the tile
-  uint32_t lab_j[MAX_LABELS];
-  uint32_t lab_cnt[MAX_LABELS];
-  int lab_box[MAX_LABELS][6];
-  uint32_t q_count, q_base;
+  uint32_t q_count;                       // entries flushed by the tile that just finished
+  uint32_t cur_pos, cur_end;              // the CTA's current chunk of the survivor queue
+  uint32_t next_base, next_valid;         // the chunk reserved after it
   uint32_t n_valid, n_dropped, n_ignored;
 };
 
 // slot of detection j in the tile's label table (-1 when more than MAX_LABELS detections meet in one tile)
-__device__ __forceinline__ int tile_label_slot(TileSmem &s, uint32_t j) {
+__device__ __forceinline__ int tile_label_slot_in(uint32_t *lab_j, uint32_t j) {
   uint32_t h = j % MAX_LABELS;
   for (int probe = 0; probe < MAX_LABELS; ++probe) {
-    uint32_t l = *(volatile uint32_t *)&s.lab_j[h];
+    uint32_t l = *(volatile uint32_t *)&lab_j[h];
     if (l == NONE32) {
-      l = atomicCAS(&s.lab_j[h], NONE32, j);
+      l = atomicCAS(&lab_j[h], NONE32, j);
       if (l == NONE32) l = j;
     }
     if (l == j) return (int)h;
@@ -179,13 +185,13 @@ __device__ __forceinline__ int tile_label_slot(TileSmem &s, uint32_t j) {
   return -1;
 }
 
-// accumulate a run (cnt pixels, box as ordered ints) of detection j into the tile's per-detection accumulators
-__device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, int li, uint32_t j, uint32_t cnt, int mn0,
-                                            int mn1, int mn2, int mx0, int mx1, int mx2) {
+// accumulate cnt pixels and their box (ordered ints) of detection j into the tile's per-detection accumulators
+__device__ __forceinline__ void label_add_in(uint32_t *lab_cnt, int (*lab_box)[6], const DevMap &m, int li, uint32_t j,
+                                             uint32_t cnt, int mn0, int mn1, int mn2, int mx0, int mx1, int mx2) {
   if (li >= 0) {
-    atomicAdd(&s.lab_cnt[li], cnt);
-    atomicMin(&s.lab_box[li][0], mn0), atomicMin(&s.lab_box[li][1], mn1), atomicMin(&s.lab_box[li][2], mn2);
-    atomicMax(&s.lab_box[li][3], mx0), atomicMax(&s.lab_box[li][4], mx1), atomicMax(&s.lab_box[li][5], mx2);
+    atomicAdd(&lab_cnt[li], cnt);
+    atomicMin(&lab_box[li][0], mn0), atomicMin(&lab_box[li][1], mn1), atomicMin(&lab_box[li][2], mn2);
+    atomicMax(&lab_box[li][3], mx0), atomicMax(&lab_box[li][4], mx1), atomicMax(&lab_box[li][5], mx2);
     return;
   }
   atomicAdd(&m.det_npx[j], cnt);
@@ -196,8 +202,8 @@ __device__ __noinline__ void tile_label_add(TileSmem &s, const DevMap &m, int li
 // OR the voxel bits (lo, hi) of block `bkey` into the tile's entry of (label slot li, block).  Exact: the tag
 // holds the whole block key and the label slot.  Without a label slot, or when the tile table is full, the
 // record goes straight to the global queue (the probe kernel's pair set keeps the result exact).
-__device__ __noinline__ void tile_block_add(TileSmem &s, const DevMap &m, int li, uint32_t j, unsigned long long bkey,
-                                            uint32_t lo, uint32_t hi) {
+__device__ __forceinline__ void tile_block_add(TileSmem &s, const DevMap &m, int li, uint32_t j, unsigned long long bkey,
+                                               uint32_t lo, uint32_t hi) {
   if (li >= 0) {
     const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
     uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
@@ -225,9 +231,9 @@ struct TileRegs {
 };
 
 template <bool VEC>
-__device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a, int tile, int tiles_x, int tiles_y, int tid) {
-  const int f = tile / (tiles_x * tiles_y);
-  const int trem = tile - f * tiles_x * tiles_y;
+__device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a, int tile, int tiles_x, int tiles_xy, int tid) {
+  const int f = tile / tiles_xy;
+  const int trem = tile - f * tiles_xy;
   const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
   const int v = ty * TILE_H + (tid >> 3);
   const int u0 = tx * TILE_W + (tid & 7) * 8;
@@ -257,199 +263,262 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
 }
 
 // ---------------------------------------------------------------------------------------------------
-// lift kernel (steps 1-2).  One 64x16 pixel tile per CTA iteration; each thread owns 8 consecutive pixels of
-// one row (2 x 128-bit depth loads + 1 x 128-bit mask load).  A thread folds its pixels into runs of equal
-// (detection, block): the voxel of a pixel is one bit of the block's 64-bit mask, so the per-detection
-// dedupe (R7) is a bitwise OR -- in registers along the run, across the lanes of a warp that end on the same
-// block (match.any + redux.or), and into the tile's shared-memory table (atomicOr).  Output: per-detection
-// pixel counts and point boxes, and one (block, detection, voxel bits) record per tile entry appended to the
-// call's survivor queue.
+// lift kernel (steps 1-2).  Persistent CTAs; one 64x16 pixel tile per iteration, each thread owns 8
+// consecutive pixels of one row (2 x 128-bit depth loads + 1 x 128-bit mask load, issued one tile ahead).
+//   Phase 1 (straight-line fp32/int code per pixel): validity (R3, R4), back-projection (R5), voxel index
+//     (R6) -> block key + voxel bit, point box.
+//   Phase 2 (warp-synchronous): the voxel of a pixel is one bit of its block's 64-bit mask, so the
+//     per-detection dedupe (R7) is a bitwise OR -- over the thread's pixels of one block, over the lanes of
+//     the warp that hold the same (detection, block) (match.any + redux.or), and into the tile's
+//     shared-memory table (atomicOr).
+//   Flush: one (block, detection, voxel bits) record per table entry goes to the call's survivor queue.  The
+//     CTA reserves queue space in chunks of TILE_ENT records one tile ahead, so no thread ever waits for a
+//     global atomic; the unused tail of the last chunk is padded with empty records (bits == 0).
+// Two barriers per tile.  Per-detection pixel counts and point boxes go through shared-memory
+// accumulators (REDUX fast path when a warp holds one detection) to one set of global atomics per
+// (tile, detection).
 template <bool VEC>
-__global__ void __launch_bounds__(LIFT_THREADS) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+__global__ void __launch_bounds__(LIFT_THREADS, 4) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   __shared__ TileSmem s;
+  __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads
+  __shared__ uint32_t lab_cnt2[2][MAX_LABELS];  // its copy while tile t+1 initialises the other
+  __shared__ int lab_box2[2][MAX_LABELS][6];
   const int tid = threadIdx.x, lane = tid & 31;
-  const int n_tiles = tiles_x * tiles_y * a.F;
-  // Each CTA walks tiles blockIdx.x, +gridDim.x, ...; the loads of the next tile are issued before the current
-  // one is processed (register double buffering), so DRAM latency hides behind the arithmetic.
-  TileRegs cur = load_tile<VEC>(m, a, blockIdx.x, tiles_x, tiles_y, tid);
-  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  const int tiles_xy = tiles_x * tiles_y;
+  const int n_tiles = tiles_xy * a.F;
+  const float inv_vs = m.inv_vs, z_min = m.z_min, z_max = m.z_max;
+  const float INF = __int_as_float(0x7F800000);
+  constexpr unsigned FULL = 0xFFFFFFFFu;
+  for (int i = tid; i < TILE_ENT; i += LIFT_THREADS) {
+    s.tag[i] = BLK_EMPTY;
+    s.mlo[i] = 0;
+    s.mhi[i] = 0;
+  }
+  if (tid == 0) {
+    s.q_count = 0, s.cur_pos = 0, s.cur_end = 0, s.next_base = 0, s.next_valid = 0;
+    s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
+  }
+  uint32_t acc_valid = 0, acc_dropped = 0, acc_ignored = 0;  // per-thread counters over all tiles
+  int par = 0;
+  TileRegs cur = load_tile<VEC>(m, a, blockIdx.x, tiles_x, tiles_xy, tid);
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, par ^= 1) {
     TileRegs nxt = cur;
-    if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_y, tid);
-    const int f = tile / (tiles_x * tiles_y);
-    const int trem = tile - f * tiles_x * tiles_y;
+    if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_xy, tid);
+    const int f = tile / tiles_xy;
+    const int trem = tile - f * tiles_xy;
     const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
     const int v = ty * TILE_H + (tid >> 3);
     const int u0 = tx * TILE_W + (tid & 7) * 8;
-    float z[8];
-    uint32_t lab[8];
-    z[0] = cur.d0.x, z[1] = cur.d0.y, z[2] = cur.d0.z, z[3] = cur.d0.w;
-    z[4] = cur.d1.x, z[5] = cur.d1.y, z[6] = cur.d1.z, z[7] = cur.d1.w;
-    lab[0] = cur.mk.x & 0xFFFF, lab[1] = cur.mk.x >> 16, lab[2] = cur.mk.y & 0xFFFF, lab[3] = cur.mk.y >> 16;
-    lab[4] = cur.mk.z & 0xFFFF, lab[5] = cur.mk.z >> 16, lab[6] = cur.mk.w & 0xFFFF, lab[7] = cur.mk.w >> 16;
-    for (int i = tid; i < TILE_ENT; i += LIFT_THREADS) {
-      s.tag[i] = BLK_EMPTY;
-      s.mlo[i] = 0;
-      s.mhi[i] = 0;
-    }
-    if (tid < MAX_LABELS) {
-      s.lab_j[tid] = NONE32;
-      s.lab_cnt[tid] = 0;
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        s.lab_box[tid][k] = 0x7FFFFFFF;
-        s.lab_box[tid][3 + k] = (int)0x80000000;
-      }
-    }
-    if (tid == 0) s.q_count = 0, s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
-    const Camera cam = load_camera(a.K + 9 * f, a.T + 16 * f);
+    // camera of the frame, prepared by prep_kernel: (inv_fx, inv_fy, cx, cy), (r00 r01 r02 tx), (r10 ..), (r20 ..)
+    const float4 *cp = reinterpret_cast<const float4 *>(m.cam + 16 * f);
+    const float4 c0 = __ldg(cp), c1 = __ldg(cp + 1), c2 = __ldg(cp + 2), c3 = __ldg(cp + 3);
     const int det_base = a.base[f];
     const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
-    // R5 term shared by the thread's 8 pixels (same row)
-    const float yn = __fmul_rn(__fsub_rn((float)v, cam.cy), cam.inv_fy);
-    const float u0f = (float)u0;  // (float)(u0 + i) == u0f + (float)i exactly (integers below 2^24)
-    __syncthreads();
+    uint32_t *lab_j = lab_j2[par], *lab_cnt = lab_cnt2[par];
+    int(*lab_box)[6] = lab_box2[par];
+    if (tid < MAX_LABELS) {
+      lab_j[tid] = NONE32;
+      lab_cnt[tid] = 0;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        lab_box[tid][k] = 0x7FFFFFFF;
+        lab_box[tid][3 + k] = (int)0x80000000;
+      }
+    }
+    __syncthreads();  // B1: label table ready; every warp has finished the flush of the previous tile
+    if (tid == 0) {
+      // account for the records the previous tile flushed; reserve the next queue chunk one tile ahead
+      uint32_t pos = s.cur_pos + s.q_count;
+      s.q_count = 0;
+      if (pos >= s.cur_end && s.next_valid) {
+        pos = s.next_base + (pos - s.cur_end);
+        s.cur_end = s.next_base + TILE_ENT;
+        s.next_valid = 0;
+      }
+      s.cur_pos = pos;
+      if (s.cur_end - pos < (uint32_t)TILE_ENT && !s.next_valid) {
+        s.next_base = atomicAdd(&m.counters[2], (uint32_t)TILE_ENT);
+        s.next_valid = 1;
+      }
+    }
 
-    // ---- per pixel: validity (R3, R4), back-projection (R5), voxel index (R6), run of equal (label, block)
-    const float INF = __int_as_float(0x7F800000);
-    uint32_t cur_l = 0, cur_cnt = 0;  // current run of equal labels (label 0 = none)
-    int cur_li = -1;
+    // ---- phase 1
+    const float z[8] = {cur.d0.x, cur.d0.y, cur.d0.z, cur.d0.w, cur.d1.x, cur.d1.y, cur.d1.z, cur.d1.w};
+    const uint32_t lab[8] = {cur.mk.x & 0xFFFF, cur.mk.x >> 16, cur.mk.y & 0xFFFF, cur.mk.y >> 16,
+                             cur.mk.z & 0xFFFF, cur.mk.z >> 16, cur.mk.w & 0xFFFF, cur.mk.w >> 16};
+    const float yn = __fmul_rn(__fsub_rn((float)v, c0.w), c0.y);  // R5 term shared by the thread's 8 pixels
+    const float u0f = (float)u0;  // (float)(u0 + i) == u0f + (float)i exactly (integers below 2^24)
+    unsigned long long ikey[8];
+    uint32_t ibit_lo = 0, ibit_hi = 0;  // 6-bit voxel index inside the block, pixels 0-3 / 4-7
+    float P0[8], P1[8], P2[8];
+    uint32_t valid = 0, L0 = 0;
+    bool multi = false;
     float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
-    unsigned long long cur_b = BLK_EMPTY;  // current run of equal blocks inside the label run
-    uint32_t blo = 0, bhi = 0;
-    uint32_t n_valid = 0, n_dropped = 0, n_ignored = 0;
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
+      ikey[i] = BLK_EMPTY;
+      P0[i] = P1[i] = P2[i] = 0.f;
       const uint32_t l = lab[i];
       if (l != 0) {
         if (l > n_det_f) {
-          n_ignored++;
-        } else if (depth_valid(z[i], m.z_min, m.z_max)) {
-          float p[3];
-          const float xn = __fmul_rn(__fsub_rn(__fadd_rn(u0f, (float)i), cam.cx), cam.inv_fx);
+          acc_ignored++;
+        } else if (depth_valid(z[i], z_min, z_max)) {
+          const float xn = __fmul_rn(__fsub_rn(__fadd_rn(u0f, (float)i), c0.z), c0.x);
           const float xc = __fmul_rn(xn, z[i]), yc = __fmul_rn(yn, z[i]);
-#pragma unroll
-          for (int k = 0; k < 3; ++k)
-            p[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(cam.r[3 * k], xc), __fmul_rn(cam.r[3 * k + 1], yc)),
-                                       __fmul_rn(cam.r[3 * k + 2], z[i])),
-                             cam.t[k]);
+          float p[3];
+          p[0] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c1.x, xc), __fmul_rn(c1.y, yc)), __fmul_rn(c1.z, z[i])), c1.w);
+          p[1] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c2.x, xc), __fmul_rn(c2.y, yc)), __fmul_rn(c2.z, z[i])), c2.w);
+          p[2] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c3.x, xc), __fmul_rn(c3.y, yc)), __fmul_rn(c3.z, z[i])), c3.w);
           uint32_t ix, iy, iz;
-          if (voxel_index(p, m.inv_vs, ix, iy, iz)) {
-            n_valid++;
-            if (l != cur_l) {
-              if (cur_l) {
-                const uint32_t j = (uint32_t)det_base + cur_l - 1;
-                if (cur_b != BLK_EMPTY) tile_block_add(s, m, cur_li, j, cur_b, blo, bhi);
-                tile_label_add(s, m, cur_li, j, cur_cnt, f2ord(mn0), f2ord(mn1), f2ord(mn2), f2ord(mx0), f2ord(mx1),
-                               f2ord(mx2));
-              }
-              cur_l = l, cur_cnt = 0;
-              cur_li = tile_label_slot(s, (uint32_t)det_base + l - 1);
-              mn0 = mn1 = mn2 = INF, mx0 = mx1 = mx2 = -INF;
-              cur_b = BLK_EMPTY, blo = bhi = 0;
-            }
-            cur_cnt++;
+          if (voxel_index(p, inv_vs, ix, iy, iz)) {
+            valid |= 1u << i;
+            ikey[i] = block_key(ix, iy, iz);
+            const uint32_t bit = block_bit(ix, iy, iz);
+            if (i < 4) ibit_lo |= bit << (6 * i); else ibit_hi |= bit << (6 * (i - 4));
+            P0[i] = p[0], P1[i] = p[1], P2[i] = p[2];
+            if (L0 == 0) L0 = l;
+            multi |= l != L0;
             mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
             mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
-            const unsigned long long bkey = block_key(ix, iy, iz);
-            const uint32_t bit = block_bit(ix, iy, iz);
-            if (bkey != cur_b) {
-              if (cur_b != BLK_EMPTY) tile_block_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_b, blo, bhi);
-              cur_b = bkey, blo = bhi = 0;
-            }
-            const uint32_t one = 1u << (bit & 31);
-            blo |= (bit & 32) ? 0u : one;
-            bhi |= (bit & 32) ? one : 0u;
           } else {
-            n_dropped++;
+            acc_dropped++;
           }
         }
       }
     }
-    // ---- the thread's last block run: OR across the lanes of the warp that ended on the same (label, block)
-    {
-      if (cur_b != BLK_EMPTY && cur_li < 0) {  // no label slot: nothing to merge with, straight to the global queue
-        tile_block_add(s, m, -1, (uint32_t)det_base + cur_l - 1, cur_b, blo, bhi);
-        cur_b = BLK_EMPTY;
+    acc_valid += __popc(valid);
+
+    // ---- phase 2: one round per detection present in the warp's threads (one round unless a thread straddles two)
+    const bool any_multi = __any_sync(FULL, multi);
+    uint32_t todo = valid;
+    while (__any_sync(FULL, todo != 0)) {
+      uint32_t L = L0, mine = todo;
+      float b0 = mn0, b1 = mn1, b2 = mn2, b3 = mx0, b4 = mx1, b5 = mx2;
+      if (any_multi) {  // warp-uniform slow path: restrict the round to the label of the thread's first open pixel
+        L = 0;
+#pragma unroll
+        for (int i = 7; i >= 0; --i)
+          if ((todo >> i) & 1u) L = lab[i];
+        mine = 0;
+        b0 = b1 = b2 = INF, b3 = b4 = b5 = -INF;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          if (((todo >> i) & 1u) && lab[i] == L) {
+            mine |= 1u << i;
+            b0 = fminf(b0, P0[i]), b1 = fminf(b1, P1[i]), b2 = fminf(b2, P2[i]);
+            b3 = fmaxf(b3, P0[i]), b4 = fmaxf(b4, P1[i]), b5 = fmaxf(b5, P2[i]);
+          }
       }
-      const bool has = cur_b != BLK_EMPTY;
-      const unsigned act = __ballot_sync(0xFFFFFFFFu, has);
-      if (has) {
-        const unsigned long long tag = cur_b | ((unsigned long long)cur_li << LABEL_SHIFT);
-        const unsigned same = __match_any_sync(act, tag);
-        const uint32_t lo = __reduce_or_sync(same, blo), hi = __reduce_or_sync(same, bhi);
-        if (lane == __ffs(same) - 1) tile_block_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_b, lo, hi);
-      }
-    }
-    // ---- per-detection pixel count and point AABB (R7): warp-uniform fast path through REDUX, else per thread
-    {
-      const unsigned has = __ballot_sync(0xFFFFFFFFu, cur_l != 0);
-      if (has) {
+      todo &= ~mine;
+      const uint32_t j = (uint32_t)det_base + L - 1;
+      int li = -1;
+      if (mine) li = tile_label_slot_in(lab_j, j);
+      // per-detection pixel count and point AABB (R7): REDUX when the warp holds one detection
+      {
+        const unsigned has = __ballot_sync(FULL, mine != 0);
         const int src = __ffs(has) - 1;
-        const uint32_t lead_l = __shfl_sync(0xFFFFFFFFu, cur_l, src);
-        const int lead_li = __shfl_sync(0xFFFFFFFFu, cur_li, src);
-        const bool uniform = __all_sync(0xFFFFFFFFu, cur_l == 0 || cur_l == lead_l);
-        const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
+        const uint32_t lead_L = __shfl_sync(FULL, L, src);
+        const int lead_li = __shfl_sync(FULL, li, src);
+        const bool uniform = __all_sync(FULL, mine == 0 || L == lead_L);
+        const int o0 = f2ord(b0), o1 = f2ord(b1), o2 = f2ord(b2), o3 = f2ord(b3), o4 = f2ord(b4), o5 = f2ord(b5);
+        const uint32_t cnt = __popc(mine);
         if (uniform) {
-          const uint32_t cnt = __reduce_add_sync(0xFFFFFFFFu, cur_cnt);
-          const int r0 = __reduce_min_sync(0xFFFFFFFFu, o0), r1 = __reduce_min_sync(0xFFFFFFFFu, o1),
-                    r2 = __reduce_min_sync(0xFFFFFFFFu, o2), r3 = __reduce_max_sync(0xFFFFFFFFu, o3),
-                    r4 = __reduce_max_sync(0xFFFFFFFFu, o4), r5 = __reduce_max_sync(0xFFFFFFFFu, o5);
-          if (lane == 0) tile_label_add(s, m, lead_li, (uint32_t)det_base + lead_l - 1, cnt, r0, r1, r2, r3, r4, r5);
-        } else if (cur_l != 0) {
-          tile_label_add(s, m, cur_li, (uint32_t)det_base + cur_l - 1, cur_cnt, o0, o1, o2, o3, o4, o5);
+          const uint32_t tot = __reduce_add_sync(FULL, cnt);
+          const int r0 = __reduce_min_sync(FULL, o0), r1 = __reduce_min_sync(FULL, o1), r2 = __reduce_min_sync(FULL, o2),
+                    r3 = __reduce_max_sync(FULL, o3), r4 = __reduce_max_sync(FULL, o4), r5 = __reduce_max_sync(FULL, o5);
+          if (lane == 0) label_add_in(lab_cnt, lab_box, m, lead_li, (uint32_t)det_base + lead_L - 1, tot, r0, r1, r2, r3, r4, r5);
+        } else if (mine) {
+          label_add_in(lab_cnt, lab_box, m, li, j, cnt, o0, o1, o2, o3, o4, o5);
         }
       }
-      n_valid = __reduce_add_sync(0xFFFFFFFFu, n_valid);
-      n_dropped = __reduce_add_sync(0xFFFFFFFFu, n_dropped);
-      n_ignored = __reduce_add_sync(0xFFFFFFFFu, n_ignored);
-      if (lane == 0) {
-        if (n_valid) atomicAdd(&s.n_valid, n_valid);
-        if (n_dropped) atomicAdd(&s.n_dropped, n_dropped);
-        if (n_ignored) atomicAdd(&s.n_ignored, n_ignored);
+      // blocks of this detection: one pass per distinct block among the thread's pixels
+      uint32_t rem = mine;
+      while (__any_sync(FULL, rem != 0)) {
+        unsigned long long kb = BLK_EMPTY;
+#pragma unroll
+        for (int i = 7; i >= 0; --i)
+          if ((rem >> i) & 1u) kb = ikey[i];
+        uint32_t lo = 0, hi = 0, hit = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          if (((rem >> i) & 1u) && ikey[i] == kb) {
+            hit |= 1u << i;
+            const uint32_t bit = ((i < 4 ? ibit_lo >> (6 * i) : ibit_hi >> (6 * (i - 4)))) & 63u;
+            const uint32_t one = 1u << (bit & 31);
+            lo |= (bit & 32) ? 0u : one;
+            hi |= (bit & 32) ? one : 0u;
+          }
+        rem &= ~hit;
+        if (hit && li < 0) survivor_store(m, atomicAdd(&m.counters[2], 1u), kb, j, lo, hi);  // no label slot
+        const bool tab = hit && li >= 0;
+        const unsigned act = __ballot_sync(FULL, tab);
+        if (tab) {
+          const unsigned long long tag = kb | ((unsigned long long)li << LABEL_SHIFT);
+          const unsigned same = __match_any_sync(act, tag);
+          lo = __reduce_or_sync(same, lo), hi = __reduce_or_sync(same, hi);
+          if (lane == __ffs(same) - 1) tile_block_add(s, m, li, j, kb, lo, hi);
+        }
       }
     }
-    __syncthreads();
+    __syncthreads();  // B2: the tile's table is complete; thread 0 has published the queue chunk
 
-    // ---- flush: tile entries -> survivor queue (one global atomic per tile), per-detection accumulators, counters
-    uint32_t my_pos[TILE_ENT / LIFT_THREADS];
+    // ---- flush: table entries -> survivor queue (positions inside the CTA's reserved chunks), then clear them
+    {
+      const uint32_t cpos = s.cur_pos, cend = s.cur_end, nbase = s.next_base;
 #pragma unroll
-    for (int r = 0; r < TILE_ENT / LIFT_THREADS; ++r) {
-      const bool has = s.tag[tid + r * LIFT_THREADS] != BLK_EMPTY;
-      const unsigned b = __ballot_sync(0xFFFFFFFFu, has);
-      uint32_t base = 0;
-      if (lane == 0 && b) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      my_pos[r] = has ? base + __popc(b & ((1u << lane) - 1)) : NONE32;
-    }
-    if (tid < MAX_LABELS && s.lab_j[tid] != NONE32) {
-      const uint32_t j = s.lab_j[tid];
-      atomicAdd(&m.det_npx[j], s.lab_cnt[tid]);
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        atomicMin(&m.det_box[j * 6 + k], s.lab_box[tid][k]);
-        atomicMax(&m.det_box[j * 6 + 3 + k], s.lab_box[tid][3 + k]);
-      }
-    }
-    __syncthreads();
-    if (tid == 0) {
-      if (s.q_count) s.q_base = atomicAdd(&m.counters[2], s.q_count);
-      if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
-      if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
-      if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
-    }
-    __syncthreads();
-    const uint32_t qb = s.q_base;
-#pragma unroll
-    for (int r = 0; r < TILE_ENT / LIFT_THREADS; ++r) {
-      if (my_pos[r] != NONE32) {
+      for (int r = 0; r < TILE_ENT / LIFT_THREADS; ++r) {
         const int e = tid + r * LIFT_THREADS;
         const unsigned long long tag = s.tag[e];
-        survivor_store(m, qb + my_pos[r], tag & ((1ull << LABEL_SHIFT) - 1), s.lab_j[(uint32_t)(tag >> LABEL_SHIFT)], s.mlo[e],
-                       s.mhi[e]);
+        const bool has = tag != BLK_EMPTY;
+        const unsigned b = __ballot_sync(FULL, has);
+        uint32_t base = 0;
+        if (lane == 0 && b) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
+        base = __shfl_sync(FULL, base, 0);
+        if (has) {
+          uint32_t pos = cpos + base + __popc(b & ((1u << lane) - 1));
+          if (pos >= cend) pos = nbase + (pos - cend);
+          survivor_store(m, pos, tag & ((1ull << LABEL_SHIFT) - 1), lab_j[(uint32_t)(tag >> LABEL_SHIFT)], s.mlo[e], s.mhi[e]);
+          s.tag[e] = BLK_EMPTY;
+          s.mlo[e] = 0;
+          s.mhi[e] = 0;
+        }
+      }
+      if (tid < MAX_LABELS && lab_j[tid] != NONE32) {
+        const uint32_t j = lab_j[tid];
+        atomicAdd(&m.det_npx[j], lab_cnt[tid]);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          atomicMin(&m.det_box[j * 6 + k], lab_box[tid][k]);
+          atomicMax(&m.det_box[j * 6 + 3 + k], lab_box[tid][3 + k]);
+        }
       }
     }
-    __syncthreads();  // the tile's shared state is re-initialised by the next iteration
     cur = nxt;
+  }
+  // ---- end of the CTA's tiles: statistics, and empty records over the unused part of the reserved chunks
+  acc_valid = __reduce_add_sync(FULL, acc_valid);
+  acc_dropped = __reduce_add_sync(FULL, acc_dropped);
+  acc_ignored = __reduce_add_sync(FULL, acc_ignored);
+  if (lane == 0) {
+    if (acc_valid) atomicAdd(&s.n_valid, acc_valid);
+    if (acc_dropped) atomicAdd(&s.n_dropped, acc_dropped);
+    if (acc_ignored) atomicAdd(&s.n_ignored, acc_ignored);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    if (s.n_valid) atomicAdd(&m.stats->valid_points, (unsigned long long)s.n_valid);
+    if (s.n_dropped) atomicAdd(&m.stats->dropped_points, (unsigned long long)s.n_dropped);
+    if (s.n_ignored) atomicAdd(&m.stats->ignored_pixels, (unsigned long long)s.n_ignored);
+  }
+  {
+    uint32_t pos = s.cur_pos + s.q_count, end = s.cur_end;
+    if (pos >= end && s.next_valid) {
+      pos = s.next_base + (pos - end);
+      end = s.next_base + TILE_ENT;
+    } else if (s.next_valid) {  // a reserved chunk that was never reached
+      for (uint32_t p = s.next_base + tid; p < s.next_base + TILE_ENT; p += LIFT_THREADS) survivor_store(m, p, 0ull, 0u, 0u, 0u);
+    }
+    for (uint32_t p = pos + tid; p < end; p += LIFT_THREADS) survivor_store(m, p, 0ull, 0u, 0u, 0u);
   }
 }
 
@@ -477,7 +546,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
       const unsigned long long bkey = __ldcs(&m.surv_key[i]);
       const unsigned long long bits = __ldcs(&m.surv_bits[i]);
       j = __ldcs(&m.surv_j[i]);
-      slot = block_find_or_insert(m, bkey);
+      if (bits) slot = block_find_or_insert(m, bkey);  // bits == 0: padding of a reserved queue chunk
       if (slot != NONE32) {
         const unsigned long long pv = ((unsigned long long)((a.epoch << 16) | j) << 32) | slot;
         const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
@@ -617,7 +686,7 @@ int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
   const int n_tiles = tiles_x * tiles_y * a.F;
-  const int grid = n_tiles < 148 * 8 ? n_tiles : 148 * 8;
+  const int grid = n_tiles < 148 * 4 ? n_tiles : 148 * 4;  // persistent: 4 resident CTAs per SM
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
   if (vec)
     lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
