@@ -324,6 +324,8 @@ int finalise(farm_map *m) {
   A(d.totals, 1, 0);
   A(d.err, 1, 0);
 #undef A
+  configure_lift_kernels();
+  configure_assoc_kernels();
   init_objects_kernel<<<(unsigned)((NO + 255) / 256), 256, 0, m->stream>>>(d);
   m->launches++;
   CU(cudaGetLastError());

@@ -40,6 +40,9 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
       }
       const T *x = (const T *)a.desc + (size_t)j * D;
       const T *y = (const T *)m.desc_shadow + (size_t)o * D;
+      // scalars of the score, requested together with the rows (same address in every lane: one transaction)
+      const float ia = m.det_inv_norm[j], ib = m.inv_norm[o];
+      const uint32_t mn = min(__ldcg(&m.det_nv[j]), m.n_voxels[o]);
       float dot = 0.f;
       if (sizeof(T) == 2 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {
         for (int i = lane * 8; i < D; i += 256) {
@@ -56,9 +59,8 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
 #pragma unroll
       for (int sft = 16; sft; sft >>= 1) dot += __shfl_xor_sync(0xFFFFFFFFu, dot, sft);
       if (lane == 0) {
-        float cs = dot * m.det_inv_norm[j] * m.inv_norm[o];
+        float cs = dot * ia * ib;
         cs = fminf(1.f, fmaxf(-1.f, cs));                                  // R15
-        const uint32_t mn = min(m.det_nv[j], m.n_voxels[o]);
         const float g = mn ? __fdiv_rn((float)cnt, (float)mn) : 0.f;       // R10
         const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));  // R17
         atomicMax(&m.best_cand[j], pack_score(score, o));
@@ -178,8 +180,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   extern __shared__ float acc[];  // [D]
   __shared__ uint32_t list[MERGE_THREADS];
   __shared__ uint32_t warp_cnt[MERGE_WARPS];
-  __shared__ float red[MERGE_WARPS];
-  __shared__ float s_bcast;
+  __shared__ float red[MERGE_WARPS], red2[MERGE_WARPS];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if ((int)blockIdx.x < commit_blocks) {
     // 8 lanes per event (one 32-byte owner sector each), 4 events per warp and step
@@ -222,113 +223,159 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   }
   const int D = m.D;
   const int merge_blocks = gridDim.x - commit_blocks;
+  // 8 elements per thread and step (128-bit loads of the storage-dtype rows, 2 x 128-bit of the fp32 masters)
+  const bool vec = (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
   for (int j = blockIdx.x - commit_blocks; j < a.M; j += merge_blocks) {
     const int32_t t = m.assoc[j];
-    if (t < 0 || m.leader[t] != (uint32_t)j) continue;  // uniform per CTA
-    const uint32_t group = m.grp_cnt[t];
-    // old object state, loaded early by thread 0 so that the latency hides behind the descriptor work
-    uint32_t n_old_t0 = 0;
+    if (t < 0) continue;                                   // uniform per CTA
+    const uint32_t lead = __ldcg(&m.leader[t]), group = __ldcg(&m.grp_cnt[t]);
+    if (lead != (uint32_t)j) continue;
+    // everything the fold needs is requested up front so that the loads overlap
+    const uint32_t n_old = m.n_obs[t];
+    float *master = m.desc_master + (size_t)t * D;
+    T *shadow = (T *)m.desc_shadow + (size_t)t * D;
     unsigned long long pts_old = 0, best_old = 0;
     int box_old[6];
     if (tid == 0) {
-      n_old_t0 = m.n_obs[t];
       pts_old = m.n_points[t];
       best_old = m.best_view[t];
 #pragma unroll
       for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
     }
-    for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = 0.f;
     uint32_t k_members = 0;
     unsigned long long pts = 0, best = 0;
     int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
     int best_frame = -1;
-    __syncthreads();
-    const int scan_end = group > 1 ? a.M : j + 1;  // a group of one is just the leader itself
-    for (int base = j & ~(MERGE_THREADS - 1); base < scan_end; base += MERGE_THREADS) {  // members have index >= j
-      const int jj = base + tid;
-      const bool flag = jj < scan_end && jj >= j && m.assoc[jj] == t;
-      const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
-      if (lane == 0) warp_cnt[warp] = __popc(b);
-      __syncthreads();
-      uint32_t before = 0, total = 0;
+    auto member_evidence = [&](uint32_t jm) {  // thread 0: R22 / R23 contribution of one member
+      k_members++;
+      const uint32_t npx = m.det_npx[jm];
+      pts += npx;
 #pragma unroll
-      for (int w = 0; w < MERGE_WARPS; ++w) {
-        before += w < warp ? warp_cnt[w] : 0;
-        total += warp_cnt[w];
+      for (int c = 0; c < 3; ++c) {
+        bmn[c] = min(bmn[c], m.det_box[jm * 6 + c]);
+        bmx[c] = max(bmx[c], m.det_box[jm * 6 + 3 + c]);
       }
-      if (flag) list[before + __popc(b & ((1u << lane) - 1))] = (uint32_t)jj;
-      __syncthreads();
-      for (uint32_t q = 0; q < total; ++q) {
-        const uint32_t jm = list[q];
-        const float inv = m.det_inv_norm[jm];  // zero-norm rows contribute nothing (R21)
-        const T *row = (const T *)a.desc + (size_t)jm * D;
-        for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = fmaf(to_f32<T>(row[i]), inv, acc[i]);
-        if (tid == 0) {
-          k_members++;
-          const uint32_t npx = m.det_npx[jm];
-          pts += npx;
+      int f = 0;
+      while (f + 1 < a.F && (int)jm >= a.base[f + 1]) ++f;
+      const unsigned long long seq = frame_seq0 + f;
+      const uint32_t det = jm - a.base[f];
+      // R23: most pixels wins, ties -> smallest (frame_seq, det)
+      const unsigned long long pv = ((unsigned long long)(npx & 0xFFFFFFu) << 40) | ((~seq & 0xFFFFFFull) << 16) |
+                                    (unsigned long long)(~det & 0xFFFFu);
+      if (pv > best) best = pv, best_frame = f;
+    };
+    auto add_row = [&](uint32_t jm, bool first) {  // acc (+)= a_jm / |a_jm|; zero-norm rows contribute nothing (R21)
+      const float inv = m.det_inv_norm[jm];
+      const T *row = (const T *)a.desc + (size_t)jm * D;
+      if (vec && sizeof(T) == 2) {
+        for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
+          const uint4 w = *reinterpret_cast<const uint4 *>(row + i);
+          const T *e = reinterpret_cast<const T *>(&w);
 #pragma unroll
-          for (int c = 0; c < 3; ++c) {
-            bmn[c] = min(bmn[c], m.det_box[jm * 6 + c]);
-            bmx[c] = max(bmx[c], m.det_box[jm * 6 + 3 + c]);
-          }
-          int f = 0;
-          while (f + 1 < a.F && (int)jm >= a.base[f + 1]) ++f;
-          const unsigned long long seq = frame_seq0 + f;
-          const uint32_t det = jm - a.base[f];
-          // R23: most pixels wins, ties -> smallest (frame_seq, det)
-          const unsigned long long pv = ((unsigned long long)(npx & 0xFFFFFFu) << 40) |
-                                        ((~seq & 0xFFFFFFull) << 16) | (unsigned long long)(~det & 0xFFFFu);
-          if (pv > best) best = pv, best_frame = f;
+          for (int q = 0; q < 8; ++q) acc[i + q] = first ? to_f32<T>(e[q]) * inv : fmaf(to_f32<T>(e[q]), inv, acc[i + q]);
+        }
+      } else {
+        for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = first ? to_f32<T>(row[i]) * inv : fmaf(to_f32<T>(row[i]), inv, acc[i]);
+      }
+    };
+    __syncthreads();  // acc of the previous iteration is no longer read
+    if (group <= 1) {  // the common case: the leader is the only member
+      add_row((uint32_t)j, true);
+      if (tid == 0) member_evidence((uint32_t)j);
+    } else {
+      bool first = true;
+      for (int base = j & ~(MERGE_THREADS - 1); base < a.M; base += MERGE_THREADS) {  // members have index >= j
+        const int jj = base + tid;
+        const bool flag = jj < a.M && jj >= j && m.assoc[jj] == t;
+        const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
+        if (lane == 0) warp_cnt[warp] = __popc(b);
+        __syncthreads();
+        uint32_t before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < MERGE_WARPS; ++w) {
+          before += w < warp ? warp_cnt[w] : 0;
+          total += warp_cnt[w];
+        }
+        if (flag) list[before + __popc(b & ((1u << lane) - 1))] = (uint32_t)jj;
+        __syncthreads();
+        for (uint32_t q = 0; q < total; ++q) {  // members in index order: deterministic summation
+          add_row(list[q], first);
+          first = false;
+          if (tid == 0) member_evidence(list[q]);
+        }
+        __syncthreads();
+      }
+    }
+    // f_o <- normalise(n_obs * f_o + sum)   (R21); each thread revisits exactly the elements it accumulated
+    float ss = 0.f;
+    if (vec && sizeof(T) == 2) {
+      for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
+        float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0;
+        if (n_old) m0 = *reinterpret_cast<const float4 *>(master + i), m1 = *reinterpret_cast<const float4 *>(master + i + 4);
+        const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          const float v = n_old ? fmaf((float)n_old, mv[q], acc[i + q]) : acc[i + q];
+          acc[i + q] = v;
+          ss = fmaf(v, v, ss);
         }
       }
-      __syncthreads();
-    }
-    // f_o <- normalise(n_obs * f_o + sum)   (R21)
-    const uint32_t n_old = m.n_obs[t];
-    float *master = m.desc_master + (size_t)t * D;
-    T *shadow = (T *)m.desc_shadow + (size_t)t * D;
-    float ss = 0.f;
-    for (int i = tid; i < D; i += MERGE_THREADS) {
-      const float v = n_old ? fmaf((float)n_old, master[i], acc[i]) : acc[i];
-      acc[i] = v;
-      ss = fmaf(v, v, ss);
+    } else {
+      for (int i = tid; i < D; i += MERGE_THREADS) {
+        const float v = n_old ? fmaf((float)n_old, master[i], acc[i]) : acc[i];
+        acc[i] = v;
+        ss = fmaf(v, v, ss);
+      }
     }
 #pragma unroll
     for (int sft = 16; sft; sft >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, sft);
     if (lane == 0) red[warp] = ss;
     __syncthreads();
-    if (tid == 0) {
-      float tot = 0.f;
-      for (int w = 0; w < MERGE_WARPS; ++w) tot += red[w];
-      s_bcast = tot;
-    }
-    __syncthreads();
-    const float tot = s_bcast;
+    float tot = 0.f;
+#pragma unroll
+    for (int w = 0; w < MERGE_WARPS; ++w) tot += red[w];
     if (tot > 0.f) {  // a zero sum keeps the old value
       const float inv = 1.0f / sqrtf(tot);
       float s2 = 0.f;
-      for (int i = tid; i < D; i += MERGE_THREADS) {
-        const float v = acc[i] * inv;
-        master[i] = v;
-        const T sh = from_f32<T>(v);  // round-to-nearest-even shadow (R1, R14)
-        shadow[i] = sh;
-        const float sv = to_f32<T>(sh);
-        s2 = fmaf(sv, sv, s2);
+      if (vec && sizeof(T) == 2) {
+        for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
+          float v[8];
+          uint4 w;
+          T *e = reinterpret_cast<T *>(&w);
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            v[q] = acc[i + q] * inv;
+            e[q] = from_f32<T>(v[q]);  // round-to-nearest-even shadow (R1, R14)
+            const float sv = to_f32<T>(e[q]);
+            s2 = fmaf(sv, sv, s2);
+          }
+          *reinterpret_cast<float4 *>(master + i) = make_float4(v[0], v[1], v[2], v[3]);
+          *reinterpret_cast<float4 *>(master + i + 4) = make_float4(v[4], v[5], v[6], v[7]);
+          *reinterpret_cast<uint4 *>(shadow + i) = w;
+        }
+      } else {
+        for (int i = tid; i < D; i += MERGE_THREADS) {
+          const float v = acc[i] * inv;
+          master[i] = v;
+          const T sh = from_f32<T>(v);
+          shadow[i] = sh;
+          const float sv = to_f32<T>(sh);
+          s2 = fmaf(sv, sv, s2);
+        }
       }
 #pragma unroll
       for (int sft = 16; sft; sft >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, sft);
-      __syncthreads();
-      if (lane == 0) red[warp] = s2;
+      if (lane == 0) red2[warp] = s2;
       __syncthreads();
       if (tid == 0) {
         float t2 = 0.f;
-        for (int w = 0; w < MERGE_WARPS; ++w) t2 += red[w];
+#pragma unroll
+        for (int w = 0; w < MERGE_WARPS; ++w) t2 += red2[w];
         m.inv_norm[t] = t2 > 0.f ? 1.0f / sqrtf(t2) : 0.f;
       }
     }
     if (tid == 0) {
-      m.n_obs[t] = n_old_t0 + k_members;
+      m.n_obs[t] = n_old + k_members;
       m.n_points[t] = pts_old + pts;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {  // R22
@@ -345,7 +392,6 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       m.leader[t] = NONE32;
       m.grp_cnt[t] = 0;
     }
-    __syncthreads();
   }
 }
 
@@ -355,6 +401,16 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   if (m.dtype == FARM_DTYPE_F32) { using T = float; call; }   \
   else if (m.dtype == FARM_DTYPE_F16) { using T = __half; call; } \
   else { using T = __nv_bfloat16; call; }
+
+void configure_assoc_kernels() {
+  const int pref = (int)cudaSharedmemCarveoutMaxShared;
+  cudaFuncSetAttribute(cand_associate_kernel<float>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(cand_associate_kernel<__half>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(cand_associate_kernel<__nv_bfloat16>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(commit_merge_kernel<float>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(commit_merge_kernel<__half>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(commit_merge_kernel<__nv_bfloat16>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+}
 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int grid = a.M > 0 ? 37 : 1;  // 37 x 32 warps = one warp per candidate for ~1.2k candidates per wave

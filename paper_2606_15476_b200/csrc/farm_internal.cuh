@@ -203,6 +203,12 @@ template <>
 __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
 
 // host-side launchers (one per translation unit); each returns the number of kernels it launched
+// One-time kernel attributes.  Every kernel of the path asks for the maximum shared-memory carve-out: an SM cannot
+// change its L1/shared split while CTAs are resident, so a kernel with another preference would keep the
+// 197 KB similarity CTA off every SM it occupies (measured: the similarity grid then starts only when the other
+// kernel has drained).
+void configure_lift_kernels();
+void configure_assoc_kernels();
 int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);

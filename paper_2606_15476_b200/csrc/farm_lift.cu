@@ -100,9 +100,21 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
   if (warp >= a.M) return;
   const T *row = (const T *)a.desc + (size_t)warp * m.D;
   float s = 0.f;
-  for (int i = lane; i < m.D; i += 32) {
-    const float x = to_f32<T>(row[i]);
-    s = fmaf(x, x, s);
+  if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
+    for (int i = lane * 8; i < m.D; i += 256) {
+      const uint4 w = __ldg(reinterpret_cast<const uint4 *>(row + i));
+      const T *e = reinterpret_cast<const T *>(&w);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const float x = to_f32<T>(e[q]);
+        s = fmaf(x, x, s);
+      }
+    }
+  } else {
+    for (int i = lane; i < m.D; i += 32) {
+      const float x = to_f32<T>(row[i]);
+      s = fmaf(x, x, s);
+    }
   }
 #pragma unroll
   for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
@@ -262,6 +274,49 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
   return r;
 }
 
+// Rare path of the lift kernel: one pixel whose detection differs from the first detection of its thread.  It
+// is added on its own: count 1, box = the point, one voxel bit of its block.
+__device__ __noinline__ void stray_pixel(TileSmem &s, uint32_t *lab_j, uint32_t *lab_cnt, int (*lab_box)[6], uint32_t *det_npx,
+                                         int *det_box, unsigned long long *surv_key, unsigned long long *surv_bits,
+                                         uint32_t *surv_j, uint32_t surv_cap, uint32_t *counters, uint32_t *err, uint32_t j,
+                                         unsigned long long bkey, uint32_t bit, float p0, float p1, float p2) {
+  const int li = tile_label_slot_in(lab_j, j);
+  const int o0 = f2ord(p0), o1 = f2ord(p1), o2 = f2ord(p2);
+  const uint32_t lo = (bit & 32) ? 0u : 1u << (bit & 31), hi = (bit & 32) ? 1u << (bit & 31) : 0u;
+  if (li >= 0) {
+    atomicAdd(&lab_cnt[li], 1u);
+    atomicMin(&lab_box[li][0], o0), atomicMin(&lab_box[li][1], o1), atomicMin(&lab_box[li][2], o2);
+    atomicMax(&lab_box[li][3], o0), atomicMax(&lab_box[li][4], o1), atomicMax(&lab_box[li][5], o2);
+    const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
+    uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
+    for (int probe = 0; probe < TILE_ENT; ++probe) {
+      unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
+      if (cur == BLK_EMPTY) {
+        cur = atomicCAS(&s.tag[h], BLK_EMPTY, tag);
+        if (cur == BLK_EMPTY) cur = tag;
+      }
+      if (cur == tag) {
+        if (lo) atomicOr(&s.mlo[h], lo);
+        if (hi) atomicOr(&s.mhi[h], hi);
+        return;
+      }
+      h = (h + 1) & (TILE_ENT - 1);
+    }
+  } else {
+    atomicAdd(&det_npx[j], 1u);
+    atomicMin(&det_box[j * 6 + 0], o0), atomicMin(&det_box[j * 6 + 1], o1), atomicMin(&det_box[j * 6 + 2], o2);
+    atomicMax(&det_box[j * 6 + 3], o0), atomicMax(&det_box[j * 6 + 4], o1), atomicMax(&det_box[j * 6 + 5], o2);
+  }
+  const uint32_t pos = atomicAdd(&counters[2], 1u);
+  if (pos < surv_cap) {
+    surv_key[pos] = bkey;
+    surv_bits[pos] = ((unsigned long long)hi << 32) | lo;
+    surv_j[pos] = j;
+  } else {
+    atomicOr(err, ERR_PAIR_TABLE_FULL);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // lift kernel (steps 1-2).  Persistent CTAs; one 64x16 pixel tile per iteration, each thread owns 8
 // consecutive pixels of one row (2 x 128-bit depth loads + 1 x 128-bit mask load, issued one tile ahead).
@@ -278,7 +333,7 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
 // accumulators (REDUX fast path when a warp holds one detection) to one set of global atomics per
 // (tile, detection).
 template <bool VEC>
-__global__ void __launch_bounds__(LIFT_THREADS, 4) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+__global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads
   __shared__ uint32_t lab_cnt2[2][MAX_LABELS];  // its copy while tile t+1 initialises the other
@@ -350,14 +405,11 @@ __global__ void __launch_bounds__(LIFT_THREADS, 4) lift_voxelise_kernel(DevMap m
     const float u0f = (float)u0;  // (float)(u0 + i) == u0f + (float)i exactly (integers below 2^24)
     unsigned long long ikey[8];
     uint32_t ibit_lo = 0, ibit_hi = 0;  // 6-bit voxel index inside the block, pixels 0-3 / 4-7
-    float P0[8], P1[8], P2[8];
-    uint32_t valid = 0, L0 = 0;
-    bool multi = false;
+    uint32_t valid = 0, L0 = 0;         // pixels of the thread's first detection L0 (almost always the only one)
     float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       ikey[i] = BLK_EMPTY;
-      P0[i] = P1[i] = P2[i] = 0.f;
       const uint32_t l = lab[i];
       if (l != 0) {
         if (l > n_det_f) {
@@ -371,68 +423,52 @@ __global__ void __launch_bounds__(LIFT_THREADS, 4) lift_voxelise_kernel(DevMap m
           p[2] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c3.x, xc), __fmul_rn(c3.y, yc)), __fmul_rn(c3.z, z[i])), c3.w);
           uint32_t ix, iy, iz;
           if (voxel_index(p, inv_vs, ix, iy, iz)) {
-            valid |= 1u << i;
-            ikey[i] = block_key(ix, iy, iz);
+            acc_valid++;
+            const unsigned long long bk = block_key(ix, iy, iz);
             const uint32_t bit = block_bit(ix, iy, iz);
-            if (i < 4) ibit_lo |= bit << (6 * i); else ibit_hi |= bit << (6 * (i - 4));
-            P0[i] = p[0], P1[i] = p[1], P2[i] = p[2];
             if (L0 == 0) L0 = l;
-            multi |= l != L0;
-            mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
-            mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
+            if (l == L0) {
+              valid |= 1u << i;
+              ikey[i] = bk;
+              if (i < 4) ibit_lo |= bit << (6 * i); else ibit_hi |= bit << (6 * (i - 4));
+              mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
+              mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
+            } else {  // rare: the thread's 8 pixels straddle two detections -- this pixel goes in on its own
+              stray_pixel(s, lab_j, lab_cnt, lab_box, m.det_npx, m.det_box, m.surv_key, m.surv_bits, m.surv_j, m.surv_cap,
+                          m.counters, m.err, (uint32_t)det_base + l - 1, bk, bit, p[0], p[1], p[2]);
+            }
           } else {
             acc_dropped++;
           }
         }
       }
     }
-    acc_valid += __popc(valid);
 
-    // ---- phase 2: one round per detection present in the warp's threads (one round unless a thread straddles two)
-    const bool any_multi = __any_sync(FULL, multi);
-    uint32_t todo = valid;
-    while (__any_sync(FULL, todo != 0)) {
-      uint32_t L = L0, mine = todo;
-      float b0 = mn0, b1 = mn1, b2 = mn2, b3 = mx0, b4 = mx1, b5 = mx2;
-      if (any_multi) {  // warp-uniform slow path: restrict the round to the label of the thread's first open pixel
-        L = 0;
-#pragma unroll
-        for (int i = 7; i >= 0; --i)
-          if ((todo >> i) & 1u) L = lab[i];
-        mine = 0;
-        b0 = b1 = b2 = INF, b3 = b4 = b5 = -INF;
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-          if (((todo >> i) & 1u) && lab[i] == L) {
-            mine |= 1u << i;
-            b0 = fminf(b0, P0[i]), b1 = fminf(b1, P1[i]), b2 = fminf(b2, P2[i]);
-            b3 = fmaxf(b3, P0[i]), b4 = fmaxf(b4, P1[i]), b5 = fmaxf(b5, P2[i]);
-          }
-      }
-      todo &= ~mine;
-      const uint32_t j = (uint32_t)det_base + L - 1;
+    // ---- phase 2 (warp-synchronous): detection L0 of every thread
+    if (__any_sync(FULL, valid != 0)) {
+      const uint32_t j = (uint32_t)det_base + L0 - 1;
       int li = -1;
-      if (mine) li = tile_label_slot_in(lab_j, j);
+      if (valid) li = tile_label_slot_in(lab_j, j);
       // per-detection pixel count and point AABB (R7): REDUX when the warp holds one detection
       {
-        const unsigned has = __ballot_sync(FULL, mine != 0);
+        const unsigned has = __ballot_sync(FULL, valid != 0);
         const int src = __ffs(has) - 1;
-        const uint32_t lead_L = __shfl_sync(FULL, L, src);
+        const uint32_t lead_L = __shfl_sync(FULL, L0, src);
         const int lead_li = __shfl_sync(FULL, li, src);
-        const bool uniform = __all_sync(FULL, mine == 0 || L == lead_L);
-        const int o0 = f2ord(b0), o1 = f2ord(b1), o2 = f2ord(b2), o3 = f2ord(b3), o4 = f2ord(b4), o5 = f2ord(b5);
-        const uint32_t cnt = __popc(mine);
+        const bool uniform = __all_sync(FULL, valid == 0 || L0 == lead_L);
+        const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
+        const uint32_t cnt = __popc(valid);
         if (uniform) {
           const uint32_t tot = __reduce_add_sync(FULL, cnt);
           const int r0 = __reduce_min_sync(FULL, o0), r1 = __reduce_min_sync(FULL, o1), r2 = __reduce_min_sync(FULL, o2),
                     r3 = __reduce_max_sync(FULL, o3), r4 = __reduce_max_sync(FULL, o4), r5 = __reduce_max_sync(FULL, o5);
           if (lane == 0) label_add_in(lab_cnt, lab_box, m, lead_li, (uint32_t)det_base + lead_L - 1, tot, r0, r1, r2, r3, r4, r5);
-        } else if (mine) {
+        } else if (valid) {
           label_add_in(lab_cnt, lab_box, m, li, j, cnt, o0, o1, o2, o3, o4, o5);
         }
       }
-      // blocks of this detection: one pass per distinct block among the thread's pixels
-      uint32_t rem = mine;
+      // blocks: one pass per distinct block among the thread's pixels
+      uint32_t rem = valid;
       while (__any_sync(FULL, rem != 0)) {
         unsigned long long kb = BLK_EMPTY;
 #pragma unroll
@@ -670,7 +706,21 @@ __global__ void debug_backproject_kernel(DevMap m, const float *__restrict__ dep
   keys[i] = key;
 }
 
+template <typename K>
+void max_shared_carveout(K kernel) {
+  cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
 }  // namespace
+
+void configure_lift_kernels() {
+  max_shared_carveout(prep_kernel<float>);
+  max_shared_carveout(prep_kernel<__half>);
+  max_shared_carveout(prep_kernel<__nv_bfloat16>);
+  max_shared_carveout(lift_voxelise_kernel<true>);
+  max_shared_carveout(lift_voxelise_kernel<false>);
+  max_shared_carveout(probe_kernel);
+}
 
 int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int blocks = a.M > 0 ? (a.M + 3) / 4 : 1;
@@ -686,7 +736,8 @@ int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
   const int n_tiles = tiles_x * tiles_y * a.F;
-  const int grid = n_tiles < 148 * 4 ? n_tiles : 148 * 4;  // persistent: 4 resident CTAs per SM
+  // persistent, 4 CTAs per SM: 4 x 128 x 80 registers fit beside the similarity CTA (256 x 80) in the 64 K register file
+  const int grid = n_tiles < 148 * 4 ? n_tiles : 148 * 4;
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
   if (vec)
     lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);

@@ -11,7 +11,9 @@
 //   warp 0      TMA producer: A tile 128 x 64 and B tile 256 x 64 per stage, SWIZZLE_128B, 4-stage mbarrier ring
 //   warp 1      MMA issuer: one elected thread, tcgen05.mma.cta_group::1.kind::f16, UMMA 128 x 256 x 16
 //   warp 2      TMEM allocator (512 columns = two 128 x 256 fp32 accumulators, double buffered)
-//   warps 4-7   epilogue: tcgen05.ld 32 lanes x 32 columns at a time, one detection row per thread
+//   warps 4-7   epilogue: tcgen05.ld 32 lanes x 32 columns at a time, one detection row per lane, four independent
+//               (max, argmax) chains per thread so that the compare/select dependency chain stays short
+//               (EPI_SPLIT = 2 puts two warps on each TMEM lane quadrant, each scanning half of the columns)
 // Detections sit on the UMMA M axis (TMEM lanes) so that the per-detection max over objects is a scan
 // along TMEM columns inside one thread -- no cross-thread reduction.
 // N is read from device memory (no host sync); tiles are enumerated m-fastest so that concurrently
@@ -28,7 +30,9 @@ constexpr int BLOCK_N = 256;  // objects per tile (UMMA N)
 constexpr int BLOCK_K = 64;   // 64 x 16-bit = one 128-byte swizzle row
 constexpr int UMMA_K = 16;
 constexpr int STAGES = 4;
-constexpr int TC_THREADS = 256;
+constexpr int EPI_SPLIT = 1;    // epilogue warps per TMEM lane quadrant (each scans BLOCK_N / EPI_SPLIT columns)
+constexpr int EPI_THREADS = 128 * EPI_SPLIT;
+constexpr int TC_THREADS = 128 + EPI_THREADS;  // warps 0-2 producer / MMA / TMEM, warp 3 idle, then the epilogue warps
 constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2;  // 16 KB
 constexpr uint32_t B_BYTES = BLOCK_N * BLOCK_K * 2;  // 32 KB
 constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
@@ -106,7 +110,8 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-__global__ void __launch_bounds__(TC_THREADS, 1)
+// 80 registers per thread (no spills): 256 x 80 leaves room for four 128 x 80 lift CTAs on the same SM
+__global__ void __maxnreg__(80)
 similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
                      int M, uint32_t idesc) {
   extern __shared__ uint8_t smem_raw[];
@@ -133,7 +138,7 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&tfull_bar[i]), 1);
-      mbar_init(smem_u32(&tempty_bar[i]), 4);
+      mbar_init(smem_u32(&tempty_bar[i]), EPI_THREADS / 32);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -189,26 +194,29 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
       }
     }
   } else if (warp >= 4) {
-    // ===== epilogue: one detection row per thread =====
+    // ===== epilogue: one detection row per lane, half of the tile's columns per warp =====
     const int q = warp & 3;            // TMEM lane quadrant this warp may access
+    const int half = (warp - 4) >> 2;  // which BLOCK_N / EPI_SPLIT column range of the tile this warp scans
     const int row_in_tile = q * 32 + lane;
-    const int et = threadIdx.x - 128;  // 0..127
+    const int et = threadIdx.x - 128;  // 0..EPI_THREADS-1
     uint32_t as = 0, aphase = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       const int tm = tile % tiles_m, tn = tile / tiles_m;
       const int n0 = tn * BLOCK_N;
       const int ncols = min(BLOCK_N, N - n0);
       float *ib = ib_s + as * BLOCK_N;
-      ib[et] = et < ncols ? m.inv_norm[n0 + et] : 0.f;
-      ib[et + 128] = et + 128 < ncols ? m.inv_norm[n0 + et + 128] : 0.f;
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+#pragma unroll
+      for (int c = et; c < BLOCK_N; c += EPI_THREADS) ib[c] = c < ncols ? m.inv_norm[n0 + c] : 0.f;
+      asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
       mbar_wait(smem_u32(&tfull_bar[as]), aphase);
       tcgen05_fence_after();
-      float best = -3.0e38f;
-      int best_c = 0;
+      // four interleaved chains (columns = chain mod 4): strict > keeps the lowest column inside a chain
+      float bv[4] = {-3.0e38f, -3.0e38f, -3.0e38f, -3.0e38f};
+      int bc[4] = {0, 1, 2, 3};
+      const int cbeg = half * (BLOCK_N / EPI_SPLIT);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
 #pragma unroll 1
-      for (int c0 = 0; c0 < BLOCK_N; c0 += 32) {
+      for (int c0 = cbeg; c0 < cbeg + BLOCK_N / EPI_SPLIT; c0 += 32) {
         if (c0 >= ncols) break;
         uint32_t r[32];
         tmem_ld32(taddr + c0, r);
@@ -217,21 +225,27 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
 #pragma unroll
           for (int i = 0; i < 32; ++i) {
             const float v = __uint_as_float(r[i]) * ib[c0 + i];
-            if (v > best) best = v, best_c = c0 + i;
+            if (v > bv[i & 3]) bv[i & 3] = v, bc[i & 3] = c0 + i;
           }
         } else {
 #pragma unroll
           for (int i = 0; i < 32; ++i) {
             const float v = __uint_as_float(r[i]) * ib[c0 + i];
-            if (c0 + i < ncols && v > best) best = v, best_c = c0 + i;
+            if (c0 + i < ncols && v > bv[i & 3]) bv[i & 3] = v, bc[i & 3] = c0 + i;
           }
         }
       }
       tcgen05_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+      // combine the chains: larger value wins, equal values -> lower column (R18 tie rule)
+      float best = bv[0];
+      int best_c = bc[0];
+#pragma unroll
+      for (int k = 1; k < 4; ++k)
+        if (bv[k] > best || (bv[k] == best && bc[k] < best_c)) best = bv[k], best_c = bc[k];
       const int row = tm * BLOCK_M + row_in_tile;
-      if (row < M) {
+      if (row < M && cbeg < ncols) {
         const float ia = m.det_inv_norm[row];
         float cs = best * ia;
         cs = fminf(1.f, fmaxf(-1.f, cs));                    // R15 clamp
