@@ -125,9 +125,10 @@ int farm_map_integrate_batch(farm_map *m, int n_frames, const float *depth, cons
                              const float *K, const float *T_world_cam, const void *det_descriptors,
                              const int *n_det);
 
-/* Same call with HOST buffers (pinned memory recommended): the library copies the batch into its own
- * device staging buffers with cudaMemcpyAsync on the map's stream, then runs the identical kernels.
- * The host buffers may be reused once the stream has passed the copies (farm_map_sync / last_assoc). */
+/* Same call with HOST buffers (pinned memory recommended): the library copies the batch into one of its two
+ * device staging sets with cudaMemcpyAsync on an internal copy stream, then runs the identical kernels on the
+ * map's stream.  The call does not block: the copy of call t+1 overlaps the kernels of call t.  The host
+ * buffers may be reused once the map's stream has passed the call (farm_map_sync / farm_map_last_assoc). */
 int farm_map_integrate_batch_host(farm_map *m, int n_frames, const float *depth, const uint16_t *instance_mask,
                                   const float *K, const float *T_world_cam, const void *det_descriptors,
                                   const int *n_det);
@@ -136,6 +137,12 @@ int farm_map_integrate_batch_host(farm_map *m, int n_frames, const float *depth,
  * obj_id: object the detection was merged into (-1 = skipped, R8); is_new: 1 if that object was spawned by it;
  * best_score: R18.  Synchronises the stream; returns the sticky device error if set. */
 int farm_map_last_assoc(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score, farm_frame_stats *stats);
+
+/* Non-blocking form of farm_map_last_assoc: enqueues the device->host copies of the LAST call's results on the
+ * map's stream and returns.  The HOST buffers (pinned memory, else the copy blocks) are valid after the next
+ * farm_map_sync / farm_map_last_assoc / farm_map_read; the sticky device error is reported there. */
+int farm_map_last_assoc_async(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score,
+                              farm_frame_stats *stats);
 
 /* Export (HOST buffers).  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
  * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary

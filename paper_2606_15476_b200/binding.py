@@ -37,7 +37,8 @@ TOTALS_DTYPE = np.dtype([("frames", "<u8"), ("calls", "<u8"), ("valid_points", "
                          ("matches", "<u8"), ("spawns", "<u8")])
 
 EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm_map_set_option_f",
-           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_read",
+           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async",
+           "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
@@ -69,6 +70,7 @@ def load_library():
         lib.farm_map_integrate_batch_host.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp]
         lib.farm_map_stage_times.argtypes = [vp, vp, vp, ci]
         lib.farm_map_last_assoc.argtypes = [vp, vp, vp, vp, vp]
+        lib.farm_map_last_assoc_async.argtypes = [vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
         lib.farm_map_sync.argtypes = [vp, vp]
@@ -179,6 +181,15 @@ class FarmMap:
         st = np.zeros(1, STATS_DTYPE)
         _check(load_library().farm_map_last_assoc(self._h, _hp(obj), _hp(is_new), _hp(best), _hp(st)))
         return obj, is_new, best, st[0]
+
+    def last_assoc_async(self, obj_id, is_new, best_score, stats):
+        """Enqueue the D2H copies of the last call's results into pinned torch CPU tensors / numpy arrays (any may be
+        None); valid after the next sync()."""
+        def hp(x):
+            if x is None:
+                return None
+            return C.c_void_p(x.data_ptr()) if hasattr(x, "data_ptr") else _hp(x)
+        _check(load_library().farm_map_last_assoc_async(self._h, hp(obj_id), hp(is_new), hp(best_score), hp(stats)))
 
     def read(self, voxels=True, descriptors=True):
         lib = load_library()

@@ -56,10 +56,17 @@ struct farm_map {
   std::vector<cudaEvent_t> ev_free;
   double stage_ms[FARM_N_STAGES] = {};
   long long stage_launches[FARM_N_STAGES] = {};
-  // staging buffers of farm_map_integrate_batch_host
-  float *h_depth = nullptr, *h_K = nullptr, *h_T = nullptr;
-  uint16_t *h_mask = nullptr;
-  void *h_desc = nullptr;
+  // farm_map_integrate_batch_host: two device staging sets filled on a copy stream, so that the H2D copy of call
+  // t+1 overlaps the kernels of call t
+  struct Staging {
+    float *depth = nullptr, *K = nullptr, *T = nullptr;
+    uint16_t *mask = nullptr;
+    void *desc = nullptr;
+    cudaEvent_t copied = nullptr, free = nullptr;
+    bool used = false;
+  } stg[2];
+  cudaStream_t cstream = nullptr;
+  unsigned long long host_calls = 0;
   size_t elem() const { return dtype == FARM_DTYPE_F32 ? 4 : 2; }
 };
 
@@ -298,6 +305,7 @@ int finalise(farm_map *m) {
   A(d.ov_cnt, (size_t)ocap, 0);
   d.ov_mask = (uint32_t)(ocap - 1);
   A(d.cand_slot, (size_t)ccap, 0);
+  A(d.cand_key, (size_t)ccap, 0);
   A(d.cand_j, (size_t)ccap, 0);
   A(d.cand_o, (size_t)ccap, 0);
   A(d.cand_c, (size_t)ccap, 0);
@@ -389,6 +397,11 @@ int farm_map_destroy(farm_map *m) {
   if (!m) return FARM_OK;
   if (m->finalised || !m->allocs.empty()) cudaStreamSynchronize(m->stream);
   if (m->side) cudaStreamSynchronize(m->side), cudaStreamDestroy(m->side);
+  if (m->cstream) cudaStreamSynchronize(m->cstream), cudaStreamDestroy(m->cstream);
+  for (auto &g : m->stg) {
+    if (g.copied) cudaEventDestroy(g.copied);
+    if (g.free) cudaEventDestroy(g.free);
+  }
   if (m->ev_fork) cudaEventDestroy(m->ev_fork);
   if (m->ev_join) cudaEventDestroy(m->ev_join);
   if (m->tc) tc_state_destroy(m->tc);
@@ -709,20 +722,43 @@ int farm_map_integrate_batch_host(farm_map *m, int F, const float *depth, const 
   int rc = finalise(m);
   if (rc != FARM_OK) return rc;
   const size_t px = (size_t)m->H * m->W;
-  if (!m->h_depth) {  // device staging, sized for the largest call
-    void *p;
-    CU(cudaMalloc(&p, px * m->max_frames * 4)); m->allocs.push_back(p); m->h_depth = (float *)p;
-    CU(cudaMalloc(&p, px * m->max_frames * 2)); m->allocs.push_back(p); m->h_mask = (uint16_t *)p;
-    CU(cudaMalloc(&p, (size_t)m->max_frames * 9 * 4)); m->allocs.push_back(p); m->h_K = (float *)p;
-    CU(cudaMalloc(&p, (size_t)m->max_frames * 16 * 4)); m->allocs.push_back(p); m->h_T = (float *)p;
-    CU(cudaMalloc(&p, (size_t)m->max_det * m->D * m->elem())); m->allocs.push_back(p); m->h_desc = p;
+  if (!m->cstream) {  // device staging, sized for the largest call
+    CU(cudaStreamCreateWithFlags(&m->cstream, cudaStreamNonBlocking));
+    for (auto &g : m->stg) {
+      void *p;
+      CU(cudaMalloc(&p, px * m->max_frames * 4)); m->allocs.push_back(p); g.depth = (float *)p;
+      CU(cudaMalloc(&p, px * m->max_frames * 2)); m->allocs.push_back(p); g.mask = (uint16_t *)p;
+      CU(cudaMalloc(&p, (size_t)m->max_frames * 9 * 4)); m->allocs.push_back(p); g.K = (float *)p;
+      CU(cudaMalloc(&p, (size_t)m->max_frames * 16 * 4)); m->allocs.push_back(p); g.T = (float *)p;
+      CU(cudaMalloc(&p, (size_t)m->max_det * m->D * m->elem())); m->allocs.push_back(p); g.desc = p;
+      CU(cudaEventCreateWithFlags(&g.copied, cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&g.free, cudaEventDisableTiming));
+    }
   }
-  CU(cudaMemcpyAsync(m->h_depth, depth, px * F * 4, cudaMemcpyHostToDevice, m->stream));
-  CU(cudaMemcpyAsync(m->h_mask, mask, px * F * 2, cudaMemcpyHostToDevice, m->stream));
-  CU(cudaMemcpyAsync(m->h_K, K, (size_t)F * 36, cudaMemcpyHostToDevice, m->stream));
-  CU(cudaMemcpyAsync(m->h_T, T, (size_t)F * 64, cudaMemcpyHostToDevice, m->stream));
-  if (M) CU(cudaMemcpyAsync(m->h_desc, desc, (size_t)M * m->D * m->elem(), cudaMemcpyHostToDevice, m->stream));
-  return farm_map_integrate_batch(m, F, m->h_depth, m->h_mask, m->h_K, m->h_T, M ? m->h_desc : nullptr, n_det);
+  farm_map::Staging &g = m->stg[m->host_calls++ & 1];
+  if (g.used) CU(cudaStreamWaitEvent(m->cstream, g.free, 0));  // the call that last read this set has finished
+  CU(cudaMemcpyAsync(g.depth, depth, px * F * 4, cudaMemcpyHostToDevice, m->cstream));
+  CU(cudaMemcpyAsync(g.mask, mask, px * F * 2, cudaMemcpyHostToDevice, m->cstream));
+  CU(cudaMemcpyAsync(g.K, K, (size_t)F * 36, cudaMemcpyHostToDevice, m->cstream));
+  CU(cudaMemcpyAsync(g.T, T, (size_t)F * 64, cudaMemcpyHostToDevice, m->cstream));
+  if (M) CU(cudaMemcpyAsync(g.desc, desc, (size_t)M * m->D * m->elem(), cudaMemcpyHostToDevice, m->cstream));
+  CU(cudaEventRecord(g.copied, m->cstream));
+  CU(cudaStreamWaitEvent(m->stream, g.copied, 0));
+  rc = farm_map_integrate_batch(m, F, g.depth, g.mask, g.K, g.T, M ? g.desc : nullptr, n_det);
+  CU(cudaEventRecord(g.free, m->stream));
+  g.used = true;
+  return rc;
+}
+
+int farm_map_last_assoc_async(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score, farm_frame_stats *stats) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  const size_t M = (size_t)m->last_M;
+  if (obj_id && M) CU(cudaMemcpyAsync(obj_id, m->dm.assoc, M * 4, cudaMemcpyDeviceToHost, m->stream));
+  if (is_new && M) CU(cudaMemcpyAsync(is_new, m->dm.is_new, M, cudaMemcpyDeviceToHost, m->stream));
+  if (best_score && M) CU(cudaMemcpyAsync(best_score, m->dm.best_score, M * 4, cudaMemcpyDeviceToHost, m->stream));
+  if (stats) CU(cudaMemcpyAsync(stats, m->dm.stats, sizeof(CallStats), cudaMemcpyDeviceToHost, m->stream));
+  return FARM_OK;
 }
 
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset) {

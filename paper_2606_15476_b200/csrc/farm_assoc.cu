@@ -27,10 +27,10 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     const int D = m.D;
     for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < n_cand; c += warps) {
       const uint32_t slot = m.cand_slot[c];
-      const unsigned long long kv = m.ov_keys[slot];
+      const unsigned long long kv = m.cand_key[c];
       const uint32_t j = (uint32_t)(kv >> 32) & ((1u << DET_BITS) - 1);
       const uint32_t o = (uint32_t)kv;
-      const uint32_t cnt = m.ov_cnt[slot];
+      const uint32_t cnt = __ldcg(&m.ov_cnt[slot]);
       __syncwarp();
       if (lane == 0) {
         m.ov_cnt[slot] = 0;  // invariant: counts are zero between calls (the tables are epoch tagged)
@@ -67,6 +67,21 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
       }
     }
   }
+  // ---- everything the association scan needs except best_cand is final before this kernel starts: requested here,
+  // ahead of the ticket, so that the scan of the last CTA starts with its operands in registers (M <= 2048)
+  const uint32_t N = __ldcg(m.n_objects);
+  unsigned long long valid_points = 0;
+  if (tid == 0) valid_points = __ldcg(&m.stats->valid_points);
+  uint32_t pre_nv[2], pre_npx[2];
+  unsigned long long pre_bd[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    const int j = q * 1024 + tid;
+    const bool in = j < a.M;
+    pre_nv[q] = in ? __ldcg(&m.det_nv[j]) : 0u;
+    pre_npx[q] = in ? __ldcg(&m.det_npx[j]) : 0u;
+    pre_bd[q] = in ? __ldcg(&m.best_dense[j]) : 0ull;
+  }
   // ---- ticket: the last CTA to arrive runs the association
   __syncthreads();
   if (tid == 0) {
@@ -79,22 +94,23 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  const uint32_t N = __ldcg(m.n_objects);
-  unsigned long long valid_points = 0;
-  if (tid == 0) valid_points = __ldcg(&m.stats->valid_points);
   for (int base = 0; base < a.M; base += 1024) {
     const int j = base + tid;
+    const int q = base >> 10;
     uint32_t spawn = 0, matched = 0, skipped = 0;
     int32_t target = -1;
     float score = 0.f;
-    const uint32_t nv = __reduce_add_sync(0xFFFFFFFFu, j < a.M ? __ldcg(&m.det_nv[j]) : 0u);
+    const bool in = j < a.M;
+    const uint32_t my_nv = q == 0 ? pre_nv[0] : q == 1 ? pre_nv[1] : (in ? __ldcg(&m.det_nv[j]) : 0u);
+    const uint32_t my_npx = q == 0 ? pre_npx[0] : q == 1 ? pre_npx[1] : (in ? __ldcg(&m.det_npx[j]) : 0u);
+    const unsigned long long bd = q == 0 ? pre_bd[0] : q == 1 ? pre_bd[1] : (in ? __ldcg(&m.best_dense[j]) : 0ull);
+    const uint32_t nv = __reduce_add_sync(0xFFFFFFFFu, my_nv);
     if (lane == 0 && nv) atomicAdd(&s_uvox, (unsigned long long)nv);
-    if (j < a.M) {
-      if (__ldcg(&m.det_npx[j]) == 0) {
+    if (in) {
+      if (my_npx == 0) {
         skipped = 1;  // R8
       } else {
         unsigned long long best = __ldcg(&m.best_cand[j]);
-        const unsigned long long bd = __ldcg(&m.best_dense[j]);
         if (bd) {
           // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
           const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd)));
@@ -168,8 +184,8 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
 }
 
 // ---- voxel commit + object merge, one launch.
-// CTAs [0, commit_blocks): R12 pass 2 -- the claim winner of every key inserted by this call sets the owner.
-// CTAs [commit_blocks, ...): the lowest-index detection of every target object folds the whole group
+// The last commit_blocks CTAs: R12 pass 2 -- the claim winner of every voxel inserted by this call sets the owner.
+// The CTAs before them (one per detection): the lowest-index detection of every target object folds the whole group
 //   (R21 count-weighted descriptor mean, R22 AABB, R23 view evidence).  No atomics on the object, deterministic
 //   summation order.  Groups of one (the common case) skip the member scan.
 constexpr int MERGE_THREADS = 128, MERGE_WARPS = MERGE_THREADS / 32;
@@ -182,12 +198,14 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   __shared__ uint32_t warp_cnt[MERGE_WARPS];
   __shared__ float red[MERGE_WARPS], red2[MERGE_WARPS];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if ((int)blockIdx.x < commit_blocks) {
+  const int merge_blocks = gridDim.x - commit_blocks;
+  if ((int)blockIdx.x >= merge_blocks) {  // the long-running merge CTAs come first in launch order
+    const uint32_t cb = blockIdx.x - merge_blocks;
     // 8 lanes per event (one 32-byte owner sector each), 4 events per warp and step
     const uint32_t n = min(m.counters[0], m.pair_cap);
     const int sec = lane & 7;
     const uint32_t step = (uint32_t)commit_blocks * MERGE_WARPS * 4;
-    for (uint32_t e0 = (blockIdx.x * MERGE_WARPS + warp) * 4; e0 < n; e0 += step) {
+    for (uint32_t e0 = (cb * MERGE_WARPS + warp) * 4; e0 < n; e0 += step) {
       const uint32_t e = e0 + (lane >> 3);
       int32_t t = -1;
       uint32_t cnt = 0;
@@ -222,10 +240,9 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
     return;
   }
   const int D = m.D;
-  const int merge_blocks = gridDim.x - commit_blocks;
   // 8 elements per thread and step (128-bit loads of the storage-dtype rows, 2 x 128-bit of the fp32 masters)
   const bool vec = (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
-  for (int j = blockIdx.x - commit_blocks; j < a.M; j += merge_blocks) {
+  for (int j = blockIdx.x; j < a.M; j += merge_blocks) {
     const int32_t t = m.assoc[j];
     if (t < 0) continue;                                   // uniform per CTA
     const uint32_t lead = __ldcg(&m.leader[t]), group = __ldcg(&m.grp_cnt[t]);
@@ -419,7 +436,7 @@ int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
-  const int commit_blocks = 148 * 8;
+  const int commit_blocks = 148 * 4;
   const int merge_blocks = a.M < 148 * 16 ? a.M : 148 * 16;  // one CTA per detection: a single wave
   FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, MERGE_THREADS, (size_t)m.D * sizeof(float), s>>>(
       m, a, frame_seq0, commit_blocks)));

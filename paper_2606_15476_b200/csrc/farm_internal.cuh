@@ -91,6 +91,7 @@ struct DevMap {
   uint32_t *ov_cnt;
   uint32_t ov_mask;
   uint32_t *cand_slot;               // list of overlap-map slots created this call
+  unsigned long long *cand_key;      //   and their (epoch, j, owner) keys, so that scoring needs no dependent lookup
   uint32_t cand_cap;
   uint32_t *cand_j;                  // compact copy for the debug read
   int32_t *cand_o;

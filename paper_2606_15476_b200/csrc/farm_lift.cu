@@ -643,7 +643,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
             } else {
               if (r == 1) {
                 const uint32_t c = atomicAdd(&m.counters[1], 1u);
-                if (c < m.cand_cap) m.cand_slot[c] = os; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+                if (c < m.cand_cap) m.cand_slot[c] = os, m.cand_key[c] = ov; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
               }
               atomicAdd(&m.ov_cnt[os], 1u);
             }
@@ -665,7 +665,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
           } else {
             if (r == 1) {
               const uint32_t c = atomicAdd(&m.counters[1], 1u);
-              if (c < m.cand_cap) m.cand_slot[c] = os; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+              if (c < m.cand_cap) m.cand_slot[c] = os, m.cand_key[c] = ov; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
             }
             atomicAdd(&m.ov_cnt[os], tot);
           }

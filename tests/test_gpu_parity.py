@@ -245,6 +245,37 @@ def test_host_buffer_entry_point_matches_device_path(oracle):
     compare_maps(g, o)
 
 
+def test_pipelined_host_calls_with_async_result_reads(oracle):
+    """Back-to-back host-buffer calls (copy of call t+1 overlaps the kernels of call t, two staging sets) with
+    non-blocking result reads: every call's results and the final map equal the oracle's."""
+    import torch
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    from helpers import stack_frames
+    n_calls, expected, got, keep = 7, [], [], []
+    for k in range(n_calls):
+        fr = sc.frame(k)
+        integrate_frames(o, [fr])
+        ao, no, bo, so, sto = o.last_assoc()
+        expected.append((ao.copy(), no.copy(), bo.copy()))
+        depth, mask, K, T, desc, n_det = stack_frames([fr])
+        pins = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in (depth, mask.view(np.int16), K, T, desc)]
+        keep.append(pins)                                   # host buffers stay alive until the sync
+        g.integrate_batch_host(1, pins[0], pins[1], pins[2], pins[3], pins[4], n_det)
+        M = int(n_det.sum())
+        res = (torch.empty(M, dtype=torch.int32).pin_memory(), torch.empty(M, dtype=torch.uint8).pin_memory(),
+               torch.empty(M, dtype=torch.float32).pin_memory())
+        g.last_assoc_async(res[0], res[1], res[2], None)
+        got.append(res)
+    g.sync()
+    for (ao, no, bo), (ag, ng, bg) in zip(expected, got):
+        assert np.array_equal(ag.numpy(), ao)
+        assert np.array_equal(ng.numpy(), no)
+        assert np.abs(bg.numpy() - bo).max(initial=0) <= 1e-4
+    compare_maps(g, o)
+
+
 def test_tile_queue_overflow_every_pixel_its_own_voxel(oracle):
     """Degenerate case: (almost) every pixel of a tile lands in its own voxel, more distinct pairs per tile
     than the lift kernel's shared-memory queue holds (overflow goes straight to the global queue)."""
