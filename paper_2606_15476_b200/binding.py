@@ -204,6 +204,13 @@ class FarmMap:
                                  C.byref(nv) if voxels else None))
         return objs, desc, keys, owners
 
+    def counts(self):
+        """(number of objects, number of owned voxels) without copying the map out."""
+        n = C.c_int(0)
+        nv = C.c_longlong(0)
+        _check(load_library().farm_map_read(self._h, None, C.byref(n), None, None, None, C.byref(nv)))
+        return n.value, nv.value
+
     def import_(self, objects, descriptors, voxel_keys, voxel_owner):
         objects = np.ascontiguousarray(objects, OBJECT_DTYPE)
         descriptors = np.ascontiguousarray(descriptors, np.float32)
