@@ -16,8 +16,8 @@ constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 //   exclusive scan in detection index order (R20), per-target leader / group size for the merge.
 template <typename T>
 __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs a) {
-  __shared__ uint32_t warp_sum[32];
-  __shared__ uint32_t s_running, s_matches, s_skipped;
+  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per chunk of 1024 detections
+  __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -89,11 +89,12 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     const uint32_t t = atomicAdd(&m.counters[3], 1u);
     s_last = t == gridDim.x - 1;
     if (s_last) m.counters[3] = 0;
-    s_running = 0, s_matches = 0, s_skipped = 0, s_uvox = 0ull;
+    s_matches = 0, s_skipped = 0, s_uvox = 0ull;
   }
   __syncthreads();
   if (!s_last) return;
   __threadfence();
+  uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier chunks (every thread)
   for (int base = 0; base < a.M; base += 1024) {
     const int j = base + tid;
     const int q = base >> 10;
@@ -104,8 +105,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     const uint32_t my_nv = q == 0 ? pre_nv[0] : q == 1 ? pre_nv[1] : (in ? __ldcg(&m.det_nv[j]) : 0u);
     const uint32_t my_npx = q == 0 ? pre_npx[0] : q == 1 ? pre_npx[1] : (in ? __ldcg(&m.det_npx[j]) : 0u);
     const unsigned long long bd = q == 0 ? pre_bd[0] : q == 1 ? pre_bd[1] : (in ? __ldcg(&m.best_dense[j]) : 0ull);
-    const uint32_t nv = __reduce_add_sync(0xFFFFFFFFu, my_nv);
-    if (lane == 0 && nv) atomicAdd(&s_uvox, (unsigned long long)nv);
+    nv_sum += my_nv;
     if (in) {
       if (my_npx == 0) {
         skipped = 1;  // R8
@@ -127,17 +127,19 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
         spawn = matched ? 0u : 1u;
       }
     }
-    // block exclusive scan of the spawn flags
+    // block exclusive scan of the spawn flags: ballot inside the warp, shuffle scan over the 32 warp counts
     const unsigned b = __ballot_sync(0xFFFFFFFFu, spawn);
-    if (lane == 0) warp_sum[warp] = __popc(b);
+    uint32_t *ws = warp_sum2[q & 1];
+    if (lane == 0) ws[warp] = __popc(b);
     __syncthreads();
-    uint32_t before = 0, total = 0;
-    for (int w = 0; w < 32; ++w) {
-      const uint32_t c = warp_sum[w];
-      before += w < warp ? c : 0;
-      total += c;
+    uint32_t incl = ws[lane];
+#pragma unroll
+    for (int sft = 1; sft < 32; sft <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, sft);
+      if (lane >= sft) incl += up;
     }
-    const uint32_t running = s_running;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    const uint32_t before = __shfl_sync(0xFFFFFFFFu, incl, warp) - __shfl_sync(0xFFFFFFFFu, ws[lane], warp);
     if (spawn) {
       const uint32_t id = N + running + before + __popc(b & ((1u << lane) - 1));
       if (id < m.max_objects) {
@@ -147,7 +149,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
         spawn = 0, skipped = 1;
       }
     }
-    if (j < a.M) {
+    if (in) {
       m.assoc[j] = target;
       m.is_new[j] = (uint8_t)spawn;
       m.best_score[j] = score;
@@ -156,17 +158,20 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
         atomicAdd(&m.grp_cnt[target], 1u);
       }
     }
-    const unsigned bm = __ballot_sync(0xFFFFFFFFu, matched), bs = __ballot_sync(0xFFFFFFFFu, skipped);
-    if (lane == 0) {
-      if (bm) atomicAdd(&s_matches, (uint32_t)__popc(bm));
-      if (bs) atomicAdd(&s_skipped, (uint32_t)__popc(bs));
-    }
-    __syncthreads();
-    if (tid == 0) s_running = running + total;
-    __syncthreads();
+    n_matched += matched, n_skipped += skipped;
+    running += total;
   }
+  n_matched = __reduce_add_sync(0xFFFFFFFFu, n_matched);
+  n_skipped = __reduce_add_sync(0xFFFFFFFFu, n_skipped);
+  nv_sum = __reduce_add_sync(0xFFFFFFFFu, nv_sum);
+  if (lane == 0) {
+    if (n_matched) atomicAdd(&s_matches, n_matched);
+    if (n_skipped) atomicAdd(&s_skipped, n_skipped);
+    if (nv_sum) atomicAdd(&s_uvox, (unsigned long long)nv_sum);
+  }
+  __syncthreads();
   if (tid == 0) {
-    uint32_t spawns = s_running;
+    uint32_t spawns = running;
     if (N + spawns > m.max_objects) spawns = m.max_objects - N;
     const unsigned long long pairs = s_uvox;
     *m.n_objects = N + spawns;
@@ -188,82 +193,118 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
 // The CTAs before them (one per detection): the lowest-index detection of every target object folds the whole group
 //   (R21 count-weighted descriptor mean, R22 AABB, R23 view evidence).  No atomics on the object, deterministic
 //   summation order.  Groups of one (the common case) skip the member scan.
-constexpr int MERGE_THREADS = 128, MERGE_WARPS = MERGE_THREADS / 32;
+constexpr int MERGE_THREADS = 256, MERGE_WARPS = MERGE_THREADS / 32;
+constexpr int MLIST = 64;  // members of one target object kept in shared memory; larger groups are re-scanned
 
 template <typename T>
 __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0,
                                                            int commit_blocks) {
-  extern __shared__ float acc[];  // [D]
-  __shared__ uint32_t list[MERGE_THREADS];
-  __shared__ uint32_t warp_cnt[MERGE_WARPS];
-  __shared__ float red[MERGE_WARPS], red2[MERGE_WARPS];
+  __shared__ uint32_t mlist[MERGE_WARPS][MLIST];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int merge_blocks = gridDim.x - commit_blocks;
-  if ((int)blockIdx.x >= merge_blocks) {  // the long-running merge CTAs come first in launch order
+  if ((int)blockIdx.x >= merge_blocks) {  // the merge CTAs come first in launch order
     const uint32_t cb = blockIdx.x - merge_blocks;
-    // 8 lanes per event (one 32-byte owner sector each), 4 events per warp and step
+    // 8 lanes per event (one 32-byte owner sector each), 4 events per warp and group, two groups in flight
     const uint32_t n = min(m.counters[0], m.pair_cap);
     const int sec = lane & 7;
-    const uint32_t step = (uint32_t)commit_blocks * MERGE_WARPS * 4;
-    for (uint32_t e0 = (cb * MERGE_WARPS + warp) * 4; e0 < n; e0 += step) {
-      const uint32_t e = e0 + (lane >> 3);
-      int32_t t = -1;
-      uint32_t cnt = 0;
-      if (e < n) {
-        const uint32_t jp = m.pl_j[e];
-        if (sec == 0) m.pair_bits[m.pl_ps[e]] = 0ull;  // invariant: the pair set's voxel bits are zero between calls
-        const uint32_t byte = (uint32_t)(m.pl_bits[e] >> (8 * sec)) & 0xFFu;
-        if ((jp >> 31) && byte) {  // some voxel of the event was unowned at entry
-          const uint32_t j = jp & 0x7FFFFFFFu;
-          t = m.assoc[j];
-          uint32_t *base = m.blk_owner + (size_t)m.pl_slot[e] * BLK_VOXELS + sec * 8;
-          const uint4 w0 = __ldcg(reinterpret_cast<const uint4 *>(base));
-          const uint4 w1 = __ldcg(reinterpret_cast<const uint4 *>(base) + 1);
-          const uint32_t own[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
-          if (t >= 0) {
+    const uint32_t half = (uint32_t)commit_blocks * MERGE_WARPS * 4;
+    for (uint32_t e0 = (cb * MERGE_WARPS + warp) * 4; e0 < n; e0 += 2 * half) {
+      uint32_t e[2], jp[2], slot[2], byte[2], own[2][8];
+      int32_t t[2] = {-1, -1};
+      uint32_t cnt[2] = {0, 0};
+      bool act[2];
 #pragma unroll
-            for (int b = 0; b < 8; ++b)
-              if (((byte >> b) & 1u) && own[b] == (OWNER_PENDING | j)) {  // this detection holds the claim (R12)
-                base[b] = (uint32_t)t;
-                cnt++;
-              }
-          }
-        }
+      for (int u = 0; u < 2; ++u) {  // stage 1: the event records
+        e[u] = e0 + u * half + (lane >> 3);
+        act[u] = e[u] < n;
+        jp[u] = act[u] ? m.pl_j[e[u]] : 0u;
+        slot[u] = act[u] ? m.pl_slot[e[u]] : 0u;
+        byte[u] = act[u] ? (uint32_t)(m.pl_bits[e[u]] >> (8 * sec)) & 0xFFu : 0u;
+        if (act[u] && sec == 0) m.pair_bits[m.pl_ps[e[u]]] = 0ull;  // invariant: pair-set voxel bits are zero between calls
+        act[u] = act[u] && (jp[u] >> 31) && byte[u];              // some voxel of the event was unowned at entry
       }
-      const unsigned act = __ballot_sync(0xFFFFFFFFu, cnt != 0);
-      if (cnt) {
-        const unsigned same = __match_any_sync(act, t);
-        const uint32_t tot = __reduce_add_sync(same, cnt);
-        if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t], tot);
+#pragma unroll
+      for (int u = 0; u < 2; ++u)  // stage 2: target object and owner sector
+        if (act[u]) {
+          t[u] = m.assoc[jp[u] & 0x7FFFFFFFu];
+          const uint4 *base = reinterpret_cast<const uint4 *>(m.blk_owner + (size_t)slot[u] * BLK_VOXELS + sec * 8);
+          const uint4 w0 = __ldcg(base), w1 = __ldcg(base + 1);
+          own[u][0] = w0.x, own[u][1] = w0.y, own[u][2] = w0.z, own[u][3] = w0.w;
+          own[u][4] = w1.x, own[u][5] = w1.y, own[u][6] = w1.z, own[u][7] = w1.w;
+        }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {  // stage 3: the claim winner sets the owner (R12)
+        if (act[u] && t[u] >= 0) {
+          uint32_t *base = m.blk_owner + (size_t)slot[u] * BLK_VOXELS + sec * 8;
+          const uint32_t mine = OWNER_PENDING | (jp[u] & 0x7FFFFFFFu);
+#pragma unroll
+          for (int b = 0; b < 8; ++b)
+            if (((byte[u] >> b) & 1u) && own[u][b] == mine) {
+              base[b] = (uint32_t)t[u];
+              cnt[u]++;
+            }
+        }
+        const unsigned am = __ballot_sync(0xFFFFFFFFu, cnt[u] != 0);
+        if (cnt[u]) {
+          const unsigned same = __match_any_sync(am, t[u]);
+          const uint32_t tot = __reduce_add_sync(same, cnt[u]);
+          if (lane == __ffs(same) - 1) atomicAdd(&m.n_voxels[t[u]], tot);
+        }
       }
     }
     return;
   }
+  // ---- merge: one WARP per detection; only the lowest-index detection of a target object works (R21-R23)
+  const int j = blockIdx.x * MERGE_WARPS + warp;
+  if (j >= a.M) return;
+  const int32_t t = m.assoc[j];
+  if (t < 0) return;
+  const uint32_t lead = __ldcg(&m.leader[t]), group = __ldcg(&m.grp_cnt[t]);
+  if (lead != (uint32_t)j) return;
   const int D = m.D;
-  // 8 elements per thread and step (128-bit loads of the storage-dtype rows, 2 x 128-bit of the fp32 masters)
-  const bool vec = (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
-  for (int j = blockIdx.x; j < a.M; j += merge_blocks) {
-    const int32_t t = m.assoc[j];
-    if (t < 0) continue;                                   // uniform per CTA
-    const uint32_t lead = __ldcg(&m.leader[t]), group = __ldcg(&m.grp_cnt[t]);
-    if (lead != (uint32_t)j) continue;
-    // everything the fold needs is requested up front so that the loads overlap
-    const uint32_t n_old = m.n_obs[t];
-    float *master = m.desc_master + (size_t)t * D;
-    T *shadow = (T *)m.desc_shadow + (size_t)t * D;
-    unsigned long long pts_old = 0, best_old = 0;
-    int box_old[6];
-    if (tid == 0) {
-      pts_old = m.n_points[t];
-      best_old = m.best_view[t];
-#pragma unroll
-      for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
+  const uint32_t n_old = m.n_obs[t];
+  const float nf = (float)n_old;
+  float *master = m.desc_master + (size_t)t * D;
+  T *shadow = (T *)m.desc_shadow + (size_t)t * D;
+  const T *desc = (const T *)a.desc;
+  // members in index order (deterministic summation): kept in shared memory when they fit
+  uint32_t n_listed = 1;
+  if (group > 1) {
+    n_listed = 0;
+    for (int base = j & ~31; base < a.M && n_listed < MLIST; base += 32) {
+      const int jj = base + lane;
+      const bool flag = jj < a.M && jj >= j && m.assoc[jj] == t;
+      const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
+      const uint32_t pos = n_listed + __popc(b & ((1u << lane) - 1));
+      if (flag && pos < MLIST) mlist[warp][pos] = (uint32_t)jj;
+      n_listed += __popc(b);
     }
-    uint32_t k_members = 0;
-    unsigned long long pts = 0, best = 0;
-    int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
-    int best_frame = -1;
-    auto member_evidence = [&](uint32_t jm) {  // thread 0: R22 / R23 contribution of one member
+    __syncwarp();
+  }
+  const bool listed = group <= MLIST;
+  // f(jm) for every member jm of the group, ascending
+  auto for_each_member = [&](auto &&f) {
+    if (group <= 1) {
+      f((uint32_t)j);
+    } else if (listed) {
+      for (uint32_t k = 0; k < group; ++k) f(mlist[warp][k]);
+    } else {
+      for (int jj = j; jj < a.M; ++jj)
+        if (m.assoc[jj] == t) f((uint32_t)jj);
+    }
+  };
+  // lane 0: view evidence and point box of the members (R22, R23); its loads overlap the descriptor work
+  uint32_t k_members = 0;
+  unsigned long long pts = 0, best = 0, pts_old = 0, best_old = 0;
+  int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+  int box_old[6] = {0, 0, 0, 0, 0, 0};
+  int best_frame = -1;
+  if (lane == 0) {
+    pts_old = m.n_points[t];
+    best_old = m.best_view[t];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
+    for_each_member([&](uint32_t jm) {
       k_members++;
       const uint32_t npx = m.det_npx[jm];
       pts += npx;
@@ -280,135 +321,102 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       const unsigned long long pv = ((unsigned long long)(npx & 0xFFFFFFu) << 40) | ((~seq & 0xFFFFFFull) << 16) |
                                     (unsigned long long)(~det & 0xFFFFu);
       if (pv > best) best = pv, best_frame = f;
-    };
-    auto add_row = [&](uint32_t jm, bool first) {  // acc (+)= a_jm / |a_jm|; zero-norm rows contribute nothing (R21)
-      const float inv = m.det_inv_norm[jm];
-      const T *row = (const T *)a.desc + (size_t)jm * D;
-      if (vec && sizeof(T) == 2) {
-        for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
-          const uint4 w = *reinterpret_cast<const uint4 *>(row + i);
-          const T *e = reinterpret_cast<const T *>(&w);
+    });
+  }
+  // f_o <- normalise(n_obs * f_o + sum_m a_m / |a_m|)   (R21).  Two passes over the rows (the second one hits
+  // L1/L2): pass 1 the squared norm, pass 2 the same values again, scaled and written with their shadows.
+  const bool vec = sizeof(T) == 2 && group <= 1 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
+  auto value = [&](int i) -> float {  // generic path, one element
+    float acc = 0.f;
+    bool first = true;
+    for_each_member([&](uint32_t jm) {
+      const float x = to_f32<T>(desc[(size_t)jm * D + i]), inv = m.det_inv_norm[jm];  // zero-norm rows contribute nothing
+      acc = first ? x * inv : fmaf(x, inv, acc);
+      first = false;
+    });
+    return n_old ? fmaf(nf, master[i], acc) : acc;
+  };
+  const float inv_j = m.det_inv_norm[j];
+  const T *row_j = desc + (size_t)j * D;
+  auto value8 = [&](int i, float (&v)[8]) {  // vector path: the leader is the only member
+    const uint4 w = *reinterpret_cast<const uint4 *>(row_j + i);
+    const T *e = reinterpret_cast<const T *>(&w);
+    float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0;
+    if (n_old) m0 = *reinterpret_cast<const float4 *>(master + i), m1 = *reinterpret_cast<const float4 *>(master + i + 4);
+    const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
 #pragma unroll
-          for (int q = 0; q < 8; ++q) acc[i + q] = first ? to_f32<T>(e[q]) * inv : fmaf(to_f32<T>(e[q]), inv, acc[i + q]);
-        }
-      } else {
-        for (int i = tid; i < D; i += MERGE_THREADS) acc[i] = first ? to_f32<T>(row[i]) * inv : fmaf(to_f32<T>(row[i]), inv, acc[i]);
-      }
-    };
-    __syncthreads();  // acc of the previous iteration is no longer read
-    if (group <= 1) {  // the common case: the leader is the only member
-      add_row((uint32_t)j, true);
-      if (tid == 0) member_evidence((uint32_t)j);
-    } else {
-      bool first = true;
-      for (int base = j & ~(MERGE_THREADS - 1); base < a.M; base += MERGE_THREADS) {  // members have index >= j
-        const int jj = base + tid;
-        const bool flag = jj < a.M && jj >= j && m.assoc[jj] == t;
-        const unsigned b = __ballot_sync(0xFFFFFFFFu, flag);
-        if (lane == 0) warp_cnt[warp] = __popc(b);
-        __syncthreads();
-        uint32_t before = 0, total = 0;
-#pragma unroll
-        for (int w = 0; w < MERGE_WARPS; ++w) {
-          before += w < warp ? warp_cnt[w] : 0;
-          total += warp_cnt[w];
-        }
-        if (flag) list[before + __popc(b & ((1u << lane) - 1))] = (uint32_t)jj;
-        __syncthreads();
-        for (uint32_t q = 0; q < total; ++q) {  // members in index order: deterministic summation
-          add_row(list[q], first);
-          first = false;
-          if (tid == 0) member_evidence(list[q]);
-        }
-        __syncthreads();
-      }
+    for (int q = 0; q < 8; ++q) {
+      const float x = to_f32<T>(e[q]) * inv_j;
+      v[q] = n_old ? fmaf(nf, mv[q], x) : x;
     }
-    // f_o <- normalise(n_obs * f_o + sum)   (R21); each thread revisits exactly the elements it accumulated
-    float ss = 0.f;
-    if (vec && sizeof(T) == 2) {
-      for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
-        float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0;
-        if (n_old) m0 = *reinterpret_cast<const float4 *>(master + i), m1 = *reinterpret_cast<const float4 *>(master + i + 4);
-        const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+  };
+  float ss = 0.f;
+  if (vec) {
+    for (int i = lane * 8; i < D; i += 256) {
+      float v[8];
+      value8(i, v);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) ss = fmaf(v[q], v[q], ss);
+    }
+  } else {
+    for (int i = lane; i < D; i += 32) {
+      const float v = value(i);
+      ss = fmaf(v, v, ss);
+    }
+  }
+#pragma unroll
+  for (int sft = 16; sft; sft >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, sft);
+  if (ss > 0.f) {  // a zero sum keeps the old value
+    const float inv = 1.0f / sqrtf(ss);
+    float s2 = 0.f;
+    if (vec) {
+      for (int i = lane * 8; i < D; i += 256) {
+        float v[8];
+        value8(i, v);
+        uint4 w;
+        T *e = reinterpret_cast<T *>(&w);
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-          const float v = n_old ? fmaf((float)n_old, mv[q], acc[i + q]) : acc[i + q];
-          acc[i + q] = v;
-          ss = fmaf(v, v, ss);
-        }
-      }
-    } else {
-      for (int i = tid; i < D; i += MERGE_THREADS) {
-        const float v = n_old ? fmaf((float)n_old, master[i], acc[i]) : acc[i];
-        acc[i] = v;
-        ss = fmaf(v, v, ss);
-      }
-    }
-#pragma unroll
-    for (int sft = 16; sft; sft >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, sft);
-    if (lane == 0) red[warp] = ss;
-    __syncthreads();
-    float tot = 0.f;
-#pragma unroll
-    for (int w = 0; w < MERGE_WARPS; ++w) tot += red[w];
-    if (tot > 0.f) {  // a zero sum keeps the old value
-      const float inv = 1.0f / sqrtf(tot);
-      float s2 = 0.f;
-      if (vec && sizeof(T) == 2) {
-        for (int i = tid * 8; i < D; i += MERGE_THREADS * 8) {
-          float v[8];
-          uint4 w;
-          T *e = reinterpret_cast<T *>(&w);
-#pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            v[q] = acc[i + q] * inv;
-            e[q] = from_f32<T>(v[q]);  // round-to-nearest-even shadow (R1, R14)
-            const float sv = to_f32<T>(e[q]);
-            s2 = fmaf(sv, sv, s2);
-          }
-          *reinterpret_cast<float4 *>(master + i) = make_float4(v[0], v[1], v[2], v[3]);
-          *reinterpret_cast<float4 *>(master + i + 4) = make_float4(v[4], v[5], v[6], v[7]);
-          *reinterpret_cast<uint4 *>(shadow + i) = w;
-        }
-      } else {
-        for (int i = tid; i < D; i += MERGE_THREADS) {
-          const float v = acc[i] * inv;
-          master[i] = v;
-          const T sh = from_f32<T>(v);
-          shadow[i] = sh;
-          const float sv = to_f32<T>(sh);
+          v[q] *= inv;
+          e[q] = from_f32<T>(v[q]);  // round-to-nearest-even shadow (R1, R14)
+          const float sv = to_f32<T>(e[q]);
           s2 = fmaf(sv, sv, s2);
         }
+        *reinterpret_cast<float4 *>(master + i) = make_float4(v[0], v[1], v[2], v[3]);
+        *reinterpret_cast<float4 *>(master + i + 4) = make_float4(v[4], v[5], v[6], v[7]);
+        *reinterpret_cast<uint4 *>(shadow + i) = w;
       }
-#pragma unroll
-      for (int sft = 16; sft; sft >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, sft);
-      if (lane == 0) red2[warp] = s2;
-      __syncthreads();
-      if (tid == 0) {
-        float t2 = 0.f;
-#pragma unroll
-        for (int w = 0; w < MERGE_WARPS; ++w) t2 += red2[w];
-        m.inv_norm[t] = t2 > 0.f ? 1.0f / sqrtf(t2) : 0.f;
+    } else {
+      for (int i = lane; i < D; i += 32) {
+        const float v = value(i) * inv;
+        master[i] = v;
+        const T sh = from_f32<T>(v);
+        shadow[i] = sh;
+        const float sv = to_f32<T>(sh);
+        s2 = fmaf(sv, sv, s2);
       }
     }
-    if (tid == 0) {
-      m.n_obs[t] = n_old + k_members;
-      m.n_points[t] = pts_old + pts;
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {  // R22
-        m.aabb[t * 6 + c] = min(box_old[c], bmn[c]);
-        m.aabb[t * 6 + 3 + c] = max(box_old[3 + c], bmx[c]);
-      }
-      if (best > best_old) {
-        m.best_view[t] = best;
-        const float *Tf = a.T + 16 * best_frame;
-        m.best_cam[t * 3 + 0] = Tf[3];
-        m.best_cam[t * 3 + 1] = Tf[7];
-        m.best_cam[t * 3 + 2] = Tf[11];
-      }
-      m.leader[t] = NONE32;
-      m.grp_cnt[t] = 0;
+    for (int sft = 16; sft; sft >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, sft);
+    if (lane == 0) m.inv_norm[t] = s2 > 0.f ? 1.0f / sqrtf(s2) : 0.f;
+  }
+  if (lane == 0) {
+    m.n_obs[t] = n_old + k_members;
+    m.n_points[t] = pts_old + pts;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {  // R22
+      m.aabb[t * 6 + c] = min(box_old[c], bmn[c]);
+      m.aabb[t * 6 + 3 + c] = max(box_old[3 + c], bmx[c]);
     }
+    if (best > best_old) {
+      m.best_view[t] = best;
+      const float *Tf = a.T + 16 * best_frame;
+      m.best_cam[t * 3 + 0] = Tf[3];
+      m.best_cam[t * 3 + 1] = Tf[7];
+      m.best_cam[t * 3 + 2] = Tf[11];
+    }
+    m.leader[t] = NONE32;
+    m.grp_cnt[t] = 0;
   }
 }
 
@@ -437,9 +445,8 @@ int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
   const int commit_blocks = 148 * 4;
-  const int merge_blocks = a.M < 148 * 16 ? a.M : 148 * 16;  // one CTA per detection: a single wave
-  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, MERGE_THREADS, (size_t)m.D * sizeof(float), s>>>(
-      m, a, frame_seq0, commit_blocks)));
+  const int merge_blocks = (a.M + MERGE_WARPS - 1) / MERGE_WARPS;  // one warp per detection
+  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, MERGE_THREADS, 0, s>>>(m, a, frame_seq0, commit_blocks)));
   return 1;
 }
 
