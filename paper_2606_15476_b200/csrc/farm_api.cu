@@ -12,7 +12,7 @@
 #include "farm_internal.cuh"
 
 namespace farm {
-int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state);
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
 bool tc_supported(const DevMap &m);
@@ -43,6 +43,7 @@ struct farm_map {
   long long launches = 0;
   unsigned long long frame_seq = 0;
   uint32_t epoch = 0;
+  uint32_t prep_target = 0;  // cumulative number of prep_kernel CTAs launched (device counter dm.prep_done)
   uint32_t n_upper = 0;  // host upper bound of N (no device sync on the integrate path)
   int last_M = 0;
   bool has_last = false;
@@ -327,6 +328,7 @@ int finalise(farm_map *m) {
   A(d.assoc, MD, 0);
   A(d.is_new, MD, 0);
   A(d.best_score, MD, 0);
+  A(d.prep_done, 1, 0);
   A(d.cam, (size_t)MAX_FRAMES * 16, 0);
   A(d.stats, 1, 0);
   A(d.totals, 1, 0);
@@ -537,15 +539,26 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   //                3 = lift first, then similarity || probe
   const bool fork = m->overlap && m->side && a.M > 0 && m->n_upper > 0;
   cudaStream_t sim_stream = fork ? m->side : st;
-  stage(FARM_STAGE_PREP, st, [&] { return launch_prep(d, a, st); });
+  // The tensor-core similarity kernel needs prep's output (row norms, zeroed best_dense) only in its epilogue and
+  // waits for it on the device (dm.prep_done), so it is forked BEFORE prep: prep leaves the critical path.
+  const bool early_fork = fork && m->tc && m->overlap == 1;
+  if (early_fork) {
+    cudaEventRecord(m->ev_fork, st);
+    cudaStreamWaitEvent(m->side, m->ev_fork, 0);
+  }
+  stage(FARM_STAGE_PREP, st, [&] {
+    m->prep_target += (uint32_t)launch_prep(d, a, st);
+    return 1;
+  });
   if (fork && m->overlap == 3) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
-  if (fork) {
+  if (fork && !early_fork) {
     cudaEventRecord(m->ev_fork, st);
     cudaStreamWaitEvent(m->side, m->ev_fork, 0);
   }
   // similarity is enqueued first so that its one-CTA-per-SM grid is resident before the other kernels fill the SMs
   stage(FARM_STAGE_SIMILARITY, sim_stream, [&] {
-    return m->tc ? launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc) : launch_similarity_fma(d, a, m->n_upper, sim_stream);
+    return m->tc ? launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc, m->prep_target)
+                 : launch_similarity_fma(d, a, m->n_upper, sim_stream);
   });
   if (fork) cudaEventRecord(m->ev_join, m->side);
   if (!(fork && m->overlap == 3)) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });

@@ -110,6 +110,7 @@ struct DevMap {
   int32_t *assoc;
   uint8_t *is_new;
   float *best_score;
+  uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
   CallStats *stats;
   Totals *totals;
@@ -210,7 +211,7 @@ __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { retu
 // kernel has drained).
 void configure_lift_kernels();
 void configure_assoc_kernels();
-int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);  // returns the number of CTAs it launched
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,

@@ -97,7 +97,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
 #pragma unroll
     for (int i = 0; i < 3; ++i) o[4 + 4 * i] = c.r[3 * i], o[5 + 4 * i] = c.r[3 * i + 1], o[6 + 4 * i] = c.r[3 * i + 2], o[7 + 4 * i] = c.t[i];
   }
-  if (warp >= a.M) return;
+  if (warp < a.M) {
   const T *row = (const T *)a.desc + (size_t)warp * m.D;
   float s = 0.f;
   if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
@@ -129,6 +129,13 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     m.best_score[warp] = 0.f;
   }
   if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
+  }
+  // publish: the similarity kernel runs on another stream and waits for every prep CTA before its first epilogue
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(m.prep_done, 1u);
+  }
 }
 
 
@@ -730,7 +737,7 @@ int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
     prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a);
   else
     prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a);
-  return 1;
+  return blocks;
 }
 
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {

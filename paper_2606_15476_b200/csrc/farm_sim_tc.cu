@@ -113,7 +113,7 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // 80 registers per thread (no spills): 256 x 80 leaves room for four 128 x 80 lift CTAs on the same SM
 __global__ void __maxnreg__(80)
 similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
-                     int M, uint32_t idesc) {
+                     int M, uint32_t idesc, uint32_t prep_target) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // SWIZZLE_128B needs 1024-byte alignment
   float *ib_s = (float *)(smem + STAGES * STAGE_BYTES);                         // [2][BLOCK_N] inverse norms of B
@@ -200,6 +200,16 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     const int row_in_tile = q * 32 + lane;
     const int et = threadIdx.x - 128;  // 0..EPI_THREADS-1
     uint32_t as = 0, aphase = 0;
+    // prep_kernel (main stream) may still be running: its row norms and the zeroed best_dense words are first
+    // needed here, one tile of MMAs after the kernel started
+    {
+      uint32_t done;
+      for (;;) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(m.prep_done) : "memory");
+        if ((int)(done - prep_target) >= 0) break;
+        __nanosleep(200);
+      }
+    }
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       const int tm = tile % tiles_m, tn = tile / tiles_m;
       const int n0 = tn * BLOCK_N;
@@ -321,14 +331,14 @@ void *tc_state_create(const DevMap &m) {
 
 void tc_state_destroy(void *p) { delete (TcState *)p; }
 
-int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state) {
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state, uint32_t prep_target) {
   TcState *st = (TcState *)state;
   if (a.M == 0 || n_upper == 0) return 0;
   CUtensorMap map_a;
   if (!encode_2d(st, &map_a, a.desc, (uint64_t)a.M, (uint64_t)m.D, BLOCK_M)) return -1;  // loud: the caller fails the call
   const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
   const int grid = (int)(tiles < st->num_sms ? tiles : st->num_sms);
-  similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc);
+  similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
   return 1;
 }
 
