@@ -17,6 +17,12 @@
 // back-projection of hand-placed points, floor-vs-truncate voxel cases, brute-force set intersection,
 // library GEMM for the cosine matrix, closed-form running mean, conservation / containment /
 // idempotence invariants.  No function here is "parity unpinned".
+//
+// Paper-faithful geometry carried beside the voxel rule (rules G1-G4 of DESIGN.md §11):
+// per-detection 3D Gaussian over the masked depth points, entity Gaussian by sufficient-
+// statistics merge, Hellinger distance between Gaussians.  Pins G-P1..G-P4 in
+// tests/test_oracle_gaussian.py: numpy mean/cov of the same points, union-of-halves, textbook closed forms
+// of the Hellinger distance and numpy.linalg for the general formula.  The association decision is NOT changed.
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -82,6 +88,9 @@ struct Object {  // R1
   std::vector<float> f;       // fp32 master descriptor, unit norm
   std::vector<float> shadow;  // round_to_storage(f), carried as fp32
   BestView best;
+  // G2: sufficient statistics of the entity Gaussian, M1 = w*mu, M2 = w*(Sigma + mu mu^T),
+  // w = number of merged points; packed symmetric order xx, xy, xz, yy, yz, zz ("6-vector")
+  double gW = 0.0, gM1[3] = {0, 0, 0}, gM2[6] = {0, 0, 0, 0, 0, 0};
 };
 
 struct Stats {  // per call
@@ -104,8 +113,47 @@ struct Map {
   std::vector<uint32_t> n_px;                        // R7
   std::vector<float> box;                            // R7, [M,6]
   std::vector<std::map<uint32_t, uint32_t>> overlap; // R9
+  std::vector<double> gS1, gS2;                      // G1: per detection sum p [M,3], sum p p^T [M,6]
+  std::vector<float> hell;                           // G4: Hellinger distance to the matched entity, -1 if none
   Stats stats;
 };
+
+// G1/G2: mean and population covariance from (w, M1, M2); packed order xx, xy, xz, yy, yz, zz
+void gaussian_from_moments(double w, const double *M1, const double *M2, double mu[3], double cov[6]) {
+  for (int a = 0; a < 3; ++a) mu[a] = M1[a] / w;
+  static const int ia[6] = {0, 0, 0, 1, 1, 2}, ib[6] = {0, 1, 2, 1, 2, 2};
+  for (int k = 0; k < 6; ++k) cov[k] = M2[k] / w - mu[ia[k]] * mu[ib[k]];
+}
+
+double det3(const double c[6]) {  // symmetric 3x3 from packed xx, xy, xz, yy, yz, zz
+  return c[0] * (c[3] * c[5] - c[4] * c[4]) - c[1] * (c[1] * c[5] - c[4] * c[2]) + c[2] * (c[1] * c[4] - c[3] * c[2]);
+}
+
+// G3 ("the Hellinger distance between two Gaussians is unitless and bounded in [0,1]"):
+//   H^2 = 1 - |S1|^(1/4) |S2|^(1/4) / |Sbar|^(1/2) * exp(-1/8 dmu^T Sbar^-1 dmu),  Sbar = (S1 + S2)/2,
+// with S = Sigma + eps2 * I on both sides (reading G3: masked depth patches are near-planar, their sample
+// covariance is near-singular; the paper does not say how it conditions it; eps = voxel_size is the only
+// length scale of this formulation).
+double hellinger(const double mu1[3], const double c1[6], const double mu2[3], const double c2[6], double eps2) {
+  double s1[6], s2[6], sb[6];
+  for (int k = 0; k < 6; ++k) {
+    const double reg = (k == 0 || k == 3 || k == 5) ? eps2 : 0.0;
+    s1[k] = c1[k] + reg;
+    s2[k] = c2[k] + reg;
+    sb[k] = 0.5 * (s1[k] + s2[k]);
+  }
+  const double d1 = det3(s1), d2 = det3(s2), db = det3(sb);
+  // inverse of Sbar by the adjugate (symmetric)
+  const double inv[6] = {(sb[3] * sb[5] - sb[4] * sb[4]) / db, (sb[2] * sb[4] - sb[1] * sb[5]) / db,
+                         (sb[1] * sb[4] - sb[2] * sb[3]) / db, (sb[0] * sb[5] - sb[2] * sb[2]) / db,
+                         (sb[1] * sb[2] - sb[0] * sb[4]) / db, (sb[0] * sb[3] - sb[1] * sb[1]) / db};
+  const double d[3] = {mu1[0] - mu2[0], mu1[1] - mu2[1], mu1[2] - mu2[2]};
+  const double q = d[0] * (inv[0] * d[0] + inv[1] * d[1] + inv[2] * d[2]) + d[1] * (inv[1] * d[0] + inv[3] * d[1] + inv[4] * d[2]) +
+                   d[2] * (inv[2] * d[0] + inv[4] * d[1] + inv[5] * d[2]);
+  const double bc = std::pow(d1, 0.25) * std::pow(d2, 0.25) / std::sqrt(db) * std::exp(-0.125 * q);
+  const double h2 = 1.0 - bc;
+  return h2 > 0.0 ? std::sqrt(h2) : 0.0;
+}
 
 // R5 (BASELINE.json "same fp32 operation order and FMA contraction disabled"):
 // back-projection of pixel (u = column, v = row) at depth z.  Every * and + is an individually rounded
@@ -251,6 +299,9 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
   m.n_px.assign(M, 0);
   m.box.assign((size_t)M * 6, 0.0f);
   m.overlap.assign(M, {});
+  m.gS1.assign((size_t)M * 3, 0.0);
+  m.gS2.assign((size_t)M * 6, 0.0);
+  m.hell.assign(M, -1.0f);
   m.stats = Stats();
   std::vector<int> det_frame(M), det_local(M);
 
@@ -284,6 +335,12 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
         }
         m.n_px[j]++;
         m.V[j].insert(key);                                       // R7
+        {                                                         // G1: moments of the detection's points
+          const double x = p[0], y = p[1], z = p[2];
+          double *s1 = &m.gS1[(size_t)j * 3], *s2 = &m.gS2[(size_t)j * 6];
+          s1[0] += x, s1[1] += y, s1[2] += z;
+          s2[0] += x * x, s2[1] += x * y, s2[2] += x * z, s2[3] += y * y, s2[4] += y * z, s2[5] += z * z;
+        }
         m.stats.valid_points++;
       }
   }
@@ -330,6 +387,12 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
       target[j] = best_o;
       m.assoc[j] = best_o;
       m.stats.matches++;
+      if (m.objs[best_o].gW > 0.0) {  // G4: distance to the matched entity's Gaussian as it was at entry (R2)
+        double mu_d[3], c_d[6], mu_o[3], c_o[6];
+        gaussian_from_moments((double)m.n_px[j], &m.gS1[(size_t)j * 3], &m.gS2[(size_t)j * 6], mu_d, c_d);
+        gaussian_from_moments(m.objs[best_o].gW, m.objs[best_o].gM1, m.objs[best_o].gM2, mu_o, c_o);
+        m.hell[j] = (float)hellinger(mu_d, c_d, mu_o, c_o, (double)m.voxel_size * (double)m.voxel_size);
+      }
     } else {  // R20: new ids in order of j
       target[j] = next_id++;
       m.assoc[j] = target[j];
@@ -376,6 +439,9 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     for (int j : by_target[o]) {
       ob.n_obs += 1;
       ob.n_points += m.n_px[j];
+      ob.gW += (double)m.n_px[j];                                  // G2: sufficient-statistics merge
+      for (int k = 0; k < 3; ++k) ob.gM1[k] += m.gS1[(size_t)j * 3 + k];
+      for (int k = 0; k < 6; ++k) ob.gM2[k] += m.gS2[(size_t)j * 6 + k];
       const float *b = &m.box[(size_t)j * 6];
       for (int k = 0; k < 3; ++k) {  // R22
         ob.amin[k] = std::fmin(ob.amin[k], b[k]);
@@ -517,6 +583,31 @@ int oracle_import(void *h, const oracle_object *objs, int n_objects, const float
 }
 
 // storage-dtype conversions exposed so the tests can pin them against torch
+// G1: Gaussians of the last call's detections (mu [M,3], cov [M,6]; zeros for skipped ones) and G4 distances [M]
+void oracle_last_gaussians(void *h, float *mu, float *cov, float *hell) {
+  Map &m = *(Map *)h;
+  for (int j = 0; j < m.M; ++j) {
+    double mu_d[3] = {0, 0, 0}, c_d[6] = {0, 0, 0, 0, 0, 0};
+    if (m.n_px[j]) gaussian_from_moments((double)m.n_px[j], &m.gS1[(size_t)j * 3], &m.gS2[(size_t)j * 6], mu_d, c_d);
+    for (int k = 0; k < 3; ++k) mu[(size_t)j * 3 + k] = (float)mu_d[k];
+    for (int k = 0; k < 6; ++k) cov[(size_t)j * 6 + k] = (float)c_d[k];
+    hell[j] = m.hell[j];
+  }
+}
+// G2: entity Gaussians (weight [N] = merged points, 0 = none; mu [N,3]; cov [N,6])
+void oracle_read_gaussians(void *h, double *weight, float *mu, float *cov) {
+  Map &m = *(Map *)h;
+  for (size_t o = 0; o < m.objs.size(); ++o) {
+    double mu_o[3] = {0, 0, 0}, c_o[6] = {0, 0, 0, 0, 0, 0};
+    if (m.objs[o].gW > 0.0) gaussian_from_moments(m.objs[o].gW, m.objs[o].gM1, m.objs[o].gM2, mu_o, c_o);
+    weight[o] = m.objs[o].gW;
+    for (int k = 0; k < 3; ++k) mu[o * 3 + k] = (float)mu_o[k];
+    for (int k = 0; k < 6; ++k) cov[o * 6 + k] = (float)c_o[k];
+  }
+}
+double oracle_hellinger(const double *mu1, const double *cov1, const double *mu2, const double *cov2, double eps2) {
+  return hellinger(mu1, cov1, mu2, cov2, eps2);
+}
 float oracle_round_to_storage(float f, int dtype) { return round_to_storage(f, dtype); }
 float oracle_cosine(const float *a, const float *b, int D) { return cosine(a, b, D); }
 

@@ -39,6 +39,8 @@ def lib():
         _lib.oracle_round_to_storage.restype = C.c_float
         _lib.oracle_round_to_storage.argtypes = [C.c_float, C.c_int]
         _lib.oracle_cosine.restype = C.c_float
+        _lib.oracle_hellinger.restype = C.c_double
+        _lib.oracle_hellinger.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
     return _lib
 
 
@@ -117,6 +119,24 @@ class OracleMap:
         lib().oracle_last_overlaps(self.h, _p(off), _p(obj), _p(cnt))
         return off, obj, cnt
 
+    def last_gaussians(self):
+        """G1 / G4: (mu [M,3], cov [M,6] packed xx xy xz yy yz zz, hellinger [M]) of the last call's detections."""
+        M = lib().oracle_last_M(self.h)
+        mu = np.zeros((M, 3), np.float32)
+        cov = np.zeros((M, 6), np.float32)
+        hell = np.zeros(M, np.float32)
+        lib().oracle_last_gaussians(self.h, _p(mu), _p(cov), _p(hell))
+        return mu, cov, hell
+
+    def read_gaussians(self):
+        """G2: (weight [N] float64, mu [N,3], cov [N,6]) of the map's entities."""
+        N = lib().oracle_n_objects(self.h)
+        w = np.zeros(N, np.float64)
+        mu = np.zeros((N, 3), np.float32)
+        cov = np.zeros((N, 6), np.float32)
+        lib().oracle_read_gaussians(self.h, _p(w), _p(mu), _p(cov))
+        return w, mu, cov
+
     def read(self, voxels=True):
         N = lib().oracle_n_objects(self.h)
         nv = lib().oracle_n_voxels(self.h)
@@ -143,6 +163,12 @@ def round_to_storage(x, dtype):
     for i in range(flat_in.size):
         flat_out[i] = lib().oracle_round_to_storage(float(flat_in[i]), dtype)
     return out
+
+
+def hellinger(mu1, cov1, mu2, cov2, eps2):
+    """G3: Hellinger distance of two 3-D Gaussians; cov packed xx xy xz yy yz zz; eps2 added to the diagonals."""
+    a = [np.ascontiguousarray(x, np.float64) for x in (mu1, cov1, mu2, cov2)]
+    return float(lib().oracle_hellinger(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), C.c_double(eps2)))
 
 
 def cosine(a, b):
