@@ -70,6 +70,9 @@ extern "C" {
                                         0 one stream; 2 / 3 experimental orders (see farm_api.cu)                      */
 #define FARM_OPT_MAX_BLOCKS 13       /* capacity in 4x4x4 voxel blocks (256 B each); table = next pow2 >= 2x;
                                         default MAX_VOXELS / 4.  Exceeding it sets the sticky capacity error           */
+#define FARM_OPT_GAUSSIAN 14         /* 1: also carry the paper's geometry: a 3-D Gaussian per
+                                        detection and per object and the Hellinger distance of every match; default 0.
+                                        The association rule is unchanged                                              */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -143,6 +146,17 @@ int farm_map_last_assoc(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *be
  * farm_map_sync / farm_map_last_assoc / farm_map_read; the sticky device error is reported there. */
 int farm_map_last_assoc_async(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score,
                               farm_frame_stats *stats);
+
+/* Paper-faithful geometry (needs FARM_OPT_GAUSSIAN = 1; HOST buffers, any may be NULL; both calls synchronise).
+ * "Each detection is lifted into a 3D Gaussian (mu_d, Sigma_d) over the masked depth points, with
+ * Sigma_d stored in a 6-vector packed form" -- mu [.,3], cov [.,6] = population covariance packed xx xy xz yy yz zz.
+ * the entity Gaussian is the sufficient-statistics merge M1 = w mu, M2 = w (Sigma + mu mu^T) over its
+ * detections, w = number of points (weight [N], 0 for imported objects that have not been observed).
+ * hellinger [M] = Hellinger distance in [0,1] between the detection's Gaussian and the Gaussian
+ * of the object it was matched to, as that object was at entry of the call; -1 for spawned / skipped detections
+ * and for objects without a Gaussian.  voxel_size^2 is added to both covariance diagonals (reading G3). */
+int farm_map_last_gaussians(farm_map *m, float *mu, float *cov, float *hellinger);
+int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov);
 
 /* Export (HOST buffers).  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
  * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary

@@ -35,7 +35,7 @@ struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
   long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
-  int sim_path = 0;
+  int sim_path = 0, gaussian = 0;
   cudaStream_t stream = 0;
   bool finalised = false;
   DevMap dm{};
@@ -236,6 +236,25 @@ __global__ void gather_events_kernel(DevMap m, uint32_t n, unsigned long long *b
   bkeys[i] = m.blk_key[m.pl_slot[i]];
 }
 
+// G1/G2 export: mean and population covariance from sufficient statistics (zeros where the weight is 0)
+__global__ void export_gaussians_kernel(const double *w, const uint32_t *w_u32, const double *g, uint32_t n, double *weight,
+                                        float *mu, float *cov) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double wi = w ? w[i] : (double)w_u32[i];
+  float o[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  if (wi > 0.0) {
+    const double *q = g + (size_t)i * 9;
+    const double m0 = q[0] / wi, m1 = q[1] / wi, m2 = q[2] / wi;
+    o[0] = (float)m0, o[1] = (float)m1, o[2] = (float)m2;
+    o[3] = (float)(q[3] / wi - m0 * m0), o[4] = (float)(q[4] / wi - m0 * m1), o[5] = (float)(q[5] / wi - m0 * m2);
+    o[6] = (float)(q[6] / wi - m1 * m1), o[7] = (float)(q[7] / wi - m1 * m2), o[8] = (float)(q[8] / wi - m2 * m2);
+  }
+  if (weight) weight[i] = wi;
+  for (int k = 0; k < 3; ++k) mu[(size_t)i * 3 + k] = o[k];
+  for (int k = 0; k < 6; ++k) cov[(size_t)i * 6 + k] = o[3 + k];
+}
+
 long long next_pow2(long long x) {
   long long p = 1;
   while (p < x) p <<= 1;
@@ -329,6 +348,13 @@ int finalise(farm_map *m) {
   A(d.is_new, MD, 0);
   A(d.best_score, MD, 0);
   A(d.prep_done, 1, 0);
+  d.eps2 = m->voxel_size * m->voxel_size;
+  if (m->gaussian) {
+    A(d.det_gm, MD * 9, 0);
+    A(d.hell, MD, 0);
+    A(d.obj_gw, NO, 0);
+    A(d.obj_gm, NO * 9, 0);
+  }
   A(d.cam, (size_t)MAX_FRAMES * 16, 0);
   A(d.stats, 1, 0);
   A(d.totals, 1, 0);
@@ -465,6 +491,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
     case FARM_OPT_OVERLAP:
       if (v < 0 || v > 3) return fail(FARM_ERR_INVALID_ARG, "bad OVERLAP");
       m->overlap = (int)v;
+      break;
+    case FARM_OPT_GAUSSIAN:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad GAUSSIAN");
+      m->gaussian = (int)v;
       break;
     case FARM_OPT_TIMING:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
@@ -772,6 +802,46 @@ int farm_map_last_assoc_async(farm_map *m, int32_t *obj_id, uint8_t *is_new, flo
   if (best_score && M) CU(cudaMemcpyAsync(best_score, m->dm.best_score, M * 4, cudaMemcpyDeviceToHost, m->stream));
   if (stats) CU(cudaMemcpyAsync(stats, m->dm.stats, sizeof(CallStats), cudaMemcpyDeviceToHost, m->stream));
   return FARM_OK;
+}
+
+static int export_gaussians(farm_map *m, const double *w, const uint32_t *w_u32, const double *g, uint32_t n, double *weight,
+                            float *mu, float *cov) {
+  if (!n) return FARM_OK;
+  double *dw = nullptr;
+  float *dmu, *dcov;
+  if (weight) CU(cudaMalloc(&dw, (size_t)n * 8));
+  CU(cudaMalloc(&dmu, (size_t)n * 12));
+  CU(cudaMalloc(&dcov, (size_t)n * 24));
+  export_gaussians_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(w, w_u32, g, n, dw, dmu, dcov);
+  m->launches++;
+  if (weight) CU(cudaMemcpyAsync(weight, dw, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream));
+  if (mu) CU(cudaMemcpyAsync(mu, dmu, (size_t)n * 12, cudaMemcpyDeviceToHost, m->stream));
+  if (cov) CU(cudaMemcpyAsync(cov, dcov, (size_t)n * 24, cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  cudaFree(dw), cudaFree(dmu), cudaFree(dcov);
+  return FARM_OK;
+}
+
+int farm_map_last_gaussians(farm_map *m, float *mu, float *cov, float *hellinger) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->gaussian) return fail(FARM_ERR_STATE, "FARM_OPT_GAUSSIAN is off");
+  if (!m->has_last) return fail(FARM_ERR_STATE, "no integrate call yet");
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  const uint32_t M = (uint32_t)m->last_M;
+  if (hellinger && M) CU(cudaMemcpy(hellinger, m->dm.hell, (size_t)M * 4, cudaMemcpyDeviceToHost));
+  return export_gaussians(m, nullptr, m->dm.det_npx, m->dm.det_gm, M, nullptr, mu, cov);
+}
+
+int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (!m->gaussian) return fail(FARM_ERR_STATE, "FARM_OPT_GAUSSIAN is off");
+  if (!m->finalised) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  return export_gaussians(m, m->dm.obj_gw, nullptr, m->dm.obj_gm, N, weight, mu, cov);
 }
 
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset) {

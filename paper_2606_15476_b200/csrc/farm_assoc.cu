@@ -9,6 +9,33 @@ namespace {
 
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 
+// ---- paper-faithful geometry (rules G1-G4): Gaussian from sufficient statistics, Hellinger distance (double)
+__device__ __forceinline__ void gaussian_of(double w, const double *g, double mu[3], double c[6]) {
+  mu[0] = g[0] / w, mu[1] = g[1] / w, mu[2] = g[2] / w;
+  c[0] = g[3] / w - mu[0] * mu[0], c[1] = g[4] / w - mu[0] * mu[1], c[2] = g[5] / w - mu[0] * mu[2];
+  c[3] = g[6] / w - mu[1] * mu[1], c[4] = g[7] / w - mu[1] * mu[2], c[5] = g[8] / w - mu[2] * mu[2];
+}
+__device__ __forceinline__ double det_sym3(const double c[6]) {
+  return c[0] * (c[3] * c[5] - c[4] * c[4]) - c[1] * (c[1] * c[5] - c[4] * c[2]) + c[2] * (c[1] * c[4] - c[3] * c[2]);
+}
+// G3: H = sqrt(1 - BC), BC = |S1|^(1/4) |S2|^(1/4) / |Sb|^(1/2) * exp(-dmu^T Sb^-1 dmu / 8),
+// S = Sigma + eps2 I, Sb = (S1 + S2) / 2
+__device__ float hellinger_gauss(const double mu1[3], double s1[6], const double mu2[3], double s2[6], double eps2) {
+  s1[0] += eps2, s1[3] += eps2, s1[5] += eps2;
+  s2[0] += eps2, s2[3] += eps2, s2[5] += eps2;
+  double sb[6];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) sb[k] = 0.5 * (s1[k] + s2[k]);
+  const double db = det_sym3(sb);
+  const double a00 = sb[3] * sb[5] - sb[4] * sb[4], a01 = sb[2] * sb[4] - sb[1] * sb[5], a02 = sb[1] * sb[4] - sb[2] * sb[3];
+  const double a11 = sb[0] * sb[5] - sb[2] * sb[2], a12 = sb[1] * sb[2] - sb[0] * sb[4], a22 = sb[0] * sb[3] - sb[1] * sb[1];
+  const double d0 = mu1[0] - mu2[0], d1 = mu1[1] - mu2[1], d2 = mu1[2] - mu2[2];
+  const double q = (d0 * (a00 * d0 + a01 * d1 + a02 * d2) + d1 * (a01 * d0 + a11 * d1 + a12 * d2) + d2 * (a02 * d0 + a12 * d1 + a22 * d2)) / db;
+  const double bc = sqrt(sqrt(det_sym3(s1) * det_sym3(s2))) / sqrt(db) * exp(-0.125 * q);
+  const double h2 = 1.0 - bc;
+  return h2 > 0.0 ? (float)sqrt(h2) : 0.f;
+}
+
 // ---- candidate scoring + association, one launch.
 // Phase 1 (all CTAs): one warp per non-zero overlap entry (d, o, c): cos(a_d, shadow_o) by a gather dot, g (R10),
 //   score (R17), atomicMax into best_cand[d].
@@ -150,6 +177,17 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
       }
     }
     if (in) {
+      if (m.det_gm && matched) {  // G4: distance to the matched entity's Gaussian as it was at entry (R2)
+        const double wo = m.obj_gw[target];
+        if (wo > 0.0) {
+          double gd[9], go[9], mu_d[3], c_d[6], mu_o[3], c_o[6];
+#pragma unroll
+          for (int k = 0; k < 9; ++k) gd[k] = __ldcg(&m.det_gm[(size_t)j * 9 + k]), go[k] = m.obj_gm[(size_t)target * 9 + k];
+          gaussian_of((double)my_npx, gd, mu_d, c_d);
+          gaussian_of(wo, go, mu_o, c_o);
+          m.hell[j] = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)m.eps2);
+        }
+      }
       m.assoc[j] = target;
       m.is_new[j] = (uint8_t)spawn;
       m.best_score[j] = score;
@@ -299,6 +337,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
   int box_old[6] = {0, 0, 0, 0, 0, 0};
   int best_frame = -1;
+  double gsum[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // G2: sufficient statistics of the members
   if (lane == 0) {
     pts_old = m.n_points[t];
     best_old = m.best_view[t];
@@ -308,6 +347,10 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       k_members++;
       const uint32_t npx = m.det_npx[jm];
       pts += npx;
+      if (m.det_gm) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) gsum[k] += m.det_gm[(size_t)jm * 9 + k];
+      }
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         bmn[c] = min(bmn[c], m.det_box[jm * 6 + c]);
@@ -403,6 +446,11 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   if (lane == 0) {
     m.n_obs[t] = n_old + k_members;
     m.n_points[t] = pts_old + pts;
+    if (m.det_gm) {  // G2: M1 += sum w mu, M2 += sum w (Sigma + mu mu^T), w = points
+      m.obj_gw[t] += (double)pts;
+#pragma unroll
+      for (int k = 0; k < 9; ++k) m.obj_gm[(size_t)t * 9 + k] += gsum[k];
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {  // R22
       m.aabb[t * 6 + c] = min(box_old[c], bmn[c]);

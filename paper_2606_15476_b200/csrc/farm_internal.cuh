@@ -110,6 +110,11 @@ struct DevMap {
   int32_t *assoc;
   uint8_t *is_new;
   float *best_score;
+  // paper-faithful geometry carried beside the voxel rule (rules G1-G4); null when disabled
+  double *det_gm;                    // [max_det,9] per detection: sum p (3), sum p p^T (6: xx xy xz yy yz zz)
+  double *obj_gw, *obj_gm;           // [max_objects], [max_objects,9]: entity sufficient statistics w, M1, M2
+  float *hell;                       // [max_det] Hellinger distance to the matched entity (entry snapshot), -1 if none
+  float eps2;                        // voxel_size^2, added to both covariance diagonals (reading G3)
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
   CallStats *stats;

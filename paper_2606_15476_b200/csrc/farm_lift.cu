@@ -129,6 +129,10 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     m.best_score[warp] = 0.f;
   }
   if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
+  if (m.det_gm) {
+    if (lane < 9) m.det_gm[(size_t)warp * 9 + lane] = 0.0;
+    if (lane == 9) m.hell[warp] = -1.f;
+  }
   }
   // publish: the similarity kernel runs on another stream and waits for every prep CTA before its first epilogue
   __syncthreads();
@@ -285,8 +289,15 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
 // is added on its own: count 1, box = the point, one voxel bit of its block.
 __device__ __noinline__ void stray_pixel(TileSmem &s, uint32_t *lab_j, uint32_t *lab_cnt, int (*lab_box)[6], uint32_t *det_npx,
                                          int *det_box, unsigned long long *surv_key, unsigned long long *surv_bits,
-                                         uint32_t *surv_j, uint32_t surv_cap, uint32_t *counters, uint32_t *err, uint32_t j,
-                                         unsigned long long bkey, uint32_t bit, float p0, float p1, float p2) {
+                                         uint32_t *surv_j, uint32_t surv_cap, uint32_t *counters, uint32_t *err, double *det_gm,
+                                         uint32_t j, unsigned long long bkey, uint32_t bit, float p0, float p1, float p2) {
+  if (det_gm) {  // G1: the point's contribution to the detection's moments
+    double *g = det_gm + (size_t)j * 9;
+    const double x = p0, y = p1, z = p2;
+    atomicAdd(g + 0, x), atomicAdd(g + 1, y), atomicAdd(g + 2, z);
+    atomicAdd(g + 3, x * x), atomicAdd(g + 4, x * y), atomicAdd(g + 5, x * z);
+    atomicAdd(g + 6, y * y), atomicAdd(g + 7, y * z), atomicAdd(g + 8, z * z);
+  }
   const int li = tile_label_slot_in(lab_j, j);
   const int o0 = f2ord(p0), o1 = f2ord(p1), o2 = f2ord(p2);
   const uint32_t lo = (bit & 32) ? 0u : 1u << (bit & 31), hi = (bit & 32) ? 1u << (bit & 31) : 0u;
@@ -339,8 +350,8 @@ __device__ __noinline__ void stray_pixel(TileSmem &s, uint32_t *lab_j, uint32_t 
 // Two barriers per tile.  Per-detection pixel counts and point boxes go through shared-memory
 // accumulators (REDUX fast path when a warp holds one detection) to one set of global atomics per
 // (tile, detection).
-template <bool VEC>
-__global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+template <bool VEC, bool GAUSS>
+__global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads
   __shared__ uint32_t lab_cnt2[2][MAX_LABELS];  // its copy while tile t+1 initialises the other
@@ -414,6 +425,9 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
     uint32_t ibit_lo = 0, ibit_hi = 0;  // 6-bit voxel index inside the block, pixels 0-3 / 4-7
     uint32_t valid = 0, L0 = 0;         // pixels of the thread's first detection L0 (almost always the only one)
     float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
+    // G1: moments of the thread's points about its first point (fp32 stays exact enough: offsets of a few cm)
+    float gc0 = 0.f, gc1 = 0.f, gc2 = 0.f, g1x = 0.f, g1y = 0.f, g1z = 0.f;
+    float gxx = 0.f, gxy = 0.f, gxz = 0.f, gyy = 0.f, gyz = 0.f, gzz = 0.f;
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       ikey[i] = BLK_EMPTY;
@@ -440,9 +454,16 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
               if (i < 4) ibit_lo |= bit << (6 * i); else ibit_hi |= bit << (6 * (i - 4));
               mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
               mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
+              if (GAUSS) {
+                if (valid == (1u << i)) gc0 = p[0], gc1 = p[1], gc2 = p[2];  // first point of the thread
+                const float dx = p[0] - gc0, dy = p[1] - gc1, dz = p[2] - gc2;
+                g1x += dx, g1y += dy, g1z += dz;
+                gxx = fmaf(dx, dx, gxx), gxy = fmaf(dx, dy, gxy), gxz = fmaf(dx, dz, gxz);
+                gyy = fmaf(dy, dy, gyy), gyz = fmaf(dy, dz, gyz), gzz = fmaf(dz, dz, gzz);
+              }
             } else {  // rare: the thread's 8 pixels straddle two detections -- this pixel goes in on its own
               stray_pixel(s, lab_j, lab_cnt, lab_box, m.det_npx, m.det_box, m.surv_key, m.surv_bits, m.surv_j, m.surv_cap,
-                          m.counters, m.err, (uint32_t)det_base + l - 1, bk, bit, p[0], p[1], p[2]);
+                          m.counters, m.err, GAUSS ? m.det_gm : nullptr, (uint32_t)det_base + l - 1, bk, bit, p[0], p[1], p[2]);
             }
           } else {
             acc_dropped++;
@@ -472,6 +493,31 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
           if (lane == 0) label_add_in(lab_cnt, lab_box, m, lead_li, (uint32_t)det_base + lead_L - 1, tot, r0, r1, r2, r3, r4, r5);
         } else if (valid) {
           label_add_in(lab_cnt, lab_box, m, li, j, cnt, o0, o1, o2, o3, o4, o5);
+        }
+      }
+      if (GAUSS) {  // G1: raw moments in double (parallel-axis shift from the thread's centre), one set of atomics per warp
+        const double n = (double)__popc(valid), c0 = gc0, c1 = gc1, c2 = gc2, sx = g1x, sy = g1y, sz = g1z;
+        double g[9] = {sx + n * c0, sy + n * c1, sz + n * c2,
+                       gxx + 2.0 * c0 * sx + n * c0 * c0, gxy + c0 * sy + c1 * sx + n * c0 * c1, gxz + c0 * sz + c2 * sx + n * c0 * c2,
+                       gyy + 2.0 * c1 * sy + n * c1 * c1, gyz + c1 * sz + c2 * sy + n * c1 * c2, gzz + 2.0 * c2 * sz + n * c2 * c2};
+        const unsigned has = __ballot_sync(FULL, valid != 0);
+        const uint32_t lead_L = __shfl_sync(FULL, L0, __ffs(has) - 1);
+        if (__all_sync(FULL, valid == 0 || L0 == lead_L)) {
+#pragma unroll
+          for (int k = 0; k < 9; ++k) {
+            if (!valid) g[k] = 0.0;
+#pragma unroll
+            for (int sft = 16; sft; sft >>= 1) g[k] += __shfl_xor_sync(FULL, g[k], sft);
+          }
+          if (lane < 9) {
+            double v = g[0];
+#pragma unroll
+            for (int k = 1; k < 9; ++k) v = lane == k ? g[k] : v;
+            atomicAdd(m.det_gm + (size_t)((uint32_t)det_base + lead_L - 1) * 9 + lane, v);
+          }
+        } else if (valid) {
+#pragma unroll
+          for (int k = 0; k < 9; ++k) atomicAdd(m.det_gm + (size_t)j * 9 + k, g[k]);
         }
       }
       // blocks: one pass per distinct block among the thread's pixels
@@ -724,8 +770,10 @@ void configure_lift_kernels() {
   max_shared_carveout(prep_kernel<float>);
   max_shared_carveout(prep_kernel<__half>);
   max_shared_carveout(prep_kernel<__nv_bfloat16>);
-  max_shared_carveout(lift_voxelise_kernel<true>);
-  max_shared_carveout(lift_voxelise_kernel<false>);
+  max_shared_carveout(lift_voxelise_kernel<true, false>);
+  max_shared_carveout(lift_voxelise_kernel<false, false>);
+  max_shared_carveout(lift_voxelise_kernel<true, true>);
+  max_shared_carveout(lift_voxelise_kernel<false, true>);
   max_shared_carveout(probe_kernel);
 }
 
@@ -746,10 +794,16 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   // persistent, 4 CTAs per SM: 4 x 128 x 80 registers fit beside the similarity CTA (256 x 80) in the 64 K register file
   const int grid = n_tiles < 148 * 4 ? n_tiles : 148 * 4;
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
-  if (vec)
-    lift_voxelise_kernel<true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
-  else
-    lift_voxelise_kernel<false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  if (m.det_gm) {
+    if (vec)
+      lift_voxelise_kernel<true, true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+    else
+      lift_voxelise_kernel<false, true><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  } else if (vec) {
+    lift_voxelise_kernel<true, false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  } else {
+    lift_voxelise_kernel<false, false><<<grid, LIFT_THREADS, 0, s>>>(m, a, tiles_x, tiles_y);
+  }
   return 1;
 }
 

@@ -317,6 +317,60 @@ def test_config4_full_size_sampled_against_oracle(oracle):
     assert int(tot["frames"]) == 2 * F and int(tot["matches"]) == F * DET
 
 
+def _compare_gaussians(g, o):
+    mu_o, cov_o, hell_o = o.last_gaussians()
+    mu_g, cov_g, hell_g = g.last_gaussians()
+    assert np.abs(mu_g - mu_o).max(initial=0) <= TOL
+    assert np.abs(cov_g - cov_o).max(initial=0) <= TOL
+    assert np.array_equal(hell_g < 0, hell_o < 0)
+    assert np.abs(hell_g - hell_o).max(initial=0) <= TOL
+    return hell_o
+
+
+@pytest.mark.parametrize("cfg_id,n_calls,per_call", [(0, 20, 1), (1, 4, 1), (0, 4, 3)])
+def test_gaussian_geometry_matches_oracle(oracle, cfg_id, n_calls, per_call):
+    """Rules G1-G4: per-detection Gaussians, Hellinger distance of every match and the
+    sufficient-statistics entity Gaussians, carried beside the unchanged voxel rule."""
+    cfg = S.get_config(cfg_id)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg, gaussian=1)
+    k, n_match = 0, 0
+    for _ in range(n_calls):
+        frames = margin_filter(o.clone, [sc.frame(k + i) for i in range(per_call)], cfg.tau)
+        k += per_call
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o, check_sets=False)
+        hell = _compare_gaussians(g, o)
+        n_match += int((hell >= 0).sum())
+        assert ((hell < 0) | (hell <= 1.0)).all()
+    assert n_match > 3
+    compare_maps(g, o, voxels=False)
+    w_o, mu_o, cov_o = o.read_gaussians()
+    w_g, mu_g, cov_g = g.read_gaussians()
+    assert np.array_equal(w_g, w_o)                                # point counts: exact
+    assert np.abs(mu_g - mu_o).max(initial=0) <= TOL and np.abs(cov_g - cov_o).max(initial=0) <= TOL
+
+
+def test_gaussian_mini_stress_and_off_by_default(oracle):
+    sc = S.StressScene(n_batches=2, frames_per_batch=4, n_objects=700)
+    o, g = _stress_pair(oracle, sc, gaussian=1)
+    for b in range(2):
+        frames = margin_filter(o.clone, sc.batch(b), sc.cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, sc.cfg.dtype)
+        compare_call(g, o, check_sets=False)
+        hell = _compare_gaussians(g, o)
+        assert (hell < 0).all()                                     # imported objects carry no Gaussian (weight 0)
+    w_o, mu_o, cov_o = o.read_gaussians()
+    w_g, mu_g, cov_g = g.read_gaussians()
+    assert np.array_equal(w_g, w_o) and np.abs(mu_g - mu_o).max() <= TOL and np.abs(cov_g - cov_o).max() <= TOL
+    from paper_2606_15476_b200.binding import FarmError
+    _, g2 = make_pair(oracle, S.get_config(0))
+    with pytest.raises(FarmError):
+        g2.read_gaussians()
+
+
 def test_host_buffer_entry_point_matches_device_path(oracle):
     cfg = S.get_config(0)
     sc = S.BoxScene(cfg)
