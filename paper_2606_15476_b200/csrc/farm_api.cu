@@ -548,20 +548,27 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   const DevMap &d = m->dm;
   cudaStream_t st = m->stream;
   bool launch_failed = false;
+  cudaEvent_t pending_e0 = nullptr;
   auto stage = [&](int id, cudaStream_t st, auto &&fn) {
-    const bool timed = m->timing >= 2 || (m->timing == 1 && (id == FARM_STAGE_LIFT || id == FARM_STAGE_PROBE || id == FARM_STAGE_SIMILARITY));
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (timed) {
-      e0 = get_event(m), e1 = get_event(m);
+    // timing 1: similarity on its own, lift + probe as ONE bracket (reported under LIFT) so that no event sits
+    // between the two kernels and the probe's programmatic dependent launch stays effective; timing 2: every kernel
+    const bool self = m->timing >= 2 || (m->timing == 1 && id == FARM_STAGE_SIMILARITY);
+    const bool opens = m->timing == 1 && id == FARM_STAGE_LIFT, closes = m->timing == 1 && id == FARM_STAGE_PROBE;
+    cudaEvent_t e0 = nullptr;
+    if (self || opens) {
+      e0 = get_event(m);
       cudaEventRecord(e0, st);
+      if (opens) pending_e0 = e0;
     }
     int n = fn();
     if (n < 0) launch_failed = true, n = 0;
     m->launches += n;
     m->stage_launches[id] += n;
-    if (timed) {
+    if (self || (closes && pending_e0)) {
+      cudaEvent_t e1 = get_event(m);
       cudaEventRecord(e1, st);
-      m->ev_pending[id].push_back({e0, e1});
+      m->ev_pending[self ? id : FARM_STAGE_LIFT].push_back({self ? e0 : pending_e0, e1});
+      if (!self) pending_e0 = nullptr;
     }
   };
   // DAG of one call:  prep -> { similarity (side stream) || lift + probe } -> cand_score+associate -> commit+merge

@@ -48,6 +48,7 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_trigger();  // the merge kernel may become resident while the decision scan runs
   {
     const uint32_t n_cand = min(m.counters[1], m.cand_cap);
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
@@ -239,6 +240,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
                                                            int commit_blocks) {
   __shared__ uint32_t mlist[MERGE_WARPS][MLIST];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_wait();  // launched with PDL behind cand_associate: decisions, leaders and group sizes are final from here on
   const int merge_blocks = gridDim.x - commit_blocks;
   if ((int)blockIdx.x >= merge_blocks) {  // the merge CTAs come first in launch order
     const uint32_t cb = blockIdx.x - merge_blocks;
@@ -494,7 +496,8 @@ int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long f
   if (a.M == 0) return 0;
   const int commit_blocks = 148 * 4;
   const int merge_blocks = (a.M + MERGE_WARPS - 1) / MERGE_WARPS;  // one warp per detection
-  FARM_DISPATCH((commit_merge_kernel<T><<<commit_blocks + merge_blocks, MERGE_THREADS, 0, s>>>(m, a, frame_seq0, commit_blocks)));
+  FARM_DISPATCH((launch_pdl(commit_merge_kernel<T>, dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s, m, a, frame_seq0,
+                            commit_blocks)));
   return 1;
 }
 

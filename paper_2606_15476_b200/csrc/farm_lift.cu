@@ -352,6 +352,7 @@ __device__ __noinline__ void stray_pixel(TileSmem &s, uint32_t *lab_j, uint32_t 
 // (tile, detection).
 template <bool VEC, bool GAUSS>
 __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+  pdl_trigger();  // the probe kernel may become resident as soon as CTAs of this grid retire
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads
   __shared__ uint32_t lab_cnt2[2][MAX_LABELS];  // its copy while tile t+1 initialises the other
@@ -623,6 +624,7 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
 constexpr int PROBE_THREADS = 256;
 
 __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs a) {
+  pdl_wait();  // launched with PDL behind the lift kernel: its survivor queue is complete from here on
   const uint32_t nq = min(m.counters[2], m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;
@@ -808,7 +810,7 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 }
 
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  probe_kernel<<<148 * 4, PROBE_THREADS, 0, s>>>(m, a);
+  launch_pdl(probe_kernel, dim3(148 * 4), dim3(PROBE_THREADS), 0, s, m, a);
   return 1;
 }
 
