@@ -65,8 +65,8 @@ extern "C" {
 #define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
 #define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
 #define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
-#define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around similarity and around lift+probe (one bracket,
-                                        reported under LIFT); 2 every kernel                                           */
+#define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the similarity kernel only; 2 around every kernel (this
+                                        serialises the programmatically chained kernels).  May be changed at any time    */
 #define FARM_OPT_OVERLAP 12          /* 1 (default): similarity on an internal side stream, concurrent with lift+probe;
                                         0 one stream; 2 / 3 experimental orders (see farm_api.cu)                      */
 #define FARM_OPT_MAX_BLOCKS 13       /* capacity in 4x4x4 voxel blocks (256 B each); table = next pow2 >= 2x;

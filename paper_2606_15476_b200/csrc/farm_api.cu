@@ -12,7 +12,8 @@
 #include "farm_internal.cuh"
 
 namespace farm {
-int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target);
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target,
+                         int *n_ctas);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
 bool tc_supported(const DevMap &m);
@@ -43,6 +44,7 @@ struct farm_map {
   long long launches = 0;
   unsigned long long frame_seq = 0;
   uint32_t epoch = 0;
+  uint32_t sim_target = 0;   // cumulative number of similarity CTAs launched (device counter dm.sim_done)
   uint32_t prep_target = 0;  // cumulative number of prep_kernel CTAs launched (device counter dm.prep_done)
   uint32_t n_upper = 0;  // host upper bound of N (no device sync on the integrate path)
   int last_M = 0;
@@ -348,6 +350,7 @@ int finalise(farm_map *m) {
   A(d.is_new, MD, 0);
   A(d.best_score, MD, 0);
   A(d.prep_done, 1, 0);
+  A(d.sim_done, 1, 0);
   d.eps2 = m->voxel_size * m->voxel_size;
   if (m->gaussian) {
     A(d.det_gm, MD * 9, 0);
@@ -443,7 +446,7 @@ int farm_map_destroy(farm_map *m) {
 
 int farm_map_set_option_i(farm_map *m, int key, long long v) {
   if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
-  if (m->finalised) return fail(FARM_ERR_STATE, "options are frozen after the first integrate / import");
+  if (m->finalised && key != FARM_OPT_TIMING) return fail(FARM_ERR_STATE, "options are frozen after the first integrate / import");
   switch (key) {
     case FARM_OPT_DESC_DTYPE:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad dtype");
@@ -548,27 +551,23 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   const DevMap &d = m->dm;
   cudaStream_t st = m->stream;
   bool launch_failed = false;
-  cudaEvent_t pending_e0 = nullptr;
   auto stage = [&](int id, cudaStream_t st, auto &&fn) {
-    // timing 1: similarity on its own, lift + probe as ONE bracket (reported under LIFT) so that no event sits
-    // between the two kernels and the probe's programmatic dependent launch stays effective; timing 2: every kernel
-    const bool self = m->timing >= 2 || (m->timing == 1 && id == FARM_STAGE_SIMILARITY);
-    const bool opens = m->timing == 1 && id == FARM_STAGE_LIFT, closes = m->timing == 1 && id == FARM_STAGE_PROBE;
+    // timing 1: only the similarity kernel (it has the side stream to itself, so its events do not sit between
+    // the PDL-chained kernels of the main stream); timing 2: every kernel (serialises the main-stream chain)
+    const bool timed = m->timing >= 2 || (m->timing == 1 && id == FARM_STAGE_SIMILARITY);
     cudaEvent_t e0 = nullptr;
-    if (self || opens) {
+    if (timed) {
       e0 = get_event(m);
       cudaEventRecord(e0, st);
-      if (opens) pending_e0 = e0;
     }
     int n = fn();
     if (n < 0) launch_failed = true, n = 0;
     m->launches += n;
     m->stage_launches[id] += n;
-    if (self || (closes && pending_e0)) {
+    if (timed) {
       cudaEvent_t e1 = get_event(m);
       cudaEventRecord(e1, st);
-      m->ev_pending[self ? id : FARM_STAGE_LIFT].push_back({self ? e0 : pending_e0, e1});
-      if (!self) pending_e0 = nullptr;
+      m->ev_pending[id].push_back({e0, e1});
     }
   };
   // DAG of one call:  prep -> { similarity (side stream) || lift + probe } -> cand_score+associate -> commit+merge
@@ -594,16 +593,25 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   }
   // similarity is enqueued first so that its one-CTA-per-SM grid is resident before the other kernels fill the SMs
   stage(FARM_STAGE_SIMILARITY, sim_stream, [&] {
-    return m->tc ? launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc, m->prep_target)
-                 : launch_similarity_fma(d, a, m->n_upper, sim_stream);
+    if (!m->tc) return launch_similarity_fma(d, a, m->n_upper, sim_stream);
+    int ctas = 0;
+    const int n = launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc, m->prep_target, &ctas);
+    m->sim_target += (uint32_t)ctas;
+    return n;
   });
+  // With the early fork the association kernel is not joined to the side stream: it is launched (PDL) right behind
+  // the probe, scores the candidates while the similarity kernel finishes, and its decision scan waits for
+  // dm.sim_done on the device.  The stream join moves behind the merge kernel, off the critical path.
+  a.wait_sim = early_fork ? 1 : 0;
+  a.sim_target = m->sim_target;
   if (fork) cudaEventRecord(m->ev_join, m->side);
   if (!(fork && m->overlap == 3)) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork && m->overlap == 2) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st); });
-  if (fork && m->overlap != 2) cudaStreamWaitEvent(st, m->ev_join, 0);
+  if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
+  if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   CU(cudaGetLastError());
   if (launch_failed) return fail(FARM_ERR_CUDA, "similarity: cuTensorMapEncodeTiled failed (descriptor pointer must be 16-byte aligned)");
   m->frame_seq += F;

@@ -41,14 +41,17 @@ __device__ float hellinger_gauss(const double mu1[3], double s1[6], const double
 //   score (R17), atomicMax into best_cand[d].
 // Phase 2 (the last CTA to finish, found by a ticket): decisions for all detections (R18), new ids by an
 //   exclusive scan in detection index order (R20), per-target leader / group size for the merge.
+constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PRE = 4;  // 512 x 52 registers fit beside the similarity CTA
+
 template <typename T>
-__global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs a) {
-  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per chunk of 1024 detections
+__global__ void __launch_bounds__(CAND_THREADS) cand_associate_kernel(DevMap m, CallArgs a) {
+  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per chunk of CAND_THREADS detections
   __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   pdl_trigger();  // the merge kernel may become resident while the decision scan runs
+  pdl_wait();     // launched with PDL behind the probe kernel: candidates and overlap counts are final from here on
   {
     const uint32_t n_cand = min(m.counters[1], m.cand_cap);
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
@@ -100,15 +103,15 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
   const uint32_t N = __ldcg(m.n_objects);
   unsigned long long valid_points = 0;
   if (tid == 0) valid_points = __ldcg(&m.stats->valid_points);
-  uint32_t pre_nv[2], pre_npx[2];
-  unsigned long long pre_bd[2];
+  uint32_t pre_nv[CAND_PRE], pre_npx[CAND_PRE];
+  unsigned long long pre_bd[CAND_PRE];
 #pragma unroll
-  for (int q = 0; q < 2; ++q) {
-    const int j = q * 1024 + tid;
+  for (int q = 0; q < CAND_PRE; ++q) {
+    const int j = q * CAND_THREADS + tid;
     const bool in = j < a.M;
     pre_nv[q] = in ? __ldcg(&m.det_nv[j]) : 0u;
     pre_npx[q] = in ? __ldcg(&m.det_npx[j]) : 0u;
-    pre_bd[q] = in ? __ldcg(&m.best_dense[j]) : 0ull;
+    pre_bd[q] = (in && !a.wait_sim) ? __ldcg(&m.best_dense[j]) : 0ull;  // final only once similarity has finished
   }
   // ---- ticket: the last CTA to arrive runs the association
   __syncthreads();
@@ -121,18 +124,40 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
   }
   __syncthreads();
   if (!s_last) return;
+  if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid, then fetch its row maxima
+    if (tid == 0) {
+      uint32_t done;
+      for (;;) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(m.sim_done) : "memory");
+        if ((int)(done - a.sim_target) >= 0) break;
+        __nanosleep(200);
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < CAND_PRE; ++q) {
+      const int j = q * CAND_THREADS + tid;
+      pre_bd[q] = j < a.M ? __ldcg(&m.best_dense[j]) : 0ull;
+    }
+  }
   __threadfence();
   uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier chunks (every thread)
-  for (int base = 0; base < a.M; base += 1024) {
+  for (int base = 0; base < a.M; base += CAND_THREADS) {
     const int j = base + tid;
-    const int q = base >> 10;
+    const int q = base / CAND_THREADS;
     uint32_t spawn = 0, matched = 0, skipped = 0;
     int32_t target = -1;
     float score = 0.f;
     const bool in = j < a.M;
-    const uint32_t my_nv = q == 0 ? pre_nv[0] : q == 1 ? pre_nv[1] : (in ? __ldcg(&m.det_nv[j]) : 0u);
-    const uint32_t my_npx = q == 0 ? pre_npx[0] : q == 1 ? pre_npx[1] : (in ? __ldcg(&m.det_npx[j]) : 0u);
-    const unsigned long long bd = q == 0 ? pre_bd[0] : q == 1 ? pre_bd[1] : (in ? __ldcg(&m.best_dense[j]) : 0ull);
+    uint32_t my_nv = 0, my_npx = 0;
+    unsigned long long bd = 0;
+    if (q < CAND_PRE) {
+#pragma unroll
+      for (int k = 0; k < CAND_PRE; ++k)
+        if (k == q) my_nv = pre_nv[k], my_npx = pre_npx[k], bd = pre_bd[k];
+    } else if (in) {
+      my_nv = __ldcg(&m.det_nv[j]), my_npx = __ldcg(&m.det_npx[j]), bd = __ldcg(&m.best_dense[j]);
+    }
     nv_sum += my_nv;
     if (in) {
       if (my_npx == 0) {
@@ -160,14 +185,14 @@ __global__ void __launch_bounds__(1024) cand_associate_kernel(DevMap m, CallArgs
     uint32_t *ws = warp_sum2[q & 1];
     if (lane == 0) ws[warp] = __popc(b);
     __syncthreads();
-    uint32_t incl = ws[lane];
+    uint32_t incl = lane < CAND_WARPS ? ws[lane] : 0u;
 #pragma unroll
     for (int sft = 1; sft < 32; sft <<= 1) {
       const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, sft);
       if (lane >= sft) incl += up;
     }
     const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    const uint32_t before = __shfl_sync(0xFFFFFFFFu, incl, warp) - __shfl_sync(0xFFFFFFFFu, ws[lane], warp);
+    const uint32_t before = __shfl_sync(0xFFFFFFFFu, incl, warp) - ws[warp];
     if (spawn) {
       const uint32_t id = N + running + before + __popc(b & ((1u << lane) - 1));
       if (id < m.max_objects) {
@@ -488,8 +513,8 @@ void configure_assoc_kernels() {
 }
 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  const int grid = a.M > 0 ? 37 : 1;  // 37 x 32 warps = one warp per candidate for ~1.2k candidates per wave
-  FARM_DISPATCH((cand_associate_kernel<T><<<grid, 1024, 0, s>>>(m, a)));
+  const int grid = a.M > 0 ? 74 : 1;  // 74 x 16 warps = one warp per candidate for ~1.2k candidates per wave
+  FARM_DISPATCH((launch_pdl(cand_associate_kernel<T>, dim3(grid), dim3(CAND_THREADS), 0, s, m, a)));
   return 1;
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {

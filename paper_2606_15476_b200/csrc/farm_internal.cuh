@@ -115,6 +115,7 @@ struct DevMap {
   double *obj_gw, *obj_gm;           // [max_objects], [max_objects,9]: entity sufficient statistics w, M1, M2
   float *hell;                       // [max_det] Hellinger distance to the matched entity (entry snapshot), -1 if none
   float eps2;                        // voxel_size^2, added to both covariance diagonals (reading G3)
+  uint32_t *sim_done;                // cumulative count of finished similarity CTAs (the association scan waits on it)
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
   CallStats *stats;
@@ -125,6 +126,8 @@ struct DevMap {
 struct CallArgs {
   int F, M;
   uint32_t epoch;
+  uint32_t sim_target;  // value dm.sim_done reaches when this call's similarity kernel has finished
+  int wait_sim;         // 1: cand_associate is launched without a stream join and waits for sim_target itself
   const float *depth;
   const uint16_t *mask;
   const float *K;

@@ -624,7 +624,8 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
 constexpr int PROBE_THREADS = 256;
 
 __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs a) {
-  pdl_wait();  // launched with PDL behind the lift kernel: its survivor queue is complete from here on
+  pdl_trigger();  // cand_associate may become resident behind this grid
+  pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
   const uint32_t nq = min(m.counters[2], m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;

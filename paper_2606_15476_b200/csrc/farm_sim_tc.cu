@@ -266,7 +266,9 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     }
   }
   tcgen05_fence_before();
+  __threadfence();  // the epilogue's atomicMax results precede the completion count below
   __syncthreads();
+  if (threadIdx.x == 0) atomicAdd(m.sim_done, 1u);  // cand_associate's decision scan waits for every CTA of this grid
   if (warp == 2) {
     tcgen05_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS));
@@ -331,7 +333,8 @@ void *tc_state_create(const DevMap &m) {
 
 void tc_state_destroy(void *p) { delete (TcState *)p; }
 
-int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state, uint32_t prep_target) {
+int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state, uint32_t prep_target,
+                         int *n_ctas) {
   TcState *st = (TcState *)state;
   if (a.M == 0 || n_upper == 0) return 0;
   CUtensorMap map_a;
@@ -339,6 +342,7 @@ int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, c
   const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
   const int grid = (int)(tiles < st->num_sms ? tiles : st->num_sms);
   similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+  if (n_ctas) *n_ctas = grid;
   return 1;
 }
 
