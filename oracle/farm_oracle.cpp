@@ -21,7 +21,8 @@
 // Paper-faithful geometry carried beside the voxel rule (rules G1-G4 of DESIGN.md §11):
 // per-detection 3D Gaussian over the masked depth points, entity Gaussian by sufficient-
 // statistics merge, Hellinger distance between Gaussians.  Pins G-P1..G-P4 in
-// tests/test_oracle_gaussian.py: numpy mean/cov of the same points, union-of-halves, textbook closed forms
+// tests/test_oracle_gaussian.py (covisibility bitset of PAPER.md:354, rule C1, pinned there as well by brute-force
+// pair enumeration, symmetry and monotonicity): numpy mean/cov of the same points, union-of-halves, textbook closed forms
 // of the Hellinger distance and numpy.linalg for the general formula.  The association decision is NOT changed.
 #include <cmath>
 #include <cstdint>
@@ -115,6 +116,10 @@ struct Map {
   std::vector<std::map<uint32_t, uint32_t>> overlap; // R9
   std::vector<double> gS1, gS2;                      // G1: per detection sum p [M,3], sum p p^T [M,6]
   std::vector<float> hell;                           // G4: Hellinger distance to the matched entity, -1 if none
+  // C1 ("A bitset adjacency (N x ceil(N/64) blocks) marks all pairs of entities that were jointly
+  // visible in the current batch"): row a, bit b set iff a != b and both received a detection in one call.
+  // Rows grow with N; bits are never cleared.
+  std::vector<std::vector<uint64_t>> covis;
   Stats stats;
 };
 
@@ -458,6 +463,18 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
       }
     }
   }
+  // C1: every pair of distinct entities observed in this call (matched or spawned) becomes covisible
+  {
+    std::set<int> seen;
+    for (int j = 0; j < M; ++j)
+      if (target[j] >= 0) seen.insert(target[j]);
+    const size_t words = ((size_t)next_id + 63) / 64;
+    m.covis.resize(next_id);
+    for (auto &row : m.covis) row.resize(words, 0);
+    for (int a : seen)
+      for (int b : seen)
+        if (a != b) m.covis[a][(size_t)b >> 6] |= 1ull << (b & 63);
+  }
   m.frame_seq += F;
   return 0;
 }
@@ -604,6 +621,14 @@ void oracle_read_gaussians(void *h, double *weight, float *mu, float *cov) {
     for (int k = 0; k < 3; ++k) mu[o * 3 + k] = (float)mu_o[k];
     for (int k = 0; k < 6; ++k) cov[o * 6 + k] = (float)c_o[k];
   }
+}
+// C1: rows [N, ceil(N/64)] of the covisibility bitset
+int oracle_covis_words(void *h) { return (int)((((Map *)h)->objs.size() + 63) / 64); }
+void oracle_read_covis(void *h, uint64_t *rows) {
+  Map &m = *(Map *)h;
+  const size_t N = m.objs.size(), words = (N + 63) / 64;
+  for (size_t a = 0; a < N; ++a)
+    for (size_t w = 0; w < words; ++w) rows[a * words + w] = a < m.covis.size() && w < m.covis[a].size() ? m.covis[a][w] : 0;
 }
 double oracle_hellinger(const double *mu1, const double *cov1, const double *mu2, const double *cov2, double eps2) {
   return hellinger(mu1, cov1, mu2, cov2, eps2);

@@ -137,6 +137,14 @@ class OracleMap:
         lib().oracle_read_gaussians(self.h, _p(w), _p(mu), _p(cov))
         return w, mu, cov
 
+    def read_covisibility(self):
+        """C1: uint64 [N, ceil(N/64)]; bit b of row a = entities a and b were observed in one call."""
+        N = lib().oracle_n_objects(self.h)
+        words = lib().oracle_covis_words(self.h)
+        rows = np.zeros((N, words), np.uint64)
+        lib().oracle_read_covis(self.h, _p(rows))
+        return rows
+
     def read(self, voxels=True):
         N = lib().oracle_n_objects(self.h)
         nv = lib().oracle_n_voxels(self.h)

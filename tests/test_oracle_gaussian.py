@@ -120,3 +120,30 @@ def test_GP4_hellinger_of_a_match_uses_the_entry_snapshot(oracle):
     assert m.last_assoc()[0][0] == 0
     expect = oracle.hellinger(muB[0], covB[0], mu1[0], cov1[0], vs * vs)
     assert abs(hell[0] - expect) < 1e-6 and 0.0 < hell[0] < 1.0
+
+
+def test_CP1_covisibility_bitset_is_the_set_of_co_observed_pairs(oracle):
+    """C1 ("A bitset adjacency (N x ceil(N/64) blocks) marks all pairs of entities that were jointly
+    visible in the current batch"): brute-force pair enumeration over the per-call association lists; symmetric, no
+    diagonal, bits only accumulate."""
+    from paper_2606_15476_b200 import scenes as S
+    from helpers import integrate_frames
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    m = oracle.OracleMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, cfg.dtype, cfg.H, cfg.W)
+    pairs, prev = set(), None
+    for k in range(0, 12, 2):
+        integrate_frames(m, [sc.frame(k), sc.frame(k + 1)])        # one call = one batch of two frames
+        assoc = m.last_assoc()[0]
+        seen = sorted(set(int(a) for a in assoc if a >= 0))
+        pairs |= {(a, b) for a in seen for b in seen if a != b}
+        rows = m.read_covisibility()
+        N = rows.shape[0]
+        assert rows.shape[1] == (N + 63) // 64
+        got = {(a, b) for a in range(N) for b in range(N) if (int(rows[a, b >> 6]) >> (b & 63)) & 1}
+        assert got == pairs
+        assert all((b, a) in got for a, b in got) and all(a != b for a, b in got)
+        if prev is not None:
+            assert prev <= got
+        prev = got
+    assert len(pairs) > 10
