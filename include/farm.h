@@ -74,6 +74,8 @@ extern "C" {
 #define FARM_OPT_GAUSSIAN 14         /* 1: also carry the paper's geometry: a 3-D Gaussian per
                                         detection and per object and the Hellinger distance of every match; default 0.
                                         The association rule is unchanged                                              */
+#define FARM_OPT_COVISIBILITY 15     /* 1: maintain the N x ceil(N/64) covisibility bitset of PAPER.md:354 (step 7): all pairs
+                                        of distinct objects that received a detection in one call; default 0            */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -158,6 +160,12 @@ int farm_map_last_assoc_async(farm_map *m, int32_t *obj_id, uint8_t *is_new, flo
  * and for objects without a Gaussian.  voxel_size^2 is added to both covariance diagonals (reading G3). */
 int farm_map_last_gaussians(farm_map *m, float *mu, float *cov, float *hellinger);
 int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov);
+
+/* Covisibility bitset (needs FARM_OPT_COVISIBILITY = 1; "A bitset adjacency (N x ceil(N/64) blocks) marks
+ * all pairs of entities that were jointly visible in the current batch").  Two-call pattern: rows == NULL writes only
+ * *words = ceil(N/64); else rows is a HOST buffer [N, *words] of uint64; bit b of row a is set iff objects a != b both
+ * received a detection in one integrate call.  Bits are never cleared.  Synchronises. */
+int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words);
 
 /* Export (HOST buffers).  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
  * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary

@@ -22,6 +22,7 @@ OPT_TIMING = 11
 OPT_OVERLAP = 12
 OPT_MAX_BLOCKS = 13
 OPT_GAUSSIAN = 14
+OPT_COVISIBILITY = 15
 N_STAGES = 7
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "unused", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
@@ -38,7 +39,7 @@ TOTALS_DTYPE = np.dtype([("frames", "<u8"), ("calls", "<u8"), ("valid_points", "
                          ("matches", "<u8"), ("spawns", "<u8")])
 
 EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm_map_set_option_f",
-           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians",
+           "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians", "farm_map_read_covisibility",
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
@@ -74,6 +75,7 @@ def load_library():
         lib.farm_map_last_assoc_async.argtypes = [vp, vp, vp, vp, vp]
         lib.farm_map_last_gaussians.argtypes = [vp, vp, vp, vp]
         lib.farm_map_read_gaussians.argtypes = [vp, vp, vp, vp]
+        lib.farm_map_read_covisibility.argtypes = [vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
         lib.farm_map_sync.argtypes = [vp, vp]
@@ -112,7 +114,7 @@ class FarmMap:
 
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
                  max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
-                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None):
+                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._h = C.c_void_p()
@@ -123,7 +125,7 @@ class FarmMap:
         for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels), (OPT_MAX_BLOCKS, max_blocks),
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
-                       (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian)):
+                       (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:
@@ -222,6 +224,17 @@ class FarmMap:
         w, mu, cov = np.zeros(N, np.float64), np.zeros((N, 3), np.float32), np.zeros((N, 6), np.float32)
         _check(load_library().farm_map_read_gaussians(self._h, _hp(w), _hp(mu), _hp(cov)))
         return w, mu, cov
+
+    def read_covisibility(self):
+        """uint64 [N, ceil(N/64)] covisibility bitset (FARM_OPT_COVISIBILITY)."""
+        lib = load_library()
+        w = C.c_int(0)
+        _check(lib.farm_map_read_covisibility(self._h, None, C.byref(w)))
+        n = C.c_int(0)
+        _check(lib.farm_map_read(self._h, None, C.byref(n), None, None, None, None))
+        rows = np.zeros((n.value, w.value), np.uint64)
+        _check(lib.farm_map_read_covisibility(self._h, _hp(rows), C.byref(w)))
+        return rows
 
     def counts(self):
         """(number of objects, number of owned voxels) without copying the map out."""

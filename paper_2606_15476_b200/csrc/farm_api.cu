@@ -36,7 +36,7 @@ struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
   long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
-  int sim_path = 0, gaussian = 0;
+  int sim_path = 0, gaussian = 0, covis = 0;
   cudaStream_t stream = 0;
   bool finalised = false;
   DevMap dm{};
@@ -352,6 +352,11 @@ int finalise(farm_map *m) {
   A(d.prep_done, 1, 0);
   A(d.sim_done, 1, 0);
   d.eps2 = m->voxel_size * m->voxel_size;
+  if (m->covis) {
+    d.covis_words = (uint32_t)((NO + 63) / 64);
+    if ((size_t)d.covis_words * 8 > 96 * 1024) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_COVISIBILITY supports MAX_OBJECTS <= 786432");
+    A(d.covis, NO * d.covis_words, 0);
+  }
   if (m->gaussian) {
     A(d.det_gm, MD * 9, 0);
     A(d.hell, MD, 0);
@@ -499,6 +504,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad GAUSSIAN");
       m->gaussian = (int)v;
       break;
+    case FARM_OPT_COVISIBILITY:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad COVISIBILITY");
+      m->covis = (int)v;
+      break;
     case FARM_OPT_TIMING:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
       m->timing = (int)v;
@@ -611,6 +620,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
+  stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
   if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   CU(cudaGetLastError());
   if (launch_failed) return fail(FARM_ERR_CUDA, "similarity: cuTensorMapEncodeTiled failed (descriptor pointer must be 16-byte aligned)");
@@ -857,6 +867,22 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov) 
   uint32_t N = 0;
   CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
   return export_gaussians(m, m->dm.obj_gw, nullptr, m->dm.obj_gm, N, weight, mu, cov);
+}
+
+int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words) {
+  if (!m || !words) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->covis) return fail(FARM_ERR_STATE, "FARM_OPT_COVISIBILITY is off");
+  *words = 0;
+  if (!m->finalised) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  const uint32_t w = (N + 63) / 64;
+  *words = (int)w;
+  if (rows && N)  // strided device rows -> dense [N, w]
+    CU(cudaMemcpy2D(rows, (size_t)w * 8, m->dm.covis, (size_t)m->dm.covis_words * 8, (size_t)w * 8, N, cudaMemcpyDeviceToHost));
+  return FARM_OK;
 }
 
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset) {

@@ -265,7 +265,8 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
                                                            int commit_blocks) {
   __shared__ uint32_t mlist[MERGE_WARPS][MLIST];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  pdl_wait();  // launched with PDL behind cand_associate: decisions, leaders and group sizes are final from here on
+  pdl_trigger();  // the optional covisibility kernel may become resident behind this grid
+  pdl_wait();     // launched with PDL behind cand_associate: decisions, leaders and group sizes are final from here on
   const int merge_blocks = gridDim.x - commit_blocks;
   if ((int)blockIdx.x >= merge_blocks) {  // the merge CTAs come first in launch order
     const uint32_t cb = blockIdx.x - merge_blocks;
@@ -495,6 +496,39 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   }
 }
 
+// ---- covisibility (rule C1; PAPER.md:354 step 7): every pair of distinct entities that received a detection in
+// this call is marked in the N x ceil(N/64) bitset.  Each CTA builds the call's entity bitmap in shared memory
+// (a few KB) and ORs it, minus the diagonal bit, into the rows of its entities, writing only the words that change.  A row is written only by the CTAs of detections that target it, and they all write the
+// same words, so no atomics are needed.
+constexpr int COVIS_THREADS = 256;
+
+__global__ void __launch_bounds__(COVIS_THREADS) covisibility_kernel(DevMap m, CallArgs a) {
+  extern __shared__ unsigned long long bm[];  // [words]
+  pdl_wait();
+  const uint32_t N = *m.n_objects;
+  const uint32_t words = (N + 63) >> 6;
+  for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) bm[w] = 0ull;
+  __syncthreads();
+  for (int j = threadIdx.x; j < a.M; j += COVIS_THREADS) {
+    const int32_t t = m.assoc[j];
+    if (t >= 0) atomicOr(&bm[(uint32_t)t >> 6], 1ull << (t & 63));
+  }
+  __syncthreads();
+  for (int j = blockIdx.x; j < a.M; j += gridDim.x) {
+    const int32_t t = m.assoc[j];
+    if (t < 0) continue;
+    unsigned long long *row = m.covis + (size_t)t * m.covis_words;
+    for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) {
+      unsigned long long add = bm[w];
+      if (w == ((uint32_t)t >> 6)) add &= ~(1ull << (t & 63));  // no diagonal
+      if (add) {
+        const unsigned long long old = row[w];
+        if ((old | add) != old) row[w] = old | add;
+      }
+    }
+  }
+}
+
 }  // namespace
 
 #define FARM_DISPATCH(call)                                   \
@@ -510,11 +544,19 @@ void configure_assoc_kernels() {
   cudaFuncSetAttribute(commit_merge_kernel<float>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
   cudaFuncSetAttribute(commit_merge_kernel<__half>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
   cudaFuncSetAttribute(commit_merge_kernel<__nv_bfloat16>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(covisibility_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
+  cudaFuncSetAttribute(covisibility_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
 }
 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int grid = a.M > 0 ? 74 : 1;  // 74 x 16 warps = one warp per candidate for ~1.2k candidates per wave
   FARM_DISPATCH((launch_pdl(cand_associate_kernel<T>, dim3(grid), dim3(CAND_THREADS), 0, s, m, a)));
+  return 1;
+}
+int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  if (a.M == 0 || !m.covis) return 0;
+  const int grid = a.M < 148 * 4 ? a.M : 148 * 4;
+  launch_pdl(covisibility_kernel, dim3(grid), dim3(COVIS_THREADS), (size_t)m.covis_words * 8, s, m, a);
   return 1;
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {

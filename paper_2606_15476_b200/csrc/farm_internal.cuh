@@ -115,6 +115,8 @@ struct DevMap {
   double *obj_gw, *obj_gm;           // [max_objects], [max_objects,9]: entity sufficient statistics w, M1, M2
   float *hell;                       // [max_det] Hellinger distance to the matched entity (entry snapshot), -1 if none
   float eps2;                        // voxel_size^2, added to both covariance diagonals (reading G3)
+  unsigned long long *covis;         // [max_objects, covis_words] covisibility bitset (rule C1); null when disabled
+  uint32_t covis_words;
   uint32_t *sim_done;                // cumulative count of finished similarity CTAs (the association scan waits on it)
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
@@ -243,5 +245,6 @@ int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t
 int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
+int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s);
 
 }  // namespace farm

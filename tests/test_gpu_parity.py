@@ -371,6 +371,30 @@ def test_gaussian_mini_stress_and_off_by_default(oracle):
         g2.read_gaussians()
 
 
+def test_covisibility_bitset_matches_oracle(oracle):
+    """Rule C1 (PAPER.md:354 step 7): the N x ceil(N/64) bitset of co-observed entity pairs, bit-exact, on batched
+    config-0 calls and on the mini stress scene (imported map, 400 detections per call)."""
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg, covisibility=1)
+    for k in range(0, 18, 3):
+        frames = margin_filter(o.clone, [sc.frame(k + i) for i in range(3)], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o, check_sets=False)
+        assert np.array_equal(g.read_covisibility(), o.read_covisibility())
+    assert int(np.unpackbits(o.read_covisibility().view(np.uint8)).sum()) > 20
+    sc4 = S.StressScene(n_batches=2, frames_per_batch=4, n_objects=700)
+    o4, g4 = _stress_pair(oracle, sc4, covisibility=1)
+    for b in range(2):
+        frames = margin_filter(o4.clone, sc4.batch(b), sc4.cfg.tau)
+        integrate_frames(o4, frames)
+        gpu_integrate(g4, frames, sc4.cfg.dtype)
+        compare_call(g4, o4, check_sets=False)
+    ro, rg = o4.read_covisibility(), g4.read_covisibility()
+    assert np.array_equal(rg, ro)
+
+
 def test_host_buffer_entry_point_matches_device_path(oracle):
     cfg = S.get_config(0)
     sc = S.BoxScene(cfg)
