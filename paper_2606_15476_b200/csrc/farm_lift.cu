@@ -225,26 +225,36 @@ __device__ __forceinline__ void label_add_in(uint32_t *lab_cnt, int (*lab_box)[6
 // OR the voxel bits (lo, hi) of block `bkey` into the tile's entry of (label slot li, block).  Exact: the tag
 // holds the whole block key and the label slot.  Without a label slot, or when the tile table is full, the
 // record goes straight to the global queue (the probe kernel's pair set keeps the result exact).
-__device__ __forceinline__ void tile_block_add(TileSmem &s, const DevMap &m, int li, uint32_t j, unsigned long long bkey,
-                                               uint32_t lo, uint32_t hi) {
-  if (li >= 0) {
-    const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
-    uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
-    for (int probe = 0; probe < TILE_ENT; ++probe) {
-      unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
-      if (cur == BLK_EMPTY) {
-        cur = atomicCAS(&s.tag[h], BLK_EMPTY, tag);
-        if (cur == BLK_EMPTY) cur = tag;
-      }
-      if (cur == tag) {
-        if (lo) atomicOr(&s.mlo[h], lo);
-        if (hi) atomicOr(&s.mhi[h], hi);
-        return;
-      }
-      h = (h + 1) & (TILE_ENT - 1);
+__device__ __forceinline__ bool tile_block_add(TileSmem &s, int li, unsigned long long bkey, uint32_t lo, uint32_t hi) {
+  if (li < 0) return false;
+  const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
+  uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
+  for (int probe = 0; probe < 16; ++probe) {  // a short probe sequence: a miss only costs one more queue record
+    unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
+    if (cur == BLK_EMPTY) {
+      cur = atomicCAS(&s.tag[h], BLK_EMPTY, tag);
+      if (cur == BLK_EMPTY) cur = tag;
     }
+    if (cur == tag) {
+      if (lo) atomicOr(&s.mlo[h], lo);
+      if (hi) atomicOr(&s.mhi[h], hi);
+      return true;
+    }
+    h = (h + 1) & (TILE_ENT - 1);
   }
-  survivor_store(m, atomicAdd(&m.counters[2], 1u), bkey, j, lo, hi);
+  return false;
+}
+
+// Records the tile table could not absorb (no label slot, table full: far, noisy surfaces put every pixel into its
+// own block) go straight to the global queue -- one atomicAdd per warp, not per lane.  Warp-synchronous.
+__device__ __forceinline__ void emit_overflow(const DevMap &m, bool ovf, unsigned long long bkey, uint32_t j, uint32_t lo, uint32_t hi) {
+  const unsigned b = __ballot_sync(0xFFFFFFFFu, ovf);
+  if (!b) return;
+  const int lane = threadIdx.x & 31;
+  uint32_t base = 0;
+  if (lane == __ffs(b) - 1) base = atomicAdd(&m.counters[2], (uint32_t)__popc(b));
+  base = __shfl_sync(0xFFFFFFFFu, base, __ffs(b) - 1);
+  if (ovf) survivor_store(m, base + __popc(b & ((1u << lane) - 1)), bkey, j, lo, hi);
 }
 
 // raw registers of one thread's 8 pixels (2 x 128-bit depth + 1 x 128-bit mask)
@@ -539,15 +549,16 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
             hi |= (bit & 32) ? one : 0u;
           }
         rem &= ~hit;
-        if (hit && li < 0) survivor_store(m, atomicAdd(&m.counters[2], 1u), kb, j, lo, hi);  // no label slot
+        bool ovf = hit && li < 0;  // no label slot
         const bool tab = hit && li >= 0;
         const unsigned act = __ballot_sync(FULL, tab);
         if (tab) {
           const unsigned long long tag = kb | ((unsigned long long)li << LABEL_SHIFT);
           const unsigned same = __match_any_sync(act, tag);
           lo = __reduce_or_sync(same, lo), hi = __reduce_or_sync(same, hi);
-          if (lane == __ffs(same) - 1) tile_block_add(s, m, li, j, kb, lo, hi);
+          if (lane == __ffs(same) - 1) ovf = !tile_block_add(s, li, kb, lo, hi);
         }
+        emit_overflow(m, ovf, kb, j, lo, hi);
       }
     }
     __syncthreads();  // B2: the tile's table is complete; thread 0 has published the queue chunk
