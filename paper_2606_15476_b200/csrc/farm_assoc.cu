@@ -36,6 +36,21 @@ __device__ float hellinger_gauss(const double mu1[3], double s1[6], const double
   return h2 > 0.0 ? (float)sqrt(h2) : 0.f;
 }
 
+// G4: Hellinger distance between detection j and the entity it was matched to, as that entity was at entry (R2).
+// Out of line so that its double-precision temporaries do not inflate the association kernel's register budget
+// (512 threads x <= 64 registers must fit beside the similarity CTA).
+__device__ __noinline__ void match_hellinger(const double *det_gm, const double *obj_gw, const double *obj_gm, float *hell,
+                                             float eps2, int j, int32_t target, uint32_t npx) {
+  const double wo = obj_gw[target];
+  if (!(wo > 0.0)) return;
+  double gd[9], go[9], mu_d[3], c_d[6], mu_o[3], c_o[6];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) gd[k] = __ldcg(&det_gm[(size_t)j * 9 + k]), go[k] = obj_gm[(size_t)target * 9 + k];
+  gaussian_of((double)npx, gd, mu_d, c_d);
+  gaussian_of(wo, go, mu_o, c_o);
+  hell[j] = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)eps2);
+}
+
 // ---- candidate scoring + association, one launch.
 // Phase 1 (all CTAs): one warp per non-zero overlap entry (d, o, c): cos(a_d, shadow_o) by a gather dot, g (R10),
 //   score (R17), atomicMax into best_cand[d].
@@ -44,7 +59,8 @@ __device__ float hellinger_gauss(const double mu1[3], double s1[6], const double
 constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PRE = 4;  // 512 x 52 registers fit beside the similarity CTA
 
 template <typename T>
-__global__ void __launch_bounds__(CAND_THREADS) cand_associate_kernel(DevMap m, CallArgs a) {
+// 80 registers: 512 x 80 fits beside the similarity CTA (256 x 80) and the phase-1 dot products overlap its tail
+__global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
   __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per chunk of CAND_THREADS detections
   __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
@@ -203,17 +219,7 @@ __global__ void __launch_bounds__(CAND_THREADS) cand_associate_kernel(DevMap m, 
       }
     }
     if (in) {
-      if (m.det_gm && matched) {  // G4: distance to the matched entity's Gaussian as it was at entry (R2)
-        const double wo = m.obj_gw[target];
-        if (wo > 0.0) {
-          double gd[9], go[9], mu_d[3], c_d[6], mu_o[3], c_o[6];
-#pragma unroll
-          for (int k = 0; k < 9; ++k) gd[k] = __ldcg(&m.det_gm[(size_t)j * 9 + k]), go[k] = m.obj_gm[(size_t)target * 9 + k];
-          gaussian_of((double)my_npx, gd, mu_d, c_d);
-          gaussian_of(wo, go, mu_o, c_o);
-          m.hell[j] = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)m.eps2);
-        }
-      }
+      if (m.det_gm && matched) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, target, my_npx);  // G4
       m.assoc[j] = target;
       m.is_new[j] = (uint8_t)spawn;
       m.best_score[j] = score;
