@@ -460,3 +460,84 @@ def test_tile_queue_overflow_every_pixel_its_own_voxel(oracle):
         _, _, _, st = g.last_assoc()
         assert st["unique_voxels"] > 0.9 * H * W
     compare_maps(g, o)
+
+
+def test_many_detections_in_one_tile_label_slots_overflow(oracle):
+    """Every pixel of a 64x16 tile carries its own detection (hundreds of labels per tile): more than the lift
+    kernel's 32 per-tile label slots, threads whose 8 pixels straddle 8 detections (stray-pixel path), and
+    records that bypass the tile table."""
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.05, 8, 0.5, 0.5, 0.5, 0
+    H, W = 32, 128
+    n_det = 300
+    g0 = np.random.default_rng(3)
+    o, g = make_pair(oracle, Cfg, H=H, W=W, max_det_per_call=512)
+    K = np.array([[100, 0, 64], [0, 100, 16], [0, 0, 1]], np.float32)
+    for it in range(2):
+        depth = (1.0 + 2.0 * g0.random((H, W))).astype(np.float32)
+        mask = (g0.integers(0, n_det + 40, size=(H, W))).astype(np.uint16)      # also labels > n_det (ignored, R3) and 0
+        mask[4:8, 16:48] = 7                                                      # one block of a single label as well
+        fr = S.Frame(depth, mask, K, np.eye(4, dtype=np.float32), unit_rows(n_det, 8, 9 + it), n_det, np.zeros(n_det, np.int64))
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+        _, _, _, st = g.last_assoc()
+        assert st["ignored_pixels"] > 0
+    compare_maps(g, o)
+
+
+@pytest.mark.parametrize("n_same", [5, 90])
+def test_many_detections_fuse_into_one_entity(oracle, n_same):
+    """several detections may claim one entity and all fuse into it.  n_same detections of one call
+    match the same object: member lists that fit the merge kernel's shared-memory list (5) and that do not (90)."""
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.25, 16, 0.5, 0.5, 0.5, 0
+    H, W = 96, 128
+    I4 = np.eye(4, dtype=np.float32)
+    base = unit_rows(1, 16, 2)
+    o, g = make_pair(oracle, Cfg, H=H, W=W, max_det_per_call=128)
+    # call 1: one detection creates the object; call 2: n_same detections over the same voxels with nearby descriptors
+    px = [(u, v, 2.0, 1) for v in range(40, 48) for u in range(60, 76)]
+    d1, m1 = hand_frame(H, W, px)
+    fr1 = S.Frame(d1, m1, pow2_K(), I4, base, 1, np.zeros(1, np.int64))
+    rng = np.random.default_rng(4)
+    desc = base + 0.02 * rng.standard_normal((n_same, 16)).astype(np.float32)
+    desc /= np.linalg.norm(desc, axis=1, keepdims=True)
+    px2 = [(60 + (k % 16), 40 + k // 16, 2.0, k + 1) for k in range(n_same)]         # one pixel per detection
+    d2, m2 = hand_frame(H, W, px2)
+    fr2 = S.Frame(d2, m2, pow2_K(), I4, desc.astype(np.float32), n_same, np.zeros(n_same, np.int64))
+    for fr in (fr1, fr2, fr2):
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+    a, n, _, _ = g.last_assoc()
+    assert (a == 0).all() and not n.any()
+    objs, _, _, _ = g.read()
+    assert len(objs) == 1 and objs["n_obs"][0] == 1 + 2 * n_same
+    compare_maps(g, o)
+
+
+@pytest.mark.parametrize("dtype,D", [(1, 20), (2, 36), (0, 7)])
+def test_descriptor_lengths_off_the_vector_paths(oracle, dtype, D):
+    """D not a multiple of 8 (no 128-bit row loads, no TMA: CUDA-core similarity) for f16 / bf16 / f32."""
+    cfg = S.get_config(0)
+
+    class Cfg:
+        voxel, w_geo, w_sem, tau = cfg.voxel, cfg.w_geo, cfg.w_sem, cfg.tau
+    Cfg.D, Cfg.dtype = D, dtype
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, Cfg, H=cfg.H, W=cfg.W)
+    rng = np.random.default_rng(8)
+    basis = unit_rows(64, D, 1)
+    for k in range(6):
+        fr = sc.frame(k)
+        # re-describe the frame's detections with D-long descriptors tied to the underlying box id
+        ids = np.asarray(fr.box_ids) % 64
+        d = basis[ids[:fr.n_det]] + 0.01 * rng.standard_normal((fr.n_det, D)).astype(np.float32)
+        d /= np.linalg.norm(d, axis=1, keepdims=True)
+        fr2 = S.Frame(fr.depth, fr.mask, fr.K, fr.T, S.to_storage(d.astype(np.float32), dtype), fr.n_det, np.zeros(fr.n_det, np.int64))
+        frames = margin_filter(o.clone, [fr2], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, dtype)
+        compare_call(g, o)
+    compare_maps(g, o)
