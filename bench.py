@@ -306,6 +306,29 @@ def run_ours(args):
         del m2, pinned
         torch.cuda.empty_cache()
 
+    # ---------------- context: the library GEMM of the same shape (cuBLAS through torch.matmul), which has to write the
+    # M x N matrix that the fused kernel never materialises and would still need a row-max kernel after it
+    lib_gemm_ms = None
+    if rank == 0:
+        try:
+            Mg, Ng = FRAMES_PER_BATCH * DET_PER_FRAME, int(n_after)
+            ga = torch.randn(Mg, cfg.D, device=dev, dtype=torch.bfloat16)
+            gb = torch.randn(Ng, cfg.D, device=dev, dtype=torch.bfloat16)
+            gout = torch.empty(Mg, Ng, device=dev, dtype=torch.bfloat16)
+            ts = []
+            for it in range(8):
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record()
+                torch.matmul(ga, gb.t(), out=gout)
+                g1.record()
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(g0.elapsed_time(g1))
+            lib_gemm_ms = min(ts)
+            del ga, gb, gout
+            torch.cuda.empty_cache()
+        except Exception:  # context only
+            lib_gemm_ms = None
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -358,6 +381,9 @@ def run_ours(args):
         "stage_ms_per_step": {n: float(stage_ms[i]) / max(K_steps, 1) for i, n in enumerate(binding.STAGE_NAMES)},
         "stage_ms_breakdown_pass": {n: float(bd_ms[i]) for i, n in enumerate(binding.STAGE_NAMES)},
         "stage_launches": {n: int(stage_launches[i]) for i, n in enumerate(binding.STAGE_NAMES)},
+        "library_gemm_context": {"what": "torch.matmul (cuBLAS) bf16, same M x N x D as the similarity step at the end of the run, "
+                                         "writes the M x N matrix, no row max; best of 5, timed alone", "ms": lib_gemm_ms,
+                                 "N": int(n_after)},
     }
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(sc, keys, owner, n_vox, desc, n_steps=1)
