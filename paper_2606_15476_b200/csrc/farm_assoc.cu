@@ -56,12 +56,12 @@ __device__ __noinline__ void match_hellinger(const double *det_gm, const double 
 //   score (R17), atomicMax into best_cand[d].
 // Phase 2 (the last CTA to finish, found by a ticket): decisions for all detections (R18), new ids by an
 //   exclusive scan in detection index order (R20), per-target leader / group size for the merge.
-constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PRE = 4;  // 512 x 52 registers fit beside the similarity CTA
+constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PER = 4;  // 512 x 52 registers fit beside the similarity CTA
 
 template <typename T>
 // 80 registers: 512 x 80 fits beside the similarity CTA (256 x 80) and the phase-1 dot products overlap its tail
 __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
-  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per chunk of CAND_THREADS detections
+  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per pass
   __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
@@ -114,22 +114,8 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
       }
     }
   }
-  // ---- everything the association scan needs except best_cand is final before this kernel starts: requested here,
-  // ahead of the ticket, so that the scan of the last CTA starts with its operands in registers (M <= 2048)
-  const uint32_t N = __ldcg(m.n_objects);
-  unsigned long long valid_points = 0;
-  if (tid == 0) valid_points = __ldcg(&m.stats->valid_points);
-  uint32_t pre_nv[CAND_PRE], pre_npx[CAND_PRE];
-  unsigned long long pre_bd[CAND_PRE];
-#pragma unroll
-  for (int q = 0; q < CAND_PRE; ++q) {
-    const int j = q * CAND_THREADS + tid;
-    const bool in = j < a.M;
-    pre_nv[q] = in ? __ldcg(&m.det_nv[j]) : 0u;
-    pre_npx[q] = in ? __ldcg(&m.det_npx[j]) : 0u;
-    pre_bd[q] = (in && !a.wait_sim) ? __ldcg(&m.best_dense[j]) : 0ull;  // final only once similarity has finished
-  }
   // ---- ticket: the last CTA to arrive runs the association
+  const uint32_t N = __ldcg(m.n_objects);
   __syncthreads();
   if (tid == 0) {
     __threadfence();
@@ -140,7 +126,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
   }
   __syncthreads();
   if (!s_last) return;
-  if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid, then fetch its row maxima
+  if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid before reading its row maxima
     if (tid == 0) {
       uint32_t done;
       for (;;) {
@@ -150,85 +136,95 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
       }
     }
     __syncthreads();
-#pragma unroll
-    for (int q = 0; q < CAND_PRE; ++q) {
-      const int j = q * CAND_THREADS + tid;
-      pre_bd[q] = j < a.M ? __ldcg(&m.best_dense[j]) : 0ull;
-    }
   }
   __threadfence();
-  uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier chunks (every thread)
-  for (int base = 0; base < a.M; base += CAND_THREADS) {
-    const int j = base + tid;
-    const int q = base / CAND_THREADS;
-    uint32_t spawn = 0, matched = 0, skipped = 0;
-    int32_t target = -1;
-    float score = 0.f;
-    const bool in = j < a.M;
-    uint32_t my_nv = 0, my_npx = 0;
-    unsigned long long bd = 0;
-    if (q < CAND_PRE) {
+  // Each thread decides CAND_PER consecutive detections; one pass (one barrier) per CAND_THREADS * CAND_PER detections.
+  uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier passes (every thread)
+  for (int base = 0; base < a.M; base += CAND_THREADS * CAND_PER) {
+    const int j0 = base + tid * CAND_PER;
+    unsigned long long bc[CAND_PER], bd[CAND_PER];
+    uint32_t npx[CAND_PER];
 #pragma unroll
-      for (int k = 0; k < CAND_PRE; ++k)
-        if (k == q) my_nv = pre_nv[k], my_npx = pre_npx[k], bd = pre_bd[k];
-    } else if (in) {
-      my_nv = __ldcg(&m.det_nv[j]), my_npx = __ldcg(&m.det_npx[j]), bd = __ldcg(&m.best_dense[j]);
+    for (int k = 0; k < CAND_PER; ++k) {  // all loads of the pass up front
+      const bool in = j0 + k < a.M;
+      bc[k] = in ? __ldcg(&m.best_cand[j0 + k]) : 0ull;
+      bd[k] = in ? __ldcg(&m.best_dense[j0 + k]) : 0ull;
+      npx[k] = in ? __ldcg(&m.det_npx[j0 + k]) : 0u;
+      nv_sum += in ? __ldcg(&m.det_nv[j0 + k]) : 0u;
     }
-    nv_sum += my_nv;
-    if (in) {
-      if (my_npx == 0) {
-        skipped = 1;  // R8
-      } else {
-        unsigned long long best = __ldcg(&m.best_cand[j]);
-        if (bd) {
-          // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
-          const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd)));
-          const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd) : 0u);
-          best = pd > best ? pd : best;
-        }
-        if (best) {
-          score = unpack_score(best);
-          if (score > m.tau) {  // strict (R18)
-            matched = 1;
-            target = (int32_t)unpack_id(best);
-          }
-        }
-        spawn = matched ? 0u : 1u;
+    uint32_t spawn_bits = 0, match_bits = 0, skip_bits = 0;
+    int32_t target[CAND_PER];
+    float score[CAND_PER];
+#pragma unroll
+    for (int k = 0; k < CAND_PER; ++k) {
+      target[k] = -1, score[k] = 0.f;
+      if (j0 + k >= a.M) continue;
+      if (npx[k] == 0) {
+        skip_bits |= 1u << k;  // R8
+        continue;
       }
+      unsigned long long best = bc[k];
+      if (bd[k]) {
+        // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
+        const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd[k])));
+        const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd[k]) : 0u);
+        best = pd > best ? pd : best;
+      }
+      bool matched = false;
+      if (best) {
+        score[k] = unpack_score(best);
+        if (score[k] > m.tau) {  // strict (R18)
+          matched = true;
+          target[k] = (int32_t)unpack_id(best);
+        }
+      }
+      if (matched) match_bits |= 1u << k; else spawn_bits |= 1u << k;
     }
-    // block exclusive scan of the spawn flags: ballot inside the warp, shuffle scan over the 32 warp counts
-    const unsigned b = __ballot_sync(0xFFFFFFFFu, spawn);
-    uint32_t *ws = warp_sum2[q & 1];
-    if (lane == 0) ws[warp] = __popc(b);
-    __syncthreads();
-    uint32_t incl = lane < CAND_WARPS ? ws[lane] : 0u;
+    // block exclusive scan of the spawn counts (detections are consecutive inside a thread, threads inside a warp)
+    const uint32_t mine = __popc(spawn_bits);
+    uint32_t incl = mine;
 #pragma unroll
     for (int sft = 1; sft < 32; sft <<= 1) {
       const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, sft);
       if (lane >= sft) incl += up;
     }
-    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    const uint32_t before = __shfl_sync(0xFFFFFFFFu, incl, warp) - ws[warp];
-    if (spawn) {
-      const uint32_t id = N + running + before + __popc(b & ((1u << lane) - 1));
-      if (id < m.max_objects) {
-        target = (int32_t)id;
-      } else {
-        atomicOr(m.err, ERR_OBJECT_CAPACITY);
-        spawn = 0, skipped = 1;
+    uint32_t *ws = warp_sum2[(base / (CAND_THREADS * CAND_PER)) & 1];
+    if (lane == 31) ws[warp] = incl;
+    __syncthreads();
+    uint32_t wincl = lane < CAND_WARPS ? ws[lane] : 0u;
+#pragma unroll
+    for (int sft = 1; sft < 32; sft <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, wincl, sft);
+      if (lane >= sft) wincl += up;
+    }
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, wincl, 31);
+    const uint32_t before_warp = __shfl_sync(0xFFFFFFFFu, wincl, warp) - ws[warp];
+    uint32_t next_id = N + running + before_warp + (incl - mine);
+#pragma unroll
+    for (int k = 0; k < CAND_PER; ++k) {
+      const int j = j0 + k;
+      if (j >= a.M) continue;
+      uint32_t is_new = 0;
+      if ((spawn_bits >> k) & 1u) {
+        if (next_id < m.max_objects) {
+          target[k] = (int32_t)next_id;
+          is_new = 1;
+        } else {
+          atomicOr(m.err, ERR_OBJECT_CAPACITY);
+          skip_bits |= 1u << k;
+        }
+        ++next_id;
+      }
+      if (m.det_gm && ((match_bits >> k) & 1u)) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, target[k], npx[k]);  // G4
+      m.assoc[j] = target[k];
+      m.is_new[j] = (uint8_t)is_new;
+      m.best_score[j] = score[k];
+      if (target[k] >= 0) {
+        atomicMin(&m.leader[target[k]], (uint32_t)j);
+        atomicAdd(&m.grp_cnt[target[k]], 1u);
       }
     }
-    if (in) {
-      if (m.det_gm && matched) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, target, my_npx);  // G4
-      m.assoc[j] = target;
-      m.is_new[j] = (uint8_t)spawn;
-      m.best_score[j] = score;
-      if (target >= 0) {
-        atomicMin(&m.leader[target], (uint32_t)j);
-        atomicAdd(&m.grp_cnt[target], 1u);
-      }
-    }
-    n_matched += matched, n_skipped += skipped;
+    n_matched += __popc(match_bits), n_skipped += __popc(skip_bits);
     running += total;
   }
   n_matched = __reduce_add_sync(0xFFFFFFFFu, n_matched);
@@ -251,7 +247,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
     m.stats->unique_voxels = pairs;
     atomicAdd(&m.totals->frames, (unsigned long long)a.F);
     atomicAdd(&m.totals->calls, 1ull);
-    atomicAdd(&m.totals->valid_points, valid_points);
+    atomicAdd(&m.totals->valid_points, __ldcg(&m.stats->valid_points));
     atomicAdd(&m.totals->unique_voxels, pairs);
     atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
     atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
