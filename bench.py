@@ -51,6 +51,7 @@ def peaks():
     if os.path.exists(path):
         d = json.load(open(path))
         return {"hbm_gbs": d["hbm_gbs"], "tf_burst": d["bf16_tflops"], "tf_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
                 "source": "measured (MEASURED_PEAKS.json)"}
     return {"hbm_gbs": 6650.0, "tf_burst": 1590.0, "tf_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
 
@@ -358,6 +359,19 @@ def run_ours(args):
     roofline_hbm = {"kernel": "lift_voxelise + probe (steps 1-3)", "bound": "hbm", "achieved": lift_gbs, "peak": pk["hbm_gbs"],
                     "unit": "GB/s", "frac": (lift_gbs / pk["hbm_gbs"]) if lift_gbs else None,
                     "traffic": tinfo.get("lift_dram_bytes_per_launch"), "ms_per_launch": lift_ms, "bytes_per_launch": lift_bytes}
+    # The lift kernel is bound by instruction issue, not by bytes: warp instructions per launch
+    # from the committed ncu capture (profiles/traffic.json), peak = 148 SMs x 4 schedulers x 1 instruction per clock
+    # at the maximum SM clock; time from the breakdown pass (kernel bracketed by events, similarity running beside it)
+    lift_only_ms = float(bd_ms[binding.STAGE_NAMES.index("lift")])
+    lift_inst = tinfo.get("lift_warp_instructions_per_launch")
+    issue_peak = 148 * 4 * pk.get("sm_max_mhz", 1965.0) * 1e6
+    roofline_alu = None
+    if lift_inst and lift_only_ms > 0:
+        ach = lift_inst / (lift_only_ms * 1e-3)
+        roofline_alu = {"kernel": "lift_voxelise (steps 1-2)", "bound": "alu", "achieved": ach, "peak": issue_peak,
+                        "unit": "warp-instructions/s", "frac": ach / issue_peak, "ms_per_launch": lift_only_ms,
+                        "warp_instructions_per_launch": lift_inst,
+                        "peak_source": "148 SMs x 4 issue slots per clock x max SM clock (guide unit counts)"}
     step_bytes = px_bytes + M * cfg.D * 2 + n_mean * cfg.D * 2 + pairs * (8 + 16 + 16) + M * cfg.D * (4 + 4 + 2)
     out = {
         "metric": "mapping_frames_per_sec", "value": value, "unit": "frames/s", "n_gpus": world, "steps": K_steps,
@@ -376,6 +390,7 @@ def run_ours(args):
         "e2e": e2e,
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
+        "roofline_lift_alu": roofline_alu,
         "step_algorithmic_bytes": step_bytes,
         "step_hbm_frac_literal": step_bytes / (ms / K_steps * 1e-3) / 1e9 / pk["hbm_gbs"],
         "stage_ms_per_step": {n: float(stage_ms[i]) / max(K_steps, 1) for i, n in enumerate(binding.STAGE_NAMES)},
