@@ -66,7 +66,6 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  pdl_trigger();  // the merge kernel may become resident while the decision scan runs
   pdl_wait();     // launched with PDL behind the probe kernel: candidates and overlap counts are final from here on
   {
     const uint32_t n_cand = min(m.counters[1], m.cand_cap);
@@ -137,6 +136,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
     }
     __syncthreads();
   }
+  pdl_trigger();  // the merge kernel becomes resident now, not while the similarity kernel still runs
   __threadfence();
   // Each thread decides CAND_PER consecutive detections; one pass (one barrier) per CAND_THREADS * CAND_PER detections.
   uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier passes (every thread)
