@@ -117,6 +117,7 @@ class FarmMap:
                  stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
+        self._last_M = 0
         self._h = C.c_void_p()
         _check(lib.farm_map_create(voxel_size, D, w_geo, w_sem, tau, C.byref(self._h)))
         self.set_option_i(OPT_IMG_H, H)

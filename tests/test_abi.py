@@ -46,6 +46,17 @@ def test_host_side_validation_without_gpu(lib):
         m.set_option_i(999, 1)
     with pytest.raises(FarmError):
         m.set_option_i(1, 7)                                 # bad dtype
+    from paper_2606_15476_b200 import binding
+    for key, bad in ((binding.OPT_MAX_BLOCKS, 0), (binding.OPT_GAUSSIAN, 2), (binding.OPT_COVISIBILITY, -1),
+                     (binding.OPT_MAX_DET_PER_CALL, 1 << 16), (binding.OPT_MAX_FRAMES_PER_CALL, 65)):
+        with pytest.raises(FarmError):
+            m.set_option_i(key, bad)
+    for key, good in ((binding.OPT_MAX_BLOCKS, 1 << 12), (binding.OPT_GAUSSIAN, 1), (binding.OPT_COVISIBILITY, 1),
+                      (binding.OPT_TIMING, 2)):
+        m.set_option_i(key, good)
+    with pytest.raises(FarmError) as ei:
+        m.last_gaussians()                                   # no integrate call yet: FARM_ERR_STATE, not a crash
+    assert ei.value.code == -4
     objs, desc, keys, owners = m.read()                      # empty, never touched the device
     assert len(objs) == 0 and len(keys) == 0
     m.destroy()
