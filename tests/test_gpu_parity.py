@@ -541,3 +541,32 @@ def test_descriptor_lengths_off_the_vector_paths(oracle, dtype, D):
         gpu_integrate(g, frames, dtype)
         compare_call(g, o)
     compare_maps(g, o)
+
+
+def test_epoch_tag_wraparound_after_65534_calls(oracle):
+    """The per-call scratch tables are never cleared: their keys carry a 16-bit call epoch, and the tables are
+    wiped once when it wraps.  65,700 calls that keep re-observing the same two objects must leave exactly the
+    oracle's map, and the calls right after the wrap must still report exact voxel sets and overlaps."""
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.25, 4, 0.5, 0.5, 0.5, 0
+    H, W = 16, 32
+    I4 = np.eye(4, dtype=np.float32)
+    e = np.eye(4, dtype=np.float32)
+    o, g = make_pair(oracle, Cfg, H=H, W=W)
+    px = [(u, v, 2.0, 1) for v in range(4, 8) for u in range(4, 12)] + [(u, v, 3.0, 2) for v in range(9, 13) for u in range(16, 28)]
+    depth, mask = hand_frame(H, W, px)
+    K = np.array([[16, 0, 16], [0, 16, 8], [0, 0, 1]], np.float32)
+    fr = S.Frame(depth, mask, K, I4, np.ascontiguousarray(e[:2]), 2, np.zeros(2, np.int64))
+    d = upload([fr], 0)
+    n_calls, o_calls = 65700, 0
+    for k in range(n_calls):
+        g.integrate_batch(1, d["depth"], d["mask"], d["K"], d["T"], d["desc"], d["n_det"])
+        if k in (0, 1, 65532, 65533, 65534, 65535, 65536, n_calls - 1):
+            while o_calls <= k:                                      # bring the oracle to the same call
+                integrate_frames(o, [fr])
+                o_calls += 1
+            compare_call(g, o)
+    compare_maps(g, o)
+    objs, _, _, _ = g.read()
+    assert len(objs) == 2 and objs["n_obs"][0] == n_calls
+
