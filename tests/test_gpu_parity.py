@@ -570,3 +570,27 @@ def test_epoch_tag_wraparound_after_65534_calls(oracle):
     objs, _, _, _ = g.read()
     assert len(objs) == 2 and objs["n_obs"][0] == n_calls
 
+
+
+def test_block_table_and_scratch_overflow_are_loud(oracle):
+    """Data-dependent capacity failures never truncate silently: too few voxel blocks, or too few per-call pair
+    slots, set the sticky device error that the next sync / read / last_assoc returns as FARM_ERR_CAPACITY."""
+    from paper_2606_15476_b200 import FarmError
+    H, W = 24, 256
+    g0 = np.random.default_rng(11)
+    depth = (1.0 + 4.0 * g0.random((H, W))).astype(np.float32)       # ~ every pixel in its own voxel block
+    mask = np.ones((H, W), np.uint16)
+    K = np.array([[100, 0, 128], [0, 100, 12], [0, 0, 1]], np.float32)
+    fr = S.Frame(depth, mask, K, np.eye(4, dtype=np.float32), unit_rows(1, 8, 5), 1, np.zeros(1, np.int64))
+    g = FarmMap(0.01, 8, 0.5, 0.5, 0.5, H=H, W=W, max_blocks=64)      # 1024 block slots for ~6000 blocks
+    gpu_integrate(g, [fr], 0)
+    with pytest.raises(FarmError) as ei:
+        g.sync()
+    assert ei.value.code == -3 and "voxel table full" in str(ei.value)
+    with pytest.raises(FarmError):                                   # sticky
+        g.read()
+    g2 = FarmMap(0.01, 8, 0.5, 0.5, 0.5, H=H, W=W, max_pairs_per_call=1024)
+    gpu_integrate(g2, [fr], 0)
+    with pytest.raises(FarmError) as ei:
+        g2.last_assoc()
+    assert ei.value.code == -3
