@@ -42,7 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if failed:
         raise RuntimeError("nvcc failed")
     if force or procs or _stale(LIB, objs):
-        subprocess.check_call([NVCC, "-shared", "-o", LIB + ".tmp"] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+        subprocess.check_call([NVCC, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB + ".tmp"] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
         os.replace(LIB + ".tmp", LIB)
     return LIB
 
