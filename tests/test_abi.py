@@ -82,3 +82,36 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "farm_oracle" not in src and "import oracle" not in src and "from oracle" not in src, f
+
+
+def test_header_is_plain_c_and_links_from_c(lib, tmp_path):
+    """The boundary is a C ABI: include/farm.h compiles as C99 (-pedantic) and a plain C program links against
+    libfarm_map.so and drives the host-side part of it (no GPU needed: nothing here touches the device)."""
+    import shutil
+    import subprocess
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    from paper_2606_15476_b200 import binding
+    src = tmp_path / "t.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "farm.h"
+int main(void) {
+  farm_map *m = NULL;
+  int n = -1;
+  long long nv = -1;
+  if (farm_map_create(0.05f, 64, 0.5f, 0.5f, 0.5f, &m) != FARM_OK) return 1;
+  if (farm_map_set_option_i(m, FARM_OPT_IMG_W, 160) || farm_map_set_option_i(m, FARM_OPT_IMG_H, 120)) return 2;
+  if (farm_map_set_option_i(m, FARM_OPT_DESC_DTYPE, 9) != FARM_ERR_INVALID_ARG) return 3;
+  if (farm_map_read(m, NULL, &n, NULL, NULL, NULL, &nv) != FARM_OK || n != 0 || nv != 0) return 4;
+  printf("%s|%d\n", farm_last_error(), (int)sizeof(farm_object));
+  return farm_map_destroy(m);
+}
+''')
+    exe = tmp_path / "t"
+    libdir = os.path.dirname(binding.LIB_PATH)
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                           str(src), "-o", str(exe), "-L", libdir, "-lfarm_map", f"-Wl,-rpath,{libdir}"])
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, out
+    assert out.stdout.strip() == f"bad dtype|{binding.OBJECT_DTYPE.itemsize}"
