@@ -58,13 +58,15 @@ def test_config0_full_sequence(oracle):
 def test_config1_prefix_f16(oracle):
     """configs[1] (room, D=512 fp16, misses and false positives): a prefix spanning many tiles."""
     cfg = S.get_config(1)
-    _run_sequence(oracle, cfg, 1, 10, start=25)
+    o, g = _run_sequence(oracle, cfg, 1, 36, start=20)
+    objs, _, _, _ = g.read(voxels=False)
+    assert len(objs) > 40 and objs["n_obs"].max() > 5          # the map grows and objects are re-observed
 
 
 def test_config2_prefix_bf16(oracle):
     """configs[2] (house, D=1024 bf16, 0.9-cosine distractor clusters)."""
     cfg = S.get_config(2)
-    _run_sequence(oracle, cfg, 1, 6, start=0)
+    _run_sequence(oracle, cfg, 1, 14, start=0)
 
 
 def test_config3_prefix_outdoor_bf16(oracle):
