@@ -278,7 +278,7 @@ def test_config4_full_size_sampled_against_oracle(oracle):
     assert int(stg["n_det"]) == F * DET and int(stg["matches"]) == F * DET // 2 and int(stg["spawns"]) == F * DET // 2
     assert int(stg["unique_voxels"]) == int(offg[-1])
     checked = 0
-    for f in (0, 7, 15):
+    for f in (0, 3, 7, 10, 12, 15):
         oc = o.clone()
         integrate_frames(oc, [frames[f]])
         ao, no, bo, so, sto = oc.last_assoc()
@@ -300,7 +300,7 @@ def test_config4_full_size_sampled_against_oracle(oracle):
             if not no[d]:
                 assert ag[j] == ao[d]                      # matched: same object; spawned ids depend on the whole call
             checked += 1
-    assert checked > 250
+    assert checked > 500
     # new ids in detection index order (R20)
     new_ids = ag[ng.astype(bool)]
     assert np.array_equal(new_ids, N0 + np.arange(len(new_ids)))
