@@ -596,3 +596,18 @@ def test_block_table_and_scratch_overflow_are_loud(oracle):
     with pytest.raises(FarmError) as ei:
         g2.last_assoc()
     assert ei.value.code == -3
+
+
+@pytest.mark.parametrize("overlap,sim_path", [(0, 0), (2, 0), (3, 0), (1, 1), (1, 2)])
+def test_stream_orders_and_similarity_paths_give_the_same_map(oracle, overlap, sim_path):
+    """The launch orders (FARM_OPT_OVERLAP 0 / 2 / 3 beside the default 1) and the forced similarity paths
+    (CUDA-core FMA, tcgen05) are different schedules of the same rules: every one must reproduce the oracle."""
+    cfg = S.get_config(1)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg, overlap=overlap, sim_path=sim_path)
+    for k in range(20, 28):
+        frames = margin_filter(o.clone, [sc.frame(k)], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+    compare_maps(g, o)
