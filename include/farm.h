@@ -45,7 +45,7 @@ extern "C" {
 #define FARM_ERR_CUDA (-2)
 #define FARM_ERR_CAPACITY (-3)
 #define FARM_ERR_STATE (-4)
-#define FARM_ERR_RANGE (-5)
+#define FARM_ERR_RANGE (-5) /* reserved: points outside the key range are dropped and counted (stats), never an error */
 
 #define FARM_KEY_EMPTY 0xFFFFFFFFFFFFFFFFull
 
