@@ -100,6 +100,14 @@ class OracleMap:
         lib().oracle_last_assoc(self.h, _p(assoc), _p(is_new), _p(best), _p(second), _p(st))
         return assoc, is_new, best, second, st[0]
 
+    def last_dense(self):
+        """R16: (max_o clamp(cos) [M], argmax [M], lowest id on ties; (0, -1) for skipped detections / empty map)."""
+        M = lib().oracle_last_M(self.h)
+        mc = np.zeros(M, np.float32)
+        am = np.zeros(M, np.int32)
+        lib().oracle_last_dense(self.h, _p(mc), _p(am))
+        return mc, am
+
     def last_voxels(self):
         M = lib().oracle_last_M(self.h)
         off = np.empty(M + 1, np.int64)
