@@ -68,7 +68,10 @@ extern "C" {
 #define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the similarity kernel only; 2 around every kernel (this
                                         serialises the programmatically chained kernels).  May be changed at any time    */
 #define FARM_OPT_OVERLAP 12          /* 1 (default): similarity on an internal side stream, concurrent with lift+probe;
-                                        0 one stream; 2 / 3 experimental orders (see farm_api.cu)                      */
+                                        0 one stream; 2 / 3 experimental orders (see farm_api.cu).  Mode 1 needs the grids of
+                                        one call to be co-resident (device-side waits between them, bounded: on expiry the
+                                        sticky error reports FARM_ERR_STATE); with CUDA_LAUNCH_BLOCKING set the library
+                                        uses mode 0                                                                    */
 #define FARM_OPT_MAX_BLOCKS 13       /* capacity in 4x4x4 voxel blocks (256 B each); table = next pow2 >= 2x;
                                         default MAX_VOXELS / 4.  Exceeding it sets the sticky capacity error           */
 #define FARM_OPT_GAUSSIAN 14         /* 1: also carry the paper's geometry: a 3-D Gaussian per
@@ -167,15 +170,18 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov);
  * received a detection in one integrate call.  Bits are never cleared.  Synchronises. */
 int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words);
 
-/* Export (HOST buffers).  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
+/* Export (HOST buffers) -- with farm_map_import the "scene state" persistence of PAPER.md:597 ("the memory is persisted
+ * as a scene state") reduced to this path's fields.  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
  * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary
  * order (may be NULL).  Synchronises; returns the sticky device error if set. */
 int farm_map_read(farm_map *m, farm_object *objects, int *n_objects, float *descriptors, uint64_t *voxel_keys,
                   uint32_t *voxel_owner, long long *n_voxels);
 
-/* Bulk load into an EMPTY map (checkpoint resume; pre-populated maps).  HOST pointers.  Objects are
+/* Bulk load into an EMPTY map (PAPER.md:597 scene-state resume; pre-populated maps).  HOST pointers.  Objects are
  * installed verbatim (ids must be 0..n-1 in order), descriptors are renormalised and shadowed (R26), every
- * voxel key must be unique and its owner < n_objects, else FARM_ERR_INVALID_ARG. */
+ * voxel key must be unique, its owner < n_objects, and objects[i].n_voxels must equal the number of voxels listed
+ * for i, else FARM_ERR_INVALID_ARG.  The frame counter is not part of the object records: a resumed map continues
+ * its numbering with farm_map_set_frame_seq (else new frames start at 0 and tie with imported best views). */
 int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, const float *descriptors,
                     const uint64_t *voxel_keys, const uint32_t *voxel_owner, long long n_voxels);
 
@@ -185,18 +191,23 @@ int farm_map_sync(farm_map *m, farm_totals *totals);
 /* Per-stage device time accumulated since the last reset (needs FARM_OPT_TIMING >= 1; stages that are not
  * bracketed report 0) and kernel launches per stage.  ms / launches: HOST arrays [FARM_N_STAGES], may be
  * NULL.  Synchronises the stream. */
-#define FARM_N_STAGES 7
+#define FARM_N_STAGES 6
 #define FARM_STAGE_PREP 0        /* reset of per-call state + detection row norms            */
 #define FARM_STAGE_LIFT 1        /* steps 1-2: back-project, voxelise, tile-level dedupe       */
 #define FARM_STAGE_SIMILARITY 2  /* step 4: dense cosine with fused row max / argmax          */
 #define FARM_STAGE_PROBE 3       /* step 3: voxel hash probe / insert, exact dedupe, overlap   */
 #define FARM_STAGE_ASSOCIATE 4   /* step 5a: candidate scores, argmax, threshold, new ids     */
-#define FARM_STAGE_UNUSED 5
-#define FARM_STAGE_MERGE 6       /* step 5b: voxel commit, descriptors, AABB, view evidence   */
+#define FARM_STAGE_MERGE 5       /* step 5b: voxel commit, descriptors, AABB, view evidence   */
 int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset);
 
 /* Number of kernels this library has launched for the map so far (host counter). */
 long long farm_map_kernel_launches(const farm_map *m);
+
+/* Frame sequence number the next integrated frame will get (R23 best-view records carry it).  It starts at 0, advances
+ * by the number of frames of every integrate call, can only be moved forward, and must stay <= INT32_MAX
+ * (farm_object.best_frame is 32-bit): integrate returns FARM_ERR_STATE beyond that. */
+int farm_map_get_frame_seq(farm_map *m, long long *frame_seq);
+int farm_map_set_frame_seq(farm_map *m, long long frame_seq);
 
 /* Thread-local description of the last error returned on this thread. */
 const char *farm_last_error(void);

@@ -110,7 +110,7 @@ struct Map {
   std::vector<int32_t> assoc;
   std::vector<uint8_t> is_new;
   std::vector<float> best_score, second_score;
-  std::vector<float> dense_max;                      // R16: max_o clamp(cos(a_d, shadow_o)) over ALL entry objects
+  std::vector<float> dense_max, dense_second;        // R16: max_o clamp(cos(a_d, shadow_o)) over ALL entry objects; runner-up
   std::vector<int32_t> dense_arg;                    //      and its argmax (lowest id on ties), -1 if N = 0 / skipped
   std::vector<std::set<uint64_t>> V;                 // R7
   std::vector<uint32_t> n_px;                        // R7
@@ -303,6 +303,7 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
   m.best_score.assign(M, 0.0f);
   m.second_score.assign(M, -std::numeric_limits<float>::infinity());
   m.dense_max.assign(M, 0.0f);
+  m.dense_second.assign(M, -std::numeric_limits<float>::infinity());
   m.dense_arg.assign(M, -1);
   m.V.assign(M, {});
   m.n_px.assign(M, 0);
@@ -377,8 +378,11 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     for (int o = 0; o < N; ++o) {                                // R16: every pair
       const float c = cosine(a.data(), m.objs[o].shadow.data(), D);  // R15
       if (m.dense_arg[j] < 0 || c > m.dense_max[j]) {            // R16 dense row max, ties -> lowest id
+        if (m.dense_arg[j] >= 0) m.dense_second[j] = std::fmax(m.dense_second[j], m.dense_max[j]);
         m.dense_max[j] = c;
         m.dense_arg[j] = o;
+      } else {
+        m.dense_second[j] = std::fmax(m.dense_second[j], c);
       }
       float g = 0.0f;                                            // R10
       auto it = m.overlap[j].find((uint32_t)o);
@@ -510,11 +514,12 @@ void oracle_last_assoc(void *h, int32_t *assoc, uint8_t *is_new, float *best, fl
 }
 // R16 / R19: dense row maximum of the clamped cosine over all entry objects and its argmax (lowest id on ties);
 // (0, -1) for skipped detections and for an empty map.
-void oracle_last_dense(void *h, float *max_cos, int32_t *argmax) {
+void oracle_last_dense(void *h, float *max_cos, int32_t *argmax, float *second) {
   Map &m = *(Map *)h;
   for (int j = 0; j < m.M; ++j) {
     if (max_cos) max_cos[j] = m.dense_max[j];
     if (argmax) argmax[j] = m.dense_arg[j];
+    if (second) second[j] = m.dense_second[j];  // runner-up value (-inf when N < 2); used by tests for margins only
   }
 }
 // CSR of V_d (keys ascending inside a detection), n_px, box.  offsets has M+1 entries.

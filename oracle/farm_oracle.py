@@ -105,8 +105,15 @@ class OracleMap:
         M = lib().oracle_last_M(self.h)
         mc = np.zeros(M, np.float32)
         am = np.zeros(M, np.int32)
-        lib().oracle_last_dense(self.h, _p(mc), _p(am))
+        lib().oracle_last_dense(self.h, _p(mc), _p(am), None)
         return mc, am
+
+    def last_dense_second(self):
+        """runner-up of the dense row maximum (-inf when N < 2); tests use it to skip near-ties"""
+        M = lib().oracle_last_M(self.h)
+        sec = np.zeros(M, np.float32)
+        lib().oracle_last_dense(self.h, None, None, _p(sec))
+        return sec
 
     def last_voxels(self):
         M = lib().oracle_last_M(self.h)

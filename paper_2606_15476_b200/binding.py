@@ -23,8 +23,8 @@ OPT_OVERLAP = 12
 OPT_MAX_BLOCKS = 13
 OPT_GAUSSIAN = 14
 OPT_COVISIBILITY = 15
-N_STAGES = 7
-STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "unused", "merge"]
+N_STAGES = 6
+STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
 KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
 
@@ -42,6 +42,7 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians", "farm_map_read_covisibility",
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
+           "farm_map_get_frame_seq", "farm_map_set_frame_seq",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -81,6 +82,8 @@ def load_library():
         lib.farm_map_sync.argtypes = [vp, vp]
         lib.farm_map_kernel_launches.argtypes = [vp]
         lib.farm_map_kernel_launches.restype = ll
+        lib.farm_map_get_frame_seq.argtypes = [vp, C.POINTER(ll)]
+        lib.farm_map_set_frame_seq.argtypes = [vp, ll]
         lib.farm_last_error.restype = C.c_char_p
         lib.farm_debug_backproject.argtypes = [vp, vp, vp, vp, vp, ci, vp, vp]
         lib.farm_debug_last_voxels.argtypes = [vp, vp, vp, vp, vp]
@@ -259,6 +262,14 @@ class FarmMap:
 
     def kernel_launches(self):
         return int(load_library().farm_map_kernel_launches(self._h))
+
+    def get_frame_seq(self):
+        v = C.c_longlong(0)
+        _check(load_library().farm_map_get_frame_seq(self._h, C.byref(v)))
+        return v.value
+
+    def set_frame_seq(self, frame_seq):
+        _check(load_library().farm_map_set_frame_seq(self._h, int(frame_seq)))
 
     # ---- parity / debug
     def debug_backproject(self, depth, instance_mask, K, T_world_cam, n_det, xyz, keys):

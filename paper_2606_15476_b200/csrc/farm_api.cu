@@ -14,6 +14,7 @@
 namespace farm {
 int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target,
                          int *n_ctas);
+bool tc_prepare(void *tc_state, const DevMap &m, const CallArgs &a);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
 bool tc_supported(const DevMap &m);
@@ -98,11 +99,11 @@ __global__ void export_objects_kernel(DevMap m, farm_object *out, uint32_t n) {
     o.aabb_max[k] = ord2f(m.aabb[i * 6 + 3 + k]);
     o.best_cam_pos[k] = m.best_cam[i * 3 + k];
   }
-  const unsigned long long bv = m.best_view[i];
-  if (bv) {
-    o.best_pixels = (uint32_t)(bv >> 40);
-    o.best_frame = (int32_t)(~(bv >> 16) & 0xFFFFFFull);
-    o.best_det = (int32_t)(~bv & 0xFFFFull);
+  const uint32_t bp = m.best_px[i];
+  if (bp) {
+    o.best_pixels = bp;
+    o.best_frame = (int32_t)m.best_seq[i];  // integrate refuses frame sequence numbers beyond INT32_MAX (FARM_ERR_STATE)
+    o.best_det = (int32_t)m.best_det[i];
   } else {
     o.best_pixels = 0, o.best_frame = -1, o.best_det = -1;
   }
@@ -122,10 +123,20 @@ __global__ void import_objects_kernel(DevMap m, const farm_object *in, uint32_t 
     m.aabb[i * 6 + 3 + k] = f2ord(o.aabb_max[k]);
     m.best_cam[i * 3 + k] = o.best_cam_pos[k];
   }
-  m.best_view[i] = o.best_frame < 0 ? 0ull
-                                    : ((unsigned long long)(o.best_pixels & 0xFFFFFFu) << 40) |
-                                          ((~(unsigned long long)o.best_frame & 0xFFFFFFull) << 16) |
-                                          (~(unsigned long long)o.best_det & 0xFFFFull);
+  const bool has = o.best_frame >= 0 && o.best_pixels > 0;
+  m.best_px[i] = has ? o.best_pixels : 0u;
+  m.best_seq[i] = has ? (unsigned long long)o.best_frame : 0ull;
+  m.best_det[i] = has ? (uint32_t)o.best_det : 0u;
+}
+
+// import check: objects[i].n_voxels must equal the number of imported voxels owned by i (R10 divides by it)
+__global__ void count_owner_kernel(const uint32_t *owners, long long n, uint32_t n_objects, uint32_t *cnt) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    if (owners[i] < n_objects) atomicAdd(&cnt[owners[i]], 1u);
+}
+__global__ void check_owner_count_kernel(DevMap m, const uint32_t *cnt, uint32_t n_objects) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_objects && cnt[i] != m.n_voxels[i]) atomicOr(m.err, ERR_IMPORT_COUNT);
 }
 
 // R26: renormalise imported fp32 rows (fp32 arithmetic), write master, shadow and inverse shadow norm
@@ -274,12 +285,42 @@ int dev_alloc(farm_map *m, T **p, size_t count, int fill_byte) {
   return FARM_OK;
 }
 
+int finalise_impl(farm_map *m);
 int finalise(farm_map *m) {
   if (m->finalised) return FARM_OK;
+  const int rc = finalise_impl(m);
+  if (rc != FARM_OK) {  // leave nothing half-built behind: the next call starts from scratch
+    const std::string msg = g_err;
+    cudaDeviceSynchronize();
+    for (void *p : m->allocs) cudaFree(p);
+    m->allocs.clear();
+    if (m->tc) tc_state_destroy(m->tc), m->tc = nullptr;
+    if (m->side) cudaStreamDestroy(m->side), m->side = nullptr;
+    if (m->ev_fork) cudaEventDestroy(m->ev_fork), m->ev_fork = nullptr;
+    if (m->ev_join) cudaEventDestroy(m->ev_join), m->ev_join = nullptr;
+    m->dm = DevMap{};
+    cudaGetLastError();
+    g_err = msg;
+  }
+  return rc;
+}
+int finalise_impl(farm_map *m) {
   if (m->H <= 0 || m->W <= 0) return fail(FARM_ERR_STATE, "FARM_OPT_IMG_W / FARM_OPT_IMG_H must be set before the first call");
+  if ((long long)m->H * m->W > (1ll << 31) - 1) return fail(FARM_ERR_INVALID_ARG, "IMG_W * IMG_H must be below 2^31 (pixel counts are 32-bit)");
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
     return fail(FARM_ERR_CUDA, "no CUDA device: the FARM mapping path has no CPU fallback");
+  {
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    m->dm.num_sms = sms > 0 ? sms : 1;
+  }
+  // The default launch order (FARM_OPT_OVERLAP = 1 with the tensor-core similarity) needs grids of one call to be
+  // co-resident: the similarity epilogue waits for prep, the decision scan for the similarity grid.  When the
+  // process serialises kernel execution, fall back to the single-stream order, which has no device-side waits.
+  if (const char *lb = getenv("CUDA_LAUNCH_BLOCKING"))
+    if (lb[0] && lb[0] != '0') m->overlap = 0;
   if (m->max_blocks <= 0) m->max_blocks = std::max<long long>(m->max_voxels / 4, 1024);
   if (m->max_blocks > (1ll << 30)) return fail(FARM_ERR_INVALID_ARG, "voxel-block table too large (FARM_OPT_MAX_BLOCKS <= 2^30)");
   if (m->max_pairs <= 0) m->max_pairs = std::min<long long>((long long)m->H * m->W * std::min<long long>(m->max_frames, 4), 1ll << 23);
@@ -304,7 +345,9 @@ int finalise(farm_map *m) {
   A(d.n_obs, NO, 0);
   A(d.n_points, NO, 0);
   A(d.aabb, NO * 6, 0);
-  A(d.best_view, NO, 0);
+  A(d.best_px, NO, 0);
+  A(d.best_seq, NO, 0);
+  A(d.best_det, NO, 0);
   A(d.best_cam, NO * 3, 0);
   A(d.leader, NO, 0xFF);
   A(d.grp_cnt, NO, 0);
@@ -332,7 +375,7 @@ int finalise(farm_map *m) {
   A(d.cand_o, (size_t)ccap, 0);
   A(d.cand_c, (size_t)ccap, 0);
   d.cand_cap = (uint32_t)ccap;
-  const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30) + 148 * 8 * 512;  // + chunk padding of the lift CTAs
+  const long long scap = std::min<long long>(2 * m->max_pairs, 1ll << 30) + (long long)d.num_sms * 8 * 512;  // + chunk padding of the lift CTAs
   A(d.surv_key, (size_t)scap, 0);
   A(d.surv_bits, (size_t)scap, 0);
   A(d.surv_j, (size_t)scap, 0);
@@ -402,12 +445,15 @@ int device_error(farm_map *m) {
   CU(cudaMemcpyAsync(&e, m->dm.err, 4, cudaMemcpyDeviceToHost, m->stream));
   CU(cudaStreamSynchronize(m->stream));
   if (e == 0) return FARM_OK;
-  char buf[160];
-  snprintf(buf, sizeof buf, "sticky device error 0x%x:%s%s%s%s%s", e, (e & ERR_VOXEL_TABLE_FULL) ? " voxel table full" : "",
+  char buf[320];
+  snprintf(buf, sizeof buf, "sticky device error 0x%x:%s%s%s%s%s%s%s", e, (e & ERR_VOXEL_TABLE_FULL) ? " voxel table full" : "",
            (e & ERR_PAIR_TABLE_FULL) ? " per-call pair scratch full" : "",
            (e & ERR_OVERLAP_TABLE_FULL) ? " per-call overlap scratch full" : "",
-           (e & ERR_OBJECT_CAPACITY) ? " object capacity" : "", (e & ERR_IMPORT_DUPLICATE) ? " import: duplicate key or bad owner" : "");
-  return fail((e & ERR_IMPORT_DUPLICATE) ? FARM_ERR_INVALID_ARG : FARM_ERR_CAPACITY, buf);
+           (e & ERR_OBJECT_CAPACITY) ? " object capacity" : "", (e & ERR_IMPORT_DUPLICATE) ? " import: duplicate key or bad owner" : "",
+           (e & ERR_IMPORT_COUNT) ? " import: an object's n_voxels differs from the voxels listed for it" : "",
+           (e & ERR_SYNC_TIMEOUT) ? " a device-side wait between the grids of one call expired (kernels serialised? use FARM_OPT_OVERLAP = 0)" : "");
+  if (e & (ERR_IMPORT_DUPLICATE | ERR_IMPORT_COUNT)) return fail(FARM_ERR_INVALID_ARG, buf);
+  return fail((e & ERR_SYNC_TIMEOUT) ? FARM_ERR_STATE : FARM_ERR_CAPACITY, buf);
 }
 
 }  // namespace
@@ -554,10 +600,15 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
     CU(cudaMemsetAsync(m->dm.ov_keys, 0, ((size_t)m->dm.ov_mask + 1) * 8, m->stream));
     m->epoch = 0;
   }
+  if (m->frame_seq + (unsigned long long)F > 0x7FFFFFFFull)
+    return fail(FARM_ERR_STATE, "frame sequence number would exceed INT32_MAX (farm_object.best_frame is 32-bit)");
   a.M = (int)M;
-  a.epoch = ++m->epoch;
   a.depth = depth, a.mask = mask, a.K = K, a.T = T, a.desc = desc;
   const DevMap &d = m->dm;
+  // everything that can fail on the host is checked before the first enqueue: the map stays untouched on error
+  if (m->tc && M > 0 && m->n_upper > 0 && !tc_prepare(m->tc, d, a))
+    return fail(FARM_ERR_INVALID_ARG, "similarity: det_descriptors must be 16-byte aligned for the 16-bit dtypes (TMA operand)");
+  a.epoch = ++m->epoch;
   cudaStream_t st = m->stream;
   bool launch_failed = false;
   auto stage = [&](int id, cudaStream_t st, auto &&fn) {
@@ -622,12 +673,13 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
   if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
-  CU(cudaGetLastError());
-  if (launch_failed) return fail(FARM_ERR_CUDA, "similarity: cuTensorMapEncodeTiled failed (descriptor pointer must be 16-byte aligned)");
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
   m->last_M = (int)M;
   m->has_last = true;
+  // the host counters above describe what was enqueued, whatever the launch status says
+  CU(cudaGetLastError());
+  if (launch_failed) return fail(FARM_ERR_CUDA, "a kernel launch of the call failed");
   return FARM_OK;
 }
 
@@ -651,6 +703,20 @@ int farm_map_sync(farm_map *m, farm_totals *totals) {
 }
 
 long long farm_map_kernel_launches(const farm_map *m) { return m ? m->launches : 0; }
+
+int farm_map_get_frame_seq(farm_map *m, long long *frame_seq) {
+  if (!m || !frame_seq) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  *frame_seq = (long long)m->frame_seq;
+  return FARM_OK;
+}
+
+int farm_map_set_frame_seq(farm_map *m, long long frame_seq) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (frame_seq < 0 || frame_seq > 0x7FFFFFFFll) return fail(FARM_ERR_INVALID_ARG, "frame_seq must be in 0..INT32_MAX");
+  if ((unsigned long long)frame_seq < m->frame_seq) return fail(FARM_ERR_STATE, "frame_seq can only move forward");
+  m->frame_seq = (unsigned long long)frame_seq;
+  return FARM_OK;
+}
 
 int farm_map_last_assoc(farm_map *m, int32_t *obj_id, uint8_t *is_new, float *best_score, farm_frame_stats *stats) {
   if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
@@ -683,7 +749,7 @@ int farm_map_read(farm_map *m, farm_object *objects, int *n_objects, float *desc
     unsigned long long *cnt;
     CU(cudaMalloc(&cnt, 8));
     CU(cudaMemsetAsync(cnt, 0, 8, m->stream));
-    count_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm, cnt);
+    count_voxels_kernel<<<m->dm.num_sms * 8, 256, 0, m->stream>>>(m->dm, cnt);
     m->launches++;
     CU(cudaMemcpyAsync(&nv, cnt, 8, cudaMemcpyDeviceToHost, m->stream));
     CU(cudaStreamSynchronize(m->stream));
@@ -694,7 +760,7 @@ int farm_map_read(farm_map *m, farm_object *objects, int *n_objects, float *desc
       CU(cudaMalloc(&dk, nv * 8));
       CU(cudaMalloc(&dvo, nv * 4));
       CU(cudaMemsetAsync(cnt, 0, 8, m->stream));
-      export_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(m->dm, dk, dvo, cnt, nv);
+      export_voxels_kernel<<<m->dm.num_sms * 8, 256, 0, m->stream>>>(m->dm, dk, dvo, cnt, nv);
       m->launches++;
       if (voxel_keys) CU(cudaMemcpyAsync(voxel_keys, dk, nv * 8, cudaMemcpyDeviceToHost, m->stream));
       if (voxel_owner) CU(cudaMemcpyAsync(voxel_owner, dvo, nv * 4, cudaMemcpyDeviceToHost, m->stream));
@@ -739,7 +805,7 @@ int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, cons
     CU(cudaMemcpyAsync(dobj, objects, (size_t)n_objects * sizeof(farm_object), cudaMemcpyHostToDevice, m->stream));
     import_objects_kernel<<<(n_objects + 255) / 256, 256, 0, m->stream>>>(d, dobj, (uint32_t)n_objects);
     CU(cudaMemcpyAsync(d.desc_master, descriptors, (size_t)n_objects * m->D * 4, cudaMemcpyHostToDevice, m->stream));
-    const int grid = std::min(n_objects, 148 * 8);
+    const int grid = std::min(n_objects, d.num_sms * 8);
     if (m->dtype == FARM_DTYPE_F32)
       renorm_rows_kernel<float><<<grid, 256, 0, m->stream>>>(d, (uint32_t)n_objects);
     else if (m->dtype == FARM_DTYPE_F16)
@@ -754,6 +820,11 @@ int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, cons
   }
   // voxels in chunks so that the staging buffers stay small
   const long long chunk = 1ll << 24;
+  uint32_t *ocnt = nullptr;  // voxels listed per owner, checked against objects[i].n_voxels
+  if (n_objects) {
+    CU(cudaMalloc(&ocnt, (size_t)n_objects * 4));
+    CU(cudaMemsetAsync(ocnt, 0, (size_t)n_objects * 4, m->stream));
+  }
   if (n_voxels) {
     unsigned long long *dk;
     uint32_t *dow;
@@ -763,12 +834,19 @@ int farm_map_import(farm_map *m, const farm_object *objects, int n_objects, cons
       const long long n = std::min(chunk, n_voxels - off);
       CU(cudaMemcpyAsync(dk, voxel_keys + off, (size_t)n * 8, cudaMemcpyHostToDevice, m->stream));
       CU(cudaMemcpyAsync(dow, voxel_owner + off, (size_t)n * 4, cudaMemcpyHostToDevice, m->stream));
-      import_voxels_kernel<<<148 * 8, 256, 0, m->stream>>>(d, dk, dow, n, (uint32_t)n_objects);
-      m->launches++;
+      import_voxels_kernel<<<d.num_sms * 8, 256, 0, m->stream>>>(d, dk, dow, n, (uint32_t)n_objects);
+      if (ocnt) count_owner_kernel<<<d.num_sms * 8, 256, 0, m->stream>>>(dow, n, (uint32_t)n_objects, ocnt);
+      m->launches += ocnt ? 2 : 1;
       CU(cudaStreamSynchronize(m->stream));
     }
     cudaFree(dk);
     cudaFree(dow);
+  }
+  if (ocnt) {
+    check_owner_count_kernel<<<(n_objects + 255) / 256, 256, 0, m->stream>>>(d, ocnt, (uint32_t)n_objects);
+    m->launches++;
+    CU(cudaStreamSynchronize(m->stream));
+    cudaFree(ocnt);
   }
   CU(cudaGetLastError());
   m->n_upper = (uint32_t)n_objects;

@@ -126,14 +126,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
   __syncthreads();
   if (!s_last) return;
   if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid before reading its row maxima
-    if (tid == 0) {
-      uint32_t done;
-      for (;;) {
-        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(m.sim_done) : "memory");
-        if ((int)(done - a.sim_target) >= 0) break;
-        __nanosleep(200);
-      }
-    }
+    if (tid == 0) spin_until(m.sim_done, a.sim_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
     __syncthreads();
   }
   pdl_trigger();  // the merge kernel becomes resident now, not while the similarity kernel still runs
@@ -363,14 +356,15 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   };
   // lane 0: view evidence and point box of the members (R22, R23); its loads overlap the descriptor work
   uint32_t k_members = 0;
-  unsigned long long pts = 0, best = 0, pts_old = 0, best_old = 0;
+  unsigned long long pts = 0, pts_old = 0, best_seq = 0;
+  uint32_t best = 0, best_old = 0, best_det = 0;
   int bmn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, bmx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
   int box_old[6] = {0, 0, 0, 0, 0, 0};
   int best_frame = -1;
   double gsum[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // G2: sufficient statistics of the members
   if (lane == 0) {
     pts_old = m.n_points[t];
-    best_old = m.best_view[t];
+    best_old = m.best_px[t];
 #pragma unroll
     for (int c = 0; c < 6; ++c) box_old[c] = m.aabb[t * 6 + c];
     for_each_member([&](uint32_t jm) {
@@ -388,12 +382,9 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       }
       int f = 0;
       while (f + 1 < a.F && (int)jm >= a.base[f + 1]) ++f;
-      const unsigned long long seq = frame_seq0 + f;
-      const uint32_t det = jm - a.base[f];
-      // R23: most pixels wins, ties -> smallest (frame_seq, det)
-      const unsigned long long pv = ((unsigned long long)(npx & 0xFFFFFFu) << 40) | ((~seq & 0xFFFFFFull) << 16) |
-                                    (unsigned long long)(~det & 0xFFFFu);
-      if (pv > best) best = pv, best_frame = f;
+      // R23: most pixels wins, ties -> smallest (frame_seq, det): members come in ascending (frame, det) order and every
+      // stored view is older than this call, so a strict > keeps the earliest
+      if (npx > best) best = npx, best_frame = f, best_seq = frame_seq0 + f, best_det = jm - a.base[f];
     });
   }
   // f_o <- normalise(n_obs * f_o + sum_m a_m / |a_m|)   (R21).  Two passes over the rows (the second one hits
@@ -487,7 +478,9 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       m.aabb[t * 6 + 3 + c] = max(box_old[3 + c], bmx[c]);
     }
     if (best > best_old) {
-      m.best_view[t] = best;
+      m.best_px[t] = best;
+      m.best_seq[t] = best_seq;
+      m.best_det[t] = best_det;
       const float *Tf = a.T + 16 * best_frame;
       m.best_cam[t * 3 + 0] = Tf[3];
       m.best_cam[t * 3 + 1] = Tf[7];
@@ -551,19 +544,19 @@ void configure_assoc_kernels() {
 }
 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  const int grid = a.M > 0 ? 74 : 1;  // 74 x 16 warps = one warp per candidate for ~1.2k candidates per wave
+  const int grid = a.M > 0 ? (m.num_sms + 1) / 2 : 1;  // half the SMs x 16 warps: one warp per candidate, ~1.2k candidates per wave
   FARM_DISPATCH((launch_pdl(cand_associate_kernel<T>, dim3(grid), dim3(CAND_THREADS), 0, s, m, a)));
   return 1;
 }
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   if (a.M == 0 || !m.covis) return 0;
-  const int grid = a.M < 148 * 4 ? a.M : 148 * 4;
+  const int grid = a.M < m.num_sms * 4 ? a.M : m.num_sms * 4;
   launch_pdl(covisibility_kernel, dim3(grid), dim3(COVIS_THREADS), (size_t)m.covis_words * 8, s, m, a);
   return 1;
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
-  const int commit_blocks = 148 * 4;
+  const int commit_blocks = m.num_sms * 4;
   const int merge_blocks = (a.M + MERGE_WARPS - 1) / MERGE_WARPS;  // one warp per detection
   FARM_DISPATCH((launch_pdl(commit_merge_kernel<T>, dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s, m, a, frame_seq0,
                             commit_blocks)));

@@ -25,6 +25,9 @@ constexpr uint32_t ERR_PAIR_TABLE_FULL = 2u;
 constexpr uint32_t ERR_OVERLAP_TABLE_FULL = 4u;
 constexpr uint32_t ERR_OBJECT_CAPACITY = 8u;
 constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
+constexpr uint32_t ERR_SYNC_TIMEOUT = 32u;       // a device-side wait for another grid of the same call expired
+constexpr uint32_t ERR_IMPORT_COUNT = 64u;       // import: objects[i].n_voxels differs from the voxels listed for i
+constexpr uint32_t SPIN_LIMIT = 1u << 23;        // polls of ~0.25 us each (about 2 s) before a device-side wait gives up
 
 // Global voxel -> object hash (R11: one owner per key), stored as a hash of 4x4x4 VOXEL BLOCKS so that the
 // voxels of one surface patch share DRAM lines:
@@ -63,6 +66,7 @@ struct DevMap {
   // parameters
   float inv_vs, w_geo, w_sem, tau, z_min, z_max;
   int D, dtype, H, W;
+  int num_sms;                       // multiprocessors of the device (queried once; sizes every persistent grid)
   // objects (SoA).  HBM layout: descriptors are [max_objects, D] row-major, D contiguous.
   uint32_t max_objects;
   uint32_t *n_objects;               // device scalar N
@@ -72,7 +76,9 @@ struct DevMap {
   uint32_t *n_voxels, *n_obs;
   unsigned long long *n_points;
   int *aabb;                         // [max_objects,6] order-preserving int image of fp32 min xyz, max xyz
-  unsigned long long *best_view;     // packed (n_px, ~frame_seq, ~det) for max()
+  uint32_t *best_px;                 // best view (R23): valid pixel count, 0 = none
+  unsigned long long *best_seq;      //   frame sequence number (full 64 bit) and
+  uint32_t *best_det;                //   detection index inside that frame
   float *best_cam;                   // [max_objects,3]
   uint32_t *leader;                  // scratch: lowest j of the call that targets the object
   uint32_t *grp_cnt;                 // scratch: number of detections of the call that target the object
@@ -158,15 +164,6 @@ __device__ __forceinline__ unsigned long long pack_score(float s, uint32_t id) {
 __device__ __forceinline__ float unpack_score(unsigned long long p) { return ord2f((int)((uint32_t)(p >> 32) ^ 0x80000000u)); }
 __device__ __forceinline__ uint32_t unpack_id(unsigned long long p) { return 0xFFFFFFFFu - (uint32_t)p; }
 
-__device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
-  x ^= x >> 33;
-  x *= 0xff51afd7ed558ccdull;
-  x ^= x >> 33;
-  x *= 0xc4ceb9fe1a85ec53ull;
-  x ^= x >> 33;
-  return x;
-}
-
 // cheap 2-word hash (multiply-xorshift); used for the voxel table, the per-call scratch tables and the tile set
 __device__ __forceinline__ uint32_t hash32(uint32_t a, uint32_t b) {
   uint32_t h = (a * 0x9E3779B1u) ^ (b * 0x85EBCA77u);
@@ -217,6 +214,21 @@ __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { retu
 // Programmatic dependent launch (PDL): a kernel launched with launch_pdl may start while its predecessor in the
 // stream is still running; it must call pdl_wait() before it touches anything the predecessor wrote.  The
 // predecessor calls pdl_trigger() early so that the dependent's CTAs become resident as soon as SM resources free up.
+// Bounded wait until the cumulative device counter *ctr has reached `target` (another grid of the same call
+// increments it).  Needs that grid to be co-resident or already finished; if it never arrives (serialised kernel
+// execution, a co-tenant holding the SMs) the wait expires, sets the sticky ERR_SYNC_TIMEOUT and returns false
+// instead of hanging the device.
+__device__ __forceinline__ bool spin_until(const uint32_t *ctr, uint32_t target, uint32_t *err) {
+  for (uint32_t it = 0; it < SPIN_LIMIT; ++it) {
+    uint32_t done;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(ctr) : "memory");
+    if ((int)(done - target) >= 0) return true;
+    __nanosleep(200);
+  }
+  atomicOr(err, ERR_SYNC_TIMEOUT);
+  return false;
+}
+
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 template <typename... KArgs, typename... Args>

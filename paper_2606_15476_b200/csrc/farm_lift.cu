@@ -806,7 +806,7 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
   const int n_tiles = tiles_x * tiles_y * a.F;
   // persistent, 4 CTAs per SM: 4 x 128 x 80 registers fit beside the similarity CTA (256 x 80) in the 64 K register file
-  const int grid = n_tiles < 148 * 4 ? n_tiles : 148 * 4;
+  const int grid = n_tiles < m.num_sms * 4 ? n_tiles : m.num_sms * 4;
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
   if (m.det_gm) {
     if (vec)
@@ -822,7 +822,7 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 }
 
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  launch_pdl(probe_kernel, dim3(148 * 4), dim3(PROBE_THREADS), 0, s, m, a);
+  launch_pdl(probe_kernel, dim3(m.num_sms * 4), dim3(PROBE_THREADS), 0, s, m, a);
   return 1;
 }
 

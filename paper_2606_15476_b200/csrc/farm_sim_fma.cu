@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(SIM_THREADS) similarity_fma_kernel(DevMap m, C
 int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s) {
   if (a.M == 0 || n_upper == 0) return 0;
   const long long tiles = (long long)((a.M + BM - 1) / BM) * ((n_upper + BN - 1) / BN);
-  const int grid = (int)(tiles < 148 * 4 ? tiles : 148 * 4);
+  const int grid = (int)(tiles < m.num_sms * 4 ? tiles : m.num_sms * 4);
   if (m.dtype == FARM_DTYPE_F32)
     similarity_fma_kernel<float><<<grid, SIM_THREADS, 0, s>>>(m, a);
   else if (m.dtype == FARM_DTYPE_F16)

@@ -202,14 +202,7 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     uint32_t as = 0, aphase = 0;
     // prep_kernel (main stream) may still be running: its row norms and the zeroed best_dense words are first
     // needed here, one tile of MMAs after the kernel started
-    {
-      uint32_t done;
-      for (;;) {
-        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(m.prep_done) : "memory");
-        if ((int)(done - prep_target) >= 0) break;
-        __nanosleep(200);
-      }
-    }
+    spin_until(m.prep_done, prep_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       const int tm = tile % tiles_m, tn = tile / tiles_m;
       const int n0 = tn * BLOCK_N;
@@ -217,13 +210,16 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
       float *ib = ib_s + as * BLOCK_N;
 #pragma unroll
       for (int c = et; c < BLOCK_N; c += EPI_THREADS) ib[c] = c < ncols ? m.inv_norm[n0 + c] : 0.f;
+      const int cbeg = half * (BLOCK_N / EPI_SPLIT);
+      const int row = tm * BLOCK_M + row_in_tile;
+      const bool row_ok = row < M && cbeg < ncols;
+      const float ia = row_ok ? m.det_inv_norm[row] : 0.f;  // requested before the wait for the accumulator
       asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
       mbar_wait(smem_u32(&tfull_bar[as]), aphase);
       tcgen05_fence_after();
       // four interleaved chains (columns = chain mod 4): strict > keeps the lowest column inside a chain
       float bv[4] = {-3.0e38f, -3.0e38f, -3.0e38f, -3.0e38f};
       int bc[4] = {0, 1, 2, 3};
-      const int cbeg = half * (BLOCK_N / EPI_SPLIT);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
 #pragma unroll 1
       for (int c0 = cbeg; c0 < cbeg + BLOCK_N / EPI_SPLIT; c0 += 32) {
@@ -245,19 +241,34 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
           }
         }
       }
-      tcgen05_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
       // combine the chains: larger value wins, equal values -> lower column (R18 tie rule)
       float best = bv[0];
       int best_c = bc[0];
 #pragma unroll
       for (int k = 1; k < 4; ++k)
         if (bv[k] > best || (bv[k] == best && bc[k] < best_c)) best = bv[k], best_c = bc[k];
-      const int row = tm * BLOCK_M + row_in_tile;
-      if (row < M && cbeg < ncols) {
-        const float ia = m.det_inv_norm[row];
-        float cs = best * ia;
+      float cs = best * ia;
+      // R15 clamps before R18 compares: every column whose cosine reaches 1 ties at exactly 1.0 and the lowest id wins.
+      // Rare (duplicates of the detection in the map): the warp re-scans its accumulator for the first such column.
+      const bool sat = row_ok && cs >= 1.0f;
+      if (__any_sync(0xFFFFFFFFu, sat)) {
+        int first = best_c;
+#pragma unroll 1
+        for (int c0 = cbeg; c0 < cbeg + BLOCK_N / EPI_SPLIT; c0 += 32) {
+          if (c0 >= ncols) break;
+          uint32_t r[32];
+          tmem_ld32(taddr + c0, r);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (sat && c0 + i < ncols && c0 + i < first && __uint_as_float(r[i]) * ib[c0 + i] * ia >= 1.0f) first = c0 + i;
+        }
+        best_c = first;
+      }
+      tcgen05_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+      if (row_ok) {
         cs = fminf(1.f, fmaxf(-1.f, cs));                    // R15 clamp
         if (ia == 0.f) cs = 0.f, best_c = 0;                 // zero-norm detection: cos = 0 for every object
         atomicMax(&m.best_dense[row], pack_score(cs, (uint32_t)(n0 + best_c)));
@@ -281,10 +292,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 struct TcState {
   EncodeTiledFn encode = nullptr;
-  CUtensorMap map_b;
+  CUtensorMap map_a, map_b;  // map_a is re-encoded per call by tc_prepare (host work only)
   CUtensorMapDataType dt;
   uint32_t idesc;
-  int num_sms = 148;
   bool ok = false;
 };
 
@@ -320,9 +330,6 @@ void *tc_state_create(const DevMap &m) {
     delete st;
     return nullptr;
   }
-  int dev = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&st->num_sms, cudaDevAttrMultiProcessorCount, dev);
   if (cudaFuncSetAttribute(similarity_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
     delete st;
     return nullptr;
@@ -333,14 +340,22 @@ void *tc_state_create(const DevMap &m) {
 
 void tc_state_destroy(void *p) { delete (TcState *)p; }
 
+// Encode the call's A operand (detection rows).  Called before anything of the call is enqueued, so that a
+// descriptor pointer TMA cannot address (not 16-byte aligned) fails the call with the map untouched.
+bool tc_prepare(void *state, const DevMap &m, const CallArgs &a) {
+  TcState *st = (TcState *)state;
+  if (a.M == 0) return true;
+  if (((uintptr_t)a.desc & 15) != 0) return false;
+  return encode_2d(st, &st->map_a, a.desc, (uint64_t)a.M, (uint64_t)m.D, BLOCK_M);
+}
+
 int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state, uint32_t prep_target,
                          int *n_ctas) {
   TcState *st = (TcState *)state;
   if (a.M == 0 || n_upper == 0) return 0;
-  CUtensorMap map_a;
-  if (!encode_2d(st, &map_a, a.desc, (uint64_t)a.M, (uint64_t)m.D, BLOCK_M)) return -1;  // loud: the caller fails the call
+  const CUtensorMap &map_a = st->map_a;
   const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
-  const int grid = (int)(tiles < st->num_sms ? tiles : st->num_sms);
+  const int grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
   similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
   if (n_ctas) *n_ctas = grid;
   return 1;

@@ -88,3 +88,29 @@ def compare_maps(g: FarmMap, o, voxels=True):
         order = np.argsort(keyg)
         assert np.array_equal(keyg[order], keyo)
         assert np.array_equal(owng[order], owno)
+
+
+def compare_dense(g: FarmMap, o):
+    """R16/R18: dense row maximum of the clamped cosine and its argmax (lowest id on ties) of the last call.  The argmax
+    is compared wherever the oracle's runner-up is more than 1e-4 away, and on exact ties (bit-identical map rows),
+    which the id rule decides on both sides.  Returns the number of rows whose argmax was compared."""
+    mc_o, am_o = o.last_dense()
+    sec = o.last_dense_second()
+    mc_g, am_g = g.debug_last_dense()
+    ok = o.last_assoc()[0] >= 0                                   # skipped detections have no dense row in the oracle
+    assert np.abs(mc_g - mc_o)[ok].max(initial=0) <= TOL
+    clear = ok & (am_o >= 0) & ((mc_o - sec > 1e-4) | (mc_o == sec))
+    assert np.array_equal(am_g[clear], am_o[clear]), (am_g[clear], am_o[clear])
+    return int(clear.sum())
+
+
+def dense_decided(o):
+    """number of detections of the oracle's last call matched to an object they share NO voxel with: the dense
+    argmax supplied the matched object (R19)"""
+    assoc, is_new, _, _, _ = o.last_assoc()
+    off, obj, _ = o.last_overlaps()
+    n = 0
+    for d in range(len(assoc)):
+        if assoc[d] >= 0 and not is_new[d] and assoc[d] not in set(obj[off[d]:off[d + 1]].tolist()):
+            n += 1
+    return n

@@ -1,0 +1,221 @@
+"""`-m gpu`, round 2: the decision paths and sizes round 1 left without evidence.
+
+* w_sem > tau: a non-overlapping object can pass the threshold, so the matched object's id comes from the dense
+  similarity epilogue (row argmax, lowest id on ties, R16/R18/R19) -- on the tcgen05 path (several tiles on both
+  axes), the CUDA-core FMA path, and with exact ties (bit-identical map rows).
+* `farm_debug_last_dense` against the oracle's dense (max, argmax).
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from helpers import generate_frames, hand_frame, integrate_frames, margin_filter, pack_key, pow2_K, unit_rows
+from paper_2606_15476_b200 import FarmMap, scenes as S
+from parity import TOL, compare_call, compare_dense, compare_maps, dense_decided, gpu_integrate, make_pair
+
+pytestmark = pytest.mark.gpu
+
+WEIGHTS = [(0.3, 0.7, 0.5), (0.0, 1.0, 0.6)]
+
+
+def _with_weights(cfg, w):
+    return dataclasses.replace(cfg, w_geo=w[0], w_sem=w[1], tau=w[2])
+
+
+@pytest.mark.parametrize("w", WEIGHTS)
+def test_dense_argmax_decides_on_config2_distractor_clusters(oracle, w):
+    """configs[2] (0.9-cosine distractor clusters, D=1024 bf16, tcgen05 path) with w_sem > tau: cluster members match
+    one another without sharing a voxel, so the dense argmax decides."""
+    cfg = _with_weights(S.get_config(2), w)
+    frames_all = generate_frames(2, range(0, 40))
+    o, g = make_pair(oracle, cfg)
+    n_dense, n_rows = 0, 0
+    for fr in frames_all:
+        frames = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+        n_rows += compare_dense(g, o)
+        n_dense += dense_decided(o)
+    compare_maps(g, o)
+    assert n_dense >= 5 and n_rows > 500, (n_dense, n_rows)
+
+
+def _stress_frames_with_far_matches(sc, b, desc_map, rng):
+    """batch b of the mini stress scene; the detections that look at empty space get the descriptor of a random FILLER
+    object (+ view noise) instead of a fresh one: with w_sem > tau they match that object without any voxel overlap"""
+    out = []
+    n_t = len(sc._blob_ijk)
+    for fr in sc.batch(b):
+        desc = S.storage_to_f32(fr.desc, sc.cfg.dtype).copy()
+        for d in np.nonzero(fr.box_ids < 0)[0]:
+            tgt = int(rng.integers(n_t, len(desc_map)))
+            v = desc_map[tgt] + (0.1 / np.sqrt(desc.shape[1])) * rng.standard_normal(desc.shape[1])
+            desc[d] = v / np.linalg.norm(v)
+        out.append(S.Frame(fr.depth, fr.mask, fr.K, fr.T, S.to_storage(desc.astype(np.float32), sc.cfg.dtype), fr.n_det, fr.box_ids))
+    return out
+
+
+@pytest.mark.parametrize("w", WEIGHTS)
+def test_dense_argmax_decides_multi_tile_tensor_path(oracle, w):
+    """M = 400 detections x N >= 700 objects, D = 1024 bf16: more than one tile on both axes of similarity_tc_kernel
+    (128 x 256); half of the detections can only match through the dense argmax."""
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    sc = S.StressScene(n_batches=2, frames_per_batch=4, n_objects=700)
+    cfg = _with_weights(sc.cfg, w)
+    ijk, owner, n_vox, desc = sc.build_map()
+    keys = pack_key(ijk[:, 0], ijk[:, 1], ijk[:, 2])
+    objs = np.zeros(len(n_vox), OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(len(n_vox)), n_vox, 1, -1, -1
+    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, sim_path=2)
+    assert o.import_(objs, desc, keys, owner) == 0
+    g.import_(objs, desc, keys, owner)
+    rng = np.random.default_rng(17)
+    n_dense = 0
+    for b in range(2):
+        frames = margin_filter(o.clone, _stress_frames_with_far_matches(sc, b, desc, rng), cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+        assert compare_dense(g, o) > 300
+        n_dense += dense_decided(o)
+    compare_maps(g, o)
+    assert n_dense > 250, n_dense
+
+
+@pytest.mark.parametrize("cfg_id,sim_path,n", [(0, 0, 20), (1, 1, 30), (1, 2, 30)])
+@pytest.mark.parametrize("w", WEIGHTS)
+def test_dense_argmax_decides_fma_and_small_tensor_paths(oracle, w, cfg_id, sim_path, n):
+    """fp32 (configs[0], CUDA-core FMA), and configs[1] (f16) forced through the FMA path and the tcgen05 path."""
+    cfg = _with_weights(S.get_config(cfg_id), w)
+    frames_all = generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n))
+    o, g = make_pair(oracle, cfg, sim_path=sim_path)
+    rows = 0
+    for fr in frames_all:
+        frames = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+        rows += compare_dense(g, o)
+    compare_maps(g, o)
+    assert rows > 50
+
+
+@pytest.mark.parametrize("dtype,sim_path", [(0, 0), (1, 1), (1, 2), (2, 1), (2, 2)])
+def test_exact_ties_go_to_the_lowest_id(oracle, dtype, sim_path):
+    """R18 with bit-identical map rows (same tile, neighbouring tiles, far tiles of the 128 x 256 tensor tiling) and
+    detections equal to them: cosine clamps to exactly 1 for all of them and the lowest id must win -- in the dense
+    argmax and in the decision (w_geo = 0, w_sem = 1, tau = 0.6: the dense argmax IS the decision)."""
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    D, N = 64, 900
+    H, W = 96, 128
+    rows = unit_rows(N, D, 41)
+    groups = [[5, 300, 301], [310, 400], [255, 256], [700, 12, 899]]
+    for grp in groups:
+        for i in grp[1:]:
+            rows[i] = rows[grp[0]]
+    det = np.stack([rows[g[0]] for g in groups] + [rows[77]]).astype(np.float32)
+    Mdet = len(det)
+
+    class Cfg:
+        voxel, w_geo, w_sem, tau = 0.25, 0.0, 1.0, 0.6
+    Cfg.D, Cfg.dtype = D, dtype
+    o, g = make_pair(oracle, Cfg, H=H, W=W, sim_path=sim_path)
+    objs = np.zeros(N, OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(N), 1, 1, -1, -1
+    keys = pack_key(np.arange(N) + 500, np.zeros(N, int), np.zeros(N, int))
+    assert o.import_(objs, rows, keys, np.arange(N, dtype=np.uint32)) == 0
+    g.import_(objs, rows, keys, np.arange(N, dtype=np.uint32))
+    depth, mask = hand_frame(H, W, [(8 + 16 * d, 48, 2.0, d + 1) for d in range(Mdet)])
+    fr = S.Frame(depth, mask, pow2_K(), np.eye(4, dtype=np.float32), S.to_storage(det, dtype), Mdet, np.zeros(Mdet, np.int64))
+    integrate_frames(o, [fr])
+    gpu_integrate(g, [fr], dtype)
+    ao, no, bo, _, _ = o.last_assoc()
+    ag, ng, bg, _ = g.last_assoc()
+    assert np.array_equal(ag, ao) and np.array_equal(ng, no) and np.abs(bg - bo).max() <= TOL
+    mc_o, am_o = o.last_dense()
+    mc_g, am_g = g.debug_last_dense()
+    assert np.array_equal(am_g, am_o) and np.abs(mc_g - mc_o).max() <= TOL
+    assert list(ao) == [5, 310, 255, 12, 77] and not no.any()
+    compare_maps(g, o)
+
+
+def test_resume_continues_frame_numbering_and_import_checks_counts(oracle):
+    """Scene-state resume: export, import into a new map, set the frame counter, continue -- best-view
+    records keep global frame numbers.  An object whose n_voxels disagrees with its voxel list is rejected."""
+    from paper_2606_15476_b200 import FarmError
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    o, g = make_pair(oracle, cfg)
+    for k in range(6):
+        fr = sc.frame(k)
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], cfg.dtype)
+    assert g.get_frame_seq() == 6
+    objs, desc, keys, owners = g.read()
+    g2 = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype)
+    g2.import_(objs, desc, keys, owners)
+    g2.set_frame_seq(6)
+    with pytest.raises(FarmError):
+        g2.set_frame_seq(3)                                        # only forward
+    for k in range(6, 12):
+        frames = margin_filter(o.clone, [sc.frame(k)], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g2, frames, cfg.dtype)
+        compare_call(g2, o)
+    compare_maps(g2, o)                                            # includes best_frame of views taken after the resume
+    assert g2.get_frame_seq() == 12
+    bad = objs.copy()
+    bad["n_voxels"][0] += 1
+    g3 = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype)
+    with pytest.raises(FarmError) as ei:
+        g3.import_(bad, desc, keys, owners)
+    assert ei.value.code == -1 and "n_voxels" in str(ei.value)
+
+
+def test_misaligned_descriptors_fail_before_anything_is_enqueued(oracle):
+    """A 16-bit descriptor pointer that TMA cannot address is refused with FARM_ERR_INVALID_ARG and the map, the frame
+    counter and the per-call results are untouched; the next (aligned) call is exact."""
+    import torch
+    from paper_2606_15476_b200 import FarmError
+    from parity import upload
+    cfg = S.get_config(1)
+    frames = generate_frames(1, range(20, 24))
+    o, g = make_pair(oracle, cfg, sim_path=2)
+    for fr in frames[:2]:
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], cfg.dtype)
+    before = g.read()
+    d = upload([frames[2]], cfg.dtype)
+    raw = torch.empty(d["desc"].numel() + 8, dtype=d["desc"].dtype, device="cuda")
+    off = raw[1:1 + d["desc"].numel()].view(d["desc"].shape)        # 2 bytes off a 16-byte boundary
+    off.copy_(d["desc"])
+    assert off.data_ptr() % 16 != 0
+    with pytest.raises(FarmError) as ei:
+        g.integrate_batch(1, d["depth"], d["mask"], d["K"], d["T"], off.data_ptr(), d["n_det"])
+    assert ei.value.code == -1
+    assert g.get_frame_seq() == 2
+    after = g.read()
+    assert all(np.array_equal(a, b) for a, b in zip(before, after))
+    for fr in frames[2:]:
+        fl = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, fl)
+        gpu_integrate(g, fl, cfg.dtype)
+        compare_call(g, o)
+    compare_maps(g, o)
+
+
+def test_launch_blocking_environment_selects_the_single_stream_order(oracle, monkeypatch):
+    """CUDA_LAUNCH_BLOCKING serialises kernels, which the device-side waits of the default order cannot survive: the
+    library then uses the single-stream order (no waits) and still reproduces the oracle."""
+    monkeypatch.setenv("CUDA_LAUNCH_BLOCKING", "1")
+    cfg = S.get_config(1)
+    frames_all = generate_frames(1, range(20, 26))
+    o, g = make_pair(oracle, cfg)
+    for fr in frames_all:
+        frames = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+    compare_maps(g, o)

@@ -119,6 +119,7 @@ def test_dense_row_max_and_argmax_vs_library_gemm(oracle, dtype):
     cos = np.clip((A @ B.T) / np.outer(np.linalg.norm(A, axis=1), np.linalg.norm(B, axis=1)), -1, 1)
     ref_arg = cos.argmax(axis=1)                                # numpy: first maximum = lowest id
     assert np.abs(mc - cos.max(axis=1)).max() <= 1e-6
+    assert np.abs(m.last_dense_second() - np.sort(cos, axis=1)[:, -2]).max() <= 1e-6
     far = np.sort(cos, axis=1)[:, -1] - np.sort(cos, axis=1)[:, -2] > 1e-5
     far[3] = True                                               # the exact tie is decided by the id rule
     assert np.array_equal(am[far], ref_arg[far])
