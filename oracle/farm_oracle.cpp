@@ -24,6 +24,17 @@
 // tests/test_oracle_gaussian.py (covisibility bitset of PAPER.md:354, rule C1, pinned there as well by brute-force
 // pair enumeration, symmetry and monotonicity): numpy mean/cov of the same points, union-of-halves, textbook closed forms
 // of the Hellinger distance and numpy.linalg for the general formula.  The association decision is NOT changed.
+//
+// Round 2 additions (SURVEY.md §8(f) NEXT-1..4; readings in DESIGN.md §10-§13), every one off by default:
+//   U1-U4  correspondence by union-find over the sparse match graph with entity-entity merges
+//   H1-H3  the paper's geometry as the geometric term of the decision: similarity prefilter, then Hellinger distance
+//          between the detection's and the entity's Gaussian within a budget
+//   V1-V3  high-quality view selection: up to k views per entity, kept if the viewing direction is new or the view is
+//          sufficiently closer (PAPER.md:63 item (iii))
+//   Q1-Q5  retrieval-side scoring: reciprocal-rank fusion over four query channels, closed-form predicates over the
+//          entity centroids, composite score, top-K
+// Pins: tests/test_oracle_next.py (brute-force union-find, conservation laws, hand cases, closed forms, numpy ranks).
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -82,7 +93,16 @@ struct BestView {  // R23
   float cam[3] = {0, 0, 0};
 };
 
+struct View {  // V1: one retained viewpoint of an entity
+  int32_t frame = -1, det = -1;
+  uint32_t n_px = 0;
+  float cam[3] = {0, 0, 0}, dir[3] = {0, 0, 0}, dist = 0;
+};
+
 struct Object {  // R1
+  bool alive = true;     // U4: false once the entity has been absorbed by another one
+  int32_t alias = -1;    // U4: the entity that absorbed this one (-1 while alive)
+  std::vector<View> views;  // V2: at most views_k retained viewpoints, in the order they were retained
   uint32_t n_voxels = 0, n_obs = 0;
   uint64_t n_points = 0;
   float amin[3], amax[3];
@@ -102,6 +122,15 @@ struct Stats {  // per call
 struct Map {
   float voxel_size, inv_vs, w_geo, w_sem, tau, z_min, z_max;
   int D, dtype, H, W;
+  // options (oracle_set_option); all off by default
+  int opt_corr = 0;              // U: union-find correspondence with entity-entity merges
+  int opt_geom = 0;              // H: 0 = voxel overlap (BASELINE.json rule), 1 = Hellinger distance between Gaussians
+  float prefilter_cos = 0.5f;    // H1: candidates are the entities with cos > prefilter_cos
+  float hell_budget = 1.0f;      // H2: candidates with H > hell_budget are dropped (1 = no gate: H <= 1 always)
+  int views_k = 0;               // V: views kept per entity (0 = off)
+  float view_cos = 0.8660254f;   // V2: a direction is new if its cosine with every kept direction is below this (30 degrees)
+  float view_closer = 0.8f;      // V2: or the view is closer than view_closer x the closest kept view
+  std::vector<int32_t> merged_from, merged_into;  // U4: (loser, winner) pairs of the last call
   std::map<uint64_t, uint32_t> owner;  // R11: one owner per key
   std::vector<Object> objs;
   int64_t frame_seq = 0;
@@ -222,6 +251,65 @@ float cosine(const float *a, const float *b, int D) {
   return (float)c;
 }
 
+// U3: union-find with path compression; the root of a set is its smallest node index
+int uf_find(std::vector<int> &parent, int x) {
+  int r = x;
+  while (parent[r] != r) r = parent[r];
+  while (parent[x] != r) {
+    const int nx = parent[x];
+    parent[x] = r;
+    x = nx;
+  }
+  return r;
+}
+void uf_union(std::vector<int> &parent, int a, int b) {
+  a = uf_find(parent, a), b = uf_find(parent, b);
+  if (a == b) return;
+  if (a < b) parent[b] = a; else parent[a] = b;
+}
+
+// V1-V2 ("A new viewpoint is retained for an entity only if its viewing direction differs from all
+// existing retained viewpoints by more than a fixed angular threshold, or if it is sufficiently closer than the
+// closest existing viewpoint"; "up to k representative views").  All arithmetic in fp32, one rounded
+// operation at a time, because it decides which views are kept (both implementations take the decision in fp32).
+// Readings: the viewing direction is the unit vector from the camera position to the centre of the detection's point
+// box; a full set replaces its farthest view (earliest on ties) if the new view is closer than that one, else the
+// new view is dropped.
+bool make_view(const float *box, const float *cam, int32_t frame, int32_t det, uint32_t n_px, View *out) {
+  float d[3];
+  for (int k = 0; k < 3; ++k) {
+    const float c = 0.5f * (box[k] + box[3 + k]);
+    d[k] = c - cam[k];
+  }
+  const float d2 = (d[0] * d[0] + d[1] * d[1]) + d[2] * d[2];
+  const float dist = std::sqrt(d2);
+  if (!(dist > 0.0f)) return false;
+  out->frame = frame, out->det = det, out->n_px = n_px, out->dist = dist;
+  for (int k = 0; k < 3; ++k) out->cam[k] = cam[k], out->dir[k] = d[k] / dist;
+  return true;
+}
+bool offer_view(const Map &m, Object &ob, const View &v) {
+  bool fresh = true;
+  float closest = std::numeric_limits<float>::infinity();
+  for (const View &k : ob.views) {
+    const float dot = (v.dir[0] * k.dir[0] + v.dir[1] * k.dir[1]) + v.dir[2] * k.dir[2];
+    if (!(dot < m.view_cos)) fresh = false;
+    closest = std::fmin(closest, k.dist);
+  }
+  const bool closer = !ob.views.empty() && v.dist < m.view_closer * closest;
+  if (!ob.views.empty() && !fresh && !closer) return false;
+  if ((int)ob.views.size() < m.views_k) {
+    ob.views.push_back(v);
+    return true;
+  }
+  size_t far = 0;
+  for (size_t i = 1; i < ob.views.size(); ++i)
+    if (ob.views[i].dist > ob.views[far].dist) far = i;
+  if (!(v.dist < ob.views[far].dist)) return false;
+  ob.views[far] = v;
+  return true;
+}
+
 }  // namespace
 
 extern "C" {
@@ -259,6 +347,21 @@ void *oracle_create(float voxel_size, int D, float w_geo, float w_sem, float tau
 }
 void oracle_destroy(void *h) { delete (Map *)h; }
 void *oracle_clone(void *h) { return new Map(*(Map *)h); }  // deep copy (tests: margin filter, what-if runs)
+
+// options: 1 correspondence (U), 2 geometry (H), 3 prefilter cosine, 4 Hellinger budget, 5 views k, 6 view cosine, 7 view closer
+int oracle_set_option(void *h, int key, double v) {
+  Map &m = *(Map *)h;
+  switch (key) {
+    case 1: if (v != 0 && !(m.tau >= 0.0f)) return -1; m.opt_corr = v != 0; return 0;
+    case 2: m.opt_geom = (int)v; return 0;
+    case 3: m.prefilter_cos = (float)v; return 0;
+    case 4: m.hell_budget = (float)v; return 0;
+    case 5: m.views_k = (int)v; return 0;
+    case 6: m.view_cos = (float)v; return 0;
+    case 7: m.view_closer = (float)v; return 0;
+  }
+  return -1;
+}
 
 // Debug: dense per-pixel world point (NaN where invalid) and key (KEY_EMPTY where invalid or dropped). R3-R6.
 void oracle_backproject(void *h, const float *depth, const uint16_t *mask, const float *K, const float *T,
@@ -366,7 +469,9 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
   // ---- steps 4-5a (R10, R14-R20): dense cosine, score, argmax, threshold
   std::vector<float> a(D);
   std::vector<int> target(M, -1);
-  int next_id = N;
+  std::vector<int> best_obj(M, -1);
+  std::vector<std::vector<int>> retained(M);  // U1: entities with score > tau (the sparse match graph)
+  const double eps2 = (double)m.voxel_size * (double)m.voxel_size;
   for (int j = 0; j < M; ++j) {
     if (m.n_px[j] == 0) {  // R8: empty detection is skipped
       m.stats.skipped++;
@@ -375,6 +480,8 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     for (int i = 0; i < D; ++i) a[i] = load_storage(desc, m.dtype, (size_t)j * D + i);  // R14
     float best = 0.0f, second = -std::numeric_limits<float>::infinity();
     int best_o = -1;
+    double mu_d[3], c_d[6];
+    if (m.opt_geom == 1) gaussian_from_moments((double)m.n_px[j], &m.gS1[(size_t)j * 3], &m.gS2[(size_t)j * 6], mu_d, c_d);
     for (int o = 0; o < N; ++o) {                                // R16: every pair
       const float c = cosine(a.data(), m.objs[o].shadow.data(), D);  // R15
       if (m.dense_arg[j] < 0 || c > m.dense_max[j]) {            // R16 dense row max, ties -> lowest id
@@ -384,12 +491,29 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
       } else {
         m.dense_second[j] = std::fmax(m.dense_second[j], c);
       }
-      float g = 0.0f;                                            // R10
-      auto it = m.overlap[j].find((uint32_t)o);
-      const uint32_t cnt = it == m.overlap[j].end() ? 0u : it->second;
-      const uint32_t mn = std::min<uint32_t>((uint32_t)m.V[j].size(), m.objs[o].n_voxels);
-      if (mn > 0) g = (float)cnt / (float)mn;
+      float g = 0.0f;
+      if (m.opt_geom == 0) {                                     // R10
+        auto it = m.overlap[j].find((uint32_t)o);
+        const uint32_t cnt = it == m.overlap[j].end() ? 0u : it->second;
+        const uint32_t mn = std::min<uint32_t>((uint32_t)m.V[j].size(), m.objs[o].n_voxels);
+        if (mn > 0) g = (float)cnt / (float)mn;
+      } else {
+        // H1 ("restrict candidates to active entities whose per-detection feature is sufficiently
+        // similar"): only entities with cos > prefilter_cos are candidates at all.
+        if (!(c > m.prefilter_cos)) continue;
+        // H2 ("then compute the Hellinger distance between the detection's 3D Gaussian and each candidate entity's
+        // Gaussian, retaining every candidate entity within a fixed Hellinger budget"); H3: g = 1 - H.  An entity
+        // without a Gaussian (imported, never observed) stays a candidate with g = 0.
+        if (m.objs[o].gW > 0.0) {
+          double mu_o[3], c_o[6];
+          gaussian_from_moments(m.objs[o].gW, m.objs[o].gM1, m.objs[o].gM2, mu_o, c_o);
+          const float hf = (float)hellinger(mu_d, c_d, mu_o, c_o, eps2);
+          if (hf > m.hell_budget) continue;
+          g = 1.0f - hf;
+        }
+      }
       const float score = m.w_geo * g + m.w_sem * c;             // R17 (fp32: two mul, one add)
+      if (m.opt_corr && score > m.tau) retained[j].push_back(o); // U1
       if (best_o < 0 || score > best) {                          // R18: ties -> lowest id
         if (best_o >= 0) second = std::fmax(second, best);
         best = score;
@@ -400,22 +524,94 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     }
     m.best_score[j] = best_o >= 0 ? best : 0.0f;
     m.second_score[j] = second;
-    if (best_o >= 0 && best > m.tau) {  // R18: strict
-      target[j] = best_o;
-      m.assoc[j] = best_o;
-      m.stats.matches++;
-      if (m.objs[best_o].gW > 0.0) {  // G4: distance to the matched entity's Gaussian as it was at entry (R2)
-        double mu_d[3], c_d[6], mu_o[3], c_o[6];
-        gaussian_from_moments((double)m.n_px[j], &m.gS1[(size_t)j * 3], &m.gS2[(size_t)j * 6], mu_d, c_d);
-        gaussian_from_moments(m.objs[best_o].gW, m.objs[best_o].gM1, m.objs[best_o].gM2, mu_o, c_o);
-        m.hell[j] = (float)hellinger(mu_d, c_d, mu_o, c_o, (double)m.voxel_size * (double)m.voxel_size);
-      }
-    } else {  // R20: new ids in order of j
-      target[j] = next_id++;
-      m.assoc[j] = target[j];
-      m.is_new[j] = 1;
-      m.stats.spawns++;
+    best_obj[j] = (best_o >= 0 && best > m.tau) ? best_o : -1;   // R18: strict
+    if (best_obj[j] >= 0 && m.objs[best_o].gW > 0.0) {  // G4: distance to the matched entity's Gaussian as it was at entry (R2)
+      double mu_d2[3], c_d2[6], mu_o[3], c_o[6];
+      gaussian_from_moments((double)m.n_px[j], &m.gS1[(size_t)j * 3], &m.gS2[(size_t)j * 6], mu_d2, c_d2);
+      gaussian_from_moments(m.objs[best_o].gW, m.objs[best_o].gM1, m.objs[best_o].gM2, mu_o, c_o);
+      m.hell[j] = (float)hellinger(mu_d2, c_d2, mu_o, c_o, eps2);
     }
+  }
+
+  int next_id = N;
+  std::vector<int> loser_of;  // U4: entities absorbed in this call, ascending
+  std::vector<int> parent;
+  m.merged_from.clear();
+  m.merged_into.clear();
+  if (!m.opt_corr) {
+    for (int j = 0; j < M; ++j) {
+      if (m.n_px[j] == 0) continue;
+      if (best_obj[j] >= 0) {
+        target[j] = best_obj[j];
+        m.assoc[j] = best_obj[j];
+        m.stats.matches++;
+      } else {  // R20: new ids in order of j
+        target[j] = next_id++;
+        m.assoc[j] = target[j];
+        m.is_new[j] = 1;
+        m.stats.spawns++;
+      }
+    }
+  } else {
+    // U2 (reading; repairs the duplicate spawns that R2 makes possible): a detection d that retained no entity is
+    // linked to an earlier detection e of the same call when they see the same new space and look alike:
+    //   c_dd(d, e) = number of keys of V_d that are unowned at entry and whose R12 claimant (the lowest-index detection
+    //   of the call containing the key) is e;  g = c_dd / min(|V_d|, |V_e|);  score = w_geo*g + w_sem*cos(a_d, a_e) > tau.
+    std::map<uint64_t, int> claim;
+    for (int j = 0; j < M; ++j) {
+      if (m.n_px[j] == 0) continue;
+      for (uint64_t key : m.V[j])
+        if (m.owner.find(key) == m.owner.end()) claim.emplace(key, j);
+    }
+    parent.resize(N + M);
+    for (int i = 0; i < N + M; ++i) parent[i] = i;
+    std::vector<float> b(D);
+    for (int j = 0; j < M; ++j) {
+      if (m.n_px[j] == 0) continue;
+      for (int o : retained[j]) uf_union(parent, N + j, o);      // U1 edges; a detection retaining two entities bridges them
+      if (!retained[j].empty()) continue;
+      std::map<int, uint32_t> cdd;
+      for (uint64_t key : m.V[j]) {
+        auto it = claim.find(key);
+        if (it != claim.end() && it->second != j) cdd[it->second]++;
+      }
+      for (int i = 0; i < D; ++i) a[i] = load_storage(desc, m.dtype, (size_t)j * D + i);
+      for (auto &kv : cdd) {
+        const int e = kv.first;
+        const uint32_t mn = std::min<uint32_t>((uint32_t)m.V[j].size(), (uint32_t)m.V[e].size());
+        const float g = mn ? (float)kv.second / (float)mn : 0.0f;
+        for (int i = 0; i < D; ++i) b[i] = load_storage(desc, m.dtype, (size_t)e * D + i);
+        const float score = m.w_geo * g + m.w_sem * cosine(a.data(), b.data(), D);
+        if (score > m.tau) uf_union(parent, N + j, N + e);
+      }
+    }
+    // U3 ("A union-find pass over the match graph with path compression resolves the case where multiple
+    // detections claim the same entity, and the case where one detection bridges two previously separate entities"):
+    // the root of a component is its smallest node; entities are numbered before detections, so a component that holds
+    // an entity is won by its lowest-id entity (reading: the oldest identity survives), and a component of detections
+    // only becomes ONE new entity, numbered in the order of its lowest detection index (R20).
+    std::map<int, int> new_id_of_root;
+    for (int j = 0; j < M; ++j) {
+      if (m.n_px[j] == 0) continue;
+      const int r = uf_find(parent, N + j);
+      if (r < N) {
+        target[j] = r;
+        m.stats.matches++;
+      } else {
+        auto it = new_id_of_root.find(r);
+        if (it == new_id_of_root.end()) {
+          it = new_id_of_root.emplace(r, next_id++).first;
+          m.is_new[j] = 1;  // the component's lowest detection creates the entity
+          m.stats.spawns++;
+        } else {
+          m.stats.matches++;
+        }
+        target[j] = it->second;
+      }
+      m.assoc[j] = target[j];
+    }
+    for (int o = 0; o < N; ++o)
+      if (uf_find(parent, o) != o) loser_of.push_back(o);
   }
 
   // ---- step 5b: merge, after all decisions (R12, R13, R21-R23)
@@ -426,6 +622,55 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     for (int k = 0; k < 3; ++k) {
       m.objs[o].amin[k] = std::numeric_limits<float>::infinity();
       m.objs[o].amax[k] = -std::numeric_limits<float>::infinity();
+    }
+  }
+  // U4 ("Entity-level merges flagged by the correspondence pass are also executed here, absorbing the
+  // loser's covisibility, captions, view records, and identity history into the winner"): before the call's detections
+  // are fused, every loser L is absorbed by its winner W -- voxels re-owned, counts summed, boxes united, best view by
+  // R23, Gaussian statistics summed, views offered under V2, covisibility row ORed in and column renamed.  The
+  // count-weighted descriptors of the losers enter the winner's R21 fold below.  L stays as a dead id (alias -> W).
+  std::vector<std::vector<int>> losers_of_winner(next_id);
+  if (!loser_of.empty()) {
+    std::map<uint32_t, uint32_t> win;
+    for (int L : loser_of) win[(uint32_t)L] = (uint32_t)uf_find(parent, L);
+    for (auto &kv : m.owner) {
+      auto it = win.find(kv.second);
+      if (it != win.end()) kv.second = it->second;
+    }
+    for (int L : loser_of) {
+      const int Wn = uf_find(parent, L);
+      Object &lo = m.objs[L], &wo = m.objs[Wn];
+      losers_of_winner[Wn].push_back(L);
+      m.merged_from.push_back(L);
+      m.merged_into.push_back(Wn);
+      wo.n_voxels += lo.n_voxels;
+      wo.n_points += lo.n_points;
+      for (int k = 0; k < 3; ++k) {
+        wo.amin[k] = std::fmin(wo.amin[k], lo.amin[k]);
+        wo.amax[k] = std::fmax(wo.amax[k], lo.amax[k]);
+      }
+      if (lo.best.n_px > wo.best.n_px ||
+          (lo.best.n_px == wo.best.n_px && lo.best.n_px > 0 &&
+           (lo.best.frame < wo.best.frame || (lo.best.frame == wo.best.frame && lo.best.det < wo.best.det))))
+        wo.best = lo.best;
+      wo.gW += lo.gW;
+      for (int k = 0; k < 3; ++k) wo.gM1[k] += lo.gM1[k];
+      for (int k = 0; k < 6; ++k) wo.gM2[k] += lo.gM2[k];
+      for (const View &v : lo.views) offer_view(m, wo, v);
+      // covisibility: row W |= row L; every bit L becomes bit W; no diagonal
+      if ((size_t)L < m.covis.size() && (size_t)Wn < m.covis.size()) {
+        for (size_t w = 0; w < m.covis[L].size(); ++w) m.covis[Wn][w] |= m.covis[L][w];
+        for (size_t r = 0; r < m.covis.size(); ++r) {
+          auto &row = m.covis[r];
+          if (row.empty()) continue;
+          if (row[(size_t)L >> 6] >> (L & 63) & 1ull) {
+            row[(size_t)L >> 6] &= ~(1ull << (L & 63));
+            if ((int)r != Wn) row[(size_t)Wn >> 6] |= 1ull << (Wn & 63);
+          }
+        }
+        m.covis[Wn][(size_t)Wn >> 6] &= ~(1ull << (Wn & 63));
+        std::fill(m.covis[L].begin(), m.covis[L].end(), 0ull);
+      }
     }
   }
   // R12: keys unowned at entry go to the lowest-j detection of this call that contains them
@@ -443,6 +688,10 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
     Object &ob = m.objs[o];
     std::vector<double> sum(D);
     for (int i = 0; i < D; ++i) sum[i] = (double)ob.n_obs * (double)ob.f[i];
+    for (int L : losers_of_winner[o]) {  // U4: the losers' descriptors, weighted by their detection counts
+      for (int i = 0; i < D; ++i) sum[i] += (double)m.objs[L].n_obs * (double)m.objs[L].f[i];
+      ob.n_obs += m.objs[L].n_obs;
+    }
     for (int j : by_target[o]) {
       std::vector<double> ad(D);
       for (int i = 0; i < D; ++i) ad[i] = (double)load_storage(desc, m.dtype, (size_t)j * D + i);
@@ -464,16 +713,39 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
         ob.amin[k] = std::fmin(ob.amin[k], b[k]);
         ob.amax[k] = std::fmax(ob.amax[k], b[3 + k]);
       }
+      const float *Tf = T + 16 * det_frame[j];
+      const float cam[3] = {Tf[3], Tf[7], Tf[11]};
       if (m.n_px[j] > ob.best.n_px) {  // R23: strict > keeps the earliest (frame_seq, det) on ties
         ob.best.n_px = m.n_px[j];
         ob.best.frame = (int32_t)(m.frame_seq + det_frame[j]);
         ob.best.det = det_local[j];
-        const float *Tf = T + 16 * det_frame[j];
-        ob.best.cam[0] = Tf[3];
-        ob.best.cam[1] = Tf[7];
-        ob.best.cam[2] = Tf[11];
+        ob.best.cam[0] = cam[0];
+        ob.best.cam[1] = cam[1];
+        ob.best.cam[2] = cam[2];
+      }
+      if (m.views_k > 0) {  // V: detections offer their view in index order
+        View v;
+        if (make_view(b, cam, (int32_t)(m.frame_seq + det_frame[j]), det_local[j], m.n_px[j], &v)) offer_view(m, ob, v);
       }
     }
+  }
+  for (int L : loser_of) {  // U4: the absorbed entities stay as dead ids
+    Object &lo = m.objs[L];
+    lo.alive = false;
+    lo.alias = uf_find(parent, L);
+    lo.n_voxels = lo.n_obs = 0;
+    lo.n_points = 0;
+    std::fill(lo.f.begin(), lo.f.end(), 0.0f);
+    std::fill(lo.shadow.begin(), lo.shadow.end(), 0.0f);
+    for (int k = 0; k < 3; ++k) {
+      lo.amin[k] = std::numeric_limits<float>::infinity();
+      lo.amax[k] = -std::numeric_limits<float>::infinity();
+    }
+    lo.best = BestView();
+    lo.gW = 0.0;
+    for (int k = 0; k < 3; ++k) lo.gM1[k] = 0.0;
+    for (int k = 0; k < 6; ++k) lo.gM2[k] = 0.0;
+    lo.views.clear();
   }
   // C1: every pair of distinct entities observed in this call (matched or spawned) becomes covisible
   {
@@ -652,6 +924,166 @@ void oracle_read_covis(void *h, uint64_t *rows) {
   for (size_t a = 0; a < N; ++a)
     for (size_t w = 0; w < words; ++w) rows[a * words + w] = a < m.covis.size() && w < m.covis[a].size() ? m.covis[a][w] : 0;
 }
+// U4: alias[o] = o for a live entity, else the live entity that (transitively) absorbed it
+void oracle_read_alias(void *h, int32_t *alias) {
+  Map &m = *(Map *)h;
+  for (size_t o = 0; o < m.objs.size(); ++o) {
+    size_t r = o;
+    while (!m.objs[r].alive) r = (size_t)m.objs[r].alias;
+    alias[o] = (int32_t)r;
+  }
+}
+// U4: (loser, winner) pairs of the last call; returns their number
+int oracle_last_merges(void *h, int32_t *from, int32_t *into) {
+  Map &m = *(Map *)h;
+  for (size_t i = 0; i < m.merged_from.size(); ++i) {
+    if (from) from[i] = m.merged_from[i];
+    if (into) into[i] = m.merged_into[i];
+  }
+  return (int)m.merged_from.size();
+}
+// V: retained views, [N, k] records of 12 floats/ints each: frame, det, n_px, cam[3], dir[3], dist; counts [N]
+typedef struct {
+  int32_t frame, det;
+  uint32_t n_px;
+  float cam[3], dir[3], dist;
+} oracle_view;
+void oracle_read_views(void *h, oracle_view *views, int32_t *counts, int k) {
+  Map &m = *(Map *)h;
+  for (size_t o = 0; o < m.objs.size(); ++o) {
+    counts[o] = (int32_t)m.objs[o].views.size();
+    for (int i = 0; i < k; ++i) {
+      oracle_view &q = views[o * (size_t)k + i];
+      std::memset(&q, 0, sizeof q);
+      q.frame = q.det = -1;
+      if (i < (int)m.objs[o].views.size()) {
+        const View &v = m.objs[o].views[i];
+        q.frame = v.frame, q.det = v.det, q.n_px = v.n_px, q.dist = v.dist;
+        for (int c = 0; c < 3; ++c) q.cam[c] = v.cam[c], q.dir[c] = v.dir[c];
+      }
+    }
+  }
+}
+
+// ---- Q1-Q5: retrieval-side scoring, a second workload over the finished memory.
+// Inputs (the three retrieval embedding spaces of PAPER.md:356 are INPUTS here, as descriptors are for the mapper):
+//   emb[s]  [N, dim[s]] fp32 values of the storage dtype, s = 0 caption text, 1 image (SigLIP2-like), 2 image (VL-like)
+//   cls     [N] class id per entity (int), centroid [N,3] entity centroids (Gaussian mean where the entity has one)
+//   alive   [N] 0/1
+//   channels of ONE query variable: q[0] target description in space 0 (w = 1.0), q[1] raw utterance in space 0
+//   (w = 0.5), q[2] prompt (ensemble mean) in space 1 (w = 0.75), q[3] target description in space 2 (w = 1.0).
+// Q1 per channel: cos of the query with every live entity (R15 arithmetic), rank 1 = largest, ties -> lower id.
+// Q2 s_sem(o) = sum_c w_c / (mu + rank_c(o)), mu = 5  ("each channel contributes w/(mu+rank) with offset mu = 5").
+// Q3 class factor: s_sem *= 0.3 when target_class >= 0 and cls[o] != target_class.
+// Q4 predicates, each with its own landmark variable (4 channels); the landmark is bound greedily to its top-scoring
+//    live entity (largest fused rank score, ties -> lowest id).  Near: exp(-d^2 / (2 sigma^2)), sigma = 0.5 m; NextTo:
+//    sigma = 1.0 m, d = inter-centroid distance.  Closest / Farthest: 1 / (|rank - r*| + 1) with rank = position of the
+//    entity among the live entities ordered by d (1 = nearest, ties -> lower id), r* = 1 / n_live.
+// Q5 gbar = geometric mean of the predicate scores (1 with no predicate); s = s_sem * ((1 - w) + w * gbar), w = 0.5.
+// Output: s_sem [N], gbar [N], s [N] (0 for dead entities), landmark ids [P], and the top-K ids by s (ties -> lower id).
+namespace {
+struct RankItem {
+  float c;
+  int o;
+};
+void rrf_scores(int N, const uint8_t *alive, const float *const *emb, const int *dim, const float *const *q,
+                std::vector<double> &out, std::vector<float> *cos_out) {
+  static const int space_of[4] = {0, 0, 1, 2};
+  static const double wch[4] = {1.0, 0.5, 0.75, 1.0};
+  out.assign(N, 0.0);
+  for (int ch = 0; ch < 4; ++ch) {
+    const int sp = space_of[ch], Dn = dim[sp];
+    std::vector<RankItem> items;
+    for (int o = 0; o < N; ++o) {
+      if (!alive[o]) continue;
+      const float c = cosine(q[ch], emb[sp] + (size_t)o * Dn, Dn);
+      items.push_back({c, o});
+      if (cos_out) cos_out[ch][o] = c;
+    }
+    std::stable_sort(items.begin(), items.end(), [](const RankItem &x, const RankItem &y) { return x.c > y.c; });
+    for (size_t r = 0; r < items.size(); ++r) out[items[r].o] += wch[ch] / (5.0 + (double)(r + 1));
+  }
+}
+}  // namespace
+
+int oracle_query(int N, const uint8_t *alive, const float *emb0, const float *emb1, const float *emb2, int d0, int d1, int d2,
+                 const int32_t *cls, const float *centroid, const float *q_target /*concat of 4 channel vectors*/,
+                 int target_class, int P, const int32_t *pred_type, const float *q_landmarks /*P x concat of 4*/,
+                 int topk, float *s_sem_out, float *gbar_out, float *s_out, int32_t *landmark_out, int32_t *top_out,
+                 float *cos_out /*[4,N] target channels, may be NULL*/) {
+  const float *emb[3] = {emb0, emb1, emb2};
+  const int dim[3] = {d0, d1, d2};
+  const int qlen = d0 + d0 + d1 + d2;
+  auto split = [&](const float *base, const float *q[4]) {
+    q[0] = base, q[1] = base + d0, q[2] = base + 2 * d0, q[3] = base + 2 * d0 + d1;
+  };
+  const float *qt[4];
+  split(q_target, qt);
+  std::vector<double> ssem;
+  std::vector<float> cosbuf[4];
+  if (cos_out)
+    for (int c = 0; c < 4; ++c) cosbuf[c].assign(N, 0.0f);
+  rrf_scores(N, alive, emb, dim, qt, ssem, cos_out ? cosbuf : nullptr);
+  if (cos_out)
+    for (int c = 0; c < 4; ++c) std::memcpy(cos_out + (size_t)c * N, cosbuf[c].data(), sizeof(float) * N);
+  int n_live = 0;
+  for (int o = 0; o < N; ++o) n_live += alive[o] ? 1 : 0;
+  std::vector<double> logsum(N, 0.0);
+  std::vector<char> zero(N, 0);
+  for (int p = 0; p < P; ++p) {
+    const float *ql[4];
+    split(q_landmarks + (size_t)p * qlen, ql);
+    std::vector<double> ls;
+    rrf_scores(N, alive, emb, dim, ql, ls, nullptr);
+    int lm = -1;
+    for (int o = 0; o < N; ++o)
+      if (alive[o] && (lm < 0 || ls[o] > ls[lm])) lm = o;
+    landmark_out[p] = lm;
+    if (lm < 0) continue;
+    std::vector<double> dist(N, 0.0);
+    for (int o = 0; o < N; ++o) {
+      double d2s = 0;
+      for (int k = 0; k < 3; ++k) {
+        const double d = (double)centroid[3 * o + k] - (double)centroid[3 * lm + k];
+        d2s += d * d;
+      }
+      dist[o] = std::sqrt(d2s);
+    }
+    std::vector<int> order;
+    for (int o = 0; o < N; ++o)
+      if (alive[o]) order.push_back(o);
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return dist[x] < dist[y]; });
+    std::vector<int> rank(N, 0);
+    for (size_t r = 0; r < order.size(); ++r) rank[order[r]] = (int)r + 1;
+    for (int o = 0; o < N; ++o) {
+      if (!alive[o]) continue;
+      double g = 0;
+      switch (pred_type[p]) {
+        case 0: g = std::exp(-dist[o] * dist[o] / (2.0 * 0.5 * 0.5)); break;           // Near, sigma = 0.5 m
+        case 1: g = std::exp(-dist[o] * dist[o] / (2.0 * 1.0 * 1.0)); break;           // NextTo, sigma = 1.0 m
+        case 2: g = 1.0 / (std::abs(rank[o] - 1) + 1.0); break;                         // Closest: r* = 1
+        case 3: g = 1.0 / (std::abs(rank[o] - n_live) + 1.0); break;                    // Farthest: r* = n_live
+        default: return -1;
+      }
+      if (g > 0) logsum[o] += std::log(g); else zero[o] = 1;
+    }
+  }
+  std::vector<RankItem> fin;
+  for (int o = 0; o < N; ++o) {
+    double ss = alive[o] ? ssem[o] : 0.0;
+    if (alive[o] && target_class >= 0 && cls[o] != target_class) ss *= 0.3;         // Q3 soft class factor
+    const double gb = !alive[o] ? 0.0 : (P == 0 ? 1.0 : (zero[o] ? 0.0 : std::exp(logsum[o] / P)));
+    const double sc = ss * ((1.0 - 0.5) + 0.5 * gb);                                  // Q5, w = 0.5
+    s_sem_out[o] = (float)ss;
+    gbar_out[o] = (float)gb;
+    s_out[o] = (float)sc;
+    if (alive[o]) fin.push_back({(float)sc, o});
+  }
+  std::stable_sort(fin.begin(), fin.end(), [](const RankItem &x, const RankItem &y) { return x.c > y.c; });
+  for (int k = 0; k < topk; ++k) top_out[k] = k < (int)fin.size() ? fin[k].o : -1;
+  return 0;
+}
+
 double oracle_hellinger(const double *mu1, const double *cov1, const double *mu2, const double *cov2, double eps2) {
   return hellinger(mu1, cov1, mu2, cov2, eps2);
 }

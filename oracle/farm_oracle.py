@@ -22,6 +22,9 @@ STATS_DTYPE = np.dtype(
     [("valid_points", "<u8"), ("dropped_points", "<u8"), ("ignored_pixels", "<u8"), ("unique_voxels", "<u8"),
      ("matches", "<u4"), ("spawns", "<u4"), ("skipped", "<u4"), ("n_det", "<u4")], align=True)
 assert OBJECT_DTYPE.itemsize == 72
+VIEW_DTYPE = np.dtype([("frame", "<i4"), ("det", "<i4"), ("n_px", "<u4"), ("cam", "<f4", 3), ("dir", "<f4", 3), ("dist", "<f4")])
+assert VIEW_DTYPE.itemsize == 40
+PRED_NEAR, PRED_NEXTTO, PRED_CLOSEST, PRED_FARTHEST = 0, 1, 2, 3
 
 _lib = None
 
@@ -39,6 +42,7 @@ def lib():
         _lib.oracle_round_to_storage.restype = C.c_float
         _lib.oracle_round_to_storage.argtypes = [C.c_float, C.c_int]
         _lib.oracle_cosine.restype = C.c_float
+        _lib.oracle_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _lib.oracle_hellinger.restype = C.c_double
         _lib.oracle_hellinger.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
     return _lib
@@ -58,9 +62,43 @@ class OracleMap:
             lib().oracle_destroy(self.h)
             self.h = None
 
+    # ---- round-2 options (all off by default): U correspondence, H geometry, V views
+    OPT_CORRESPONDENCE, OPT_GEOMETRY, OPT_PREFILTER_COS, OPT_HELLINGER_BUDGET, OPT_VIEWS_K, OPT_VIEW_COS, OPT_VIEW_CLOSER = 1, 2, 3, 4, 5, 6, 7
+
+    def set_option(self, key, value):
+        rc = lib().oracle_set_option(self.h, C.c_int(key), C.c_double(value))
+        assert rc == 0, f"oracle option {key} = {value} rejected"
+        if key == self.OPT_VIEWS_K:
+            self.views_k = int(value)
+
+    def read_alias(self):
+        """U4: alias [N]: the live entity every id now stands for (itself while alive)."""
+        N = lib().oracle_n_objects(self.h)
+        al = np.zeros(N, np.int32)
+        lib().oracle_read_alias(self.h, _p(al))
+        return al
+
+    def last_merges(self):
+        """U4: (loser [n], winner [n]) entity merges executed by the last call."""
+        n = lib().oracle_last_merges(self.h, None, None)
+        a, b = np.zeros(n, np.int32), np.zeros(n, np.int32)
+        lib().oracle_last_merges(self.h, _p(a), _p(b))
+        return a, b
+
+    def read_views(self):
+        """V: (views [N, k] VIEW_DTYPE, counts [N])"""
+        N = lib().oracle_n_objects(self.h)
+        k = getattr(self, "views_k", 0)
+        views = np.zeros((N, max(k, 1)), VIEW_DTYPE)
+        counts = np.zeros(N, np.int32)
+        if k:
+            lib().oracle_read_views(self.h, _p(views), _p(counts), C.c_int(k))
+        return views[:, :k], counts
+
     def clone(self):
         c = OracleMap.__new__(OracleMap)
         c.D, c.dtype, c.H, c.W = self.D, self.dtype, self.H, self.W
+        c.views_k = getattr(self, "views_k", 0)
         c.h = C.c_void_p(lib().oracle_clone(self.h))
         return c
 
@@ -198,3 +236,30 @@ def cosine(a, b):
     a = np.ascontiguousarray(a, np.float32)
     b = np.ascontiguousarray(b, np.float32)
     return float(lib().oracle_cosine(_p(a), _p(b), C.c_int(a.size)))
+
+
+def query(alive, emb, cls, centroid, q_target, target_class, pred_types, q_landmarks, topk, want_cos=False):
+    """Q1-Q5 retrieval scoring.  emb: three [N, d_s] float32 arrays; q_target: four channel vectors (d0, d0, d1, d2);
+    q_landmarks: one such list of four per predicate.  Returns dict(s_sem, gbar, s, landmarks, top[, cos])."""
+    N = len(alive)
+    alive = np.ascontiguousarray(alive, np.uint8)
+    emb = [np.ascontiguousarray(e, np.float32) for e in emb]
+    dims = [e.shape[1] for e in emb]
+    cls = np.ascontiguousarray(cls, np.int32)
+    centroid = np.ascontiguousarray(centroid, np.float32)
+    qt = np.ascontiguousarray(np.concatenate([np.asarray(x, np.float32).ravel() for x in q_target]), np.float32)
+    P = len(pred_types)
+    pt = np.ascontiguousarray(pred_types, np.int32)
+    ql = np.ascontiguousarray(np.concatenate([np.asarray(x, np.float32).ravel() for lm in q_landmarks for x in lm]) if P else np.zeros(1), np.float32)
+    s_sem, gbar, sc = np.zeros(N, np.float32), np.zeros(N, np.float32), np.zeros(N, np.float32)
+    lms = np.zeros(max(P, 1), np.int32)
+    top = np.zeros(topk, np.int32)
+    cos = np.zeros((4, N), np.float32) if want_cos else None
+    rc = lib().oracle_query(C.c_int(N), _p(alive), _p(emb[0]), _p(emb[1]), _p(emb[2]), C.c_int(dims[0]), C.c_int(dims[1]),
+                            C.c_int(dims[2]), _p(cls), _p(centroid), _p(qt), C.c_int(target_class), C.c_int(P), _p(pt), _p(ql),
+                            C.c_int(topk), _p(s_sem), _p(gbar), _p(sc), _p(lms), _p(top), _p(cos))
+    assert rc == 0
+    out = {"s_sem": s_sem, "gbar": gbar, "s": sc, "landmarks": lms[:P], "top": top}
+    if want_cos:
+        out["cos"] = cos
+    return out

@@ -16,7 +16,9 @@ namespace {
 constexpr int TILE_W = 64;        // 8 threads x 8 pixels per row
 constexpr int TILE_H = 16;
 constexpr int LIFT_THREADS = 128;
-constexpr int TILE_ENT = 256;     // (detection, block) entries per tile; overflow goes straight to the global queue
+constexpr int LIFT_WARPS = LIFT_THREADS / 32;
+constexpr int TILE_ENT = 128;     // (detection, block) entries per tile; overflow goes straight to the global queue
+constexpr int STAGE_PX = 128;     // compacted pixels per warp and round (4 of a lane's 8 pixels)
 constexpr int MAX_LABELS = 32;    // per-tile detection accumulators (the entry tag holds a 5-bit label slot)
 constexpr int LABEL_SHIFT = 57;   // block keys use bits 0..56
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
@@ -187,6 +189,8 @@ __device__ __forceinline__ void survivor_store(const DevMap &m, uint32_t pos, un
 struct TileSmem {
   unsigned long long tag[TILE_ENT];       // block key | label slot << 57, BLK_EMPTY when free
   uint32_t mlo[TILE_ENT], mhi[TILE_ENT];  // voxel bits of the block seen for that detection inside the tile
+  unsigned long long stage[LIFT_WARPS][STAGE_PX];  // per warp, the compacted masked pixels of one round:
+                                                   // (label << 16 | row in tile << 8 | column in tile) << 32 | depth bits
   uint32_t q_count;                       // entries flushed by the tile that just finished
   uint32_t cur_pos, cur_end;              // the CTA's current chunk of the survivor queue
   uint32_t next_base, next_valid;         // the chunk reserved after it
@@ -208,25 +212,10 @@ __device__ __forceinline__ int tile_label_slot_in(uint32_t *lab_j, uint32_t j) {
   return -1;
 }
 
-// accumulate cnt pixels and their box (ordered ints) of detection j into the tile's per-detection accumulators
-__device__ __forceinline__ void label_add_in(uint32_t *lab_cnt, int (*lab_box)[6], const DevMap &m, int li, uint32_t j,
-                                             uint32_t cnt, int mn0, int mn1, int mn2, int mx0, int mx1, int mx2) {
-  if (li >= 0) {
-    atomicAdd(&lab_cnt[li], cnt);
-    atomicMin(&lab_box[li][0], mn0), atomicMin(&lab_box[li][1], mn1), atomicMin(&lab_box[li][2], mn2);
-    atomicMax(&lab_box[li][3], mx0), atomicMax(&lab_box[li][4], mx1), atomicMax(&lab_box[li][5], mx2);
-    return;
-  }
-  atomicAdd(&m.det_npx[j], cnt);
-  atomicMin(&m.det_box[j * 6 + 0], mn0), atomicMin(&m.det_box[j * 6 + 1], mn1), atomicMin(&m.det_box[j * 6 + 2], mn2);
-  atomicMax(&m.det_box[j * 6 + 3], mx0), atomicMax(&m.det_box[j * 6 + 4], mx1), atomicMax(&m.det_box[j * 6 + 5], mx2);
-}
-
 // OR the voxel bits (lo, hi) of block `bkey` into the tile's entry of (label slot li, block).  Exact: the tag
-// holds the whole block key and the label slot.  Without a label slot, or when the tile table is full, the
-// record goes straight to the global queue (the probe kernel's pair set keeps the result exact).
+// holds the whole block key and the label slot.  When the tile table is full the record goes straight to the
+// global queue (the probe kernel's pair set keeps the result exact).
 __device__ __forceinline__ bool tile_block_add(TileSmem &s, int li, unsigned long long bkey, uint32_t lo, uint32_t hi) {
-  if (li < 0) return false;
   const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
   uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
   for (int probe = 0; probe < 16; ++probe) {  // a short probe sequence: a miss only costs one more queue record
@@ -263,18 +252,17 @@ struct TileRegs {
   uint4 mk;
 };
 
+// A warp owns a 16-column x 16-row patch of the tile: lane -> row = lane >> 1, 8 consecutive pixels at column
+// 16 * warp + 8 * (lane & 1)  (32 contiguous bytes of depth and 16 of mask per lane: whole DRAM sectors).
+// (f, ty, tx) = frame and tile coordinates.
 template <bool VEC>
-__device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a, int tile, int tiles_x, int tiles_xy, int tid) {
-  const int f = tile / tiles_xy;
-  const int trem = tile - f * tiles_xy;
-  const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
-  const int v = ty * TILE_H + (tid >> 3);
-  const int u0 = tx * TILE_W + (tid & 7) * 8;
-  const size_t frame_off = (size_t)f * m.H * m.W;
+__device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a, int f, int ty, int tx, int row, int cg) {
+  const int v = ty * TILE_H + row;
+  const int u0 = tx * TILE_W + cg * 8;
   const bool row_ok = v < m.H;
+  const size_t off = ((size_t)f * m.H + v) * m.W + u0;
   TileRegs r;
   if (VEC && row_ok && u0 + 7 < m.W) {
-    const size_t off = frame_off + (size_t)v * m.W + u0;
     r.d0 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off));
     r.d1 = __ldcs(reinterpret_cast<const float4 *>(a.depth + off + 4));
     r.mk = __ldcs(reinterpret_cast<const uint4 *>(a.mask + off));
@@ -284,9 +272,8 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const bool ok = row_ok && u0 + i < m.W;
-      const size_t off = frame_off + (size_t)v * m.W + u0 + i;
-      lab[i] = ok ? (uint32_t)__ldcs(a.mask + off) : 0u;
-      z[i] = ok ? __ldcs(a.depth + off) : 0.f;
+      lab[i] = ok ? (uint32_t)__ldcs(a.mask + off + i) : 0u;
+      z[i] = ok ? __ldcs(a.depth + off + i) : 0.f;
     }
     r.d0 = make_float4(z[0], z[1], z[2], z[3]);
     r.d1 = make_float4(z[4], z[5], z[6], z[7]);
@@ -295,84 +282,87 @@ __device__ __forceinline__ TileRegs load_tile(const DevMap &m, const CallArgs &a
   return r;
 }
 
-// Rare path of the lift kernel: one pixel whose detection differs from the first detection of its thread.  It
-// is added on its own: count 1, box = the point, one voxel bit of its block.
-__device__ __noinline__ void stray_pixel(TileSmem &s, uint32_t *lab_j, uint32_t *lab_cnt, int (*lab_box)[6], uint32_t *det_npx,
-                                         int *det_box, unsigned long long *surv_key, unsigned long long *surv_bits,
-                                         uint32_t *surv_j, uint32_t surv_cap, uint32_t *counters, uint32_t *err, double *det_gm,
-                                         uint32_t j, unsigned long long bkey, uint32_t bit, float p0, float p1, float p2) {
-  if (det_gm) {  // G1: the point's contribution to the detection's moments
-    double *g = det_gm + (size_t)j * 9;
-    const double x = p0, y = p1, z = p2;
-    atomicAdd(g + 0, x), atomicAdd(g + 1, y), atomicAdd(g + 2, z);
-    atomicAdd(g + 3, x * x), atomicAdd(g + 4, x * y), atomicAdd(g + 5, x * z);
-    atomicAdd(g + 6, y * y), atomicAdd(g + 7, y * z), atomicAdd(g + 8, z * z);
-  }
-  const int li = tile_label_slot_in(lab_j, j);
-  const int o0 = f2ord(p0), o1 = f2ord(p1), o2 = f2ord(p2);
-  const uint32_t lo = (bit & 32) ? 0u : 1u << (bit & 31), hi = (bit & 32) ? 1u << (bit & 31) : 0u;
-  if (li >= 0) {
-    atomicAdd(&lab_cnt[li], 1u);
-    atomicMin(&lab_box[li][0], o0), atomicMin(&lab_box[li][1], o1), atomicMin(&lab_box[li][2], o2);
-    atomicMax(&lab_box[li][3], o0), atomicMax(&lab_box[li][4], o1), atomicMax(&lab_box[li][5], o2);
-    const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
-    uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
-    for (int probe = 0; probe < TILE_ENT; ++probe) {
-      unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
-      if (cur == BLK_EMPTY) {
-        cur = atomicCAS(&s.tag[h], BLK_EMPTY, tag);
-        if (cur == BLK_EMPTY) cur = tag;
-      }
-      if (cur == tag) {
-        if (lo) atomicOr(&s.mlo[h], lo);
-        if (hi) atomicOr(&s.mhi[h], hi);
-        return;
-      }
-      h = (h + 1) & (TILE_ENT - 1);
-    }
-  } else {
-    atomicAdd(&det_npx[j], 1u);
-    atomicMin(&det_box[j * 6 + 0], o0), atomicMin(&det_box[j * 6 + 1], o1), atomicMin(&det_box[j * 6 + 2], o2);
-    atomicMax(&det_box[j * 6 + 3], o0), atomicMax(&det_box[j * 6 + 4], o1), atomicMax(&det_box[j * 6 + 5], o2);
-  }
-  const uint32_t pos = atomicAdd(&counters[2], 1u);
-  if (pos < surv_cap) {
-    surv_key[pos] = bkey;
-    surv_bits[pos] = ((unsigned long long)hi << 32) | lo;
-    surv_j[pos] = j;
-  } else {
-    atomicOr(err, ERR_PAIR_TABLE_FULL);
+// per-lane running evidence of the detection and voxel block the lane is currently looking at
+// (R7: voxel bits of the block, pixel count, point box; G1: moments)
+template <bool GAUSS>
+struct LaneAcc {
+  uint32_t j, cnt;          // detection (NONE32 = none yet in this tile) and its pixels seen by the lane
+  int li;                   // its label slot in the tile (-1: none left)
+  uint32_t klo, khi;        // current block key (64 bit, two halves) and
+  uint32_t mlo, mhi;        //   the voxel bits of that block seen by the lane
+  float mn0, mn1, mn2, mx0, mx1, mx2;
+  float gc0, gc1, gc2, g1x, g1y, g1z, gxx, gxy, gxz, gyy, gyz, gzz;  // G1, about the lane's first point (GAUSS only)
+};
+
+// G1: raw moments in double from the lane's centred fp32 sums (parallel-axis shift)
+template <bool GAUSS>
+__device__ __forceinline__ void lane_raw_moments(const LaneAcc<GAUSS> &c, double g[9]) {
+  const double n = (double)c.cnt, c0 = c.gc0, c1 = c.gc1, c2 = c.gc2, sx = c.g1x, sy = c.g1y, sz = c.g1z;
+  g[0] = sx + n * c0, g[1] = sy + n * c1, g[2] = sz + n * c2;
+  g[3] = c.gxx + 2.0 * c0 * sx + n * c0 * c0, g[4] = c.gxy + c0 * sy + c1 * sx + n * c0 * c1, g[5] = c.gxz + c0 * sz + c2 * sx + n * c0 * c2;
+  g[6] = c.gyy + 2.0 * c1 * sy + n * c1 * c1, g[7] = c.gyz + c1 * sz + c2 * sy + n * c1 * c2, g[8] = c.gzz + 2.0 * c2 * sz + n * c2 * c2;
+}
+
+// rare: the lane's detection changes inside a patch -- its partial evidence goes to the detection on its own
+template <bool GAUSS>
+__device__ __forceinline__ void lane_flush_own(const DevMap &m, const LaneAcc<GAUSS> &c) {
+  const uint32_t j = c.j;
+  atomicAdd(&m.det_npx[j], c.cnt);
+  atomicMin(&m.det_box[j * 6 + 0], f2ord(c.mn0)), atomicMin(&m.det_box[j * 6 + 1], f2ord(c.mn1)), atomicMin(&m.det_box[j * 6 + 2], f2ord(c.mn2));
+  atomicMax(&m.det_box[j * 6 + 3], f2ord(c.mx0)), atomicMax(&m.det_box[j * 6 + 4], f2ord(c.mx1)), atomicMax(&m.det_box[j * 6 + 5], f2ord(c.mx2));
+  if (GAUSS) {
+    double g[9];
+    lane_raw_moments<GAUSS>(c, g);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) atomicAdd(m.det_gm + (size_t)j * 9 + k, g[k]);
   }
 }
 
+// the lane's voxel bits of its current (detection, block) -> the tile's table; to the global queue when the table
+// cannot take them (no label slot, table full).  Called when the lane moves on to another block.
+template <bool GAUSS>
+__device__ __forceinline__ void lane_flush_block(const DevMap &m, TileSmem &s, const LaneAcc<GAUSS> &c) {
+  const unsigned long long bkey = ((unsigned long long)c.khi << 32) | c.klo;
+  if (c.li >= 0 && tile_block_add(s, c.li, bkey, c.mlo, c.mhi)) return;
+  survivor_store(m, atomicAdd(&m.counters[2], 1u), bkey, c.j, c.mlo, c.mhi);
+}
+
 // ---------------------------------------------------------------------------------------------------
-// lift kernel (steps 1-2).  Persistent CTAs; one 64x16 pixel tile per iteration, each thread owns 8
-// consecutive pixels of one row (2 x 128-bit depth loads + 1 x 128-bit mask load, issued one tile ahead).
-//   Phase 1 (straight-line fp32/int code per pixel): validity (R3, R4), back-projection (R5), voxel index
-//     (R6) -> block key + voxel bit, point box.
-//   Phase 2 (warp-synchronous): the voxel of a pixel is one bit of its block's 64-bit mask, so the
-//     per-detection dedupe (R7) is a bitwise OR -- over the thread's pixels of one block, over the lanes of
-//     the warp that hold the same (detection, block) (match.any + redux.or), and into the tile's
-//     shared-memory table (atomicOr).
-//   Flush: one (block, detection, voxel bits) record per table entry goes to the call's survivor queue.  The
-//     CTA reserves queue space in chunks of TILE_ENT records one tile ahead, so no thread ever waits for a
-//     global atomic; the unused tail of the last chunk is padded with empty records (bits == 0).
-// Two barriers per tile.  Per-detection pixel counts and point boxes go through shared-memory
-// accumulators (REDUX fast path when a warp holds one detection) to one set of global atomics per
-// (tile, detection).
+// lift kernel (steps 1-2).  Persistent CTAs; one 64x16 pixel tile per iteration; each warp owns a 16x16 patch of
+// it and each lane 8 consecutive pixels of one row (2 x 128-bit depth loads + 1 x 128-bit mask load, issued one
+// tile ahead).
+//   Compaction (BASELINE.json: "warp-ballot compaction of masked pixels"): the lanes mark their valid masked
+//     pixels (R3, R4); per pixel position one ballot gives every valid pixel its dense slot (prefix popcount), and
+//     depth + (label, row, column) go to the warp's staging area in shared memory as one 64-bit word, 4 of a lane's 8
+//     pixels per round.  The arithmetic below then runs over DENSE slots -- one pixel per lane, every lane busy
+//     except in the last iteration of a round.
+//   Per pixel (straight-line fp32/int code): back-projection (R5, every operation individually rounded), voxel
+//     index (R6; floor by a round-down add of 1.5 * 2^23, exact for |x| < 2^22), block key + voxel bit.
+//   Dedupe (R7): the voxel of a pixel is one bit of its block's 64-bit mask.  A lane ORs the bits of consecutive
+//     pixels that fall into the same (detection, block) in registers (neighbouring pixels nearly always do), together
+//     with the pixel count and point box (and G1 moments) of the detection; when it moves on to another block the bits go
+//     to the tile's shared-memory table (atomicOr), and at the end of the patch the lanes holding the same
+//     (detection, block) combine theirs first (match.any + redux.or).  No per-pixel warp-collective work.
+//   Flush: one (block, detection, voxel bits) record per table entry goes to the call's survivor queue.  The CTA
+//     reserves queue space in chunks of TILE_ENT records one tile ahead, so no thread ever waits for a global
+//     atomic; the unused tail of the last chunk is padded with empty records (bits == 0).  The lanes' pixel counts
+//     and boxes are combined per detection over the warp (REDUX) and leave as one set of global atomics per
+//     (warp patch, detection).
+// Two barriers per tile.
 template <bool VEC, bool GAUSS>
 __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   pdl_trigger();  // the probe kernel may become resident as soon as CTAs of this grid retire
   __shared__ TileSmem s;
-  __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads
-  __shared__ uint32_t lab_cnt2[2][MAX_LABELS];  // its copy while tile t+1 initialises the other
-  __shared__ int lab_box2[2][MAX_LABELS][6];
-  const int tid = threadIdx.x, lane = tid & 31;
+  __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads its copy
+                                              // while tile t+1 initialises the other
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tiles_xy = tiles_x * tiles_y;
   const int n_tiles = tiles_xy * a.F;
-  const float inv_vs = m.inv_vs, z_min = m.z_min, z_max = m.z_max;
+  const float inv_vs = m.inv_vs, z_min = m.z_min;
+  const float z_max = fminf(m.z_max, 3.402823466e+38f);  // z <= z_max then also rejects +inf and NaN (R4: finite)
   const float INF = __int_as_float(0x7F800000);
   constexpr unsigned FULL = 0xFFFFFFFFu;
+  const unsigned lt_mask = (1u << lane) - 1u;
   for (int i = tid; i < TILE_ENT; i += LIFT_THREADS) {
     s.tag[i] = BLK_EMPTY;
     s.mlo[i] = 0;
@@ -383,32 +373,34 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
     s.n_valid = 0, s.n_dropped = 0, s.n_ignored = 0;
   }
   uint32_t acc_valid = 0, acc_dropped = 0, acc_ignored = 0;  // per-thread counters over all tiles
+  const int row = lane >> 1, cg = warp * 2 + (lane & 1);     // the lane's row and 8-pixel column group inside a tile
+  unsigned long long *stage = s.stage[warp];
+  // tile coordinates advance incrementally (no per-tile divisions): this CTA's tiles are blockIdx.x + k * gridDim.x
+  int f = blockIdx.x / tiles_xy, ty = (blockIdx.x - f * tiles_xy) / tiles_x, tx = blockIdx.x - f * tiles_xy - ty * tiles_x;
+  const int df = gridDim.x / tiles_xy, dty = (gridDim.x - df * tiles_xy) / tiles_x, dtx = gridDim.x - df * tiles_xy - dty * tiles_x;
+  auto advance = [&](int &ff, int &yy, int &xx) {
+    xx += dtx;
+    if (xx >= tiles_x) xx -= tiles_x, ++yy;
+    yy += dty;
+    if (yy >= tiles_y) yy -= tiles_y, ++ff;
+    ff += df;
+  };
   int par = 0;
-  TileRegs cur = load_tile<VEC>(m, a, blockIdx.x, tiles_x, tiles_xy, tid);
+  TileRegs cur = load_tile<VEC>(m, a, f, ty, tx, row, cg);
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, par ^= 1) {
+    int nf = f, nty = ty, ntx = tx;
+    advance(nf, nty, ntx);
     TileRegs nxt = cur;
-    if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, tile + gridDim.x, tiles_x, tiles_xy, tid);
-    const int f = tile / tiles_xy;
-    const int trem = tile - f * tiles_xy;
-    const int ty = trem / tiles_x, tx = trem - ty * tiles_x;
-    const int v = ty * TILE_H + (tid >> 3);
-    const int u0 = tx * TILE_W + (tid & 7) * 8;
+    if (tile + (int)gridDim.x < n_tiles) nxt = load_tile<VEC>(m, a, nf, nty, ntx, row, cg);
+    // (float)u = as_float(0x4B000000 | u) - 2^23 for u < 2^23: the tile origin is folded into the integer constant
+    const uint32_t v_magic = 0x4B000000u + (uint32_t)(ty * TILE_H), u_magic = 0x4B000000u + (uint32_t)(tx * TILE_W);
     // camera of the frame, prepared by prep_kernel: (inv_fx, inv_fy, cx, cy), (r00 r01 r02 tx), (r10 ..), (r20 ..)
     const float4 *cp = reinterpret_cast<const float4 *>(m.cam + 16 * f);
     const float4 c0 = __ldg(cp), c1 = __ldg(cp + 1), c2 = __ldg(cp + 2), c3 = __ldg(cp + 3);
     const int det_base = a.base[f];
     const uint32_t n_det_f = (uint32_t)(a.base[f + 1] - det_base);
-    uint32_t *lab_j = lab_j2[par], *lab_cnt = lab_cnt2[par];
-    int(*lab_box)[6] = lab_box2[par];
-    if (tid < MAX_LABELS) {
-      lab_j[tid] = NONE32;
-      lab_cnt[tid] = 0;
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        lab_box[tid][k] = 0x7FFFFFFF;
-        lab_box[tid][3 + k] = (int)0x80000000;
-      }
-    }
+    uint32_t *lab_j = lab_j2[par];
+    if (tid < MAX_LABELS) lab_j[tid] = NONE32;
     __syncthreads();  // B1: label table ready; every warp has finished the flush of the previous tile
     if (tid == 0) {
       // account for the records the previous tile flushed; reserve the next queue chunk one tile ahead
@@ -426,139 +418,155 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
       }
     }
 
-    // ---- phase 1
-    const float z[8] = {cur.d0.x, cur.d0.y, cur.d0.z, cur.d0.w, cur.d1.x, cur.d1.y, cur.d1.z, cur.d1.w};
-    const uint32_t lab[8] = {cur.mk.x & 0xFFFF, cur.mk.x >> 16, cur.mk.y & 0xFFFF, cur.mk.y >> 16,
-                             cur.mk.z & 0xFFFF, cur.mk.z >> 16, cur.mk.w & 0xFFFF, cur.mk.w >> 16};
-    const float yn = __fmul_rn(__fsub_rn((float)v, c0.w), c0.y);  // R5 term shared by the thread's 8 pixels
-    const float u0f = (float)u0;  // (float)(u0 + i) == u0f + (float)i exactly (integers below 2^24)
-    unsigned long long ikey[8];
-    uint32_t ibit_lo = 0, ibit_hi = 0;  // 6-bit voxel index inside the block, pixels 0-3 / 4-7
-    uint32_t valid = 0, L0 = 0;         // pixels of the thread's first detection L0 (almost always the only one)
-    float mn0 = INF, mn1 = INF, mn2 = INF, mx0 = -INF, mx1 = -INF, mx2 = -INF;
-    // G1: moments of the thread's points about its first point (fp32 stays exact enough: offsets of a few cm)
-    float gc0 = 0.f, gc1 = 0.f, gc2 = 0.f, g1x = 0.f, g1y = 0.f, g1z = 0.f;
-    float gxx = 0.f, gxy = 0.f, gxz = 0.f, gyy = 0.f, gyz = 0.f, gzz = 0.f;
+    // ---- validity of the lane's 8 pixels (R3, R4)
+    const float z8[8] = {cur.d0.x, cur.d0.y, cur.d0.z, cur.d0.w, cur.d1.x, cur.d1.y, cur.d1.z, cur.d1.w};
+    const uint32_t lab8[8] = {cur.mk.x & 0xFFFF, cur.mk.x >> 16, cur.mk.y & 0xFFFF, cur.mk.y >> 16,
+                              cur.mk.z & 0xFFFF, cur.mk.z >> 16, cur.mk.w & 0xFFFF, cur.mk.w >> 16};
+    uint32_t vm = 0, ig = 0;
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-      ikey[i] = BLK_EMPTY;
-      const uint32_t l = lab[i];
-      if (l != 0) {
-        if (l > n_det_f) {
-          acc_ignored++;
-        } else if (depth_valid(z[i], z_min, z_max)) {
-          const float xn = __fmul_rn(__fsub_rn(__fadd_rn(u0f, (float)i), c0.z), c0.x);
-          const float xc = __fmul_rn(xn, z[i]), yc = __fmul_rn(yn, z[i]);
-          float p[3];
-          p[0] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c1.x, xc), __fmul_rn(c1.y, yc)), __fmul_rn(c1.z, z[i])), c1.w);
-          p[1] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c2.x, xc), __fmul_rn(c2.y, yc)), __fmul_rn(c2.z, z[i])), c2.w);
-          p[2] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c3.x, xc), __fmul_rn(c3.y, yc)), __fmul_rn(c3.z, z[i])), c3.w);
-          uint32_t ix, iy, iz;
-          if (voxel_index(p, inv_vs, ix, iy, iz)) {
-            acc_valid++;
-            const unsigned long long bk = block_key(ix, iy, iz);
-            const uint32_t bit = block_bit(ix, iy, iz);
-            if (L0 == 0) L0 = l;
-            if (l == L0) {
-              valid |= 1u << i;
-              ikey[i] = bk;
-              if (i < 4) ibit_lo |= bit << (6 * i); else ibit_hi |= bit << (6 * (i - 4));
-              mn0 = fminf(mn0, p[0]), mn1 = fminf(mn1, p[1]), mn2 = fminf(mn2, p[2]);
-              mx0 = fmaxf(mx0, p[0]), mx1 = fmaxf(mx1, p[1]), mx2 = fmaxf(mx2, p[2]);
-              if (GAUSS) {
-                if (valid == (1u << i)) gc0 = p[0], gc1 = p[1], gc2 = p[2];  // first point of the thread
-                const float dx = p[0] - gc0, dy = p[1] - gc1, dz = p[2] - gc2;
-                g1x += dx, g1y += dy, g1z += dz;
-                gxx = fmaf(dx, dx, gxx), gxy = fmaf(dx, dy, gxy), gxz = fmaf(dx, dz, gxz);
-                gyy = fmaf(dy, dy, gyy), gyz = fmaf(dy, dz, gyz), gzz = fmaf(dz, dz, gzz);
-              }
-            } else {  // rare: the thread's 8 pixels straddle two detections -- this pixel goes in on its own
-              stray_pixel(s, lab_j, lab_cnt, lab_box, m.det_npx, m.det_box, m.surv_key, m.surv_bits, m.surv_j, m.surv_cap,
-                          m.counters, m.err, GAUSS ? m.det_gm : nullptr, (uint32_t)det_base + l - 1, bk, bit, p[0], p[1], p[2]);
-            }
-          } else {
-            acc_dropped++;
-          }
-        }
-      }
+      const bool lab_ok = lab8[i] - 1u < n_det_f;                    // 1 <= label <= n_det
+      const bool z_ok = z8[i] > z_min && z8[i] <= z_max;
+      vm |= (lab_ok && z_ok) ? 1u << i : 0u;
+      ig |= lab8[i] > n_det_f ? 1u << i : 0u;
     }
+    acc_ignored += __popc(ig);
+    LaneAcc<GAUSS> ac;
+    ac.j = NONE32, ac.cnt = 0, ac.li = -1, ac.klo = ac.khi = 0xFFFFFFFFu, ac.mlo = ac.mhi = 0;
+    ac.mn0 = INF, ac.mn1 = INF, ac.mn2 = INF, ac.mx0 = -INF, ac.mx1 = -INF, ac.mx2 = -INF;
+    ac.gc0 = ac.gc1 = ac.gc2 = ac.g1x = ac.g1y = ac.g1z = ac.gxx = ac.gxy = ac.gxz = ac.gyy = ac.gyz = ac.gzz = 0.f;
 
-    // ---- phase 2 (warp-synchronous): detection L0 of every thread
-    if (__any_sync(FULL, valid != 0)) {
-      const uint32_t j = (uint32_t)det_base + L0 - 1;
-      int li = -1;
-      if (valid) li = tile_label_slot_in(lab_j, j);
-      // per-detection pixel count and point AABB (R7): REDUX when the warp holds one detection
-      {
-        const unsigned has = __ballot_sync(FULL, valid != 0);
-        const int src = __ffs(has) - 1;
-        const uint32_t lead_L = __shfl_sync(FULL, L0, src);
-        const int lead_li = __shfl_sync(FULL, li, src);
-        const bool uniform = __all_sync(FULL, valid == 0 || L0 == lead_L);
-        const int o0 = f2ord(mn0), o1 = f2ord(mn1), o2 = f2ord(mn2), o3 = f2ord(mx0), o4 = f2ord(mx1), o5 = f2ord(mx2);
-        const uint32_t cnt = __popc(valid);
-        if (uniform) {
-          const uint32_t tot = __reduce_add_sync(FULL, cnt);
-          const int r0 = __reduce_min_sync(FULL, o0), r1 = __reduce_min_sync(FULL, o1), r2 = __reduce_min_sync(FULL, o2),
-                    r3 = __reduce_max_sync(FULL, o3), r4 = __reduce_max_sync(FULL, o4), r5 = __reduce_max_sync(FULL, o5);
-          if (lane == 0) label_add_in(lab_cnt, lab_box, m, lead_li, (uint32_t)det_base + lead_L - 1, tot, r0, r1, r2, r3, r4, r5);
-        } else if (valid) {
-          label_add_in(lab_cnt, lab_box, m, li, j, cnt, o0, o1, o2, o3, o4, o5);
+    if (__any_sync(FULL, vm != 0)) {
+#pragma unroll 1
+      for (int r = 0; r < 2; ++r) {
+        // ---- compaction of pixels 4r .. 4r+3 of every lane into dense slots: slot = pixels before it in (i, lane) order
+        const uint32_t m4 = (vm >> (4 * r)) & 0xFu;
+        const float zq[4] = {r ? z8[4] : z8[0], r ? z8[5] : z8[1], r ? z8[6] : z8[2], r ? z8[7] : z8[3]};
+        const uint32_t lq[4] = {r ? lab8[4] : lab8[0], r ? lab8[5] : lab8[1], r ? lab8[6] : lab8[2], r ? lab8[7] : lab8[3]};
+        const uint32_t meta0 = ((uint32_t)row << 8) | (uint32_t)(cg * 8 + 4 * r);
+        uint32_t n = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const bool on_i = (m4 >> i) & 1u;
+          const unsigned b = __ballot_sync(FULL, on_i);
+          if (on_i)
+            stage[n + __popc(b & lt_mask)] = ((unsigned long long)((lq[i] << 16) | (meta0 + i)) << 32) | __float_as_uint(zq[i]);
+          n += __popc(b);
         }
-      }
-      if (GAUSS) {  // G1: raw moments in double (parallel-axis shift from the thread's centre), one set of atomics per warp
-        const double n = (double)__popc(valid), c0 = gc0, c1 = gc1, c2 = gc2, sx = g1x, sy = g1y, sz = g1z;
-        double g[9] = {sx + n * c0, sy + n * c1, sz + n * c2,
-                       gxx + 2.0 * c0 * sx + n * c0 * c0, gxy + c0 * sy + c1 * sx + n * c0 * c1, gxz + c0 * sz + c2 * sx + n * c0 * c2,
-                       gyy + 2.0 * c1 * sy + n * c1 * c1, gyz + c1 * sz + c2 * sy + n * c1 * c2, gzz + 2.0 * c2 * sz + n * c2 * c2};
-        const unsigned has = __ballot_sync(FULL, valid != 0);
-        const uint32_t lead_L = __shfl_sync(FULL, L0, __ffs(has) - 1);
-        if (__all_sync(FULL, valid == 0 || L0 == lead_L)) {
-#pragma unroll
-          for (int k = 0; k < 9; ++k) {
-            if (!valid) g[k] = 0.0;
-#pragma unroll
-            for (int sft = 16; sft; sft >>= 1) g[k] += __shfl_xor_sync(FULL, g[k], sft);
-          }
-          if (lane < 9) {
-            double v = g[0];
-#pragma unroll
-            for (int k = 1; k < 9; ++k) v = lane == k ? g[k] : v;
-            atomicAdd(m.det_gm + (size_t)((uint32_t)det_base + lead_L - 1) * 9 + lane, v);
-          }
-        } else if (valid) {
-#pragma unroll
-          for (int k = 0; k < 9; ++k) atomicAdd(m.det_gm + (size_t)j * 9 + k, g[k]);
-        }
-      }
-      // blocks: one pass per distinct block among the thread's pixels
-      uint32_t rem = valid;
-      while (__any_sync(FULL, rem != 0)) {
-        unsigned long long kb = BLK_EMPTY;
-#pragma unroll
-        for (int i = 7; i >= 0; --i)
-          if ((rem >> i) & 1u) kb = ikey[i];
-        uint32_t lo = 0, hi = 0, hit = 0;
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-          if (((rem >> i) & 1u) && ikey[i] == kb) {
-            hit |= 1u << i;
-            const uint32_t bit = ((i < 4 ? ibit_lo >> (6 * i) : ibit_hi >> (6 * (i - 4)))) & 63u;
+        if (n == 0) continue;  // warp-uniform
+        __syncwarp();
+        // ---- dense pass: one pixel per lane
+#pragma unroll 1
+        for (uint32_t base = 0; base < n; base += 32) {
+          const uint32_t slot = base + lane;
+          const bool on = slot < n;
+          const unsigned long long sv = stage[on ? slot : 0];
+          const float z = __uint_as_float((uint32_t)sv);
+          const uint32_t meta = (uint32_t)(sv >> 32);
+          const uint32_t j = (uint32_t)det_base + (meta >> 16) - 1u;
+          // (float)u, (float)v exactly (integers below 2^23), then R5 in its fixed order
+          const float uf = __fsub_rn(__uint_as_float(u_magic + (meta & 0xFFu)), 8388608.0f);
+          const float vf = __fsub_rn(__uint_as_float(v_magic + ((meta >> 8) & 0xFFu)), 8388608.0f);
+          const float xn = __fmul_rn(__fsub_rn(uf, c0.z), c0.x), yn = __fmul_rn(__fsub_rn(vf, c0.w), c0.y);
+          const float xc = __fmul_rn(xn, z), yc = __fmul_rn(yn, z);
+          const float p0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c1.x, xc), __fmul_rn(c1.y, yc)), __fmul_rn(c1.z, z)), c1.w);
+          const float p1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c2.x, xc), __fmul_rn(c2.y, yc)), __fmul_rn(c2.z, z)), c2.w);
+          const float p2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c3.x, xc), __fmul_rn(c3.y, yc)), __fmul_rn(c3.z, z)), c3.w);
+          // R6: floor(fp32(X * inv_vs)) by a round-down add of 1.5 * 2^23 (exact for |x| < 2^22; the pre-test keeps
+          // |x| < 2e6 and rejects NaN / inf), biased by 2^20
+          const float fx = __fmul_rn(p0, inv_vs), fy = __fmul_rn(p1, inv_vs), fz = __fmul_rn(p2, inv_vs);
+          const bool finite = fabsf(fx) < 2.0e6f && fabsf(fy) < 2.0e6f && fabsf(fz) < 2.0e6f;
+          constexpr int UNBIAS = 0x4B400000 - KEY_BIAS;
+          const uint32_t ix = (uint32_t)(__float_as_int(__fadd_rd(fx, 12582912.0f)) - UNBIAS);
+          const uint32_t iy = (uint32_t)(__float_as_int(__fadd_rd(fy, 12582912.0f)) - UNBIAS);
+          const uint32_t iz = (uint32_t)(__float_as_int(__fadd_rd(fz, 12582912.0f)) - UNBIAS);
+          const bool ok = on && finite && ((ix | iy | iz) >> 21) == 0;
+          acc_dropped += (on && !ok) ? 1u : 0u;
+          acc_valid += ok ? 1u : 0u;
+          // block key halves (bx << 38 | by << 19 | bz with b = i >> 2) and the voxel's bit inside the block
+          const uint32_t bx = ix >> 2, by = iy >> 2, bz = iz >> 2;
+          const uint32_t klo = bz | (by << 19), khi = (by >> 13) | (bx << 6);
+          const uint32_t bit = ((ix & 3u) << 4) | ((iy & 3u) << 2) | (iz & 3u);
+          if (ok) {
+            if (klo != ac.klo || khi != ac.khi || j != ac.j) {  // the lane moves on to another block (or detection)
+              if (ac.mlo | ac.mhi) lane_flush_block<GAUSS>(m, s, ac);
+              ac.klo = klo, ac.khi = khi, ac.mlo = 0, ac.mhi = 0;
+              if (j != ac.j) {  // first pixel of the lane in this tile, or (rare) another detection
+                if (ac.cnt) lane_flush_own<GAUSS>(m, ac);
+                ac.j = j, ac.cnt = 0;
+                ac.li = tile_label_slot_in(lab_j, j);
+                ac.mn0 = INF, ac.mn1 = INF, ac.mn2 = INF, ac.mx0 = -INF, ac.mx1 = -INF, ac.mx2 = -INF;
+                if (GAUSS) {
+                  ac.gc0 = p0, ac.gc1 = p1, ac.gc2 = p2;
+                  ac.g1x = ac.g1y = ac.g1z = ac.gxx = ac.gxy = ac.gxz = ac.gyy = ac.gyz = ac.gzz = 0.f;
+                }
+              }
+            }
             const uint32_t one = 1u << (bit & 31);
-            lo |= (bit & 32) ? 0u : one;
-            hi |= (bit & 32) ? one : 0u;
+            ac.mlo |= (bit & 32) ? 0u : one, ac.mhi |= (bit & 32) ? one : 0u;
+            ac.cnt++;
+            ac.mn0 = fminf(ac.mn0, p0), ac.mn1 = fminf(ac.mn1, p1), ac.mn2 = fminf(ac.mn2, p2);
+            ac.mx0 = fmaxf(ac.mx0, p0), ac.mx1 = fmaxf(ac.mx1, p1), ac.mx2 = fmaxf(ac.mx2, p2);
+            if (GAUSS) {
+              const float dx = p0 - ac.gc0, dy = p1 - ac.gc1, dz = p2 - ac.gc2;
+              ac.g1x += dx, ac.g1y += dy, ac.g1z += dz;
+              ac.gxx = fmaf(dx, dx, ac.gxx), ac.gxy = fmaf(dx, dy, ac.gxy), ac.gxz = fmaf(dx, dz, ac.gxz);
+              ac.gyy = fmaf(dy, dy, ac.gyy), ac.gyz = fmaf(dy, dz, ac.gyz), ac.gzz = fmaf(dz, dz, ac.gzz);
+            }
           }
-        rem &= ~hit;
-        bool ovf = hit && li < 0;  // no label slot
-        const bool tab = hit && li >= 0;
-        const unsigned act = __ballot_sync(FULL, tab);
-        if (tab) {
-          const unsigned long long tag = kb | ((unsigned long long)li << LABEL_SHIFT);
-          const unsigned same = __match_any_sync(act, tag);
-          lo = __reduce_or_sync(same, lo), hi = __reduce_or_sync(same, hi);
-          if (lane == __ffs(same) - 1) ovf = !tile_block_add(s, li, kb, lo, hi);
         }
-        emit_overflow(m, ovf, kb, j, lo, hi);
+        __syncwarp();  // the staging area is rewritten by the next round
+      }
+      // ---- end of the patch: the lanes' last blocks, combined over the lanes that hold the same (detection, block)
+      {
+        const bool has = (ac.mlo | ac.mhi) != 0;
+        const bool tab = has && ac.li >= 0;
+        const unsigned long long bkey = ((unsigned long long)ac.khi << 32) | ac.klo;
+        const unsigned long long tag = tab ? (bkey | ((unsigned long long)ac.li << LABEL_SHIFT)) : BLK_EMPTY;
+        const unsigned same = __match_any_sync(FULL, tag);
+        const uint32_t lo = __reduce_or_sync(same, ac.mlo), hi = __reduce_or_sync(same, ac.mhi);
+        bool ovf = has && ac.li < 0;  // no label slot: the lane's record goes to the global queue on its own
+        if (tab && lane == __ffs(same) - 1) ovf = !tile_block_add(s, ac.li, bkey, lo, hi);
+        emit_overflow(m, ovf, bkey, ac.j, tab ? lo : ac.mlo, tab ? hi : ac.mhi);
+      }
+      // ---- the lanes' evidence per detection (R7): combined over the warp, one set of global atomics per detection
+      {
+        const uint32_t key = ac.cnt ? ac.j : NONE32;
+        const unsigned grp = __match_any_sync(FULL, key);
+        const uint32_t tot = __reduce_add_sync(grp, ac.cnt);
+        const int r0 = __reduce_min_sync(grp, f2ord(ac.mn0)), r1 = __reduce_min_sync(grp, f2ord(ac.mn1)),
+                  r2 = __reduce_min_sync(grp, f2ord(ac.mn2)), r3 = __reduce_max_sync(grp, f2ord(ac.mx0)),
+                  r4 = __reduce_max_sync(grp, f2ord(ac.mx1)), r5 = __reduce_max_sync(grp, f2ord(ac.mx2));
+        if (ac.cnt && lane == __ffs(grp) - 1) {
+          atomicAdd(&m.det_npx[key], tot);
+          atomicMin(&m.det_box[key * 6 + 0], r0), atomicMin(&m.det_box[key * 6 + 1], r1), atomicMin(&m.det_box[key * 6 + 2], r2);
+          atomicMax(&m.det_box[key * 6 + 3], r3), atomicMax(&m.det_box[key * 6 + 4], r4), atomicMax(&m.det_box[key * 6 + 5], r5);
+        }
+        if (GAUSS) {  // G1: raw moments in double, one set of atomics per warp when it holds one detection
+          double g[9];
+          lane_raw_moments<GAUSS>(ac, g);
+          const unsigned hasg = __ballot_sync(FULL, ac.cnt != 0);
+          if (hasg) {
+            const uint32_t lead_j = __shfl_sync(FULL, ac.j, __ffs(hasg) - 1);
+            if (__all_sync(FULL, ac.cnt == 0 || ac.j == lead_j)) {
+#pragma unroll
+              for (int k = 0; k < 9; ++k) {
+                if (!ac.cnt) g[k] = 0.0;
+#pragma unroll
+                for (int sft = 16; sft; sft >>= 1) g[k] += __shfl_xor_sync(FULL, g[k], sft);
+              }
+              if (lane < 9) {
+                double v = g[0];
+#pragma unroll
+                for (int k = 1; k < 9; ++k) v = lane == k ? g[k] : v;
+                atomicAdd(m.det_gm + (size_t)lead_j * 9 + lane, v);
+              }
+            } else if (ac.cnt) {
+#pragma unroll
+              for (int k = 0; k < 9; ++k) atomicAdd(m.det_gm + (size_t)ac.j * 9 + k, g[k]);
+            }
+          }
+        }
       }
     }
     __syncthreads();  // B2: the tile's table is complete; thread 0 has published the queue chunk
@@ -576,7 +584,7 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
         if (lane == 0 && b) base = atomicAdd(&s.q_count, (uint32_t)__popc(b));
         base = __shfl_sync(FULL, base, 0);
         if (has) {
-          uint32_t pos = cpos + base + __popc(b & ((1u << lane) - 1));
+          uint32_t pos = cpos + base + __popc(b & lt_mask);
           if (pos >= cend) pos = nbase + (pos - cend);
           survivor_store(m, pos, tag & ((1ull << LABEL_SHIFT) - 1), lab_j[(uint32_t)(tag >> LABEL_SHIFT)], s.mlo[e], s.mhi[e]);
           s.tag[e] = BLK_EMPTY;
@@ -584,17 +592,9 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
           s.mhi[e] = 0;
         }
       }
-      if (tid < MAX_LABELS && lab_j[tid] != NONE32) {
-        const uint32_t j = lab_j[tid];
-        atomicAdd(&m.det_npx[j], lab_cnt[tid]);
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-          atomicMin(&m.det_box[j * 6 + k], lab_box[tid][k]);
-          atomicMax(&m.det_box[j * 6 + 3 + k], lab_box[tid][3 + k]);
-        }
-      }
     }
     cur = nxt;
+    f = nf, ty = nty, tx = ntx;
   }
   // ---- end of the CTA's tiles: statistics, and empty records over the unused part of the reserved chunks
   acc_valid = __reduce_add_sync(FULL, acc_valid);

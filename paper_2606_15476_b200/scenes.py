@@ -456,6 +456,31 @@ class BoxScene:
         return [self.frame(k) for k in range(k0, k1)]
 
 
+# ---- parallel frame generation: the ray caster is single-threaded numpy and frames are independent by construction
+# (every frame draws from its own Philox stream).  spawn context: the parent may hold a CUDA context.
+_GEN_SCENE: dict = {}
+
+
+def _gen_one(args):
+    ci, k = args
+    if ci not in _GEN_SCENE:
+        _GEN_SCENE[ci] = BoxScene(get_config(ci))
+    return k, _GEN_SCENE[ci].frame(k)
+
+
+def generate_frames(cfg_index: int, ks, procs: Optional[int] = None) -> List[Frame]:
+    """[BoxScene(get_config(cfg_index)).frame(k) for k in ks], generated by a pool of worker processes."""
+    import multiprocessing as mp
+    import os
+    ks = list(ks)
+    procs = min(procs or max(1, (os.cpu_count() or 2) - 2), 14, max(len(ks), 1))
+    if procs <= 1 or len(ks) < 4:
+        return [_gen_one((cfg_index, k))[1] for k in ks]
+    with mp.get_context("spawn").Pool(procs) as pool:
+        out = dict(pool.imap_unordered(_gen_one, [(cfg_index, k) for k in ks], chunksize=max(1, len(ks) // (procs * 4))))
+    return [out[k] for k in ks]
+
+
 # --------------------------------------------------------------------------------------- config 4: stress
 class StressScene:
     """Config 4 (batched throughput stress): a pre-populated map of `n_objects` voxel blobs plus batches of
