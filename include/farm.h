@@ -79,9 +79,15 @@ extern "C" {
                                         The association rule is unchanged                                              */
 #define FARM_OPT_COVISIBILITY 15     /* 1: maintain the N x ceil(N/64) covisibility bitset of PAPER.md:354 (step 7): all pairs
                                         of distinct objects that received a detection in one call; default 0            */
+#define FARM_OPT_VIEWS 16            /* k in 0..8: keep up to k representative views per object (PAPER.md:63 item (iii),
+                                        PAPER.md:353 step 6 "High-quality view selection"); default 0 = off               */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
+#define FARM_OPTF_VIEW_COS 103       /* a viewing direction is new if its cosine with every kept direction is below this;
+                                        default cos(30 deg) = 0.8660254 (the paper's "fixed angular threshold" is unstated)  */
+#define FARM_OPTF_VIEW_CLOSER 104    /* or the view is kept if its distance is below this ratio x the closest kept view;
+                                        default 0.8 (the paper's "sufficiently closer" is unstated)                        */
 
 typedef struct farm_map farm_map; /* opaque; the library owns all map memory */
 
@@ -169,6 +175,20 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov);
  * *words = ceil(N/64); else rows is a HOST buffer [N, *words] of uint64; bit b of row a is set iff objects a != b both
  * received a detection in one integrate call.  Bits are never cleared.  Synchronises. */
 int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words);
+
+/* Retained views (needs FARM_OPT_VIEWS = k > 0; HOST buffers; synchronises).  PAPER.md:353: "A new viewpoint is retained
+ * for an entity only if its viewing direction differs from all existing retained viewpoints by more than a fixed
+ * angular threshold, or if it is sufficiently closer than the closest existing viewpoint."  Readings (V1-V2):
+ * direction = unit vector from the camera position to the centre of the detection's point box, all decisions in fp32;
+ * merged detections offer their view in index order; a full set replaces its farthest view (earliest on ties) if the
+ * new view is closer than that one, else the new view is dropped.  views: [N, k] records, counts: [N] (<= k). */
+typedef struct {
+  int32_t frame, det;       /* frame sequence number and detection index inside the frame      */
+  uint32_t n_px;            /* valid masked pixels of that detection                            */
+  float cam[3], dir[3];     /* camera position; unit viewing direction camera -> object         */
+  float dist;               /* distance camera -> centre of the detection's point box           */
+} farm_view;
+int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts);
 
 /* Export (HOST buffers) -- with farm_map_import the "scene state" persistence of PAPER.md:597 ("the memory is persisted
  * as a scene state") reduced to this path's fields.  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.

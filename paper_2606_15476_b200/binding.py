@@ -23,9 +23,11 @@ OPT_OVERLAP = 12
 OPT_MAX_BLOCKS = 13
 OPT_GAUSSIAN = 14
 OPT_COVISIBILITY = 15
+OPT_VIEWS = 16
 N_STAGES = 6
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "merge"]
-OPTF_Z_MIN, OPTF_Z_MAX = 101, 102
+OPTF_Z_MIN, OPTF_Z_MAX, OPTF_VIEW_COS, OPTF_VIEW_CLOSER = 101, 102, 103, 104
+VIEW_DTYPE = np.dtype([("frame", "<i4"), ("det", "<i4"), ("n_px", "<u4"), ("cam", "<f4", 3), ("dir", "<f4", 3), ("dist", "<f4")])
 KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
 
 OBJECT_DTYPE = np.dtype(
@@ -42,7 +44,7 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians", "farm_map_read_covisibility",
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
-           "farm_map_get_frame_seq", "farm_map_set_frame_seq",
+           "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -77,6 +79,7 @@ def load_library():
         lib.farm_map_last_gaussians.argtypes = [vp, vp, vp, vp]
         lib.farm_map_read_gaussians.argtypes = [vp, vp, vp, vp]
         lib.farm_map_read_covisibility.argtypes = [vp, vp, vp]
+        lib.farm_map_read_views.argtypes = [vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
         lib.farm_map_sync.argtypes = [vp, vp]
@@ -117,7 +120,8 @@ class FarmMap:
 
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
                  max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
-                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None):
+                 stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None,
+                 views=None, view_cos=None, view_closer=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._last_M = 0
@@ -129,13 +133,19 @@ class FarmMap:
         for key, v in ((OPT_MAX_OBJECTS, max_objects), (OPT_MAX_VOXELS, max_voxels), (OPT_MAX_BLOCKS, max_blocks),
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
-                       (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility)):
+                       (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility),
+                       (OPT_VIEWS, views)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:
             self.set_option_f(OPTF_Z_MIN, z_min)
         if z_max is not None:
             self.set_option_f(OPTF_Z_MAX, z_max)
+        if view_cos is not None:
+            self.set_option_f(OPTF_VIEW_COS, view_cos)
+        if view_closer is not None:
+            self.set_option_f(OPTF_VIEW_CLOSER, view_closer)
+        self.views_k = int(views or 0)
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -228,6 +238,15 @@ class FarmMap:
         w, mu, cov = np.zeros(N, np.float64), np.zeros((N, 3), np.float32), np.zeros((N, 6), np.float32)
         _check(load_library().farm_map_read_gaussians(self._h, _hp(w), _hp(mu), _hp(cov)))
         return w, mu, cov
+
+    def read_views(self):
+        """(views [N, k] VIEW_DTYPE, counts [N]) retained views per object (FARM_OPT_VIEWS = k)."""
+        n = C.c_int(0)
+        _check(load_library().farm_map_read(self._h, None, C.byref(n), None, None, None, None))
+        views = np.zeros((n.value, max(self.views_k, 1)), VIEW_DTYPE)
+        counts = np.zeros(n.value, np.int32)
+        _check(load_library().farm_map_read_views(self._h, _hp(views), _hp(counts)))
+        return views[:, :self.views_k], counts
 
     def read_covisibility(self):
         """uint64 [N, ceil(N/64)] covisibility bitset (FARM_OPT_COVISIBILITY)."""

@@ -37,7 +37,8 @@ struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
   long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
-  int sim_path = 0, gaussian = 0, covis = 0;
+  int sim_path = 0, gaussian = 0, covis = 0, views_k = 0;
+  float view_cos = 0.8660254f, view_closer = 0.8f;
   cudaStream_t stream = 0;
   bool finalised = false;
   DevMap dm{};
@@ -400,6 +401,11 @@ int finalise_impl(farm_map *m) {
     if ((size_t)d.covis_words * 8 > 96 * 1024) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_COVISIBILITY supports MAX_OBJECTS <= 786432");
     A(d.covis, NO * d.covis_words, 0);
   }
+  if (m->views_k > 0) {
+    d.views_k = m->views_k, d.view_cos = m->view_cos, d.view_closer = m->view_closer;
+    A(d.views, NO * (size_t)m->views_k, 0);
+    A(d.view_cnt, NO, 0);
+  }
   if (m->gaussian) {
     A(d.det_gm, MD * 9, 0);
     A(d.hell, MD, 0);
@@ -554,6 +560,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad COVISIBILITY");
       m->covis = (int)v;
       break;
+    case FARM_OPT_VIEWS:
+      if (v < 0 || v > 8) return fail(FARM_ERR_INVALID_ARG, "bad VIEWS (0..8)");
+      m->views_k = (int)v;
+      break;
     case FARM_OPT_TIMING:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
       m->timing = (int)v;
@@ -572,6 +582,10 @@ int farm_map_set_option_f(farm_map *m, int key, float v) {
     m->z_min = v;
   else if (key == FARM_OPTF_Z_MAX)
     m->z_max = v;
+  else if (key == FARM_OPTF_VIEW_COS)
+    m->view_cos = v;
+  else if (key == FARM_OPTF_VIEW_CLOSER)
+    m->view_closer = v;
   else
     return fail(FARM_ERR_INVALID_ARG, "unknown float option");
   return FARM_OK;
@@ -945,6 +959,19 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov) 
   uint32_t N = 0;
   CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
   return export_gaussians(m, m->dm.obj_gw, nullptr, m->dm.obj_gm, N, weight, mu, cov);
+}
+
+int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (m->views_k <= 0) return fail(FARM_ERR_STATE, "FARM_OPT_VIEWS is off");
+  if (!m->finalised) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  if (views && N) CU(cudaMemcpy(views, m->dm.views, (size_t)N * m->views_k * sizeof(farm_view), cudaMemcpyDeviceToHost));
+  if (counts && N) CU(cudaMemcpy(counts, m->dm.view_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost));
+  return FARM_OK;
 }
 
 int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words) {

@@ -51,6 +51,41 @@ __device__ __noinline__ void match_hellinger(const double *det_gm, const double 
   hell[j] = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)eps2);
 }
 
+// V1-V2: the view of one merged detection, offered to its object's retained set.  fp32, one rounded
+// operation at a time: the comparisons decide which views are kept and the oracle takes them in the same precision.
+__device__ __noinline__ void offer_view(const DevMap &m, int32_t t, const int *box, const float *cam, int32_t frame, int32_t det,
+                                        uint32_t n_px) {
+  float d[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) d[k] = __fsub_rn(__fmul_rn(0.5f, __fadd_rn(ord2f(box[k]), ord2f(box[3 + k]))), cam[k]);
+  const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(d[0], d[0]), __fmul_rn(d[1], d[1])), __fmul_rn(d[2], d[2]));
+  const float dist = __fsqrt_rn(d2);
+  if (!(dist > 0.f)) return;
+  farm_view v;
+  v.frame = frame, v.det = det, v.n_px = n_px, v.dist = dist;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) v.cam[k] = cam[k], v.dir[k] = __fdiv_rn(d[k], dist);
+  farm_view *set = m.views + (size_t)t * m.views_k;
+  const uint32_t n = m.view_cnt[t];
+  bool fresh = true;
+  float closest = __int_as_float(0x7F800000);
+  uint32_t far = 0;
+  for (uint32_t i = 0; i < n; ++i) {
+    const float dot = __fadd_rn(__fadd_rn(__fmul_rn(v.dir[0], set[i].dir[0]), __fmul_rn(v.dir[1], set[i].dir[1])), __fmul_rn(v.dir[2], set[i].dir[2]));
+    if (!(dot < m.view_cos)) fresh = false;
+    closest = fminf(closest, set[i].dist);
+    if (set[i].dist > set[far].dist) far = i;
+  }
+  const bool closer = n > 0 && dist < __fmul_rn(m.view_closer, closest);
+  if (n > 0 && !fresh && !closer) return;
+  if (n < (uint32_t)m.views_k) {
+    set[n] = v;
+    m.view_cnt[t] = n + 1;
+  } else if (dist < set[far].dist) {
+    set[far] = v;
+  }
+}
+
 // ---- candidate scoring + association, one launch.
 // Phase 1 (all CTAs): one warp per non-zero overlap entry (d, o, c): cos(a_d, shadow_o) by a gather dot, g (R10),
 //   score (R17), atomicMax into best_cand[d].
@@ -385,6 +420,11 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       // R23: most pixels wins, ties -> smallest (frame_seq, det): members come in ascending (frame, det) order and every
       // stored view is older than this call, so a strict > keeps the earliest
       if (npx > best) best = npx, best_frame = f, best_seq = frame_seq0 + f, best_det = jm - a.base[f];
+      if (m.views) {  // V: detections offer their view in index order
+        const float *Tf = a.T + 16 * f;
+        const float cam[3] = {Tf[3], Tf[7], Tf[11]};
+        offer_view(m, t, m.det_box + jm * 6, cam, (int32_t)(frame_seq0 + f), (int32_t)(jm - a.base[f]), npx);
+      }
     });
   }
   // f_o <- normalise(n_obs * f_o + sum_m a_m / |a_m|)   (R21).  Two passes over the rows (the second one hits

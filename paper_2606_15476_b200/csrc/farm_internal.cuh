@@ -123,6 +123,11 @@ struct DevMap {
   float eps2;                        // voxel_size^2, added to both covariance diagonals (reading G3)
   unsigned long long *covis;         // [max_objects, covis_words] covisibility bitset (rule C1); null when disabled
   uint32_t covis_words;
+  // V1-V2: up to views_k retained views per object; null when disabled
+  farm_view *views;                  // [max_objects, views_k]
+  uint32_t *view_cnt;                // [max_objects]
+  int views_k;
+  float view_cos, view_closer;
   uint32_t *sim_done;                // cumulative count of finished similarity CTAs (the association scan waits on it)
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel

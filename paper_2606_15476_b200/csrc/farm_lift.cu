@@ -189,7 +189,7 @@ __device__ __forceinline__ void survivor_store(const DevMap &m, uint32_t pos, un
 struct TileSmem {
   unsigned long long tag[TILE_ENT];       // block key | label slot << 57, BLK_EMPTY when free
   uint32_t mlo[TILE_ENT], mhi[TILE_ENT];  // voxel bits of the block seen for that detection inside the tile
-  unsigned long long stage[LIFT_WARPS][STAGE_PX];  // per warp, the compacted masked pixels of one round:
+  unsigned long long stage[LIFT_WARPS][STAGE_PX + 1];  // per warp, the compacted masked pixels of one round (+ a dump slot):
                                                    // (label << 16 | row in tile << 8 | column in tile) << 32 | depth bits
   uint32_t q_count;                       // entries flushed by the tile that just finished
   uint32_t cur_pos, cur_end;              // the CTA's current chunk of the survivor queue
@@ -217,7 +217,9 @@ __device__ __forceinline__ int tile_label_slot_in(uint32_t *lab_j, uint32_t j) {
 // global queue (the probe kernel's pair set keeps the result exact).
 __device__ __forceinline__ bool tile_block_add(TileSmem &s, int li, unsigned long long bkey, uint32_t lo, uint32_t hi) {
   const unsigned long long tag = bkey | ((unsigned long long)li << LABEL_SHIFT);
-  uint32_t h = hash32((uint32_t)tag, (uint32_t)(tag >> 32)) & (TILE_ENT - 1);
+  // multiplicative hash of the 64-bit tag, top bits (neighbouring blocks differ in the low bits of the key fields)
+  uint32_t h = (((uint32_t)tag * 0x9E3779B1u) ^ ((uint32_t)(tag >> 32) * 0x85EBCA77u)) >> (32 - 7);
+  static_assert(TILE_ENT == 128, "hash width");
   for (int probe = 0; probe < 16; ++probe) {  // a short probe sequence: a miss only costs one more queue record
     unsigned long long cur = *(volatile unsigned long long *)&s.tag[h];
     if (cur == BLK_EMPTY) {
@@ -422,35 +424,34 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
     const float z8[8] = {cur.d0.x, cur.d0.y, cur.d0.z, cur.d0.w, cur.d1.x, cur.d1.y, cur.d1.z, cur.d1.w};
     const uint32_t lab8[8] = {cur.mk.x & 0xFFFF, cur.mk.x >> 16, cur.mk.y & 0xFFFF, cur.mk.y >> 16,
                               cur.mk.z & 0xFFFF, cur.mk.z >> 16, cur.mk.w & 0xFFFF, cur.mk.w >> 16};
-    uint32_t vm = 0, ig = 0;
+    uint32_t vm = 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const bool lab_ok = lab8[i] - 1u < n_det_f;                    // 1 <= label <= n_det
-      const bool z_ok = z8[i] > z_min && z8[i] <= z_max;
-      vm |= (lab_ok && z_ok) ? 1u << i : 0u;
-      ig |= lab8[i] > n_det_f ? 1u << i : 0u;
+    for (int i = 0; i < 8; ++i)
+      if (lab8[i] - 1u < n_det_f && z8[i] > z_min && z8[i] <= z_max) vm |= 1u << i;   // 1 <= label <= n_det, depth valid
+    // labels without a descriptor row (R3: ignored, counted) are rare: look for them only where the packed words say so
+    const uint32_t lab_max2 = __vmaxu2(__vmaxu2(cur.mk.x, cur.mk.y), __vmaxu2(cur.mk.z, cur.mk.w));  // per 16-bit half
+    if (max(lab_max2 & 0xFFFFu, lab_max2 >> 16) > n_det_f) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) acc_ignored += lab8[i] > n_det_f ? 1u : 0u;
     }
-    acc_ignored += __popc(ig);
     LaneAcc<GAUSS> ac;
     ac.j = NONE32, ac.cnt = 0, ac.li = -1, ac.klo = ac.khi = 0xFFFFFFFFu, ac.mlo = ac.mhi = 0;
     ac.mn0 = INF, ac.mn1 = INF, ac.mn2 = INF, ac.mx0 = -INF, ac.mx1 = -INF, ac.mx2 = -INF;
     ac.gc0 = ac.gc1 = ac.gc2 = ac.g1x = ac.g1y = ac.g1z = ac.gxx = ac.gxy = ac.gxz = ac.gyy = ac.gyz = ac.gzz = 0.f;
 
     if (__any_sync(FULL, vm != 0)) {
-#pragma unroll 1
+#pragma unroll
       for (int r = 0; r < 2; ++r) {
         // ---- compaction of pixels 4r .. 4r+3 of every lane into dense slots: slot = pixels before it in (i, lane) order
-        const uint32_t m4 = (vm >> (4 * r)) & 0xFu;
-        const float zq[4] = {r ? z8[4] : z8[0], r ? z8[5] : z8[1], r ? z8[6] : z8[2], r ? z8[7] : z8[3]};
-        const uint32_t lq[4] = {r ? lab8[4] : lab8[0], r ? lab8[5] : lab8[1], r ? lab8[6] : lab8[2], r ? lab8[7] : lab8[3]};
+        // (invalid pixels are written to the dump slot: no divergent branch)
         const uint32_t meta0 = ((uint32_t)row << 8) | (uint32_t)(cg * 8 + 4 * r);
         uint32_t n = 0;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const bool on_i = (m4 >> i) & 1u;
+          const bool on_i = (vm >> (4 * r + i)) & 1u;
           const unsigned b = __ballot_sync(FULL, on_i);
-          if (on_i)
-            stage[n + __popc(b & lt_mask)] = ((unsigned long long)((lq[i] << 16) | (meta0 + i)) << 32) | __float_as_uint(zq[i]);
+          const uint2 val = make_uint2(__float_as_uint(z8[4 * r + i]), (lab8[4 * r + i] << 16) | (meta0 + i));
+          *reinterpret_cast<uint2 *>(&stage[on_i ? n + __popc(b & lt_mask) : STAGE_PX]) = val;
           n += __popc(b);
         }
         if (n == 0) continue;  // warp-uniform
@@ -460,9 +461,9 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
         for (uint32_t base = 0; base < n; base += 32) {
           const uint32_t slot = base + lane;
           const bool on = slot < n;
-          const unsigned long long sv = stage[on ? slot : 0];
-          const float z = __uint_as_float((uint32_t)sv);
-          const uint32_t meta = (uint32_t)(sv >> 32);
+          const uint2 sv = *reinterpret_cast<const uint2 *>(&stage[on ? slot : 0]);
+          const float z = __uint_as_float(sv.x);
+          const uint32_t meta = sv.y;
           const uint32_t j = (uint32_t)det_base + (meta >> 16) - 1u;
           // (float)u, (float)v exactly (integers below 2^23), then R5 in its fixed order
           const float uf = __fsub_rn(__uint_as_float(u_magic + (meta & 0xFFu)), 8388608.0f);

@@ -223,3 +223,35 @@ def test_launch_blocking_environment_selects_the_single_stream_order(oracle, mon
         gpu_integrate(g, frames, cfg.dtype)
         compare_call(g, o)
     compare_maps(g, o)
+
+
+def _compare_views(g, o):
+    vo, co = o.read_views()
+    vg, cg = g.read_views()
+    assert np.array_equal(cg, co)
+    for i in range(len(co)):
+        k = int(co[i])
+        for fld in ("frame", "det", "n_px"):
+            assert np.array_equal(vg[i][fld][:k], vo[i][fld][:k]), (i, fld)
+        for fld in ("cam", "dir", "dist"):
+            assert np.array_equal(vg[i][fld][:k], vo[i][fld][:k]), (i, fld)      # fp32 on both sides, same operation order
+    return int(co.sum())
+
+
+@pytest.mark.parametrize("cfg_id,n,per_call,k", [(0, 20, 1, 3), (0, 18, 3, 2), (1, 40, 1, 4)])
+def test_view_diversity_sets_match_oracle(oracle, cfg_id, n, per_call, k):
+    """V1-V2 (PAPER.md:353 step 6, "up to k representative views"): which views every object keeps, and their
+    records, bit-exact -- single-frame and batched calls, set sizes 2..4 so that replacement of the farthest view occurs."""
+    cfg = S.get_config(cfg_id)
+    frames_all = generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n))
+    o, g = make_pair(oracle, cfg, views=k)
+    o.set_option(o.OPT_VIEWS_K, k)
+    for c in range(0, n, per_call):
+        frames = margin_filter(o.clone, frames_all[c:c + per_call], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o, check_sets=False)
+        total = _compare_views(g, o)
+    compare_maps(g, o, voxels=False)
+    _, counts = o.read_views()
+    assert total > len(counts) and counts.max() == k           # some objects hold several views, some sets are full
