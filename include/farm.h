@@ -190,6 +190,31 @@ typedef struct {
 } farm_view;
 int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts);
 
+/* Retrieval-side scoring over the finished memory (a second workload beside the mapper, rules Q1-Q5 of
+ * DESIGN.md).  The three per-entity retrieval embedding matrices of PAPER.md:356 (caption text, image, image-VL), the
+ * class ids and the query vectors are INPUTS; parser, encoders and the VLM reranker are out of scope.
+ *   emb0/1/2  DEVICE [N, d0/d1/d2] in emb_dtype (FARM_DTYPE_*), N = current number of objects; cls DEVICE [N] or NULL
+ *   q_target  HOST fp32 [2*d0 + d1 + d2]: the four query channels of the target -- description in space 0 (w = 1.0),
+ *             raw utterance in space 0 (w = 0.5), prompt-ensemble mean in space 1 (w = 0.75), description in space 2
+ *             (w = 1.0) ("each channel contributes w/(mu+rank) with offset mu = 5")
+ *   n_pred predicates, pred_type HOST [n_pred] in FARM_PRED_*, each with its own landmark variable q_landmarks HOST
+ *             [n_pred, 2*d0 + d1 + d2]; the landmark is bound to its top-scoring live entity
+ *   Near / NextTo: exp(-d^2 / (2 sigma^2)) of the inter-centroid distance, sigma = 0.5 m / 1.0 m; Closest / Farthest:
+ *             1 / (|rank - r*| + 1), rank by that distance among the live entities; centroid = Gaussian mean where the
+ *             entity has one (FARM_OPT_GAUSSIAN), else the centre of its AABB
+ *   s = s_sem * (0.5 + 0.5 * gbar), gbar = geometric mean of the predicate scores, s_sem * 0.3 on a class mismatch
+ *             (target_class < 0: no class factor)
+ * Outputs (HOST, any may be NULL): top_ids / top_scores [topk] by s (ties -> lower id, -1 past the live entities),
+ * landmarks [n_pred], s_sem / gbar / s [N] (0 for entities without observations).  Synchronises. */
+#define FARM_PRED_NEAR 0
+#define FARM_PRED_NEXTTO 1
+#define FARM_PRED_CLOSEST 2
+#define FARM_PRED_FARTHEST 3
+int farm_map_query(farm_map *m, const void *emb0, const void *emb1, const void *emb2, int d0, int d1, int d2, int emb_dtype,
+                   const int32_t *cls, const float *q_target, int target_class, int n_pred, const int32_t *pred_type,
+                   const float *q_landmarks, int topk, int32_t *top_ids, float *top_scores, int32_t *landmarks, float *s_sem,
+                   float *gbar, float *s);
+
 /* Export (HOST buffers) -- with farm_map_import the "scene state" persistence of PAPER.md:597 ("the memory is persisted
  * as a scene state") reduced to this path's fields.  Two-call pattern: with objects == NULL only *n_objects / *n_voxels are written.
  * descriptors: [N, D] fp32 masters (may be NULL).  voxel_keys / voxel_owner: [n_voxels] pairs in arbitrary

@@ -44,7 +44,7 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians", "farm_map_read_covisibility",
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
-           "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views",
+           "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views", "farm_map_query",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -80,6 +80,7 @@ def load_library():
         lib.farm_map_read_gaussians.argtypes = [vp, vp, vp, vp]
         lib.farm_map_read_covisibility.argtypes = [vp, vp, vp]
         lib.farm_map_read_views.argtypes = [vp, vp, vp]
+        lib.farm_map_query.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, ci, ci, vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
         lib.farm_map_sync.argtypes = [vp, vp]
@@ -238,6 +239,26 @@ class FarmMap:
         w, mu, cov = np.zeros(N, np.float64), np.zeros((N, 3), np.float32), np.zeros((N, 6), np.float32)
         _check(load_library().farm_map_read_gaussians(self._h, _hp(w), _hp(mu), _hp(cov)))
         return w, mu, cov
+
+    def query(self, emb, emb_dtype, cls, q_target, target_class, pred_types, q_landmarks, topk):
+        """farm_map_query.  emb: three CUDA tensors [N, d_s]; cls: CUDA int32 tensor [N] or None; q_target: four host
+        vectors (d0, d0, d1, d2); q_landmarks: one such list of four per predicate.  Returns dict(top, top_scores,
+        landmarks, s_sem, gbar, s)."""
+        n = C.c_int(0)
+        _check(load_library().farm_map_read(self._h, None, C.byref(n), None, None, None, None))
+        N, P = n.value, len(pred_types)
+        dims = [int(e.shape[1]) for e in emb]
+        qt = np.ascontiguousarray(np.concatenate([np.asarray(x, np.float32).ravel() for x in q_target]), np.float32)
+        ql = np.ascontiguousarray(np.concatenate([np.asarray(x, np.float32).ravel() for lm in q_landmarks for x in lm])
+                                  if P else np.zeros(1), np.float32)
+        pt = np.ascontiguousarray(pred_types if P else [0], np.int32)
+        top, tsc = np.full(topk, -1, np.int32), np.zeros(topk, np.float32)
+        lms = np.full(max(P, 1), -1, np.int32)
+        s_sem, gbar, s = np.zeros(N, np.float32), np.zeros(N, np.float32), np.zeros(N, np.float32)
+        _check(load_library().farm_map_query(self._h, _dp(emb[0]), _dp(emb[1]), _dp(emb[2]), dims[0], dims[1], dims[2],
+                                             int(emb_dtype), _dp(cls), _hp(qt), int(target_class), P, _hp(pt), _hp(ql), int(topk),
+                                             _hp(top), _hp(tsc), _hp(lms), _hp(s_sem), _hp(gbar), _hp(s)))
+        return {"top": top, "top_scores": tsc, "landmarks": lms[:P], "s_sem": s_sem, "gbar": gbar, "s": s}
 
     def read_views(self):
         """(views [N, k] VIEW_DTYPE, counts [N]) retained views per object (FARM_OPT_VIEWS = k)."""

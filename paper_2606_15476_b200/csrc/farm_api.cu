@@ -14,6 +14,10 @@
 namespace farm {
 int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target,
                          int *n_ctas);
+int run_query(const DevMap &m, cudaStream_t st, uint32_t N, const void *const emb[3], const int dim[3], int emb_dtype, const int32_t *cls,
+              const float *q_target, int target_class, int P, const int32_t *pred_type, const float *q_landmarks, int topk,
+              int32_t *top_ids, float *top_scores, int32_t *landmarks, float *s_sem, float *gbar, float *s, long long *launches,
+              std::string *err);
 bool tc_prepare(void *tc_state, const DevMap &m, const CallArgs &a);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
@@ -959,6 +963,31 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov) 
   uint32_t N = 0;
   CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
   return export_gaussians(m, m->dm.obj_gw, nullptr, m->dm.obj_gm, N, weight, mu, cov);
+}
+
+int farm_map_query(farm_map *m, const void *emb0, const void *emb1, const void *emb2, int d0, int d1, int d2, int emb_dtype,
+                   const int32_t *cls, const float *q_target, int target_class, int n_pred, const int32_t *pred_type,
+                   const float *q_landmarks, int topk, int32_t *top_ids, float *top_scores, int32_t *landmarks, float *s_sem,
+                   float *gbar, float *s) {
+  if (!m || !emb0 || !emb1 || !emb2 || !q_target) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (d0 < 1 || d1 < 1 || d2 < 1 || d0 > 8192 || d1 > 8192 || d2 > 8192) return fail(FARM_ERR_INVALID_ARG, "embedding sizes must be in 1..8192");
+  if (emb_dtype < 0 || emb_dtype > 2) return fail(FARM_ERR_INVALID_ARG, "bad emb_dtype");
+  if (n_pred < 0 || n_pred > 3 || (n_pred && (!pred_type || !q_landmarks))) return fail(FARM_ERR_INVALID_ARG, "n_pred must be in 0..3");
+  for (int p = 0; p < n_pred; ++p)
+    if (pred_type[p] < 0 || pred_type[p] > 3) return fail(FARM_ERR_INVALID_ARG, "unknown predicate type");
+  if (topk < 0 || topk > 4096) return fail(FARM_ERR_INVALID_ARG, "topk must be in 0..4096");
+  int rc = finalise(m);
+  if (rc != FARM_OK) return rc;
+  rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  const void *const emb[3] = {emb0, emb1, emb2};
+  const int dim[3] = {d0, d1, d2};
+  std::string err;
+  rc = run_query(m->dm, m->stream, N, emb, dim, emb_dtype, cls, q_target, target_class, n_pred, pred_type, q_landmarks, topk, top_ids,
+                 top_scores, landmarks, s_sem, gbar, s, &m->launches, &err);
+  return rc == FARM_OK ? FARM_OK : fail(rc, err);
 }
 
 int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts) {

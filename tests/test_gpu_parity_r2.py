@@ -238,14 +238,16 @@ def _compare_views(g, o):
     return int(co.sum())
 
 
-@pytest.mark.parametrize("cfg_id,n,per_call,k", [(0, 20, 1, 3), (0, 18, 3, 2), (1, 40, 1, 4)])
-def test_view_diversity_sets_match_oracle(oracle, cfg_id, n, per_call, k):
+@pytest.mark.parametrize("cfg_id,n,per_call,k,vcos", [(0, 20, 1, 3, None), (0, 18, 3, 2, None), (1, 40, 1, 2, 0.97)])
+def test_view_diversity_sets_match_oracle(oracle, cfg_id, n, per_call, k, vcos):
     """V1-V2 (PAPER.md:353 step 6, "up to k representative views"): which views every object keeps, and their
     records, bit-exact -- single-frame and batched calls, set sizes 2..4 so that replacement of the farthest view occurs."""
     cfg = S.get_config(cfg_id)
     frames_all = generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n))
-    o, g = make_pair(oracle, cfg, views=k)
+    o, g = make_pair(oracle, cfg, views=k, view_cos=vcos)
     o.set_option(o.OPT_VIEWS_K, k)
+    if vcos is not None:
+        o.set_option(o.OPT_VIEW_COS, vcos)
     for c in range(0, n, per_call):
         frames = margin_filter(o.clone, frames_all[c:c + per_call], cfg.tau)
         integrate_frames(o, frames)
@@ -255,3 +257,109 @@ def test_view_diversity_sets_match_oracle(oracle, cfg_id, n, per_call, k):
     compare_maps(g, o, voxels=False)
     _, counts = o.read_views()
     assert total > len(counts) and counts.max() == k           # some objects hold several views, some sets are full
+
+
+# ------------------------------------------------------------------------------------------------ retrieval scoring (Q1-Q5)
+def _ternary_rows(n, d, nnz, rng):
+    """rows with exactly nnz entries of +-1: all norms equal and every dot product is an exact small integer, so the
+    cosine ORDER (hence every rank) is the same in any accumulation order and precision"""
+    out = np.zeros((n, d), np.float32)
+    for i in range(n):
+        idx = rng.choice(d, nnz, replace=False)
+        out[i, idx] = rng.choice([-1.0, 1.0], nnz)
+    return out
+
+
+def _query_scene(oracle, gaussian):
+    """mini stress scene, imported with random object boxes, one batch integrated (new objects carry Gaussians)"""
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    sc = S.StressScene(n_batches=1, frames_per_batch=4, n_objects=700)
+    cfg = sc.cfg
+    ijk, owner, n_vox, desc = sc.build_map()
+    keys = pack_key(ijk[:, 0], ijk[:, 1], ijk[:, 2])
+    rng = np.random.default_rng(5)
+    objs = np.zeros(len(n_vox), OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(len(n_vox)), n_vox, 1, -1, -1
+    c = rng.uniform(-4, 4, (len(n_vox), 3)).astype(np.float32)
+    objs["aabb_min"], objs["aabb_max"] = c - 0.25, c + 0.25
+    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, gaussian=gaussian)
+    assert o.import_(objs, desc, keys, owner) == 0
+    g.import_(objs, desc, keys, owner)
+    frames = margin_filter(o.clone, sc.batch(0), cfg.tau)
+    integrate_frames(o, frames)
+    gpu_integrate(g, frames, cfg.dtype)
+    compare_call(g, o, check_sets=False)
+    objs_o, _, _, _ = o.read(voxels=False)
+    alive = (objs_o["n_obs"] > 0).astype(np.uint8)
+    cen = (0.5 * (objs_o["aabb_min"].astype(np.float64) + objs_o["aabb_max"].astype(np.float64))).astype(np.float32)
+    if gaussian:
+        w, mu, _ = o.read_gaussians()
+        cen[w > 0] = mu[w > 0]
+    return o, g, alive, cen
+
+
+@pytest.mark.parametrize("emb_dtype,gaussian", [(0, 1), (2, 0)])
+def test_retrieval_scoring_exact_ranks(oracle, emb_dtype, gaussian):
+    """Q1-Q5 against the oracle on ~1,100 entities: reciprocal-rank fusion over four channels in three
+    embedding spaces, landmark binding, Near / NextTo / Closest / Farthest, composite score, class factor, top-K.
+    Embeddings are +-1/0 rows of equal norm, so every rank is decided by exact integer dot products on both sides."""
+    import torch
+    o, g, alive, cen = _query_scene(oracle, gaussian)
+    N = len(alive)
+    rng = np.random.default_rng(23)
+    dims, nnz = (64, 48, 96), (24, 16, 32)
+    emb = [_ternary_rows(N, d, z, rng) for d, z in zip(dims, nnz)]
+    cls = rng.integers(0, 5, N).astype(np.int32)
+    tdt = {0: torch.float32, 1: torch.float16, 2: torch.bfloat16}[emb_dtype]
+    emb_dev = [torch.from_numpy(e).to("cuda").to(tdt).contiguous() for e in emb]
+    cls_dev = torch.from_numpy(cls).to("cuda")
+    qv = lambda sp: _ternary_rows(1, dims[sp], nnz[sp], rng)[0]
+    qt = [qv(0), qv(0), qv(1), qv(2)]
+    lm_ids = [int(rng.integers(0, N)), int(rng.integers(0, N)), int(rng.integers(0, N))]
+    # each landmark variable asks for one particular entity: its own embeddings, rank 1 in every channel
+    qls = [[emb[0][i], emb[0][i], emb[1][i], emb[2][i]] for i in lm_ids]
+    cases = [([], [], -1), ([oracle.PRED_NEAR], qls[:1], 3), ([oracle.PRED_NEXTTO, oracle.PRED_CLOSEST], qls[:2], -1),
+             ([oracle.PRED_FARTHEST, oracle.PRED_NEAR, oracle.PRED_CLOSEST], qls, 1)]
+    for ptypes, ql, tcls in cases:
+        ro = oracle.query(alive, emb, cls, cen, qt, tcls, ptypes, ql, 20)
+        rg = g.query(emb_dev, emb_dtype, cls_dev, qt, tcls, ptypes, ql, 20)
+        assert np.array_equal(rg["landmarks"], ro["landmarks"])
+        assert np.abs(rg["s_sem"] - ro["s_sem"]).max() <= 1e-6
+        assert np.abs(rg["gbar"] - ro["gbar"]).max() <= 1e-5
+        assert np.abs(rg["s"] - ro["s"]).max() <= 1e-6
+        so = np.sort(ro["s"])[::-1]
+        k_ok = 20
+        for k in range(20):                                        # compare the prefix whose scores are clearly separated
+            if so[k] - so[k + 1] <= 1e-6:
+                k_ok = k
+                break
+        assert np.array_equal(rg["top"][:k_ok], ro["top"][:k_ok]) and k_ok >= 3
+        assert np.abs(rg["top_scores"][:k_ok] - ro["s"][ro["top"][:k_ok]]).max() <= 1e-6
+    assert list(ro["landmarks"]) == [min(np.nonzero((emb[0] == emb[0][i]).all(1))[0]) for i in lm_ids]
+
+
+def test_retrieval_scoring_float_embeddings_robust_entities(oracle):
+    """random unit float embeddings (bf16): cosines within 1e-3 of the oracle's; s_sem equal for every entity whose cosine is
+    separated from both of its rank neighbours by more than 1e-5 in every channel (a swap of two near-tied entities
+    changes only those two)."""
+    import torch
+    o, g, alive, cen = _query_scene(oracle, 0)
+    N = len(alive)
+    dims = (128, 64, 256)
+    emb = [S.bf16_bits_to_f32(S.f32_to_bf16_bits(unit_rows(N, d, 70 + i))) for i, d in enumerate(dims)]
+    emb_dev = [torch.from_numpy(e).to("cuda").to(torch.bfloat16).contiguous() for e in emb]
+    qt = [unit_rows(1, dims[0], 80)[0], unit_rows(1, dims[0], 81)[0], unit_rows(1, dims[1], 82)[0], unit_rows(1, dims[2], 83)[0]]
+    ro = oracle.query(alive, emb, np.zeros(N, np.int32), cen, qt, -1, [], [], 10, want_cos=True)
+    rg = g.query(emb_dev, 2, None, qt, -1, [], [], 10)
+    robust = np.ones(N, bool)
+    for ch in range(4):
+        c = ro["cos"][ch].astype(np.float64)
+        order = np.argsort(-c, kind="stable")
+        gap = np.full(N, np.inf)
+        d = np.abs(np.diff(c[order]))
+        gap[order[1:]] = np.minimum(gap[order[1:]], d)
+        gap[order[:-1]] = np.minimum(gap[order[:-1]], d)
+        robust &= gap > 1e-5
+    assert robust.sum() > 0.5 * N
+    assert np.abs(rg["s_sem"] - ro["s_sem"])[robust].max() <= 1e-6
+    assert np.abs(rg["s_sem"] - ro["s_sem"]).max() <= 0.02
