@@ -81,11 +81,22 @@ extern "C" {
                                         of distinct objects that received a detection in one call; default 0            */
 #define FARM_OPT_VIEWS 16            /* k in 0..8: keep up to k representative views per object (PAPER.md:63 item (iii),
                                         PAPER.md:353 step 6 "High-quality view selection"); default 0 = off               */
+#define FARM_OPT_CORRESPONDENCE 17    /* 1: correspondence by union-find over the sparse match graph with entity-entity merges
+                                        (steps 3-5; rules U1-U4 of DESIGN.md): every entity whose score
+                                        exceeds tau is retained, a detection retaining two or more entities bridges them, the
+                                        lowest id wins, same-call duplicate spawns are joined.  Needs tau >= 0.  Default 0 */
+#define FARM_OPT_GEOMETRY 18          /* 0 (default): voxel overlap (BASELINE.json rule);  1: the paper's geometry -- similarity
+                                        prefilter, then g = 1 - Hellinger distance between the detection's and the entity's
+                                        Gaussian (rules H1-H3).  Needs FARM_OPT_GAUSSIAN = 1            */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
 #define FARM_OPTF_VIEW_COS 103       /* a viewing direction is new if its cosine with every kept direction is below this;
                                         default cos(30 deg) = 0.8660254 (the paper's "fixed angular threshold" is unstated)  */
+#define FARM_OPTF_PREFILTER_COS 105   /* H1: candidates are the entities with cosine > this; default 0.5 (the paper's
+                                        "sufficiently similar" is unstated)                                              */
+#define FARM_OPTF_HELLINGER_BUDGET 106 /* H2: candidates with H > this are dropped; default 1 (no gate; the paper's "fixed
+                                        Hellinger budget" is unstated)                                                   */
 #define FARM_OPTF_VIEW_CLOSER 104    /* or the view is kept if its distance is below this ratio x the closest kept view;
                                         default 0.8 (the paper's "sufficiently closer" is unstated)                        */
 
@@ -175,6 +186,13 @@ int farm_map_read_gaussians(farm_map *m, double *weight, float *mu, float *cov);
  * *words = ceil(N/64); else rows is a HOST buffer [N, *words] of uint64; bit b of row a is set iff objects a != b both
  * received a detection in one integrate call.  Bits are never cleared.  Synchronises. */
 int farm_map_read_covisibility(farm_map *m, uint64_t *rows, int *words);
+
+/* Identity history of the entity merges (needs FARM_OPT_CORRESPONDENCE; HOST buffers; synchronises).  alias [N]: the live
+ * entity every id stands for now (itself while alive); an absorbed entity keeps its id as a dead record (no observations,
+ * no voxels, zero descriptor).  farm_map_last_merges: the (loser, winner) pairs of the LAST integrate call, arbitrary
+ * order; pass loser == NULL to get only *n. */
+int farm_map_read_alias(farm_map *m, int32_t *alias);
+int farm_map_last_merges(farm_map *m, int32_t *loser, int32_t *winner, int *n);
 
 /* Retained views (needs FARM_OPT_VIEWS = k > 0; HOST buffers; synchronises).  PAPER.md:353: "A new viewpoint is retained
  * for an entity only if its viewing direction differs from all existing retained viewpoints by more than a fixed

@@ -139,6 +139,7 @@ struct Map {
   std::vector<int32_t> assoc;
   std::vector<uint8_t> is_new;
   std::vector<float> best_score, second_score;
+  std::vector<float> tau_gap;                        // min over all scored pairs of |score - tau| (tests: margin filter)
   std::vector<float> dense_max, dense_second;        // R16: max_o clamp(cos(a_d, shadow_o)) over ALL entry objects; runner-up
   std::vector<int32_t> dense_arg;                    //      and its argmax (lowest id on ties), -1 if N = 0 / skipped
   std::vector<std::set<uint64_t>> V;                 // R7
@@ -405,6 +406,7 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
   m.is_new.assign(M, 0);
   m.best_score.assign(M, 0.0f);
   m.second_score.assign(M, -std::numeric_limits<float>::infinity());
+  m.tau_gap.assign(M, std::numeric_limits<float>::infinity());
   m.dense_max.assign(M, 0.0f);
   m.dense_second.assign(M, -std::numeric_limits<float>::infinity());
   m.dense_arg.assign(M, -1);
@@ -513,6 +515,7 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
         }
       }
       const float score = m.w_geo * g + m.w_sem * c;             // R17 (fp32: two mul, one add)
+      m.tau_gap[j] = std::fmin(m.tau_gap[j], std::fabs(score - m.tau));
       if (m.opt_corr && score > m.tau) retained[j].push_back(o); // U1
       if (best_o < 0 || score > best) {                          // R18: ties -> lowest id
         if (best_o >= 0) second = std::fmax(second, best);
@@ -582,6 +585,7 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
         const float g = mn ? (float)kv.second / (float)mn : 0.0f;
         for (int i = 0; i < D; ++i) b[i] = load_storage(desc, m.dtype, (size_t)e * D + i);
         const float score = m.w_geo * g + m.w_sem * cosine(a.data(), b.data(), D);
+        m.tau_gap[j] = std::fmin(m.tau_gap[j], std::fabs(score - m.tau));
         if (score > m.tau) uf_union(parent, N + j, N + e);
       }
     }
@@ -923,6 +927,11 @@ void oracle_read_covis(void *h, uint64_t *rows) {
   const size_t N = m.objs.size(), words = (N + 63) / 64;
   for (size_t a = 0; a < N; ++a)
     for (size_t w = 0; w < words; ++w) rows[a * words + w] = a < m.covis.size() && w < m.covis[a].size() ? m.covis[a][w] : 0;
+}
+// tests only: per detection the smallest |score - tau| over every pair that was scored (entities, and detection pairs of U2)
+void oracle_last_tau_gap(void *h, float *gap) {
+  Map &m = *(Map *)h;
+  for (int j = 0; j < m.M; ++j) gap[j] = m.tau_gap[j];
 }
 // U4: alias[o] = o for a live entity, else the live entity that (transitively) absorbed it
 void oracle_read_alias(void *h, int32_t *alias) {

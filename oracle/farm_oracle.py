@@ -71,6 +71,13 @@ class OracleMap:
         if key == self.OPT_VIEWS_K:
             self.views_k = int(value)
 
+    def last_tau_gap(self):
+        """per detection the smallest |score - tau| over every scored pair (tests: margin filter with correspondence)"""
+        M = lib().oracle_last_M(self.h)
+        gap = np.zeros(M, np.float32)
+        lib().oracle_last_tau_gap(self.h, _p(gap))
+        return gap
+
     def read_alias(self):
         """U4: alias [N]: the live entity every id now stands for (itself while alive)."""
         N = lib().oracle_n_objects(self.h)

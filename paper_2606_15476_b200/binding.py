@@ -24,9 +24,11 @@ OPT_MAX_BLOCKS = 13
 OPT_GAUSSIAN = 14
 OPT_COVISIBILITY = 15
 OPT_VIEWS = 16
+OPT_CORRESPONDENCE = 17
+OPT_GEOMETRY = 18
 N_STAGES = 6
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "merge"]
-OPTF_Z_MIN, OPTF_Z_MAX, OPTF_VIEW_COS, OPTF_VIEW_CLOSER = 101, 102, 103, 104
+OPTF_Z_MIN, OPTF_Z_MAX, OPTF_VIEW_COS, OPTF_VIEW_CLOSER, OPTF_PREFILTER_COS, OPTF_HELLINGER_BUDGET = 101, 102, 103, 104, 105, 106
 VIEW_DTYPE = np.dtype([("frame", "<i4"), ("det", "<i4"), ("n_px", "<u4"), ("cam", "<f4", 3), ("dir", "<f4", 3), ("dist", "<f4")])
 KEY_EMPTY = 0xFFFFFFFFFFFFFFFF
 
@@ -44,7 +46,8 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_integrate", "farm_map_integrate_batch", "farm_map_integrate_batch_host", "farm_map_stage_times", "farm_map_last_assoc", "farm_map_last_assoc_async", "farm_map_last_gaussians", "farm_map_read_gaussians", "farm_map_read_covisibility",
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
-           "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views", "farm_map_query",
+           "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views", "farm_map_query", "farm_map_read_alias",
+           "farm_map_last_merges",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -80,6 +83,8 @@ def load_library():
         lib.farm_map_read_gaussians.argtypes = [vp, vp, vp, vp]
         lib.farm_map_read_covisibility.argtypes = [vp, vp, vp]
         lib.farm_map_read_views.argtypes = [vp, vp, vp]
+        lib.farm_map_read_alias.argtypes = [vp, vp]
+        lib.farm_map_last_merges.argtypes = [vp, vp, vp, vp]
         lib.farm_map_query.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, ci, ci, vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         lib.farm_map_import.argtypes = [vp, vp, ci, vp, vp, vp, ll]
@@ -122,7 +127,8 @@ class FarmMap:
     def __init__(self, voxel_size, D, w_geo, w_sem, tau, *, H, W, dtype=DTYPE_F32, max_objects=None,
                  max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
                  stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None,
-                 views=None, view_cos=None, view_closer=None):
+                 views=None, view_cos=None, view_closer=None, correspondence=None, geometry=None, prefilter_cos=None,
+                 hellinger_budget=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._last_M = 0
@@ -135,7 +141,7 @@ class FarmMap:
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
                        (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility),
-                       (OPT_VIEWS, views)):
+                       (OPT_VIEWS, views), (OPT_CORRESPONDENCE, correspondence), (OPT_GEOMETRY, geometry)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:
@@ -146,6 +152,10 @@ class FarmMap:
             self.set_option_f(OPTF_VIEW_COS, view_cos)
         if view_closer is not None:
             self.set_option_f(OPTF_VIEW_CLOSER, view_closer)
+        if prefilter_cos is not None:
+            self.set_option_f(OPTF_PREFILTER_COS, prefilter_cos)
+        if hellinger_budget is not None:
+            self.set_option_f(OPTF_HELLINGER_BUDGET, hellinger_budget)
         self.views_k = int(views or 0)
 
     def destroy(self):
@@ -259,6 +269,24 @@ class FarmMap:
                                              int(emb_dtype), _dp(cls), _hp(qt), int(target_class), P, _hp(pt), _hp(ql), int(topk),
                                              _hp(top), _hp(tsc), _hp(lms), _hp(s_sem), _hp(gbar), _hp(s)))
         return {"top": top, "top_scores": tsc, "landmarks": lms[:P], "s_sem": s_sem, "gbar": gbar, "s": s}
+
+    def read_alias(self):
+        """alias [N]: the live entity every id stands for (FARM_OPT_CORRESPONDENCE)."""
+        n = C.c_int(0)
+        _check(load_library().farm_map_read(self._h, None, C.byref(n), None, None, None, None))
+        al = np.zeros(n.value, np.int32)
+        _check(load_library().farm_map_read_alias(self._h, _hp(al)))
+        return al
+
+    def last_merges(self):
+        """(loser [n], winner [n]) entity merges of the last call, sorted by loser (FARM_OPT_CORRESPONDENCE)."""
+        n = C.c_int(0)
+        _check(load_library().farm_map_last_merges(self._h, None, None, C.byref(n)))
+        a, b = np.zeros(n.value, np.int32), np.zeros(n.value, np.int32)
+        if n.value:
+            _check(load_library().farm_map_last_merges(self._h, _hp(a), _hp(b), C.byref(n)))
+        order = np.argsort(a)
+        return a[order], b[order]
 
     def read_views(self):
         """(views [N, k] VIEW_DTYPE, counts [N]) retained views per object (FARM_OPT_VIEWS = k)."""

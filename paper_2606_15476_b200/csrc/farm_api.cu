@@ -41,8 +41,8 @@ struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
   long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
-  int sim_path = 0, gaussian = 0, covis = 0, views_k = 0;
-  float view_cos = 0.8660254f, view_closer = 0.8f;
+  int sim_path = 0, gaussian = 0, covis = 0, views_k = 0, corr = 0, geom = 0;
+  float view_cos = 0.8660254f, view_closer = 0.8f, prefilter_cos = 0.5f, hell_budget = 1.0f;
   cudaStream_t stream = 0;
   bool finalised = false;
   DevMap dm{};
@@ -80,6 +80,12 @@ struct farm_map {
 };
 
 namespace {
+
+__global__ void init_forest_kernel(DevMap m) {  // U: alias and union-find forest start as the identity
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < m.max_objects) m.alias[i] = i;
+  if (i < m.max_objects + m.max_det) m.uf_parent[i] = i;
+}
 
 __global__ void init_objects_kernel(DevMap m) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -240,7 +246,7 @@ __global__ void export_voxels_kernel(DevMap m, unsigned long long *keys, uint32_
       if (own[b] != OWNER_INIT) {
         if (pos < cap) {
           keys[pos] = voxel_key_of(bkey, (uint32_t)(i & 7) * 8 + b);
-          owners[pos] = own[b];
+          owners[pos] = m.alias ? m.alias[own[b]] : own[b];  // U4: voxels of an absorbed entity belong to its winner
         }
         ++pos;
       }
@@ -385,7 +391,7 @@ int finalise_impl(farm_map *m) {
   A(d.surv_bits, (size_t)scap, 0);
   A(d.surv_j, (size_t)scap, 0);
   d.surv_cap = (uint32_t)scap;
-  A(d.counters, 4, 0);
+  A(d.counters, 16, 0);
   const size_t MD = (size_t)m->max_det;
   d.max_det = (uint32_t)MD;
   A(d.det_nv, MD, 0);
@@ -404,6 +410,36 @@ int finalise_impl(farm_map *m) {
     d.covis_words = (uint32_t)((NO + 63) / 64);
     if ((size_t)d.covis_words * 8 > 96 * 1024) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_COVISIBILITY supports MAX_OBJECTS <= 786432");
     A(d.covis, NO * d.covis_words, 0);
+  }
+  d.dense_thr = 3.0e38f;  // the similarity epilogues emit nothing unless an option below asks for it
+  d.corr = m->corr, d.geom = m->geom, d.prefilter_cos = m->prefilter_cos, d.hell_budget = m->hell_budget;
+  if (m->geom == 1 && !m->gaussian) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_GEOMETRY = 1 needs FARM_OPT_GAUSSIAN = 1");
+  if (m->corr && !(m->tau >= 0.f)) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_CORRESPONDENCE needs tau >= 0");
+  if (m->corr && m->covis) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_CORRESPONDENCE and FARM_OPT_COVISIBILITY cannot be combined yet");
+  if (m->corr || m->geom == 1) {
+    // pairs the similarity epilogue must emit: H1 the prefilter; U1 with the voxel rule every pair whose semantic term alone
+    // passes tau (possible only when w_sem > tau)
+    if (m->geom == 1) d.dense_thr = m->prefilter_cos;
+    else if (m->w_sem > m->tau && m->w_sem > 0.f) d.dense_thr = m->tau / m->w_sem * 0.9999f - 1e-6f;
+    const size_t dcap = std::max<size_t>((size_t)MD * 64, 1 << 16);
+    A(d.dense_d, dcap, 0);
+    A(d.dense_o, dcap, 0);
+    A(d.dense_c, dcap, 0);
+    d.dense_cap = (uint32_t)dcap;
+    const size_t ecap = dcap + (size_t)ccap;
+    A(d.edge_a, ecap, 0);
+    A(d.edge_b, ecap, 0);
+    A(d.dd_d, ecap, 0);
+    A(d.dd_e, ecap, 0);
+    A(d.loser, ecap, 0);
+    A(d.winner, ecap, 0);
+    d.edge_cap = (uint32_t)ecap;
+    A(d.det_flags, MD, 0);
+    A(d.det_newid, MD, 0);
+  }
+  if (m->corr) {
+    A(d.alias, NO, 0);
+    A(d.uf_parent, NO + MD, 0);
   }
   if (m->views_k > 0) {
     d.views_k = m->views_k, d.view_cos = m->view_cos, d.view_closer = m->view_closer;
@@ -425,6 +461,10 @@ int finalise_impl(farm_map *m) {
   configure_assoc_kernels();
   init_objects_kernel<<<(unsigned)((NO + 255) / 256), 256, 0, m->stream>>>(d);
   m->launches++;
+  if (m->corr) {
+    init_forest_kernel<<<(unsigned)((NO + MD + 255) / 256), 256, 0, m->stream>>>(d);
+    m->launches++;
+  }
   CU(cudaGetLastError());
   if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
   if (m->overlap) {
@@ -564,6 +604,14 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad COVISIBILITY");
       m->covis = (int)v;
       break;
+    case FARM_OPT_CORRESPONDENCE:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad CORRESPONDENCE");
+      m->corr = (int)v;
+      break;
+    case FARM_OPT_GEOMETRY:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad GEOMETRY");
+      m->geom = (int)v;
+      break;
     case FARM_OPT_VIEWS:
       if (v < 0 || v > 8) return fail(FARM_ERR_INVALID_ARG, "bad VIEWS (0..8)");
       m->views_k = (int)v;
@@ -586,6 +634,10 @@ int farm_map_set_option_f(farm_map *m, int key, float v) {
     m->z_min = v;
   else if (key == FARM_OPTF_Z_MAX)
     m->z_max = v;
+  else if (key == FARM_OPTF_PREFILTER_COS)
+    m->prefilter_cos = v;
+  else if (key == FARM_OPTF_HELLINGER_BUDGET)
+    m->hell_budget = v;
   else if (key == FARM_OPTF_VIEW_COS)
     m->view_cos = v;
   else if (key == FARM_OPTF_VIEW_CLOSER)
@@ -685,11 +737,12 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (fork) cudaEventRecord(m->ev_join, m->side);
   if (!(fork && m->overlap == 3)) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork && m->overlap == 2) cudaStreamWaitEvent(st, m->ev_join, 0);
-  stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st); });
+  stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st) + launch_dd_overlap(d, a, st); });
   if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
+  stage(FARM_STAGE_MERGE, st, [&] { return launch_alias_compress(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
@@ -990,6 +1043,33 @@ int farm_map_query(farm_map *m, const void *emb0, const void *emb1, const void *
   return rc == FARM_OK ? FARM_OK : fail(rc, err);
 }
 
+int farm_map_read_alias(farm_map *m, int32_t *alias) {
+  if (!m || !alias) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->corr) return fail(FARM_ERR_STATE, "FARM_OPT_CORRESPONDENCE is off");
+  if (!m->finalised) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t N = 0;
+  CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
+  if (N) CU(cudaMemcpy(alias, m->dm.alias, (size_t)N * 4, cudaMemcpyDeviceToHost));
+  return FARM_OK;
+}
+
+int farm_map_last_merges(farm_map *m, int32_t *loser, int32_t *winner, int *n) {
+  if (!m || !n) return fail(FARM_ERR_INVALID_ARG, "NULL argument");
+  if (!m->corr) return fail(FARM_ERR_STATE, "FARM_OPT_CORRESPONDENCE is off");
+  *n = 0;
+  if (!m->has_last) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t k = 0;
+  CU(cudaMemcpy(&k, m->dm.counters + 7, 4, cudaMemcpyDeviceToHost));
+  *n = (int)k;
+  if (k && loser) CU(cudaMemcpy(loser, m->dm.loser, (size_t)k * 4, cudaMemcpyDeviceToHost));
+  if (k && winner) CU(cudaMemcpy(winner, m->dm.winner, (size_t)k * 4, cudaMemcpyDeviceToHost));
+  return FARM_OK;
+}
+
 int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts) {
   if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
   if (m->views_k <= 0) return fail(FARM_ERR_STATE, "FARM_OPT_VIEWS is off");
@@ -1112,13 +1192,15 @@ int farm_debug_last_overlaps(farm_map *m, long long *offsets, int32_t *obj_id, u
   }
   std::vector<long long> cnt(M + 1, 0);
   for (uint32_t i = 0; i < n; ++i)
-    if ((int)js[i] < M) cnt[js[i] + 1]++;
+    if (os[i] < 0) js[i] = 0xFFFFFFFFu;  // detection-detection entries (U2) are not part of the overlap histogram
+  for (uint32_t i = 0; i < n; ++i)
+    if ((int)js[i] < M && (int)js[i] >= 0) cnt[js[i] + 1]++;
   for (int j = 0; j < M; ++j) cnt[j + 1] += cnt[j];
   for (int j = 0; j <= M; ++j) offsets[j] = cnt[j];
   if (obj_id || count) {
     std::vector<long long> cur(cnt.begin(), cnt.end() - 1);
     for (uint32_t i = 0; i < n; ++i)
-      if ((int)js[i] < M) {
+      if ((int)js[i] < M && (int)js[i] >= 0) {
         const long long p = cur[js[i]]++;
         if (obj_id) obj_id[p] = os[i];
         if (count) count[p] = cs[i];

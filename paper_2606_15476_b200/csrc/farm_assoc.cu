@@ -53,18 +53,8 @@ __device__ __noinline__ void match_hellinger(const double *det_gm, const double 
 
 // V1-V2: the view of one merged detection, offered to its object's retained set.  fp32, one rounded
 // operation at a time: the comparisons decide which views are kept and the oracle takes them in the same precision.
-__device__ __noinline__ void offer_view(const DevMap &m, int32_t t, const int *box, const float *cam, int32_t frame, int32_t det,
-                                        uint32_t n_px) {
-  float d[3];
-#pragma unroll
-  for (int k = 0; k < 3; ++k) d[k] = __fsub_rn(__fmul_rn(0.5f, __fadd_rn(ord2f(box[k]), ord2f(box[3 + k]))), cam[k]);
-  const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(d[0], d[0]), __fmul_rn(d[1], d[1])), __fmul_rn(d[2], d[2]));
-  const float dist = __fsqrt_rn(d2);
-  if (!(dist > 0.f)) return;
-  farm_view v;
-  v.frame = frame, v.det = det, v.n_px = n_px, v.dist = dist;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) v.cam[k] = cam[k], v.dir[k] = __fdiv_rn(d[k], dist);
+__device__ __noinline__ void offer_view_record(const DevMap &m, int32_t t, const farm_view &v) {
+  const float dist = v.dist;
   farm_view *set = m.views + (size_t)t * m.views_k;
   const uint32_t n = m.view_cnt[t];
   bool fresh = true;
@@ -85,6 +75,257 @@ __device__ __noinline__ void offer_view(const DevMap &m, int32_t t, const int *b
     set[far] = v;
   }
 }
+__device__ __noinline__ void offer_view(const DevMap &m, int32_t t, const int *box, const float *cam, int32_t frame, int32_t det,
+                                        uint32_t n_px) {
+  float d[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) d[k] = __fsub_rn(__fmul_rn(0.5f, __fadd_rn(ord2f(box[k]), ord2f(box[3 + k]))), cam[k]);
+  const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(d[0], d[0]), __fmul_rn(d[1], d[1])), __fmul_rn(d[2], d[2]));
+  const float dist = __fsqrt_rn(d2);
+  if (!(dist > 0.f)) return;
+  farm_view v;
+  v.frame = frame, v.det = det, v.n_px = n_px, v.dist = dist;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) v.cam[k] = cam[k], v.dir[k] = __fdiv_rn(d[k], dist);
+  offer_view_record(m, t, v);
+}
+
+// U4 ("Entity-level merges ... absorbing the loser's covisibility, captions, view records, and identity
+// history into the winner"): the scalar state of every loser of winner t goes into t -- voxel count, points, box, best
+// view (R23 order), Gaussian statistics, retained views.  Run by one lane of t's merge leader BEFORE the call's
+// detections are fused; the losers' descriptors enter the R21 fold and the losers are retired after it.
+__device__ __noinline__ void absorb_losers(const DevMap &m, int32_t t, uint32_t nL) {
+  for (uint32_t k = 0; k < nL; ++k) {
+    if (m.winner[k] != (uint32_t)t) continue;
+    const uint32_t L = m.loser[k];
+    atomicAdd(&m.n_voxels[t], m.n_voxels[L]);  // commit CTAs add this call's new voxels concurrently
+    m.n_voxels[L] = 0;
+    m.n_points[t] += m.n_points[L];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      m.aabb[t * 6 + c] = min(m.aabb[t * 6 + c], m.aabb[L * 6 + c]);
+      m.aabb[t * 6 + 3 + c] = max(m.aabb[t * 6 + 3 + c], m.aabb[L * 6 + 3 + c]);
+    }
+    const uint32_t pl = m.best_px[L], pt = m.best_px[t];
+    if (pl > pt || (pl == pt && pl > 0 &&
+                    (m.best_seq[L] < m.best_seq[t] || (m.best_seq[L] == m.best_seq[t] && m.best_det[L] < m.best_det[t])))) {
+      m.best_px[t] = pl, m.best_seq[t] = m.best_seq[L], m.best_det[t] = m.best_det[L];
+      for (int c = 0; c < 3; ++c) m.best_cam[t * 3 + c] = m.best_cam[L * 3 + c];
+    }
+    if (m.obj_gw) {
+      m.obj_gw[t] += m.obj_gw[L];
+      for (int c = 0; c < 9; ++c) m.obj_gm[(size_t)t * 9 + c] += m.obj_gm[(size_t)L * 9 + c];
+    }
+    if (m.views)
+      for (uint32_t i = 0; i < m.view_cnt[L]; ++i) offer_view_record(m, t, m.views[(size_t)L * m.views_k + i]);
+  }
+}
+// the absorbed entities stay as dead ids: no observations, no voxels, zero descriptor (cosine 0 with everything)
+__device__ __noinline__ void retire_loser(const DevMap &m, uint32_t L, int32_t t) {
+  m.n_obs[L] = 0;
+  m.n_points[L] = 0;
+  m.inv_norm[L] = 0.f;
+  for (int c = 0; c < 3; ++c) {
+    m.aabb[L * 6 + c] = 0x7F800000;            // ordered image of +inf
+    m.aabb[L * 6 + 3 + c] = (int)0x807FFFFF;   // ordered image of -inf
+    m.best_cam[L * 3 + c] = 0.f;
+  }
+  m.best_px[L] = 0, m.best_seq[L] = 0, m.best_det[L] = 0;
+  if (m.obj_gw) {
+    m.obj_gw[L] = 0.0;
+    for (int c = 0; c < 9; ++c) m.obj_gm[(size_t)L * 9 + c] = 0.0;
+  }
+  if (m.views) m.view_cnt[L] = 0;
+  m.alias[L] = (uint32_t)t;
+  m.leader[L] = NONE32;
+}
+
+// ---- U3: lock-free union-find over the match graph.  The root of a set is its smallest node; entities
+// are numbered before detections (node of detection j = max_objects + j), so a component that holds an entity is won
+// by its lowest-id entity and a component of detections only by its lowest detection.
+__device__ __forceinline__ uint32_t uf_find(const uint32_t *p, uint32_t x) {
+  for (;;) {
+    const uint32_t q = __ldcg(&p[x]);
+    if (q == x) return x;
+    x = q;
+  }
+}
+__device__ __forceinline__ void uf_union(uint32_t *p, uint32_t x, uint32_t y) {
+  for (;;) {
+    x = uf_find(p, x), y = uf_find(p, y);
+    if (x == y) return;
+    const uint32_t hi = max(x, y), lo = min(x, y);
+    if (atomicCAS(&p[hi], hi, lo) == hi) return;
+  }
+}
+__device__ __forceinline__ void add_edge(const DevMap &m, uint32_t j, uint32_t o) {  // U1: detection j retained entity o
+  atomicOr(&m.det_flags[j], 1u);
+  const uint32_t e = atomicAdd(&m.counters[5], 1u);
+  if (e < m.edge_cap) m.edge_a[e] = m.max_objects + j, m.edge_b[e] = o; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+}
+
+// H2-H3: one pair above the similarity prefilter -- Hellinger distance between the detection's and the
+// entity's Gaussian, budget, g = 1 - H, score.  Out of line (double precision temporaries).
+__device__ __noinline__ void hellinger_candidate(const DevMap &m, uint32_t d, uint32_t o, float cs) {
+  const uint32_t npx = __ldcg(&m.det_npx[d]);
+  if (npx == 0) return;  // R8: skipped detection
+  float g = 0.f;
+  const double wo = m.obj_gw[o];
+  if (wo > 0.0) {
+    double gd[9], go[9], mu_d[3], c_d[6], mu_o[3], c_o[6];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) gd[k] = __ldcg(&m.det_gm[(size_t)d * 9 + k]), go[k] = m.obj_gm[(size_t)o * 9 + k];
+    gaussian_of((double)npx, gd, mu_d, c_d);
+    gaussian_of(wo, go, mu_o, c_o);
+    const float hf = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)m.eps2);
+    if (hf > m.hell_budget) return;  // H2: outside the budget -- not a candidate
+    g = __fsub_rn(1.0f, hf);         // H3
+  }
+  const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));
+  atomicMax(&m.best_cand[d], pack_score(score, o));
+  if (m.corr && score > m.tau) add_edge(m, d, o);
+}
+
+// ---- U3 decisions (only with FARM_OPT_CORRESPONDENCE; run by the last CTA of cand_associate_kernel in place of the plain
+// decision scan): union-find over the call's match graph, then per detection the component's root -- an entity (the
+// detection is fused into the winner) or a detection (the component becomes one new entity, numbered in the order of
+// its lowest detection, R20).  Entities that are not their component's root are recorded as (loser, winner) merges.
+constexpr int CORR_THREADS = 512;
+constexpr uint32_t LOSER_MARK = 0xFFFFFFFEu;
+__device__ __noinline__ void correspondence_decide(const DevMap &m, const CallArgs &a, uint32_t N) {
+  __shared__ uint32_t ws[32];
+  __shared__ uint32_t s_running, s_matches, s_skipped;
+  __shared__ unsigned long long s_uvox;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t nodeD = m.max_objects;
+  uint32_t *p = m.uf_parent;
+  if (tid == 0) s_running = 0, s_matches = 0, s_skipped = 0, s_uvox = 0ull;
+  const uint32_t nE = min(__ldcg(&m.counters[5]), m.edge_cap), nDD = min(__ldcg(&m.counters[6]), m.edge_cap);
+  for (uint32_t e = tid; e < nE; e += CORR_THREADS) uf_union(p, __ldcg(&m.edge_a[e]), __ldcg(&m.edge_b[e]));
+  for (uint32_t e = tid; e < nDD; e += CORR_THREADS) {
+    const uint32_t d = __ldcg(&m.dd_d[e]);
+    if (!(__ldcg(&m.det_flags[d]) & 1u)) uf_union(p, nodeD + d, nodeD + __ldcg(&m.dd_e[e]));  // U2: only if d retained nothing
+  }
+  __threadfence();
+  __syncthreads();
+  // pass 1: roots; new entities for the components rooted at a detection, in index order
+  uint32_t n_skipped = 0, nv_sum = 0, n_live = 0;
+  for (int base = 0; base < a.M; base += CORR_THREADS) {
+    const int j = base + tid;
+    bool is_root = false;
+    if (j < a.M) {
+      nv_sum += __ldcg(&m.det_nv[j]);
+      if (__ldcg(&m.det_npx[j]) == 0) {
+        ++n_skipped;  // R8
+      } else {
+        ++n_live;
+        is_root = uf_find(p, nodeD + j) == nodeD + (uint32_t)j;
+      }
+    }
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, is_root);
+    if (lane == 0) ws[warp] = __popc(b);
+    __syncthreads();
+    uint32_t before = s_running, total = 0;
+    for (int w = 0; w < CORR_THREADS / 32; ++w) {
+      if (w < warp) before += ws[w];
+      total += ws[w];
+    }
+    if (is_root) {
+      const uint32_t id = N + before + __popc(b & ((1u << lane) - 1));
+      if (id < m.max_objects) {
+        m.det_newid[j] = id;
+      } else {
+        m.det_newid[j] = NONE32;
+        atomicOr(m.err, ERR_OBJECT_CAPACITY);
+      }
+    }
+    __syncthreads();
+    if (tid == 0) s_running += total;
+    __syncthreads();
+  }
+  __threadfence();
+  __syncthreads();
+  // pass 2: targets, scores, merge groups
+  uint32_t n_new = 0;
+  for (int j = tid; j < a.M; j += CORR_THREADS) {
+    const uint32_t npx = __ldcg(&m.det_npx[j]);
+    int32_t target = -1;
+    uint32_t is_new = 0;
+    float score = 0.f;
+    if (npx != 0) {
+      unsigned long long best = __ldcg(&m.best_cand[j]);
+      const unsigned long long bd = __ldcg(&m.best_dense[j]);
+      if (bd && m.geom == 0) {
+        const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd)));
+        const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd) : 0u);
+        best = pd > best ? pd : best;
+      }
+      if (best) {
+        score = unpack_score(best);
+        if (m.det_gm && score > m.tau) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, (int32_t)unpack_id(best), npx);  // G4
+      }
+      const uint32_t r = uf_find(p, nodeD + (uint32_t)j);
+      if (r < nodeD) {
+        target = (int32_t)r;
+      } else {
+        const uint32_t id = __ldcg(&m.det_newid[r - nodeD]);
+        if (id != NONE32) {
+          target = (int32_t)id;
+          is_new = r == nodeD + (uint32_t)j;  // the component's lowest detection creates the entity
+          n_new += is_new;
+        }
+      }
+    }
+    m.assoc[j] = target;
+    m.is_new[j] = (uint8_t)is_new;
+    m.best_score[j] = score;
+    if (target >= 0) {
+      atomicMin(&m.leader[target], (uint32_t)j);
+      atomicAdd(&m.grp_cnt[target], 1u);
+    } else if (npx != 0) {
+      ++n_skipped;  // object capacity: the detection is dropped
+      --n_live;
+    }
+  }
+  // losers: the entity end of every edge that is not its component's root
+  for (uint32_t e = tid; e < nE; e += CORR_THREADS) {
+    const uint32_t o = __ldcg(&m.edge_b[e]);
+    const uint32_t r = uf_find(p, o);
+    if (r != o && atomicCAS(&m.leader[o], NONE32, LOSER_MARK) == NONE32) {
+      const uint32_t k = atomicAdd(&m.counters[7], 1u);
+      m.loser[k] = o, m.winner[k] = r;  // at most one entry per entity: k < edge_cap
+    }
+  }
+  n_skipped = __reduce_add_sync(0xFFFFFFFFu, n_skipped);
+  nv_sum = __reduce_add_sync(0xFFFFFFFFu, nv_sum);
+  n_live = __reduce_add_sync(0xFFFFFFFFu, n_live);
+  n_new = __reduce_add_sync(0xFFFFFFFFu, n_new);
+  if (lane == 0) {
+    atomicAdd(&s_skipped, n_skipped);
+    atomicAdd(&s_matches, n_live - n_new);
+    atomicAdd(&s_uvox, (unsigned long long)nv_sum);
+  }
+  __threadfence();
+  __syncthreads();
+  // the forest returns to the identity for the next call
+  for (uint32_t e = tid; e < nE; e += CORR_THREADS) p[m.edge_a[e]] = m.edge_a[e], p[m.edge_b[e]] = m.edge_b[e];
+  for (uint32_t e = tid; e < nDD; e += CORR_THREADS) p[nodeD + m.dd_d[e]] = nodeD + m.dd_d[e], p[nodeD + m.dd_e[e]] = nodeD + m.dd_e[e];
+  if (tid == 0) {
+    uint32_t spawns = s_running;
+    if (N + spawns > m.max_objects) spawns = m.max_objects - N;
+    *m.n_objects = N + spawns;
+    m.stats->matches = s_matches;
+    m.stats->spawns = spawns;
+    m.stats->skipped = s_skipped;
+    m.stats->unique_voxels = s_uvox;
+    atomicAdd(&m.totals->frames, (unsigned long long)a.F);
+    atomicAdd(&m.totals->calls, 1ull);
+    atomicAdd(&m.totals->valid_points, __ldcg(&m.stats->valid_points));
+    atomicAdd(&m.totals->unique_voxels, s_uvox);
+    atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
+    atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
+  }
+}
 
 // ---- candidate scoring + association, one launch.
 // Phase 1 (all CTAs): one warp per non-zero overlap entry (d, o, c): cos(a_d, shadow_o) by a gather dot, g (R10),
@@ -95,7 +336,7 @@ constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PER = 4; 
 
 template <typename T>
 // 80 registers: 512 x 80 fits beside the similarity CTA (256 x 80) and the phase-1 dot products overlap its tail
-__global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
+__global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ DevMap m, const __grid_constant__ CallArgs a) {
   __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per pass
   __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
@@ -110,20 +351,23 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
       const uint32_t slot = m.cand_slot[c];
       const unsigned long long kv = m.cand_key[c];
       const uint32_t j = (uint32_t)(kv >> 32) & ((1u << DET_BITS) - 1);
-      const uint32_t o = (uint32_t)kv;
+      const uint32_t o32 = (uint32_t)kv;
+      const bool dd = (o32 & DD_FLAG) != 0;  // U2: the "owner" is detection e of this call, not an entity
+      const uint32_t o = o32 & ~DD_FLAG;
       const uint32_t cnt = __ldcg(&m.ov_cnt[slot]);
       __syncwarp();
       if (lane == 0) {
         m.ov_cnt[slot] = 0;  // invariant: counts are zero between calls (the tables are epoch tagged)
         m.cand_j[c] = j;
-        m.cand_o[c] = (int32_t)o;
+        m.cand_o[c] = (int32_t)o32;  // negative for detection-detection entries: the debug read skips them
         m.cand_c[c] = cnt;
       }
+      if (m.geom == 1 && !dd) continue;  // H: entity candidates come from the similarity prefilter, not from overlap
       const T *x = (const T *)a.desc + (size_t)j * D;
-      const T *y = (const T *)m.desc_shadow + (size_t)o * D;
+      const T *y = dd ? (const T *)a.desc + (size_t)o * D : (const T *)m.desc_shadow + (size_t)o * D;
       // scalars of the score, requested together with the rows (same address in every lane: one transaction)
-      const float ia = m.det_inv_norm[j], ib = m.inv_norm[o];
-      const uint32_t mn = min(__ldcg(&m.det_nv[j]), m.n_voxels[o]);
+      const float ia = m.det_inv_norm[j], ib = dd ? m.det_inv_norm[o] : m.inv_norm[o];
+      const uint32_t mn = min(__ldcg(&m.det_nv[j]), dd ? __ldcg(&m.det_nv[o]) : m.n_voxels[o]);
       float dot = 0.f;
       if (sizeof(T) == 2 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {
         for (int i = lane * 8; i < D; i += 256) {
@@ -144,7 +388,33 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
         cs = fminf(1.f, fmaxf(-1.f, cs));                                  // R15
         const float g = mn ? __fdiv_rn((float)cnt, (float)mn) : 0.f;       // R10
         const float score = __fadd_rn(__fmul_rn(m.w_geo, g), __fmul_rn(m.w_sem, cs));  // R17
-        atomicMax(&m.best_cand[j], pack_score(score, o));
+        if (dd) {  // U2: detection j is linked to the earlier detection o if they see the same new space and look alike
+          if (score > m.tau) {
+            const uint32_t e = atomicAdd(&m.counters[6], 1u);
+            if (e < m.edge_cap) m.dd_d[e] = j, m.dd_e[e] = o; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+          }
+        } else {
+          atomicMax(&m.best_cand[j], pack_score(score, o));
+          if (m.corr && score > m.tau) add_edge(m, j, o);  // U1
+        }
+      }
+    }
+    // pairs above the similarity threshold (emitted by the similarity epilogue): H candidates / U1 edges without overlap
+    if (m.dense_d && (m.geom == 1 || m.corr)) {
+      if (a.wait_sim) {  // the list is complete only when the similarity grid has finished
+        if (tid == 0) spin_until(m.sim_done, a.sim_target, m.err);
+        __syncthreads();
+      }
+      const uint32_t n_dense = min(__ldcg(&m.counters[4]), m.dense_cap);
+      for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < n_dense; e += gridDim.x * blockDim.x) {
+        const uint32_t d = __ldcg(&m.dense_d[e]), o = __ldcg(&m.dense_o[e]);
+        const float cs = __ldcg(&m.dense_c[e]);
+        if (m.geom == 1) {
+          hellinger_candidate(m, d, o, cs);
+        } else if (__ldcg(&m.det_npx[d]) != 0) {
+          const float score = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, cs));
+          if (score > m.tau) add_edge(m, d, o);
+        }
       }
     }
   }
@@ -166,6 +436,10 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
   }
   pdl_trigger();  // the merge kernel becomes resident now, not while the similarity kernel still runs
   __threadfence();
+  if (m.corr) {  // U: union-find over the match graph instead of the per-detection argmax
+    correspondence_decide(m, a, N);
+    return;
+  }
   // Each thread decides CAND_PER consecutive detections; one pass (one barrier) per CAND_THREADS * CAND_PER detections.
   uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier passes (every thread)
   for (int base = 0; base < a.M; base += CAND_THREADS * CAND_PER) {
@@ -192,7 +466,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(DevMap m, CallArgs a) {
         continue;
       }
       unsigned long long best = bc[k];
-      if (bd[k]) {
+      if (bd[k] && m.geom == 0) {
         // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
         const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd[k])));
         const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd[k]) : 0u);
@@ -291,8 +565,8 @@ constexpr int MERGE_THREADS = 256, MERGE_WARPS = MERGE_THREADS / 32;
 constexpr int MLIST = 64;  // members of one target object kept in shared memory; larger groups are re-scanned
 
 template <typename T>
-__global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, CallArgs a, unsigned long long frame_seq0,
-                                                           int commit_blocks) {
+__global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __grid_constant__ DevMap m, const __grid_constant__ CallArgs a,
+                                                                     unsigned long long frame_seq0, int commit_blocks) {
   __shared__ uint32_t mlist[MERGE_WARPS][MLIST];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   pdl_trigger();  // the optional covisibility kernel may become resident behind this grid
@@ -358,6 +632,16 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   const uint32_t lead = __ldcg(&m.leader[t]), group = __ldcg(&m.grp_cnt[t]);
   if (lead != (uint32_t)j) return;
   const int D = m.D;
+  // U4: entities absorbed by t in this call
+  const uint32_t nL = m.corr ? min(__ldcg(&m.counters[7]), m.edge_cap) : 0u;
+  uint32_t loser_obs = 0, n_losers = 0;
+  for (uint32_t k = 0; k < nL; ++k)
+    if (__ldcg(&m.winner[k]) == (uint32_t)t) loser_obs += m.n_obs[__ldcg(&m.loser[k])], ++n_losers;
+  const bool has_losers = n_losers != 0;
+  if (has_losers) {
+    if (lane == 0) absorb_losers(m, t, nL);
+    __syncwarp();
+  }
   const uint32_t n_old = m.n_obs[t];
   const float nf = (float)n_old;
   float *master = m.desc_master + (size_t)t * D;
@@ -429,7 +713,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
   }
   // f_o <- normalise(n_obs * f_o + sum_m a_m / |a_m|)   (R21).  Two passes over the rows (the second one hits
   // L1/L2): pass 1 the squared norm, pass 2 the same values again, scaled and written with their shadows.
-  const bool vec = sizeof(T) == 2 && group <= 1 && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
+  const bool vec = sizeof(T) == 2 && group <= 1 && !has_losers && (D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0;
   auto value = [&](int i) -> float {  // generic path, one element
     float acc = 0.f;
     bool first = true;
@@ -438,7 +722,14 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
       acc = first ? x * inv : fmaf(x, inv, acc);
       first = false;
     });
-    return n_old ? fmaf(nf, master[i], acc) : acc;
+    if (n_old) acc = fmaf(nf, master[i], acc);
+    if (has_losers)  // U4: the losers' descriptors, weighted by their detection counts
+      for (uint32_t k = 0; k < nL; ++k)
+        if (m.winner[k] == (uint32_t)t) {
+          const uint32_t L = m.loser[k];
+          acc = fmaf((float)m.n_obs[L], m.desc_master[(size_t)L * D + i], acc);
+        }
+    return acc;
   };
   const float inv_j = m.det_inv_norm[j];
   const T *row_j = desc + (size_t)j * D;
@@ -505,7 +796,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
     if (lane == 0) m.inv_norm[t] = s2 > 0.f ? 1.0f / sqrtf(s2) : 0.f;
   }
   if (lane == 0) {
-    m.n_obs[t] = n_old + k_members;
+    m.n_obs[t] = n_old + loser_obs + k_members;
     m.n_points[t] = pts_old + pts;
     if (m.det_gm) {  // G2: M1 += sum w mu, M2 += sum w (Sigma + mu mu^T), w = points
       m.obj_gw[t] += (double)pts;
@@ -528,6 +819,18 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(DevMap m, C
     }
     m.leader[t] = NONE32;
     m.grp_cnt[t] = 0;
+  }
+  if (has_losers) {  // the fold above was the last reader of the losers' rows
+    __syncwarp();
+    for (uint32_t k = 0; k < nL; ++k)
+      if (m.winner[k] == (uint32_t)t) {
+        const uint32_t L = m.loser[k];
+        for (int i = lane; i < D; i += 32) {
+          m.desc_master[(size_t)L * D + i] = 0.f;
+          ((T *)m.desc_shadow)[(size_t)L * D + i] = from_f32<T>(0.f);
+        }
+        if (lane == 0) retire_loser(m, L, t);
+      }
   }
 }
 

@@ -26,6 +26,7 @@ constexpr uint32_t ERR_OVERLAP_TABLE_FULL = 4u;
 constexpr uint32_t ERR_OBJECT_CAPACITY = 8u;
 constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
 constexpr uint32_t ERR_SYNC_TIMEOUT = 32u;       // a device-side wait for another grid of the same call expired
+constexpr uint32_t DD_FLAG = 0x80000000u;        // overlap-map "owner" field: DD_FLAG | e = detection e of the same call (U2)
 constexpr uint32_t ERR_IMPORT_COUNT = 64u;       // import: objects[i].n_voxels differs from the voxels listed for i
 constexpr uint32_t SPIN_LIMIT = 1u << 23;        // polls of ~0.25 us each (about 2 s) before a device-side wait gives up
 
@@ -107,6 +108,7 @@ struct DevMap {
   uint32_t *surv_j;
   uint32_t surv_cap;
   uint32_t *counters;                // [0]=event_count [1]=cand_count [2]=survivor_count [3]=block ticket
+                                     // [4]=dense pairs [5]=edges [6]=detection-detection edges [7]=entity merges
   // per detection [max_det]
   uint32_t max_det;
   uint32_t *det_nv, *det_npx;
@@ -123,6 +125,23 @@ struct DevMap {
   float eps2;                        // voxel_size^2, added to both covariance diagonals (reading G3)
   unsigned long long *covis;         // [max_objects, covis_words] covisibility bitset (rule C1); null when disabled
   uint32_t covis_words;
+  // U1-U4 correspondence by union-find with entity merges, H1-H3 Hellinger
+  // distance as the geometric term; everything below is null / 0 when both are disabled
+  int corr, geom;                    // FARM_OPT_CORRESPONDENCE, FARM_OPT_GEOMETRY
+  float prefilter_cos, hell_budget;  // H1, H2
+  float dense_thr;                   // cosine above which the similarity epilogue emits the pair (+inf: never)
+  uint32_t *dense_d, *dense_o;       // emitted pairs (detection, object, clamped cosine); counters[4] = count
+  float *dense_c;
+  uint32_t dense_cap;
+  uint32_t *alias;                   // [max_objects] the live entity every id stands for (itself while alive); U4
+  uint32_t *uf_parent;               // [max_objects + max_det] union-find forest, identity between calls; node of
+                                     //   detection j = max_objects + j, so that entities order before detections
+  uint32_t *det_flags;               // [max_det] bit 0: the detection retained an entity (U1)
+  uint32_t *det_newid;               // [max_det] id of the entity created by the component rooted at the detection
+  uint32_t *edge_a, *edge_b;         // match-graph edges (node, node); counters[5] = count
+  uint32_t *dd_d, *dd_e;             // detection-detection edges, used only if dd_d retained nothing (U2); counters[6]
+  uint32_t edge_cap;
+  uint32_t *loser, *winner;          // entity merges of the call (U4); counters[7] = count
   // V1-V2: up to views_k retained views per object; null when disabled
   farm_view *views;                  // [max_objects, views_k]
   uint32_t *view_cnt;                // [max_objects]
@@ -263,5 +282,17 @@ int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_dd_overlap(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_alias_compress(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
+
+// one pair above the similarity threshold, from the similarity epilogues (H1 prefilter / U1 dense edges)
+__device__ __forceinline__ void dense_emit(const DevMap &m, uint32_t d, uint32_t o, float cs) {
+  const uint32_t pos = atomicAdd(&m.counters[4], 1u);
+  if (pos < m.dense_cap) {
+    m.dense_d[pos] = d, m.dense_o[pos] = o, m.dense_c[pos] = cs;
+  } else {
+    atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+  }
+}
 
 }  // namespace farm

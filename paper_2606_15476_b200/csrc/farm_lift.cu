@@ -88,6 +88,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     m.counters[0] = 0;
     m.counters[1] = 0;
     m.counters[2] = 0;
+    m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0;
     CallStats z = {};
     z.n_det = (uint32_t)a.M;
     *m.stats = z;
@@ -129,6 +130,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     m.assoc[warp] = -1;
     m.is_new[warp] = 0;
     m.best_score[warp] = 0.f;
+    if (m.det_flags) m.det_flags[warp] = 0;
   }
   if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
   if (m.det_gm) {
@@ -696,7 +698,8 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
 #pragma unroll
         for (int b = 0; b < 8; ++b) {
           if (!((byte >> b) & 1u)) continue;
-          const uint32_t o = own[b];
+          uint32_t o = own[b];
+          if (o < OWNER_PENDING && m.alias) o = __ldg(&m.alias[o]);  // U4: voxels of an absorbed entity count for its winner
           if (o >= OWNER_PENDING) {  // unowned at entry (free, or claimed by a detection of this call)
             unowned = true;
             atomicMin(base + b, OWNER_PENDING | rj);  // R12: lowest detection index wins
@@ -752,6 +755,81 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
         atomicOr(m.err, ERR_PAIR_TABLE_FULL);
       }
     }
+  }
+}
+
+// U2 (detection-detection overlap, only with FARM_OPT_CORRESPONDENCE): after every probe has run, the owner word of a
+// voxel that was unowned at entry holds OWNER_PENDING | e, e = the lowest-index detection of the call containing it
+// (the R12 claimant).  For every event (detection j, block, new voxel bits) the voxels claimed by another detection
+// e != j are counted into the overlap map under the key (j, DD_FLAG | e): c_dd(j, e).  Eight lanes per event.
+__global__ void __launch_bounds__(256) dd_overlap_kernel(DevMap m, CallArgs a) {
+  pdl_wait();
+  const uint32_t n = min(m.counters[0], m.pair_cap);
+  const int lane = threadIdx.x & 31, sec = lane & 7;
+  const uint32_t per_pass = (gridDim.x * blockDim.x) >> 3;
+  const uint32_t n_pad = (n + 3u) & ~3u;  // whole groups of 4 events per warp
+  for (uint32_t e0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 3; e0 < n_pad; e0 += per_pass) {
+    const bool act = e0 < n;
+    const uint32_t jp = act ? m.pl_j[e0] : 0u;
+    const uint32_t j = jp & 0x7FFFFFFFu;
+    const uint32_t byte = (act && (jp >> 31)) ? (uint32_t)(m.pl_bits[e0] >> (8 * sec)) & 0xFFu : 0u;
+    uint32_t e1 = NONE32, c1 = 0;
+    if (byte) {
+      const uint32_t *base = m.blk_owner + (size_t)m.pl_slot[e0] * BLK_VOXELS + sec * 8;
+      const uint4 w0 = __ldcg(reinterpret_cast<const uint4 *>(base)), w1 = __ldcg(reinterpret_cast<const uint4 *>(base) + 1);
+      const uint32_t own[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+      for (int b = 0; b < 8; ++b) {
+        if (!((byte >> b) & 1u) || own[b] < OWNER_PENDING) continue;
+        const uint32_t e = own[b] & 0x7FFFFFFFu;
+        if (e == j) continue;
+        if (e1 == NONE32 || e == e1) {
+          e1 = e, c1++;
+        } else {  // a second claimant inside one sector: counted on its own
+          const unsigned long long ov = ((unsigned long long)a.epoch << 48) | ((unsigned long long)j << 32) | (DD_FLAG | e);
+          uint32_t os;
+          const int r = epoch_insert(m.ov_keys, m.ov_mask, ov, a.epoch, &os);
+          if (r < 0) { atomicOr(m.err, ERR_OVERLAP_TABLE_FULL); continue; }
+          if (r == 1) {
+            const uint32_t c = atomicAdd(&m.counters[1], 1u);
+            if (c < m.cand_cap) m.cand_slot[c] = os, m.cand_key[c] = ov; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+          }
+          atomicAdd(&m.ov_cnt[os], 1u);
+        }
+      }
+    }
+    const unsigned oact = __ballot_sync(0xFFFFFFFFu, c1 != 0);
+    if (c1) {
+      const unsigned long long je = ((unsigned long long)j << 32) | (DD_FLAG | e1);
+      const unsigned same = __match_any_sync(oact, je);
+      const uint32_t tot = __reduce_add_sync(same, c1);
+      if (lane == __ffs(same) - 1) {
+        const unsigned long long ov = ((unsigned long long)a.epoch << 48) | je;
+        uint32_t os;
+        const int r = epoch_insert(m.ov_keys, m.ov_mask, ov, a.epoch, &os);
+        if (r < 0) {
+          atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+        } else {
+          if (r == 1) {
+            const uint32_t c = atomicAdd(&m.counters[1], 1u);
+            if (c < m.cand_cap) m.cand_slot[c] = os, m.cand_key[c] = ov; else atomicOr(m.err, ERR_OVERLAP_TABLE_FULL);
+          }
+          atomicAdd(&m.ov_cnt[os], tot);
+        }
+      }
+    }
+  }
+}
+
+// U4: after the merges of a call, every id that pointed at an absorbed entity points at the entity that absorbed it
+__global__ void alias_compress_kernel(DevMap m, uint32_t n_upper) {
+  pdl_wait();
+  if (m.counters[7] == 0) return;
+  const uint32_t N = min(*m.n_objects, n_upper);
+  for (uint32_t o = blockIdx.x * blockDim.x + threadIdx.x; o < N; o += gridDim.x * blockDim.x) {
+    uint32_t r = m.alias[o];
+    for (int hop = 0; hop < 64 && m.alias[r] != r; ++hop) r = m.alias[r];
+    if (r != m.alias[o]) m.alias[o] = r;
   }
 }
 
@@ -824,6 +902,18 @@ int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
 
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   launch_pdl(probe_kernel, dim3(m.num_sms * 4), dim3(PROBE_THREADS), 0, s, m, a);
+  return 1;
+}
+
+int launch_dd_overlap(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+  if (!m.corr || a.M == 0) return 0;
+  launch_pdl(dd_overlap_kernel, dim3(m.num_sms * 2), dim3(256), 0, s, m, a);
+  return 1;
+}
+
+int launch_alias_compress(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s) {
+  if (!m.corr || a.M == 0) return 0;
+  launch_pdl(alias_compress_kernel, dim3(m.num_sms), dim3(256), 0, s, m, n_upper);
   return 1;
 }
 

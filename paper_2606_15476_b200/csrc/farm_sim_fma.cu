@@ -58,6 +58,7 @@ __global__ void __launch_bounds__(SIM_THREADS) similarity_fma_kernel(DevMap m, C
         if (col < N) {
           float cs = acc[r][c] * ia * m.inv_norm[col];
           cs = fminf(1.f, fmaxf(-1.f, cs));
+          if (row < M && cs > m.dense_thr) dense_emit(m, (uint32_t)row, (uint32_t)col, cs);  // H1 / U1 (off: thr = +inf)
           const unsigned long long p = pack_score(cs, (uint32_t)col);
           best = p > best ? p : best;
         }

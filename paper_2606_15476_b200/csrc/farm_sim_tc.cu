@@ -111,6 +111,7 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // 80 registers per thread (no spills): 256 x 80 leaves room for four 128 x 80 lift CTAs on the same SM
+template <bool EMIT>  // EMIT: pairs whose cosine exceeds m.dense_thr also go to the dense list (H1 prefilter / U1 edges)
 __global__ void __maxnreg__(80)
 similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
                      int M, uint32_t idesc, uint32_t prep_target) {
@@ -220,6 +221,9 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
       // four interleaved chains (columns = chain mod 4): strict > keeps the lowest column inside a chain
       float bv[4] = {-3.0e38f, -3.0e38f, -3.0e38f, -3.0e38f};
       int bc[4] = {0, 1, 2, 3};
+      // raw threshold of the row: acc * ib > thr / ia  <=>  cos > thr (slightly low: the exact test follows in the emit)
+      const float thr_t = m.dense_thr / ia;
+      const float thr_row = (EMIT && row_ok && ia > 0.f) ? thr_t - fabsf(thr_t) * 1e-5f - 1e-30f : 3.0e38f;
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
 #pragma unroll 1
       for (int c0 = cbeg; c0 < cbeg + BLOCK_N / EPI_SPLIT; c0 += 32) {
@@ -232,12 +236,20 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
           for (int i = 0; i < 32; ++i) {
             const float v = __uint_as_float(r[i]) * ib[c0 + i];
             if (v > bv[i & 3]) bv[i & 3] = v, bc[i & 3] = c0 + i;
+            if (EMIT && v > thr_row) {
+              const float cs = fminf(1.f, fmaxf(-1.f, v * ia));
+              if (cs > m.dense_thr) dense_emit(m, (uint32_t)row, (uint32_t)(n0 + c0 + i), cs);
+            }
           }
         } else {
 #pragma unroll
           for (int i = 0; i < 32; ++i) {
             const float v = __uint_as_float(r[i]) * ib[c0 + i];
             if (c0 + i < ncols && v > bv[i & 3]) bv[i & 3] = v, bc[i & 3] = c0 + i;
+            if (EMIT && c0 + i < ncols && v > thr_row) {
+              const float cs = fminf(1.f, fmaxf(-1.f, v * ia));
+              if (cs > m.dense_thr) dense_emit(m, (uint32_t)row, (uint32_t)(n0 + c0 + i), cs);
+            }
           }
         }
       }
@@ -330,7 +342,8 @@ void *tc_state_create(const DevMap &m) {
     delete st;
     return nullptr;
   }
-  if (cudaFuncSetAttribute(similarity_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
+  if (cudaFuncSetAttribute(similarity_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
     delete st;
     return nullptr;
   }
@@ -356,7 +369,10 @@ int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, c
   const CUtensorMap &map_a = st->map_a;
   const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
   const int grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
-  similarity_tc_kernel<<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+  if (m.dense_d && m.dense_thr < 2.0f)
+    similarity_tc_kernel<true><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+  else
+    similarity_tc_kernel<false><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
   if (n_ctas) *n_ctas = grid;
   return 1;
 }

@@ -363,3 +363,169 @@ def test_retrieval_scoring_float_embeddings_robust_entities(oracle):
     assert robust.sum() > 0.5 * N
     assert np.abs(rg["s_sem"] - ro["s_sem"])[robust].max() <= 1e-6
     assert np.abs(rg["s_sem"] - ro["s_sem"]).max() <= 0.02
+
+
+# ------------------------------------------------------------------------------------------------ correspondence (U1-U4)
+def _compare_corr(g, o):
+    assert np.array_equal(g.read_alias(), o.read_alias())
+    lg, wg = g.last_merges()
+    lo, wo = o.last_merges()
+    order = np.argsort(lo)
+    assert np.array_equal(lg, lo[order]) and np.array_equal(wg, wo[order])
+    return len(lo)
+
+
+def test_correspondence_hand_cases(oracle):
+    """The oracle's U pins through the CUDA path: a detection bridging two entities (winner = lowest id, voxels re-owned,
+    count-weighted descriptor), a chain of three entities joined by two detections, and a same-call duplicate spawn."""
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    H, W = 128, 128
+    I4 = np.eye(4, dtype=np.float32)
+    E = np.eye(8, dtype=np.float32)
+
+    class Cfg:
+        voxel, D, w_geo, w_sem, tau, dtype = 0.25, 8, 0.5, 0.5, 0.5, 0
+
+    def pair():
+        o, g = make_pair(oracle, Cfg, H=H, W=W, correspondence=1)
+        o.set_option(o.OPT_CORRESPONDENCE, 1)
+        return o, g
+
+    def objs(nv, nobs=None):
+        ob = np.zeros(len(nv), OBJECT_DTYPE)
+        ob["id"], ob["n_voxels"], ob["n_obs"], ob["best_frame"], ob["best_det"] = np.arange(len(nv)), nv, nobs or 1, -1, -1
+        return ob
+
+    def frame(px, desc):
+        depth, mask = hand_frame(H, W, px)
+        return S.Frame(depth, mask, pow2_K(), I4, np.ascontiguousarray(desc, np.float32), len(desc), np.zeros(len(desc), np.int64))
+
+    four = lambda lab, v: [(64 + 16 * i, v, 2.0, lab) for i in range(4)]
+    # (1) bridge
+    o, g = pair()
+    keys = np.array([pack_key(0, 0, 8), pack_key(1, 0, 8), pack_key(2, 0, 8), pack_key(3, 0, 8), pack_key(90, 0, 0)], np.uint64)
+    owners = np.array([0, 0, 1, 1, 2], np.uint32)
+    ob, desc = objs([2, 2, 1], [3, 1, 1]), np.stack([E[0], E[1], E[5]])
+    assert o.import_(ob, desc, keys, owners) == 0
+    g.import_(ob, desc, keys, owners)
+    fr = frame(four(1, 48), [(E[0] + E[1]) / np.sqrt(2)])
+    for _ in range(2):
+        integrate_frames(o, [fr])
+        gpu_integrate(g, [fr], 0)
+        compare_call(g, o)
+        _compare_corr(g, o)
+    assert list(g.read_alias()) == [0, 0, 2]
+    compare_maps(g, o)
+    # (2) chain of three
+    o, g = pair()
+    keys = np.array([pack_key(i, 0, 8) for i in range(4)] + [pack_key(i, 4, 8) for i in range(4)], np.uint64)
+    owners = np.array([0, 0, 1, 1, 1, 1, 2, 2], np.uint32)
+    ob, desc = objs([2, 4, 2]), np.stack([E[0], E[0], E[0]])
+    assert o.import_(ob, desc, keys, owners) == 0
+    g.import_(ob, desc, keys, owners)
+    fr = frame(four(1, 48) + four(2, 112), [E[0], E[0]])
+    integrate_frames(o, [fr])
+    gpu_integrate(g, [fr], 0)
+    compare_call(g, o)
+    assert _compare_corr(g, o) == 2 and list(g.read_alias()) == [0, 0, 0]
+    compare_maps(g, o)
+    # (3) two frames of one call see the same new voxel with the same descriptor: one entity, not two
+    o, g = pair()
+    fa, fb = frame([(64, 48, 2.0, 1)], [E[0]]), frame([(64, 48, 2.0, 1), (96, 48, 2.0, 2)], [E[0], E[2]])
+    integrate_frames(o, [fa, fb])
+    gpu_integrate(g, [fa, fb], 0)
+    compare_call(g, o)
+    a, n, _, st = g.last_assoc()
+    assert list(a) == [0, 0, 1] and list(n) == [1, 0, 1] and st["spawns"] == 2 and st["matches"] == 1
+    integrate_frames(o, [fa, fb])
+    gpu_integrate(g, [fa, fb], 0)
+    compare_call(g, o)
+    compare_maps(g, o)
+
+
+@pytest.mark.parametrize("w", [(0.7, 0.3, 0.25), (0.5, 0.5, 0.5)])
+def test_correspondence_split_map_scene(oracle, w):
+    """A generated scene that forces bridges: the map of a plain configs[0] run with every object cut into two entities;
+    later detections of an object overlap both halves and merge them.  Per call: decisions, merges, alias; at the end
+    the whole map (voxel owners resolved through the merges, count-weighted descriptors, dead ids)."""
+    from test_oracle_next import split_map_arrays
+    cfg = _with_weights(S.get_config(0), w)
+    sc = S.BoxScene(cfg)
+    plain = oracle.OracleMap(cfg.voxel, cfg.D, 0.5, 0.5, 0.5, cfg.dtype, cfg.H, cfg.W)
+    for k in range(9):
+        fr = sc.frame(k)
+        plain.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
+    arrays = split_map_arrays(*plain.read())
+    o, g = make_pair(oracle, cfg, correspondence=1, gaussian=1)
+    o.set_option(o.OPT_CORRESPONDENCE, 1)
+    assert o.import_(*arrays) == 0
+    g.import_(*arrays)
+    merges = 0
+    for call in range(3, 6):
+        frames = margin_filter(o.clone, [sc.frame(3 * call + i) for i in range(3)], cfg.tau, all_pairs=True)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+        merges += _compare_corr(g, o)
+    compare_maps(g, o)
+    w_o, mu_o, cov_o = o.read_gaussians()
+    w_g, mu_g, cov_g = g.read_gaussians()
+    assert np.array_equal(w_g, w_o) and np.abs(mu_g - mu_o).max() <= TOL and np.abs(cov_g - cov_o).max() <= TOL
+    assert merges >= 3, merges
+
+
+def test_correspondence_dense_edges_on_the_tensor_path(oracle):
+    """w_sem > tau (0, 1, 0.6), mini stress scene, tcgen05 similarity with the emitting epilogue: half of the detections
+    that look at an existing object carry a descriptor half-way between that object's and a filler object's, so they
+    retain BOTH (the filler without any voxel overlap: a dense edge) and bridge them."""
+    from paper_2606_15476_b200.binding import OBJECT_DTYPE
+    sc = S.StressScene(n_batches=1, frames_per_batch=4, n_objects=700)
+    cfg = _with_weights(sc.cfg, (0.0, 1.0, 0.6))
+    ijk, owner, n_vox, desc = sc.build_map()
+    keys = pack_key(ijk[:, 0], ijk[:, 1], ijk[:, 2])
+    objs = np.zeros(len(n_vox), OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(len(n_vox)), n_vox, 1, -1, -1
+    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, sim_path=2, correspondence=1)
+    o.set_option(o.OPT_CORRESPONDENCE, 1)
+    assert o.import_(objs, desc, keys, owner) == 0
+    g.import_(objs, desc, keys, owner)
+    rng = np.random.default_rng(3)
+    n_t = len(sc._blob_ijk)
+    frames = []
+    for fr in sc.batch(0):
+        d = S.storage_to_f32(fr.desc, cfg.dtype).copy()
+        for k in np.nonzero(fr.box_ids > 0)[0][::2]:
+            v = d[k] + desc[int(rng.integers(n_t, len(desc)))]
+            d[k] = v / np.linalg.norm(v)
+        frames.append(S.Frame(fr.depth, fr.mask, fr.K, fr.T, S.to_storage(d.astype(np.float32), cfg.dtype), fr.n_det, fr.box_ids))
+    frames = margin_filter(o.clone, frames, cfg.tau, all_pairs=True)
+    integrate_frames(o, frames)
+    gpu_integrate(g, frames, cfg.dtype)
+    compare_call(g, o)
+    assert _compare_corr(g, o) > 50
+    compare_maps(g, o)
+
+
+# ------------------------------------------------------------------------------------------------ Hellinger geometry (H1-H3)
+@pytest.mark.parametrize("cfg_id,n,per_call,corr", [(0, 20, 1, 0), (0, 18, 3, 1), (1, 30, 1, 0)])
+def test_hellinger_geometry_decisions(oracle, cfg_id, n, per_call, corr):
+    """FARM_OPT_GEOMETRY = 1: the paper's own association: similarity prefilter from the similarity
+    epilogue, g = 1 - Hellinger distance between Gaussians, same score / threshold / spawn rule; with and without the
+    union-find correspondence."""
+    cfg = S.get_config(cfg_id)
+    frames_all = generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n))
+    o, g = make_pair(oracle, cfg, gaussian=1, geometry=1, prefilter_cos=0.3, correspondence=corr)
+    o.set_option(o.OPT_GEOMETRY, 1)
+    o.set_option(o.OPT_PREFILTER_COS, 0.3)
+    o.set_option(o.OPT_CORRESPONDENCE, corr)
+    matched = 0
+    for c in range(0, n, per_call):
+        frames = margin_filter(o.clone, frames_all[c:c + per_call], cfg.tau, all_pairs=bool(corr))
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o)
+        matched += int(o.last_assoc()[4]["matches"])
+        if corr:
+            _compare_corr(g, o)
+    compare_maps(g, o)
+    assert matched > 10
