@@ -415,7 +415,6 @@ int finalise_impl(farm_map *m) {
   d.corr = m->corr, d.geom = m->geom, d.prefilter_cos = m->prefilter_cos, d.hell_budget = m->hell_budget;
   if (m->geom == 1 && !m->gaussian) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_GEOMETRY = 1 needs FARM_OPT_GAUSSIAN = 1");
   if (m->corr && !(m->tau >= 0.f)) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_CORRESPONDENCE needs tau >= 0");
-  if (m->corr && m->covis) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_CORRESPONDENCE and FARM_OPT_COVISIBILITY cannot be combined yet");
   if (m->corr || m->geom == 1) {
     // pairs the similarity epilogue must emit: H1 the prefilter; U1 with the voxel rule every pair whose semantic term alone
     // passes tau (possible only when w_sem > tau)
@@ -741,6 +740,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
+  stage(FARM_STAGE_MERGE, st, [&] { return launch_covis_absorb(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_alias_compress(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);

@@ -840,6 +840,41 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
 // same words, so no atomics are needed.
 constexpr int COVIS_THREADS = 256;
 
+// U4 + C1: an absorbed entity's covisibility goes to its winner.  Pass 1 (one thread per row): every bit L of a loser
+// becomes bit W of its winner.  Pass 2 (one CTA per merge): row W |= row L, row L = 0.  The diagonal bit this can leave
+// in row W is cleared by covisibility_kernel, which visits every winner (a winner always received a detection).
+__global__ void __launch_bounds__(COVIS_THREADS) covis_rename_kernel(DevMap m, uint32_t n_upper) {
+  pdl_wait();
+  const uint32_t nL = min(m.counters[7], m.edge_cap);
+  if (nL == 0) return;
+  const uint32_t N = min(*m.n_objects, n_upper);
+  for (uint32_t r = blockIdx.x * blockDim.x + threadIdx.x; r < N; r += gridDim.x * blockDim.x) {
+    unsigned long long *row = m.covis + (size_t)r * m.covis_words;
+    for (uint32_t k = 0; k < nL; ++k) {
+      const uint32_t L = m.loser[k], W = m.winner[k];
+      if ((row[L >> 6] >> (L & 63)) & 1ull) {
+        row[L >> 6] &= ~(1ull << (L & 63));
+        row[W >> 6] |= 1ull << (W & 63);
+      }
+    }
+  }
+}
+__global__ void __launch_bounds__(COVIS_THREADS) covis_fold_kernel(DevMap m) {
+  pdl_wait();
+  const uint32_t nL = min(m.counters[7], m.edge_cap);
+  const uint32_t words = (*m.n_objects + 63) >> 6;
+  for (uint32_t k = blockIdx.x; k < nL; k += gridDim.x) {
+    unsigned long long *rl = m.covis + (size_t)m.loser[k] * m.covis_words, *rw = m.covis + (size_t)m.winner[k] * m.covis_words;
+    for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) {
+      const unsigned long long v = rl[w];
+      if (v) {
+        atomicOr(&rw[w], v);  // several losers may fold into one winner concurrently
+        rl[w] = 0ull;
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(COVIS_THREADS) covisibility_kernel(DevMap m, CallArgs a) {
   extern __shared__ unsigned long long bm[];  // [words]
   pdl_wait();
@@ -857,12 +892,10 @@ __global__ void __launch_bounds__(COVIS_THREADS) covisibility_kernel(DevMap m, C
     if (t < 0) continue;
     unsigned long long *row = m.covis + (size_t)t * m.covis_words;
     for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) {
-      unsigned long long add = bm[w];
-      if (w == ((uint32_t)t >> 6)) add &= ~(1ull << (t & 63));  // no diagonal
-      if (add) {
-        const unsigned long long old = row[w];
-        if ((old | add) != old) row[w] = old | add;
-      }
+      unsigned long long add = bm[w], keep = ~0ull;
+      if (w == ((uint32_t)t >> 6)) keep = ~(1ull << (t & 63)), add &= keep;  // no diagonal (U4: a fold may have left one)
+      const unsigned long long old = row[w], now = (old | add) & keep;
+      if (now != old) row[w] = now;
     }
   }
 }
@@ -890,6 +923,12 @@ int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int grid = a.M > 0 ? (m.num_sms + 1) / 2 : 1;  // half the SMs x 16 warps: one warp per candidate, ~1.2k candidates per wave
   FARM_DISPATCH((launch_pdl(cand_associate_kernel<T>, dim3(grid), dim3(CAND_THREADS), 0, s, m, a)));
   return 1;
+}
+int launch_covis_absorb(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s) {
+  if (a.M == 0 || !m.covis || !m.corr) return 0;
+  launch_pdl(covis_rename_kernel, dim3(m.num_sms), dim3(COVIS_THREADS), 0, s, m, n_upper);
+  launch_pdl(covis_fold_kernel, dim3(m.num_sms), dim3(COVIS_THREADS), 0, s, m);
+  return 2;
 }
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   if (a.M == 0 || !m.covis) return 0;

@@ -282,6 +282,7 @@ int launch_similarity_fma(const DevMap &m, const CallArgs &a, uint32_t n_upper, 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s);
+int launch_covis_absorb(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
 int launch_dd_overlap(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_alias_compress(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
 

@@ -456,8 +456,9 @@ def test_correspondence_split_map_scene(oracle, w):
         fr = sc.frame(k)
         plain.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
     arrays = split_map_arrays(*plain.read())
-    o, g = make_pair(oracle, cfg, correspondence=1, gaussian=1)
+    o, g = make_pair(oracle, cfg, correspondence=1, gaussian=1, covisibility=1, views=2)
     o.set_option(o.OPT_CORRESPONDENCE, 1)
+    o.set_option(o.OPT_VIEWS_K, 2)
     assert o.import_(*arrays) == 0
     g.import_(*arrays)
     merges = 0
@@ -467,6 +468,8 @@ def test_correspondence_split_map_scene(oracle, w):
         gpu_integrate(g, frames, cfg.dtype)
         compare_call(g, o)
         merges += _compare_corr(g, o)
+        assert np.array_equal(g.read_covisibility(), o.read_covisibility())     # C1 + U4: the losers' rows and columns absorbed
+        _compare_views(g, o)                                                     # V + U4: the losers' views offered to the winner
     compare_maps(g, o)
     w_o, mu_o, cov_o = o.read_gaussians()
     w_g, mu_g, cov_g = g.read_gaussians()
