@@ -409,7 +409,7 @@ def run_ours(args):
     # lift + probe: from the breakdown pass (inside the timed region they are chained by PDL without events between)
     lift_ms = float(bd_ms[binding.STAGE_NAMES.index("lift")] + bd_ms[binding.STAGE_NAMES.index("probe")])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")   # numbers of the committed ncu capture (profiles/r01_traffic.md)
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")   # numbers of the committed ncu capture (profiles/r02_traffic.md)
     tinfo = {}
     if os.path.exists(tpath):
         import csv
@@ -440,7 +440,7 @@ def run_ours(args):
                     "unit": "GB/s", "frac": (lift_gbs / pk["hbm_gbs"]) if lift_gbs else None,
                     "traffic": tinfo.get("lift_dram_bytes_per_launch"), "ms_per_launch": lift_ms, "bytes_per_launch": lift_bytes}
     # The lift kernel is bound by instruction issue, not by bytes: warp instructions per launch
-    # from the committed ncu capture (profiles/r01_traffic.csv), peak = 148 SMs x 4 schedulers x 1 instruction per clock
+    # from the committed ncu capture (profiles/r02_traffic.csv), peak = 148 SMs x 4 schedulers x 1 instruction per clock
     # at the maximum SM clock; time from the breakdown pass (kernel bracketed by events, similarity running beside it)
     lift_only_ms = float(bd_ms[binding.STAGE_NAMES.index("lift")])
     lift_inst = tinfo.get("lift_warp_instructions_per_launch")
