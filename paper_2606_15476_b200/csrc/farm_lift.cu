@@ -638,6 +638,7 @@ __global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_ker
 constexpr int PROBE_THREADS = 256;
 
 __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs a) {
+  __shared__ uint8_t s_pairs[PROBE_THREADS / 32][256];  // per warp: (record lane << 3 | sector) of the sectors with new voxels
   pdl_trigger();  // cand_associate may become resident behind this grid
   pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
   const uint32_t nq = min(m.counters[2], m.surv_cap);
@@ -676,17 +677,37 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
     uint32_t ev = 0;
     if (lane == 0) ev = atomicAdd(&m.counters[0], (uint32_t)__popc(act));
     ev = __shfl_sync(0xFFFFFFFFu, ev, 0) + __popc(act & ((1u << lane) - 1));
-    // ---- phase B: 4 records per step, 8 lanes (owner sectors) per record
-    const int sec = lane & 7;
+    // ---- phase B: one lane per (record, owner sector) that holds a new voxel.  The non-empty sectors of the warp's 32
+    // records are compacted (prefix sum of the per-record sector counts, list in shared memory), so that a round handles
+    // 32 of them whatever their spread over the records: a sparse warp (single-frame calls: a few real records among the
+    // padding of the queue) needs one round of dependent memory accesses, not one per group of four records.
+    uint32_t smask = 0;  // sectors (bytes of nb) with a new voxel
+#pragma unroll
+    for (int sc = 0; sc < 8; ++sc) smask |= ((uint32_t)(nb >> (8 * sc)) & 0xFFu) ? 1u << sc : 0u;
+    const uint32_t cnt_s = __popc(smask);
+    uint32_t incl = cnt_s;
+#pragma unroll
+    for (int sft = 1; sft < 32; sft <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, sft);
+      if (lane >= sft) incl += up;
+    }
+    const uint32_t n_pairs = __shfl_sync(0xFFFFFFFFu, incl, 31), off_s = incl - cnt_s;
+    uint8_t *plist = s_pairs[threadIdx.x >> 5];
+    {
+      uint32_t pos = off_s;
+      for (uint32_t sm = smask; sm; sm &= sm - 1) plist[pos++] = (uint8_t)((lane << 3) | (__ffs(sm) - 1));
+    }
+    __syncwarp();
     uint32_t pend_mine = 0;  // lane r: does record r have a voxel that was unowned at entry
 #pragma unroll 1
-    for (int step = 0; step < 8; ++step) {
-      if (((act >> (step * 4)) & 0xFu) == 0) continue;  // warp-uniform
-      const int src = step * 4 + (lane >> 3);
+    for (uint32_t p0 = 0; p0 < n_pairs; p0 += 32) {
+      const bool on = p0 + lane < n_pairs;
+      const uint32_t pr = on ? plist[p0 + lane] : 0u;
+      const int src = pr >> 3, sec = pr & 7;
       const unsigned long long rnb = __shfl_sync(0xFFFFFFFFu, nb, src);
       const uint32_t rslot = __shfl_sync(0xFFFFFFFFu, slot, src);
       const uint32_t rj = __shfl_sync(0xFFFFFFFFu, j, src);
-      const uint32_t byte = (uint32_t)(rnb >> (8 * sec)) & 0xFFu;
+      const uint32_t byte = on ? (uint32_t)(rnb >> (8 * sec)) & 0xFFu : 0u;
       uint32_t own[8];
       bool unowned = false;
       uint32_t o1 = NONE32, c1 = 0;  // first owner seen by this lane and how many of its voxels have it
@@ -742,9 +763,12 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
           }
         }
       }
+      // the sectors of record `lane` occupy list positions off_s .. off_s + cnt_s - 1: those that fall into this round
       const unsigned ub = __ballot_sync(0xFFFFFFFFu, unowned);
-      if ((lane >> 2) == step) pend_mine = (ub >> ((lane & 3) * 8)) & 0xFFu;
+      const int lo = max((int)off_s - (int)p0, 0), hi = min((int)(off_s + cnt_s) - (int)p0, 32);
+      if (hi > lo) pend_mine |= ub & ((hi - lo == 32 ? 0xFFFFFFFFu : ((1u << (hi - lo)) - 1u)) << lo);
     }
+    __syncwarp();  // the list is rewritten by the warp's next 32 records
     if (nb) {
       if (ev < m.pair_cap) {
         m.pl_bits[ev] = nb;
