@@ -337,7 +337,6 @@ constexpr int CAND_THREADS = 512, CAND_WARPS = CAND_THREADS / 32, CAND_PER = 4; 
 template <typename T>
 // 80 registers: 512 x 80 fits beside the similarity CTA (256 x 80) and the phase-1 dot products overlap its tail
 __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ DevMap m, const __grid_constant__ CallArgs a) {
-  __shared__ uint32_t warp_sum2[2][32];  // double buffered: one barrier per pass
   __shared__ uint32_t s_matches, s_skipped;
   __shared__ unsigned long long s_uvox;
   __shared__ bool s_last;
@@ -430,101 +429,119 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
   }
   __syncthreads();
   if (!s_last) return;
+  // Everything the decisions need except the dense row maxima is final once the last CTA is here (lift, probe and all
+  // candidate scores are done): request it BEFORE waiting for the similarity grid, so that only best_dense is loaded after.
+  unsigned long long pre_bc[CAND_PER];
+  uint32_t pre_npx[CAND_PER], pre_nv[CAND_PER];
+#pragma unroll
+  for (int k = 0; k < CAND_PER; ++k) {
+    const int j = k * CAND_THREADS + tid;
+    const bool in = j < a.M;
+    pre_bc[k] = in ? __ldcg(&m.best_cand[j]) : 0ull;
+    pre_npx[k] = in ? __ldcg(&m.det_npx[j]) : 0u;
+    pre_nv[k] = in ? __ldcg(&m.det_nv[j]) : 0u;
+  }
+  const unsigned long long pre_valid = tid == 0 ? __ldcg(&m.stats->valid_points) : 0ull;
   if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid before reading its row maxima
     if (tid == 0) spin_until(m.sim_done, a.sim_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
     __syncthreads();
   }
   pdl_trigger();  // the merge kernel becomes resident now, not while the similarity kernel still runs
-  __threadfence();
   if (m.corr) {  // U: union-find over the match graph instead of the per-detection argmax
     correspondence_decide(m, a, N);
     return;
   }
-  // Each thread decides CAND_PER consecutive detections; one pass (one barrier) per CAND_THREADS * CAND_PER detections.
+  // Each thread decides CAND_PER detections, CAND_THREADS apart (detection base + k * CAND_THREADS + tid), so that every
+  // load and store of the pass is coalesced over the warp; one pass (one barrier) per CAND_THREADS * CAND_PER detections.
+  // New ids in detection index order (R20): sub-block k of the pass comes before sub-block k + 1, warps in order inside
+  // a sub-block, lanes in order inside a warp.
+  __shared__ uint32_t wcnt[2][CAND_PER][CAND_WARPS];  // spawns per (sub-block, warp); double buffered over the passes
   uint32_t running = 0, n_matched = 0, n_skipped = 0, nv_sum = 0;  // running: spawns of the earlier passes (every thread)
   for (int base = 0; base < a.M; base += CAND_THREADS * CAND_PER) {
-    const int j0 = base + tid * CAND_PER;
     unsigned long long bc[CAND_PER], bd[CAND_PER];
     uint32_t npx[CAND_PER];
 #pragma unroll
     for (int k = 0; k < CAND_PER; ++k) {  // all loads of the pass up front
-      const bool in = j0 + k < a.M;
-      bc[k] = in ? __ldcg(&m.best_cand[j0 + k]) : 0ull;
-      bd[k] = in ? __ldcg(&m.best_dense[j0 + k]) : 0ull;
-      npx[k] = in ? __ldcg(&m.det_npx[j0 + k]) : 0u;
-      nv_sum += in ? __ldcg(&m.det_nv[j0 + k]) : 0u;
+      const int j = base + k * CAND_THREADS + tid;
+      const bool in = j < a.M;
+      bd[k] = in ? __ldcg(&m.best_dense[j]) : 0ull;
+      if (base == 0) {  // the first pass was requested before the wait
+        bc[k] = pre_bc[k], npx[k] = pre_npx[k], nv_sum += pre_nv[k];
+      } else {
+        bc[k] = in ? __ldcg(&m.best_cand[j]) : 0ull;
+        npx[k] = in ? __ldcg(&m.det_npx[j]) : 0u;
+        nv_sum += in ? __ldcg(&m.det_nv[j]) : 0u;
+      }
     }
     uint32_t spawn_bits = 0, match_bits = 0, skip_bits = 0;
     int32_t target[CAND_PER];
     float score[CAND_PER];
+    unsigned sb[CAND_PER];  // spawn ballots of the warp, per sub-block
+    uint32_t(*wc)[CAND_WARPS] = wcnt[(base / (CAND_THREADS * CAND_PER)) & 1];
 #pragma unroll
     for (int k = 0; k < CAND_PER; ++k) {
       target[k] = -1, score[k] = 0.f;
-      if (j0 + k >= a.M) continue;
-      if (npx[k] == 0) {
-        skip_bits |= 1u << k;  // R8
-        continue;
-      }
-      unsigned long long best = bc[k];
-      if (bd[k] && m.geom == 0) {
-        // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
-        const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd[k])));
-        const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd[k]) : 0u);
-        best = pd > best ? pd : best;
-      }
-      bool matched = false;
-      if (best) {
-        score[k] = unpack_score(best);
-        if (score[k] > m.tau) {  // strict (R18)
-          matched = true;
-          target[k] = (int32_t)unpack_id(best);
+      bool spawn = false;
+      if (base + k * CAND_THREADS + tid < a.M) {
+        if (npx[k] == 0) {
+          skip_bits |= 1u << k;  // R8
+        } else {
+          unsigned long long best = bc[k];
+          if (bd[k] && m.geom == 0) {
+            // objects without overlap have g = 0: score = w_geo*0 + w_sem*cos (R19)
+            const float sd = __fadd_rn(__fmul_rn(m.w_geo, 0.f), __fmul_rn(m.w_sem, unpack_score(bd[k])));
+            const unsigned long long pd = pack_score(sd, m.w_sem > 0.f ? unpack_id(bd[k]) : 0u);
+            best = pd > best ? pd : best;
+          }
+          bool matched = false;
+          if (best) {
+            score[k] = unpack_score(best);
+            if (score[k] > m.tau) {  // strict (R18)
+              matched = true;
+              target[k] = (int32_t)unpack_id(best);
+            }
+          }
+          if (matched) match_bits |= 1u << k; else spawn_bits |= 1u << k, spawn = true;
         }
       }
-      if (matched) match_bits |= 1u << k; else spawn_bits |= 1u << k;
+      sb[k] = __ballot_sync(0xFFFFFFFFu, spawn);
+      if (lane == 0) wc[k][warp] = __popc(sb[k]);
     }
-    // block exclusive scan of the spawn counts (detections are consecutive inside a thread, threads inside a warp)
-    const uint32_t mine = __popc(spawn_bits);
-    uint32_t incl = mine;
-#pragma unroll
-    for (int sft = 1; sft < 32; sft <<= 1) {
-      const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, sft);
-      if (lane >= sft) incl += up;
-    }
-    uint32_t *ws = warp_sum2[(base / (CAND_THREADS * CAND_PER)) & 1];
-    if (lane == 31) ws[warp] = incl;
     __syncthreads();
-    uint32_t wincl = lane < CAND_WARPS ? ws[lane] : 0u;
-#pragma unroll
-    for (int sft = 1; sft < 32; sft <<= 1) {
-      const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, wincl, sft);
-      if (lane >= sft) wincl += up;
-    }
-    const uint32_t total = __shfl_sync(0xFFFFFFFFu, wincl, 31);
-    const uint32_t before_warp = __shfl_sync(0xFFFFFFFFu, wincl, warp) - ws[warp];
-    uint32_t next_id = N + running + before_warp + (incl - mine);
+    uint32_t total = 0;
 #pragma unroll
     for (int k = 0; k < CAND_PER; ++k) {
-      const int j = j0 + k;
-      if (j >= a.M) continue;
-      uint32_t is_new = 0;
-      if ((spawn_bits >> k) & 1u) {
-        if (next_id < m.max_objects) {
-          target[k] = (int32_t)next_id;
-          is_new = 1;
-        } else {
-          atomicOr(m.err, ERR_OBJECT_CAPACITY);
-          skip_bits |= 1u << k;
+      // spawns before this thread's detection of sub-block k: earlier passes, earlier sub-blocks, earlier warps, earlier lanes
+      uint32_t before = 0, sub_total = 0;
+#pragma unroll
+      for (int w = 0; w < CAND_WARPS; ++w) {
+        const uint32_t c = wc[k][w];
+        before += w < warp ? c : 0u;
+        sub_total += c;
+      }
+      const int j = base + k * CAND_THREADS + tid;
+      if (j < a.M) {
+        uint32_t is_new = 0;
+        if ((spawn_bits >> k) & 1u) {
+          const uint32_t id = N + running + total + before + __popc(sb[k] & ((1u << lane) - 1));
+          if (id < m.max_objects) {
+            target[k] = (int32_t)id;
+            is_new = 1;
+          } else {
+            atomicOr(m.err, ERR_OBJECT_CAPACITY);
+            skip_bits |= 1u << k;
+          }
         }
-        ++next_id;
+        if (m.det_gm && ((match_bits >> k) & 1u)) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, target[k], npx[k]);  // G4
+        m.assoc[j] = target[k];
+        m.is_new[j] = (uint8_t)is_new;
+        m.best_score[j] = score[k];
+        if (target[k] >= 0) {
+          atomicMin(&m.leader[target[k]], (uint32_t)j);
+          atomicAdd(&m.grp_cnt[target[k]], 1u);
+        }
       }
-      if (m.det_gm && ((match_bits >> k) & 1u)) match_hellinger(m.det_gm, m.obj_gw, m.obj_gm, m.hell, m.eps2, j, target[k], npx[k]);  // G4
-      m.assoc[j] = target[k];
-      m.is_new[j] = (uint8_t)is_new;
-      m.best_score[j] = score[k];
-      if (target[k] >= 0) {
-        atomicMin(&m.leader[target[k]], (uint32_t)j);
-        atomicAdd(&m.grp_cnt[target[k]], 1u);
-      }
+      total += sub_total;
     }
     n_matched += __popc(match_bits), n_skipped += __popc(skip_bits);
     running += total;
@@ -549,7 +566,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
     m.stats->unique_voxels = pairs;
     atomicAdd(&m.totals->frames, (unsigned long long)a.F);
     atomicAdd(&m.totals->calls, 1ull);
-    atomicAdd(&m.totals->valid_points, __ldcg(&m.stats->valid_points));
+    atomicAdd(&m.totals->valid_points, pre_valid);
     atomicAdd(&m.totals->unique_voxels, pairs);
     atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
     atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
@@ -746,7 +763,21 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
     }
   };
   float ss = 0.f;
-  if (vec) {
+  // vector path with D <= 1024: the row is read ONCE (all loads in flight together) and kept in registers between the
+  // norm and the write-back -- one dependent round trip fewer on the critical tail of the call
+  const bool keep = vec && D <= 1024;
+  float kv[4][8];
+  if (keep) {
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+      const int i = lane * 8 + it * 256;
+      if (i < D) {
+        value8(i, kv[it]);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) ss = fmaf(kv[it][q], kv[it][q], ss);
+      }
+    }
+  } else if (vec) {
     for (int i = lane * 8; i < D; i += 256) {
       float v[8];
       value8(i, v);
@@ -764,22 +795,31 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
   if (ss > 0.f) {  // a zero sum keeps the old value
     const float inv = 1.0f / sqrtf(ss);
     float s2 = 0.f;
-    if (vec) {
+    auto store8 = [&](int i, float (&v)[8]) {
+      uint4 w;
+      T *e = reinterpret_cast<T *>(&w);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        v[q] *= inv;
+        e[q] = from_f32<T>(v[q]);  // round-to-nearest-even shadow (R1, R14)
+        const float sv = to_f32<T>(e[q]);
+        s2 = fmaf(sv, sv, s2);
+      }
+      *reinterpret_cast<float4 *>(master + i) = make_float4(v[0], v[1], v[2], v[3]);
+      *reinterpret_cast<float4 *>(master + i + 4) = make_float4(v[4], v[5], v[6], v[7]);
+      *reinterpret_cast<uint4 *>(shadow + i) = w;
+    };
+    if (keep) {
+#pragma unroll
+      for (int it = 0; it < 4; ++it) {
+        const int i = lane * 8 + it * 256;
+        if (i < D) store8(i, kv[it]);
+      }
+    } else if (vec) {
       for (int i = lane * 8; i < D; i += 256) {
         float v[8];
         value8(i, v);
-        uint4 w;
-        T *e = reinterpret_cast<T *>(&w);
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          v[q] *= inv;
-          e[q] = from_f32<T>(v[q]);  // round-to-nearest-even shadow (R1, R14)
-          const float sv = to_f32<T>(e[q]);
-          s2 = fmaf(sv, sv, s2);
-        }
-        *reinterpret_cast<float4 *>(master + i) = make_float4(v[0], v[1], v[2], v[3]);
-        *reinterpret_cast<float4 *>(master + i + 4) = make_float4(v[4], v[5], v[6], v[7]);
-        *reinterpret_cast<uint4 *>(shadow + i) = w;
+        store8(i, v);
       }
     } else {
       for (int i = lane; i < D; i += 32) {
