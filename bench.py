@@ -43,6 +43,7 @@ def parse():
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--overlap", type=int, default=1, help="0 = run similarity on the main stream (no lift || similarity overlap)")
     p.add_argument("--breakdown", action="store_true", help="bracket every kernel with CUDA events (perturbs `value`)")
+    p.add_argument("--sim-path", type=int, default=0, help="FARM_OPT_SIM_PATH: 0 auto, 2 tcgen05 single CTA, 3 tcgen05 CTA pairs")
     p.add_argument("--no-single-frame", action="store_true", help="skip the single-frame latency series of configs[0..3]")
     p.add_argument("--full-oracle-batch", action="store_true",
                    help="cpu_baseline / --impl reference: time ONE full 16-frame, 1600-detection batch (minutes on one core)")
@@ -255,7 +256,7 @@ def run_ours(args):
         m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
                     max_objects=max_objects, max_voxels=max_voxels, max_blocks=max_blocks, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
                     max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
-                    timing=timing, overlap=args.overlap)
+                    timing=timing, overlap=args.overlap, sim_path=args.sim_path)
         m.import_(objs, desc, keys, owner)
         return m
 

@@ -64,7 +64,7 @@ extern "C" {
 #define FARM_OPT_STREAM 7            /* cudaStream_t as integer, default 0 (legacy default stream)             */
 #define FARM_OPT_MAX_PAIRS_PER_CALL 8 /* distinct (detection, voxel) pairs per call; default = pixels per call  */
 #define FARM_OPT_MAX_FRAMES_PER_CALL 9 /* default 16, max 64                                                    */
-#define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path         */
+#define FARM_OPT_SIM_PATH 10         /* 0 auto, 1 force CUDA-core fp32 FMA, 2 force tcgen05 tensor path, 3 tcgen05 with CTA pairs (cta_group::2) */
 #define FARM_OPT_TIMING 11           /* 0 off; 1 CUDA events around the similarity kernel only; 2 around every kernel (this
                                         serialises the programmatically chained kernels).  May be changed at any time    */
 #define FARM_OPT_OVERLAP 12          /* 1 (default): similarity on an internal side stream, concurrent with lift+probe;

@@ -21,6 +21,7 @@ int run_query(const DevMap &m, cudaStream_t st, uint32_t N, const void *const em
 bool tc_prepare(void *tc_state, const DevMap &m, const CallArgs &a);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
+void tc_state_set_pair(void *, int pair);
 bool tc_supported(const DevMap &m);
 }  // namespace farm
 
@@ -466,6 +467,7 @@ int finalise_impl(farm_map *m) {
   }
   CU(cudaGetLastError());
   if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
+  if (m->tc && m->sim_path == 3) tc_state_set_pair(m->tc, 1);
   if (m->overlap) {
     int prio_lo = 0, prio_hi = 0;
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -473,7 +475,7 @@ int finalise_impl(farm_map *m) {
     CU(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
     CU(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
   }
-  if (m->sim_path == 2 && !m->tc) return fail(FARM_ERR_INVALID_ARG, "tensor-core similarity path not available for this dtype / D");
+  if (m->sim_path >= 2 && !m->tc) return fail(FARM_ERR_INVALID_ARG, "tensor-core similarity path not available for this dtype / D");
   m->finalised = true;
   return FARM_OK;
 }
@@ -588,7 +590,7 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       m->max_frames = v;
       break;
     case FARM_OPT_SIM_PATH:
-      if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad SIM_PATH");
+      if (v < 0 || v > 3) return fail(FARM_ERR_INVALID_ARG, "bad SIM_PATH");
       m->sim_path = (int)v;
       break;
     case FARM_OPT_OVERLAP:

@@ -51,8 +51,9 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done;
+  uint32_t done, polls = 0;
   do {
+    if (++polls == (1u << 28)) __trap();  // a protocol error must end the kernel, not hang the device
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -70,6 +71,47 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
       "l"(map), "r"(bar), "r"(c0), "r"(c1)
       : "memory");
 }
+// ---- CTA-pair (cta_group::2) variants: a cluster of two CTAs computes a 256 x 256 tile, each CTA loading its own 128 rows of
+// A and HALF of the B tile (the tensor cores of the pair share B), all transfers signalling the leader CTA's barrier
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t leader_addr(uint32_t local) {  // the same location in the shared memory of cluster rank 0
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, 0;" : "=r"(r) : "r"(local));
+  return r;
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap *map, uint32_t leader_bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+      "l"(map), "r"(leader_bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {  // arrives on the barrier at this offset in BOTH CTAs
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+               "h"((uint16_t)3)
+               : "memory");
+}
+
 __device__ __forceinline__ void tcgen05_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tcgen05_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
@@ -111,20 +153,29 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // 80 registers per thread (no spills): 256 x 80 leaves room for four 128 x 80 lift CTAs on the same SM
-template <bool EMIT>  // EMIT: pairs whose cosine exceeds m.dense_thr also go to the dense list (H1 prefilter / U1 edges)
+// NCTA = 2: CTA pairs (cluster of 2, tcgen05 cta_group::2, UMMA 256 x 256 x 16): per stage a CTA holds its A tile and half
+// of the B tile (32 KB instead of 48 KB: six stages instead of four in the same shared memory, a third less L2 traffic).
+template <bool EMIT, int NCTA>  // EMIT: pairs whose cosine exceeds m.dense_thr also go to the dense list (H1 prefilter / U1 edges)
 __global__ void __maxnreg__(80)
 similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
                      int M, uint32_t idesc, uint32_t prep_target) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // SWIZZLE_128B needs 1024-byte alignment
+  constexpr int NSTAGES = NCTA == 2 ? 6 : STAGES;
+  constexpr uint32_t B_LOAD_BYTES = B_BYTES / NCTA;              // B rows this CTA loads per stage
+  constexpr uint32_t STG_BYTES = A_BYTES + B_LOAD_BYTES;         // 48 KB, or 32 KB for a CTA of a pair
+  static_assert(NSTAGES * STG_BYTES == STAGES * STAGE_BYTES, "both variants use the same shared memory");
   float *ib_s = (float *)(smem + STAGES * STAGE_BYTES);                         // [2][BLOCK_N] inverse norms of B
   uint64_t *bars = (uint64_t *)(ib_s + 2 * BLOCK_N);
-  uint64_t *full_bar = bars, *empty_bar = bars + STAGES, *tfull_bar = bars + 2 * STAGES, *tempty_bar = bars + 2 * STAGES + 2;
-  uint32_t *tmem_slot = (uint32_t *)(bars + 2 * STAGES + 4);
+  uint64_t *full_bar = bars, *empty_bar = bars + NSTAGES, *tfull_bar = bars + 2 * NSTAGES, *tempty_bar = bars + 2 * NSTAGES + 2;
+  uint32_t *tmem_slot = (uint32_t *)(bars + 2 * NSTAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int N = (int)*m.n_objects;
-  const int tiles_m = (M + BLOCK_M - 1) / BLOCK_M, tiles_n = (N + BLOCK_N - 1) / BLOCK_N;
+  const int rank = NCTA == 2 ? (int)cluster_ctarank() : 0;       // rank 0 = leader: issues the MMAs of the pair
+  const int unit = blockIdx.x / NCTA, n_units = gridDim.x / NCTA; // a unit = one CTA, or one CTA pair
+  // tiles_m counts tiles of BLOCK_M * NCTA rows; CTA `rank` of a pair owns rows [tm * 256 + rank * 128, + 128)
+  const int tiles_m = (M + BLOCK_M * NCTA - 1) / (BLOCK_M * NCTA), tiles_n = (N + BLOCK_N - 1) / BLOCK_N;
   const int n_tiles = tiles_m * tiles_n;
   const int k_blocks = (m.D + BLOCK_K - 1) / BLOCK_K;
 
@@ -133,22 +184,28 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     asm volatile("prefetch.tensormap [%0];" ::"l"(&map_b) : "memory");
   }
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < STAGES; ++i) {
+    for (int i = 0; i < NSTAGES; ++i) {
       mbar_init(smem_u32(&full_bar[i]), 1);
       mbar_init(smem_u32(&empty_bar[i]), 1);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&tfull_bar[i]), 1);
-      mbar_init(smem_u32(&tempty_bar[i]), EPI_THREADS / 32);
+      mbar_init(smem_u32(&tempty_bar[i]), NCTA * EPI_THREADS / 32);  // the epilogue warps of BOTH CTAs of a pair
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(TMEM_COLS));
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    if (NCTA == 2) {  // issued by the same warp of both CTAs of the pair
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(TMEM_COLS));
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(TMEM_COLS));
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
   }
   tcgen05_fence_before();
   __syncthreads();
+  if (NCTA == 2) cluster_sync_all();  // the peer's barriers are initialised before anything signals them
   tcgen05_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
@@ -156,41 +213,53 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     // ===== TMA producer =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int tile = unit; tile < n_tiles; tile += n_units) {
         const int tm = tile % tiles_m, tn = tile / tiles_m;
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
           const uint32_t fb = smem_u32(&full_bar[stage]);
-          mbar_expect_tx(fb, STAGE_BYTES);
-          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES);
-          tma_load_2d(sa, &map_a, fb, kb * BLOCK_K, tm * BLOCK_M);
-          tma_load_2d(sa + A_BYTES, &map_b, fb, kb * BLOCK_K, tn * BLOCK_N);
-          if (++stage == STAGES) stage = 0, phase ^= 1;
+          const uint32_t sa = smem_u32(smem + stage * STG_BYTES);
+          if (NCTA == 2) {
+            // the leader's barrier collects the bytes of both CTAs; the peer only issues its loads
+            if (rank == 0) mbar_expect_tx(fb, 2 * STG_BYTES);
+            const uint32_t lb = fb & 0xFEFFFFFFu;  // shared::cluster address of the same barrier in the pair's even CTA
+            tma_load_2d_pair(sa, &map_a, lb, kb * BLOCK_K, (tm * NCTA + rank) * BLOCK_M);
+            tma_load_2d_pair(sa + A_BYTES, &map_b, lb, kb * BLOCK_K, tn * BLOCK_N + rank * (BLOCK_N / NCTA));
+          } else {
+            mbar_expect_tx(fb, STG_BYTES);
+            tma_load_2d(sa, &map_a, fb, kb * BLOCK_K, tm * BLOCK_M);
+            tma_load_2d(sa + A_BYTES, &map_b, fb, kb * BLOCK_K, tn * BLOCK_N);
+          }
+          if (++stage == NSTAGES) stage = 0, phase ^= 1;
         }
       }
     }
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (lane == 0) {
+    if (lane == 0 && rank == 0) {  // a pair's MMAs are issued by its leader CTA alone
       uint32_t stage = 0, phase = 0, as = 0, aphase = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);  // epilogue has drained this accumulator
+      for (int tile = unit; tile < n_tiles; tile += n_units) {
+        mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);  // epilogue has drained this accumulator (in both CTAs of a pair)
         tcgen05_fence_after();
         const uint32_t tmem_d = tmem_base + as * BLOCK_N;
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(smem_u32(&full_bar[stage]), phase);
           tcgen05_fence_after();
-          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES);
+          const uint32_t sa = smem_u32(smem + stage * STG_BYTES);
           const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
             // advance 32 bytes (16 elements) along K inside the 128-byte swizzle row: +2 in 16-byte units
-            umma_f16(tmem_d, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+            if (NCTA == 2)
+              umma_f16_pair(tmem_d, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+            else
+              umma_f16(tmem_d, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
           }
-          umma_commit(smem_u32(&empty_bar[stage]));  // frees the smem stage when these MMAs retire
-          if (++stage == STAGES) stage = 0, phase ^= 1;
+          // frees the smem stage (in both CTAs of a pair) when these MMAs retire
+          if (NCTA == 2) umma_commit_pair(smem_u32(&empty_bar[stage])); else umma_commit(smem_u32(&empty_bar[stage]));
+          if (++stage == NSTAGES) stage = 0, phase ^= 1;
         }
-        umma_commit(smem_u32(&tfull_bar[as]));  // accumulator complete
+        if (NCTA == 2) umma_commit_pair(smem_u32(&tfull_bar[as])); else umma_commit(smem_u32(&tfull_bar[as]));  // accumulator complete
         if (++as == 2) as = 0, aphase ^= 1;
       }
     }
@@ -204,8 +273,9 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     // prep_kernel (main stream) may still be running: its row norms and the zeroed best_dense words are first
     // needed here, one tile of MMAs after the kernel started
     spin_until(m.prep_done, prep_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      const int tm = tile % tiles_m, tn = tile / tiles_m;
+    const uint32_t tempty_leader0 = NCTA == 2 ? leader_addr(smem_u32(&tempty_bar[0])) : 0u;
+    for (int tile = unit; tile < n_tiles; tile += n_units) {
+      const int tm = (tile % tiles_m) * NCTA + rank, tn = tile / tiles_m;
       const int n0 = tn * BLOCK_N;
       const int ncols = min(BLOCK_N, N - n0);
       float *ib = ib_s + as * BLOCK_N;
@@ -279,7 +349,9 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
       }
       tcgen05_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+      if (lane == 0) {
+        if (NCTA == 2) mbar_arrive_remote(tempty_leader0 + as * 8u); else mbar_arrive(smem_u32(&tempty_bar[as]));
+      }
       if (row_ok) {
         cs = fminf(1.f, fmaxf(-1.f, cs));                    // R15 clamp
         if (ia == 0.f) cs = 0.f, best_c = 0;                 // zero-norm detection: cos = 0 for every object
@@ -292,9 +364,13 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
   __threadfence();  // the epilogue's atomicMax results precede the completion count below
   __syncthreads();
   if (threadIdx.x == 0) atomicAdd(m.sim_done, 1u);  // cand_associate's decision scan waits for every CTA of this grid
+  if (NCTA == 2) cluster_sync_all();  // no CTA of a pair leaves (or frees TMEM) while its peer still uses the pair's resources
   if (warp == 2) {
     tcgen05_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS));
+    if (NCTA == 2)
+      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS));
+    else
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS));
   }
 }
 
@@ -305,6 +381,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 struct TcState {
   EncodeTiledFn encode = nullptr;
   CUtensorMap map_a, map_b;  // map_a is re-encoded per call by tc_prepare (host work only)
+  CUtensorMap map_b_half;    // CTA pairs: each CTA loads half of the B tile
+  uint32_t idesc_pair = 0;
+  int pair = 0;              // 1: launch CTA pairs (cluster of 2, cta_group::2)
   CUtensorMapDataType dt;
   uint32_t idesc;
   bool ok = false;
@@ -338,12 +417,16 @@ void *tc_state_create(const DevMap &m) {
   const uint32_t fmt = m.dtype == FARM_DTYPE_F16 ? 0u : 1u;
   // instruction descriptor, kind::f16: D = fp32, A/B = fmt, both K-major, N = 256, M = 128
   st->idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(BLOCK_M >> 4) << 24);
-  if (!encode_2d(st, &st->map_b, m.desc_shadow, m.max_objects, (uint64_t)m.D, BLOCK_N)) {
+  st->idesc_pair = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)((2 * BLOCK_M) >> 4) << 24);
+  if (!encode_2d(st, &st->map_b, m.desc_shadow, m.max_objects, (uint64_t)m.D, BLOCK_N) ||
+      !encode_2d(st, &st->map_b_half, m.desc_shadow, m.max_objects, (uint64_t)m.D, BLOCK_N / 2)) {
     delete st;
     return nullptr;
   }
-  if (cudaFuncSetAttribute(similarity_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
-      cudaFuncSetAttribute(similarity_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
+  if (cudaFuncSetAttribute(similarity_tc_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
     delete st;
     return nullptr;
   }
@@ -352,6 +435,7 @@ void *tc_state_create(const DevMap &m) {
 }
 
 void tc_state_destroy(void *p) { delete (TcState *)p; }
+void tc_state_set_pair(void *p, int pair) { ((TcState *)p)->pair = pair; }
 
 // Encode the call's A operand (detection rows).  Called before anything of the call is enqueued, so that a
 // descriptor pointer TMA cannot address (not 16-byte aligned) fails the call with the map untouched.
@@ -367,12 +451,28 @@ int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, c
   TcState *st = (TcState *)state;
   if (a.M == 0 || n_upper == 0) return 0;
   const CUtensorMap &map_a = st->map_a;
-  const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
-  const int grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
-  if (m.dense_d && m.dense_thr < 2.0f)
-    similarity_tc_kernel<true><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
-  else
-    similarity_tc_kernel<false><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+  const bool emit = m.dense_d && m.dense_thr < 2.0f;
+  int grid;
+  if (st->pair) {  // CTA pairs: one cluster of two CTAs per 256 x 256 tile
+    const long long tiles = (long long)((a.M + 2 * BLOCK_M - 1) / (2 * BLOCK_M)) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
+    grid = 2 * (int)(tiles < m.num_sms / 2 ? tiles : m.num_sms / 2);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid), cfg.blockDim = dim3(TC_THREADS), cfg.dynamicSmemBytes = SMEM_BYTES, cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2, attr[0].val.clusterDim.y = 1, attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr, cfg.numAttrs = 1;
+    const cudaError_t e = emit ? cudaLaunchKernelEx(&cfg, similarity_tc_kernel<true, 2>, map_a, st->map_b_half, m, a.M, st->idesc_pair, prep_target)
+                               : cudaLaunchKernelEx(&cfg, similarity_tc_kernel<false, 2>, map_a, st->map_b_half, m, a.M, st->idesc_pair, prep_target);
+    if (e != cudaSuccess) return -1;
+  } else {
+    const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
+    grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
+    if (emit)
+      similarity_tc_kernel<true, 1><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+    else
+      similarity_tc_kernel<false, 1><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+  }
   if (n_ctas) *n_ctas = grid;
   return 1;
 }

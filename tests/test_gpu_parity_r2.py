@@ -57,8 +57,9 @@ def _stress_frames_with_far_matches(sc, b, desc_map, rng):
     return out
 
 
+@pytest.mark.parametrize("sim_path", [2, 3])
 @pytest.mark.parametrize("w", WEIGHTS)
-def test_dense_argmax_decides_multi_tile_tensor_path(oracle, w):
+def test_dense_argmax_decides_multi_tile_tensor_path(oracle, w, sim_path):
     """M = 400 detections x N >= 700 objects, D = 1024 bf16: more than one tile on both axes of similarity_tc_kernel
     (128 x 256); half of the detections can only match through the dense argmax."""
     from paper_2606_15476_b200.binding import OBJECT_DTYPE
@@ -68,7 +69,7 @@ def test_dense_argmax_decides_multi_tile_tensor_path(oracle, w):
     keys = pack_key(ijk[:, 0], ijk[:, 1], ijk[:, 2])
     objs = np.zeros(len(n_vox), OBJECT_DTYPE)
     objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(len(n_vox)), n_vox, 1, -1, -1
-    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, sim_path=2)
+    o, g = make_pair(oracle, cfg, max_det_per_call=1600, max_objects=len(n_vox) + 8000, sim_path=sim_path)
     assert o.import_(objs, desc, keys, owner) == 0
     g.import_(objs, desc, keys, owner)
     rng = np.random.default_rng(17)
@@ -102,7 +103,7 @@ def test_dense_argmax_decides_fma_and_small_tensor_paths(oracle, w, cfg_id, sim_
     assert rows > 50
 
 
-@pytest.mark.parametrize("dtype,sim_path", [(0, 0), (1, 1), (1, 2), (2, 1), (2, 2)])
+@pytest.mark.parametrize("dtype,sim_path", [(0, 0), (1, 1), (1, 2), (2, 1), (2, 2), (1, 3), (2, 3)])
 def test_exact_ties_go_to_the_lowest_id(oracle, dtype, sim_path):
     """R18 with bit-identical map rows (same tile, neighbouring tiles, far tiles of the 128 x 256 tensor tiling) and
     detections equal to them: cosine clamps to exactly 1 for all of them and the lowest id must win -- in the dense
