@@ -115,3 +115,43 @@ int main(void) {
     out = subprocess.run([str(exe)], capture_output=True, text=True)
     assert out.returncode == 0, out
     assert out.stdout.strip() == f"bad dtype|{binding.OBJECT_DTYPE.itemsize}"
+
+
+def test_round2_options_and_calls_validate_on_the_host(lib):
+    """The options and entry points added in round 2 validate their host-visible arguments without a device; calls that
+    need an option that is off fail with FARM_ERR_STATE."""
+    from paper_2606_15476_b200 import FarmError, FarmMap, binding
+    m = FarmMap(0.05, 8, 0.5, 0.5, 0.5, H=8, W=8)
+    for key, bad in ((binding.OPT_VIEWS, 9), (binding.OPT_VIEWS, -1), (binding.OPT_CORRESPONDENCE, 2), (binding.OPT_GEOMETRY, 2),
+                     (binding.OPT_SIM_PATH, 4)):
+        with pytest.raises(FarmError):
+            m.set_option_i(key, bad)
+    for key, good in ((binding.OPT_VIEWS, 4), (binding.OPT_CORRESPONDENCE, 1), (binding.OPT_GEOMETRY, 1), (binding.OPT_SIM_PATH, 3)):
+        m.set_option_i(key, good)
+    for key in (binding.OPTF_VIEW_COS, binding.OPTF_VIEW_CLOSER, binding.OPTF_PREFILTER_COS, binding.OPTF_HELLINGER_BUDGET):
+        m.set_option_f(key, 0.5)
+        with pytest.raises(FarmError):
+            m.set_option_f(key, float("nan"))
+    with pytest.raises(FarmError):
+        m.set_frame_seq(-1)
+    m.set_frame_seq(5)
+    assert m.get_frame_seq() == 5
+    with pytest.raises(FarmError) as ei:
+        m.set_frame_seq(4)                                   # only forward
+    assert ei.value.code == -4
+    m.destroy()
+    m2 = FarmMap(0.05, 8, 0.5, 0.5, 0.5, H=8, W=8)
+    for call in (m2.read_alias, m2.last_merges, m2.read_views):
+        with pytest.raises(FarmError) as ei:
+            call()                                           # option off
+        assert ei.value.code == -4
+    import numpy as np
+    lib_ = binding.load_library()
+    q = np.zeros(32, np.float32)
+    rc = lib_.farm_map_query(m2._h, None, None, None, 8, 8, 8, 0, None, q.ctypes.data, -1, 0, None, None, 1, None, None, None, None, None, None)
+    assert rc == binding.ERR_INVALID_ARG                     # NULL embeddings
+    one = np.zeros(8, np.float32)
+    rc = lib_.farm_map_query(m2._h, one.ctypes.data, one.ctypes.data, one.ctypes.data, 8, 8, 8, 0, None, q.ctypes.data, -1, 7, None, None, 1,
+                             None, None, None, None, None, None)
+    assert rc == binding.ERR_INVALID_ARG                     # too many predicates
+    m2.destroy()

@@ -533,3 +533,44 @@ def test_hellinger_geometry_decisions(oracle, cfg_id, n, per_call, corr):
             _compare_corr(g, o)
     compare_maps(g, o)
     assert matched > 10
+
+
+def test_retrieval_skips_absorbed_entities(oracle):
+    """Q1: only live entities are ranked.  On the split-map scene (correspondence on, several merges) the dead ids get
+    rank / score 0 on both sides and the ranks of the live ones close up."""
+    import torch
+    from test_oracle_next import split_map_arrays
+    cfg = _with_weights(S.get_config(0), (0.7, 0.3, 0.25))
+    sc = S.BoxScene(cfg)
+    plain = oracle.OracleMap(cfg.voxel, cfg.D, 0.5, 0.5, 0.5, cfg.dtype, cfg.H, cfg.W)
+    for k in range(9):
+        fr = sc.frame(k)
+        plain.integrate(fr.depth, fr.mask, fr.K, fr.T, fr.desc, fr.n_det)
+    arrays = split_map_arrays(*plain.read())
+    o, g = make_pair(oracle, cfg, correspondence=1)
+    o.set_option(o.OPT_CORRESPONDENCE, 1)
+    assert o.import_(*arrays) == 0
+    g.import_(*arrays)
+    for call in range(3, 6):
+        frames = margin_filter(o.clone, [sc.frame(3 * call + i) for i in range(3)], cfg.tau, all_pairs=True)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+    objs_o, _, _, _ = o.read(voxels=False)
+    alive = (objs_o["n_obs"] > 0).astype(np.uint8)
+    N = len(alive)
+    assert 0 < alive.sum() < N                                     # some entities were absorbed
+    cen = (0.5 * (objs_o["aabb_min"].astype(np.float64) + objs_o["aabb_max"].astype(np.float64))).astype(np.float32)
+    cen[alive == 0] = 0
+    rng = np.random.default_rng(2)
+    dims, nnz = (32, 32, 32), (12, 12, 12)
+    emb = [_ternary_rows(N, d, z, rng) for d, z in zip(dims, nnz)]
+    emb_dev = [torch.from_numpy(e).to("cuda").contiguous() for e in emb]
+    live_ids = np.nonzero(alive)[0]
+    lm = int(live_ids[len(live_ids) // 2])
+    qt = [_ternary_rows(1, 32, 12, rng)[0] for _ in range(4)]
+    ql = [[emb[0][lm], emb[0][lm], emb[1][lm], emb[2][lm]]]
+    ro = oracle.query(alive, emb, np.zeros(N, np.int32), cen, qt, -1, [oracle.PRED_NEXTTO], ql, 5)
+    rg = g.query(emb_dev, 0, None, qt, -1, [oracle.PRED_NEXTTO], ql, 5)
+    assert np.array_equal(rg["landmarks"], ro["landmarks"])
+    assert np.abs(rg["s_sem"] - ro["s_sem"]).max() <= 1e-6 and np.abs(rg["s"] - ro["s"]).max() <= 1e-6
+    assert (rg["s"][alive == 0] == 0).all() and (rg["top"] >= 0).all() and alive[rg["top"]].all()
