@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- mapping throughput of the FARM hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--sim-path 0|2|3]
+                    [--full-oracle-batch] [--no-single-frame] [--no-e2e] [--no-cpu-baseline]
 
 Workload (N=1 and every rank of N>1): BASELINE.json configs[4], the batched throughput stress -- a map
 pre-populated with 50,000 objects (random connected voxel blobs, mean ~2,000 voxels at 2.5 cm, D=1024 bf16
