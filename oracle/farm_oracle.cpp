@@ -123,6 +123,11 @@ struct Map {
   float voxel_size, inv_vs, w_geo, w_sem, tau, z_min, z_max;
   int D, dtype, H, W;
   // options (oracle_set_option); all off by default
+  int edges_k = 0;               // W: weighted covisibility edges over a kNN graph in Hellinger distance (0 = off)
+  float edge_decay = 0.9f;       // W4: temporal decay per call
+  float edge_cutoff = 2.0f;      // W3: soft median cutoff, as a multiple of the median kNN distance
+  long long call_index = 0;      // integrate calls so far (W4: the clock of the decay)
+  std::map<std::pair<int, int>, std::pair<double, long long>> edges;  // W4: {a < b} -> (weight, call of the last update)
   int opt_corr = 0;              // U: union-find correspondence with entity-entity merges
   int opt_geom = 0;              // H: 0 = voxel overlap (BASELINE.json rule), 1 = Hellinger distance between Gaussians
   float prefilter_cos = 0.5f;    // H1: candidates are the entities with cos > prefilter_cos
@@ -190,6 +195,28 @@ double hellinger(const double mu1[3], const double c1[6], const double mu2[3], c
   const double bc = std::pow(d1, 0.25) * std::pow(d2, 0.25) / std::sqrt(db) * std::exp(-0.125 * q);
   const double h2 = 1.0 - bc;
   return h2 > 0.0 ? std::sqrt(h2) : 0.0;
+}
+
+// W2: Bhattacharyya distance DB = 1/8 dmu^T Sbar^-1 dmu + 1/2 ln(|Sbar| / sqrt(|S1| |S2|)) of the same regularised
+// Gaussians.  The Hellinger distance is a strictly increasing function of it, H = sqrt(1 - exp(-DB)), so "nearest in
+// Hellinger distance" and "nearest in DB" are the same order -- but H rounds to 1 for every pair more than a few object
+// sizes apart, where DB still separates them.
+double bhattacharyya(const double mu1[3], const double c1[6], const double mu2[3], const double c2[6], double eps2) {
+  double s1[6], s2[6], sb[6];
+  for (int k = 0; k < 6; ++k) {
+    const double reg = (k == 0 || k == 3 || k == 5) ? eps2 : 0.0;
+    s1[k] = c1[k] + reg;
+    s2[k] = c2[k] + reg;
+    sb[k] = 0.5 * (s1[k] + s2[k]);
+  }
+  const double d1 = det3(s1), d2 = det3(s2), db = det3(sb);
+  const double inv[6] = {(sb[3] * sb[5] - sb[4] * sb[4]) / db, (sb[2] * sb[4] - sb[1] * sb[5]) / db,
+                         (sb[1] * sb[4] - sb[2] * sb[3]) / db, (sb[0] * sb[5] - sb[2] * sb[2]) / db,
+                         (sb[1] * sb[2] - sb[0] * sb[4]) / db, (sb[0] * sb[3] - sb[1] * sb[1]) / db};
+  const double d[3] = {mu1[0] - mu2[0], mu1[1] - mu2[1], mu1[2] - mu2[2]};
+  const double q = d[0] * (inv[0] * d[0] + inv[1] * d[1] + inv[2] * d[2]) + d[1] * (inv[1] * d[0] + inv[3] * d[1] + inv[4] * d[2]) +
+                   d[2] * (inv[2] * d[0] + inv[4] * d[1] + inv[5] * d[2]);
+  return 0.125 * q + 0.5 * std::log(db / std::sqrt(d1 * d2));
 }
 
 // R5 (BASELINE.json "same fp32 operation order and FMA contraction disabled"):
@@ -360,6 +387,9 @@ int oracle_set_option(void *h, int key, double v) {
     case 5: m.views_k = (int)v; return 0;
     case 6: m.view_cos = (float)v; return 0;
     case 7: m.view_closer = (float)v; return 0;
+    case 8: m.edges_k = (int)v; return 0;
+    case 9: m.edge_decay = (float)v; return 0;
+    case 10: m.edge_cutoff = (float)v; return 0;
   }
   return -1;
 }
@@ -763,6 +793,45 @@ int oracle_integrate_batch(void *h, int F, const float *depth, const uint16_t *m
       for (int b : seen)
         if (a != b) m.covis[a][(size_t)b >> 6] |= 1ull << (b & 63);
   }
+  // W1-W4 ("a parallel weighted edge dictionary accumulates their co-occurrence, restricted to spatially
+  // proximal pairs (a k-nearest-neighbor graph in Gaussian Hellinger distance with a soft median cutoff) and discounted
+  // by a temporal decay").  Readings (none of the constants is printed):
+  //   W1 S = the distinct entities that received a detection in this call (they all carry a Gaussian afterwards);
+  //   W2 N_k(a) = the k entities of S \ {a} nearest to a in Hellinger distance between the entity Gaussians after this
+  //      call's merge, ordered through the Bhattacharyya distance d = DB (fp32; H = sqrt(1 - exp(-DB)) is increasing
+  //      in it and saturates at 1 in floating point where DB still separates pairs), ties -> lower id;
+  //   W3 "soft median cutoff": b in N_k(a) is kept iff d(a, b) <= cutoff * (lower median of a's kNN distances);
+  //   W4 every unordered pair {a, b} with b kept for a or a kept for b: w <- w * decay^(calls since its last update) + 1.
+  m.call_index++;
+  if (m.edges_k > 0) {
+    std::set<int> seen;
+    for (int j = 0; j < M; ++j)
+      if (target[j] >= 0 && m.objs[target[j]].gW > 0.0) seen.insert(target[j]);
+    std::vector<int> S(seen.begin(), seen.end());
+    std::set<std::pair<int, int>> touched;
+    for (int a : S) {
+      double mu_a[3], c_a[6];
+      gaussian_from_moments(m.objs[a].gW, m.objs[a].gM1, m.objs[a].gM2, mu_a, c_a);
+      std::vector<std::pair<float, int>> dist;
+      for (int b : S) {
+        if (b == a) continue;
+        double mu_b[3], c_b[6];
+        gaussian_from_moments(m.objs[b].gW, m.objs[b].gM1, m.objs[b].gM2, mu_b, c_b);
+        dist.push_back({(float)bhattacharyya(mu_a, c_a, mu_b, c_b, eps2), b});
+      }
+      std::sort(dist.begin(), dist.end());  // by distance, then by id
+      const size_t kk = std::min<size_t>((size_t)m.edges_k, dist.size());
+      if (kk == 0) continue;
+      const float med = dist[(kk - 1) / 2].first;
+      for (size_t i = 0; i < kk; ++i)
+        if (dist[i].first <= m.edge_cutoff * med) touched.insert({std::min(a, dist[i].second), std::max(a, dist[i].second)});
+    }
+    for (auto &e : touched) {
+      auto &rec = m.edges[e];
+      rec.first = rec.first * std::pow((double)m.edge_decay, (double)(m.call_index - rec.second)) + 1.0;
+      rec.second = m.call_index;
+    }
+  }
   m.frame_seq += F;
   return 0;
 }
@@ -933,6 +1002,18 @@ void oracle_last_tau_gap(void *h, float *gap) {
   Map &m = *(Map *)h;
   for (int j = 0; j < m.M; ++j) gap[j] = m.tau_gap[j];
 }
+// W: the weighted edges, weights decayed to the current call count; a < b; ascending (a, b).  Returns their number.
+long long oracle_read_edges(void *h, int32_t *a, int32_t *b, float *w) {
+  Map &m = *(Map *)h;
+  long long n = 0;
+  for (auto &kv : m.edges) {
+    if (a) a[n] = kv.first.first;
+    if (b) b[n] = kv.first.second;
+    if (w) w[n] = (float)(kv.second.first * std::pow((double)m.edge_decay, (double)(m.call_index - kv.second.second)));
+    ++n;
+  }
+  return n;
+}
 // U4: alias[o] = o for a live entity, else the live entity that (transitively) absorbed it
 void oracle_read_alias(void *h, int32_t *alias) {
   Map &m = *(Map *)h;
@@ -1093,6 +1174,9 @@ int oracle_query(int N, const uint8_t *alive, const float *emb0, const float *em
   return 0;
 }
 
+double oracle_bhattacharyya(const double *mu1, const double *cov1, const double *mu2, const double *cov2, double eps2) {
+  return bhattacharyya(mu1, cov1, mu2, cov2, eps2);
+}
 double oracle_hellinger(const double *mu1, const double *cov1, const double *mu2, const double *cov2, double eps2) {
   return hellinger(mu1, cov1, mu2, cov2, eps2);
 }

@@ -64,6 +64,7 @@ class OracleMap:
 
     # ---- round-2 options (all off by default): U correspondence, H geometry, V views
     OPT_CORRESPONDENCE, OPT_GEOMETRY, OPT_PREFILTER_COS, OPT_HELLINGER_BUDGET, OPT_VIEWS_K, OPT_VIEW_COS, OPT_VIEW_CLOSER = 1, 2, 3, 4, 5, 6, 7
+    OPT_EDGES_K, OPT_EDGE_DECAY, OPT_EDGE_CUTOFF = 8, 9, 10
 
     def set_option(self, key, value):
         rc = lib().oracle_set_option(self.h, C.c_int(key), C.c_double(value))
@@ -77,6 +78,14 @@ class OracleMap:
         gap = np.zeros(M, np.float32)
         lib().oracle_last_tau_gap(self.h, _p(gap))
         return gap
+
+    def read_edges(self):
+        """W: (a [n], b [n], w [n]) weighted covisibility edges, a < b, ascending, weights decayed to now."""
+        lib().oracle_read_edges.restype = C.c_longlong
+        n = lib().oracle_read_edges(self.h, None, None, None)
+        a, b, w = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.float32)
+        lib().oracle_read_edges(self.h, _p(a), _p(b), _p(w))
+        return a, b, w
 
     def read_alias(self):
         """U4: alias [N]: the live entity every id now stands for (itself while alive)."""
@@ -237,6 +246,14 @@ def hellinger(mu1, cov1, mu2, cov2, eps2):
     """G3: Hellinger distance of two 3-D Gaussians; cov packed xx xy xz yy yz zz; eps2 added to the diagonals."""
     a = [np.ascontiguousarray(x, np.float64) for x in (mu1, cov1, mu2, cov2)]
     return float(lib().oracle_hellinger(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), C.c_double(eps2)))
+
+
+def bhattacharyya(mu1, cov1, mu2, cov2, eps2):
+    """W2: Bhattacharyya distance of two 3-D Gaussians (H = sqrt(1 - exp(-DB))); cov packed xx xy xz yy yz zz."""
+    lib().oracle_bhattacharyya.restype = C.c_double
+    lib().oracle_bhattacharyya.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
+    a = [np.ascontiguousarray(x, np.float64) for x in (mu1, cov1, mu2, cov2)]
+    return float(lib().oracle_bhattacharyya(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), C.c_double(eps2)))
 
 
 def cosine(a, b):

@@ -490,3 +490,102 @@ def test_Q_predicates_closed_forms_and_composite(oracle):
     assert np.abs(r["gbar"] - gm).max() < 1e-6
     s = base["s_sem"] * (0.5 + 0.5 * gm)
     assert np.abs(r["s"] - s).max() < 1e-6 and list(r["top"]) == list(np.argsort(-r["s"], kind="stable"))
+
+
+# ================================================================================================ W: weighted covisibility edges
+def _bhatt_np(mu1, S1, mu2, S2):
+    Sb = 0.5 * (S1 + S2)
+    d = mu1 - mu2
+    return 0.125 * d @ np.linalg.solve(Sb, d) + 0.5 * np.log(np.linalg.det(Sb) / np.sqrt(np.linalg.det(S1) * np.linalg.det(S2)))
+
+
+def test_W_bhattacharyya_closed_forms(oracle):
+    """W2's distance: equal isotropic covariances -> DB = |dmu|^2 / (8 sigma^2); equal means -> the log term alone;
+    H = sqrt(1 - exp(-DB)) against the pinned Hellinger routine; the general formula through numpy.linalg."""
+    iso = lambda v: np.array([v, 0, 0, v, 0, v], np.float64)
+    z = np.zeros(3)
+    assert abs(oracle.bhattacharyya(z, iso(0.04), np.array([1.0, 0, 0]), iso(0.04), 0.0) - 1.0 / (8 * 0.04)) < 1e-12
+    assert abs(oracle.bhattacharyya(z, iso(1.0), z, iso(4.0), 0.0) - 1.5 * np.log(2.5 / 2.0)) < 1e-12
+    g = np.random.default_rng(4)
+    pk = lambda M_: np.array([M_[0, 0], M_[0, 1], M_[0, 2], M_[1, 1], M_[1, 2], M_[2, 2]])
+    for _ in range(30):
+        A, B = g.standard_normal((3, 3)), g.standard_normal((3, 3))
+        S1, S2 = A @ A.T + 0.1 * np.eye(3), B @ B.T + 0.1 * np.eye(3)
+        mu1, mu2 = g.standard_normal(3), g.standard_normal(3) * 2
+        db = oracle.bhattacharyya(mu1, pk(S1), mu2, pk(S2), 0.01)
+        assert abs(db - _bhatt_np(mu1, S1 + 0.01 * np.eye(3), mu2, S2 + 0.01 * np.eye(3))) < 1e-9
+        assert abs(np.sqrt(1 - np.exp(-db)) - oracle.hellinger(mu1, pk(S1), mu2, pk(S2), 0.01)) < 1e-9
+    # far apart: H has saturated, DB still orders the pairs
+    far1 = oracle.bhattacharyya(z, iso(0.01), np.array([5.0, 0, 0]), iso(0.01), 0.0)
+    far2 = oracle.bhattacharyya(z, iso(0.01), np.array([6.0, 0, 0]), iso(0.01), 0.0)
+    assert far2 > far1 > 100 and oracle.hellinger(z, iso(0.01), np.array([5.0, 0, 0]), iso(0.01), 0.0) == 1.0
+
+
+def _two_patches(labels=(1, 2)):
+    px = [(40 + du, 40 + dv, 2.0, labels[0]) for du in range(4) for dv in range(4)]
+    if len(labels) > 1:
+        px += [(90 + du, 40 + dv, 2.0, labels[1]) for du in range(4) for dv in range(4)]
+    return hand_frame(H, W, px)
+
+
+def test_W_decay_closed_form(oracle):
+    """W4 with decay 0.5 and k = 1: the pair {0, 1} is co-observed in calls 1, 2 and 4 (call 3 sees object 0 alone):
+    w = ((1 * 0.5 + 1) * 0.25) + 1 = 1.375 at call 4, 0.6875 one call later without an observation."""
+    e = np.eye(4, dtype=np.float32)
+    m = oracle.OracleMap(0.25, 4, 0.5, 0.5, 0.5, 0, H, W)
+    m.set_option(m.OPT_EDGES_K, 1)
+    m.set_option(m.OPT_EDGE_DECAY, 0.5)
+    both, one = _two_patches(), _two_patches((1,))
+    for call, (fr, n) in enumerate([(both, 2), (both, 2), (one, 1), (both, 2)]):
+        m.integrate(fr[0], fr[1], pow2_K(), I4, e[:n], n)
+    a, b, w = m.read_edges()
+    assert list(a) == [0] and list(b) == [1] and abs(w[0] - 1.375) < 1e-6
+    m.integrate(one[0], one[1], pow2_K(), I4, e[:1], 1)
+    assert abs(m.read_edges()[2][0] - 0.6875) < 1e-6
+    assert len(m.read()[0]) == 2
+
+
+@pytest.mark.parametrize("k,cut", [(2, 2.0), (3, 1.05)])
+def test_W_knn_graph_against_brute_force(oracle, k, cut):
+    """W1-W4 on configs[0] in batches of 3 frames: the kNN graph in Hellinger order (through the Bhattacharyya distance,
+    W2), the median cutoff and the decayed weights rebuilt in Python from the exported (pinned: G-P1, G-P2) entity
+    Gaussians with a numpy.linalg Bhattacharyya distance."""
+    cfg = S.get_config(0)
+    sc = S.BoxScene(cfg)
+    m = oracle.OracleMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, cfg.dtype, cfg.H, cfg.W)
+    m.set_option(m.OPT_EDGES_K, k)
+    m.set_option(m.OPT_EDGE_CUTOFF, cut)
+    decay, eps2 = 0.9, float(np.float32(cfg.voxel)) ** 2
+    edges, n_dropped = {}, 0
+    for call in range(1, 7):
+        frames = [sc.frame(3 * (call - 1) + i) for i in range(3)]
+        depth = np.stack([f.depth for f in frames]); mask = np.stack([f.mask for f in frames])
+        K = np.stack([f.K for f in frames]); T = np.stack([f.T for f in frames])
+        m.integrate_batch(depth, mask, K, T, np.concatenate([f.desc for f in frames]), [f.n_det for f in frames])
+        assoc = m.last_assoc()[0]
+        wgt, mu, cov = m.read_gaussians()
+        Sset = sorted({int(t) for t in assoc if t >= 0 and wgt[t] > 0})
+        touched = set()
+        for a in Sset:
+            d = sorted((np.float32(_bhatt_np(mu[a].astype(np.float64), _unpack(cov[a]) + eps2 * np.eye(3),
+                                             mu[b].astype(np.float64), _unpack(cov[b]) + eps2 * np.eye(3))), b) for b in Sset if b != a)
+            kk = min(k, len(d))
+            if kk == 0:
+                continue
+            med = d[(kk - 1) // 2][0]
+            if kk < len(d):
+                assert d[kk][0] - d[kk - 1][0] > 1e-5 * d[kk][0], "kNN boundary too close: change the seed"
+            for dist, b in d[:kk]:
+                assert abs(float(dist) - cut * float(med)) > 1e-5 * float(dist) or dist == med, "cutoff too close"
+                if dist <= np.float32(cut) * med:
+                    touched.add((min(a, b), max(a, b)))
+                else:
+                    n_dropped += 1
+        for e in touched:
+            w, t = edges.get(e, (0.0, call))
+            edges[e] = (w * decay ** (call - t) + 1.0, call)
+        a_, b_, w_ = m.read_edges()
+        exp = sorted(edges.items())
+        assert list(zip(a_.tolist(), b_.tolist())) == [e for e, _ in exp]
+        assert np.abs(w_ - np.array([w * decay ** (call - t) for _, (w, t) in exp])).max() < 1e-5
+    assert len(edges) > 5 and (cut > 1.5 or n_dropped > 0)
