@@ -45,6 +45,9 @@ def parse():
     p.add_argument("--overlap", type=int, default=1, help="0 = run similarity on the main stream (no lift || similarity overlap)")
     p.add_argument("--breakdown", action="store_true", help="bracket every kernel with CUDA events (perturbs `value`)")
     p.add_argument("--sim-path", type=int, default=0, help="FARM_OPT_SIM_PATH: 0 auto, 2 tcgen05 single CTA, 3 tcgen05 CTA pairs")
+    p.add_argument("--extras", nargs="?", const="gaussian,covisibility,views,edges", default="",
+                   help="also maintain optional structures, a comma list of gaussian, covisibility, views (4), edges (k = 4; needs "
+                        "gaussian); no value = all four (not the headline configuration; config.extras says so)")
     p.add_argument("--no-single-frame", action="store_true", help="skip the single-frame latency series of configs[0..3]")
     p.add_argument("--full-oracle-batch", action="store_true",
                    help="cpu_baseline / --impl reference: time ONE full 16-frame, 1600-detection batch (minutes on one core)")
@@ -257,7 +260,8 @@ def run_ours(args):
         m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
                     max_objects=max_objects, max_voxels=max_voxels, max_blocks=max_blocks, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
                     max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
-                    timing=timing, overlap=args.overlap, sim_path=args.sim_path)
+                    timing=timing, overlap=args.overlap, sim_path=args.sim_path,
+                    **{k: {"gaussian": 1, "covisibility": 1, "views": 4, "edges": 4}[k] for k in args.extras.split(",") if k})
         m.import_(objs, desc, keys, owner)
         return m
 
@@ -463,6 +467,7 @@ def run_ours(args):
                    "image": f"{cfg.W}x{cfg.H}", "detections_per_frame": DET_PER_FRAME, "D": cfg.D, "voxel_m": cfg.voxel,
                    "map_objects_at_start": n_before, "map_objects_at_end": n_after, "map_voxels_at_import": int(len(keys)),
                    "parallelism": "replicas" if world > 1 else "single",
+                   "extras": (args.extras + " (NOT the headline configuration)") if args.extras else "none",
                    "l2": "inputs larger than L2: every step reads a fresh 29.5 MB batch (all batches staged, >1 GB) and probes a multi-GB voxel table"},
         "masked_points_per_sec": total_points / (ms * 1e-3),
         "masked_points_per_step": points / max(K_steps, 1),

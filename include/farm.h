@@ -88,6 +88,9 @@ extern "C" {
 #define FARM_OPT_GEOMETRY 18          /* 0 (default): voxel overlap (BASELINE.json rule);  1: the paper's geometry -- similarity
                                         prefilter, then g = 1 - Hellinger distance between the detection's and the entity's
                                         Gaussian (rules H1-H3).  Needs FARM_OPT_GAUSSIAN = 1            */
+#define FARM_OPT_EDGES 19             /* k in 0..16: maintain the weighted covisibility edge dictionary of PAPER.md:354 (rules
+                                        W1-W4 of DESIGN.md; see farm_map_read_edges); default 0 = off.  Needs
+                                        FARM_OPT_GAUSSIAN = 1; not available together with FARM_OPT_CORRESPONDENCE          */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */
@@ -97,6 +100,10 @@ extern "C" {
                                         "sufficiently similar" is unstated)                                              */
 #define FARM_OPTF_HELLINGER_BUDGET 106 /* H2: candidates with H > this are dropped; default 1 (no gate; the paper's "fixed
                                         Hellinger budget" is unstated)                                                   */
+#define FARM_OPTF_EDGE_DECAY 107      /* W4: weight discount per integrate call, in (0, 1]; default 0.9 (the paper's "temporal
+                                        decay" is unstated)                                                              */
+#define FARM_OPTF_EDGE_CUTOFF 108     /* W3: a neighbour farther than this multiple of the median kNN distance is dropped;
+                                        >= 0, default 2 (the paper's "soft median cutoff" is unstated)                    */
 #define FARM_OPTF_VIEW_CLOSER 104    /* or the view is kept if its distance is below this ratio x the closest kept view;
                                         default 0.8 (the paper's "sufficiently closer" is unstated)                        */
 
@@ -207,6 +214,18 @@ typedef struct {
   float dist;               /* distance camera -> centre of the detection's point box           */
 } farm_view;
 int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts);
+
+/* Weighted covisibility edges (needs FARM_OPT_EDGES = k > 0; HOST buffers; synchronises).  PAPER.md:354: "a parallel
+ * weighted edge dictionary accumulates their co-occurrence, restricted to spatially proximal pairs (a k-nearest-neighbor
+ * graph in Gaussian Hellinger distance with a soft median cutoff) and discounted by a temporal decay".  Readings
+ * (W1-W4): per call, S = the distinct entities that received a detection; for a in S, N_k(a) = its k nearest
+ * members of S in Hellinger distance between the entity Gaussians after the call's merge (ordered through the
+ * Bhattacharyya distance DB, of which H = sqrt(1 - exp(-DB)) is an increasing function that saturates at 1 in floating
+ * point; fp32 value, ties -> lower id); b in N_k(a) is kept iff DB(a, b) <= cutoff x the lower median of a's kNN
+ * distances; every unordered pair kept from either side gets w <- w * decay^(calls since its last update) + 1.
+ * Writes the n edges (a < b, sorted by (a, b)) with w discounted to the last integrate call; *n_out = n even when
+ * capacity < n (then only the first `capacity` are written and FARM_ERR_CAPACITY is returned).  a, b, w may be NULL. */
+int farm_map_read_edges(farm_map *m, uint32_t *a, uint32_t *b, double *w, uint64_t capacity, uint64_t *n_out);
 
 /* Retrieval-side scoring over the finished memory (a second workload beside the mapper, rules Q1-Q5 of
  * DESIGN.md).  The three per-entity retrieval embedding matrices of PAPER.md:356 (caption text, image, image-VL), the

@@ -1003,13 +1003,13 @@ void oracle_last_tau_gap(void *h, float *gap) {
   for (int j = 0; j < m.M; ++j) gap[j] = m.tau_gap[j];
 }
 // W: the weighted edges, weights decayed to the current call count; a < b; ascending (a, b).  Returns their number.
-long long oracle_read_edges(void *h, int32_t *a, int32_t *b, float *w) {
+long long oracle_read_edges(void *h, int32_t *a, int32_t *b, double *w) {
   Map &m = *(Map *)h;
   long long n = 0;
   for (auto &kv : m.edges) {
     if (a) a[n] = kv.first.first;
     if (b) b[n] = kv.first.second;
-    if (w) w[n] = (float)(kv.second.first * std::pow((double)m.edge_decay, (double)(m.call_index - kv.second.second)));
+    if (w) w[n] = kv.second.first * std::pow((double)m.edge_decay, (double)(m.call_index - kv.second.second));
     ++n;
   }
   return n;

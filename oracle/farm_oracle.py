@@ -83,7 +83,7 @@ class OracleMap:
         """W: (a [n], b [n], w [n]) weighted covisibility edges, a < b, ascending, weights decayed to now."""
         lib().oracle_read_edges.restype = C.c_longlong
         n = lib().oracle_read_edges(self.h, None, None, None)
-        a, b, w = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.float32)
+        a, b, w = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.float64)
         lib().oracle_read_edges(self.h, _p(a), _p(b), _p(w))
         return a, b, w
 

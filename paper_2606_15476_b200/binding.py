@@ -26,6 +26,8 @@ OPT_COVISIBILITY = 15
 OPT_VIEWS = 16
 OPT_CORRESPONDENCE = 17
 OPT_GEOMETRY = 18
+OPT_EDGES = 19
+OPTF_EDGE_DECAY, OPTF_EDGE_CUTOFF = 107, 108
 N_STAGES = 6
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "merge"]
 OPTF_Z_MIN, OPTF_Z_MAX, OPTF_VIEW_COS, OPTF_VIEW_CLOSER, OPTF_PREFILTER_COS, OPTF_HELLINGER_BUDGET = 101, 102, 103, 104, 105, 106
@@ -47,7 +49,7 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
            "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views", "farm_map_query", "farm_map_read_alias",
-           "farm_map_last_merges",
+           "farm_map_last_merges", "farm_map_read_edges",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -84,6 +86,7 @@ def load_library():
         lib.farm_map_read_covisibility.argtypes = [vp, vp, vp]
         lib.farm_map_read_views.argtypes = [vp, vp, vp]
         lib.farm_map_read_alias.argtypes = [vp, vp]
+        lib.farm_map_read_edges.argtypes = [vp, vp, vp, vp, C.c_uint64, vp]
         lib.farm_map_last_merges.argtypes = [vp, vp, vp, vp]
         lib.farm_map_query.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, ci, ci, vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -128,7 +131,7 @@ class FarmMap:
                  max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
                  stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None,
                  views=None, view_cos=None, view_closer=None, correspondence=None, geometry=None, prefilter_cos=None,
-                 hellinger_budget=None):
+                 hellinger_budget=None, edges=None, edge_decay=None, edge_cutoff=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._last_M = 0
@@ -141,7 +144,8 @@ class FarmMap:
                        (OPT_MAX_DET_PER_CALL, max_det_per_call), (OPT_MAX_PAIRS_PER_CALL, max_pairs_per_call),
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
                        (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility),
-                       (OPT_VIEWS, views), (OPT_CORRESPONDENCE, correspondence), (OPT_GEOMETRY, geometry)):
+                       (OPT_VIEWS, views), (OPT_CORRESPONDENCE, correspondence), (OPT_GEOMETRY, geometry),
+                       (OPT_EDGES, edges)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:
@@ -156,6 +160,10 @@ class FarmMap:
             self.set_option_f(OPTF_PREFILTER_COS, prefilter_cos)
         if hellinger_budget is not None:
             self.set_option_f(OPTF_HELLINGER_BUDGET, hellinger_budget)
+        if edge_decay is not None:
+            self.set_option_f(OPTF_EDGE_DECAY, edge_decay)
+        if edge_cutoff is not None:
+            self.set_option_f(OPTF_EDGE_CUTOFF, edge_cutoff)
         self.views_k = int(views or 0)
 
     def destroy(self):
@@ -296,6 +304,16 @@ class FarmMap:
         counts = np.zeros(n.value, np.int32)
         _check(load_library().farm_map_read_views(self._h, _hp(views), _hp(counts)))
         return views[:, :self.views_k], counts
+
+    def read_edges(self):
+        """(a [n] uint32, b [n] uint32, w [n] float64): weighted covisibility edges a < b sorted by (a, b), weights
+        discounted to the last integrate call (FARM_OPT_EDGES = k)."""
+        lib = load_library()
+        n = C.c_uint64(0)
+        _check(lib.farm_map_read_edges(self._h, None, None, None, 0, C.byref(n)))
+        a, b, w = np.zeros(n.value, np.uint32), np.zeros(n.value, np.uint32), np.zeros(n.value, np.float64)
+        _check(lib.farm_map_read_edges(self._h, _hp(a), _hp(b), _hp(w), n.value, C.byref(n)))
+        return a, b, w
 
     def read_covisibility(self):
         """uint64 [N, ceil(N/64)] covisibility bitset (FARM_OPT_COVISIBILITY)."""

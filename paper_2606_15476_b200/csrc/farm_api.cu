@@ -42,7 +42,9 @@ struct farm_map {
   float voxel_size, w_geo, w_sem, tau, z_min = 0.f, z_max = std::numeric_limits<float>::infinity();
   int D, dtype = FARM_DTYPE_F32, H = 0, W = 0;
   long long max_objects = 65536, max_voxels = 1ll << 22, max_det = 4096, max_pairs = 0, max_frames = 16, max_blocks = 0;
-  int sim_path = 0, gaussian = 0, covis = 0, views_k = 0, corr = 0, geom = 0;
+  int sim_path = 0, gaussian = 0, covis = 0, views_k = 0, corr = 0, geom = 0, edges_k = 0;
+  float edge_decay = 0.9f, edge_cutoff = 2.0f;
+  uint32_t edge_calls = 0;  // integrate calls so far: the clock of W4's decay
   float view_cos = 0.8660254f, view_closer = 0.8f, prefilter_cos = 0.5f, hell_budget = 1.0f;
   cudaStream_t stream = 0;
   bool finalised = false;
@@ -446,6 +448,19 @@ int finalise_impl(farm_map *m) {
     A(d.views, NO * (size_t)m->views_k, 0);
     A(d.view_cnt, NO, 0);
   }
+  if (m->edges_k > 0) {
+    if (!m->gaussian) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_EDGES needs FARM_OPT_GAUSSIAN = 1");
+    if (m->corr) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_EDGES is not available together with FARM_OPT_CORRESPONDENCE");
+    if ((NO + 63) / 64 * 8 > 96 * 1024) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_EDGES supports MAX_OBJECTS <= 786432");
+    d.edges_k = m->edges_k, d.edge_decay = m->edge_decay, d.edge_cutoff = m->edge_cutoff;
+    A(d.eg_list, MD, 0);
+    A(d.eg_gauss, MD * 10, 0);
+    const long long ecap = next_pow2(std::max<long long>(8ll * m->edges_k * (long long)NO, 4096));
+    A(d.ed_key, (size_t)ecap, 0xFF);
+    A(d.ed_w, (size_t)ecap, 0);
+    A(d.ed_t, (size_t)ecap, 0);
+    d.ed_mask = (uint32_t)(ecap - 1);
+  }
   if (m->gaussian) {
     A(d.det_gm, MD * 9, 0);
     A(d.hell, MD, 0);
@@ -459,6 +474,7 @@ int finalise_impl(farm_map *m) {
 #undef A
   configure_lift_kernels();
   configure_assoc_kernels();
+  configure_edge_kernels();
   init_objects_kernel<<<(unsigned)((NO + 255) / 256), 256, 0, m->stream>>>(d);
   m->launches++;
   if (m->corr) {
@@ -497,11 +513,12 @@ int device_error(farm_map *m) {
   CU(cudaStreamSynchronize(m->stream));
   if (e == 0) return FARM_OK;
   char buf[320];
-  snprintf(buf, sizeof buf, "sticky device error 0x%x:%s%s%s%s%s%s%s", e, (e & ERR_VOXEL_TABLE_FULL) ? " voxel table full" : "",
+  snprintf(buf, sizeof buf, "sticky device error 0x%x:%s%s%s%s%s%s%s%s", e, (e & ERR_VOXEL_TABLE_FULL) ? " voxel table full" : "",
            (e & ERR_PAIR_TABLE_FULL) ? " per-call pair scratch full" : "",
            (e & ERR_OVERLAP_TABLE_FULL) ? " per-call overlap scratch full" : "",
            (e & ERR_OBJECT_CAPACITY) ? " object capacity" : "", (e & ERR_IMPORT_DUPLICATE) ? " import: duplicate key or bad owner" : "",
            (e & ERR_IMPORT_COUNT) ? " import: an object's n_voxels differs from the voxels listed for it" : "",
+           (e & ERR_EDGE_TABLE_FULL) ? " edge dictionary full" : "",
            (e & ERR_SYNC_TIMEOUT) ? " a device-side wait between the grids of one call expired (kernels serialised? use FARM_OPT_OVERLAP = 0)" : "");
   if (e & (ERR_IMPORT_DUPLICATE | ERR_IMPORT_COUNT)) return fail(FARM_ERR_INVALID_ARG, buf);
   return fail((e & ERR_SYNC_TIMEOUT) ? FARM_ERR_STATE : FARM_ERR_CAPACITY, buf);
@@ -617,6 +634,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 8) return fail(FARM_ERR_INVALID_ARG, "bad VIEWS (0..8)");
       m->views_k = (int)v;
       break;
+    case FARM_OPT_EDGES:
+      if (v < 0 || v > 16) return fail(FARM_ERR_INVALID_ARG, "bad EDGES (0..16)");
+      m->edges_k = (int)v;
+      break;
     case FARM_OPT_TIMING:
       if (v < 0 || v > 2) return fail(FARM_ERR_INVALID_ARG, "bad TIMING");
       m->timing = (int)v;
@@ -643,6 +664,13 @@ int farm_map_set_option_f(farm_map *m, int key, float v) {
     m->view_cos = v;
   else if (key == FARM_OPTF_VIEW_CLOSER)
     m->view_closer = v;
+  else if (key == FARM_OPTF_EDGE_DECAY) {
+    if (!(v > 0.f && v <= 1.f)) return fail(FARM_ERR_INVALID_ARG, "EDGE_DECAY must be in (0, 1]");
+    m->edge_decay = v;
+  } else if (key == FARM_OPTF_EDGE_CUTOFF) {
+    if (!(v >= 0.f) || !std::isfinite(v)) return fail(FARM_ERR_INVALID_ARG, "EDGE_CUTOFF must be finite and >= 0");
+    m->edge_cutoff = v;
+  }
   else
     return fail(FARM_ERR_INVALID_ARG, "unknown float option");
   return FARM_OK;
@@ -745,6 +773,8 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covis_absorb(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_alias_compress(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
+  m->edge_calls++;
+  stage(FARM_STAGE_MERGE, st, [&] { return launch_edges(d, a, m->edge_calls, st); });
   if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
@@ -1082,6 +1112,49 @@ int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts) {
   CU(cudaMemcpy(&N, m->dm.n_objects, 4, cudaMemcpyDeviceToHost));
   if (views && N) CU(cudaMemcpy(views, m->dm.views, (size_t)N * m->views_k * sizeof(farm_view), cudaMemcpyDeviceToHost));
   if (counts && N) CU(cudaMemcpy(counts, m->dm.view_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost));
+  return FARM_OK;
+}
+
+int farm_map_read_edges(farm_map *m, uint32_t *ea, uint32_t *eb, double *ew, uint64_t capacity, uint64_t *n_out) {
+  if (!m) return fail(FARM_ERR_INVALID_ARG, "map is NULL");
+  if (m->edges_k <= 0) return fail(FARM_ERR_STATE, "FARM_OPT_EDGES is off");
+  if (n_out) *n_out = 0;
+  if (!m->finalised) return FARM_OK;
+  int rc = device_error(m);
+  if (rc != FARM_OK) return rc;
+  uint32_t n = 0;
+  CU(cudaMemcpy(&n, m->dm.counters + 9, 4, cudaMemcpyDeviceToHost));
+  if (n_out) *n_out = n;
+  if (n == 0) return FARM_OK;
+  // compacted on the device, ordered on the host (an export, not part of the integrate path)
+  uint32_t *da = nullptr, *db = nullptr, *dc = nullptr;
+  double *dw = nullptr;
+  auto release = [&] { cudaFree(da), cudaFree(db), cudaFree(dc), cudaFree(dw); };
+  if (cudaMalloc(&da, (size_t)n * 4) || cudaMalloc(&db, (size_t)n * 4) || cudaMalloc(&dw, (size_t)n * 8) || cudaMalloc(&dc, 4)) {
+    release();
+    cudaGetLastError();
+    return fail(FARM_ERR_CUDA, "farm_map_read_edges: out of device memory");
+  }
+  cudaMemsetAsync(dc, 0, 4, m->stream);
+  m->launches += launch_edge_export(m->dm, m->edge_calls, da, db, dw, n, dc, m->stream);
+  std::vector<uint32_t> ha(n), hb(n);
+  std::vector<double> hw(n);
+  cudaError_t e = cudaMemcpyAsync(ha.data(), da, (size_t)n * 4, cudaMemcpyDeviceToHost, m->stream);
+  if (!e) e = cudaMemcpyAsync(hb.data(), db, (size_t)n * 4, cudaMemcpyDeviceToHost, m->stream);
+  if (!e) e = cudaMemcpyAsync(hw.data(), dw, (size_t)n * 8, cudaMemcpyDeviceToHost, m->stream);
+  if (!e) e = cudaStreamSynchronize(m->stream);
+  release();
+  if (e) return fail(FARM_ERR_CUDA, std::string("farm_map_read_edges: ") + cudaGetErrorString(e));
+  std::vector<uint32_t> order(n);
+  for (uint32_t i = 0; i < n; ++i) order[i] = i;
+  std::sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return ha[x] != ha[y] ? ha[x] < ha[y] : hb[x] < hb[y]; });
+  const uint64_t lim = std::min<uint64_t>(n, capacity);
+  for (uint64_t i = 0; i < lim; ++i) {
+    if (ea) ea[i] = ha[order[i]];
+    if (eb) eb[i] = hb[order[i]];
+    if (ew) ew[i] = hw[order[i]];
+  }
+  if (capacity < n && (ea || eb || ew)) return fail(FARM_ERR_CAPACITY, "farm_map_read_edges: capacity is smaller than the number of edges");
   return FARM_OK;
 }
 

@@ -51,6 +51,24 @@ __device__ __noinline__ void match_hellinger(const double *det_gm, const double 
   hell[j] = hellinger_gauss(mu_d, c_d, mu_o, c_o, (double)eps2);
 }
 
+// W1: entity t received a detection in this call and carries the Gaussian (w, g) after the merge: append it to S with
+// its regularised Gaussian -- mu (3), Sigma + eps2 I (6), determinant -- for the kNN kernel (farm_edges.cu).  The order
+// of S is arbitrary; nothing downstream depends on it.
+__device__ __noinline__ void edge_member(const DevMap &m, uint32_t t, double w, const double *g) {
+  const uint32_t pos = atomicAdd(&m.counters[8], 1u);
+  if (pos >= m.max_det) return;  // cannot happen: one member per detection at most
+  const double eps2 = (double)m.eps2;
+  const double mx = g[0] / w, my = g[1] / w, mz = g[2] / w;
+  double s[6] = {g[3] / w - mx * mx + eps2, g[4] / w - mx * my, g[5] / w - mx * mz,
+                 g[6] / w - my * my + eps2, g[7] / w - my * mz, g[8] / w - mz * mz + eps2};
+  double *o = m.eg_gauss + (size_t)pos * 10;
+  o[0] = mx, o[1] = my, o[2] = mz;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) o[3 + k] = s[k];
+  o[9] = det_sym3(s);
+  m.eg_list[pos] = t;
+}
+
 // V1-V2: the view of one merged detection, offered to its object's retained set.  fp32, one rounded
 // operation at a time: the comparisons decide which views are kept and the oracle takes them in the same precision.
 __device__ __noinline__ void offer_view_record(const DevMap &m, int32_t t, const farm_view &v) {
@@ -839,9 +857,13 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
     m.n_obs[t] = n_old + loser_obs + k_members;
     m.n_points[t] = pts_old + pts;
     if (m.det_gm) {  // G2: M1 += sum w mu, M2 += sum w (Sigma + mu mu^T), w = points
-      m.obj_gw[t] += (double)pts;
+      const double gw = m.obj_gw[t] + (double)pts;
+      m.obj_gw[t] = gw;
 #pragma unroll
-      for (int k = 0; k < 9; ++k) m.obj_gm[(size_t)t * 9 + k] += gsum[k];
+      for (int k = 0; k < 9; ++k) gsum[k] += m.obj_gm[(size_t)t * 9 + k];
+#pragma unroll
+      for (int k = 0; k < 9; ++k) m.obj_gm[(size_t)t * 9 + k] = gsum[k];
+      if (m.edges_k > 0 && gw > 0.0) edge_member(m, (uint32_t)t, gw, gsum);  // W1
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {  // R22

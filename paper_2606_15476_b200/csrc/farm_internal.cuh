@@ -28,6 +28,7 @@ constexpr uint32_t ERR_IMPORT_DUPLICATE = 16u;
 constexpr uint32_t ERR_SYNC_TIMEOUT = 32u;       // a device-side wait for another grid of the same call expired
 constexpr uint32_t DD_FLAG = 0x80000000u;        // overlap-map "owner" field: DD_FLAG | e = detection e of the same call (U2)
 constexpr uint32_t ERR_IMPORT_COUNT = 64u;       // import: objects[i].n_voxels differs from the voxels listed for i
+constexpr uint32_t ERR_EDGE_TABLE_FULL = 128u;   // W4: the edge dictionary is full
 constexpr uint32_t SPIN_LIMIT = 1u << 23;        // polls of ~0.25 us each (about 2 s) before a device-side wait gives up
 
 // Global voxel -> object hash (R11: one owner per key), stored as a hash of 4x4x4 VOXEL BLOCKS so that the
@@ -109,6 +110,7 @@ struct DevMap {
   uint32_t surv_cap;
   uint32_t *counters;                // [0]=event_count [1]=cand_count [2]=survivor_count [3]=block ticket
                                      // [4]=dense pairs [5]=edges [6]=detection-detection edges [7]=entity merges
+                                     // [8]=|S| of the call (W1) [9]=entries of the edge dictionary (W4)
   // per detection [max_det]
   uint32_t max_det;
   uint32_t *det_nv, *det_npx;
@@ -147,6 +149,15 @@ struct DevMap {
   uint32_t *view_cnt;                // [max_objects]
   int views_k;
   float view_cos, view_closer;
+  // W1-W4: weighted covisibility edges; null / 0 when disabled
+  int edges_k;
+  float edge_decay, edge_cutoff;
+  uint32_t *eg_list;                 // [max_det] S: the call's entities that carry a Gaussian (order arbitrary); counters[8]
+  double *eg_gauss;                  // [max_det,10] per member: mu (3), Sigma + eps2 I (6), its determinant
+  unsigned long long *ed_key;        // edge dictionary (open addressing): a << 32 | b with a < b, all ones when free
+  double *ed_w;                      //   weight as of call ed_t
+  uint32_t *ed_t;                    //   index (1-based) of the call that last updated the edge
+  uint32_t ed_mask;
   uint32_t *sim_done;                // cumulative count of finished similarity CTAs (the association scan waits on it)
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
@@ -273,6 +284,7 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 // kernel has drained).
 void configure_lift_kernels();
 void configure_assoc_kernels();
+void configure_edge_kernels();
 int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);  // returns the number of CTAs it launched
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
@@ -283,6 +295,9 @@ int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s);
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_covis_absorb(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
+int launch_edges(const DevMap &m, const CallArgs &a, uint32_t call, cudaStream_t s);
+int launch_edge_export(const DevMap &m, uint32_t call, uint32_t *out_a, uint32_t *out_b, double *out_w, uint32_t cap, uint32_t *count,
+                       cudaStream_t s);
 int launch_dd_overlap(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_alias_compress(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
 

@@ -88,7 +88,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     m.counters[0] = 0;
     m.counters[1] = 0;
     m.counters[2] = 0;
-    m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0;
+    m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
     CallStats z = {};
     z.n_det = (uint32_t)a.M;
     *m.stats = z;
@@ -354,7 +354,7 @@ __device__ __forceinline__ void lane_flush_block(const DevMap &m, TileSmem &s, c
 //     (warp patch, detection).
 // Two barriers per tile.
 template <bool VEC, bool GAUSS>
-__global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 4 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+__global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 5 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   pdl_trigger();  // the probe kernel may become resident as soon as CTAs of this grid retire
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads its copy

@@ -123,11 +123,18 @@ def test_round2_options_and_calls_validate_on_the_host(lib):
     from paper_2606_15476_b200 import FarmError, FarmMap, binding
     m = FarmMap(0.05, 8, 0.5, 0.5, 0.5, H=8, W=8)
     for key, bad in ((binding.OPT_VIEWS, 9), (binding.OPT_VIEWS, -1), (binding.OPT_CORRESPONDENCE, 2), (binding.OPT_GEOMETRY, 2),
-                     (binding.OPT_SIM_PATH, 4)):
+                     (binding.OPT_SIM_PATH, 4), (binding.OPT_EDGES, 17), (binding.OPT_EDGES, -1)):
         with pytest.raises(FarmError):
             m.set_option_i(key, bad)
-    for key, good in ((binding.OPT_VIEWS, 4), (binding.OPT_CORRESPONDENCE, 1), (binding.OPT_GEOMETRY, 1), (binding.OPT_SIM_PATH, 3)):
+    for key, good in ((binding.OPT_VIEWS, 4), (binding.OPT_CORRESPONDENCE, 1), (binding.OPT_GEOMETRY, 1), (binding.OPT_SIM_PATH, 3),
+                      (binding.OPT_EDGES, 16)):
         m.set_option_i(key, good)
+    for key, bad in ((binding.OPTF_EDGE_DECAY, 0.0), (binding.OPTF_EDGE_DECAY, 1.5), (binding.OPTF_EDGE_CUTOFF, -1.0),
+                     (binding.OPTF_EDGE_CUTOFF, float("inf")), (binding.OPTF_EDGE_DECAY, float("nan"))):
+        with pytest.raises(FarmError):
+            m.set_option_f(key, bad)
+    m.set_option_f(binding.OPTF_EDGE_DECAY, 1.0)
+    m.set_option_f(binding.OPTF_EDGE_CUTOFF, 0.0)
     for key in (binding.OPTF_VIEW_COS, binding.OPTF_VIEW_CLOSER, binding.OPTF_PREFILTER_COS, binding.OPTF_HELLINGER_BUDGET):
         m.set_option_f(key, 0.5)
         with pytest.raises(FarmError):
@@ -141,7 +148,7 @@ def test_round2_options_and_calls_validate_on_the_host(lib):
     assert ei.value.code == -4
     m.destroy()
     m2 = FarmMap(0.05, 8, 0.5, 0.5, 0.5, H=8, W=8)
-    for call in (m2.read_alias, m2.last_merges, m2.read_views):
+    for call in (m2.read_alias, m2.last_merges, m2.read_views, m2.read_edges):
         with pytest.raises(FarmError) as ei:
             call()                                           # option off
         assert ei.value.code == -4

@@ -574,3 +574,47 @@ def test_retrieval_skips_absorbed_entities(oracle):
     assert np.array_equal(rg["landmarks"], ro["landmarks"])
     assert np.abs(rg["s_sem"] - ro["s_sem"]).max() <= 1e-6 and np.abs(rg["s"] - ro["s"]).max() <= 1e-6
     assert (rg["s"][alive == 0] == 0).all() and (rg["top"] >= 0).all() and alive[rg["top"]].all()
+
+
+# ------------------------------------------------------------------------------------------ W1-W4 weighted edges
+@pytest.mark.parametrize("cfg_id,n,per_call,k,cut,decay", [(0, 20, 1, 2, 2.0, None), (0, 18, 3, 3, 1.05, 0.5), (1, 30, 1, 8, 1.5, None),
+                                                           (1, 24, 4, 4, 2.0, 0.75)])
+def test_weighted_covisibility_edges_match_oracle(oracle, cfg_id, n, per_call, k, cut, decay):
+    """W1-W4: the kNN graph in Hellinger order with the median cutoff decides WHICH pairs are counted (fp32
+    distance of an fp64 evaluation on both sides), the decayed weights are fp64: same edge list after every call, weights
+    to 1e-9.  k = 2..8 covers both register-resident top-k widths of the kernel; batched calls put 10-40 entities in S."""
+    cfg = S.get_config(cfg_id)
+    frames_all = generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n))
+    o, g = make_pair(oracle, cfg, gaussian=1, edges=k, edge_cutoff=cut, edge_decay=decay)
+    o.set_option(o.OPT_EDGES_K, k)
+    o.set_option(o.OPT_EDGE_CUTOFF, cut)
+    if decay is not None:
+        o.set_option(o.OPT_EDGE_DECAY, decay)
+    sizes = []
+    for c in range(0, n, per_call):
+        frames = margin_filter(o.clone, frames_all[c:c + per_call], cfg.tau)
+        integrate_frames(o, frames)
+        gpu_integrate(g, frames, cfg.dtype)
+        compare_call(g, o, check_sets=False)
+        ao, bo, wo = o.read_edges()
+        ag, bg, wg = g.read_edges()
+        assert np.array_equal(ag, ao) and np.array_equal(bg, bo), (c, len(ao), len(ag))
+        assert np.abs(wg - wo).max(initial=0.0) <= 1e-9 * max(1.0, float(wo.max(initial=0.0)))
+        sizes.append(len(ao))
+    compare_maps(g, o, voxels=False)
+    assert sizes[-1] > 10 and wo.max() > 1.5 and (wo < 0.999).any()     # repeated pairs accumulate, stale ones decay
+
+
+def test_weighted_edges_option_checks(oracle):
+    cfg = S.get_config(0)
+    fr = generate_frames(0, range(1))[0]
+    for kw in (dict(edges=2), dict(edges=2, gaussian=1, correspondence=1)):      # needs the Gaussians; not with entity merges
+        g = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype, **kw)
+        with pytest.raises(Exception):
+            gpu_integrate(g, [fr], cfg.dtype)
+        g.destroy()
+    g = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype, gaussian=1)
+    gpu_integrate(g, [fr], cfg.dtype)
+    with pytest.raises(Exception):
+        g.read_edges()                                                          # FARM_OPT_EDGES is off
+    g.destroy()
