@@ -454,7 +454,8 @@ int finalise_impl(farm_map *m) {
     if ((NO + 63) / 64 * 8 > 96 * 1024) return fail(FARM_ERR_INVALID_ARG, "FARM_OPT_EDGES supports MAX_OBJECTS <= 786432");
     d.edges_k = m->edges_k, d.edge_decay = m->edge_decay, d.edge_cutoff = m->edge_cutoff;
     A(d.eg_list, MD, 0);
-    A(d.eg_gauss, MD * 10, 0);
+    A(d.eg_gauss, MD * 12, 0);
+    A(d.eg_f4, MD, 0);
     const long long ecap = next_pow2(std::max<long long>(8ll * m->edges_k * (long long)NO, 4096));
     A(d.ed_key, (size_t)ecap, 0xFF);
     A(d.ed_w, (size_t)ecap, 0);

@@ -52,8 +52,8 @@ __device__ __noinline__ void match_hellinger(const double *det_gm, const double 
 }
 
 // W1: entity t received a detection in this call and carries the Gaussian (w, g) after the merge: append it to S with
-// its regularised Gaussian -- mu (3), Sigma + eps2 I (6), determinant -- for the kNN kernel (farm_edges.cu).  The order
-// of S is arbitrary; nothing downstream depends on it.
+// its regularised Gaussian for the kNN kernel (farm_edges.cu; row of 12 doubles: mu, trace, S = Sigma + eps2 I, ln |S|).
+// The order of S is arbitrary; nothing downstream depends on it.
 __device__ __noinline__ void edge_member(const DevMap &m, uint32_t t, double w, const double *g) {
   const uint32_t pos = atomicAdd(&m.counters[8], 1u);
   if (pos >= m.max_det) return;  // cannot happen: one member per detection at most
@@ -61,11 +61,12 @@ __device__ __noinline__ void edge_member(const DevMap &m, uint32_t t, double w, 
   const double mx = g[0] / w, my = g[1] / w, mz = g[2] / w;
   double s[6] = {g[3] / w - mx * mx + eps2, g[4] / w - mx * my, g[5] / w - mx * mz,
                  g[6] / w - my * my + eps2, g[7] / w - my * mz, g[8] / w - mz * mz + eps2};
-  double *o = m.eg_gauss + (size_t)pos * 10;
-  o[0] = mx, o[1] = my, o[2] = mz;
+  double *o = m.eg_gauss + (size_t)pos * 12;
+  o[0] = mx, o[1] = my, o[2] = mz, o[3] = s[0] + s[3] + s[5];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) o[3 + k] = s[k];
-  o[9] = det_sym3(s);
+  for (int k = 0; k < 6; ++k) o[4 + k] = s[k];
+  o[10] = log(det_sym3(s));
+  m.eg_f4[pos] = make_float4((float)mx, (float)my, (float)mz, __double2float_ru(o[3]));  // the kNN scan's fp32 view (trace rounded up)
   m.eg_list[pos] = t;
 }
 
@@ -898,7 +899,8 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
 
 // ---- covisibility (rule C1; PAPER.md:354 step 7): every pair of distinct entities that received a detection in
 // this call is marked in the N x ceil(N/64) bitset.  Each CTA builds the call's entity bitmap in shared memory
-// (a few KB) and ORs it, minus the diagonal bit, into the rows of its entities, writing only the words that change.  A row is written only by the CTAs of detections that target it, and they all write the
+// (a few KB), lists its non-zero words (at most one per entity of the call, whatever N is) and ORs those words, minus the
+// diagonal bit, into the rows of its entities, writing only the words that change.  A row is written only by the CTAs of detections that target it, and they all write the
 // same words, so no atomics are needed.
 constexpr int COVIS_THREADS = 256;
 
@@ -938,22 +940,37 @@ __global__ void __launch_bounds__(COVIS_THREADS) covis_fold_kernel(DevMap m) {
 }
 
 __global__ void __launch_bounds__(COVIS_THREADS) covisibility_kernel(DevMap m, CallArgs a) {
-  extern __shared__ unsigned long long bm[];  // [words]
+  extern __shared__ unsigned long long bm[];  // [words] bitmap of the call's entities, then [n_list] uint16 word indices
+  __shared__ uint32_t n_list;
   pdl_wait();
   const uint32_t N = *m.n_objects;
   const uint32_t words = (N + 63) >> 6;
+  uint16_t *list = reinterpret_cast<uint16_t *>(bm + words);  // the non-zero words of bm: a row changes nowhere else
   for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) bm[w] = 0ull;
+  if (threadIdx.x == 0) n_list = 0;
   __syncthreads();
   for (int j = threadIdx.x; j < a.M; j += COVIS_THREADS) {
     const int32_t t = m.assoc[j];
     if (t >= 0) atomicOr(&bm[(uint32_t)t >> 6], 1ull << (t & 63));
   }
   __syncthreads();
+  for (uint32_t w0 = 0; w0 < words; w0 += COVIS_THREADS) {
+    const uint32_t w = w0 + threadIdx.x;
+    const bool nz = w < words && bm[w] != 0ull;
+    const unsigned ball = __ballot_sync(0xFFFFFFFFu, nz);
+    uint32_t base = 0;
+    if ((threadIdx.x & 31) == 0 && ball) base = atomicAdd(&n_list, (uint32_t)__popc(ball));
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (nz) list[base + __popc(ball & ((1u << (threadIdx.x & 31)) - 1u))] = (uint16_t)w;
+  }
+  __syncthreads();
+  const uint32_t nl = n_list;
   for (int j = blockIdx.x; j < a.M; j += gridDim.x) {
     const int32_t t = m.assoc[j];
     if (t < 0) continue;
     unsigned long long *row = m.covis + (size_t)t * m.covis_words;
-    for (uint32_t w = threadIdx.x; w < words; w += COVIS_THREADS) {
+    for (uint32_t i = threadIdx.x; i < nl; i += COVIS_THREADS) {
+      const uint32_t w = list[i];
       unsigned long long add = bm[w], keep = ~0ull;
       if (w == ((uint32_t)t >> 6)) keep = ~(1ull << (t & 63)), add &= keep;  // no diagonal (U4: a fold may have left one)
       const unsigned long long old = row[w], now = (old | add) & keep;
@@ -978,7 +995,7 @@ void configure_assoc_kernels() {
   cudaFuncSetAttribute(commit_merge_kernel<__half>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
   cudaFuncSetAttribute(commit_merge_kernel<__nv_bfloat16>, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
   cudaFuncSetAttribute(covisibility_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pref);
-  cudaFuncSetAttribute(covisibility_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+  cudaFuncSetAttribute(covisibility_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
 }
 
 int launch_cand_associate(const DevMap &m, const CallArgs &a, cudaStream_t s) {
@@ -995,7 +1012,8 @@ int launch_covis_absorb(const DevMap &m, const CallArgs &a, uint32_t n_upper, cu
 int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   if (a.M == 0 || !m.covis) return 0;
   const int grid = a.M < m.num_sms * 4 ? a.M : m.num_sms * 4;
-  launch_pdl(covisibility_kernel, dim3(grid), dim3(COVIS_THREADS), (size_t)m.covis_words * 8, s, m, a);
+  const size_t n_list_max = m.covis_words < (uint32_t)a.M ? m.covis_words : (uint32_t)a.M;  // non-zero words <= entities
+  launch_pdl(covisibility_kernel, dim3(grid), dim3(COVIS_THREADS), (size_t)m.covis_words * 8 + n_list_max * 2, s, m, a);
   return 1;
 }
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {

@@ -153,7 +153,8 @@ struct DevMap {
   int edges_k;
   float edge_decay, edge_cutoff;
   uint32_t *eg_list;                 // [max_det] S: the call's entities that carry a Gaussian (order arbitrary); counters[8]
-  double *eg_gauss;                  // [max_det,10] per member: mu (3), Sigma + eps2 I (6), its determinant
+  float4 *eg_f4;                     // [max_det] (mu, tr S) in fp32 (trace rounded up): the kNN scan's lower-bound test
+  double *eg_gauss;                  // [max_det,12] per member: mu (3), tr S, S = Sigma + eps2 I (6), ln |S|, pad
   unsigned long long *ed_key;        // edge dictionary (open addressing): a << 32 | b with a < b, all ones when free
   double *ed_w;                      //   weight as of call ed_t
   uint32_t *ed_t;                    //   index (1-based) of the call that last updated the edge

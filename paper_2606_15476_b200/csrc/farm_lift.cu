@@ -353,8 +353,12 @@ __device__ __forceinline__ void lane_flush_block(const DevMap &m, TileSmem &s, c
 //     and boxes are combined per detection over the warp (REDUX) and leave as one set of global atomics per
 //     (warp patch, detection).
 // Two barriers per tile.
+// 6 CTAs per SM = at most 80 registers, for both variants: the grid's 4 CTAs per SM must ALL be resident beside the
+// similarity CTA (256 threads x 80 registers), otherwise the statically assigned tiles of the late CTAs run as a second
+// wave (measured with the Gaussian variant at 96 registers: 3 resident, lift 194 us instead of 139 us in the step; its
+// 84 bytes of spill at 80 registers cost less than that).
 template <bool VEC, bool GAUSS>
-__global__ void __launch_bounds__(LIFT_THREADS, GAUSS ? 5 : 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
+__global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   pdl_trigger();  // the probe kernel may become resident as soon as CTAs of this grid retire
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads its copy
