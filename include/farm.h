@@ -227,6 +227,26 @@ int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts);
  * capacity < n (then only the first `capacity` are written and FARM_ERR_CAPACITY is returned).  a, b, w may be NULL. */
 int farm_map_read_edges(farm_map *m, uint32_t *a, uint32_t *b, double *w, uint64_t capacity, uint64_t *n_out);
 
+/* Step 4 alone, for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the dense cosine of M rows of A against N rows of B with the fused row maximum / argmax of R14-R16, R18
+ * ("a single batched detection-by-entity similarity matrix") -- the arithmetic of the CUDA-core similarity
+ * kernel, operands and results given by the caller, no map.
+ *   A DEVICE [M, D], B DEVICE [N, D], row-major, both in `dtype` (FARM_DTYPE_*); rows need not be normalised
+ *   max_cos DEVICE f32 [M]: max over B rows of clamp(cos, -1, 1); argmax DEVICE i32 [M]: its row, lowest index on ties;
+ *   (0, -1) when N = 0; a zero-norm row has cosine 0 with everything.  Either output may be NULL.
+ *   stream: cudaStream_t (as void*); the kernels are enqueued on it, the call does not synchronise.
+ * The scratch of the kernels (inverse row norms, one packed word per row of A) is a file-scope device array of
+ * FARM_NOALLOC_SCRATCH_BYTES that every GPU using the library holds until the process exits; the call allocates nothing
+ * (no cudaMalloc / cudaFree / allocating library routine).  Limits: M <= FARM_NOALLOC_MAX_M, N <= FARM_NOALLOC_MAX_N,
+ * 1 <= D <= 8192; beyond them FARM_ERR_INVALID_ARG and nothing is enqueued.  ALL calls of the process on one GPU share the
+ * array, which keeps the last call's contents (each call clears what it needs): calls that overlap on the GPU -- different
+ * streams without an ordering between them -- race; calls on one stream are safe. */
+#define FARM_NOALLOC_MAX_M 4096
+#define FARM_NOALLOC_MAX_N 65536
+#define FARM_NOALLOC_SCRATCH_BYTES 311296 /* 4 * MAX_M + 4 * MAX_N + 8 * MAX_M */
+int farm_cosine_rowmax_noalloc(const void *A, int M, const void *B, int N, int D, int dtype, float *max_cos, int32_t *argmax,
+                               void *stream);
+
 /* Retrieval-side scoring over the finished memory (a second workload beside the mapper, rules Q1-Q5 of
  * DESIGN.md).  The three per-entity retrieval embedding matrices of PAPER.md:356 (caption text, image, image-VL), the
  * class ids and the query vectors are INPUTS; parser, encoders and the VLM reranker are out of scope.

@@ -49,7 +49,7 @@ EXPORTS = ["farm_map_create", "farm_map_destroy", "farm_map_set_option_i", "farm
            "farm_map_read",
            "farm_map_import", "farm_map_sync", "farm_map_kernel_launches", "farm_last_error",
            "farm_map_get_frame_seq", "farm_map_set_frame_seq", "farm_map_read_views", "farm_map_query", "farm_map_read_alias",
-           "farm_map_last_merges", "farm_map_read_edges",
+           "farm_map_last_merges", "farm_map_read_edges", "farm_cosine_rowmax_noalloc",
            "farm_debug_backproject", "farm_debug_last_voxels", "farm_debug_last_overlaps", "farm_debug_last_dense"]
 
 
@@ -87,6 +87,7 @@ def load_library():
         lib.farm_map_read_views.argtypes = [vp, vp, vp]
         lib.farm_map_read_alias.argtypes = [vp, vp]
         lib.farm_map_read_edges.argtypes = [vp, vp, vp, vp, C.c_uint64, vp]
+        lib.farm_cosine_rowmax_noalloc.argtypes = [vp, ci, vp, ci, ci, ci, vp, vp, vp]
         lib.farm_map_last_merges.argtypes = [vp, vp, vp, vp]
         lib.farm_map_query.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, ci, ci, vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.farm_map_read.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -122,6 +123,17 @@ def _dp(t):
         return C.c_void_p(t)
     assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
     return C.c_void_p(t.data_ptr())
+
+
+NOALLOC_MAX_M, NOALLOC_MAX_N = 4096, 65536
+
+
+def cosine_rowmax_noalloc(A, M, B, N, D, dtype, max_cos, argmax, stream=None):
+    """farm_cosine_rowmax_noalloc: dense cosine of A [M, D] against B [N, D] (DEVICE, `dtype`) with fused row max / argmax into
+    max_cos f32 [M] / argmax i32 [M] (DEVICE); allocates nothing (fixed scratch array in the library, M <= 4096, N <= 65536);
+    enqueued on `stream` (a cudaStream_t as int, default stream if None), not synchronised."""
+    _check(load_library().farm_cosine_rowmax_noalloc(_dp(A), int(M), _dp(B), int(N), int(D), int(dtype), _dp(max_cos), _dp(argmax),
+                                                     C.c_void_p(stream) if stream else None))
 
 
 class FarmMap:

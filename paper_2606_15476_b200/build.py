@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfarm_map.so")
-SOURCES = ["farm_api.cu", "farm_lift.cu", "farm_sim_fma.cu", "farm_sim_tc.cu", "farm_assoc.cu", "farm_query.cu", "farm_edges.cu"]
+SOURCES = ["farm_api.cu", "farm_lift.cu", "farm_sim_fma.cu", "farm_sim_tc.cu", "farm_assoc.cu", "farm_query.cu", "farm_edges.cu", "farm_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr"]

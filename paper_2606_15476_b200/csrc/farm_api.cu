@@ -18,6 +18,8 @@ int run_query(const DevMap &m, cudaStream_t st, uint32_t N, const void *const em
               const float *q_target, int target_class, int P, const int32_t *pred_type, const float *q_landmarks, int topk,
               int32_t *top_ids, float *top_scores, int32_t *landmarks, float *s_sem, float *gbar, float *s, long long *launches,
               std::string *err);
+int noalloc_cosine_rowmax(const void *A, int M, const void *B, int N, int D, int dtype, float *max_cos, int32_t *argmax,
+                          cudaStream_t s, std::string *err);
 bool tc_prepare(void *tc_state, const DevMap &m, const CallArgs &a);
 void *tc_state_create(const DevMap &m);
 void tc_state_destroy(void *);
@@ -1114,6 +1116,22 @@ int farm_map_read_views(farm_map *m, farm_view *views, int32_t *counts) {
   if (views && N) CU(cudaMemcpy(views, m->dm.views, (size_t)N * m->views_k * sizeof(farm_view), cudaMemcpyDeviceToHost));
   if (counts && N) CU(cudaMemcpy(counts, m->dm.view_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost));
   return FARM_OK;
+}
+
+int farm_cosine_rowmax_noalloc(const void *A, int M, const void *B, int N, int D, int dtype, float *max_cos, int32_t *argmax,
+                               void *stream) {
+  if (M < 0 || N < 0) return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: negative size");
+  if (M > FARM_NOALLOC_MAX_M)
+    return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: M exceeds FARM_NOALLOC_MAX_M (4096): the scratch array is fixed-size");
+  if (N > FARM_NOALLOC_MAX_N)
+    return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: N exceeds FARM_NOALLOC_MAX_N (65536): the scratch array is fixed-size");
+  if (D < 1 || D > 8192) return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: D must be in 1..8192");
+  if (dtype != FARM_DTYPE_F32 && dtype != FARM_DTYPE_F16 && dtype != FARM_DTYPE_BF16)
+    return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: bad dtype");
+  if ((M > 0 && !A) || (N > 0 && !B)) return fail(FARM_ERR_INVALID_ARG, "farm_cosine_rowmax_noalloc: NULL operand");
+  std::string err;
+  const int rc = noalloc_cosine_rowmax(A, M, B, N, D, dtype, max_cos, argmax, (cudaStream_t)stream, &err);
+  return rc == FARM_OK ? FARM_OK : fail(rc, err);
 }
 
 int farm_map_read_edges(farm_map *m, uint32_t *ea, uint32_t *eb, double *ew, uint64_t capacity, uint64_t *n_out) {
