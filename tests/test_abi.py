@@ -162,3 +162,15 @@ def test_round2_options_and_calls_validate_on_the_host(lib):
                              None, None, None, None, None, None)
     assert rc == binding.ERR_INVALID_ARG                     # too many predicates
     m2.destroy()
+
+
+def test_no_alloc_entry_point_rejects_oversized_requests_on_the_host(lib):
+    """farm_cosine_rowmax_noalloc checks its sizes against the fixed scratch array before touching the device."""
+    from paper_2606_15476_b200 import binding
+    lib_ = binding.load_library()
+    for M, N, D, dt in ((binding.NOALLOC_MAX_M + 1, 1, 8, 0), (1, binding.NOALLOC_MAX_N + 1, 8, 0), (1, 1, 0, 0), (1, 1, 8193, 0),
+                        (1, 1, 8, 3), (-1, 1, 8, 0), (1, 1, 8, 0)):            # the last one: NULL operands
+        assert lib_.farm_cosine_rowmax_noalloc(None, M, None, N, D, dt, None, None, None) == binding.ERR_INVALID_ARG
+    assert b"FARM_NOALLOC_MAX_M" in lib_.farm_last_error() or b"NULL" in lib_.farm_last_error()
+    hdr = open(os.path.join(os.path.dirname(__file__), "..", "include", "farm.h")).read()
+    assert f"#define FARM_NOALLOC_MAX_M {binding.NOALLOC_MAX_M}" in hdr and f"#define FARM_NOALLOC_MAX_N {binding.NOALLOC_MAX_N}" in hdr
