@@ -48,6 +48,10 @@ def parse():
     p.add_argument("--extras", nargs="?", const="gaussian,covisibility,views,edges", default="",
                    help="also maintain optional structures, a comma list of gaussian, covisibility, views (4), edges (k = 4; needs "
                         "gaussian); no value = all four (not the headline configuration; config.extras says so)")
+    p.add_argument("--inputs-ready", type=int, default=0,
+                   help="FARM_OPT_INPUTS_READY for the device-resident arm: every batch is staged in HBM and synchronised before the "
+                        "timed region, so the library may start a call's similarity kernel before the previous call's merge "
+                        "(0 = stream-ordered inputs, the library default)")
     p.add_argument("--no-single-frame", action="store_true", help="skip the single-frame latency series of configs[0..3]")
     p.add_argument("--full-oracle-batch", action="store_true",
                    help="cpu_baseline / --impl reference: time ONE full 16-frame, 1600-detection batch (minutes on one core)")
@@ -260,7 +264,7 @@ def run_ours(args):
         m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype,
                     max_objects=max_objects, max_voxels=max_voxels, max_blocks=max_blocks, max_det_per_call=FRAMES_PER_BATCH * DET_PER_FRAME,
                     max_frames_per_call=FRAMES_PER_BATCH, max_pairs_per_call=1 << 21, stream=stream.cuda_stream,
-                    timing=timing, overlap=args.overlap, sim_path=args.sim_path,
+                    timing=timing, overlap=args.overlap, sim_path=args.sim_path, inputs_ready=args.inputs_ready,
                     **{k: {"gaussian": 1, "covisibility": 1, "views": 4, "edges": 4}[k] for k in args.extras.split(",") if k})
         m.import_(objs, desc, keys, owner)
         return m

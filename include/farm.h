@@ -91,6 +91,18 @@ extern "C" {
 #define FARM_OPT_EDGES 19             /* k in 0..16: maintain the weighted covisibility edge dictionary of PAPER.md:354 (rules
                                         W1-W4 of DESIGN.md; see farm_map_read_edges); default 0 = off.  Needs
                                         FARM_OPT_GAUSSIAN = 1; not available together with FARM_OPT_CORRESPONDENCE          */
+#define FARM_OPT_INPUTS_READY 20      /* 1: the caller guarantees that the inputs of every integrate call are COMPLETE in device memory
+                                        when the call is made -- not merely ordered before it on the map's stream -- and stay
+                                        untouched until the call's work is done.  From the third call on, the similarity kernel of
+                                        a call then no longer waits for the previous call's merge: it starts when the previous
+                                        similarity kernel ends, computes the rows that merge does not write, and the rows it does
+                                        write afterwards (split schedule).  Results are identical.  Takes
+                                        effect with the 16-bit dtypes on the tensor-core path (FARM_OPT_SIM_PATH 0 or 2),
+                                        FARM_OPT_OVERLAP = 1, and without FARM_OPT_CORRESPONDENCE / FARM_OPT_GEOMETRY; otherwise it
+                                        is accepted and changes nothing.  farm_map_integrate_batch_host orders its own staging
+                                        copies and may always be used with it.  Measured on configs[4]: no faster than the
+                                        stream-ordered schedule.  With FARM_OPT_TIMING = 1 only every
+                                        eighth similarity kernel is bracketed by events and the sum is scaled.  Default 0      */
 /* float options (farm_map_set_option_f) */
 #define FARM_OPTF_Z_MIN 101          /* exclusive lower depth bound, default 0                                  */
 #define FARM_OPTF_Z_MAX 102          /* inclusive upper depth bound, default +inf                               */

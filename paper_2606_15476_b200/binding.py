@@ -27,6 +27,7 @@ OPT_VIEWS = 16
 OPT_CORRESPONDENCE = 17
 OPT_GEOMETRY = 18
 OPT_EDGES = 19
+OPT_INPUTS_READY = 20
 OPTF_EDGE_DECAY, OPTF_EDGE_CUTOFF = 107, 108
 N_STAGES = 6
 STAGE_NAMES = ["prep", "lift", "similarity", "probe", "associate", "merge"]
@@ -143,7 +144,7 @@ class FarmMap:
                  max_voxels=None, max_blocks=None, max_det_per_call=None, max_pairs_per_call=None, max_frames_per_call=None,
                  stream=None, z_min=None, z_max=None, sim_path=None, timing=None, overlap=None, gaussian=None, covisibility=None,
                  views=None, view_cos=None, view_closer=None, correspondence=None, geometry=None, prefilter_cos=None,
-                 hellinger_budget=None, edges=None, edge_decay=None, edge_cutoff=None):
+                 hellinger_budget=None, edges=None, edge_decay=None, edge_cutoff=None, inputs_ready=None):
         lib = load_library()
         self.D, self.dtype, self.H, self.W = D, dtype, H, W
         self._last_M = 0
@@ -157,7 +158,7 @@ class FarmMap:
                        (OPT_MAX_FRAMES_PER_CALL, max_frames_per_call), (OPT_STREAM, stream), (OPT_SIM_PATH, sim_path),
                        (OPT_TIMING, timing), (OPT_OVERLAP, overlap), (OPT_GAUSSIAN, gaussian), (OPT_COVISIBILITY, covisibility),
                        (OPT_VIEWS, views), (OPT_CORRESPONDENCE, correspondence), (OPT_GEOMETRY, geometry),
-                       (OPT_EDGES, edges)):
+                       (OPT_EDGES, edges), (OPT_INPUTS_READY, inputs_ready)):
             if v is not None:
                 self.set_option_i(key, int(v))
         if z_min is not None:

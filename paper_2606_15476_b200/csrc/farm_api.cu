@@ -12,8 +12,9 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+bool tc_can_split(void *tc_state);
 int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *tc_state, uint32_t prep_target,
-                         int *n_ctas);
+                         int *n_ctas, uint32_t *prep_after);
 int run_query(const DevMap &m, cudaStream_t st, uint32_t N, const void *const emb[3], const int dim[3], int emb_dtype, const int32_t *cls,
               const float *q_target, int target_class, int P, const int32_t *pred_type, const float *q_landmarks, int topk,
               int32_t *top_ids, float *top_scores, int32_t *landmarks, float *s_sem, float *gbar, float *s, long long *launches,
@@ -47,6 +48,27 @@ struct farm_map {
   int sim_path = 0, gaussian = 0, covis = 0, views_k = 0, corr = 0, geom = 0, edges_k = 0;
   float edge_decay = 0.9f, edge_cutoff = 2.0f;
   uint32_t edge_calls = 0;  // integrate calls so far: the clock of W4's decay
+  // FARM_OPT_INPUTS_READY: split similarity schedule
+  int inputs_ready = 0;
+  uint32_t seq = 0;             // sequence number of the last integrate call (CallArgs.seq)
+  long long sim_timed = 0, sim_all = 0;  // timing 1: similarity launches bracketed by events / all of them (since the last reset)
+  uint32_t scan_count = 0;      // decision scans launched so far (device counter dm.scan_done)
+  uint32_t merge_count = 0;     // merge warps launched so far (device counter dm.merge_done)
+  // what the lift kernel writes, double buffered by call parity: with the split schedule the lift of call c runs on its own
+  // stream while the main chain is still at call c-1
+  struct LiftSet {
+    unsigned long long *surv_key, *surv_bits;
+    uint32_t *surv_j, *surv_cnt, *det_npx;
+    int *det_box;
+    double *det_gm;
+    float *cam;
+    CallStats *stats;
+  } lset[2] = {};
+  cudaStream_t early = nullptr;                 // prep (lift part) + lift of a split call
+  cudaEvent_t ev_lift = nullptr, ev_end[2] = {nullptr, nullptr};
+  bool ev_end_set[2] = {false, false};
+  float *inv_norm2[2] = {nullptr, nullptr};               // det_inv_norm / best_dense, double buffered by call parity: the
+  unsigned long long *best_dense2[2] = {nullptr, nullptr};  //   similarity kernel of call c writes them while call c-1 still reads its own
   float view_cos = 0.8660254f, view_closer = 0.8f, prefilter_cos = 0.5f, hell_budget = 1.0f;
   cudaStream_t stream = 0;
   bool finalised = false;
@@ -55,7 +77,7 @@ struct farm_map {
   long long launches = 0;
   unsigned long long frame_seq = 0;
   uint32_t epoch = 0;
-  uint32_t sim_target = 0;   // cumulative number of similarity CTAs launched (device counter dm.sim_done)
+  uint32_t sim_target[2] = {0, 0};  // cumulative number of similarity CTAs launched, per slot of dm.sim_done (parity of CallArgs.seq)
   uint32_t prep_target = 0;  // cumulative number of prep_kernel CTAs launched (device counter dm.prep_done)
   uint32_t n_upper = 0;  // host upper bound of N (no device sync on the integrate path)
   int last_M = 0;
@@ -314,6 +336,10 @@ int finalise(farm_map *m) {
     if (m->side) cudaStreamDestroy(m->side), m->side = nullptr;
     if (m->ev_fork) cudaEventDestroy(m->ev_fork), m->ev_fork = nullptr;
     if (m->ev_join) cudaEventDestroy(m->ev_join), m->ev_join = nullptr;
+    if (m->early) cudaStreamDestroy(m->early), m->early = nullptr;
+    if (m->ev_lift) cudaEventDestroy(m->ev_lift), m->ev_lift = nullptr;
+    for (int i = 0; i < 2; ++i)
+      if (m->ev_end[i]) cudaEventDestroy(m->ev_end[i]), m->ev_end[i] = nullptr;
     m->dm = DevMap{};
     cudaGetLastError();
     g_err = msg;
@@ -409,7 +435,35 @@ int finalise_impl(farm_map *m) {
   A(d.is_new, MD, 0);
   A(d.best_score, MD, 0);
   A(d.prep_done, 1, 0);
-  A(d.sim_done, 1, 0);
+  if (m->inputs_ready && m->dtype != FARM_DTYPE_F32 && (m->sim_path == 0 || m->sim_path == 2) && m->overlap == 1 && !m->corr && m->geom == 0 &&
+      m->D % 8 == 0) {
+    A(d.scan_done, 1, 0);
+    A(d.merge_done, 1, 0);
+    A(d.touch_seq, NO, 0);
+    A(d.n_hist, 2, 0);
+    {
+      uint8_t *p;
+      A(p, (size_t)m->max_det * D * m->elem(), 0);
+      d.delta_rows = p;
+    }
+    A(d.delta_id, (size_t)m->max_det, 0);
+    A(d.delta_inv, (size_t)m->max_det, 0);
+    A(d.delta_cnt, 2, 0);
+    A(m->inv_norm2[1], MD, 0);
+    A(m->best_dense2[1], MD, 0);
+    m->inv_norm2[0] = d.det_inv_norm, m->best_dense2[0] = d.best_dense;
+    farm_map::LiftSet &s1 = m->lset[1];
+    A(s1.surv_key, (size_t)scap, 0);
+    A(s1.surv_bits, (size_t)scap, 0);
+    A(s1.surv_j, (size_t)scap, 0);
+    A(s1.surv_cnt, 1, 0);
+    A(s1.det_npx, MD, 0);
+    A(s1.det_box, MD * 6, 0);
+    if (m->gaussian) A(s1.det_gm, MD * 9, 0);
+    A(s1.cam, (size_t)MAX_FRAMES * 16, 0);
+    A(s1.stats, 1, 0);
+  }
+  A(d.sim_done, 2, 0);
   d.eps2 = m->voxel_size * m->voxel_size;
   if (m->covis) {
     d.covis_words = (uint32_t)((NO + 63) / 64);
@@ -487,6 +541,14 @@ int finalise_impl(farm_map *m) {
   CU(cudaGetLastError());
   if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
   if (m->tc && m->sim_path == 3) tc_state_set_pair(m->tc, 1);
+  d.surv_cnt = d.counters + 2;
+  m->lset[0] = {d.surv_key, d.surv_bits, d.surv_j, d.surv_cnt, d.det_npx, d.det_box, d.det_gm, d.cam, d.stats};
+  if (d.touch_seq) {
+    CU(cudaStreamCreateWithFlags(&m->early, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&m->ev_lift, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&m->ev_end[0], cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&m->ev_end[1], cudaEventDisableTiming));
+  }
   if (m->overlap) {
     int prio_lo = 0, prio_hi = 0;
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -550,6 +612,10 @@ int farm_map_destroy(farm_map *m) {
   if (!m) return FARM_OK;
   if (m->finalised || !m->allocs.empty()) cudaStreamSynchronize(m->stream);
   if (m->side) cudaStreamSynchronize(m->side), cudaStreamDestroy(m->side);
+  if (m->early) cudaStreamSynchronize(m->early), cudaStreamDestroy(m->early);
+  if (m->ev_lift) cudaEventDestroy(m->ev_lift);
+  for (int i = 0; i < 2; ++i)
+    if (m->ev_end[i]) cudaEventDestroy(m->ev_end[i]);
   if (m->cstream) cudaStreamSynchronize(m->cstream), cudaStreamDestroy(m->cstream);
   for (auto &g : m->stg) {
     if (g.copied) cudaEventDestroy(g.copied);
@@ -637,6 +703,10 @@ int farm_map_set_option_i(farm_map *m, int key, long long v) {
       if (v < 0 || v > 8) return fail(FARM_ERR_INVALID_ARG, "bad VIEWS (0..8)");
       m->views_k = (int)v;
       break;
+    case FARM_OPT_INPUTS_READY:
+      if (v < 0 || v > 1) return fail(FARM_ERR_INVALID_ARG, "bad INPUTS_READY");
+      m->inputs_ready = (int)v;
+      break;
     case FARM_OPT_EDGES:
       if (v < 0 || v > 16) return fail(FARM_ERR_INVALID_ARG, "bad EDGES (0..16)");
       m->edges_k = (int)v;
@@ -711,12 +781,25 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (m->tc && M > 0 && m->n_upper > 0 && !tc_prepare(m->tc, d, a))
     return fail(FARM_ERR_INVALID_ARG, "similarity: det_descriptors must be 16-byte aligned for the 16-bit dtypes (TMA operand)");
   a.epoch = ++m->epoch;
+  const bool maintain = m->dm.touch_seq != nullptr;  // the split similarity schedule is available on this map
+  if (maintain) {
+    a.seq = ++m->seq;
+    m->dm.det_inv_norm = m->inv_norm2[a.seq & 1], m->dm.best_dense = m->best_dense2[a.seq & 1];
+    const farm_map::LiftSet &ls = m->lset[a.seq & 1];
+    DevMap &w = m->dm;
+    w.surv_key = ls.surv_key, w.surv_bits = ls.surv_bits, w.surv_j = ls.surv_j, w.surv_cnt = ls.surv_cnt, w.det_npx = ls.det_npx;
+    w.det_box = ls.det_box, w.det_gm = ls.det_gm, w.cam = ls.cam, w.stats = ls.stats;
+  }
   cudaStream_t st = m->stream;
   bool launch_failed = false;
   auto stage = [&](int id, cudaStream_t st, auto &&fn) {
     // timing 1: only the similarity kernel (it has the side stream to itself, so its events do not sit between
     // the PDL-chained kernels of the main stream); timing 2: every kernel (serialises the main-stream chain)
-    const bool timed = m->timing >= 2 || (m->timing == 1 && id == FARM_STAGE_SIMILARITY);
+    // Split schedule: events between two similarity kernels would undo their programmatic overlap, so with timing 1 only
+    // every eighth of them is bracketed (it then runs without overlap) and farm_map_stage_times scales the sum
+    bool timed = m->timing >= 2 || (m->timing == 1 && id == FARM_STAGE_SIMILARITY);
+    if (timed && id == FARM_STAGE_SIMILARITY && a.split && (a.seq & 7) != 0) timed = false;
+    if (id == FARM_STAGE_SIMILARITY && m->timing == 1) m->sim_timed += timed ? 1 : 0, m->sim_all += 1;
     cudaEvent_t e0 = nullptr;
     if (timed) {
       e0 = get_event(m);
@@ -740,12 +823,30 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   // The tensor-core similarity kernel needs prep's output (row norms, zeroed best_dense) only in its epilogue and
   // waits for it on the device (dm.prep_done), so it is forked BEFORE prep: prep leaves the critical path.
   const bool early_fork = fork && m->tc && m->overlap == 1;
-  if (early_fork) {
+  // Split schedule (FARM_OPT_INPUTS_READY, from the third call on): no fork event -- the similarity kernel follows the
+  // previous call's similarity kernel on the side stream and takes what it needs of the previous call's scan and merge
+  // through device counters.  Not with per-kernel timing: the events would serialise the two streams.
+  a.split = (early_fork && maintain && a.seq >= 3 && m->timing < 2 && tc_can_split(m->tc)) ? 1 : 0;
+  a.scan_target = m->scan_count, a.merge_target = m->merge_count;
+  if (early_fork && !a.split) {
     cudaEventRecord(m->ev_fork, st);
     cudaStreamWaitEvent(m->side, m->ev_fork, 0);
   }
+  if (a.split) {
+    // the lift of this call does not depend on the map: it runs on its own stream, behind the call before the previous one
+    // (the last user of this parity's buffers), while the main chain is still busy with the previous call's scan and merge
+    const int par = (int)(a.seq & 1);
+    if (m->ev_end_set[par]) cudaStreamWaitEvent(m->early, m->ev_end[par], 0);
+    stage(FARM_STAGE_PREP, m->early, [&] {
+      launch_prep(d, a, m->early, 1);
+      return 1;
+    });
+    stage(FARM_STAGE_LIFT, m->early, [&] { return launch_lift(d, a, m->early); });
+    cudaEventRecord(m->ev_lift, m->early);
+    cudaStreamWaitEvent(st, m->ev_lift, 0);
+  }
   stage(FARM_STAGE_PREP, st, [&] {
-    m->prep_target += (uint32_t)launch_prep(d, a, st);
+    m->prep_target += (uint32_t)launch_prep(d, a, st, a.split ? 2 : 0);
     return 1;
   });
   if (fork && m->overlap == 3) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
@@ -757,28 +858,39 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   stage(FARM_STAGE_SIMILARITY, sim_stream, [&] {
     if (!m->tc) return launch_similarity_fma(d, a, m->n_upper, sim_stream);
     int ctas = 0;
-    const int n = launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc, m->prep_target, &ctas);
-    m->sim_target += (uint32_t)ctas;
+    uint32_t prep_after = m->prep_target;
+    const int n = launch_similarity_tc(d, a, m->n_upper, sim_stream, m->tc, m->prep_target, &ctas, &prep_after);
+    m->sim_target[a.seq & 1] += (uint32_t)ctas;
+    m->prep_target = prep_after;
     return n;
   });
+  a.prep_target = m->prep_target;
   // With the early fork the association kernel is not joined to the side stream: it is launched (PDL) right behind
   // the probe, scores the candidates while the similarity kernel finishes, and its decision scan waits for
   // dm.sim_done on the device.  The stream join moves behind the merge kernel, off the critical path.
   a.wait_sim = early_fork ? 1 : 0;
-  a.sim_target = m->sim_target;
-  if (fork) cudaEventRecord(m->ev_join, m->side);
-  if (!(fork && m->overlap == 3)) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
+  a.sim_target = m->sim_target[a.seq & 1];
+  // Split schedule: no join event.  The decision scan waits on the device for every CTA of the similarity kernel (dm.sim_done,
+  // incremented after the CTA's last write), and everything the main stream does after it is ordered behind that; an event
+  // between two similarity kernels would also undo their programmatic overlap.
+  if (fork && !a.split) cudaEventRecord(m->ev_join, m->side);
+  if (!(fork && m->overlap == 3) && !a.split) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork && m->overlap == 2) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st) + launch_dd_overlap(d, a, st); });
   if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });
+  if (maintain) m->scan_count += 1, m->merge_count += (uint32_t)merge_warps_of(a);
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covis_absorb(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_covisibility(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_alias_compress(d, a, (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects), st); });
   m->edge_calls++;
   stage(FARM_STAGE_MERGE, st, [&] { return launch_edges(d, a, m->edge_calls, st); });
-  if (early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
+  if (early_fork && !a.split) cudaStreamWaitEvent(st, m->ev_join, 0);
+  if (maintain) {
+    cudaEventRecord(m->ev_end[a.seq & 1], st);
+    m->ev_end_set[a.seq & 1] = true;
+  }
   m->frame_seq += F;
   m->n_upper = (uint32_t)std::min<long long>((long long)m->n_upper + M, m->max_objects);
   m->last_M = (int)M;
@@ -996,6 +1108,8 @@ int farm_map_integrate_batch_host(farm_map *m, int F, const float *depth, const 
   if (M) CU(cudaMemcpyAsync(g.desc, desc, (size_t)M * m->D * m->elem(), cudaMemcpyHostToDevice, m->cstream));
   CU(cudaEventRecord(g.copied, m->cstream));
   CU(cudaStreamWaitEvent(m->stream, g.copied, 0));
+  if (m->dm.touch_seq && m->side) CU(cudaStreamWaitEvent(m->side, g.copied, 0));  // the split similarity kernel reads the staged rows too
+  if (m->dm.touch_seq && m->early) CU(cudaStreamWaitEvent(m->early, g.copied, 0));  // and so does its lift kernel
   rc = farm_map_integrate_batch(m, F, g.depth, g.mask, g.K, g.T, M ? g.desc : nullptr, n_det);
   CU(cudaEventRecord(g.free, m->stream));
   g.used = true;
@@ -1205,9 +1319,12 @@ int farm_map_stage_times(farm_map *m, float *ms, long long *launches, int reset)
     }
     m->ev_pending[s].clear();
     if (ms) ms[s] = (float)m->stage_ms[s];
+    if (s == FARM_STAGE_SIMILARITY && ms && m->timing == 1 && m->sim_timed > 0 && m->sim_timed < m->sim_all)
+      ms[s] = (float)(m->stage_ms[s] * (double)m->sim_all / (double)m->sim_timed);  // split schedule: sampled launches, scaled
     if (launches) launches[s] = m->stage_launches[s];
     if (reset) m->stage_ms[s] = 0.0, m->stage_launches[s] = 0;
   }
+  if (reset) m->sim_timed = 0, m->sim_all = 0;
   return FARM_OK;
 }
 

@@ -5,6 +5,7 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+FARM_TRACE_TABLE(farm_trace_assoc)  // 0 first CTA past pdl_wait, 1 scoring over (last CTA), 3 scan start (similarity done), 5 scan end, 2 merge start, 7 merge warps end
 namespace {
 
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
@@ -361,6 +362,11 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
   __shared__ bool s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   pdl_wait();     // launched with PDL behind the probe kernel: candidates and overlap counts are final from here on
+  if (tid == 0) TRACE_MIN(farm_trace_assoc, a.seq, 0);
+  if (a.split) {  // the row norms of this call come from the similarity kernel (other stream), not from prep
+    if (tid == 0) spin_until(m.prep_done, a.prep_target, m.err);
+    __syncthreads();
+  }
   {
     const uint32_t n_cand = min(m.counters[1], m.cand_cap);
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
@@ -420,7 +426,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
     // pairs above the similarity threshold (emitted by the similarity epilogue): H candidates / U1 edges without overlap
     if (m.dense_d && (m.geom == 1 || m.corr)) {
       if (a.wait_sim) {  // the list is complete only when the similarity grid has finished
-        if (tid == 0) spin_until(m.sim_done, a.sim_target, m.err);
+        if (tid == 0) spin_until(m.sim_done + (a.seq & 1), a.sim_target, m.err);
         __syncthreads();
       }
       const uint32_t n_dense = min(__ldcg(&m.counters[4]), m.dense_cap);
@@ -448,6 +454,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
   }
   __syncthreads();
   if (!s_last) return;
+  if (tid == 0) TRACE_MAX(farm_trace_assoc, a.seq, 1);
   // Everything the decisions need except the dense row maxima is final once the last CTA is here (lift, probe and all
   // candidate scores are done): request it BEFORE waiting for the similarity grid, so that only best_dense is loaded after.
   unsigned long long pre_bc[CAND_PER];
@@ -462,9 +469,10 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
   }
   const unsigned long long pre_valid = tid == 0 ? __ldcg(&m.stats->valid_points) : 0ull;
   if (a.wait_sim) {  // no stream join before this kernel: wait here for the similarity grid before reading its row maxima
-    if (tid == 0) spin_until(m.sim_done, a.sim_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
+    if (tid == 0) spin_until(m.sim_done + (a.seq & 1), a.sim_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
     __syncthreads();
   }
+  if (tid == 0) TRACE_MAX(farm_trace_assoc, a.seq, 3);
   pdl_trigger();  // the merge kernel becomes resident now, not while the similarity kernel still runs
   if (m.corr) {  // U: union-find over the match graph instead of the per-detection argmax
     correspondence_decide(m, a, N);
@@ -558,6 +566,7 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
         if (target[k] >= 0) {
           atomicMin(&m.leader[target[k]], (uint32_t)j);
           atomicAdd(&m.grp_cnt[target[k]], 1u);
+          if (m.touch_seq && !is_new) m.touch_seq[target[k]] = a.seq;  // the next call's similarity masks this row in phase 1
         }
       }
       total += sub_total;
@@ -589,6 +598,13 @@ __global__ void __maxnreg__(80) cand_associate_kernel(const __grid_constant__ De
     atomicAdd(&m.totals->unique_voxels, pairs);
     atomicAdd(&m.totals->matches, (unsigned long long)s_matches);
     atomicAdd(&m.totals->spawns, (unsigned long long)spawns);
+    TRACE_MAX(farm_trace_assoc, a.seq, 5);
+    if (m.touch_seq) {  // split similarity: what the next two calls' kernels read
+      m.n_hist[(a.seq + 1) & 1] = N + spawns;
+      m.delta_cnt[a.seq & 1] = 0;  // this call's merge warps count their rows from here
+      __threadfence();
+      atomicAdd(m.scan_done, 1u);  // touch_seq, n_hist are final (every thread's stores precede the barrier above)
+    }
   }
 }
 
@@ -661,6 +677,23 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
     return;
   }
   // ---- merge: one WARP per detection; only the lowest-index detection of a target object works (R21-R23)
+  // Split similarity: every merge warp reports when it leaves (whichever return it takes); the next call's similarity kernel,
+  // already running, starts its phase 2 when all of them have.
+  struct Report {
+    uint32_t *ctr;
+    int lane;
+    uint32_t seq;
+    __device__ ~Report() {
+      if (lane == 0) TRACE_MAX(farm_trace_assoc, seq, 7);
+      if (!ctr) return;
+      __syncwarp();
+      if (lane == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1u);
+      }
+    }
+  } report{m.merge_done, lane, a.seq};
+  if (lane == 0) TRACE_MIN(farm_trace_assoc, a.seq, 2);
   const int j = blockIdx.x * MERGE_WARPS + warp;
   if (j >= a.M) return;
   const int32_t t = m.assoc[j];
@@ -854,6 +887,23 @@ __global__ void __launch_bounds__(MERGE_THREADS) commit_merge_kernel(const __gri
     for (int sft = 16; sft; sft >>= 1) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, sft);
     if (lane == 0) m.inv_norm[t] = s2 > 0.f ? 1.0f / sqrtf(s2) : 0.f;
   }
+  if (m.delta_rows) {
+    // split similarity: the row as it stands now (rewritten above, or kept), its id and inverse norm also go to the delta
+    // buffer -- the B operand of the next call's phase 2
+    __syncwarp();
+    uint32_t slot = 0;
+    if (lane == 0) slot = atomicAdd(&m.delta_cnt[a.seq & 1], 1u);
+    slot = __shfl_sync(0xFFFFFFFFu, slot, 0);
+    if (slot < m.max_det) {
+      T *drow = (T *)m.delta_rows + (size_t)slot * D;
+      if (sizeof(T) == 2 && (D & 7) == 0) {
+        for (int i = lane * 8; i < D; i += 256) *reinterpret_cast<uint4 *>(drow + i) = *reinterpret_cast<const uint4 *>(shadow + i);
+      } else {
+        for (int i = lane; i < D; i += 32) drow[i] = shadow[i];
+      }
+      if (lane == 0) m.delta_id[slot] = (uint32_t)t, m.delta_inv[slot] = m.inv_norm[t];
+    }
+  }
   if (lane == 0) {
     m.n_obs[t] = n_old + loser_obs + k_members;
     m.n_points[t] = pts_old + pts;
@@ -1017,12 +1067,21 @@ int launch_covisibility(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   launch_pdl(covisibility_kernel, dim3(grid), dim3(COVIS_THREADS), (size_t)m.covis_words * 8 + n_list_max * 2, s, m, a);
   return 1;
 }
+int merge_warps_of(const CallArgs &a) { return a.M > 0 ? (a.M + MERGE_WARPS - 1) / MERGE_WARPS * MERGE_WARPS : 0; }
+
 int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long frame_seq0, cudaStream_t s) {
   if (a.M == 0) return 0;
   const int commit_blocks = m.num_sms * 4;
   const int merge_blocks = (a.M + MERGE_WARPS - 1) / MERGE_WARPS;  // one warp per detection
-  FARM_DISPATCH((launch_pdl(commit_merge_kernel<T>, dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s, m, a, frame_seq0,
-                            commit_blocks)));
+  if (a.split) {
+    // Split schedule: no programmatic early launch.  CTAs of this grid that sit in pdl_wait() while the decision scan runs
+    // hold their registers (256 x 119), and the next call's similarity kernel -- which starts in exactly that window -- would
+    // find no room on those SMs until this grid has drained (measured: its last CTA started 22-25 us late).
+    FARM_DISPATCH((commit_merge_kernel<T><<<dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s>>>(m, a, frame_seq0, commit_blocks)));
+  } else {
+    FARM_DISPATCH((launch_pdl(commit_merge_kernel<T>, dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s, m, a, frame_seq0,
+                              commit_blocks)));
+  }
   return 1;
 }
 

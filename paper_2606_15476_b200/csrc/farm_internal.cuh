@@ -108,6 +108,7 @@ struct DevMap {
   unsigned long long *surv_bits;     //   tile-level aggregation
   uint32_t *surv_j;
   uint32_t surv_cap;
+  uint32_t *surv_cnt;                // records reserved in the survivor queue (counters + 2, or the call-parity copy)
   uint32_t *counters;                // [0]=event_count [1]=cand_count [2]=survivor_count [3]=block ticket
                                      // [4]=dense pairs [5]=edges [6]=detection-detection edges [7]=entity merges
                                      // [8]=|S| of the call (W1) [9]=entries of the edge dictionary (W4)
@@ -159,8 +160,20 @@ struct DevMap {
   double *ed_w;                      //   weight as of call ed_t
   uint32_t *ed_t;                    //   index (1-based) of the call that last updated the edge
   uint32_t ed_mask;
-  uint32_t *sim_done;                // cumulative count of finished similarity CTAs (the association scan waits on it)
+  uint32_t *sim_done;                // [2] cumulative count of finished similarity CTAs (the association scan waits on it); slot =
+                                     //   parity of CallArgs.seq (0 without the split schedule): kernels of consecutive calls may overlap
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
+  // FARM_OPT_INPUTS_READY (split similarity); all null when the option is off.  The similarity kernel of
+  // call c starts when that of call c-1 ends: phase 1 covers the rows that existed at the entry of call c-1 minus the rows
+  // call c-1 merged into (their columns are masked), phase 2 -- after call c-1's merge warps -- the rows of `delta`.
+  uint32_t *scan_done;               // cumulative count of finished decision scans (one per call)
+  uint32_t *merge_done;              // cumulative count of finished merge warps
+  uint32_t *touch_seq;               // [max_objects] sequence number of the last call that merged a detection into the object
+  uint32_t *n_hist;                  // [2] n_hist[(s + 1) & 1] = number of objects after the call with sequence number s
+  void *delta_rows;                  // [max_det, D] storage dtype: the rows written by the last call's merge (old and new objects)
+  uint32_t *delta_id;                // [max_det] their object ids
+  float *delta_inv;                  // [max_det] and inverse norms
+  uint32_t *delta_cnt;               // [2] rows in delta, indexed by the parity of the writing call's sequence number
   float *cam;                        // [MAX_FRAMES,16] per-frame camera block written by prep_kernel
   CallStats *stats;
   Totals *totals;
@@ -172,6 +185,12 @@ struct CallArgs {
   uint32_t epoch;
   uint32_t sim_target;  // value dm.sim_done reaches when this call's similarity kernel has finished
   int wait_sim;         // 1: cand_associate is launched without a stream join and waits for sim_target itself
+  // FARM_OPT_INPUTS_READY
+  uint32_t seq;           // sequence number of the call (1, 2, ...), the clock of touch_seq / n_hist / delta_cnt
+  int split;              // 1: the similarity kernel runs the two-phase schedule and does its own share of prep
+  uint32_t prep_target;   //   value dm.prep_done reaches when the row norms of this call are final (cand_associate waits)
+  uint32_t scan_target;   //   value dm.scan_done reaches when the PREVIOUS call's decision scan is done
+  uint32_t merge_target;  //   value dm.merge_done reaches when the PREVIOUS call's merge warps are done
   const float *depth;
   const uint16_t *mask;
   const float *K;
@@ -265,6 +284,34 @@ __device__ __forceinline__ bool spin_until(const uint32_t *ctr, uint32_t target,
   return false;
 }
 
+// -DFARM_TRACE (development builds only): %globaltimer stamps per call, one table per translation unit
+#ifdef FARM_TRACE
+#define FARM_TRACE_TABLE(name)                                                                               \
+  static __device__ unsigned long long name[16][8];                                                          \
+  extern "C" int name##_read(unsigned long long *out, int reset) {                                           \
+    cudaDeviceSynchronize();                                                                                 \
+    if (out && cudaMemcpyFromSymbol(out, name, sizeof(name)) != cudaSuccess) return -2;                      \
+    if (reset) {                                                                                             \
+      static unsigned long long init[16][8];                                                                 \
+      for (int i = 0; i < 16; ++i)                                                                           \
+        for (int k = 0; k < 8; ++k) init[i][k] = (k & 1) ? 0ull : ~0ull; /* even slots: minima, odd: maxima */ \
+      if (cudaMemcpyToSymbol(name, init, sizeof(init)) != cudaSuccess) return -2;                            \
+    }                                                                                                        \
+    return 0;                                                                                                \
+  }
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+#define TRACE_MIN(tab, seq, k) atomicMin(&tab[(seq) & 15][k], gtime())
+#define TRACE_MAX(tab, seq, k) atomicMax(&tab[(seq) & 15][k], gtime())
+#else
+#define FARM_TRACE_TABLE(name)
+#define TRACE_MIN(tab, seq, k) ((void)0)
+#define TRACE_MAX(tab, seq, k) ((void)0)
+#endif
+
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 template <typename... KArgs, typename... Args>
@@ -286,7 +333,9 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 void configure_lift_kernels();
 void configure_assoc_kernels();
 void configure_edge_kernels();
-int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);  // returns the number of CTAs it launched
+// part 0: everything; with the split schedule the lift runs ahead on its own stream: part 1 = what the lift kernel needs
+// (camera blocks, cleared survivor count, statistics and per-detection evidence), part 2 = the rest, in the main chain
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s, int part = 0);  // returns the number of CTAs that report to prep_done
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,
@@ -299,6 +348,7 @@ int launch_covis_absorb(const DevMap &m, const CallArgs &a, uint32_t n_upper, cu
 int launch_edges(const DevMap &m, const CallArgs &a, uint32_t call, cudaStream_t s);
 int launch_edge_export(const DevMap &m, uint32_t call, uint32_t *out_a, uint32_t *out_b, double *out_w, uint32_t cap, uint32_t *count,
                        cudaStream_t s);
+int merge_warps_of(const CallArgs &a);  // warps of the merge kernel that report to dm.merge_done
 int launch_dd_overlap(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_alias_compress(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s);
 

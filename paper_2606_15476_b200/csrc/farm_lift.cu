@@ -80,20 +80,27 @@ __device__ __forceinline__ bool depth_valid(float z, float z_min, float z_max) {
 
 // ---------------------------------------------------------------------------------------------------
 // prep: reset per-call state and compute detection row norms (operand A of step 4).  One warp per row.
+// part 0 = everything (one launch per call).  Split schedule: part 1 = the state the lift kernel works on (launched with the
+// lift kernel on its own stream, ahead of the previous call's tail), part 2 = the rest (main stream, behind that tail).
 template <typename T>
-__global__ void prep_kernel(DevMap m, CallArgs a) {
+__global__ void prep_kernel(DevMap m, CallArgs a, int part) {
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
+  const bool lift_part = part != 2, rest = part != 1;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
-    m.counters[0] = 0;
-    m.counters[1] = 0;
-    m.counters[2] = 0;
-    m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
-    CallStats z = {};
-    z.n_det = (uint32_t)a.M;
-    *m.stats = z;
+    if (rest) {
+      m.counters[0] = 0;
+      m.counters[1] = 0;
+      m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
+    }
+    if (lift_part) {
+      *m.surv_cnt = 0;
+      CallStats z = {};
+      z.n_det = (uint32_t)a.M;
+      *m.stats = z;
+    }
   }
-  if (blockIdx.x == 0 && (int)threadIdx.x < a.F) {  // per-frame camera block of the lift kernel (R5 reciprocals)
+  if (lift_part && blockIdx.x == 0 && (int)threadIdx.x < a.F) {  // per-frame camera block of the lift kernel (R5 reciprocals)
     const Camera c = load_camera(a.K + 9 * threadIdx.x, a.T + 16 * threadIdx.x);
     float *o = m.cam + 16 * threadIdx.x;
     o[0] = c.inv_fx, o[1] = c.inv_fy, o[2] = c.cx, o[3] = c.cy;
@@ -101,44 +108,48 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
     for (int i = 0; i < 3; ++i) o[4 + 4 * i] = c.r[3 * i], o[5 + 4 * i] = c.r[3 * i + 1], o[6 + 4 * i] = c.r[3 * i + 2], o[7 + 4 * i] = c.t[i];
   }
   if (warp < a.M) {
-  const T *row = (const T *)a.desc + (size_t)warp * m.D;
-  float s = 0.f;
-  if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
-    for (int i = lane * 8; i < m.D; i += 256) {
-      const uint4 w = __ldg(reinterpret_cast<const uint4 *>(row + i));
-      const T *e = reinterpret_cast<const T *>(&w);
+    if (rest) {
+      const T *row = (const T *)a.desc + (size_t)warp * m.D;
+      float s = 0.f;
+      if (a.split) {
+        // the similarity kernel (split schedule) computes the row norms and clears best_dense itself
+      } else if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
+        for (int i = lane * 8; i < m.D; i += 256) {
+          const uint4 w = __ldg(reinterpret_cast<const uint4 *>(row + i));
+          const T *e = reinterpret_cast<const T *>(&w);
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        const float x = to_f32<T>(e[q]);
-        s = fmaf(x, x, s);
+          for (int q = 0; q < 8; ++q) {
+            const float x = to_f32<T>(e[q]);
+            s = fmaf(x, x, s);
+          }
+        }
+      } else {
+        for (int i = lane; i < m.D; i += 32) {
+          const float x = to_f32<T>(row[i]);
+          s = fmaf(x, x, s);
+        }
       }
-    }
-  } else {
-    for (int i = lane; i < m.D; i += 32) {
-      const float x = to_f32<T>(row[i]);
-      s = fmaf(x, x, s);
-    }
-  }
 #pragma unroll
-  for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
-  if (lane == 0) {
-    m.det_inv_norm[warp] = s > 0.f ? 1.0f / sqrtf(s) : 0.f;
-    m.det_nv[warp] = 0;
-    m.det_npx[warp] = 0;
-    m.best_cand[warp] = 0ull;
-    m.best_dense[warp] = 0ull;
-    m.assoc[warp] = -1;
-    m.is_new[warp] = 0;
-    m.best_score[warp] = 0.f;
-    if (m.det_flags) m.det_flags[warp] = 0;
-  }
-  if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
-  if (m.det_gm) {
-    if (lane < 9) m.det_gm[(size_t)warp * 9 + lane] = 0.0;
-    if (lane == 9) m.hell[warp] = -1.f;
-  }
+      for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+      if (lane == 0) {
+        if (!a.split) m.det_inv_norm[warp] = s > 0.f ? 1.0f / sqrtf(s) : 0.f, m.best_dense[warp] = 0ull;
+        m.det_nv[warp] = 0;
+        m.best_cand[warp] = 0ull;
+        m.assoc[warp] = -1;
+        m.is_new[warp] = 0;
+        m.best_score[warp] = 0.f;
+        if (m.det_flags) m.det_flags[warp] = 0;
+      }
+      if (m.det_gm && lane == 9) m.hell[warp] = -1.f;
+    }
+    if (lift_part) {
+      if (lane == 0) m.det_npx[warp] = 0;
+      if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
+      if (m.det_gm && lane < 9) m.det_gm[(size_t)warp * 9 + lane] = 0.0;
+    }
   }
   // publish: the similarity kernel runs on another stream and waits for every prep CTA before its first epilogue
+  if (a.split) return;  // nothing of this kernel is awaited through prep_done then
   __syncthreads();
   if (threadIdx.x == 0) {
     __threadfence();
@@ -245,7 +256,7 @@ __device__ __forceinline__ void emit_overflow(const DevMap &m, bool ovf, unsigne
   if (!b) return;
   const int lane = threadIdx.x & 31;
   uint32_t base = 0;
-  if (lane == __ffs(b) - 1) base = atomicAdd(&m.counters[2], (uint32_t)__popc(b));
+  if (lane == __ffs(b) - 1) base = atomicAdd(m.surv_cnt, (uint32_t)__popc(b));
   base = __shfl_sync(0xFFFFFFFFu, base, __ffs(b) - 1);
   if (ovf) survivor_store(m, base + __popc(b & ((1u << lane) - 1)), bkey, j, lo, hi);
 }
@@ -328,7 +339,7 @@ template <bool GAUSS>
 __device__ __forceinline__ void lane_flush_block(const DevMap &m, TileSmem &s, const LaneAcc<GAUSS> &c) {
   const unsigned long long bkey = ((unsigned long long)c.khi << 32) | c.klo;
   if (c.li >= 0 && tile_block_add(s, c.li, bkey, c.mlo, c.mhi)) return;
-  survivor_store(m, atomicAdd(&m.counters[2], 1u), bkey, c.j, c.mlo, c.mhi);
+  survivor_store(m, atomicAdd(m.surv_cnt, 1u), bkey, c.j, c.mlo, c.mhi);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -421,7 +432,7 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
       }
       s.cur_pos = pos;
       if (s.cur_end - pos < (uint32_t)TILE_ENT && !s.next_valid) {
-        s.next_base = atomicAdd(&m.counters[2], (uint32_t)TILE_ENT);
+        s.next_base = atomicAdd(m.surv_cnt, (uint32_t)TILE_ENT);
         s.next_valid = 1;
       }
     }
@@ -645,7 +656,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
   __shared__ uint8_t s_pairs[PROBE_THREADS / 32][256];  // per warp: (record lane << 3 | sector) of the sectors with new voxels
   pdl_trigger();  // cand_associate may become resident behind this grid
   pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
-  const uint32_t nq = min(m.counters[2], m.surv_cap);
+  const uint32_t nq = min(*m.surv_cnt, m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < nq; i0 += stride) {
@@ -898,15 +909,15 @@ void configure_lift_kernels() {
   max_shared_carveout(probe_kernel);
 }
 
-int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s, int part) {
   const int blocks = a.M > 0 ? (a.M + 3) / 4 : 1;
   if (m.dtype == FARM_DTYPE_F32)
-    prep_kernel<float><<<blocks, 128, 0, s>>>(m, a);
+    prep_kernel<float><<<blocks, 128, 0, s>>>(m, a, part);
   else if (m.dtype == FARM_DTYPE_F16)
-    prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a);
+    prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a, part);
   else
-    prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a);
-  return blocks;
+    prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a, part);
+  return a.split ? 0 : blocks;
 }
 
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {

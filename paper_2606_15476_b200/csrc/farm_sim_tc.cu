@@ -23,6 +23,8 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+FARM_TRACE_TABLE(farm_trace_tiles)  // CTA 0: time its MMA issuer starts tile 0, 3, 6, ... (odd slots), epilogue done with tile 0, 6, 12, 18 (even)
+FARM_TRACE_TABLE(farm_trace_sim)  // 0 first CTA start, 1 last prep wait over, 3 last scan wait over, 2 first phase-2 wait, 5 last phase-2 wait over, 7 end
 namespace {
 
 constexpr int BLOCK_M = 128;  // detections per tile (UMMA M)
@@ -155,10 +157,25 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // 80 registers per thread (no spills): 256 x 80 leaves room for four 128 x 80 lift CTAs on the same SM
 // NCTA = 2: CTA pairs (cluster of 2, tcgen05 cta_group::2, UMMA 256 x 256 x 16): per stage a CTA holds its A tile and half
 // of the B tile (32 KB instead of 48 KB: six stages instead of four in the same shared memory, a third less L2 traffic).
-template <bool EMIT, int NCTA>  // EMIT: pairs whose cosine exceeds m.dense_thr also go to the dense list (H1 prefilter / U1 edges)
+//
+// SPLIT (FARM_OPT_INPUTS_READY): the kernel of call c is enqueued with no dependency on the main stream and
+// starts when the kernel of call c-1 ends, while that call's decision scan and merge are still to run.  R2 (every detection of
+// call c sees the map as call c-1 left it) is kept by splitting the columns:
+//   phase 1  the rows that existed at the entry of call c-1, n1 = n_hist[(seq-1)&1] of them, read as they are; the columns of
+//            the objects call c-1 merges into (touch_seq[o] == seq-1, final once its scan is done: dm.scan_done) are masked
+//            -- their rows may be half rewritten --, every other row is the same before and after that merge;
+//   phase 2  once call c-1's merge warps are done (dm.merge_done): the rows they wrote -- merged old objects and new objects
+//            -- which they also copied, with id and inverse norm, into dm.delta_*; extra tiles with the delta buffer as B.
+// Both phases feed the same packed atomicMax per row, so the result is the row max / lowest-id argmax over exactly the rows of
+// the map after call c-1.  The kernel also does the similarity's share of prep (row norms of A, cleared best_dense words).
+struct SplitArgs {
+  const void *A;  // the detection rows (what map_a describes)
+  uint32_t seq, scan_target, merge_target;
+};
+template <bool EMIT, int NCTA, bool SPLIT>  // EMIT: pairs whose cosine exceeds m.dense_thr also go to the dense list (H1 prefilter / U1 edges)
 __global__ void __maxnreg__(80)
-similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, DevMap m,
-                     int M, uint32_t idesc, uint32_t prep_target) {
+similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
+                     const __grid_constant__ CUtensorMap map_d, DevMap m, int M, uint32_t idesc, uint32_t prep_target, SplitArgs sp) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // SWIZZLE_128B needs 1024-byte alignment
   constexpr int NSTAGES = NCTA == 2 ? 6 : STAGES;
@@ -169,20 +186,41 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
   uint64_t *bars = (uint64_t *)(ib_s + 2 * BLOCK_N);
   uint64_t *full_bar = bars, *empty_bar = bars + NSTAGES, *tfull_bar = bars + 2 * NSTAGES, *tempty_bar = bars + 2 * NSTAGES + 2;
   uint32_t *tmem_slot = (uint32_t *)(bars + 2 * NSTAGES + 4);
+  // Tile schedule of the CTA: static round-robin (tile = unit, unit + n_units, ...; a device-wide tile counter was measured
+  // 1 % slower: the other kernels of a call slow all SMs alike).  With the split schedule the number of tiles is known only
+  // when the previous call's merge is done, so the producer thread decides where the sequence ends and publishes the tiles,
+  // tagged with their ordinal, in this ring; the MMA issuer and the epilogue follow it.  The producer is at most two accumulators
+  // plus one shared-memory ring ahead of the epilogue, far less than the 8 entries.
+  volatile unsigned long long *ring = (volatile unsigned long long *)(bars + 2 * NSTAGES + 6);
+  static_assert((2 * 6 + 6 + 8) * 8 <= 256, "barriers, TMEM slot and tile ring fit the 256 bytes reserved for them");
+  auto ring_get = [&](uint32_t k) -> int {
+    unsigned long long e;
+    do e = ring[k & 7]; while ((uint32_t)(e >> 32) != k + 1);
+    return (int)(uint32_t)e;  // -1: no more tiles
+  };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int N = (int)*m.n_objects;
+  const int N = SPLIT ? (int)__ldcg(&m.n_hist[(sp.seq - 1) & 1]) : (int)*m.n_objects;
   const int rank = NCTA == 2 ? (int)cluster_ctarank() : 0;       // rank 0 = leader: issues the MMAs of the pair
   const int unit = blockIdx.x / NCTA, n_units = gridDim.x / NCTA; // a unit = one CTA, or one CTA pair
   // tiles_m counts tiles of BLOCK_M * NCTA rows; CTA `rank` of a pair owns rows [tm * 256 + rank * 128, + 128)
   const int tiles_m = (M + BLOCK_M * NCTA - 1) / (BLOCK_M * NCTA), tiles_n = (N + BLOCK_N - 1) / BLOCK_N;
   const int n_tiles = tiles_m * tiles_n;
   const int k_blocks = (m.D + BLOCK_K - 1) / BLOCK_K;
+  // SPLIT: number of tiles of both phases, known once call c-1's merge warps are done; every role asks when it gets there
+  auto all_tiles = [&]() -> int {
+    spin_until(m.merge_done, sp.merge_target, m.err);
+    const int nd = (int)min(__ldcg(&m.delta_cnt[(sp.seq - 1) & 1]), m.max_det);
+    return n_tiles + tiles_m * ((nd + BLOCK_N - 1) / BLOCK_N);
+  };
 
+  if (SPLIT && threadIdx.x == 0) TRACE_MIN(farm_trace_sim, sp.seq, 0), TRACE_MAX(farm_trace_sim, sp.seq, 1);
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&map_a) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&map_b) : "memory");
+    if (SPLIT) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_d) : "memory");
   }
+  if (threadIdx.x < 8) ring[threadIdx.x] = 0ull;
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < NSTAGES; ++i) {
       mbar_init(smem_u32(&full_bar[i]), 1);
@@ -213,8 +251,32 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     // ===== TMA producer =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
-      for (int tile = unit; tile < n_tiles; tile += n_units) {
-        const int tm = tile % tiles_m, tn = tile / tiles_m;
+      int n_all = SPLIT ? -1 : n_tiles;
+      int cur = unit;
+      for (uint32_t k = 0;; ++k) {
+        int tile = cur;
+        if (tile >= n_tiles) {
+          if (SPLIT && n_all < 0) {
+            n_all = all_tiles();
+            asm volatile("fence.proxy.async;" ::: "memory");  // the delta rows were written through the generic proxy; TMA reads them
+            // Split kernels are launched with programmatic stream serialisation and never wait for their predecessor (nothing
+            // they read comes from it; the counters that tell calls apart are indexed by call parity): once every CTA is here,
+            // CTAs of the next call's kernel take over the SMs as this kernel's CTAs exit -- many have no phase-2 tile -- instead
+            // of after the whole grid plus a launch latency.  Not earlier than this point: a pending grid on the high-priority
+            // stream keeps the other streams' grids from being dispatched, and until here this kernel still waits for one of
+            // them (the previous call's merge).
+            pdl_trigger();
+          }
+          if (tile >= n_all) tile = -1;
+        }
+        ring[k & 7] = ((unsigned long long)(k + 1) << 32) | (uint32_t)tile;
+        if (tile < 0) break;
+        cur += n_units;
+        const bool ph2 = SPLIT && tile >= n_tiles;
+        if (ph2) TRACE_MIN(farm_trace_tiles, sp.seq, 6), TRACE_MAX(farm_trace_tiles, sp.seq, 7);  // producer starts a phase-2 tile
+        const int t2 = ph2 ? tile - n_tiles : tile;
+        const int tm = t2 % tiles_m, tn = t2 / tiles_m;
+        const CUtensorMap *mb = ph2 ? &map_d : &map_b;
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
           const uint32_t fb = smem_u32(&full_bar[stage]);
@@ -228,7 +290,7 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
           } else {
             mbar_expect_tx(fb, STG_BYTES);
             tma_load_2d(sa, &map_a, fb, kb * BLOCK_K, tm * BLOCK_M);
-            tma_load_2d(sa + A_BYTES, &map_b, fb, kb * BLOCK_K, tn * BLOCK_N);
+            tma_load_2d(sa + A_BYTES, mb, fb, kb * BLOCK_K, tn * BLOCK_N);
           }
           if (++stage == NSTAGES) stage = 0, phase ^= 1;
         }
@@ -238,9 +300,14 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     // ===== MMA issuer =====
     if (lane == 0 && rank == 0) {  // a pair's MMAs are issued by its leader CTA alone
       uint32_t stage = 0, phase = 0, as = 0, aphase = 0;
-      for (int tile = unit; tile < n_tiles; tile += n_units) {
+      for (uint32_t k = 0;; ++k) {
+        const int tile = ring_get(k);
+        if (tile < 0) break;
         mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);  // epilogue has drained this accumulator (in both CTAs of a pair)
         tcgen05_fence_after();
+#ifdef FARM_TRACE
+        if (SPLIT && tile >= n_tiles) TRACE_MIN(farm_trace_tiles, sp.seq, 0), TRACE_MAX(farm_trace_tiles, sp.seq, 1);  // MMA of a phase-2 tile starts
+#endif
         const uint32_t tmem_d = tmem_base + as * BLOCK_N;
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(smem_u32(&full_bar[stage]), phase);
@@ -270,17 +337,127 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
     const int row_in_tile = q * 32 + lane;
     const int et = threadIdx.x - 128;  // 0..EPI_THREADS-1
     uint32_t as = 0, aphase = 0;
+    if (SPLIT) {
+      // the similarity's share of prep_kernel, with its arithmetic (same summation order: bit-identical norms): one warp per
+      // row, rows unit, unit + n_units, ... of A; the main-stream prep skips them (CallArgs.split)
+      const uint16_t *A16 = (const uint16_t *)sp.A;
+      for (int r = unit + n_units * (warp - 4); r < M; r += n_units * (EPI_THREADS / 32)) {
+        float s = 0.f;
+        for (int i0 = lane * 8; i0 < m.D; i0 += 1024) {  // four loads in flight, then the sums in prep_kernel's order
+          uint4 w4[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if (i0 + 256 * u < m.D) w4[u] = __ldg(reinterpret_cast<const uint4 *>(A16 + (size_t)r * m.D + i0 + 256 * u));
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (i0 + 256 * u < m.D) {
+              const uint16_t *e = reinterpret_cast<const uint16_t *>(&w4[u]);
+#pragma unroll
+              for (int k = 0; k < 8; ++k) {
+                const float x = m.dtype == FARM_DTYPE_F16 ? __half2float(__ushort_as_half(e[k])) : __uint_as_float((uint32_t)e[k] << 16);
+                s = fmaf(x, x, s);
+              }
+            }
+          }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+        if (lane == 0) m.det_inv_norm[r] = s > 0.f ? 1.0f / sqrtf(s) : 0.f, m.best_dense[r] = 0ull;
+      }
+      __threadfence();
+      asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+      if (et == 0) TRACE_MAX(farm_trace_sim, sp.seq, 3), TRACE_MIN(farm_trace_sim, sp.seq, 6);
+      if (et == 0) atomicAdd(m.prep_done, 1u);
+    }
     // prep_kernel (main stream) may still be running: its row norms and the zeroed best_dense words are first
     // needed here, one tile of MMAs after the kernel started
     spin_until(m.prep_done, prep_target, m.err);  // bounded: sticky ERR_SYNC_TIMEOUT instead of a hang
+    if (SPLIT) spin_until(m.scan_done, sp.scan_target, m.err);  // touch_seq of call c-1 is final
     const uint32_t tempty_leader0 = NCTA == 2 ? leader_addr(smem_u32(&tempty_bar[0])) : 0u;
-    for (int tile = unit; tile < n_tiles; tile += n_units) {
+    for (uint32_t k = 0;; ++k) {
+      const int tile = ring_get(k);
+      if (tile < 0) break;
+      if (SPLIT && tile >= n_tiles) {
+        if (et == 0) TRACE_MIN(farm_trace_sim, sp.seq, 2), TRACE_MAX(farm_trace_sim, sp.seq, 5);
+        // ---- phase 2: B = the delta rows of call c-1; column k of the tile is object delta_id[n0 + k].  The ids are in no
+        // order, so R15 / R18 are applied literally: clamp first, then larger cosine wins, equal cosines -> lower id.
+        const int t2 = tile - n_tiles;
+        const int tm = t2 % tiles_m, n0 = (t2 / tiles_m) * BLOCK_N;
+        const int ncols = min(BLOCK_N, (int)min(__ldcg(&m.delta_cnt[(sp.seq - 1) & 1]), m.max_det) - n0);
+        float *ib = ib_s + as * BLOCK_N;
+#pragma unroll
+        for (int c = et; c < BLOCK_N; c += EPI_THREADS) ib[c] = c < ncols ? __ldcg(&m.delta_inv[n0 + c]) : 0.f;
+        const int row = tm * BLOCK_M + row_in_tile;
+        const bool row_ok = row < M;
+        const float ia = row_ok ? m.det_inv_norm[row] : 0.f;
+        asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+        mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+        tcgen05_fence_after();
+        if (et == 0) TRACE_MIN(farm_trace_tiles, sp.seq, 2), TRACE_MAX(farm_trace_tiles, sp.seq, 3);  // accumulator of a phase-2 tile complete
+        // the id of a column is needed only to break an exact tie (or for a zero-norm row, which ties everywhere): the common
+        // path keeps the column and looks the id up once at the end
+        float best = -3.0e38f;
+        int bcol = -1;
+        bool tie = false;  // some column equals the running maximum: decided by id in a second pass (rare: duplicate rows)
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
+        const bool scan_row = row_ok && ia != 0.f;
+#pragma unroll 1
+        for (int c0 = 0; c0 < ncols; c0 += 32) {
+          uint32_t r[32];
+          tmem_ld32(taddr + c0, r);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float cs = fminf(1.f, fmaxf(-1.f, __uint_as_float(r[i]) * ib[c0 + i] * ia));
+            const bool in = c0 + i < ncols;
+            tie = (in && cs == best) ? true : ((in && cs > best) ? false : tie);
+            if (in && cs > best) best = cs, bcol = c0 + i;
+          }
+        }
+        if (__any_sync(0xFFFFFFFFu, scan_row && tie)) {  // lowest id among the columns that reach the maximum
+          uint32_t low = bcol >= 0 ? __ldcg(&m.delta_id[n0 + bcol]) : 0xFFFFFFFFu;
+#pragma unroll 1
+          for (int c0 = 0; c0 < ncols; c0 += 32) {
+            uint32_t r[32];
+            tmem_ld32(taddr + c0, r);
+            tmem_ld_wait();
+#pragma unroll 1
+            for (int i = 0; i < 32; ++i) {
+              const float cs = fminf(1.f, fmaxf(-1.f, __uint_as_float(r[i]) * ib[c0 + i] * ia));
+              if (scan_row && tie && c0 + i < ncols && cs == best) {
+                const uint32_t id = __ldcg(&m.delta_id[n0 + c0 + i]);
+                if (id < low) low = id, bcol = c0 + i;
+              }
+            }
+          }
+        }
+        if (!scan_row) bcol = -1;
+        uint32_t best_id = bcol >= 0 ? __ldcg(&m.delta_id[n0 + bcol]) : 0xFFFFFFFFu;
+        if (row_ok && ia == 0.f) {  // cosine 0 with every object: the lowest id of the tile
+          best = 0.f;
+          for (int c = 0; c < ncols; ++c) best_id = min(best_id, __ldcg(&m.delta_id[n0 + c]));
+        }
+        tcgen05_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+        if (row_ok && best_id != 0xFFFFFFFFu) atomicMax(&m.best_dense[row], pack_score(best, best_id));
+        if (et == 0) TRACE_MIN(farm_trace_tiles, sp.seq, 4), TRACE_MAX(farm_trace_tiles, sp.seq, 5);  // epilogue of a phase-2 tile done
+        if (++as == 2) as = 0, aphase ^= 1;
+        continue;
+      }
       const int tm = (tile % tiles_m) * NCTA + rank, tn = tile / tiles_m;
       const int n0 = tn * BLOCK_N;
       const int ncols = min(BLOCK_N, N - n0);
       float *ib = ib_s + as * BLOCK_N;
+      if (SPLIT) {  // a column whose object call c-1 merges into: NaN never wins a comparison below; phase 2 brings its new row
+        const float masked = __int_as_float(0x7FC00000);
 #pragma unroll
-      for (int c = et; c < BLOCK_N; c += EPI_THREADS) ib[c] = c < ncols ? m.inv_norm[n0 + c] : 0.f;
+        for (int c = et; c < BLOCK_N; c += EPI_THREADS)
+          ib[c] = c < ncols ? (__ldcg(&m.touch_seq[n0 + c]) == sp.seq - 1 ? masked : m.inv_norm[n0 + c]) : 0.f;
+      } else {
+#pragma unroll
+        for (int c = et; c < BLOCK_N; c += EPI_THREADS) ib[c] = c < ncols ? m.inv_norm[n0 + c] : 0.f;
+      }
       const int cbeg = half * (BLOCK_N / EPI_SPLIT);
       const int row = tm * BLOCK_M + row_in_tile;
       const bool row_ok = row < M && cbeg < ncols;
@@ -352,18 +529,20 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
       if (lane == 0) {
         if (NCTA == 2) mbar_arrive_remote(tempty_leader0 + as * 8u); else mbar_arrive(smem_u32(&tempty_bar[as]));
       }
-      if (row_ok) {
+      if (row_ok && (!SPLIT || best > -2.0e38f || ia == 0.f)) {  // SPLIT: a row of a tile whose columns are all masked has nothing to say
         cs = fminf(1.f, fmaxf(-1.f, cs));                    // R15 clamp
         if (ia == 0.f) cs = 0.f, best_c = 0;                 // zero-norm detection: cos = 0 for every object
         atomicMax(&m.best_dense[row], pack_score(cs, (uint32_t)(n0 + best_c)));
       }
       if (++as == 2) as = 0, aphase ^= 1;
+
     }
   }
   tcgen05_fence_before();
   __threadfence();  // the epilogue's atomicMax results precede the completion count below
   __syncthreads();
-  if (threadIdx.x == 0) atomicAdd(m.sim_done, 1u);  // cand_associate's decision scan waits for every CTA of this grid
+  if (SPLIT && threadIdx.x == 0) TRACE_MAX(farm_trace_sim, sp.seq, 7);
+  if (threadIdx.x == 0) atomicAdd(m.sim_done + (sp.seq & 1), 1u);  // cand_associate's decision scan waits for every CTA of this grid
   if (NCTA == 2) cluster_sync_all();  // no CTA of a pair leaves (or frees TMEM) while its peer still uses the pair's resources
   if (warp == 2) {
     tcgen05_fence_after();
@@ -382,6 +561,8 @@ struct TcState {
   EncodeTiledFn encode = nullptr;
   CUtensorMap map_a, map_b;  // map_a is re-encoded per call by tc_prepare (host work only)
   CUtensorMap map_b_half;    // CTA pairs: each CTA loads half of the B tile
+  CUtensorMap map_d;         // split schedule: the delta rows (phase 2)
+  bool has_delta = false;
   uint32_t idesc_pair = 0;
   int pair = 0;              // 1: launch CTA pairs (cluster of 2, cta_group::2)
   CUtensorMapDataType dt;
@@ -423,10 +604,20 @@ void *tc_state_create(const DevMap &m) {
     delete st;
     return nullptr;
   }
-  if (cudaFuncSetAttribute(similarity_tc_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
-      cudaFuncSetAttribute(similarity_tc_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
-      cudaFuncSetAttribute(similarity_tc_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
-      cudaFuncSetAttribute(similarity_tc_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
+  if (m.delta_rows) {
+    if (!encode_2d(st, &st->map_d, m.delta_rows, m.max_det, (uint64_t)m.D, BLOCK_N)) {
+      delete st;
+      return nullptr;
+    }
+    st->has_delta = true;
+  } else {
+    st->map_d = st->map_b;  // never read
+  }
+  if (cudaFuncSetAttribute(similarity_tc_kernel<false, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<true, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<true, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(similarity_tc_kernel<false, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess) {
     delete st;
     return nullptr;
   }
@@ -446,12 +637,16 @@ bool tc_prepare(void *state, const DevMap &m, const CallArgs &a) {
   return encode_2d(st, &st->map_a, a.desc, (uint64_t)a.M, (uint64_t)m.D, BLOCK_M);
 }
 
+// prep_target: value dm.prep_done has when prep_kernel's CTAs of this call are done; with the split schedule (a.split) the
+// kernel does that share itself and the value becomes prep_target + its own CTAs (returned through *prep_after).
 int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, cudaStream_t s, void *state, uint32_t prep_target,
-                         int *n_ctas) {
+                         int *n_ctas, uint32_t *prep_after) {
   TcState *st = (TcState *)state;
+  if (prep_after) *prep_after = prep_target;
   if (a.M == 0 || n_upper == 0) return 0;
   const CUtensorMap &map_a = st->map_a;
   const bool emit = m.dense_d && m.dense_thr < 2.0f;
+  SplitArgs sp = {a.desc, a.seq, a.scan_target, a.merge_target};
   int grid;
   if (st->pair) {  // CTA pairs: one cluster of two CTAs per 256 x 256 tile
     const long long tiles = (long long)((a.M + 2 * BLOCK_M - 1) / (2 * BLOCK_M)) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
@@ -462,19 +657,29 @@ int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, c
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2, attr[0].val.clusterDim.y = 1, attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr, cfg.numAttrs = 1;
-    const cudaError_t e = emit ? cudaLaunchKernelEx(&cfg, similarity_tc_kernel<true, 2>, map_a, st->map_b_half, m, a.M, st->idesc_pair, prep_target)
-                               : cudaLaunchKernelEx(&cfg, similarity_tc_kernel<false, 2>, map_a, st->map_b_half, m, a.M, st->idesc_pair, prep_target);
+    const cudaError_t e =
+        emit ? cudaLaunchKernelEx(&cfg, similarity_tc_kernel<true, 2, false>, map_a, st->map_b_half, st->map_d, m, a.M, st->idesc_pair, prep_target, sp)
+             : cudaLaunchKernelEx(&cfg, similarity_tc_kernel<false, 2, false>, map_a, st->map_b_half, st->map_d, m, a.M, st->idesc_pair, prep_target, sp);
     if (e != cudaSuccess) return -1;
   } else {
+    // split: phase 2 adds up to ceil(max touched rows / 256) column tiles; the grid is sized on the rows known to the host
     const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
     grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
-    if (emit)
-      similarity_tc_kernel<true, 1><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
-    else
-      similarity_tc_kernel<false, 1><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, m, a.M, st->idesc, prep_target);
+    if (a.split) {
+      if (prep_after) *prep_after = prep_target + (uint32_t)grid;
+      if (launch_pdl(similarity_tc_kernel<false, 1, true>, dim3(grid), dim3(TC_THREADS), SMEM_BYTES, s, map_a, st->map_b, st->map_d, m, a.M,
+                     st->idesc, prep_target + (uint32_t)grid, sp) != cudaSuccess)
+        return -1;
+    } else if (emit) {
+      similarity_tc_kernel<true, 1, false><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, st->map_d, m, a.M, st->idesc, prep_target, sp);
+    } else {
+      similarity_tc_kernel<false, 1, false><<<grid, TC_THREADS, SMEM_BYTES, s>>>(map_a, st->map_b, st->map_d, m, a.M, st->idesc, prep_target, sp);
+    }
   }
   if (n_ctas) *n_ctas = grid;
   return 1;
 }
+
+bool tc_can_split(void *state) { return state && ((TcState *)state)->has_delta && !((TcState *)state)->pair; }
 
 }  // namespace farm

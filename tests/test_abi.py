@@ -123,11 +123,11 @@ def test_round2_options_and_calls_validate_on_the_host(lib):
     from paper_2606_15476_b200 import FarmError, FarmMap, binding
     m = FarmMap(0.05, 8, 0.5, 0.5, 0.5, H=8, W=8)
     for key, bad in ((binding.OPT_VIEWS, 9), (binding.OPT_VIEWS, -1), (binding.OPT_CORRESPONDENCE, 2), (binding.OPT_GEOMETRY, 2),
-                     (binding.OPT_SIM_PATH, 4), (binding.OPT_EDGES, 17), (binding.OPT_EDGES, -1)):
+                     (binding.OPT_SIM_PATH, 4), (binding.OPT_EDGES, 17), (binding.OPT_EDGES, -1), (binding.OPT_INPUTS_READY, 2)):
         with pytest.raises(FarmError):
             m.set_option_i(key, bad)
     for key, good in ((binding.OPT_VIEWS, 4), (binding.OPT_CORRESPONDENCE, 1), (binding.OPT_GEOMETRY, 1), (binding.OPT_SIM_PATH, 3),
-                      (binding.OPT_EDGES, 16)):
+                      (binding.OPT_EDGES, 16), (binding.OPT_INPUTS_READY, 1)):
         m.set_option_i(key, good)
     for key, bad in ((binding.OPTF_EDGE_DECAY, 0.0), (binding.OPTF_EDGE_DECAY, 1.5), (binding.OPTF_EDGE_CUTOFF, -1.0),
                      (binding.OPTF_EDGE_CUTOFF, float("inf")), (binding.OPTF_EDGE_DECAY, float("nan"))):
