@@ -129,3 +129,35 @@ def test_inputs_ready_exact_ties_among_rewritten_rows_go_to_the_lowest_id(oracle
         assert list(am_g) == [7, 30] and list(am_o) == [7, 30]
         compare_maps(g, o, voxels=False)
         g.destroy()
+
+
+def test_inputs_ready_with_every_optional_structure(oracle):
+    """The optional structures ride on the state the split schedule double-buffers (per-detection boxes and moments written by
+    the lift kernel on its own stream, statistics, the list of the call's entities built by the merge): Gaussians, covisibility
+    bitset, views and weighted edges on the mini stress scene, five calls back to back, against the oracle."""
+    from test_gpu_parity import _compare_gaussians
+    from test_gpu_parity_r2 import _compare_views
+    sc = S.StressScene(n_batches=5, frames_per_batch=8, n_objects=700)
+    o, g = _stress_pair(oracle, sc, inputs_ready=1, max_voxels=1 << 24, gaussian=1, covisibility=1, views=2, edges=3)
+    o.set_option(o.OPT_VIEWS_K, 2)
+    o.set_option(o.OPT_EDGES_K, 3)
+    calls = []
+    for b in range(5):
+        frames = margin_filter(o.clone, sc.batch(b), sc.cfg.tau)
+        integrate_frames(o, frames)
+        calls.append(frames)
+    staged = [upload(fr, sc.cfg.dtype) for fr in calls]
+    torch.cuda.synchronize()
+    for d, fr in zip(staged, calls):
+        g.integrate_batch(len(fr), d["depth"], d["mask"], d["K"], d["T"], d["desc"], d["n_det"])
+    compare_call(g, o, check_sets=False)
+    _compare_gaussians(g, o)
+    compare_maps(g, o, voxels=False)
+    assert np.array_equal(g.read_covisibility(), o.read_covisibility())
+    assert _compare_views(g, o) > 700
+    ao, bo, wo = o.read_edges()
+    ag, bg, wg = g.read_edges()
+    assert np.array_equal(ag, ao) and np.array_equal(bg, bo) and np.abs(wg - wo).max() <= 1e-9 * float(wo.max())
+    w_o, mu_o, cov_o = o.read_gaussians()
+    w_g, mu_g, cov_g = g.read_gaussians()
+    assert np.array_equal(w_g, w_o) and np.abs(mu_g - mu_o).max() <= 1e-4 and np.abs(cov_g - cov_o).max() <= 1e-4
