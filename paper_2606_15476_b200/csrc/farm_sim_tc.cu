@@ -23,6 +23,7 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+FARM_TRACE_TABLE(farm_trace_clock)  // CTA 0 of the call's similarity kernel: [0] SM cycles, [1] nanoseconds of its lifetime
 FARM_TRACE_TABLE(farm_trace_tiles)  // CTA 0: time its MMA issuer starts tile 0, 3, 6, ... (odd slots), epilogue done with tile 0, 6, 12, 18 (even)
 FARM_TRACE_TABLE(farm_trace_sim)  // 0 first CTA start, 1 last prep wait over, 3 last scan wait over, 2 first phase-2 wait, 5 last phase-2 wait over, 7 end
 namespace {
@@ -215,6 +216,11 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
   };
 
   if (SPLIT && threadIdx.x == 0) TRACE_MIN(farm_trace_sim, sp.seq, 0), TRACE_MAX(farm_trace_sim, sp.seq, 1);
+#ifdef FARM_TRACE
+  long long trace_c0 = 0;
+  unsigned long long trace_t0 = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) trace_c0 = clock64(), trace_t0 = gtime();
+#endif
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&map_a) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&map_b) : "memory");
@@ -542,6 +548,12 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
   __threadfence();  // the epilogue's atomicMax results precede the completion count below
   __syncthreads();
   if (SPLIT && threadIdx.x == 0) TRACE_MAX(farm_trace_sim, sp.seq, 7);
+#ifdef FARM_TRACE
+  if (blockIdx.x == 0 && threadIdx.x == 0) {  // SM clock of CTA 0 over its lifetime: cycles and nanoseconds
+    farm_trace_clock[sp.seq & 15][0] = (unsigned long long)(clock64() - trace_c0);
+    farm_trace_clock[sp.seq & 15][1] = gtime() - trace_t0;
+  }
+#endif
   if (threadIdx.x == 0) atomicAdd(m.sim_done + (sp.seq & 1), 1u);  // cand_associate's decision scan waits for every CTA of this grid
   if (NCTA == 2) cluster_sync_all();  // no CTA of a pair leaves (or frees TMEM) while its peer still uses the pair's resources
   if (warp == 2) {
