@@ -54,8 +54,8 @@ struct farm_map {
   long long sim_timed = 0, sim_all = 0;  // timing 1: similarity launches bracketed by events / all of them (since the last reset)
   uint32_t scan_count = 0;      // decision scans launched so far (device counter dm.scan_done)
   uint32_t merge_count = 0;     // merge warps launched so far (device counter dm.merge_done)
-  // what the lift kernel writes, double buffered by call parity: with the split schedule the lift of call c runs on its own
-  // stream while the main chain is still at call c-1
+  // what prep resets and the lift kernel writes, double buffered by call parity: with the split schedule prep and lift of call c
+  // run on their own stream while the main chain is still at call c-1 (whose scan, merge and result reads use the other set)
   struct LiftSet {
     unsigned long long *surv_key, *surv_bits;
     uint32_t *surv_j, *surv_cnt, *det_npx;
@@ -63,6 +63,11 @@ struct farm_map {
     double *det_gm;
     float *cam;
     CallStats *stats;
+    uint32_t *counters, *det_nv;
+    unsigned long long *best_cand;
+    int32_t *assoc;
+    uint8_t *is_new;
+    float *best_score, *hell;
   } lset[2] = {};
   cudaStream_t early = nullptr;                 // prep (lift part) + lift of a split call
   cudaEvent_t ev_lift = nullptr, ev_end[2] = {nullptr, nullptr};
@@ -462,6 +467,13 @@ int finalise_impl(farm_map *m) {
     if (m->gaussian) A(s1.det_gm, MD * 9, 0);
     A(s1.cam, (size_t)MAX_FRAMES * 16, 0);
     A(s1.stats, 1, 0);
+    A(s1.counters, 16, 0);
+    A(s1.det_nv, MD, 0);
+    A(s1.best_cand, MD, 0);
+    A(s1.assoc, MD, 0);
+    A(s1.is_new, MD, 0);
+    A(s1.best_score, MD, 0);
+    if (m->gaussian) A(s1.hell, MD, 0);
   }
   A(d.sim_done, 2, 0);
   d.eps2 = m->voxel_size * m->voxel_size;
@@ -516,6 +528,7 @@ int finalise_impl(farm_map *m) {
     A(d.ed_key, (size_t)ecap, 0xFF);
     A(d.ed_w, (size_t)ecap, 0);
     A(d.ed_t, (size_t)ecap, 0);
+    A(d.ed_cnt, 1, 0);
     d.ed_mask = (uint32_t)(ecap - 1);
   }
   if (m->gaussian) {
@@ -542,7 +555,8 @@ int finalise_impl(farm_map *m) {
   if (m->dtype != FARM_DTYPE_F32 && m->sim_path != 1 && tc_supported(d)) m->tc = tc_state_create(d);
   if (m->tc && m->sim_path == 3) tc_state_set_pair(m->tc, 1);
   d.surv_cnt = d.counters + 2;
-  m->lset[0] = {d.surv_key, d.surv_bits, d.surv_j, d.surv_cnt, d.det_npx, d.det_box, d.det_gm, d.cam, d.stats};
+  m->lset[0] = {d.surv_key, d.surv_bits, d.surv_j, d.surv_cnt, d.det_npx, d.det_box, d.det_gm, d.cam, d.stats,
+                d.counters, d.det_nv, d.best_cand, d.assoc, d.is_new, d.best_score, d.hell};
   if (d.touch_seq) {
     CU(cudaStreamCreateWithFlags(&m->early, cudaStreamNonBlocking));
     CU(cudaEventCreateWithFlags(&m->ev_lift, cudaEventDisableTiming));
@@ -789,6 +803,8 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
     DevMap &w = m->dm;
     w.surv_key = ls.surv_key, w.surv_bits = ls.surv_bits, w.surv_j = ls.surv_j, w.surv_cnt = ls.surv_cnt, w.det_npx = ls.det_npx;
     w.det_box = ls.det_box, w.det_gm = ls.det_gm, w.cam = ls.cam, w.stats = ls.stats;
+    w.counters = ls.counters, w.det_nv = ls.det_nv, w.best_cand = ls.best_cand, w.assoc = ls.assoc, w.is_new = ls.is_new;
+    w.best_score = ls.best_score, w.hell = ls.hell;
   }
   cudaStream_t st = m->stream;
   bool launch_failed = false;
@@ -838,17 +854,18 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
     const int par = (int)(a.seq & 1);
     if (m->ev_end_set[par]) cudaStreamWaitEvent(m->early, m->ev_end[par], 0);
     stage(FARM_STAGE_PREP, m->early, [&] {
-      launch_prep(d, a, m->early, 1);
+      launch_prep(d, a, m->early);  // resets this parity's buffers only: nothing the previous call still reads
       return 1;
     });
     stage(FARM_STAGE_LIFT, m->early, [&] { return launch_lift(d, a, m->early); });
     cudaEventRecord(m->ev_lift, m->early);
     cudaStreamWaitEvent(st, m->ev_lift, 0);
   }
-  stage(FARM_STAGE_PREP, st, [&] {
-    m->prep_target += (uint32_t)launch_prep(d, a, st, a.split ? 2 : 0);
-    return 1;
-  });
+  if (!a.split)
+    stage(FARM_STAGE_PREP, st, [&] {
+      m->prep_target += (uint32_t)launch_prep(d, a, st);
+      return 1;
+    });
   if (fork && m->overlap == 3) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork && !early_fork) {
     cudaEventRecord(m->ev_fork, st);
@@ -1256,7 +1273,7 @@ int farm_map_read_edges(farm_map *m, uint32_t *ea, uint32_t *eb, double *ew, uin
   int rc = device_error(m);
   if (rc != FARM_OK) return rc;
   uint32_t n = 0;
-  CU(cudaMemcpy(&n, m->dm.counters + 9, 4, cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(&n, m->dm.ed_cnt, 4, cudaMemcpyDeviceToHost));
   if (n_out) *n_out = n;
   if (n == 0) return FARM_OK;
   // compacted on the device, ordered on the host (an export, not part of the integrate path)

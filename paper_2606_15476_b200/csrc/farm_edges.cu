@@ -57,7 +57,7 @@ __device__ __forceinline__ void edge_touch(const DevMap &m, uint32_t x, uint32_t
     unsigned long long k = __ldcg(&m.ed_key[h]);
     if (k == KEY_MAX) {
       k = atomicCAS(&m.ed_key[h], KEY_MAX, key);
-      if (k == KEY_MAX) k = key, atomicAdd(&m.counters[9], 1u);
+      if (k == KEY_MAX) k = key, atomicAdd(m.ed_cnt, 1u);
     }
     if (k == key) {
       const uint32_t t_old = atomicExch(&m.ed_t[h], call);

@@ -111,7 +111,7 @@ struct DevMap {
   uint32_t *surv_cnt;                // records reserved in the survivor queue (counters + 2, or the call-parity copy)
   uint32_t *counters;                // [0]=event_count [1]=cand_count [2]=survivor_count [3]=block ticket
                                      // [4]=dense pairs [5]=edges [6]=detection-detection edges [7]=entity merges
-                                     // [8]=|S| of the call (W1) [9]=entries of the edge dictionary (W4)
+                                     // [8]=|S| of the call (W1)
   // per detection [max_det]
   uint32_t max_det;
   uint32_t *det_nv, *det_npx;
@@ -160,6 +160,7 @@ struct DevMap {
   double *ed_w;                      //   weight as of call ed_t
   uint32_t *ed_t;                    //   index (1-based) of the call that last updated the edge
   uint32_t ed_mask;
+  uint32_t *ed_cnt;                  //   entries in the dictionary (persistent, unlike the per-call `counters`)
   uint32_t *sim_done;                // [2] cumulative count of finished similarity CTAs (the association scan waits on it); slot =
                                      //   parity of CallArgs.seq (0 without the split schedule): kernels of consecutive calls may overlap
   uint32_t *prep_done;               // cumulative count of finished prep_kernel CTAs (the similarity epilogue waits on it)
@@ -333,9 +334,7 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 void configure_lift_kernels();
 void configure_assoc_kernels();
 void configure_edge_kernels();
-// part 0: everything; with the split schedule the lift runs ahead on its own stream: part 1 = what the lift kernel needs
-// (camera blocks, cleared survivor count, statistics and per-detection evidence), part 2 = the rest, in the main chain
-int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s, int part = 0);  // returns the number of CTAs that report to prep_done
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);  // returns the number of CTAs that report to prep_done
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,

@@ -80,27 +80,22 @@ __device__ __forceinline__ bool depth_valid(float z, float z_min, float z_max) {
 
 // ---------------------------------------------------------------------------------------------------
 // prep: reset per-call state and compute detection row norms (operand A of step 4).  One warp per row.
-// part 0 = everything (one launch per call).  Split schedule: part 1 = the state the lift kernel works on (launched with the
-// lift kernel on its own stream, ahead of the previous call's tail), part 2 = the rest (main stream, behind that tail).
+// With the split schedule (CallArgs.split) the kernel runs on the lift's stream ahead of the previous call's tail -- everything it
+// resets is double buffered by call parity -- and leaves the row norms and best_dense to the similarity kernel.
 template <typename T>
-__global__ void prep_kernel(DevMap m, CallArgs a, int part) {
+__global__ void prep_kernel(DevMap m, CallArgs a) {
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
-  const bool lift_part = part != 2, rest = part != 1;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
-    if (rest) {
-      m.counters[0] = 0;
-      m.counters[1] = 0;
-      m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
-    }
-    if (lift_part) {
-      *m.surv_cnt = 0;
-      CallStats z = {};
-      z.n_det = (uint32_t)a.M;
-      *m.stats = z;
-    }
+    m.counters[0] = 0;
+    m.counters[1] = 0;
+    m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
+    *m.surv_cnt = 0;
+    CallStats z = {};
+    z.n_det = (uint32_t)a.M;
+    *m.stats = z;
   }
-  if (lift_part && blockIdx.x == 0 && (int)threadIdx.x < a.F) {  // per-frame camera block of the lift kernel (R5 reciprocals)
+  if (blockIdx.x == 0 && (int)threadIdx.x < a.F) {  // per-frame camera block of the lift kernel (R5 reciprocals)
     const Camera c = load_camera(a.K + 9 * threadIdx.x, a.T + 16 * threadIdx.x);
     float *o = m.cam + 16 * threadIdx.x;
     o[0] = c.inv_fx, o[1] = c.inv_fy, o[2] = c.cx, o[3] = c.cy;
@@ -108,44 +103,42 @@ __global__ void prep_kernel(DevMap m, CallArgs a, int part) {
     for (int i = 0; i < 3; ++i) o[4 + 4 * i] = c.r[3 * i], o[5 + 4 * i] = c.r[3 * i + 1], o[6 + 4 * i] = c.r[3 * i + 2], o[7 + 4 * i] = c.t[i];
   }
   if (warp < a.M) {
-    if (rest) {
-      const T *row = (const T *)a.desc + (size_t)warp * m.D;
-      float s = 0.f;
-      if (a.split) {
-        // the similarity kernel (split schedule) computes the row norms and clears best_dense itself
-      } else if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
-        for (int i = lane * 8; i < m.D; i += 256) {
-          const uint4 w = __ldg(reinterpret_cast<const uint4 *>(row + i));
-          const T *e = reinterpret_cast<const T *>(&w);
+    const T *row = (const T *)a.desc + (size_t)warp * m.D;
+    float s = 0.f;
+    if (a.split) {
+      // the similarity kernel (split schedule) computes the row norms and clears best_dense itself
+    } else if (sizeof(T) == 2 && (m.D & 7) == 0 && (((uintptr_t)a.desc) & 15) == 0) {  // 128-bit loads, 8 elements each
+      for (int i = lane * 8; i < m.D; i += 256) {
+        const uint4 w = __ldg(reinterpret_cast<const uint4 *>(row + i));
+        const T *e = reinterpret_cast<const T *>(&w);
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            const float x = to_f32<T>(e[q]);
-            s = fmaf(x, x, s);
-          }
-        }
-      } else {
-        for (int i = lane; i < m.D; i += 32) {
-          const float x = to_f32<T>(row[i]);
+        for (int q = 0; q < 8; ++q) {
+          const float x = to_f32<T>(e[q]);
           s = fmaf(x, x, s);
         }
       }
-#pragma unroll
-      for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
-      if (lane == 0) {
-        if (!a.split) m.det_inv_norm[warp] = s > 0.f ? 1.0f / sqrtf(s) : 0.f, m.best_dense[warp] = 0ull;
-        m.det_nv[warp] = 0;
-        m.best_cand[warp] = 0ull;
-        m.assoc[warp] = -1;
-        m.is_new[warp] = 0;
-        m.best_score[warp] = 0.f;
-        if (m.det_flags) m.det_flags[warp] = 0;
+    } else {
+      for (int i = lane; i < m.D; i += 32) {
+        const float x = to_f32<T>(row[i]);
+        s = fmaf(x, x, s);
       }
-      if (m.det_gm && lane == 9) m.hell[warp] = -1.f;
     }
-    if (lift_part) {
-      if (lane == 0) m.det_npx[warp] = 0;
-      if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
-      if (m.det_gm && lane < 9) m.det_gm[(size_t)warp * 9 + lane] = 0.0;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    if (lane == 0) {
+      if (!a.split) m.det_inv_norm[warp] = s > 0.f ? 1.0f / sqrtf(s) : 0.f, m.best_dense[warp] = 0ull;
+      m.det_nv[warp] = 0;
+      m.det_npx[warp] = 0;
+      m.best_cand[warp] = 0ull;
+      m.assoc[warp] = -1;
+      m.is_new[warp] = 0;
+      m.best_score[warp] = 0.f;
+      if (m.det_flags) m.det_flags[warp] = 0;
+    }
+    if (lane < 6) m.det_box[warp * 6 + lane] = lane < 3 ? 0x7FFFFFFF : (int)0x80000000;
+    if (m.det_gm) {
+      if (lane < 9) m.det_gm[(size_t)warp * 9 + lane] = 0.0;
+      if (lane == 9) m.hell[warp] = -1.f;
     }
   }
   // publish: the similarity kernel runs on another stream and waits for every prep CTA before its first epilogue
@@ -909,14 +902,14 @@ void configure_lift_kernels() {
   max_shared_carveout(probe_kernel);
 }
 
-int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s, int part) {
+int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int blocks = a.M > 0 ? (a.M + 3) / 4 : 1;
   if (m.dtype == FARM_DTYPE_F32)
-    prep_kernel<float><<<blocks, 128, 0, s>>>(m, a, part);
+    prep_kernel<float><<<blocks, 128, 0, s>>>(m, a);
   else if (m.dtype == FARM_DTYPE_F16)
-    prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a, part);
+    prep_kernel<__half><<<blocks, 128, 0, s>>>(m, a);
   else
-    prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a, part);
+    prep_kernel<__nv_bfloat16><<<blocks, 128, 0, s>>>(m, a);
   return a.split ? 0 : blocks;
 }
 
