@@ -844,13 +844,16 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   // through device counters.  Not with per-kernel timing: the events would serialise the two streams.
   a.split = (early_fork && maintain && a.seq >= 3 && m->timing < 2 && tc_can_split(m->tc)) ? 1 : 0;
   a.scan_target = m->scan_count, a.merge_target = m->merge_count;
+  a.sim_fills_gpu = ((M + 127) / 128) * (((long long)m->n_upper + 255) / 256) >= d.num_sms ? 1 : 0;
   if (early_fork && !a.split) {
     cudaEventRecord(m->ev_fork, st);
     cudaStreamWaitEvent(m->side, m->ev_fork, 0);
   }
   if (a.split) {
     // the lift of this call does not depend on the map: it runs on its own stream, behind the call before the previous one
-    // (the last user of this parity's buffers), while the main chain is still busy with the previous call's scan and merge
+    // (the last user of this parity's buffers), while the main chain is still busy with the previous call's scan and merge.
+    // Starting it later -- behind the previous call's probe -- was measured: the
+    // lift then ends too close to its own probe and single-frame calls get 2-8 us longer.
     const int par = (int)(a.seq & 1);
     if (m->ev_end_set[par]) cudaStreamWaitEvent(m->early, m->ev_end[par], 0);
     stage(FARM_STAGE_PREP, m->early, [&] {
@@ -894,6 +897,7 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
   if (!(fork && m->overlap == 3) && !a.split) stage(FARM_STAGE_LIFT, st, [&] { return launch_lift(d, a, st); });
   if (fork && m->overlap == 2) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_PROBE, st, [&] { return launch_probe(d, a, st) + launch_dd_overlap(d, a, st); });
+
   if (fork && m->overlap != 2 && !early_fork) cudaStreamWaitEvent(st, m->ev_join, 0);
   stage(FARM_STAGE_ASSOCIATE, st, [&] { return launch_cand_associate(d, a, st); });
   stage(FARM_STAGE_MERGE, st, [&] { return launch_commit_merge(d, a, m->frame_seq, st); });

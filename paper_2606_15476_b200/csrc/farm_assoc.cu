@@ -1073,8 +1073,8 @@ int launch_commit_merge(const DevMap &m, const CallArgs &a, unsigned long long f
   if (a.M == 0) return 0;
   const int commit_blocks = m.num_sms * 4;
   const int merge_blocks = (a.M + MERGE_WARPS - 1) / MERGE_WARPS;  // one warp per detection
-  if (a.split) {
-    // Split schedule: no programmatic early launch.  CTAs of this grid that sit in pdl_wait() while the decision scan runs
+  if (a.split && a.sim_fills_gpu) {
+    // Split schedule with a similarity grid that takes every SM: no programmatic early launch.  CTAs of this grid that sit in pdl_wait() while the decision scan runs
     // hold their registers (256 x 119), and the next call's similarity kernel -- which starts in exactly that window -- would
     // find no room on those SMs until this grid has drained (measured: its last CTA started 22-25 us late).
     FARM_DISPATCH((commit_merge_kernel<T><<<dim3(commit_blocks + merge_blocks), dim3(MERGE_THREADS), 0, s>>>(m, a, frame_seq0, commit_blocks)));

@@ -189,6 +189,7 @@ struct CallArgs {
   // FARM_OPT_INPUTS_READY
   uint32_t seq;           // sequence number of the call (1, 2, ...), the clock of touch_seq / n_hist / delta_cnt
   int split;              // 1: the similarity kernel runs the two-phase schedule and does its own share of prep
+  int sim_fills_gpu;      //   1: its grid has one CTA on every SM (decides how the merge kernel is launched)
   uint32_t prep_target;   //   value dm.prep_done reaches when the row norms of this call are final (cand_associate waits)
   uint32_t scan_target;   //   value dm.scan_done reaches when the PREVIOUS call's decision scan is done
   uint32_t merge_target;  //   value dm.merge_done reaches when the PREVIOUS call's merge warps are done

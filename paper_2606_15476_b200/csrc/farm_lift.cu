@@ -10,6 +10,7 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+FARM_TRACE_TABLE(farm_trace_lift)  // 0 / 1 lift first CTA start / last CTA end, 2 / 3 probe first CTA past its wait / last CTA end, 4 prep start
 
 namespace {
 
@@ -87,6 +88,7 @@ __global__ void prep_kernel(DevMap m, CallArgs a) {
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
+    TRACE_MIN(farm_trace_lift, a.seq, 4);
     m.counters[0] = 0;
     m.counters[1] = 0;
     m.counters[4] = 0, m.counters[5] = 0, m.counters[6] = 0, m.counters[7] = 0, m.counters[8] = 0;
@@ -364,6 +366,7 @@ __device__ __forceinline__ void lane_flush_block(const DevMap &m, TileSmem &s, c
 template <bool VEC, bool GAUSS>
 __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m, CallArgs a, int tiles_x, int tiles_y) {
   pdl_trigger();  // the probe kernel may become resident as soon as CTAs of this grid retire
+  if (threadIdx.x == 0) TRACE_MIN(farm_trace_lift, a.seq, 0);
   __shared__ TileSmem s;
   __shared__ uint32_t lab_j2[2][MAX_LABELS];  // label tables are double buffered: the flush of tile t reads its copy
                                               // while tile t+1 initialises the other
@@ -632,6 +635,7 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
     }
     for (uint32_t p = pos + tid; p < end; p += LIFT_THREADS) survivor_store(m, p, 0ull, 0u, 0u, 0u);
   }
+  if (tid == 0) TRACE_MAX(farm_trace_lift, a.seq, 1);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -649,6 +653,15 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
   __shared__ uint8_t s_pairs[PROBE_THREADS / 32][256];  // per warp: (record lane << 3 | sector) of the sectors with new voxels
   pdl_trigger();  // cand_associate may become resident behind this grid
   pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
+  if (threadIdx.x == 0) TRACE_MIN(farm_trace_lift, a.seq, 2);
+#ifdef FARM_TRACE
+  struct ProbeEnd {
+    uint32_t seq;
+    __device__ ~ProbeEnd() {
+      if (threadIdx.x == 0) TRACE_MAX(farm_trace_lift, seq, 3);
+    }
+  } probe_end{a.seq};
+#endif
   const uint32_t nq = min(*m.surv_cnt, m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;

@@ -23,10 +23,53 @@ sys.path.insert(0, ROOT)
 from paper_2606_15476_b200 import binding  # noqa: E402
 
 
+def single_frame(opt, binding):
+    """single-frame calls of configs 1-3 with the split schedule: where the time of a call goes"""
+    from paper_2606_15476_b200 import FarmMap, scenes as S
+    cfg = S.get_config(opt.config)
+    n = opt.calls
+    frames = S.generate_frames(opt.config, range(20, 20 + n))
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.Stream(device=dev)
+    m = FarmMap(cfg.voxel, cfg.D, cfg.w_geo, cfg.w_sem, cfg.tau, H=cfg.H, W=cfg.W, dtype=cfg.dtype, stream=stream.cuda_stream,
+                max_objects=8192, max_voxels=1 << 24, max_det_per_call=64, inputs_ready=opt.inputs_ready)
+    staged = []
+    with torch.cuda.stream(stream):
+        for fr in frames:
+            desc = np.ascontiguousarray(fr.desc).view(np.int16)
+            staged.append((torch.from_numpy(fr.depth).to(dev), torch.from_numpy(fr.mask.view(np.int16)).to(dev),
+                           torch.from_numpy(np.ascontiguousarray(fr.K, np.float32)).to(dev),
+                           torch.from_numpy(np.ascontiguousarray(fr.T, np.float32)).to(dev), torch.from_numpy(desc).to(dev), fr.n_det))
+    torch.cuda.synchronize()
+    lib = binding.load_library()
+    names = ("sim", "assoc", "lift")
+    for name in names:
+        getattr(lib, f"farm_trace_{name}_read")(None, 1)
+    for d in staged:
+        m.integrate(*d)
+    m.sync()
+    t = {}
+    for name in names:
+        x = np.zeros((16, 8), np.uint64)
+        getattr(lib, f"farm_trace_{name}_read")(x.ctypes.data_as(C.c_void_p), 0)
+        t[name] = x.astype(np.int64)
+    print(f"configs[{opt.config}], {n} single-frame calls back to back, FARM_OPT_INPUTS_READY = {opt.inputs_ready}; us relative to the end of the"
+          " previous call's merge warps")
+    print("call | prep start | lift start / end | similarity start / end | probe start / end | scoring start / over | scan start / end |"
+          " merge start / warps end | period")
+    for c in range(n - 7, n + 1):
+        s, a, l = t["sim"][c & 15], t["assoc"][c & 15], t["lift"][c & 15]
+        t0 = t["assoc"][(c - 1) & 15][7]
+        f = lambda x: f"{(x - t0) / 1e3:6.1f}"
+        print(f"{c:4d} | {f(l[4])} | {f(l[0])} / {f(l[1])} | {f(s[0])} / {f(s[7])} | {f(l[2])} / {f(l[3])} | {f(a[0])} / {f(a[1])} | {f(a[3])} / {f(a[5])} | "
+              f"{f(a[2])} / {f(a[7])} | {(a[7] - t0) / 1e3:6.1f}")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--inputs-ready", type=int, default=1)
     ap.add_argument("--calls", type=int, default=14)
+    ap.add_argument("--config", type=int, default=4, help="4: 16-frame stress batches; 1-3: single-frame calls of that config")
     opt = ap.parse_args()
     lib_path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfarm_trace.so")
     if not os.path.exists(lib_path):
@@ -36,6 +79,8 @@ def main():
     import bench  # the stress scene and its import arrays (repo root)
     from paper_2606_15476_b200 import FarmMap, scenes as S
 
+    if opt.config != 4:
+        return single_frame(opt, binding)
     args = bench.parse()
     args.steps, args.warmup, args.extra_batches = opt.calls, 0, 0
     dev = torch.device("cuda", 0)
@@ -55,7 +100,7 @@ def main():
     torch.cuda.synchronize()
     lib = binding.load_library()
     tables = {}
-    for name in ("sim", "assoc", "tiles", "clock"):
+    for name in ("sim", "assoc", "tiles", "clock", "lift"):
         getattr(lib, f"farm_trace_{name}_read")(None, 1)
     for b in range(opt.calls):
         m.integrate_batch(16, *batches[b])
