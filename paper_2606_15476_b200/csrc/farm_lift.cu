@@ -10,6 +10,7 @@
 #include "farm_internal.cuh"
 
 namespace farm {
+FARM_TRACE_TABLE(farm_trace_probe)  // probe kernel: 0 first CTA resident; last warp with records past 1 its record loads, 3 the block hash, 5 the pair set, 7 phase B
 FARM_TRACE_TABLE(farm_trace_lift)  // 0 / 1 lift first CTA start / last CTA end, 2 / 3 probe first CTA past its wait / last CTA end, 4 prep start
 
 namespace {
@@ -648,9 +649,11 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
 //   |V_d| += popc(new bits); the (detection, block, new bits) event is appended to the event list for the
 //   commit pass.  Overlap counts are aggregated over the lanes of a warp (match.any + redux.add).
 constexpr int PROBE_THREADS = 256;
+constexpr uint32_t PROBE_DIAGONAL_MAX = 1u << 16;  // records; above this the queue is read in order
 
 __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs a) {
   __shared__ uint8_t s_pairs[PROBE_THREADS / 32][256];  // per warp: (record lane << 3 | sector) of the sectors with new voxels
+  if (threadIdx.x == 0) TRACE_MIN(farm_trace_probe, a.seq, 0);
   pdl_trigger();  // cand_associate may become resident behind this grid
   pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
   if (threadIdx.x == 0) TRACE_MIN(farm_trace_lift, a.seq, 2);
@@ -665,8 +668,16 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
   const uint32_t nq = min(*m.surv_cnt, m.surv_cap);
   const int lane = threadIdx.x & 31;
   const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < nq; i0 += stride) {
-    const uint32_t i = i0 + lane;
+  // Small queues (single-frame calls) are read along a diagonal: the real records sit at the start of each 128-record chunk that
+  // a lift CTA reserved, so a warp that took 32 consecutive records would hold either 32 real ones (and run phase B's dependent
+  // rounds seven or eight times) or none.  Lane l of warp task (g, k) takes record (k + 4 l) mod 128 of chunk 32 g + l instead:
+  // a bijection on [0, 4096) per group, every warp samples all chunk positions and gets the average fill.  Large queues (batches)
+  // keep the coalesced order -- their warps are all busy and the uncoalesced record loads would cost bandwidth.
+  const bool diagonal = nq <= PROBE_DIAGONAL_MAX;
+  const uint32_t n_end = diagonal ? (nq + 4095u) & ~4095u : nq;
+  for (uint32_t i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u; i0 < n_end; i0 += stride) {
+    const uint32_t wt = i0 >> 5;
+    const uint32_t i = diagonal ? ((wt >> 7) << 12) + ((uint32_t)lane << 7) + (((wt & 127u) + 4u * lane) & 127u) : i0 + lane;
     // ---- phase A
     uint32_t j = 0, slot = NONE32, ps = 0;
     unsigned long long nb = 0;
@@ -674,7 +685,13 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
       const unsigned long long bkey = __ldcs(&m.surv_key[i]);
       const unsigned long long bits = __ldcs(&m.surv_bits[i]);
       j = __ldcs(&m.surv_j[i]);
+#ifdef FARM_TRACE
+      if (bits && lane == __ffs(__activemask()) - 1) TRACE_MAX(farm_trace_probe, a.seq, 1);
+#endif
       if (bits) slot = block_find_or_insert(m, bkey);  // bits == 0: padding of a reserved queue chunk
+#ifdef FARM_TRACE
+      if (bits && lane == __ffs(__activemask()) - 1) TRACE_MAX(farm_trace_probe, a.seq, 3);
+#endif
       if (slot != NONE32) {
         const unsigned long long pv = ((unsigned long long)((a.epoch << 16) | j) << 32) | slot;
         const int r = epoch_insert(m.pair_set, m.pair_mask, pv, a.epoch, &ps);
@@ -688,6 +705,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
     }
     const unsigned act = __ballot_sync(0xFFFFFFFFu, nb != 0);
     if (!act) continue;
+    if (lane == 0) TRACE_MAX(farm_trace_probe, a.seq, 5);
     // |V_d| += new voxels (aggregated over the lanes of the same detection)
     if (nb) {
       const unsigned same = __match_any_sync(act, j);
@@ -790,6 +808,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
       if (hi > lo) pend_mine |= ub & ((hi - lo == 32 ? 0xFFFFFFFFu : ((1u << (hi - lo)) - 1u)) << lo);
     }
     __syncwarp();  // the list is rewritten by the warp's next 32 records
+    if (lane == 0) TRACE_MAX(farm_trace_probe, a.seq, 7);
     if (nb) {
       if (ev < m.pair_cap) {
         m.pl_bits[ev] = nb;

@@ -42,7 +42,7 @@ def single_frame(opt, binding):
                            torch.from_numpy(np.ascontiguousarray(fr.T, np.float32)).to(dev), torch.from_numpy(desc).to(dev), fr.n_det))
     torch.cuda.synchronize()
     lib = binding.load_library()
-    names = ("sim", "assoc", "lift")
+    names = ("sim", "assoc", "lift", "probe")
     for name in names:
         getattr(lib, f"farm_trace_{name}_read")(None, 1)
     for d in staged:
@@ -57,6 +57,12 @@ def single_frame(opt, binding):
           " previous call's merge warps")
     print("call | prep start | lift start / end | similarity start / end | probe start / end | scoring start / over | scan start / end |"
           " merge start / warps end | period")
+    print("probe kernel, us after its first CTA passed the wait: first CTA resident | last warp with records past its record loads |"
+          " the block hash | the pair set | phase B | last CTA end")
+    for c in range(n - 7, n + 1):
+        l, p = t["lift"][c & 15], t["probe"][c & 15]
+        g = lambda x: f"{(x - l[2]) / 1e3:6.1f}"
+        print(f"{c:4d} | {g(p[0])} | {g(p[1])} | {g(p[3])} | {g(p[5])} | {g(p[7])} | {g(l[3])}")
     for c in range(n - 7, n + 1):
         s, a, l = t["sim"][c & 15], t["assoc"][c & 15], t["lift"][c & 15]
         t0 = t["assoc"][(c - 1) & 15][7]
