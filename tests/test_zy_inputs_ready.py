@@ -73,6 +73,27 @@ def test_inputs_ready_back_to_back_calls_equal_the_stream_ordered_run(oracle):
     assert np.array_equal(maps[0][0], maps[1][0]) and np.array_equal(maps[0][1], maps[1][1])     # objects, descriptors
 
 
+@pytest.mark.parametrize("cfg_id,n", [(1, 60), (2, 50)])
+def test_inputs_ready_single_frame_series_back_to_back(oracle, cfg_id, n):
+    """The bench's single-frame series: n single-frame calls with nothing between them (prep, lift and the similarity kernel of a
+    call run beside the previous call's probe -> scoring -> scan -> merge chain; the probe kernel reads its small queue along the
+    diagonal and waits for its lift kernel on the device).  Last call and final map against the oracle."""
+    cfg = S.get_config(cfg_id)
+    o, g = make_pair(oracle, cfg, inputs_ready=1)
+    calls = []
+    for fr in generate_frames(cfg_id, range(20, 20 + n) if cfg_id == 1 else range(n)):
+        frames = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, frames)
+        calls.append(frames)
+    staged = [upload(fr, cfg.dtype) for fr in calls]
+    torch.cuda.synchronize()
+    for d, fr in zip(staged, calls):
+        g.integrate_batch(len(fr), d["depth"], d["mask"], d["K"], d["T"], d["desc"], d["n_det"])
+    compare_call(g, o)
+    compare_maps(g, o)
+    assert len(o.read(voxels=False)[0]) > 30
+
+
 @pytest.mark.parametrize("dtype", [1, 2])
 def test_inputs_ready_exact_ties_among_rewritten_rows_go_to_the_lowest_id(oracle, dtype):
     """R18 inside phase 2.  Two pairs of objects with bit-identical rows, (7, 200) and (250, 30); call 2 merges the same
