@@ -101,7 +101,7 @@ extern "C" {
                                         FARM_OPT_OVERLAP = 1, and without FARM_OPT_CORRESPONDENCE / FARM_OPT_GEOMETRY; otherwise it
                                         is accepted and changes nothing.  farm_map_integrate_batch_host orders its own staging
                                         copies and may always be used with it.  Measured: single-frame
-                                        calls 25-33 % shorter (33 / 45 / 44 us on configs 1-3); 16-frame batches of configs[4]
+                                        calls 22-25 % shorter (33 / 49 / 45 us on configs 1-3); 16-frame batches of configs[4]
                                         no faster than the stream-ordered schedule (the board is power-managed there).  With FARM_OPT_TIMING = 1 only every
                                         eighth similarity kernel is bracketed by events and the sum is scaled.  Default 0      */
 /* float options (farm_map_set_option_f) */

@@ -53,7 +53,6 @@ struct farm_map {
   uint32_t seq = 0;             // sequence number of the last integrate call (CallArgs.seq)
   long long sim_timed = 0, sim_all = 0;  // timing 1: similarity launches bracketed by events / all of them (since the last reset)
   uint32_t scan_count = 0;      // decision scans launched so far (device counter dm.scan_done)
-  uint32_t lift_count = 0;      // lift CTAs of split calls launched so far (device counter dm.lift_done)
   uint32_t merge_count = 0;     // merge warps launched so far (device counter dm.merge_done)
   // what prep resets and the lift kernel writes, double buffered by call parity: with the split schedule prep and lift of call c
   // run on their own stream while the main chain is still at call c-1 (whose scan, merge and result reads use the other set)
@@ -444,7 +443,6 @@ int finalise_impl(farm_map *m) {
   if (m->inputs_ready && m->dtype != FARM_DTYPE_F32 && (m->sim_path == 0 || m->sim_path == 2) && m->overlap == 1 && !m->corr && m->geom == 0 &&
       m->D % 8 == 0) {
     A(d.scan_done, 1, 0);
-    A(d.lift_done, 1, 0);
     A(d.merge_done, 1, 0);
     A(d.touch_seq, NO, 0);
     A(d.n_hist, 2, 0);
@@ -862,16 +860,9 @@ int farm_map_integrate_batch(farm_map *m, int F, const float *depth, const uint1
       launch_prep(d, a, m->early);  // resets this parity's buffers only: nothing the previous call still reads
       return 1;
     });
-    // Small calls: the probe kernel waits for the lift on the device (dm.lift_done), so that no event sits between the previous
-    // call's merge kernel and this probe and the probe keeps its programmatic early launch.
-    m->lift_count += (uint32_t)lift_ctas_of(d, a);
-    a.lift_target = m->lift_count;
-    a.lift_wait = a.sim_fills_gpu ? 0 : 1;
     stage(FARM_STAGE_LIFT, m->early, [&] { return launch_lift(d, a, m->early); });
-    if (!a.lift_wait) {
-      cudaEventRecord(m->ev_lift, m->early);
-      cudaStreamWaitEvent(st, m->ev_lift, 0);
-    }
+    cudaEventRecord(m->ev_lift, m->early);
+    cudaStreamWaitEvent(st, m->ev_lift, 0);
   }
   if (!a.split)
     stage(FARM_STAGE_PREP, st, [&] {

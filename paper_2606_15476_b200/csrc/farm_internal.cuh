@@ -168,7 +168,6 @@ struct DevMap {
   // call c starts when that of call c-1 ends: phase 1 covers the rows that existed at the entry of call c-1 minus the rows
   // call c-1 merged into (their columns are masked), phase 2 -- after call c-1's merge warps -- the rows of `delta`.
   uint32_t *scan_done;               // cumulative count of finished decision scans (one per call)
-  uint32_t *lift_done;               // cumulative count of finished lift CTAs of split calls
   uint32_t *merge_done;              // cumulative count of finished merge warps
   uint32_t *touch_seq;               // [max_objects] sequence number of the last call that merged a detection into the object
   uint32_t *n_hist;                  // [2] n_hist[(s + 1) & 1] = number of objects after the call with sequence number s
@@ -194,8 +193,6 @@ struct CallArgs {
   uint32_t prep_target;   //   value dm.prep_done reaches when the row norms of this call are final (cand_associate waits)
   uint32_t scan_target;   //   value dm.scan_done reaches when the PREVIOUS call's decision scan is done
   uint32_t merge_target;  //   value dm.merge_done reaches when the PREVIOUS call's merge warps are done
-  uint32_t lift_target;   //   value dm.lift_done reaches when THIS call's lift kernel (other stream) is done
-  int lift_wait;          //   the probe kernel waits for it on the device (small split calls: no event between merge and probe)
   const float *depth;
   const uint16_t *mask;
   const float *K;
@@ -339,7 +336,6 @@ void configure_lift_kernels();
 void configure_assoc_kernels();
 void configure_edge_kernels();
 int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s);  // returns the number of CTAs that report to prep_done
-int lift_ctas_of(const DevMap &m, const CallArgs &a);  // CTAs of the lift kernel of this call
 int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_probe(const DevMap &m, const CallArgs &a, cudaStream_t s);
 int launch_debug_backproject(const DevMap &m, const float *depth, const uint16_t *mask, const float *K,

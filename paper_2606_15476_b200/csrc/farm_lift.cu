@@ -636,13 +636,6 @@ __global__ void __launch_bounds__(LIFT_THREADS, 6) lift_voxelise_kernel(DevMap m
     }
     for (uint32_t p = pos + tid; p < end; p += LIFT_THREADS) survivor_store(m, p, 0ull, 0u, 0u, 0u);
   }
-  if (a.split) {  // the probe kernel of a small call waits for this count instead of a stream event
-    __syncthreads();
-    if (tid == 0) {
-      __threadfence();
-      atomicAdd(m.lift_done, 1u);
-    }
-  }
   if (tid == 0) TRACE_MAX(farm_trace_lift, a.seq, 1);
 }
 
@@ -663,10 +656,6 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
   if (threadIdx.x == 0) TRACE_MIN(farm_trace_probe, a.seq, 0);
   pdl_trigger();  // cand_associate may become resident behind this grid
   pdl_wait();     // launched with PDL behind the lift kernel: its survivor queue is complete from here on
-  if (a.lift_wait) {  // split schedule, small call: the lift ran on another stream
-    if (threadIdx.x == 0) spin_until(m.lift_done, a.lift_target, m.err);
-    __syncthreads();
-  }
   if (threadIdx.x == 0) TRACE_MIN(farm_trace_lift, a.seq, 2);
 #ifdef FARM_TRACE
   struct ProbeEnd {
@@ -693,7 +682,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(DevMap m, CallArgs
     uint32_t j = 0, slot = NONE32, ps = 0;
     unsigned long long nb = 0;
     if (i < nq) {
-      const unsigned long long bkey = __ldcg(&m.surv_key[i]);  // L2 only: with lift_wait the lift kernel may have run beside this grid
+      const unsigned long long bkey = __ldcg(&m.surv_key[i]);
       const unsigned long long bits = __ldcg(&m.surv_bits[i]);
       j = __ldcg(&m.surv_j[i]);
 #ifdef FARM_TRACE
@@ -956,16 +945,11 @@ int launch_prep(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   return a.split ? 0 : blocks;
 }
 
-int lift_ctas_of(const DevMap &m, const CallArgs &a) {
+int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
   const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
   const int n_tiles = tiles_x * tiles_y * a.F;
   // persistent, 4 CTAs per SM: 4 x 128 x 80 registers fit beside the similarity CTA (256 x 80) in the 64 K register file
-  return n_tiles < m.num_sms * 4 ? n_tiles : m.num_sms * 4;
-}
-
-int launch_lift(const DevMap &m, const CallArgs &a, cudaStream_t s) {
-  const int tiles_x = (m.W + TILE_W - 1) / TILE_W, tiles_y = (m.H + TILE_H - 1) / TILE_H;
-  const int grid = lift_ctas_of(m, a);
+  const int grid = n_tiles < m.num_sms * 4 ? n_tiles : m.num_sms * 4;
   const bool vec = (m.W % 8 == 0) && ((uintptr_t)a.depth % 16 == 0) && ((uintptr_t)a.mask % 16 == 0);
   if (m.det_gm) {
     if (vec)

@@ -94,6 +94,23 @@ def test_inputs_ready_single_frame_series_back_to_back(oracle, cfg_id, n):
     assert len(o.read(voxels=False)[0]) > 30
 
 
+def test_inputs_ready_with_host_buffers_back_to_back(oracle):
+    """farm_map_integrate_batch_host with the option: the library stages the inputs itself (two staging sets), the early and side
+    streams wait for the copy; 40 single-frame calls with nothing between them, final map against the oracle."""
+    from helpers import stack_frames
+    cfg = S.get_config(1)
+    o, g = make_pair(oracle, cfg, inputs_ready=1)
+    keep = []
+    for fr in generate_frames(1, range(20, 60)):
+        frames = margin_filter(o.clone, [fr], cfg.tau)
+        integrate_frames(o, frames)
+        depth, mask, K, T, desc, n_det = stack_frames(frames)
+        keep.append((depth, mask, K, T, np.ascontiguousarray(desc), n_det))     # host buffers stay alive until the sync
+        g.integrate_batch_host(1, *keep[-1])
+    compare_call(g, o)
+    compare_maps(g, o)
+
+
 @pytest.mark.parametrize("dtype", [1, 2])
 def test_inputs_ready_exact_ties_among_rewritten_rows_go_to_the_lowest_id(oracle, dtype):
     """R18 inside phase 2.  Two pairs of objects with bit-identical rows, (7, 200) and (250, 30); call 2 merges the same
