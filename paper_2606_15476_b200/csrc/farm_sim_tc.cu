@@ -271,7 +271,9 @@ similarity_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
             // of after the whole grid plus a launch latency.  Not earlier than this point: a pending grid on the high-priority
             // stream keeps the other streams' grids from being dispatched, and until here this kernel still waits for one of
             // them (the previous call's merge).
-            pdl_trigger();
+            // Skinny call on a large map (one row tile, several rounds): no early trigger either -- the next call's CTAs cannot
+            // all be resident beside this kernel's and would stay pending, in front of this call's probe kernel.
+            if (!(tiles_m == 1 && n_tiles > n_units)) pdl_trigger();
           }
           if (tile >= n_all) tile = -1;
         }
@@ -677,6 +679,12 @@ int launch_similarity_tc(const DevMap &m, const CallArgs &a, uint32_t n_upper, c
     // split: phase 2 adds up to ceil(max touched rows / 256) column tiles; the grid is sized on the rows known to the host
     const long long tiles = (long long)((a.M + BLOCK_M - 1) / BLOCK_M) * ((n_upper + BLOCK_N - 1) / BLOCK_N);
     grid = (int)(tiles < m.num_sms ? tiles : m.num_sms);
+    if (a.M <= BLOCK_M && tiles > m.num_sms) {
+      // Skinny call on a large map (one row tile, more column tiles than SMs): every B tile is streamed from HBM once, and a last
+      // round with a few CTAs cannot keep enough loads in flight to use the bandwidth.  Same number of rounds for every CTA.
+      const long long rounds = (tiles + m.num_sms - 1) / m.num_sms;
+      grid = (int)((tiles + rounds - 1) / rounds);
+    }
     if (a.split) {
       if (prep_after) *prep_after = prep_target + (uint32_t)grid;
       if (launch_pdl(similarity_tc_kernel<false, 1, true>, dim3(grid), dim3(TC_THREADS), SMEM_BYTES, s, map_a, st->map_b, st->map_d, m, a.M,

@@ -111,6 +111,44 @@ def test_inputs_ready_with_host_buffers_back_to_back(oracle):
     compare_maps(g, o)
 
 
+@pytest.mark.parametrize("ready", [0, 1])
+def test_skinny_calls_on_a_map_with_more_column_tiles_than_sms(oracle, ready):
+    """One row tile of detections (M = 70) against N = 40,000 objects: more 256-column tiles than SMs, so the tensor-core
+    similarity kernel runs the grid it sizes for skinny calls (the same number of rounds for every CTA) and, with the split
+    schedule, ends without its early programmatic trigger.  Five calls (the last three split when ready = 1); matches rewrite
+    rows that later calls match again.  Every call and the final map against the oracle."""
+    from helpers import hand_frame, pack_key, pow2_K, unit_rows
+    from paper_2606_15476_b200 import FarmMap, binding
+    N, D, M, Hh, Ww, dtype = 40000, 64, 70, 96, 128, S.DTYPE_BF16
+    rows = unit_rows(N, D, 3)
+    objs = np.zeros(N, binding.OBJECT_DTYPE)
+    objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(N), 1, 1, -1, -1
+    keys = pack_key(np.arange(N) + 500, np.zeros(N, int), np.zeros(N, int))
+    owner = np.arange(N, dtype=np.uint32)
+    o = oracle.OracleMap(0.25, D, 0.0, 1.0, 0.9, dtype, Hh, Ww)
+    g = FarmMap(0.25, D, 0.0, 1.0, 0.9, H=Hh, W=Ww, dtype=dtype, max_objects=N + 1024, max_det_per_call=128, inputs_ready=ready)
+    assert o.import_(objs, rows, keys, owner) == 0
+    g.import_(objs, rows, keys, owner)
+    rng = np.random.default_rng(11)
+    pool = rng.permutation(N)[:120]                      # the calls pick from one pool: rows rewritten by a call are matched again
+    n_dense = 0
+    for call in range(5):
+        pick = rng.permutation(pool)[:50]
+        near = rows[pick] + 0.02 * unit_rows(50, D, 100 + call)                   # cosine ~ 0.9998 with its row, ~ 0.5 at most elsewhere
+        det = np.concatenate([near, unit_rows(M - 50, D, 200 + call)]).astype(np.float32) * 2.0   # the last 20 match nothing: spawns
+        depth, mask = hand_frame(Hh, Ww, [(1 + (d % 120), 2 + 3 * (d // 120) + 9 * call, 2.0, d + 1) for d in range(M)])
+        fr = S.Frame(depth, mask, pow2_K(), np.eye(4, dtype=np.float32), S.to_storage(det, dtype), M, np.zeros(M, np.int64))
+        frames = margin_filter(o.clone, [fr], 0.9)
+        integrate_frames(o, frames)
+        keep = _integrate_ready(g, frames, dtype)
+        compare_call(g, o)
+        n_dense += compare_dense(g, o)
+        st = g.last_assoc()[3]
+        assert int(st["matches"]) >= 45 and int(st["spawns"]) >= 15
+    compare_maps(g, o)
+    assert n_dense >= 5 * 45
+
+
 @pytest.mark.parametrize("dtype", [1, 2])
 def test_inputs_ready_exact_ties_among_rewritten_rows_go_to_the_lowest_id(oracle, dtype):
     """R18 inside phase 2.  Two pairs of objects with bit-identical rows, (7, 200) and (250, 30); call 2 merges the same
