@@ -53,6 +53,9 @@ def parse():
                         "timed region, so the library may start a call's similarity kernel before the previous call's merge "
                         "(0 = stream-ordered inputs, the library default)")
     p.add_argument("--no-single-frame", action="store_true", help="skip the single-frame latency series of configs[0..3]")
+    p.add_argument("--skinny-scan", action="store_true",
+                   help="not a bench line: the similarity step of single-frame calls (M = 100, D = 1024, bf16) over map sizes "
+                        "13k ... 104k, descriptor-only maps (DESIGN.md section 15)")
     p.add_argument("--full-oracle-batch", action="store_true",
                    help="cpu_baseline / --impl reference: time ONE full 16-frame, 1600-detection batch (minutes on one core)")
     return p.parse_args()
@@ -175,6 +178,52 @@ def aggregate_throughput(frames_local, ms_local, world, device=None):
 
 # ------------------------------------------------------------------------------------- single-frame calls (configs 0-3)
 SINGLE_FRAME_PLAN = {0: (0, 20), 1: (0, 120), 2: (0, 60), 3: (0, 12)}     # config -> (first frame, frames)
+
+
+def skinny_scan():
+    """DESIGN.md section 15, "single frames on a large map": one row tile of detections against maps of 13k ... 104k objects
+    (descriptors only, one far-away voxel each), similarity kernel bracketed by events (FARM_OPT_TIMING = 1).  Prints one JSON
+    line; development measurement, not a bench value."""
+    import torch
+    from paper_2606_15476_b200 import FarmMap, binding, scenes as S
+    D, M, H, W, dtype, n = 1024, 100, 96, 128, S.DTYPE_BF16, 30
+    dev = torch.device("cuda", 0)
+    rows_out = []
+    for N in (13000, 26000, 52000, 104000):
+        g = np.random.default_rng(3)
+        rows = g.standard_normal((N, D)).astype(np.float32)
+        rows /= np.linalg.norm(rows, axis=1, keepdims=True)
+        objs = np.zeros(N, binding.OBJECT_DTYPE)
+        objs["id"], objs["n_voxels"], objs["n_obs"], objs["best_frame"], objs["best_det"] = np.arange(N), 1, 1, -1, -1
+        keys = ((np.arange(N, dtype=np.uint64) + np.uint64(500 + (1 << 20))) << np.uint64(42)) | (np.uint64(1 << 20) << np.uint64(21)) | np.uint64(1 << 20)
+        m = FarmMap(0.25, D, 0.0, 1.0, 2.0, H=H, W=W, dtype=dtype, max_objects=N + 4096, max_det_per_call=128, timing=1)
+        m.import_(objs, rows, keys, np.arange(N, dtype=np.uint32))
+        det = g.standard_normal((M, D)).astype(np.float32)
+        depth, mask = np.zeros((1, H, W), np.float32), np.zeros((1, H, W), np.uint16)
+        for d in range(M):                                # one pixel per detection
+            depth[0, 2 + 3 * (d // 120), 1 + d % 120], mask[0, 2 + 3 * (d // 120), 1 + d % 120] = 2.0, d + 1
+        K = np.array([[[128.0, 0, 64.0], [0, 128.0, 48.0], [0, 0, 1]]], np.float32)
+        T = np.eye(4, dtype=np.float32)[None]
+        dd = (torch.from_numpy(depth).to(dev), torch.from_numpy(mask.view(np.int16)).to(dev), torch.from_numpy(K).to(dev),
+              torch.from_numpy(T).to(dev), torch.from_numpy(S.to_storage(det, dtype).view(np.int16)).to(dev), np.array([M], np.int32))
+        torch.cuda.synchronize()
+        for _ in range(5):
+            m.integrate_batch(1, *dd)
+        m.sync()
+        m.stage_times(reset=True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            m.integrate_batch(1, *dd)
+        e1.record()
+        torch.cuda.synchronize()
+        m.sync()
+        ms, _ = m.stage_times()
+        sim_us = float(ms[2]) * 1e3 / n
+        rows_out.append({"N": N, "column_tiles": (N + 255) // 256, "similarity_us": round(sim_us, 1), "MB": round(N * D * 2 / 1e6, 1),
+                         "TB_per_s": round(N * D * 2 / (sim_us * 1e-6) / 1e12, 2), "call_us": round(e0.elapsed_time(e1) * 1e3 / n, 1)})
+        m.destroy()
+    print(json.dumps({"skinny_scan": rows_out, "M": M, "D": D, "dtype": "bf16", "note": "development measurement, not a bench value"}))
 
 
 def single_frame_series(dev, stream):
@@ -675,6 +724,8 @@ if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.skinny_scan:
+        skinny_scan()
     elif a.config != 4:
         run_box_config(a)
     else:
